@@ -1,0 +1,580 @@
+/*
+ * qr_oracle.c -- CPU ORACLE for the Q-Render hot path.  TEST INFRASTRUCTURE ONLY.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+ * legs may load this library.  The product (paper_2512_20927_b200/) never does, shares
+ * no code with it and must fail loudly when its CUDA library is missing.
+ *
+ * What it is: a plain, slow, step-by-step restatement of
+ *   - PAPER.md:79       Sigma = R S S^T R^T
+ *   - PAPER.md:80,:124  3D-GS front end "(1) tiling; (2) splatting [EWA]; (3) volume rendering";
+ *                       conventions the paper leaves to [3D-GS] follow SPEC.md:130-168 and the
+ *                       readings R1-R15 listed in DESIGN.md
+ *   - PAPER.md:81-86    Eq. 1 (V-Render)
+ *   - PAPER.md:129-158  Algorithm 1 (QuantileRender), executed literally, line by line
+ *   - SPEC.md:462-470   backward: d f~ / d f_i = w^Q_i / (1 - T^Q) * I  (selection is piecewise constant)
+ * No blocking, fusion or reordering beyond those passages.
+ *
+ * Precision.  Everything is fp64 EXCEPT the quantities that decide an integer (which
+ * Gaussians are in a ray's list I, and which of them Algorithm 1 selects).  Those are taken
+ * in fp32 -- the kernel's precision -- with the operation order fixed in DESIGN.md
+ * ("fp32 decision arithmetic"): the fp32 projection orc_project_f32, alpha', the dense
+ * transmittance T and the thresholds 1 - (k+1)/(K+1).  orc_project_f64 is the fp64 statement
+ * of the same projection, used by the tests to bound the fp32 one.
+ * Compile with -ffp-contract=off: only the fmaf() calls written below fuse.
+ *
+ * Pins (tests/test_oracle_pins.py): hand-worked rays of SPEC.md:217-219 and SURVEY 8(c) G1,
+ * V-Render micro-rays SPEC.md:208-209, telescoping identities, closed-form projections
+ * SPEC.md:58-60,:136-138,:154-156, brute-force lists == binned lists, Q -> V limiting case,
+ * Appendix-C bound PAPER.md:672-678 on discretised 1-D models, adjoint identity and finite
+ * differences for the backward.  No function here is "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct {
+    int32_t width, height;
+    float fx, fy, cx, cy;
+    float znear;
+    float w2c[12]; /* row-major 3x4 [R|t] */
+} orc_camera;
+
+#define ORC_ALPHA_MIN (1.0f / 255.0f)   /* R4: alpha' >= 1/255 */
+#define ORC_ALPHA_MAX 0.99f             /* SPEC.md:151 clamp */
+#define ORC_POWER_MIN (-4.5f)           /* R4: inside the 3-sigma ellipse, g_min = e^-4.5 */
+#define ORC_DILATION 0.3f
+#define ORC_JCLAMP 1.3f                 /* R12 */
+#define ORC_TILE 16
+
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void orc_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* ------------------------------------------------------------------------------------------
+ * A1: Sigma = R S S^T R^T from scale and unit quaternion (w,x,y,z).  PAPER.md:79.
+ * fp64, for the pins (covariance examples, eigenvalues = squared scales).
+ * ---------------------------------------------------------------------------------------- */
+static void quat_to_rot_f64(const double q[4], double R[9])
+{
+    double w = q[0], x = q[1], y = q[2], z = q[3];
+    R[0] = 1.0 - 2.0 * (y * y + z * z); R[1] = 2.0 * (x * y - w * z);       R[2] = 2.0 * (x * z + w * y);
+    R[3] = 2.0 * (x * y + w * z);       R[4] = 1.0 - 2.0 * (x * x + z * z); R[5] = 2.0 * (y * z - w * x);
+    R[6] = 2.0 * (x * z - w * y);       R[7] = 2.0 * (y * z + w * x);       R[8] = 1.0 - 2.0 * (x * x + y * y);
+}
+
+void orc_covariance3d_f64(const double scale[3], const double quat[4], double Sigma[9])
+{
+    double R[9], M[9];
+    quat_to_rot_f64(quat, R);
+    for (int r = 0; r < 3; ++r)
+        for (int c = 0; c < 3; ++c) M[3 * r + c] = R[3 * r + c] * scale[c];   /* M = R S */
+    for (int r = 0; r < 3; ++r)
+        for (int c = 0; c < 3; ++c) {
+            double s = 0.0;
+            for (int k = 0; k < 3; ++k) s += M[3 * r + k] * M[3 * c + k];      /* M M^T */
+            Sigma[3 * r + c] = s;
+        }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O1 (fp64): EWA projection.  SPEC.md:130-138, :163-168; readings R5, R12.
+ *   t = W mu + t_wc ; depth = t_z ; culled if t_z <= znear
+ *   J = [[fx/tz, 0, -fx*tx'/tz^2], [0, fy/tz, -fy*ty'/tz^2]], tx'/tz clamped to +-1.3*tan(fov/2)
+ *   cov2d = J W Sigma W^T J^T + 0.3 I ; conic = cov2d^-1 ; extent = 3 sqrt(diag cov2d)
+ *   mean2d = (fx tx/tz + cx, fy ty/tz + cy)
+ * Outputs are fp64.  visible[i] = 0 when culled (outputs of culled Gaussians are zeroed).
+ * ---------------------------------------------------------------------------------------- */
+void orc_project_f64(const orc_camera* cam, int64_t N, const float* means, const float* scales,
+                     const float* quats, const float* opac, double* mean2d, double* cov2d,
+                     double* conic_opac, double* depth, double* extent, uint8_t* visible)
+{
+    const float* W = cam->w2c;
+    const double limx = (double)ORC_JCLAMP * (0.5 * cam->width) / cam->fx;
+    const double limy = (double)ORC_JCLAMP * (0.5 * cam->height) / cam->fy;
+    for (int64_t i = 0; i < N; ++i) {
+        double mu[3] = { means[3 * i], means[3 * i + 1], means[3 * i + 2] };
+        double t[3];
+        for (int r = 0; r < 3; ++r)
+            t[r] = (double)W[4 * r] * mu[0] + (double)W[4 * r + 1] * mu[1] + (double)W[4 * r + 2] * mu[2] + (double)W[4 * r + 3];
+        mean2d[2 * i] = mean2d[2 * i + 1] = 0.0;
+        cov2d[3 * i] = cov2d[3 * i + 1] = cov2d[3 * i + 2] = 0.0;
+        conic_opac[4 * i] = conic_opac[4 * i + 1] = conic_opac[4 * i + 2] = conic_opac[4 * i + 3] = 0.0;
+        extent[2 * i] = extent[2 * i + 1] = 0.0;
+        depth[i] = t[2];
+        visible[i] = 0;
+        if (!(t[2] > (double)cam->znear)) continue;
+
+        double s[3] = { scales[3 * i], scales[3 * i + 1], scales[3 * i + 2] };
+        double q[4] = { quats[4 * i], quats[4 * i + 1], quats[4 * i + 2], quats[4 * i + 3] };
+        double Sig[9];
+        orc_covariance3d_f64(s, q, Sig);
+
+        double txz = t[0] / t[2], tyz = t[1] / t[2];
+        double cxz = fmin(limx, fmax(-limx, txz)), cyz = fmin(limy, fmax(-limy, tyz));
+        double txc = cxz * t[2], tyc = cyz * t[2];
+        double J[6] = { cam->fx / t[2], 0.0, -cam->fx * txc / (t[2] * t[2]),
+                        0.0, cam->fy / t[2], -cam->fy * tyc / (t[2] * t[2]) };
+        double Tm[6]; /* T = J * Wrot (2x3) */
+        for (int r = 0; r < 2; ++r)
+            for (int c = 0; c < 3; ++c) {
+                double a = 0.0;
+                for (int k = 0; k < 3; ++k) a += J[3 * r + k] * (double)W[4 * k + c];
+                Tm[3 * r + c] = a;
+            }
+        double TS[6]; /* T * Sigma */
+        for (int r = 0; r < 2; ++r)
+            for (int c = 0; c < 3; ++c) {
+                double a = 0.0;
+                for (int k = 0; k < 3; ++k) a += Tm[3 * r + k] * Sig[3 * k + c];
+                TS[3 * r + c] = a;
+            }
+        double cxx = 0.0, cxy = 0.0, cyy = 0.0;
+        for (int k = 0; k < 3; ++k) {
+            cxx += TS[k] * Tm[k];
+            cxy += TS[k] * Tm[3 + k];
+            cyy += TS[3 + k] * Tm[3 + k];
+        }
+        cxx += 0.3;   /* SPEC.md:166, the exact decimal in the fp64 statement */
+        cyy += 0.3;
+        double det = cxx * cyy - cxy * cxy;
+        if (!(det > 0.0)) continue;
+        cov2d[3 * i] = cxx; cov2d[3 * i + 1] = cxy; cov2d[3 * i + 2] = cyy;
+        conic_opac[4 * i] = cyy / det;
+        conic_opac[4 * i + 1] = -cxy / det;
+        conic_opac[4 * i + 2] = cxx / det;
+        conic_opac[4 * i + 3] = opac[i];
+        mean2d[2 * i] = cam->fx * txz + cam->cx;
+        mean2d[2 * i + 1] = cam->fy * tyz + cam->cy;
+        extent[2 * i] = 3.0 * sqrt(cxx);
+        extent[2 * i + 1] = 3.0 * sqrt(cyy);
+        visible[i] = 1;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O1 (fp32 decision arithmetic): the same projection evaluated in fp32 in the operation order
+ * fixed in DESIGN.md, so that `depth` (the sort key, R6) and alpha' (list membership, selection)
+ * are decided in the kernel's precision.  Every product and sum below is a separate fp32
+ * rounding unless written as fmaf().
+ * ---------------------------------------------------------------------------------------- */
+void orc_project_f32(const orc_camera* cam, int64_t N, const float* means, const float* scales,
+                     const float* quats, const float* opac, float* mean2d, float* conic_opac,
+                     float* depth, float* extent, uint8_t* visible)
+{
+    const float* W = cam->w2c;
+    const float limx = ORC_JCLAMP * (0.5f * (float)cam->width) / cam->fx;
+    const float limy = ORC_JCLAMP * (0.5f * (float)cam->height) / cam->fy;
+    for (int64_t i = 0; i < N; ++i) {
+        const float mx = means[3 * i], my = means[3 * i + 1], mz = means[3 * i + 2];
+        float t[3];
+        for (int r = 0; r < 3; ++r)
+            t[r] = fmaf(W[4 * r + 2], mz, fmaf(W[4 * r + 1], my, fmaf(W[4 * r], mx, W[4 * r + 3])));
+        mean2d[2 * i] = mean2d[2 * i + 1] = 0.0f;
+        conic_opac[4 * i] = conic_opac[4 * i + 1] = conic_opac[4 * i + 2] = conic_opac[4 * i + 3] = 0.0f;
+        extent[2 * i] = extent[2 * i + 1] = 0.0f;
+        depth[i] = t[2];
+        visible[i] = 0;
+        if (!(t[2] > cam->znear)) continue;
+
+        const float qw = quats[4 * i], qx = quats[4 * i + 1], qy = quats[4 * i + 2], qz = quats[4 * i + 3];
+        float R[9];
+        R[0] = 1.0f - 2.0f * (qy * qy + qz * qz); R[1] = 2.0f * (qx * qy - qw * qz);        R[2] = 2.0f * (qx * qz + qw * qy);
+        R[3] = 2.0f * (qx * qy + qw * qz);        R[4] = 1.0f - 2.0f * (qx * qx + qz * qz); R[5] = 2.0f * (qy * qz - qw * qx);
+        R[6] = 2.0f * (qx * qz - qw * qy);        R[7] = 2.0f * (qy * qz + qw * qx);        R[8] = 1.0f - 2.0f * (qx * qx + qy * qy);
+        float M[9];
+        for (int r = 0; r < 3; ++r)
+            for (int c = 0; c < 3; ++c) M[3 * r + c] = R[3 * r + c] * scales[3 * i + c];
+        float Sig[9];
+        for (int r = 0; r < 3; ++r)
+            for (int c = 0; c < 3; ++c)
+                Sig[3 * r + c] = (M[3 * r] * M[3 * c] + M[3 * r + 1] * M[3 * c + 1]) + M[3 * r + 2] * M[3 * c + 2];
+
+        const float tz = t[2];
+        const float txz = t[0] / tz, tyz = t[1] / tz;
+        const float cxz = fminf(limx, fmaxf(-limx, txz)), cyz = fminf(limy, fmaxf(-limy, tyz));
+        const float tz2 = tz * tz;
+        const float J00 = cam->fx / tz, J02 = -(cam->fx * (cxz * tz)) / tz2;
+        const float J11 = cam->fy / tz, J12 = -(cam->fy * (cyz * tz)) / tz2;
+        float Tm[6];
+        for (int c = 0; c < 3; ++c) {
+            Tm[c] = J00 * W[c] + J02 * W[8 + c];
+            Tm[3 + c] = J11 * W[4 + c] + J12 * W[8 + c];
+        }
+        float TS[6];
+        for (int r = 0; r < 2; ++r)
+            for (int c = 0; c < 3; ++c)
+                TS[3 * r + c] = (Tm[3 * r] * Sig[c] + Tm[3 * r + 1] * Sig[3 + c]) + Tm[3 * r + 2] * Sig[6 + c];
+        float cxx = (TS[0] * Tm[0] + TS[1] * Tm[1]) + TS[2] * Tm[2];
+        float cxy = (TS[0] * Tm[3] + TS[1] * Tm[4]) + TS[2] * Tm[5];
+        float cyy = (TS[3] * Tm[3] + TS[4] * Tm[4]) + TS[5] * Tm[5];
+        cxx = cxx + ORC_DILATION;
+        cyy = cyy + ORC_DILATION;
+        const float det = cxx * cyy - cxy * cxy;
+        if (!(det > 0.0f)) continue;
+        conic_opac[4 * i] = cyy / det;
+        conic_opac[4 * i + 1] = (-cxy) / det;
+        conic_opac[4 * i + 2] = cxx / det;
+        conic_opac[4 * i + 3] = opac[i];
+        mean2d[2 * i] = fmaf(cam->fx, txz, cam->cx);
+        mean2d[2 * i + 1] = fmaf(cam->fy, tyz, cam->cy);
+        extent[2 * i] = 3.0f * sqrtf(cxx);
+        extent[2 * i + 1] = 3.0f * sqrtf(cyy);
+        visible[i] = 1;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Tile rectangle of the 3-sigma AABB, half-open, clamped to the tile grid.
+ * A tile list built from these rectangles is a SUPERSET of every pixel's list (rule R4 is
+ * per pixel and tile independent).  tiles_touched = 0 => culled.
+ * ---------------------------------------------------------------------------------------- */
+static int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+void orc_tile_rects(const orc_camera* cam, int64_t N, const float* mean2d, const float* extent,
+                    const uint8_t* visible, int32_t* tile_rect, uint32_t* tiles_touched)
+{
+    const int TX = (cam->width + ORC_TILE - 1) / ORC_TILE, TY = (cam->height + ORC_TILE - 1) / ORC_TILE;
+    for (int64_t i = 0; i < N; ++i) {
+        int32_t* r = tile_rect + 4 * i;
+        r[0] = r[1] = r[2] = r[3] = 0;
+        tiles_touched[i] = 0;
+        if (!visible[i]) continue;
+        const float inv = 1.0f / (float)ORC_TILE;
+        const float fx0 = floorf((mean2d[2 * i] - extent[2 * i]) * inv);
+        const float fx1 = floorf((mean2d[2 * i] + extent[2 * i]) * inv);
+        const float fy0 = floorf((mean2d[2 * i + 1] - extent[2 * i + 1]) * inv);
+        const float fy1 = floorf((mean2d[2 * i + 1] + extent[2 * i + 1]) * inv);
+        /* clamp in float first so that huge footprints cannot overflow the int conversion */
+        const float big = 1.0e6f;
+        int x0 = clampi((int)fminf(fmaxf(fx0, -big), big), 0, TX);
+        int x1 = clampi((int)fminf(fmaxf(fx1, -big), big) + 1, 0, TX);
+        int y0 = clampi((int)fminf(fmaxf(fy0, -big), big), 0, TY);
+        int y1 = clampi((int)fminf(fmaxf(fy1, -big), big) + 1, 0, TY);
+        if (x1 <= x0 || y1 <= y0) continue;
+        r[0] = x0; r[1] = y0; r[2] = x1; r[3] = y1;
+        tiles_touched[i] = (uint32_t)((x1 - x0) * (y1 - y0));
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Depth order (R6): ascending camera-space z of the centre, ties by ascending source index.
+ * depth > 0 so comparing floats is the same as comparing their IEEE bit patterns.
+ * ---------------------------------------------------------------------------------------- */
+typedef struct { float depth; int32_t id; } depth_id;
+
+static int cmp_depth_id(const void* a, const void* b)
+{
+    const depth_id* x = (const depth_id*)a; const depth_id* y = (const depth_id*)b;
+    if (x->depth < y->depth) return -1;
+    if (x->depth > y->depth) return 1;
+    return (x->id > y->id) - (x->id < y->id);
+}
+
+/* Per-tile depth-sorted Gaussian lists -- the plain definition of what qr_bin_sort must produce.
+ * Call with isect == NULL to get M (returned) and tile_range; then again with isect[M]. */
+int64_t orc_tile_lists(const orc_camera* cam, int64_t N, const float* depth, const int32_t* tile_rect,
+                       const uint32_t* tiles_touched, int32_t* tile_range, uint32_t* isect)
+{
+    const int TX = (cam->width + ORC_TILE - 1) / ORC_TILE, TY = (cam->height + ORC_TILE - 1) / ORC_TILE;
+    const int T = TX * TY;
+    int64_t* cnt = (int64_t*)calloc((size_t)T + 1, sizeof(int64_t));
+    for (int64_t i = 0; i < N; ++i) {
+        if (!tiles_touched[i]) continue;
+        const int32_t* r = tile_rect + 4 * i;
+        for (int ty = r[1]; ty < r[3]; ++ty)
+            for (int tx = r[0]; tx < r[2]; ++tx) cnt[ty * TX + tx + 1]++;
+    }
+    for (int t = 0; t < T; ++t) cnt[t + 1] += cnt[t];
+    const int64_t M = cnt[T];
+    for (int t = 0; t < T; ++t) { tile_range[2 * t] = (int32_t)cnt[t]; tile_range[2 * t + 1] = (int32_t)cnt[t + 1]; }
+    if (isect) {
+        depth_id* buf = (depth_id*)malloc(sizeof(depth_id) * (size_t)(M > 0 ? M : 1));
+        int64_t* cur = (int64_t*)malloc(sizeof(int64_t) * (size_t)T);
+        for (int t = 0; t < T; ++t) cur[t] = cnt[t];
+        for (int64_t i = 0; i < N; ++i) {
+            if (!tiles_touched[i]) continue;
+            const int32_t* r = tile_rect + 4 * i;
+            for (int ty = r[1]; ty < r[3]; ++ty)
+                for (int tx = r[0]; tx < r[2]; ++tx) {
+                    depth_id* e = buf + cur[ty * TX + tx]++;
+                    e->depth = depth[i]; e->id = (int32_t)i;
+                }
+        }
+        for (int t = 0; t < T; ++t)
+            qsort(buf + cnt[t], (size_t)(cnt[t + 1] - cnt[t]), sizeof(depth_id), cmp_depth_id);
+        for (int64_t m = 0; m < M; ++m) isect[m] = (uint32_t)buf[m].id;
+        free(buf); free(cur);
+    }
+    free(cnt);
+    return M;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * alpha' at a pixel (Eq. 1: alpha'_i = alpha_i G(u)) in the fp32
+ * decision arithmetic, with inclusion rule R4:
+ *   d = (x + 0.5, y + 0.5) - mean2d                      (R5)
+ *   power = -0.5 (a dx^2 + c dy^2) - b dx dy, evaluated as
+ *       q1 = (a dx) dx ; q2 = fma(c dy, dy, q1) ; q3 = (b dx) dy ; power = fma(-0.5, q2, -q3)
+ *   included  <=>  power <= 0  and  power >= -4.5  and  alpha' = min(0.99, alpha * expf(power)) >= 1/255
+ * *borderline is set when a 1-ulp change of expf could flip the membership (reading R15).
+ * ---------------------------------------------------------------------------------------- */
+static inline int alpha_prime_f32(int x, int y, const float* m2, const float* co, float* alpha_out, int* borderline)
+{
+    const float px = (float)x + 0.5f, py = (float)y + 0.5f;
+    const float dx = px - m2[0], dy = py - m2[1];
+    const float q1 = (co[0] * dx) * dx;
+    const float q2 = fmaf(co[2] * dy, dy, q1);
+    const float q3 = (co[1] * dx) * dy;
+    const float power = fmaf(-0.5f, q2, -q3);
+    if (fabsf(power - ORC_POWER_MIN) <= 1e-6f * 4.5f) *borderline = 1;
+    if (power > 0.0f || power < ORC_POWER_MIN) return 0;
+    const float a = fminf(ORC_ALPHA_MAX, co[3] * expf(power));
+    if (fabsf(a - ORC_ALPHA_MIN) <= 1e-6f * ORC_ALPHA_MIN) *borderline = 1;
+    if (a < ORC_ALPHA_MIN) return 0;
+    *alpha_out = a;
+    return 1;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O2: per-pixel depth-ordered intersection lists I ("ordered sequence of indices",
+ * :133).  Gaussians are visited in global (depth, id) order so every pixel's
+ * list comes out sorted.  mode 0 = brute force (every pixel tests every visible Gaussian);
+ * mode 1 = binned (each Gaussian visits the pixels of its 3-sigma AABB).  The two must agree
+ * exactly.
+ * Two-pass CSR: call with gid == NULL to fill counts[HW] (and borderline[HW]); then prefix-sum
+ * into off[HW+1] and call again with gid/alpha to fill.
+ * ---------------------------------------------------------------------------------------- */
+void orc_pixel_lists(const orc_camera* cam, int64_t N, const float* mean2d, const float* conic_opac,
+                     const float* depth, const float* extent, const uint8_t* visible, int mode,
+                     int64_t* counts, uint8_t* borderline, const int64_t* off, int32_t* gid, float* alpha)
+{
+    const int Wd = cam->width, Ht = cam->height;
+    int64_t nv = 0;
+    for (int64_t i = 0; i < N; ++i) nv += visible[i] ? 1 : 0;
+    depth_id* order = (depth_id*)malloc(sizeof(depth_id) * (size_t)(nv > 0 ? nv : 1));
+    nv = 0;
+    for (int64_t i = 0; i < N; ++i)
+        if (visible[i]) { order[nv].depth = depth[i]; order[nv].id = (int32_t)i; ++nv; }
+    qsort(order, (size_t)nv, sizeof(depth_id), cmp_depth_id);
+
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int y = 0; y < Ht; ++y) {
+        int64_t* fill = NULL;
+        if (gid) {
+            fill = (int64_t*)malloc(sizeof(int64_t) * (size_t)Wd);
+            for (int x = 0; x < Wd; ++x) fill[x] = off[(int64_t)y * Wd + x];
+        } else {
+            for (int x = 0; x < Wd; ++x) { counts[(int64_t)y * Wd + x] = 0; borderline[(int64_t)y * Wd + x] = 0; }
+        }
+        for (int64_t o = 0; o < nv; ++o) {
+            const int32_t g = order[o].id;
+            int x0 = 0, x1 = Wd;
+            if (mode == 1) {
+                const float ex = extent[2 * g], ey = extent[2 * g + 1];
+                const float cy = mean2d[2 * g + 1], cx = mean2d[2 * g];
+                /* pixel rows / columns whose centres can lie inside the AABB, with one pixel of slack */
+                if ((float)y + 0.5f < cy - ey - 1.0f || (float)y + 0.5f > cy + ey + 1.0f) continue;
+                const float lo = floorf(cx - ex - 1.0f), hi = ceilf(cx + ex + 1.0f);
+                if (hi < 0.0f || lo > (float)Wd) continue;
+                x0 = lo < 0.0f ? 0 : (int)lo;
+                x1 = hi >= (float)Wd ? Wd : (int)hi + 1;
+                if (x1 > Wd) x1 = Wd;
+            }
+            for (int x = x0; x < x1; ++x) {
+                float a; int bl = 0;
+                const int inc = alpha_prime_f32(x, y, mean2d + 2 * g, conic_opac + 4 * g, &a, &bl);
+                const int64_t p = (int64_t)y * Wd + x;
+                if (!gid) {
+                    if (bl) borderline[p] = 1;
+                    if (inc) counts[p]++;
+                } else if (inc) {
+                    gid[fill[x]] = g; alpha[fill[x]] = a; fill[x]++;
+                }
+            }
+        }
+        free(fill);
+    }
+    free(order);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O3: V-Render, Eq. 1:  C~ = sum_i w_i c_i,  w_i = T_i alpha'_i,
+ * T_i = prod_{j<i} (1 - alpha'_j).  Early stop R7: before blending i compute
+ * T_test = T (1 - alpha'_i); if T_test < t_min stop WITHOUT blending i.  t_min = 0 is exact Eq. 1.
+ * Not normalised.  The stop decision is taken on the fp32 T (kernel's precision);
+ * weights and sums are fp64.  stop_margin = min_i |T_test_i - t_min| / t_min (fp64), inf when t_min = 0.
+ * ---------------------------------------------------------------------------------------- */
+static void vrender_ray(int64_t n, const int32_t* I, const float* alpha, int D, const float* F, int64_t fstride,
+                        float t_min, double* acc, double* final_T, double* stop_margin, int32_t* n_blended)
+{
+    float T = 1.0f;      /* decision precision */
+    double Td = 1.0;     /* value precision */
+    double marg = INFINITY;
+    int32_t nb = 0;
+    for (int d = 0; d < D; ++d) acc[d] = 0.0;
+    for (int64_t s = 0; s < n; ++s) {
+        const float a = alpha[s];
+        const float T_test = T * (1.0f - a);
+        if (t_min > 0.0f) {
+            const double m = fabs((double)T_test - (double)t_min) / (double)t_min;
+            if (m < marg) marg = m;
+        }
+        if (T_test < t_min) break;
+        const double w = Td * (double)a;
+        const float* f = F + (int64_t)I[s] * fstride;
+        for (int d = 0; d < D; ++d) acc[d] += w * (double)f[d];
+        T = T_test;
+        Td = Td * (1.0 - (double)a);
+        ++nb;
+    }
+    *final_T = Td; *stop_margin = marg; *n_blended = nb;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O4: Algorithm 1, QuantileRender, line by line.  Line numbers in the
+ * comments are the listing's.  Decision variables (T, T_test, thresholds, k) are fp32 and the
+ * thresholds are computed as printed: 1.0f - (float)(k+1)/(float)(K+1) (reading R3); the
+ * comparisons are strict (R2).  T^Q, w^Q, f^Q are fp64.
+ * Outputs: out[D] = f~^Q (zero when nothing selected, R8), sel_idx[K] (-1 padded, in list order),
+ * sel_w[K] = w^Q / (1 - T^Q) (0 padded), n_sel, TQ (1 when nothing selected), n_walked = list
+ * entries consumed, margin = min over walked steps and tested boundaries of |T_test - boundary|.
+ * ---------------------------------------------------------------------------------------- */
+static inline float q_threshold(int k, int K) { return 1.0f - (float)(k + 1) / (float)(K + 1); }
+
+static void qrender_ray(int64_t n, const int32_t* I, const float* alpha, int K, int D, const float* F,
+                        int64_t fstride, double* fQ, int32_t* sel_idx, double* sel_w, int32_t* n_sel_out,
+                        double* TQ_out, int32_t* n_walked, double* margin_out)
+{
+    float T = 1.0f;                       /* line 2 */
+    double TQ = 1.0;
+    int k = 0;
+    if (fQ) for (int d = 0; d < D; ++d) fQ[d] = 0.0;
+    for (int s = 0; s < K; ++s) { sel_idx[s] = -1; sel_w[s] = 0.0; }
+    int32_t ns = 0, walked = 0;
+    double marg = INFINITY;
+    const float t_break = 1.0f / (float)(K + 1);
+    for (int64_t s = 0; s < n; ++s) {     /* line 3: for i in I */
+        const int32_t i = I[s];           /* line 4: g_i, f_i */
+        const float a = alpha[s];         /*         alpha'_i */
+        const float T_test = T * (1.0f - a);                 /* line 5 */
+        ++walked;
+        for (int kk = k; kk < K; ++kk) {                     /* boundaries this step can still cross */
+            const double m = fabs((double)T_test - (double)q_threshold(kk, K));
+            if (m < marg) marg = m;
+        }
+        { const double m = fabs((double)T_test - (double)t_break); if (m < marg) marg = m; }
+        if (T_test < q_threshold(k, K)) {                    /* line 6 */
+            k = k + 1;                                       /* line 7 */
+            const double wQ = TQ * (double)a;                /* line 8 */
+            if (fQ) {
+                const float* f = F + (int64_t)i * fstride;
+                for (int d = 0; d < D; ++d) fQ[d] += wQ * (double)f[d];   /* line 9 */
+            }
+            sel_idx[ns] = i; sel_w[ns] = wQ; ++ns;
+            TQ = TQ * (1.0 - (double)a);                     /* line 10 */
+            while (T_test < q_threshold(k, K)) k = k + 1;    /* lines 11-13; thr(K) = 0 ends it */
+        }
+        if (T_test < t_break) break;                         /* lines 15-17 */
+        T = T_test;                                          /* line 18 */
+    }
+    if (ns > 0) {                                            /* line 20: f~ = f / (1 - T^Q) */
+        const double norm = 1.0 - TQ;
+        if (fQ) for (int d = 0; d < D; ++d) fQ[d] = fQ[d] / norm;
+        for (int s = 0; s < ns; ++s) sel_w[s] = sel_w[s] / norm;
+    } else {
+        TQ = 1.0;                                            /* R8 */
+    }
+    *n_sel_out = ns; *TQ_out = TQ; *n_walked = walked; *margin_out = marg;
+}
+
+/* Render `npix` pixels (pix[j] = flat pixel index into the CSR lists; pix == NULL means 0..npix-1).
+ * features may be NULL (selection only).  out_map[npix, D] fp32 (rounded from the fp64 result). */
+void orc_qrender(int64_t npix, const int64_t* pix, const int64_t* off, const int32_t* gid, const float* alpha,
+                 int K, int D, const float* features, int64_t fstride, float* out_map, int32_t* sel_idx,
+                 double* sel_w, int32_t* n_sel, double* resid_TQ, int32_t* n_walked, double* margin)
+{
+#pragma omp parallel
+    {
+        double* acc = (double*)malloc(sizeof(double) * (size_t)(D > 0 ? D : 1));
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t j = 0; j < npix; ++j) {
+            const int64_t p = pix ? pix[j] : j;
+            const int64_t b = off[p], e = off[p + 1];
+            qrender_ray(e - b, gid + b, alpha + b, K, D, features, fstride, features ? acc : NULL,
+                        sel_idx + j * K, sel_w + j * K, n_sel + j, resid_TQ + j, n_walked + j, margin + j);
+            if (features && out_map)
+                for (int d = 0; d < D; ++d) out_map[j * D + d] = (float)acc[d];
+        }
+        free(acc);
+    }
+}
+
+void orc_vrender(int64_t npix, const int64_t* pix, const int64_t* off, const int32_t* gid, const float* alpha,
+                 int D, const float* features, int64_t fstride, float t_min, float* out_map, double* final_T,
+                 double* stop_margin, int32_t* n_blended)
+{
+#pragma omp parallel
+    {
+        double* acc = (double*)malloc(sizeof(double) * (size_t)(D > 0 ? D : 1));
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t j = 0; j < npix; ++j) {
+            const int64_t p = pix ? pix[j] : j;
+            const int64_t b = off[p], e = off[p + 1];
+            vrender_ray(e - b, gid + b, alpha + b, D, features, fstride, t_min, acc, final_T + j,
+                        stop_margin + j, n_blended + j);
+            for (int d = 0; d < D; ++d) out_map[j * D + d] = (float)acc[d];
+        }
+        free(acc);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O5: backward w.r.t. features.  The selection and the
+ * weights depend only on alpha', never on features, so
+ *     dL/dF[i, :] = sum_p sum_{s : sel_idx[p,s] = i}  w^_{p,s} * dL/dmap[p, :],   w^ = w^Q / (1 - T^Q).
+ * Pixels in raster order, fp64 accumulation.  Only the rows listed in rows[n_rows] are produced
+ * (rows == NULL: all N rows, out is [N, D]).
+ * ---------------------------------------------------------------------------------------- */
+void orc_backward(int64_t npix, int K, int D, int64_t N, const int32_t* sel_idx, const double* sel_w,
+                  const int32_t* n_sel, const float* dL_dmap, int64_t n_rows, const int64_t* rows, double* out)
+{
+    int64_t* slot = NULL;
+    const int64_t R = rows ? n_rows : N;
+    if (rows) {
+        slot = (int64_t*)malloc(sizeof(int64_t) * (size_t)N);
+        for (int64_t i = 0; i < N; ++i) slot[i] = -1;
+        for (int64_t r = 0; r < n_rows; ++r) slot[rows[r]] = r;
+    }
+    memset(out, 0, sizeof(double) * (size_t)R * (size_t)D);
+    for (int64_t p = 0; p < npix; ++p) {
+        const float* g = dL_dmap + p * D;
+        for (int s = 0; s < n_sel[p]; ++s) {
+            const int64_t i = sel_idx[p * K + s];
+            const int64_t r = slot ? slot[i] : i;
+            if (r < 0) continue;
+            const double w = sel_w[p * K + s];
+            double* o = out + r * D;
+            for (int d = 0; d < D; ++d) o[d] += w * (double)g[d];
+        }
+    }
+    free(slot);
+}
