@@ -1,0 +1,359 @@
+#!/usr/bin/env python
+"""bench.py -- BASELINE.json's metric on its headline workload (config 3: 640x480, 500k Gaussians, D = 512 fp32, K = 40).
+
+A step = one pass of the whole Q-Render hot path over one synthetic frame, through the C ABI:
+    qr_preprocess -> qr_bin_count -> qr_bin_sort -> qr_forward -> (zero dL/dF) -> qr_backward
+`value` = Mpix/s of that step with inputs resident in HBM (CUDA events, max over ranks).  The dense comparator
+(qr_dense_forward) is timed beside it in the same run and reported under "dense"; it is not part
+of the step.  `roofline` describes the dominant kernel (the longer of qr_forward / qr_backward), timed with CUDA
+events around each call inside the timed steps.  `e2e` repeats the step with HOST (pinned) inputs and outputs, the
+copies inside the timed region.  `cpu_baseline` times the CPU oracle on one full frame on the box's host cores.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg3]
+N > 1: launched by torch.distributed.run, one rank per GPU, independent replicas of the same frame (weak scaling,
+no data-path collective: SURVEY 8(e)); rank 0 prints the one JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "512-D feature-map Mpix/s (fwd+bwd step: preprocess, bin/sort, Q-Render forward, backward)"
+UNIT = "Mpix/s"
+NOMINAL_HBM_GBS = 8000.0
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def scene_for(workload: str):
+    from qr_inputs import make_scene
+    return make_scene(workload, seed=0)
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle, as it stands, on the host cores
+# ----------------------------------------------------------------------------------------------------------------
+def oracle_frame(orc, sc):
+    """One full frame of the path in the oracle: O1 projection, O2b lists, O4 Algorithm 1 with features, O5 backward."""
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    rect, touched = orc.tile_rects(sc.cam, proj)
+    orc.tile_lists(sc.cam, proj.depth, rect, touched)
+    lists = orc.pixel_lists(sc.cam, proj)
+    q = orc.qrender(lists, sc.K, sc.features)
+    if sc.dL_dmap is not None:
+        sel = q.sel_idx[q.sel_idx >= 0]
+        rows = np.unique(sel).astype(np.int64)
+        orc.backward(q.sel_idx, q.sel_w, q.n_sel, sc.dL_dmap, sc.N, rows=rows)
+    return q
+
+
+def time_oracle(sc, steps: int, warmup: int):
+    from oracle import qr_oracle as orc
+    for _ in range(warmup):
+        oracle_frame(orc, sc)
+    ts = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        oracle_frame(orc, sc)
+        ts.append(time.perf_counter() - t0)
+    return ts, orc.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    sc = scene_for(args.workload)
+    steps = max(1, min(args.steps, 3))          # one frame is ~10 s of CPU work: bound the run to a few minutes
+    warm = min(args.warmup, 1)
+    ts, cores = time_oracle(sc, steps, warm)
+    npix = sc.cam.width * sc.cam.height
+    ms = 1e3 * sum(ts) / len(ts)
+    val = npix / (ms * 1e-3) / 1e6
+    sample = f"{steps} full frame(s) of {args.workload} ({npix} px, all stages O1-O5), OpenMP over rows where the oracle has it"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": warm, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(sc, args.workload),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+def workload_config(sc, name):
+    return {"workload": f"{name}: {sc.cam.width}x{sc.cam.height}, N={sc.N} Gaussians (64 blobs), D={sc.D} "
+                        f"{sc.feat_dtype}, K={sc.K}, forward+backward (BASELINE.json configs[2])",
+            "K": sc.K, "D": sc.D, "N": sc.N, "width": sc.cam.width, "height": sc.cam.height,
+            "l2": "inputs larger than L2 (features 1.02 GB, dL_dmap 629 MB, map 629 MB vs 126 MB L2); no flush needed"}
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# CUDA arm
+# ----------------------------------------------------------------------------------------------------------------
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libqr has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import paper_2512_20927_b200 as qr
+    from paper_2512_20927_b200 import pipeline as pl
+    qr.binding.load()
+
+    sc = scene_for(args.workload)
+    cam, K, D, N = sc.cam, sc.K, sc.D, sc.N
+    H, W = cam.height, cam.width
+    npix = H * W
+    dev = torch.device("cuda", local)
+    host = {k: torch.from_numpy(np.ascontiguousarray(getattr(sc, k))).pin_memory()
+            for k in ("means", "scales", "quats", "opac", "features", "dL_dmap")}
+    d = {k: v.to(dev, non_blocking=True) for k, v in host.items()}
+    dF = torch.zeros((N, D), dtype=torch.float32, device=dev)
+    fwd_out = None
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    launches = {"n": 0}
+
+    def step(timers=None):
+        nonlocal fwd_out
+        fe = pl.frontend(cam, d["means"], d["scales"], d["quats"], d["opac"])
+        if timers is not None:
+            e0, e1, e2, e3 = ev(), ev(), ev(), ev()
+            e0.record()
+        fwd_out = pl.forward(cam, fe, d["features"], K, fwd_out)
+        if timers is not None:
+            e1.record()
+        dF.zero_()
+        if timers is not None:
+            e2.record()
+        pl.backward(cam, N, fwd_out, d["dL_dmap"], dF)
+        if timers is not None:
+            e3.record()
+            timers.append((e0, e1, e2, e3))
+        tile_bits = max(1, int(np.ceil(np.log2(max(qr.qr_num_tiles(cam), 2)))))
+        passes = (32 + tile_bits + 7) // 8
+        launches["n"] += 1 + 3 + 1 + 3 * passes + 1 + 1 + 1
+        return fe
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        fe = step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches["n"] = 0
+    timers = []
+    s0, s1 = ev(), ev()
+    barrier()
+    s0.record()
+    for _ in range(args.steps):
+        fe = step(timers)
+    s1.record()
+    barrier()
+    total_ms = s0.elapsed_time(s1)
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_step = total_ms / args.steps
+    value = world * npix / (ms_step * 1e-3) / 1e6
+    fwd_ms = statistics.mean(a.elapsed_time(b) for a, b, _, _ in timers)
+    bwd_ms = statistics.mean(c.elapsed_time(e) for _, _, c, e in timers)
+    zero_ms = statistics.mean(b.elapsed_time(c) for _, b, c, _ in timers)
+
+    # dense comparator, same frame, same front end (not part of the step)
+    dense_map = torch.empty((H, W, D), dtype=torch.float32, device=dev)
+    dense_T = torch.empty((H, W), dtype=torch.float32, device=dev)
+    for _ in range(2):
+        pl.dense_forward(cam, fe, d["features"], 1e-4, dense_map, dense_T)
+    torch.cuda.synchronize()
+    a, b = ev(), ev()
+    nd = 5
+    a.record()
+    for _ in range(nd):
+        pl.dense_forward(cam, fe, d["features"], 1e-4, dense_map, dense_T)
+    b.record()
+    torch.cuda.synchronize()
+    dense_ms = a.elapsed_time(b) / nd
+    del dense_map
+    clocks = sampler.stop() if rank == 0 else None
+
+    # workload counts for the byte model (statistics only; torch ops outside every timed region)
+    n_vis = int((fe.proj.tiles_touched != 0).sum().item())
+    sel = fwd_out.sel_idx[fwd_out.sel_idx >= 0]
+    S = int(torch.unique(sel).numel())
+    nsel_mean = float(fwd_out.n_sel.float().mean().item())
+    esz = 2 if sc.feat_dtype == "f16" else 4
+    fwd_bytes = fe.M * 4 + n_vis * 32 + S * D * esz + npix * D * 4 + npix * 4
+    rec_bytes = npix * (8 * K + 4)
+    bwd_bytes = npix * D * 4 + S * D * 4 + rec_bytes
+    peak, peak_src = _peaks()
+    dom = "qr_forward" if fwd_ms >= bwd_ms else "qr_backward"
+    dom_bytes, dom_ms = (fwd_bytes, fwd_ms) if dom == "qr_forward" else (bwd_bytes, bwd_ms)
+
+    def roof(nbytes, ms, kernel, traffic=None):
+        ach = nbytes / (ms * 1e-3) / 1e9
+        return {"kernel": kernel, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "peak_source": peak_src, "frac_of_nominal_8TBs": ach / NOMINAL_HBM_GBS, "algorithmic_bytes": nbytes,
+                "ms_per_launch": ms, "traffic": traffic}
+
+    # ---- e2e: host buffers in, host buffers out, copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        out_host = torch.empty((H, W, D), dtype=torch.float32).pin_memory()
+        dF_host = torch.empty((N, D), dtype=torch.float32).pin_memory()
+        dd = {k: torch.empty_like(v) for k, v in d.items()}
+
+        def e2e_step():
+            for k in dd:
+                dd[k].copy_(host[k], non_blocking=True)
+            fe2 = pl.frontend(cam, dd["means"], dd["scales"], dd["quats"], dd["opac"])
+            o = pl.forward(cam, fe2, dd["features"], K, fwd_out)
+            dF.zero_()
+            pl.backward(cam, N, o, dd["dL_dmap"], dF)
+            out_host.copy_(o.out_map, non_blocking=True)
+            dF_host.copy_(dF, non_blocking=True)
+
+        e2e_step()
+        barrier()
+        ne = max(2, min(args.steps, 4))
+        a, b = ev(), ev()
+        a.record()
+        for _ in range(ne):
+            e2e_step()
+        b.record()
+        barrier()
+        t = torch.tensor([a.elapsed_time(b)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e_ms = float(t.item()) / ne
+        h2d = sum(v.numel() * v.element_size() for v in host.values())
+        d2h = out_host.numel() * 4 + dF_host.numel() * 4
+        e2e = {"value": world * npix / (e_ms * 1e-3) / 1e6, "unit": UNIT, "ms_per_step": e_ms, "steps": ne,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "note": "inputs (Gaussians, features, dL_dmap) from pinned host memory; out_map and dL_dfeat read back"}
+        del out_host, dF_host, dd
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        ts, cores = time_oracle(sc, 1, 0)
+        cpu_baseline = {"value": npix / ts[0] / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "seconds": ts[0],
+                        "sample": f"1 full frame of {args.workload} ({npix} px; O1 projection, O2b lists, O4 Algorithm 1 "
+                                  f"with D={D} features, O5 backward of the selected rows)"}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(sc, args.workload),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches["n"],
+                "roofline": roof(dom_bytes, dom_ms, dom, TRAFFIC.get(dom)),
+                "roofline_fwd": roof(fwd_bytes, fwd_ms, "qr_forward", TRAFFIC.get("qr_forward")),
+                "roofline_bwd": roof(bwd_bytes, bwd_ms, "qr_backward", TRAFFIC.get("qr_backward")),
+                "cpu_baseline": cpu_baseline,
+                "kernels_ms": {"qr_forward": fwd_ms, "qr_backward": bwd_ms, "zero_dL_dfeat": zero_ms,
+                               "frontend_and_rest": ms_step - fwd_ms - bwd_ms - zero_ms},
+                "mpix_s": {"fwd_kernel": npix / fwd_ms / 1e3, "fwd_bwd_kernels": npix / (fwd_ms + bwd_ms) / 1e3,
+                           "dense_fwd_kernel": npix / dense_ms / 1e3},
+                "dense": {"ms": dense_ms, "speedup_qr_forward_over_dense": dense_ms / fwd_ms, "t_min": 1e-4},
+                "workload_counts": {"M": fe.M, "N_visible": n_vis, "n_sel_mean": nsel_mean, "S_distinct_selected": S,
+                                    "selection_record_bytes": rec_bytes}}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture named in profiles/ (None
+# until a capture of the current kernels is committed).
+TRAFFIC = {"qr_forward": None, "qr_backward": None}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

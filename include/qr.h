@@ -1,0 +1,154 @@
+/*
+ * qr.h -- C ABI of libqr: the data-parallel hot path of Quantile Rendering (Q-Render) on B200 (sm_100a).
+ *
+ * The calls split  f~^Q = QuantileRender(G, F, K, I)  (Algorithm 1 at PAPER.md:129-158) at the
+ * stage boundaries of the 3D-GS pipeline the paper builds on ("(1) tiling strategy; (2) splatting
+ * algorithm [EWA]; (3) volume rendering"):
+ *
+ *   qr_preprocess      EWA projection of means / covariances to 2D conics, tile rectangles, depth
+ *   qr_bin_count       prefix sum of tiles touched -> M = number of (Gaussian, tile) intersections
+ *   qr_bin_sort        tile-intersection duplication, (tile, depth) radix sort, per-tile ranges
+ *   qr_forward         per-pixel transmittance walk, quantile selection, K-sparse feature accumulation
+ *   qr_backward        dL/dfeature scatter-add to the selected Gaussians
+ *   qr_dense_forward   Eq. 1 dense volume rendering of the same features (in-run comparator)
+ *
+ * Conventions the paper leaves to "[3D-GS]" are fixed in DESIGN.md ("Readings", R1-R15).
+ *
+ * Pointers.  Every pointer is a DEVICE pointer owned by the caller unless marked HOST.  The library allocates
+ * nothing persistent: scratch comes from caller-provided workspaces sized by the *_workspace_bytes() calls.
+ * Inputs are never modified.  Device pointers must be 16-byte aligned.
+ * Streams.   `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Every call only
+ * enqueues work on `stream` and returns, except qr_bin_count, which also waits for `stream` to deliver M.
+ * Errors.    Return value 0 = QR_OK, negative = qr_status.  No call throws, aborts or prints; on error nothing
+ * is enqueued and qr_last_error() gives a thread-local HOST string.  Degenerate but legal inputs (N = 0, M = 0,
+ * a pixel with no Gaussian) are not errors.
+ */
+#ifndef QR_H_
+#define QR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define QR_VERSION 100       /* major*10000 + minor*100 + patch */
+#define QR_TILE 16           /* tile edge in pixels (3D-GS convention) */
+#define QR_MAX_K 256         /* largest K qr_forward / qr_backward accept */
+#define QR_MAX_D 512         /* largest feature width ("up to 512-D") */
+
+typedef enum {
+    QR_OK = 0,
+    QR_ERR_INVALID_ARG = -1,          /* size / range violation (K < 1, width < 1, ...) */
+    QR_ERR_NULL_POINTER = -2,
+    QR_ERR_UNSUPPORTED = -3,          /* K > QR_MAX_K, D > QR_MAX_D, fp16 with D % 8 != 0, D % 4 != 0 with D > 128 */
+    QR_ERR_WORKSPACE_TOO_SMALL = -4,
+    QR_ERR_CAPACITY = -5,             /* M does not fit the arithmetic of the sort (M >= 2^31) */
+    QR_ERR_CUDA = -6,                 /* a CUDA runtime call failed; qr_last_error() has its message */
+    QR_ERR_MISALIGNED = -7
+} qr_status;
+
+typedef enum { QR_F32 = 0, QR_F16 = 1 } qr_dtype;
+
+/* HOST struct.  Pinhole camera; pixel (x, y) samples the image plane at (x + 0.5, y + 0.5) (reading R5). */
+typedef struct {
+    int32_t width, height;   /* >= 1 */
+    float fx, fy, cx, cy;    /* pixels */
+    float znear;             /* > 0; a Gaussian whose camera-space z <= znear is culled */
+    float world_to_cam[12];  /* row-major 3x4 [R|t], R orthonormal; camera looks along +z, y down */
+} qr_camera;
+
+int qr_version(void);
+const char* qr_last_error(void);   /* HOST string, thread-local, valid until the next failing call on this thread */
+
+/* Number of tiles of a camera: ceil(width/16) * ceil(height/16).  Returns 0 for a NULL or zero-area camera. */
+int32_t qr_num_tiles(const qr_camera* cam);
+
+/*
+ * qr_preprocess -- PAPER.md:79 (Sigma = R S S^T R^T), PAPER.md:80/:124 (EWA splatting "following [3D-GS]"),
+ * SPEC.md:130-138, :163-168.  One thread per Gaussian, fp32, operation order fixed in DESIGN.md
+ * ("fp32 decision arithmetic") so that `depth` -- the sort key -- is reproducible bit for bit.
+ *   in : means[N,3], scales[N,3] (> 0), quats[N,4] (w,x,y,z; unit), opac[N] in (0,1)
+ *   out: mean2d[N,2] pixel coordinates; conic_opac[N,4] = (a, b, c) of cov2d^-1 and the opacity;
+ *        depth[N] camera-space z (written for every Gaussian); tile_rect[N,4] = x0,y0,x1,y1 half-open tile
+ *        rectangle of the 3-sigma AABB clamped to the tile grid; tiles_touched[N] (0 = culled; all other
+ *        outputs of a culled Gaussian except depth are 0).
+ * N = 0 is legal (nothing enqueued).
+ */
+int qr_preprocess(const qr_camera* cam, int64_t N,
+                  const float* means, const float* scales, const float* quats, const float* opac,
+                  float* mean2d, float* conic_opac, float* depth,
+                  int32_t* tile_rect, uint32_t* tiles_touched, void* stream);
+
+/*
+ * qr_bin_count -- inclusive prefix sum of tiles_touched ("(1) tiling strategy").
+ *   out: offsets[N] (uint64, inclusive scan); *M_host (HOST) = offsets[N-1] = number of intersections.
+ * Performs the one device->host read of the path and synchronises `stream`.
+ */
+size_t qr_bin_workspace_bytes(int64_t N, int64_t M_capacity, int32_t num_tiles);
+int qr_bin_count(int64_t N, const uint32_t* tiles_touched, uint64_t* offsets, int64_t* M_host,
+                 void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * qr_bin_sort -- duplication + sort + ranges ("ordered sequence of indices"; SPEC.md:139-147,
+ * :167-168; reading R6: order = ascending depth, ties by ascending Gaussian index).
+ * Each un-culled Gaussian emits one 64-bit key (tile id << 32 | IEEE bits of depth) per tile of its rectangle;
+ * keys are sorted by a stable LSD radix sort written here (8-bit digits, only the used key bits).
+ *   in : depth[N], tile_rect[N,4], offsets[N] (from qr_bin_count), M (from qr_bin_count)
+ *   out: isect_gauss[M] Gaussian ids sorted by (tile, depth, id); tile_range[T,2] = [start, end) of tile t in
+ *        isect_gauss (empty tile: start == end == number of intersections in tiles < t).
+ * ws must hold qr_bin_workspace_bytes(N, M, T) bytes.  M = 0 is legal (ranges are all [0,0)).
+ */
+int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M,
+                const float* depth, const int32_t* tile_rect, const uint64_t* offsets,
+                uint32_t* isect_gauss, int32_t* tile_range, void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * qr_forward -- Algorithm 1 for every pixel, then f~^Q = f^Q / (1 - T^Q).
+ * Inclusion rule R4: Gaussian i is in pixel p's list I iff power = -1/2 d^T conic d is in [-4.5, 0] and
+ * alpha' = min(0.99, opacity * exp(power)) >= 1/255.  Strict comparisons against 1 - (k+1)/(K+1) in fp32 (R2, R3).
+ *   in : mean2d, conic_opac (qr_preprocess); isect_gauss, tile_range (qr_bin_sort);
+ *        features[N,D] row-major, fp32 or fp16 (feat_dtype); fp16 is widened exactly, accumulation is fp32.
+ *   out: out_map[H,W,D] fp32 (HWC; 0 where nothing is selected, R8)
+ *        sel_idx[H,W,K] int32 selected Gaussian ids in depth order, -1 padded
+ *        sel_w[H,W,K]   fp32 normalised weights w^Q / (1 - T^Q), 0 padded
+ *        n_sel[H,W]     int32 number selected (<= K)
+ *        resid_TQ[H,W]  fp32 T^Q after the walk (1 where nothing is selected)
+ * K in [1, QR_MAX_K]; D in [1, QR_MAX_D]; D % 4 == 0 unless D <= 128; fp16 needs D % 8 == 0.
+ */
+size_t qr_forward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D);
+int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype,
+               const float* mean2d, const float* conic_opac,
+               const uint32_t* isect_gauss, const int32_t* tile_range, const void* features,
+               float* out_map, int32_t* sel_idx, float* sel_w, int32_t* n_sel, float* resid_TQ,
+               void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * qr_backward -- PAPER.md:37, :210.  The selection is piecewise constant in alpha' and the
+ * Gaussians are frozen, so the only gradient is
+ *     dL/dF[i,:] += sum over pixels p and slots s with sel_idx[p,s] == i of  sel_w[p,s] * dL_dmap[p,:].
+ *   in : sel_idx, sel_w, n_sel (from qr_forward), dL_dmap[H,W,D] fp32
+ *   out: dL_dfeat[N,D] fp32, ACCUMULATED INTO (the caller zeroes it; rows never selected are left untouched).
+ * Summation order over pixels is not fixed (fp32 atomics): results agree to rounding, not bit for bit.
+ */
+size_t qr_backward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D);
+int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N,
+                const int32_t* sel_idx, const float* sel_w, const int32_t* n_sel, const float* dL_dmap,
+                float* dL_dfeat, void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * qr_dense_forward -- Eq. 1: out = sum_i T_i alpha'_i f_i over the same per-pixel lists, not
+ * normalised.  Early stop R7: before blending i, T_test = T (1 - alpha'_i); if
+ * T_test < t_min stop without blending i.  t_min = 0 is exact Eq. 1.
+ *   out: out_map[H,W,D] fp32; final_T[H,W] fp32 transmittance after the last blended Gaussian.
+ */
+int qr_dense_forward(const qr_camera* cam, int32_t D, qr_dtype feat_dtype, float t_min,
+                     const float* mean2d, const float* conic_opac,
+                     const uint32_t* isect_gauss, const int32_t* tile_range, const void* features,
+                     float* out_map, float* final_T, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QR_H_ */

@@ -1,0 +1,271 @@
+"""Thin ctypes binding of libqr.so (include/qr.h): argument marshalling only.
+
+Every function has the name of the C entry point it calls and does nothing but check tensor device / dtype /
+contiguity, allocate outputs through PyTorch, pass raw device pointers plus the current CUDA stream, and turn a
+negative status into ``QRError``.  No step of the path runs in Python or in PyTorch ops.  There is no CPU fallback:
+if libqr.so cannot be loaded, or a tensor is not on a CUDA device, the call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional, Tuple
+
+import torch
+
+from . import _build
+
+QR_F32, QR_F16 = 0, 1
+QR_TILE = 16
+QR_MAX_K = 256
+QR_MAX_D = 512
+
+STATUS = {0: "QR_OK", -1: "QR_ERR_INVALID_ARG", -2: "QR_ERR_NULL_POINTER", -3: "QR_ERR_UNSUPPORTED",
+          -4: "QR_ERR_WORKSPACE_TOO_SMALL", -5: "QR_ERR_CAPACITY", -6: "QR_ERR_CUDA", -7: "QR_ERR_MISALIGNED"}
+
+# every symbol include/qr.h declares (tests check that the library exports exactly these)
+SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_bin_workspace_bytes", "qr_bin_count",
+           "qr_bin_sort", "qr_forward_workspace_bytes", "qr_forward", "qr_backward_workspace_bytes", "qr_backward",
+           "qr_dense_forward"]
+
+
+class QRError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{STATUS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class qr_camera(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float), ("znear", C.c_float), ("world_to_cam", C.c_float * 12)]
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load() -> C.CDLL:
+    """Load (building if the sources are newer) libqr.so.  Raises if it cannot be had -- no fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if os.environ.get("QR_NO_BUILD", "0") != "1":
+        try:
+            path = _build.build()
+        except Exception as e:  # nvcc missing on a box that already has the .so: use it as shipped
+            if not os.path.exists(_build.LIB):
+                raise RuntimeError(f"libqr.so is missing and cannot be built: {e}") from e
+    if not os.path.exists(path):
+        raise RuntimeError("libqr.so is missing: run `python paper_2512_20927_b200/_build.py` (no CPU fallback)")
+    lib = C.CDLL(path)
+    vp, i32, i64, sz, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_size_t, C.c_float
+    cam = C.POINTER(qr_camera)
+    lib.qr_version.restype = C.c_int
+    lib.qr_last_error.restype = C.c_char_p
+    lib.qr_num_tiles.restype = i32; lib.qr_num_tiles.argtypes = [cam]
+    lib.qr_preprocess.restype = C.c_int
+    lib.qr_preprocess.argtypes = [cam, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.qr_bin_workspace_bytes.restype = sz; lib.qr_bin_workspace_bytes.argtypes = [i64, i64, i32]
+    lib.qr_bin_count.restype = C.c_int
+    lib.qr_bin_count.argtypes = [i64, vp, vp, C.POINTER(i64), vp, sz, vp]
+    lib.qr_bin_sort.restype = C.c_int
+    lib.qr_bin_sort.argtypes = [cam, i64, i64, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.qr_forward_workspace_bytes.restype = sz; lib.qr_forward_workspace_bytes.argtypes = [cam, i32, i32]
+    lib.qr_forward.restype = C.c_int
+    lib.qr_forward.argtypes = [cam, i32, i32, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.qr_backward_workspace_bytes.restype = sz; lib.qr_backward_workspace_bytes.argtypes = [cam, i32, i32]
+    lib.qr_backward.restype = C.c_int
+    lib.qr_backward.argtypes = [cam, i32, i32, i64, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.qr_dense_forward.restype = C.c_int
+    lib.qr_dense_forward.argtypes = [cam, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp]
+    _lib = lib
+    return lib
+
+
+def _check(rc: int) -> None:
+    if rc != 0:
+        raise QRError(rc, load().qr_last_error().decode("utf-8", "replace"))
+
+
+def make_camera(cam) -> qr_camera:
+    """From any object with width, height, fx, fy, cx, cy, znear, world_to_cam (e.g. qr_inputs.Camera)."""
+    if isinstance(cam, qr_camera):
+        return cam
+    c = qr_camera()
+    c.width, c.height = int(cam.width), int(cam.height)
+    c.fx, c.fy, c.cx, c.cy, c.znear = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy), float(cam.znear)
+    w = [float(v) for v in list(cam.world_to_cam.reshape(-1))]
+    for i in range(12):
+        c.world_to_cam[i] = w[i]
+    return c
+
+
+def _dev(t: torch.Tensor, dtype, name: str) -> int:
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise QRError(-1, f"{name} must be a CUDA tensor (libqr has no CPU path)")
+    if t.dtype != dtype:
+        raise QRError(-1, f"{name} must have dtype {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise QRError(-1, f"{name} must be contiguous")
+    return t.data_ptr()
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def qr_version() -> int:
+    return int(load().qr_version())
+
+
+def qr_num_tiles(cam) -> int:
+    c = make_camera(cam)
+    return int(load().qr_num_tiles(C.byref(c)))
+
+
+@dataclass
+class Projected:
+    mean2d: torch.Tensor         # [N,2] f32
+    conic_opac: torch.Tensor     # [N,4] f32
+    depth: torch.Tensor          # [N] f32
+    tile_rect: torch.Tensor      # [N,4] i32
+    tiles_touched: torch.Tensor  # [N] u32 stored as int32 bits
+
+
+def qr_preprocess(cam, means, scales, quats, opac) -> Projected:
+    c = make_camera(cam)
+    n = int(means.shape[0])
+    dev = means.device
+    out = Projected(torch.empty((n, 2), dtype=torch.float32, device=dev),
+                    torch.empty((n, 4), dtype=torch.float32, device=dev),
+                    torch.empty((n,), dtype=torch.float32, device=dev),
+                    torch.empty((n, 4), dtype=torch.int32, device=dev),
+                    torch.empty((n,), dtype=torch.int32, device=dev))
+    _check(load().qr_preprocess(C.byref(c), n, _dev(means, torch.float32, "means"), _dev(scales, torch.float32, "scales"),
+                                _dev(quats, torch.float32, "quats"), _dev(opac, torch.float32, "opac"),
+                                out.mean2d.data_ptr(), out.conic_opac.data_ptr(), out.depth.data_ptr(),
+                                out.tile_rect.data_ptr(), out.tiles_touched.data_ptr(), _stream()))
+    return out
+
+
+def qr_bin_workspace_bytes(N: int, M: int, num_tiles: int) -> int:
+    return int(load().qr_bin_workspace_bytes(int(N), int(M), int(num_tiles)))
+
+
+def qr_bin_count(tiles_touched: torch.Tensor, ws: Optional[torch.Tensor] = None) -> Tuple[torch.Tensor, int]:
+    """Returns (offsets[N] as int64 bits of the uint64 inclusive scan, M)."""
+    n = int(tiles_touched.shape[0])
+    dev = tiles_touched.device
+    offsets = torch.empty((n,), dtype=torch.int64, device=dev)
+    if ws is None:
+        ws = torch.empty((max(qr_bin_workspace_bytes(n, 0, 0), 16),), dtype=torch.uint8, device=dev)
+    m = C.c_int64(0)
+    _check(load().qr_bin_count(n, _dev(tiles_touched, torch.int32, "tiles_touched"), offsets.data_ptr(), C.byref(m),
+                               ws.data_ptr(), ws.numel(), _stream()))
+    return offsets, int(m.value)
+
+
+def qr_bin_sort(cam, M: int, depth, tile_rect, offsets, ws: Optional[torch.Tensor] = None,
+                isect_gauss: Optional[torch.Tensor] = None, tile_range: Optional[torch.Tensor] = None):
+    """Returns (isect_gauss[M] int32 bits of the uint32 ids, tile_range[T,2] int32)."""
+    c = make_camera(cam)
+    n = int(depth.shape[0])
+    dev = depth.device
+    T = qr_num_tiles(c)
+    if isect_gauss is None:
+        isect_gauss = torch.empty((max(M, 1),), dtype=torch.int32, device=dev)
+    if tile_range is None:
+        tile_range = torch.empty((T, 2), dtype=torch.int32, device=dev)
+    if ws is None:
+        ws = torch.empty((max(qr_bin_workspace_bytes(n, M, T), 16),), dtype=torch.uint8, device=dev)
+    _check(load().qr_bin_sort(C.byref(c), n, int(M), _dev(depth, torch.float32, "depth"),
+                              _dev(tile_rect, torch.int32, "tile_rect"), _dev(offsets, torch.int64, "offsets"),
+                              isect_gauss.data_ptr(), tile_range.data_ptr(), ws.data_ptr(), ws.numel(), _stream()))
+    return isect_gauss[:M], tile_range
+
+
+@dataclass
+class ForwardOut:
+    out_map: torch.Tensor   # [H,W,D] f32
+    sel_idx: torch.Tensor   # [H,W,K] i32
+    sel_w: torch.Tensor     # [H,W,K] f32
+    n_sel: torch.Tensor     # [H,W] i32
+    resid_TQ: torch.Tensor  # [H,W] f32
+
+
+def _feat_dtype(features: torch.Tensor) -> int:
+    if features.dtype == torch.float32:
+        return QR_F32
+    if features.dtype == torch.float16:
+        return QR_F16
+    raise QRError(-1, f"features must be float32 or float16, got {features.dtype}")
+
+
+def qr_forward_workspace_bytes(cam, K: int, D: int) -> int:
+    c = make_camera(cam)
+    return int(load().qr_forward_workspace_bytes(C.byref(c), int(K), int(D)))
+
+
+def qr_forward(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, features,
+               out: Optional[ForwardOut] = None) -> ForwardOut:
+    c = make_camera(cam)
+    H, W = c.height, c.width
+    D = int(features.shape[1])
+    dev = features.device
+    dt = _feat_dtype(features)
+    if out is None:
+        kk = max(int(K), 1)
+        out = ForwardOut(torch.empty((H, W, D), dtype=torch.float32, device=dev),
+                         torch.empty((H, W, kk), dtype=torch.int32, device=dev),
+                         torch.empty((H, W, kk), dtype=torch.float32, device=dev),
+                         torch.empty((H, W), dtype=torch.int32, device=dev),
+                         torch.empty((H, W), dtype=torch.float32, device=dev))
+    _check(load().qr_forward(C.byref(c), int(K), D, dt, _dev(mean2d, torch.float32, "mean2d"),
+                             _dev(conic_opac, torch.float32, "conic_opac"),
+                             _dev(isect_gauss, torch.int32, "isect_gauss"), _dev(tile_range, torch.int32, "tile_range"),
+                             _dev(features, features.dtype, "features"), out.out_map.data_ptr(), out.sel_idx.data_ptr(),
+                             out.sel_w.data_ptr(), out.n_sel.data_ptr(), out.resid_TQ.data_ptr(), None, 0, _stream()))
+    return out
+
+
+def qr_backward_workspace_bytes(cam, K: int, D: int) -> int:
+    c = make_camera(cam)
+    return int(load().qr_backward_workspace_bytes(C.byref(c), int(K), int(D)))
+
+
+def qr_backward(cam, N: int, sel_idx, sel_w, n_sel, dL_dmap, dL_dfeat: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Accumulates into dL_dfeat[N,D] (allocated zero-filled when not given)."""
+    c = make_camera(cam)
+    K = int(sel_idx.shape[-1])
+    D = int(dL_dmap.shape[-1])
+    if dL_dfeat is None:
+        dL_dfeat = torch.zeros((int(N), D), dtype=torch.float32, device=dL_dmap.device)
+    _check(load().qr_backward(C.byref(c), K, D, int(N), _dev(sel_idx, torch.int32, "sel_idx"),
+                              _dev(sel_w, torch.float32, "sel_w"), _dev(n_sel, torch.int32, "n_sel"),
+                              _dev(dL_dmap, torch.float32, "dL_dmap"), _dev(dL_dfeat, torch.float32, "dL_dfeat"),
+                              None, 0, _stream()))
+    return dL_dfeat
+
+
+def qr_dense_forward(cam, mean2d, conic_opac, isect_gauss, tile_range, features, t_min: float = 1e-4,
+                     out_map: Optional[torch.Tensor] = None, final_T: Optional[torch.Tensor] = None):
+    c = make_camera(cam)
+    H, W = c.height, c.width
+    D = int(features.shape[1])
+    dev = features.device
+    if out_map is None:
+        out_map = torch.empty((H, W, D), dtype=torch.float32, device=dev)
+    if final_T is None:
+        final_T = torch.empty((H, W), dtype=torch.float32, device=dev)
+    _check(load().qr_dense_forward(C.byref(c), D, _feat_dtype(features), float(t_min),
+                                   _dev(mean2d, torch.float32, "mean2d"), _dev(conic_opac, torch.float32, "conic_opac"),
+                                   _dev(isect_gauss, torch.int32, "isect_gauss"),
+                                   _dev(tile_range, torch.int32, "tile_range"),
+                                   _dev(features, features.dtype, "features"), out_map.data_ptr(), final_T.data_ptr(),
+                                   _stream()))
+    return out_map, final_T

@@ -1,0 +1,309 @@
+// qr_backward.cu -- dL/dF scatter-add:
+//     dL/dF[i,:] += sum_{p, s : sel_idx[p,s] = i}  sel_w[p,s] * dL_dmap[p,:]
+// The selection is piecewise constant in alpha' and the Gaussians are frozen: no other term exists.
+//
+// Band kernel (K <= kBwdMaxK): CTA = one 16x4-pixel band (64 pixels), 256 threads.
+//   1. the band's selection records are read once (coalesced) into shared memory;
+//   2. the distinct selected Gaussians of the band (the band union, ~35 rows at K = 40) are numbered with a
+//      shared-memory hash set, and the records are scattered into a dense weight block Wr[pixel][64 union rows];
+//   3. warp w owns 8 union rows x all D channels in registers (lane = 4 consecutive channels per 128-channel slab),
+//      walks the 64 pixels, loads dL_dmap[p,:] (128-bit coalesced) only if the pixel selected one of its rows and
+//      accumulates w * g from registers;
+//   4. one vector red.global.add per (union row, 4 channels): global atomics drop from (sum of n_sel) * D to
+//      (band union) * D -- a 25x pre-reduction at K = 40.
+// Pixel kernel (any K): one warp per pixel, vector atomics per selected row -- the plain statement, used for
+// K > kBwdMaxK.
+#include "qr_common.cuh"
+
+namespace qr {
+
+constexpr int kBwdThreads = 256;
+constexpr int kBwdPx = 64;        // 16 x 4 pixels per CTA
+constexpr int kBwdRows = 64;      // union rows per pass (8 warps x 8 rows)
+constexpr int kBwdMaxK = 64;
+
+struct BackwardParams {
+    Cam cam;
+    int32_t K, D;
+    int64_t N;
+    const int32_t* sel_idx;
+    const float* sel_w;
+    const int32_t* n_sel;
+    const float* dL_dmap;
+    float* dL_dfeat;
+};
+
+template <int VW> __device__ __forceinline__ void load_g(const float* src, float (&g)[VW]);
+template <> __device__ __forceinline__ void load_g<4>(const float* src, float (&g)[4])
+{
+    const float4 v = __ldg(reinterpret_cast<const float4*>(src));
+    g[0] = v.x; g[1] = v.y; g[2] = v.z; g[3] = v.w;
+}
+template <> __device__ __forceinline__ void load_g<1>(const float* src, float (&g)[1]) { g[0] = __ldg(src); }
+
+template <int VW> __device__ __forceinline__ void red_add(float* dst, const float (&a)[VW]);
+template <> __device__ __forceinline__ void red_add<4>(float* dst, const float (&a)[4])
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(a[0]), "f"(a[1]), "f"(a[2]), "f"(a[3])
+                 : "memory");
+}
+template <> __device__ __forceinline__ void red_add<1>(float* dst, const float (&a)[1]) { atomicAdd(dst, a[0]); }
+
+__device__ __forceinline__ uint32_t hash_id(uint32_t x)
+{
+    x ^= x >> 16; x *= 0x7feb352dU; x ^= x >> 15; x *= 0x846ca68bU; x ^= x >> 16;
+    return x;
+}
+
+template <int NV, int VW>
+__global__ void __launch_bounds__(kBwdThreads, 1) backward_band_kernel(const BackwardParams p, const int hs_max /*pow2*/)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int K = p.K, D = p.D;
+    float* Wr = reinterpret_cast<float*>(smem_raw);                     // [64 px][64 rows]
+    int32_t* rec_slot = reinterpret_cast<int32_t*>(Wr + kBwdPx * kBwdRows);   // [64][K] id, later union slot
+    float* rec_w = reinterpret_cast<float*>(rec_slot + kBwdPx * K);     // [64][K]
+    int32_t* nsel_s = reinterpret_cast<int32_t*>(rec_w + kBwdPx * K);   // [64]
+    int32_t* hkey = nsel_s + kBwdPx;                                    // [hs_max]
+    int32_t* hslot = hkey + hs_max;                                     // [hs_max]
+    int32_t* uid = hslot + hs_max;                                          // [64*K] union slot -> Gaussian id
+    __shared__ int32_t ucount;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tile = blockIdx.x >> 2, band = blockIdx.x & 3;
+    const int tile_x = tile % p.cam.tiles_x, tile_y = tile / p.cam.tiles_x;
+    const int x0 = tile_x * kTile, y0 = tile_y * kTile + band * 4;
+    if (y0 >= p.cam.height) return;
+    const int npx = min(kTile, p.cam.width - x0);
+
+    // ---- 1. records -> shared ----
+    if (tid == 0) ucount = 0;
+    if (tid < kBwdPx) {
+        const int px = x0 + (tid & 15), py = y0 + (tid >> 4);
+        nsel_s[tid] = (px < p.cam.width && py < p.cam.height) ? p.n_sel[(int64_t)py * p.cam.width + px] : 0;
+    }
+    __syncthreads();
+    int total = 0;
+    for (int i = 0; i < kBwdPx; ++i) total += nsel_s[i];    // broadcast reads; same value in every thread
+    if (total == 0) return;                                  // uniform: nothing selected in this band
+    int hs = 64;
+    while (hs < 2 * total) hs <<= 1;                         // <= hs_max by construction (total <= 64 K)
+    for (int i = tid; i < hs; i += kBwdThreads) hkey[i] = -1;
+    for (int r = 0; r < 4; ++r) {
+        const int py = y0 + r;
+        if (py >= p.cam.height) break;
+        const int64_t gbase = ((int64_t)py * p.cam.width + x0) * K;
+        for (int i = tid; i < npx * K; i += kBwdThreads) {
+            rec_slot[r * 16 * K + i] = p.sel_idx[gbase + i];
+            rec_w[r * 16 * K + i] = p.sel_w[gbase + i];
+        }
+    }
+    __syncthreads();
+
+    // ---- 2a. insert ids into the hash set ----
+    const int hmask = hs - 1;
+    for (int i = tid; i < kBwdPx * K; i += kBwdThreads) {
+        const int lp = i / K, s = i - lp * K;
+        if (s < nsel_s[lp]) {
+            const int32_t id = rec_slot[i];
+            uint32_t h = hash_id((uint32_t)id) & hmask;
+            while (true) {
+                const int32_t old = atomicCAS(&hkey[h], -1, id);
+                if (old == -1 || old == id) break;
+                h = (h + 1) & hmask;
+            }
+        }
+    }
+    __syncthreads();
+    // ---- 2b. number the occupied cells ----
+    for (int i = tid; i < hs; i += kBwdThreads) {
+        const int32_t id = hkey[i];
+        if (id >= 0) {
+            const int slot = atomicAdd(&ucount, 1);
+            hslot[i] = slot;
+            uid[slot] = id;
+        }
+    }
+    __syncthreads();
+    // ---- 2c. records: id -> union slot ----
+    for (int i = tid; i < kBwdPx * K; i += kBwdThreads) {
+        const int lp = i / K, s = i - lp * K;
+        if (s < nsel_s[lp]) {
+            const int32_t id = rec_slot[i];
+            uint32_t h = hash_id((uint32_t)id) & hmask;
+            while (hkey[h] != id) h = (h + 1) & hmask;
+            rec_slot[i] = hslot[h];
+        }
+    }
+    const int U = ucount;
+    __syncthreads();
+
+    // ---- 3. passes of 64 union rows ----
+    for (int c0 = 0; c0 < U; c0 += kBwdRows) {
+        for (int i = tid; i < kBwdPx * kBwdRows; i += kBwdThreads) Wr[i] = 0.0f;
+        __syncthreads();
+        for (int i = tid; i < kBwdPx * K; i += kBwdThreads) {
+            const int lp = i / K, s = i - lp * K;
+            if (s < nsel_s[lp]) {
+                const int slot = rec_slot[i] - c0;
+                if (slot >= 0 && slot < kBwdRows) Wr[lp * kBwdRows + slot] = rec_w[i];
+            }
+        }
+        __syncthreads();
+
+        if (c0 + warp * 8 < U) {     // this warp owns rows c0 + warp*8 .. +7
+            float acc[8][NV][VW];
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int j = 0; j < NV; ++j)
+#pragma unroll
+                    for (int v = 0; v < VW; ++v) acc[r][j][v] = 0.0f;
+
+            for (int lp = 0; lp < kBwdPx; ++lp) {
+                const float4 w0 = *reinterpret_cast<const float4*>(Wr + lp * kBwdRows + warp * 8);
+                const float4 w1 = *reinterpret_cast<const float4*>(Wr + lp * kBwdRows + warp * 8 + 4);
+                const float w[8] = { w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w };
+                bool any = false;
+#pragma unroll
+                for (int r = 0; r < 8; ++r) any |= (w[r] != 0.0f);
+                if (!any) continue;          // uniform
+                const int px = x0 + (lp & 15), py = y0 + (lp >> 4);
+                const float* grow = p.dL_dmap + ((int64_t)py * p.cam.width + px) * D;
+                float g[NV][VW];
+#pragma unroll
+                for (int j = 0; j < NV; ++j) {
+                    const int ch = (j * 32 + lane) * VW;
+                    if (ch < D) load_g<VW>(grow + ch, g[j]);
+                    else {
+#pragma unroll
+                        for (int v = 0; v < VW; ++v) g[j][v] = 0.0f;
+                    }
+                }
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    if (w[r] != 0.0f) {
+#pragma unroll
+                        for (int j = 0; j < NV; ++j)
+#pragma unroll
+                            for (int v = 0; v < VW; ++v) acc[r][j][v] = __fmaf_rn(w[r], g[j][v], acc[r][j][v]);
+                    }
+                }
+            }
+            // ---- 4. one vector reduction per (row, channel vector) ----
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                const int slot = c0 + warp * 8 + r;
+                if (slot < U) {
+                    float* drow = p.dL_dfeat + (int64_t)uid[slot] * D;
+#pragma unroll
+                    for (int j = 0; j < NV; ++j) {
+                        const int ch = (j * 32 + lane) * VW;
+                        if (ch < D) red_add<VW>(drow + ch, acc[r][j]);
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// plain statement: one warp per pixel
+template <int NV, int VW>
+__global__ void __launch_bounds__(256) backward_pixel_kernel(const BackwardParams p)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t pix = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (pix >= (int64_t)p.cam.width * p.cam.height) return;
+    const int ns = p.n_sel[pix];
+    if (ns == 0) return;
+    const int D = p.D, K = p.K;
+    float g[NV][VW];
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+        const int ch = (j * 32 + lane) * VW;
+        if (ch < D) load_g<VW>(p.dL_dmap + pix * D + ch, g[j]);
+    }
+    for (int s = 0; s < ns; ++s) {
+        const int32_t id = p.sel_idx[pix * K + s];
+        const float w = p.sel_w[pix * K + s];
+        float* drow = p.dL_dfeat + (int64_t)id * D;
+#pragma unroll
+        for (int j = 0; j < NV; ++j) {
+            const int ch = (j * 32 + lane) * VW;
+            if (ch < D) {
+                float a[VW];
+#pragma unroll
+                for (int v = 0; v < VW; ++v) a[v] = __fmul_rn(w, g[j][v]);
+                red_add<VW>(drow + ch, a);
+            }
+        }
+    }
+}
+
+static int next_pow2(int v) { int p = 1; while (p < v) p <<= 1; return p; }
+
+template <int NV, int VW>
+static int launch_backward(const BackwardParams& p, cudaStream_t st)
+{
+    const int T = p.cam.tiles_x * p.cam.tiles_y;
+    if (p.K <= kBwdMaxK) {
+        const int hs = next_pow2(2 * kBwdPx * p.K);
+        const size_t smem = (size_t)kBwdPx * kBwdRows * 4 + 2 * (size_t)kBwdPx * p.K * 4 + kBwdPx * 4 +
+                            2 * (size_t)hs * 4 + (size_t)kBwdPx * p.K * 4;
+        auto kern = backward_band_kernel<NV, VW>;
+        QR_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<(unsigned)T * 4u, kBwdThreads, smem, st>>>(p, hs);
+        QR_LAUNCH_OK("backward_band_kernel");
+    } else {
+        const int64_t npix = (int64_t)p.cam.width * p.cam.height;
+        backward_pixel_kernel<NV, VW><<<(unsigned)((npix + 7) / 8), 256, 0, st>>>(p);
+        QR_LAUNCH_OK("backward_pixel_kernel");
+    }
+    return QR_OK;
+}
+
+}  // namespace qr
+
+extern "C" size_t qr_backward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D)
+{
+    (void)cam; (void)K; (void)D;
+    return 0;
+}
+
+extern "C" int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N, const int32_t* sel_idx,
+                           const float* sel_w, const int32_t* n_sel, const float* dL_dmap, float* dL_dfeat, void* ws,
+                           size_t ws_bytes, void* stream)
+{
+    using namespace qr;
+    (void)ws; (void)ws_bytes;
+    if (int rc = check_cam(cam)) return rc;
+    if (K < 1) return fail(QR_ERR_INVALID_ARG, "qr_backward: K = %d < 1", K);
+    if (K > QR_MAX_K) return fail(QR_ERR_UNSUPPORTED, "qr_backward: K = %d > QR_MAX_K", K);
+    if (D < 1) return fail(QR_ERR_INVALID_ARG, "qr_backward: D = %d < 1", D);
+    if (D > QR_MAX_D) return fail(QR_ERR_UNSUPPORTED, "qr_backward: D = %d > QR_MAX_D", D);
+    if (D % 4 != 0 && D > 128) return fail(QR_ERR_UNSUPPORTED, "qr_backward: D %% 4 != 0 is only supported for D <= 128");
+    if (N < 0) return fail(QR_ERR_INVALID_ARG, "qr_backward: N < 0");
+    if (!sel_idx || !sel_w || !n_sel || !dL_dmap) return fail(QR_ERR_NULL_POINTER, "qr_backward: NULL input");
+    if (N == 0) return QR_OK;
+    if (!dL_dfeat) return fail(QR_ERR_NULL_POINTER, "qr_backward: dL_dfeat is NULL");
+    if (!aligned16(dL_dmap) || !aligned16(dL_dfeat)) return fail(QR_ERR_MISALIGNED, "qr_backward: 16-byte alignment");
+    BackwardParams p;
+    p.cam = make_cam(cam); p.K = K; p.D = D; p.N = N;
+    p.sel_idx = sel_idx; p.sel_w = sel_w; p.n_sel = n_sel; p.dL_dmap = dL_dmap; p.dL_dfeat = dL_dfeat;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (D % 4 == 0) {
+        switch ((D + 127) / 128) {
+            case 1: return launch_backward<1, 4>(p, st);
+            case 2: return launch_backward<2, 4>(p, st);
+            case 3: return launch_backward<3, 4>(p, st);
+            default: return launch_backward<4, 4>(p, st);
+        }
+    }
+    switch ((D + 31) / 32) {
+        case 1: return launch_backward<1, 1>(p, st);
+        case 2: return launch_backward<2, 1>(p, st);
+        case 3: return launch_backward<3, 1>(p, st);
+        default: return launch_backward<4, 1>(p, st);
+    }
+}

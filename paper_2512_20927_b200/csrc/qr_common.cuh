@@ -1,0 +1,62 @@
+// qr_common.cuh -- shared host/device helpers of libqr (sm_100a).  Product code: nothing here is used by oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdarg.h>
+
+#include "../../include/qr.h"
+
+namespace qr {
+
+// Conventions of DESIGN.md "Readings" (R4; R12).
+constexpr float kAlphaMin = 1.0f / 255.0f;
+constexpr float kAlphaMax = 0.99f;
+constexpr float kPowerMin = -4.5f;
+constexpr float kDilation = 0.3f;
+constexpr float kJClamp = 1.3f;
+constexpr int kTile = QR_TILE;
+
+// Camera as passed to kernels (by value, in constant bank).
+struct Cam {
+    int32_t width, height;
+    float fx, fy, cx, cy, znear;
+    float w[12];
+    int32_t tiles_x, tiles_y;
+};
+
+inline Cam make_cam(const qr_camera* c)
+{
+    Cam k;
+    k.width = c->width; k.height = c->height;
+    k.fx = c->fx; k.fy = c->fy; k.cx = c->cx; k.cy = c->cy; k.znear = c->znear;
+    for (int i = 0; i < 12; ++i) k.w[i] = c->world_to_cam[i];
+    k.tiles_x = (c->width + kTile - 1) / kTile;
+    k.tiles_y = (c->height + kTile - 1) / kTile;
+    return k;
+}
+
+// Thread-local error string (qr_last_error).
+char* err_buf();
+int fail(int code, const char* fmt, ...);
+int check_cam(const qr_camera* cam);
+
+#define QR_CUDA_OK(expr)                                                                       \
+    do {                                                                                       \
+        cudaError_t e__ = (expr);                                                              \
+        if (e__ != cudaSuccess)                                                                \
+            return qr::fail(QR_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(e__));     \
+    } while (0)
+
+#define QR_LAUNCH_OK(name)                                                                     \
+    do {                                                                                       \
+        cudaError_t e__ = cudaGetLastError();                                                  \
+        if (e__ != cudaSuccess)                                                                \
+            return qr::fail(QR_ERR_CUDA, "launch of %s failed: %s", name, cudaGetErrorString(e__)); \
+    } while (0)
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace qr

@@ -1,0 +1,40 @@
+"""Call sequences over the binding (no arithmetic): the front end (qr_preprocess -> qr_bin_count -> qr_bin_sort),
+Q-Render forward / backward and the dense comparator.  Everything stays on the device except M (one int64)."""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Optional
+
+import torch
+
+from . import binding as B
+
+
+@dataclass
+class Frontend:
+    proj: B.Projected
+    offsets: torch.Tensor
+    M: int
+    isect_gauss: torch.Tensor
+    tile_range: torch.Tensor
+
+
+def frontend(cam, means, scales, quats, opac) -> Frontend:
+    """PAPER.md:80 steps (1) tiling and (2) splatting: projection, intersection count, duplication + sort."""
+    proj = B.qr_preprocess(cam, means, scales, quats, opac)
+    offsets, M = B.qr_bin_count(proj.tiles_touched)
+    isect, rng = B.qr_bin_sort(cam, M, proj.depth, proj.tile_rect, offsets)
+    return Frontend(proj, offsets, M, isect, rng)
+
+
+def forward(cam, fe: Frontend, features: torch.Tensor, K: int, out: Optional[B.ForwardOut] = None) -> B.ForwardOut:
+    return B.qr_forward(cam, K, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, out)
+
+
+def backward(cam, N: int, fwd: B.ForwardOut, dL_dmap: torch.Tensor, dL_dfeat: Optional[torch.Tensor] = None):
+    return B.qr_backward(cam, N, fwd.sel_idx, fwd.sel_w, fwd.n_sel, dL_dmap, dL_dfeat)
+
+
+def dense_forward(cam, fe: Frontend, features: torch.Tensor, t_min: float = 1e-4, out_map=None, final_T=None):
+    return B.qr_dense_forward(cam, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, t_min,
+                              out_map, final_T)

@@ -1,0 +1,291 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Stage-isolated (each GPU stage fed the oracle's upstream outputs) and end to end, at sizes the oracle finishes in
+seconds that still span several tiles and ragged tails, plus sampled checks at BASELINE.json's config-3 size.
+"""
+import numpy as np
+import pytest
+import torch
+
+from qr_inputs import make_scene, make_camera
+import parity as P
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def qr():
+    import paper_2512_20927_b200 as q
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    q.binding.load()
+    return q
+
+
+def _i32(t):
+    return t.cpu().numpy()
+
+
+# ------------------------------------------------------------------------------------------------
+# qr_preprocess: bit-exact against the oracle's fp32 decision arithmetic
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,kw", [("cfg1", {}), ("cfg2", dict(N=20000)), ("cfg3", dict(N=60000, W=200, H=120, D=8)),
+                                     ("cfg4", dict(N=60000, W=160, H=96, D=8, pose=3, feat_dtype="f32"))])
+def test_preprocess_bit_exact(qr, orc, name, kw):
+    sc = make_scene(name, seed=1, **kw)
+    g = P.upload(sc)
+    pr = qr.qr_preprocess(sc.cam, g.means, g.scales, g.quats, g.opac)
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    rect, touched = orc.tile_rects(sc.cam, proj)
+    np.testing.assert_array_equal(pr.depth.cpu().numpy().view(np.uint32), proj.depth.view(np.uint32))
+    np.testing.assert_array_equal(pr.mean2d.cpu().numpy().view(np.uint32), proj.mean2d.view(np.uint32))
+    np.testing.assert_array_equal(pr.conic_opac.cpu().numpy().view(np.uint32), proj.conic_opac.view(np.uint32))
+    np.testing.assert_array_equal(_i32(pr.tile_rect), rect)
+    np.testing.assert_array_equal(_i32(pr.tiles_touched).view(np.uint32), touched)
+    assert touched.sum() > 0
+
+
+# ------------------------------------------------------------------------------------------------
+# qr_bin_count / qr_bin_sort: exact lists and ranges
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,kw", [("cfg1", {}), ("cfg2", dict(N=30000)), ("cfg3", dict(N=80000, W=330, H=250, D=8))])
+def test_bin_sort_exact(qr, orc, name, kw):
+    sc = make_scene(name, seed=2, **kw)
+    proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
+    # stage-isolated: feed the oracle's projection
+    offsets, M = qr.qr_bin_count(P.to_dev(touched.view(np.int32)))
+    assert M == int(touched.sum()) == len(isect)
+    np.testing.assert_array_equal(offsets.cpu().numpy(), np.cumsum(touched.astype(np.int64)))
+    ig, tr = qr.qr_bin_sort(sc.cam, M, P.to_dev(proj.depth), P.to_dev(rect), offsets)
+    np.testing.assert_array_equal(_i32(ig).view(np.uint32), isect)
+    np.testing.assert_array_equal(_i32(tr), rng)
+    # end to end
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    assert fe.M == M
+    np.testing.assert_array_equal(_i32(fe.isect_gauss).view(np.uint32), isect)
+    np.testing.assert_array_equal(_i32(fe.tile_range), rng)
+
+
+def test_bin_sort_depth_ties_break_by_index(qr, orc):
+    """R6: equal depths keep ascending Gaussian index (stable sort)."""
+    sc = make_scene("cfg1", seed=3, N=600)
+    sc.means[:, 2] = np.float32(3.0)             # all depths equal
+    proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    np.testing.assert_array_equal(_i32(fe.isect_gauss).view(np.uint32), isect)
+    for t in range(rng.shape[0]):
+        ids = isect[rng[t, 0]:rng[t, 1]]
+        assert (np.diff(ids.astype(np.int64)) > 0).all()
+
+
+def test_bin_empty_scene(qr):
+    """Everything culled (behind the camera): M = 0, all ranges empty, forward renders zeros."""
+    sc = make_scene("cfg1", seed=0, N=50)
+    sc.means[:, 2] = -1.0
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    assert fe.M == 0
+    assert (fe.tile_range.cpu().numpy() == 0).all()
+    out = qr.pipeline.forward(sc.cam, fe, g.features, 40)
+    assert (out.out_map == 0).all() and (out.n_sel == 0).all() and (out.resid_TQ == 1).all()
+    assert (out.sel_idx == -1).all() and (out.sel_w == 0).all()
+
+
+# ------------------------------------------------------------------------------------------------
+# qr_forward
+# ------------------------------------------------------------------------------------------------
+FWD_CASES = [
+    ("cfg1", dict(), 40),                                       # BASELINE config 1 as given
+    ("cfg1", dict(W=70, H=50, D=3), 40),                        # ragged tiles, scalar-channel path
+    ("cfg1", dict(W=33, H=17, D=20), 1),                        # K = 1
+    ("cfg1", dict(D=132), 7),                                   # D % 128 != 0
+    ("cfg2", dict(N=20000, W=128, H=96), 40),
+    ("cfg2", dict(N=20000, W=96, H=64, D=256), 64),
+    ("cfg3", dict(N=60000, W=160, H=112, D=512), 40),           # blob scene, camera inside, D = 512
+    ("cfg3", dict(N=60000, W=96, H=64, D=384), 10),
+    ("cfg3", dict(N=40000, W=96, H=64, D=64), 200),             # K large
+]
+
+
+@pytest.mark.parametrize("name,kw,K", FWD_CASES)
+def test_forward_stage_isolated(qr, orc, name, kw, K):
+    sc = make_scene(name, seed=4, **kw)
+    proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
+    lists = orc.pixel_lists(sc.cam, proj)
+    q = orc.qrender(lists, K, sc.features)
+    out = qr.qr_forward(sc.cam, K, P.to_dev(proj.mean2d), P.to_dev(proj.conic_opac),
+                        P.to_dev(isect.view(np.int32)), P.to_dev(rng), P.to_dev(sc.features))
+    stats = P.compare_forward(out, q, lists, K, sc.D)
+    assert stats["exempt"] < 0.01 * stats["pixels"] + 5, stats
+    print(name, kw, K, stats)
+
+
+@pytest.mark.parametrize("name,kw,K", [FWD_CASES[0], FWD_CASES[4], FWD_CASES[6]])
+def test_forward_end_to_end(qr, orc, name, kw, K):
+    sc = make_scene(name, seed=5, **kw)
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    out = qr.pipeline.forward(sc.cam, fe, g.features, K)
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    lists = orc.pixel_lists(sc.cam, proj)
+    q = orc.qrender(lists, K, sc.features)
+    stats = P.compare_forward(out, q, lists, K, sc.D)
+    print(stats)
+
+
+def test_forward_fp16_features(qr, orc):
+    sc = make_scene("cfg4", seed=6, N=60000, W=128, H=96, D=512, pose=2)      # fp16 storage, fp32 accumulation (R14)
+    assert sc.features.dtype == np.float16
+    proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
+    lists = orc.pixel_lists(sc.cam, proj)
+    for K in (4, 32):
+        q = orc.qrender(lists, K, sc.features)
+        out = qr.qr_forward(sc.cam, K, P.to_dev(proj.mean2d), P.to_dev(proj.conic_opac),
+                            P.to_dev(isect.view(np.int32)), P.to_dev(rng), P.to_dev(sc.features))
+        P.compare_forward(out, q, lists, K, sc.D, f16=True)
+
+
+def test_forward_invariants_full_scale(qr):
+    """Properties that hold at any size, checked on the GPU output of a mid-size scene."""
+    sc = make_scene("cfg3", seed=7, N=200000, W=320, H=240, D=128)
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    K = 40
+    out = qr.pipeline.forward(sc.cam, fe, g.features, K)
+    n_sel = out.n_sel.cpu().numpy()
+    w = out.sel_w.cpu().numpy().astype(np.float64)
+    assert n_sel.max() <= K and n_sel.min() >= 0
+    assert (w >= 0).all()
+    has = n_sel > 0
+    np.testing.assert_allclose(w.sum(-1)[has], 1.0, atol=1e-5)   # convex combination (G3); 1 - T^Q can be ~0.03 in fp32
+    # constant feature scene: out == f wherever something is selected (G5)
+    const = torch.ones_like(g.features) * 0.25
+    out_c = qr.pipeline.forward(sc.cam, fe, const, K)
+    np.testing.assert_allclose(out_c.out_map.cpu().numpy()[has], 0.25, rtol=1e-5)
+    assert torch.equal(out_c.sel_idx, out.sel_idx)                              # selection independent of payload (G6)
+    # payload width independence
+    out_3 = qr.pipeline.forward(sc.cam, fe, g.features[:, :3].contiguous(), K)
+    assert torch.equal(out_3.sel_idx, out.sel_idx)
+    np.testing.assert_allclose(out_3.out_map.cpu().numpy(), out.out_map[..., :3].cpu().numpy(), rtol=1e-6, atol=1e-7)
+
+
+# ------------------------------------------------------------------------------------------------
+# qr_dense_forward (Eq. 1)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,kw,t_min", [("cfg1", dict(), 1e-4), ("cfg1", dict(W=70, H=50, D=3), 0.0),
+                                           ("cfg3", dict(N=60000, W=128, H=80, D=512), 1e-4),
+                                           ("cfg2", dict(N=20000, W=96, H=96), 0.0)])
+def test_dense_forward(qr, orc, name, kw, t_min):
+    sc = make_scene(name, seed=8, **kw)
+    proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
+    lists = orc.pixel_lists(sc.cam, proj)
+    v = orc.vrender(lists, sc.features, t_min=t_min)
+    om, fT = qr.qr_dense_forward(sc.cam, P.to_dev(proj.mean2d), P.to_dev(proj.conic_opac),
+                                 P.to_dev(isect.view(np.int32)), P.to_dev(rng), P.to_dev(sc.features), t_min)
+    H, W = sc.cam.height, sc.cam.width
+    om = om.cpu().numpy().reshape(H * W, -1).astype(np.float64); fT = fT.cpu().numpy().reshape(-1)
+    ok = ~((v.stop_margin <= 1e-5) | lists.borderline.astype(bool))       # early-stop decision within rounding
+    assert ok.mean() > 0.99
+    ref = v.out_map.astype(np.float64)
+    tol = P.ATOL + P.RTOL * np.abs(ref)
+    assert (np.abs(om - ref)[ok] <= tol[ok]).all()
+    np.testing.assert_allclose(fT[ok], v.final_T[ok], rtol=1e-4, atol=1e-7)
+
+
+# ------------------------------------------------------------------------------------------------
+# qr_backward
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,kw,K", [("cfg2", dict(N=20000, W=128, H=96), 40),
+                                       ("cfg1", dict(W=70, H=50, D=3, backward=True), 40),
+                                       ("cfg3", dict(N=60000, W=112, H=80, D=512), 40),
+                                       ("cfg3", dict(N=40000, W=96, H=64, D=132), 8),
+                                       ("cfg2", dict(N=20000, W=64, H=64, D=64), 100)])     # K > 64: pixel kernel
+def test_backward_stage_isolated(qr, orc, name, kw, K):
+    sc = make_scene(name, seed=9, **kw)
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    lists = orc.pixel_lists(sc.cam, proj)
+    q = orc.qrender(lists, K, None)
+    H, W = sc.cam.height, sc.cam.width
+    ref = orc.backward(q.sel_idx, q.sel_w, q.n_sel, sc.dL_dmap, sc.N)
+    got = qr.qr_backward(sc.cam, sc.N, P.to_dev(q.sel_idx.reshape(H, W, K)),
+                         P.to_dev(q.sel_w.reshape(H, W, K).astype(np.float32)),
+                         P.to_dev(q.n_sel.reshape(H, W)), P.to_dev(sc.dL_dmap)).cpu().numpy().astype(np.float64)
+    tol = P.ATOL + P.RTOL * np.abs(ref)
+    err = np.abs(got - ref)
+    assert (err <= tol).all(), float((err / tol).max())
+    touched = np.zeros(sc.N, bool); touched[q.sel_idx[q.sel_idx >= 0]] = True
+    assert (got[~touched] == 0).all()                       # rows never selected are untouched
+    assert touched.sum() > 10
+
+
+def test_backward_accumulates_and_adjoint(qr, orc):
+    """qr_backward adds into dL_dfeat; <render(F), G> == <F, backward(G)> (render is linear in F)."""
+    sc = make_scene("cfg3", seed=10, N=60000, W=128, H=96, D=64)
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    out = qr.pipeline.forward(sc.cam, fe, g.features, 40)
+    G = P.to_dev(sc.dL_dmap)
+    dF = qr.pipeline.backward(sc.cam, sc.N, out, G)
+    lhs = float((out.out_map.double() * G.double()).sum())
+    rhs = float((g.features.double() * dF.double()).sum())
+    assert abs(lhs - rhs) <= 1e-5 * max(abs(lhs), 1.0), (lhs, rhs)
+    dF2 = qr.pipeline.backward(sc.cam, sc.N, out, G, dF.clone())
+    torch.testing.assert_close(dF2, 2.0 * dF, rtol=1e-5, atol=1e-6)
+
+
+# ------------------------------------------------------------------------------------------------
+# full-size sampled check in the configuration bench.py times (config 3)
+# ------------------------------------------------------------------------------------------------
+def test_config3_full_size_sampled(qr, orc):
+    sc = make_scene("cfg3", seed=0)
+    g = P.upload(sc)
+    K = sc.K
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    out = qr.pipeline.forward(sc.cam, fe, g.features, K)
+    G = P.to_dev(sc.dL_dmap)
+    dF = qr.pipeline.backward(sc.cam, sc.N, out, G)
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    rect, touched = orc.tile_rects(sc.cam, proj)
+    assert fe.M == int(touched.sum())
+    lists = orc.pixel_lists(sc.cam, proj)
+    rng = np.random.default_rng(0)
+    pix = np.sort(rng.choice(sc.cam.width * sc.cam.height, size=4000, replace=False))
+    q = orc.qrender(lists, K, sc.features, pixels=pix)
+    stats = P.compare_forward(out, q, lists, K, sc.D, pixels=pix)
+    print("cfg3 sampled:", stats)
+    # selection parity on every pixel (no features needed)
+    qa = orc.qrender(lists, K, None)
+    ex = P.exempt_mask(qa, lists)
+    same = (out.sel_idx.cpu().numpy().reshape(-1, K) == qa.sel_idx).all(1)
+    assert ((~same) & (~ex)).sum() == 0
+    print("cfg3 all pixels: exempt", int(ex.sum()), "mismatching exempt", int(((~same) & ex).sum()))
+    # gradient rows of sampled Gaussians from the oracle's records
+    sel = qa.sel_idx[qa.sel_idx >= 0]
+    rows = np.unique(sel)[::97][:200].astype(np.int64)
+    ref = orc.backward(qa.sel_idx, qa.sel_w, qa.n_sel, sc.dL_dmap, sc.N, rows=rows)
+    got = dF[torch.from_numpy(rows).cuda()].cpu().numpy().astype(np.float64)
+    if same.all():
+        tol = P.ATOL + P.RTOL * np.abs(ref)
+        assert (np.abs(got - ref) <= tol).all(), float((np.abs(got - ref) / tol).max())
+
+
+# ------------------------------------------------------------------------------------------------
+# argument errors are status codes, not crashes
+# ------------------------------------------------------------------------------------------------
+def test_error_codes(qr):
+    sc = make_scene("cfg1", seed=0, N=100)
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    with pytest.raises(qr.QRError) as e:
+        qr.pipeline.forward(sc.cam, fe, g.features, 0)
+    assert e.value.code == -1
+    with pytest.raises(qr.QRError) as e:
+        qr.pipeline.forward(sc.cam, fe, g.features, 1000)
+    assert e.value.code == -3
+    with pytest.raises(qr.QRError):
+        qr.qr_preprocess(sc.cam, g.means.cpu(), g.scales, g.quats, g.opac)   # no CPU path
+    bad = make_camera(0, 10)
+    with pytest.raises(qr.QRError) as e:
+        qr.qr_preprocess(bad, g.means, g.scales, g.quats, g.opac)
+    assert e.value.code == -1
