@@ -211,13 +211,28 @@ def qr_forward_workspace_bytes(cam, K: int, D: int) -> int:
     return int(load().qr_forward_workspace_bytes(C.byref(c), int(K), int(D)))
 
 
+_ws_cache = {}
+
+
+def _workspace(nbytes: int, dev) -> torch.Tensor:
+    """One cached scratch tensor per device, grown on demand (device memory only; contents are scratch)."""
+    key = str(dev)
+    t = _ws_cache.get(key)
+    if t is None or t.numel() < nbytes:
+        t = torch.empty((max(int(nbytes), 256),), dtype=torch.uint8, device=dev)
+        _ws_cache[key] = t
+    return t
+
+
 def qr_forward(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, features,
-               out: Optional[ForwardOut] = None) -> ForwardOut:
+               out: Optional[ForwardOut] = None, ws: Optional[torch.Tensor] = None) -> ForwardOut:
     c = make_camera(cam)
     H, W = c.height, c.width
     D = int(features.shape[1])
     dev = features.device
     dt = _feat_dtype(features)
+    if ws is None:
+        ws = _workspace(qr_forward_workspace_bytes(c, K, D), dev)
     if out is None:
         kk = max(int(K), 1)
         out = ForwardOut(torch.empty((H, W, D), dtype=torch.float32, device=dev),
@@ -229,7 +244,8 @@ def qr_forward(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, feature
                              _dev(conic_opac, torch.float32, "conic_opac"),
                              _dev(isect_gauss, torch.int32, "isect_gauss"), _dev(tile_range, torch.int32, "tile_range"),
                              _dev(features, features.dtype, "features"), out.out_map.data_ptr(), out.sel_idx.data_ptr(),
-                             out.sel_w.data_ptr(), out.n_sel.data_ptr(), out.resid_TQ.data_ptr(), None, 0, _stream()))
+                             out.sel_w.data_ptr(), out.n_sel.data_ptr(), out.resid_TQ.data_ptr(),
+                             ws.data_ptr(), ws.numel(), _stream()))
     return out
 
 

@@ -30,6 +30,17 @@ int check_cam(const qr_camera* cam)
     return QR_OK;
 }
 
+int check_feat(int32_t D, qr_dtype dt, const char* who)
+{
+    if (D < 1) return fail(QR_ERR_INVALID_ARG, "%s: D = %d < 1", who, D);
+    if (D > QR_MAX_D) return fail(QR_ERR_UNSUPPORTED, "%s: D = %d > QR_MAX_D", who, D);
+    if (dt != QR_F32 && dt != QR_F16) return fail(QR_ERR_INVALID_ARG, "%s: unknown feature dtype %d", who, (int)dt);
+    if (dt == QR_F16 && D % 8 != 0) return fail(QR_ERR_UNSUPPORTED, "%s: fp16 features need D %% 8 == 0", who);
+    if (dt == QR_F32 && D % 4 != 0 && D > 128)
+        return fail(QR_ERR_UNSUPPORTED, "%s: D %% 4 != 0 is only supported for D <= 128", who);
+    return QR_OK;
+}
+
 }  // namespace qr
 
 extern "C" int qr_version(void) { return QR_VERSION; }

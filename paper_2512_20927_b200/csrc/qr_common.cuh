@@ -41,6 +41,7 @@ inline Cam make_cam(const qr_camera* c)
 char* err_buf();
 int fail(int code, const char* fmt, ...);
 int check_cam(const qr_camera* cam);
+int check_feat(int32_t D, qr_dtype dt, const char* who);
 
 #define QR_CUDA_OK(expr)                                                                       \
     do {                                                                                       \

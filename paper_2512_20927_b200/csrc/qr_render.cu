@@ -1,4 +1,6 @@
-// qr_render.cu -- qr_forward (Algorithm 1) and qr_dense_forward (Eq. 1).
+// qr_render.cu -- qr_dense_forward (Eq. 1), the in-run dense comparator, as a fused band kernel.
+// (MODE 0 of the template is the first fused Q-Render kernel of this build; qr_forward now lives in qr_forward.cu
+// and MODE 0 is no longer instantiated.)
 //
 // One kernel template serves both: the only difference is the rule that turns an included Gaussian into a blending
 // weight (Q-Render: only at a quantile crossing, weight T^Q alpha'; V-Render: always, weight T alpha').
@@ -404,48 +406,7 @@ static int launch_render(const RenderParams& p, qr_dtype dt, cudaStream_t st)
     }
 }
 
-static int check_feat(int32_t D, qr_dtype dt, const char* who)
-{
-    if (D < 1) return fail(QR_ERR_INVALID_ARG, "%s: D = %d < 1", who, D);
-    if (D > QR_MAX_D) return fail(QR_ERR_UNSUPPORTED, "%s: D = %d > QR_MAX_D", who, D);
-    if (dt != QR_F32 && dt != QR_F16) return fail(QR_ERR_INVALID_ARG, "%s: unknown feature dtype %d", who, (int)dt);
-    if (dt == QR_F16 && D % 8 != 0) return fail(QR_ERR_UNSUPPORTED, "%s: fp16 features need D %% 8 == 0", who);
-    if (dt == QR_F32 && D % 4 != 0 && D > 128)
-        return fail(QR_ERR_UNSUPPORTED, "%s: D %% 4 != 0 is only supported for D <= 128", who);
-    return QR_OK;
-}
-
 }  // namespace qr
-
-extern "C" size_t qr_forward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D)
-{
-    (void)cam; (void)K; (void)D;
-    return 0;   // the fused kernel keeps its intermediates in shared memory
-}
-
-extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype, const float* mean2d,
-                          const float* conic_opac, const uint32_t* isect_gauss, const int32_t* tile_range,
-                          const void* features, float* out_map, int32_t* sel_idx, float* sel_w, int32_t* n_sel,
-                          float* resid_TQ, void* ws, size_t ws_bytes, void* stream)
-{
-    using namespace qr;
-    (void)ws; (void)ws_bytes;
-    if (int rc = check_cam(cam)) return rc;
-    if (K < 1) return fail(QR_ERR_INVALID_ARG, "qr_forward: K = %d < 1 (SPEC.md:215)", K);
-    if (K > QR_MAX_K) return fail(QR_ERR_UNSUPPORTED, "qr_forward: K = %d > QR_MAX_K", K);
-    if (int rc = check_feat(D, feat_dtype, "qr_forward")) return rc;
-    if (!tile_range || !out_map || !sel_idx || !sel_w || !n_sel || !resid_TQ)
-        return fail(QR_ERR_NULL_POINTER, "qr_forward: NULL output or tile_range");
-    if (!aligned16(out_map) || !aligned16(features) || !aligned16(conic_opac) || !aligned16(mean2d))
-        return fail(QR_ERR_MISALIGNED, "qr_forward: out_map / features / conic_opac / mean2d must be 16-byte aligned");
-    RenderParams p;
-    p.cam = make_cam(cam); p.K = K; p.D = D; p.t_min = 0.0f;
-    p.mean2d = reinterpret_cast<const float2*>(mean2d);
-    p.conic_opac = reinterpret_cast<const float4*>(conic_opac);
-    p.isect = isect_gauss; p.tile_range = reinterpret_cast<const int2*>(tile_range); p.features = features;
-    p.out_map = out_map; p.sel_idx = sel_idx; p.sel_w = sel_w; p.n_sel = n_sel; p.resid = resid_TQ;
-    return launch_render<0>(p, feat_dtype, (cudaStream_t)stream);
-}
 
 extern "C" int qr_dense_forward(const qr_camera* cam, int32_t D, qr_dtype feat_dtype, float t_min, const float* mean2d,
                                 const float* conic_opac, const uint32_t* isect_gauss, const int32_t* tile_range,
