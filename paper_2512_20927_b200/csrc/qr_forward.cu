@@ -26,9 +26,9 @@ constexpr int kWalkBatch = 256;
 constexpr int kGroupPx = 8;                  // 4x2 pixels
 constexpr int kGroupsPerTile = 32;
 
-// workspace layout: gcount[G], gid[G][cap], gw[G][cap][8]   (G = tiles * 32 groups, cap = 8 K)
+// workspace layout: tile ticket, gcount[G], gid[G][cap], gw[G][cap][8]   (G = tiles * 32 groups, cap = 8 K)
 struct FwdLayout {
-    size_t gcount, gid, gw, total;
+    size_t ticket, gcount, gid, gw, total;
     int64_t G;
     int cap;
 };
@@ -39,6 +39,7 @@ static FwdLayout fwd_layout(const Cam& cam, int K)
     L.G = (int64_t)cam.tiles_x * cam.tiles_y * kGroupsPerTile;
     L.cap = kGroupPx * K;
     size_t o = 0;
+    L.ticket = o; o = align_up(o + 4, 256);
     L.gcount = o; o = align_up(o + (size_t)L.G * 4, 256);
     L.gid = o;    o = align_up(o + (size_t)L.G * L.cap * 4, 256);
     L.gw = o;     o = align_up(o + (size_t)L.G * L.cap * 32, 256);
@@ -55,9 +56,12 @@ struct WalkParams {
     const int2* tile_range;
     int32_t* n_sel;
     float* resid;
+    int32_t* sel_idx;     // only the padding (slots >= n_sel) is written here
+    float* sel_w;
     int32_t* gcount;
     int32_t* gid;
     float* gw;
+    int32_t* tile_ticket; // blend_kernel's tile queue, reset here
 };
 
 __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
@@ -68,9 +72,11 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
     float2* ent_xy = reinterpret_cast<float2*>(ent_box + kWalkBatch);     // [256]
     int32_t* ent_id = reinterpret_cast<int32_t*>(ent_xy + kWalkBatch);    // [256]
     float* thr = reinterpret_cast<float*>(ent_id + kWalkBatch);           // [K+1]
+    __shared__ int32_t nsel_s[kTile * kTile];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x;
+    if (tile == 0 && tid == 0) *p.tile_ticket = 0;
     const int tile_x = tile % p.cam.tiles_x, tile_y = tile / p.cam.tiles_x;
     const int K = p.K;
     // warp = pixel rows 2*warp, 2*warp+1 of the tile; lane -> (x = lane & 15, y = lane >> 4)
@@ -174,22 +180,32 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
         p.n_sel[pix] = ns;
         p.resid[pix] = ns > 0 ? TQ : 1.0f;              // R8
     }
+    // ---- padding of the selection records (-1 / 0 for slots >= n_sel), coalesced: a tile row is 16*K contiguous
+    // words of sel_idx / sel_w.  The used slots are written by blend_kernel (it knows 1/(1 - T^Q) by then). ----
+    nsel_s[warp * 32 + lane] = ns;                      // index = (2*warp + (lane>>4))*16 + (lane&15) = y_local*16 + x_local
+    __syncthreads();
+    {
+        const int npx = min(kTile, p.cam.width - tile_x * kTile);
+        const int row_words = npx * K;
+        const int dq = kWalkThreads / K, dr = kWalkThreads % K;      // advancing i by 256 = dq pixels and dr slots
+        for (int r = 0; r < kTile; ++r) {
+            const int y = tile_y * kTile + r;
+            if (y >= p.cam.height) break;
+            const int64_t gbase = ((int64_t)y * p.cam.width + tile_x * kTile) * K;
+            int pxl = tid / K, sl = tid - pxl * K;
+            for (int i = tid; i < row_words; i += kWalkThreads) {
+                if (sl >= nsel_s[r * kTile + pxl]) {
+                    p.sel_idx[gbase + i] = -1;
+                    p.sel_w[gbase + i] = 0.0f;
+                }
+                pxl += dq; sl += dr;
+                if (sl >= K) { sl -= K; ++pxl; }
+            }
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-struct BlendParams {
-    Cam cam;
-    int32_t K, D, cap;
-    const void* features;
-    const int32_t* gcount;
-    const int32_t* gid;
-    const float* gw;
-    const int32_t* n_sel;
-    const float* resid;
-    float* out_map;
-    int32_t* sel_idx;
-    float* sel_w;
-};
 
 template <typename FeatT, int VW> struct Row;
 template <> struct Row<float, 4> {
@@ -228,31 +244,84 @@ template <> __device__ __forceinline__ void store_map<8>(float* dst, const float
 }
 
 constexpr int kBlendWarps = 8;
+constexpr int kBlendSlots = 64;              // ring of tiles a CTA has claimed (only ~2 are live at any time)
 
-template <typename FeatT, int NV, int VW>
+struct BlendParams {
+    Cam cam;
+    int32_t K, D, cap, num_tiles;
+    const void* features;
+    const int32_t* gcount;
+    const int32_t* gid;
+    const float* gw;
+    const int32_t* n_sel;
+    const float* resid;
+    float* out_map;
+    int32_t* sel_idx;
+    float* sel_w;
+    int32_t* tile_ticket;
+};
+
+// Persistent CTAs (one per SM).  Work is handed out without block barriers: a warp takes a ticket from the CTA's
+// shared counter; ticket / 32 is a slot of the CTA's tile ring, ticket % 32 the pixel group inside that tile.  The
+// warp that draws group 0 of a slot claims the next tile from the global queue and publishes it; the others wait
+// for that word only.  All warps of a CTA therefore work on the same one or two tiles (feature rows shared by the
+// tile's groups stay in L1) and nobody idles at a barrier when group list lengths differ.
+template <typename FeatT, int NV, int VW, bool FULL>
 __global__ void __launch_bounds__(kBlendWarps * 32, 1) blend_kernel(const BlendParams p)
 {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int tile = blockIdx.x;
-    const int tile_x = tile % p.cam.tiles_x, tile_y = tile / p.cam.tiles_x;
+    __shared__ int32_t s_ticket;
+    __shared__ unsigned long long s_slot[kBlendSlots];   // ((slot + 1) << 32) | tile, 0 = never written
+    __shared__ int32_t s_reads[kBlendSlots];             // how many of the slot's 31 other groups have read it
+    const int lane = threadIdx.x & 31;
     const int D = p.D, K = p.K;
+    if (threadIdx.x == 0) s_ticket = 0;
+    if (threadIdx.x < kBlendSlots) { s_slot[threadIdx.x] = 0ull; s_reads[threadIdx.x] = 0; }
+    __syncthreads();
 
-    for (int g = warp; g < kGroupsPerTile; g += kBlendWarps) {
+    while (true) {
+        int tile = 0, g = 0;
+        if (lane == 0) {
+            const int ticket = atomicAdd(&s_ticket, 1);
+            const int slot = ticket >> 5, idx = slot % kBlendSlots;
+            g = ticket & 31;
+            volatile unsigned long long* word = &s_slot[idx];
+            volatile int32_t* reads = &s_reads[idx];
+            if (g == 0) {
+                // claim the next tile for this slot.  The ring entry is reused every kBlendSlots tiles: wait until the
+                // 31 readers of its previous generation are through (they never wait on this warp, so this ends)
+                if (slot >= kBlendSlots) { while (*reads != 31) { } }
+                *reads = 0;
+                tile = atomicAdd(p.tile_ticket, 1);
+                __threadfence_block();
+                *word = ((unsigned long long)(slot + 1) << 32) | (unsigned int)tile;
+            } else {
+                unsigned long long v;
+                while (((v = *word) >> 32) != (unsigned long long)(slot + 1)) { }
+                tile = (int)(v & 0xffffffffull);
+                atomicAdd(&s_reads[idx], 1);
+            }
+        }
+        tile = __shfl_sync(0xffffffffu, tile, 0);
+        g = __shfl_sync(0xffffffffu, g, 0);
+        if (tile >= p.num_tiles) break;
+        const int tile_x = tile % p.cam.tiles_x, tile_y = tile / p.cam.tiles_x;
+
         // group g = (row pair g >> 2, x block g & 3); pixel q of the group: x = 4*(g&3) + (q&3), y = 2*(g>>2) + (q>>2)
         const int gx0 = tile_x * kTile + (g & 3) * 4, gy0 = tile_y * kTile + (g >> 2) * 2;
         if (gx0 >= p.cam.width || gy0 >= p.cam.height) continue;
         const int64_t group = (int64_t)tile * kGroupsPerTile + g;
         const int n = p.gcount[group];
         const int32_t* gid = p.gid + group * p.cap;
-        const float* gw = p.gw + group * p.cap * kGroupPx;
+        const float4* gw4 = reinterpret_cast<const float4*>(p.gw + group * p.cap * kGroupPx);
 
-        // lanes 0..7 own the bookkeeping of pixel q = lane: 1/(1 - T^Q), record cursor
+        // lanes 0..7 own the bookkeeping of pixel q = lane: 1/(1 - T^Q) and the record cursor
         const int mx = gx0 + (lane & 3), my = gy0 + ((lane >> 2) & 1);
         const bool mine = lane < kGroupPx && mx < p.cam.width && my < p.cam.height;
         const int64_t mpix = (int64_t)my * p.cam.width + mx;
         float minv = 0.0f;
         if (mine && p.n_sel[mpix] > 0) minv = __fdiv_rn(1.0f, __fsub_rn(1.0f, p.resid[mpix]));   // line 20; R8
-        int mcur = 0;
+        int32_t* my_idx = p.sel_idx + mpix * K;
+        float* my_w = p.sel_w + mpix * K;
 
         float acc[kGroupPx][NV][VW];
 #pragma unroll
@@ -262,29 +331,37 @@ __global__ void __launch_bounds__(kBlendWarps * 32, 1) blend_kernel(const BlendP
 #pragma unroll
                 for (int v = 0; v < VW; ++v) acc[q][j][v] = 0.0f;
 
-        for (int i = 0; i < n; ++i) {
-            const int32_t id = __ldg(gid + i);
-            const float4 w0 = __ldg(reinterpret_cast<const float4*>(gw + (size_t)i * kGroupPx));
-            const float4 w1 = __ldg(reinterpret_cast<const float4*>(gw + (size_t)i * kGroupPx) + 1);
-            float f[NV][VW];
+        // software pipeline, two register sets A / B: while record i is applied, the feature row of record i+1 and
+        // the (id, weights) of record i+2 are in flight
+        int32_t idA = 0, idB = 0;
+        float4 wA0, wA1, wB0, wB1;
+        wA0 = wA1 = wB0 = wB1 = make_float4(0.f, 0.f, 0.f, 0.f);
+        float fA[NV][VW], fB[NV][VW];
+        auto load_meta = [&](int i, int32_t& id, float4& w0, float4& w1) {
+            if (i < n) { id = __ldg(gid + i); w0 = __ldg(gw4 + 2 * i); w1 = __ldg(gw4 + 2 * i + 1); }
+        };
+        auto load_row = [&](int i, int32_t id, float (&f)[NV][VW]) {
+            if (i < n) {
 #pragma unroll
-            for (int j = 0; j < NV; ++j) {
-                const int ch = (j * 32 + lane) * VW;
-                if (ch < D) Row<FeatT, VW>::load(p.features, id, D, ch, f[j]);
-                else {
+                for (int j = 0; j < NV; ++j) {
+                    const int ch = (j * 32 + lane) * VW;
+                    if (FULL || ch < D) Row<FeatT, VW>::load(p.features, id, D, ch, f[j]);
+                    else {
 #pragma unroll
-                    for (int v = 0; v < VW; ++v) f[j][v] = 0.0f;
+                        for (int v = 0; v < VW; ++v) f[j][v] = 0.0f;
+                    }
                 }
             }
+        };
+        auto apply = [&](int32_t id, const float4& w0, const float4& w1, const float (&f)[NV][VW]) {
             const float w[kGroupPx] = { w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w };
-            // selection record of pixel q = lane (depth order = list order)
-            if (mine) {
-                const float wm = __ldg(gw + (size_t)i * kGroupPx + lane);
-                if (wm != 0.0f) {
-                    p.sel_idx[mpix * K + mcur] = id;
-                    p.sel_w[mpix * K + mcur] = __fmul_rn(wm, minv);
-                    ++mcur;
-                }
+            // selection record of pixel q = lane, in list (= depth) order
+            float wm = w[0];
+#pragma unroll
+            for (int q = 1; q < kGroupPx; ++q) wm = (lane == q) ? w[q] : wm;
+            if (mine && wm != 0.0f) {
+                *my_idx++ = id;
+                *my_w++ = __fmul_rn(wm, minv);
             }
 #pragma unroll
             for (int q = 0; q < kGroupPx; ++q) {
@@ -295,40 +372,62 @@ __global__ void __launch_bounds__(kBlendWarps * 32, 1) blend_kernel(const BlendP
                         for (int v = 0; v < VW; ++v) acc[q][j][v] = __fmaf_rn(w[q], f[j][v], acc[q][j][v]);   // line 9
                 }
             }
+        };
+        load_meta(0, idA, wA0, wA1);
+        load_meta(1, idB, wB0, wB1);
+        load_row(0, idA, fA);
+        for (int i = 0; i < n; i += 2) {
+            load_row(i + 1, idB, fB);
+            const int32_t idA_cur = idA; const float4 a0 = wA0, a1 = wA1;
+            load_meta(i + 2, idA, wA0, wA1);
+            apply(idA_cur, a0, a1, fA);
+            if (i + 1 < n) {
+                load_row(i + 2, idA, fA);
+                const int32_t idB_cur = idB; const float4 b0 = wB0, b1 = wB1;
+                load_meta(i + 3, idB, wB0, wB1);
+                apply(idB_cur, b0, b1, fB);
+            }
         }
 
-        // ---- epilogue: normalise and store ----
+        // ---- epilogue: normalise and store (512 contiguous bytes per store instruction) ----
 #pragma unroll
         for (int q = 0; q < kGroupPx; ++q) {
             const int x = gx0 + (q & 3), y = gy0 + (q >> 2);
             const float inv = __shfl_sync(0xffffffffu, minv, q);
-            const int cur = __shfl_sync(0xffffffffu, mcur, q);
             if (x < p.cam.width && y < p.cam.height) {
-                const int64_t pix = (int64_t)y * p.cam.width + x;
-                float* dst = p.out_map + pix * D;
+                float* dst = p.out_map + ((int64_t)y * p.cam.width + x) * D;
 #pragma unroll
                 for (int j = 0; j < NV; ++j) {
                     const int ch = (j * 32 + lane) * VW;
-                    if (ch < D) {
+                    if (FULL || ch < D) {
                         float o[VW];
 #pragma unroll
                         for (int v = 0; v < VW; ++v) o[v] = __fmul_rn(acc[q][j][v], inv);
                         store_map<VW>(dst + ch, o);
                     }
                 }
-                for (int s = cur + lane; s < K; s += 32) {          // pad the records
-                    p.sel_idx[pix * K + s] = -1;
-                    p.sel_w[pix * K + s] = 0.0f;
-                }
             }
         }
     }
 }
 
-template <typename FeatT, int NV, int VW>
-static int launch_blend(const BlendParams& p, int T, cudaStream_t st)
+static int sm_count()
 {
-    blend_kernel<FeatT, NV, VW><<<(unsigned)T, kBlendWarps * 32, 0, st>>>(p);
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
+            n = 148;
+    }
+    return n;
+}
+
+template <typename FeatT, int NV, int VW>
+static int launch_blend(const BlendParams& p, cudaStream_t st)
+{
+    const unsigned grid = (unsigned)min(sm_count(), p.num_tiles);
+    if (p.D == NV * 32 * VW) blend_kernel<FeatT, NV, VW, true><<<grid, kBlendWarps * 32, 0, st>>>(p);
+    else blend_kernel<FeatT, NV, VW, false><<<grid, kBlendWarps * 32, 0, st>>>(p);
     QR_LAUNCH_OK("blend_kernel");
     return QR_OK;
 }
@@ -369,7 +468,8 @@ extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype f
     wp.mean2d = reinterpret_cast<const float2*>(mean2d);
     wp.conic_opac = reinterpret_cast<const float4*>(conic_opac);
     wp.isect = isect_gauss; wp.tile_range = reinterpret_cast<const int2*>(tile_range);
-    wp.n_sel = n_sel; wp.resid = resid_TQ;
+    wp.n_sel = n_sel; wp.resid = resid_TQ; wp.sel_idx = sel_idx; wp.sel_w = sel_w;
+    wp.tile_ticket = reinterpret_cast<int32_t*>(w + L.ticket);
     wp.gcount = reinterpret_cast<int32_t*>(w + L.gcount);
     wp.gid = reinterpret_cast<int32_t*>(w + L.gid);
     wp.gw = reinterpret_cast<float*>(w + L.gw);
@@ -378,25 +478,25 @@ extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype f
     QR_LAUNCH_OK("walk_kernel");
 
     BlendParams bp;
-    bp.cam = c; bp.K = K; bp.D = D; bp.cap = L.cap;
+    bp.cam = c; bp.K = K; bp.D = D; bp.cap = L.cap; bp.num_tiles = T; bp.tile_ticket = wp.tile_ticket;
     bp.features = features; bp.gcount = wp.gcount; bp.gid = wp.gid; bp.gw = wp.gw;
     bp.n_sel = n_sel; bp.resid = resid_TQ; bp.out_map = out_map; bp.sel_idx = sel_idx; bp.sel_w = sel_w;
     if (feat_dtype == QR_F16) {
-        if ((D + 255) / 256 == 1) return launch_blend<__half, 1, 8>(bp, T, st);
-        return launch_blend<__half, 2, 8>(bp, T, st);
+        if ((D + 255) / 256 == 1) return launch_blend<__half, 1, 8>(bp, st);
+        return launch_blend<__half, 2, 8>(bp, st);
     }
     if (D % 4 == 0) {
         switch ((D + 127) / 128) {
-            case 1: return launch_blend<float, 1, 4>(bp, T, st);
-            case 2: return launch_blend<float, 2, 4>(bp, T, st);
-            case 3: return launch_blend<float, 3, 4>(bp, T, st);
-            default: return launch_blend<float, 4, 4>(bp, T, st);
+            case 1: return launch_blend<float, 1, 4>(bp, st);
+            case 2: return launch_blend<float, 2, 4>(bp, st);
+            case 3: return launch_blend<float, 3, 4>(bp, st);
+            default: return launch_blend<float, 4, 4>(bp, st);
         }
     }
     switch ((D + 31) / 32) {
-        case 1: return launch_blend<float, 1, 1>(bp, T, st);
-        case 2: return launch_blend<float, 2, 1>(bp, T, st);
-        case 3: return launch_blend<float, 3, 1>(bp, T, st);
-        default: return launch_blend<float, 4, 1>(bp, T, st);
+        case 1: return launch_blend<float, 1, 1>(bp, st);
+        case 2: return launch_blend<float, 2, 1>(bp, st);
+        case 3: return launch_blend<float, 3, 1>(bp, st);
+        default: return launch_blend<float, 4, 1>(bp, st);
     }
 }
