@@ -26,9 +26,13 @@ constexpr int kWalkBatch = 256;
 constexpr int kGroupPx = 8;                  // 4x2 pixels
 constexpr int kGroupsPerTile = 32;
 
-// workspace layout: tile ticket, gcount[G], gid[G][cap], gw[G][cap][8]   (G = tiles * 32 groups, cap = 8 K)
+// workspace layout: tile ticket, gcount[G], rec[G][cap] (G = tiles * 32 groups, cap = 8 K + kSentinels).
+// A record is 12 words (48 B, 16-byte aligned): the 8 pixels' weights w^Q, the Gaussian id, 3 words of padding.
+// Each list ends with kSentinels records of id -1 / weight 0 so that the blend pipeline can prefetch past the end.
+constexpr int kRecWords = 12;
+constexpr int kSentinels = 3;
 struct FwdLayout {
-    size_t ticket, gcount, gid, gw, total;
+    size_t ticket, gcount, rec, total;
     int64_t G;
     int cap;
 };
@@ -37,12 +41,11 @@ static FwdLayout fwd_layout(const Cam& cam, int K)
 {
     FwdLayout L;
     L.G = (int64_t)cam.tiles_x * cam.tiles_y * kGroupsPerTile;
-    L.cap = kGroupPx * K;
+    L.cap = kGroupPx * K + kSentinels;
     size_t o = 0;
     L.ticket = o; o = align_up(o + 4, 256);
     L.gcount = o; o = align_up(o + (size_t)L.G * 4, 256);
-    L.gid = o;    o = align_up(o + (size_t)L.G * L.cap * 4, 256);
-    L.gw = o;     o = align_up(o + (size_t)L.G * L.cap * 32, 256);
+    L.rec = o;    o = align_up(o + (size_t)L.G * L.cap * kRecWords * 4, 256);
     L.total = o;
     return L;
 }
@@ -59,8 +62,7 @@ struct WalkParams {
     int32_t* sel_idx;     // only the padding (slots >= n_sel) is written here
     float* sel_w;
     int32_t* gcount;
-    int32_t* gid;
-    float* gw;
+    float* rec;
     int32_t* tile_ticket; // blend_kernel's tile queue, reset here
 };
 
@@ -89,8 +91,7 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
     const int gx = (lane & 15) >> 2, q = (lane >> 4) * 4 + (lane & 3);
     const uint32_t gbits = (0xFu << (4 * gx)) | (0xFu << (16 + 4 * gx));  // lanes of my group
     const int64_t group = (int64_t)tile * kGroupsPerTile + warp * 4 + gx;
-    int32_t* my_gid = p.gid + group * p.cap;
-    float* my_gw = p.gw + group * p.cap * kGroupPx;
+    float* my_rec = p.rec + group * p.cap * kRecWords;
 
     for (int k = tid; k <= K; k += kWalkThreads)                          // thresholds as printed (R3)
         thr[k] = __fsub_rn(1.0f, __fdiv_rn((float)(k + 1), (float)(K + 1)));
@@ -165,8 +166,8 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
                 }
                 const uint32_t sm = __ballot_sync(0xffffffffu, sel);
                 if (sm & gbits) {                       // some pixel of my group selected this Gaussian
-                    my_gw[gcnt * kGroupPx + q] = wQ;    // 8 lanes write the record's 8 weights (32 contiguous bytes)
-                    if (q == 0) my_gid[gcnt] = ent_id[e];
+                    my_rec[gcnt * kRecWords + q] = wQ;  // 8 lanes write the record's 8 weights (32 contiguous bytes)
+                    if (q == 0) my_rec[gcnt * kRecWords + 8] = __int_as_float(ent_id[e]);
                     ++gcnt;
                 }
             }
@@ -175,6 +176,11 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
     }
 
     if (q == 0) p.gcount[group] = gcnt;
+#pragma unroll
+    for (int t = 0; t < kSentinels; ++t) {              // list terminators: weight 0, id -1
+        my_rec[(gcnt + t) * kRecWords + q] = 0.0f;
+        if (q == 0) my_rec[(gcnt + t) * kRecWords + 8] = __int_as_float(-1);
+    }
     if (inside) {
         const int64_t pix = (int64_t)py * p.cam.width + px;
         p.n_sel[pix] = ns;
@@ -209,22 +215,19 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
 
 template <typename FeatT, int VW> struct Row;
 template <> struct Row<float, 4> {
-    static __device__ __forceinline__ void load(const void* base, int64_t row, int D, int ch, float (&f)[4])
+    static __device__ __forceinline__ void load(const float* src, float (&f)[4])
     {
-        const float4 v = __ldg(reinterpret_cast<const float4*>(static_cast<const float*>(base) + row * D + ch));
+        const float4 v = __ldg(reinterpret_cast<const float4*>(src));
         f[0] = v.x; f[1] = v.y; f[2] = v.z; f[3] = v.w;
     }
 };
 template <> struct Row<float, 1> {
-    static __device__ __forceinline__ void load(const void* base, int64_t row, int D, int ch, float (&f)[1])
-    {
-        f[0] = __ldg(static_cast<const float*>(base) + row * D + ch);
-    }
+    static __device__ __forceinline__ void load(const float* src, float (&f)[1]) { f[0] = __ldg(src); }
 };
 template <> struct Row<__half, 8> {
-    static __device__ __forceinline__ void load(const void* base, int64_t row, int D, int ch, float (&f)[8])
+    static __device__ __forceinline__ void load(const __half* src, float (&f)[8])
     {
-        const uint4 v = __ldg(reinterpret_cast<const uint4*>(static_cast<const __half*>(base) + row * D + ch));
+        const uint4 v = __ldg(reinterpret_cast<const uint4*>(src));
         const __half2* h = reinterpret_cast<const __half2*>(&v);
 #pragma unroll
         for (int i = 0; i < 4; ++i) { const float2 t = __half22float2(h[i]); f[2 * i] = t.x; f[2 * i + 1] = t.y; }
@@ -251,8 +254,7 @@ struct BlendParams {
     int32_t K, D, cap, num_tiles;
     const void* features;
     const int32_t* gcount;
-    const int32_t* gid;
-    const float* gw;
+    const float* rec;
     const int32_t* n_sel;
     const float* resid;
     float* out_map;
@@ -278,48 +280,75 @@ __global__ void __launch_bounds__(kBlendWarps * 32, 1) blend_kernel(const BlendP
     if (threadIdx.x < kBlendSlots) { s_slot[threadIdx.x] = 0ull; s_reads[threadIdx.x] = 0; }
     __syncthreads();
 
-    while (true) {
-        int tile = 0, g = 0;
-        if (lane == 0) {
-            const int ticket = atomicAdd(&s_ticket, 1);
-            const int slot = ticket >> 5, idx = slot % kBlendSlots;
-            g = ticket & 31;
-            volatile unsigned long long* word = &s_slot[idx];
-            volatile int32_t* reads = &s_reads[idx];
-            if (g == 0) {
-                // claim the next tile for this slot.  The ring entry is reused every kBlendSlots tiles: wait until the
-                // 31 readers of its previous generation are through (they never wait on this warp, so this ends)
-                if (slot >= kBlendSlots) { while (*reads != 31) { } }
-                *reads = 0;
-                tile = atomicAdd(p.tile_ticket, 1);
-                __threadfence_block();
-                *word = ((unsigned long long)(slot + 1) << 32) | (unsigned int)tile;
-            } else {
-                unsigned long long v;
-                while (((v = *word) >> 32) != (unsigned long long)(slot + 1)) { }
-                tile = (int)(v & 0xffffffffull);
-                atomicAdd(&s_reads[idx], 1);
+    // ---- work hand-out ----
+    struct Job { int tile, g, n; int32_t ids0, ids1; float inv; };   // inv: lanes 0..7 = 1/(1 - T^Q) of pixel q = lane
+    auto draw = [&](Job& jb) {
+        // next (tile, group) of this CTA; groups outside the image are skipped; tile >= num_tiles means "no more work".
+        // The loads every record of the group's list depends on (count, first 64 ids, T^Q) are issued here, one group
+        // ahead of their use.
+        while (true) {
+            int tile = 0, g = 0;
+            if (lane == 0) {
+                const int ticket = atomicAdd(&s_ticket, 1);
+                const int slot = ticket >> 5, idx = slot % kBlendSlots;
+                g = ticket & 31;
+                volatile unsigned long long* word = &s_slot[idx];
+                volatile int32_t* reads = &s_reads[idx];
+                if (g == 0) {
+                    // claim the next tile for this slot.  The ring entry is reused every kBlendSlots tiles: wait until
+                    // the 31 readers of its previous generation are through (they never wait on this warp: this ends)
+                    if (slot >= kBlendSlots) { while (*reads != 31) { } }
+                    *reads = 0;
+                    tile = atomicAdd(p.tile_ticket, 1);
+                    __threadfence_block();
+                    *word = ((unsigned long long)(slot + 1) << 32) | (unsigned int)tile;
+                } else {
+                    unsigned long long v;
+                    while (((v = *word) >> 32) != (unsigned long long)(slot + 1)) { }
+                    tile = (int)(v & 0xffffffffull);
+                    atomicAdd(&s_reads[idx], 1);
+                }
             }
+            jb.tile = __shfl_sync(0xffffffffu, tile, 0);
+            jb.g = __shfl_sync(0xffffffffu, g, 0);
+            if (jb.tile >= p.num_tiles) return;
+            const int gx0 = (jb.tile % p.cam.tiles_x) * kTile + (jb.g & 3) * 4;
+            const int gy0 = (jb.tile / p.cam.tiles_x) * kTile + (jb.g >> 2) * 2;
+            if (gx0 >= p.cam.width || gy0 >= p.cam.height) continue;
+            const int64_t group = (int64_t)jb.tile * kGroupsPerTile + jb.g;
+            const float* rec = p.rec + group * p.cap * kRecWords;
+            jb.n = __ldg(p.gcount + group);
+            // ids of records lane and 32 + lane (inside the group's capacity whenever K >= 8; guarded otherwise)
+            jb.ids0 = lane < p.cap ? __float_as_int(__ldg(rec + lane * kRecWords + 8)) : -1;
+            jb.ids1 = lane + 32 < p.cap ? __float_as_int(__ldg(rec + (lane + 32) * kRecWords + 8)) : -1;
+            const int mx = gx0 + (lane & 3), my = gy0 + ((lane >> 2) & 1);
+            jb.inv = 0.0f;
+            if (lane < kGroupPx && mx < p.cam.width && my < p.cam.height) {
+                const int64_t mpix = (int64_t)my * p.cam.width + mx;
+                if (__ldg(p.n_sel + mpix) > 0) jb.inv = __fdiv_rn(1.0f, __fsub_rn(1.0f, __ldg(p.resid + mpix)));   // line 20; R8
+            }
+            return;
         }
-        tile = __shfl_sync(0xffffffffu, tile, 0);
-        g = __shfl_sync(0xffffffffu, g, 0);
-        if (tile >= p.num_tiles) break;
-        const int tile_x = tile % p.cam.tiles_x, tile_y = tile / p.cam.tiles_x;
+    };
 
+    Job cur, nxt;
+    draw(cur);
+    while (cur.tile < p.num_tiles) {
+        draw(nxt);
+        const int tile = cur.tile, g = cur.g, n = cur.n;
+        const int tile_x = tile % p.cam.tiles_x, tile_y = tile / p.cam.tiles_x;
         // group g = (row pair g >> 2, x block g & 3); pixel q of the group: x = 4*(g&3) + (q&3), y = 2*(g>>2) + (q>>2)
         const int gx0 = tile_x * kTile + (g & 3) * 4, gy0 = tile_y * kTile + (g >> 2) * 2;
-        if (gx0 >= p.cam.width || gy0 >= p.cam.height) continue;
         const int64_t group = (int64_t)tile * kGroupsPerTile + g;
-        const int n = p.gcount[group];
-        const int32_t* gid = p.gid + group * p.cap;
-        const float4* gw4 = reinterpret_cast<const float4*>(p.gw + group * p.cap * kGroupPx);
+        const float* recf = p.rec + group * p.cap * kRecWords;
+        const float4* rec4 = reinterpret_cast<const float4*>(recf);
+        const float* recw = recf + (lane & 7);                               // lane q < 8: its own pixel's weight
 
         // lanes 0..7 own the bookkeeping of pixel q = lane: 1/(1 - T^Q) and the record cursor
         const int mx = gx0 + (lane & 3), my = gy0 + ((lane >> 2) & 1);
         const bool mine = lane < kGroupPx && mx < p.cam.width && my < p.cam.height;
         const int64_t mpix = (int64_t)my * p.cam.width + mx;
-        float minv = 0.0f;
-        if (mine && p.n_sel[mpix] > 0) minv = __fdiv_rn(1.0f, __fsub_rn(1.0f, p.resid[mpix]));   // line 20; R8
+        const float minv = cur.inv;
         int32_t* my_idx = p.sel_idx + mpix * K;
         float* my_w = p.sel_w + mpix * K;
 
@@ -331,21 +360,29 @@ __global__ void __launch_bounds__(kBlendWarps * 32, 1) blend_kernel(const BlendP
 #pragma unroll
                 for (int v = 0; v < VW; ++v) acc[q][j][v] = 0.0f;
 
-        // software pipeline, two register sets A / B: while record i is applied, the feature row of record i+1 and
-        // the (id, weights) of record i+2 are in flight
-        int32_t idA = 0, idB = 0;
-        float4 wA0, wA1, wB0, wB1;
-        wA0 = wA1 = wB0 = wB1 = make_float4(0.f, 0.f, 0.f, 0.f);
-        float fA[NV][VW], fB[NV][VW];
-        auto load_meta = [&](int i, int32_t& id, float4& w0, float4& w1) {
-            if (i < n) { id = __ldg(gid + i); w0 = __ldg(gw4 + 2 * i); w1 = __ldg(gw4 + 2 * i + 1); }
+        // Software pipeline over three register sets: while record i is applied, the feature rows of records i+1 and
+        // i+2 and the weights of record i+3 are in flight.  Ids come from the lane-parallel prefetch (ids0 = records
+        // 32b..32b+31 of the current block b, ids1 = the next block), so a row load never waits for its id.
+        int32_t ids0 = cur.ids0, ids1 = cur.ids1;
+        int blk = 0;
+        auto id_at = [&](int i) -> int32_t {           // i in block blk or blk + 1; -1 past the end of the list
+            const int32_t v = __shfl_sync(0xffffffffu, ((i >> 5) == blk) ? ids0 : ids1, i & 31);
+            return i < n ? v : -1;
         };
-        auto load_row = [&](int i, int32_t id, float (&f)[NV][VW]) {
-            if (i < n) {
+        struct Meta { float4 w0, w1; float wm; };
+        auto load_meta = [&](int i) {
+            Meta m;
+            m.w0 = __ldg(rec4 + 3 * i);
+            m.w1 = __ldg(rec4 + 3 * i + 1);
+            m.wm = __ldg(recw + (size_t)i * kRecWords);
+            return m;
+        };
+        auto load_row = [&](int32_t id, float (&f)[NV][VW]) {
+            if (id >= 0) {
+                const FeatT* rowp = static_cast<const FeatT*>(p.features) + (int64_t)id * D + lane * VW;
 #pragma unroll
                 for (int j = 0; j < NV; ++j) {
-                    const int ch = (j * 32 + lane) * VW;
-                    if (FULL || ch < D) Row<FeatT, VW>::load(p.features, id, D, ch, f[j]);
+                    if (FULL || (j * 32 + lane) * VW < D) Row<FeatT, VW>::load(rowp + j * 32 * VW, f[j]);
                     else {
 #pragma unroll
                         for (int v = 0; v < VW; ++v) f[j][v] = 0.0f;
@@ -353,19 +390,18 @@ __global__ void __launch_bounds__(kBlendWarps * 32, 1) blend_kernel(const BlendP
                 }
             }
         };
-        auto apply = [&](int32_t id, const float4& w0, const float4& w1, const float (&f)[NV][VW]) {
-            const float w[kGroupPx] = { w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w };
+        auto apply = [&](const Meta& m, int32_t id, const float (&f)[NV][VW]) {
             // selection record of pixel q = lane, in list (= depth) order
-            float wm = w[0];
-#pragma unroll
-            for (int q = 1; q < kGroupPx; ++q) wm = (lane == q) ? w[q] : wm;
-            if (mine && wm != 0.0f) {
+            if (mine && m.wm != 0.0f) {
                 *my_idx++ = id;
-                *my_w++ = __fmul_rn(wm, minv);
+                *my_w++ = __fmul_rn(m.wm, minv);
             }
+            // which of the 8 pixels selected this Gaussian: a ballot, so the branches below are provably uniform
+            const uint32_t nz = __ballot_sync(0xffffffffu, m.wm != 0.0f) & 0xFFu;
+            const float w[kGroupPx] = { m.w0.x, m.w0.y, m.w0.z, m.w0.w, m.w1.x, m.w1.y, m.w1.z, m.w1.w };
 #pragma unroll
             for (int q = 0; q < kGroupPx; ++q) {
-                if (w[q] != 0.0f) {                     // uniform across the warp
+                if (nz & (1u << q)) {
 #pragma unroll
                     for (int j = 0; j < NV; ++j)
 #pragma unroll
@@ -373,20 +409,26 @@ __global__ void __launch_bounds__(kBlendWarps * 32, 1) blend_kernel(const BlendP
                 }
             }
         };
-        load_meta(0, idA, wA0, wA1);
-        load_meta(1, idB, wB0, wB1);
-        load_row(0, idA, fA);
-        for (int i = 0; i < n; i += 2) {
-            load_row(i + 1, idB, fB);
-            const int32_t idA_cur = idA; const float4 a0 = wA0, a1 = wA1;
-            load_meta(i + 2, idA, wA0, wA1);
-            apply(idA_cur, a0, a1, fA);
-            if (i + 1 < n) {
-                load_row(i + 2, idA, fA);
-                const int32_t idB_cur = idB; const float4 b0 = wB0, b1 = wB1;
-                load_meta(i + 3, idB, wB0, wB1);
-                apply(idB_cur, b0, b1, fB);
+        float fA[NV][VW], fB[NV][VW], fC[NV][VW];
+        int32_t iA = id_at(0), iB = id_at(1), iC = id_at(2);
+        Meta mA = load_meta(0), mB = load_meta(1), mC = load_meta(2);
+        load_row(iA, fA);
+        load_row(iB, fB);
+        for (int i = 0; i < n; i += 3) {
+            if (((i + 5) >> 5) > blk + 1) {            // the pipeline is about to leave block blk + 1: slide the id window
+                ++blk;
+                ids0 = ids1;
+                const int r = (blk + 1) * 32 + lane;
+                ids1 = r < p.cap ? __float_as_int(__ldg(recf + (size_t)r * kRecWords + 8)) : -1;
             }
+            load_row(iC, fC);
+            { const Meta m = mA; const int32_t id = iA; mA = load_meta(i + 3); iA = id_at(i + 3); apply(m, id, fA); }
+            if (i + 1 >= n) break;
+            load_row(iA, fA);
+            { const Meta m = mB; const int32_t id = iB; mB = load_meta(i + 4); iB = id_at(i + 4); apply(m, id, fB); }
+            if (i + 2 >= n) break;
+            load_row(iB, fB);
+            { const Meta m = mC; const int32_t id = iC; mC = load_meta(i + 5); iC = id_at(i + 5); apply(m, id, fC); }
         }
 
         // ---- epilogue: normalise and store (512 contiguous bytes per store instruction) ----
@@ -408,6 +450,7 @@ __global__ void __launch_bounds__(kBlendWarps * 32, 1) blend_kernel(const BlendP
                 }
             }
         }
+        cur = nxt;
     }
 }
 
@@ -471,15 +514,14 @@ extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype f
     wp.n_sel = n_sel; wp.resid = resid_TQ; wp.sel_idx = sel_idx; wp.sel_w = sel_w;
     wp.tile_ticket = reinterpret_cast<int32_t*>(w + L.ticket);
     wp.gcount = reinterpret_cast<int32_t*>(w + L.gcount);
-    wp.gid = reinterpret_cast<int32_t*>(w + L.gid);
-    wp.gw = reinterpret_cast<float*>(w + L.gw);
+    wp.rec = reinterpret_cast<float*>(w + L.rec);
     const size_t smem = kWalkBatch * (16 + 16 + 8 + 4) + (size_t)(K + 1) * 4;
     walk_kernel<<<(unsigned)T, kWalkThreads, smem, st>>>(wp);
     QR_LAUNCH_OK("walk_kernel");
 
     BlendParams bp;
     bp.cam = c; bp.K = K; bp.D = D; bp.cap = L.cap; bp.num_tiles = T; bp.tile_ticket = wp.tile_ticket;
-    bp.features = features; bp.gcount = wp.gcount; bp.gid = wp.gid; bp.gw = wp.gw;
+    bp.features = features; bp.gcount = wp.gcount; bp.rec = wp.rec;
     bp.n_sel = n_sel; bp.resid = resid_TQ; bp.out_map = out_map; bp.sel_idx = sel_idx; bp.sel_w = sel_w;
     if (feat_dtype == QR_F16) {
         if ((D + 255) / 256 == 1) return launch_blend<__half, 1, 8>(bp, st);
