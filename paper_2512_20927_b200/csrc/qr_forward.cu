@@ -167,7 +167,12 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
                 const uint32_t sm = __ballot_sync(0xffffffffu, sel);
                 if (sm & gbits) {                       // some pixel of my group selected this Gaussian
                     my_rec[gcnt * kRecWords + q] = wQ;  // 8 lanes write the record's 8 weights (32 contiguous bytes)
-                    if (q == 0) my_rec[gcnt * kRecWords + 8] = __int_as_float(ent_id[e]);
+                    if (q == 0) {
+                        // word 8 = Gaussian id, word 9 = which of the 8 pixels selected it (bit q)
+                        const uint32_t nz = ((sm >> (4 * gx)) & 0xFu) | (((sm >> (16 + 4 * gx)) & 0xFu) << 4);
+                        *reinterpret_cast<float2*>(my_rec + gcnt * kRecWords + 8) =
+                            make_float2(__int_as_float(ent_id[e]), __int_as_float((int)nz));
+                    }
                     ++gcnt;
                 }
             }
@@ -454,6 +459,416 @@ __global__ void __launch_bounds__(kBlendWarps * 32, 1) blend_kernel(const BlendP
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// blend_tu_kernel -- the O(KC) blend with the band's union of selected Gaussians staged ONCE in shared memory by TMA.
+//
+// Persistent CTA = 1 producer warp + 8 consumer warps.  Work item = one 16x4-pixel band of a tile = 8 pixel groups,
+// one per consumer warp.  The producer builds a stage: it takes up to kTuRecs records of each of the band's 8 lists,
+// numbers the distinct Gaussian ids among them (shared-memory hash set), and issues one bulk async copy
+// (cp.async.bulk ... mbarrier::complete_tx) per distinct feature row and per record list into the stage buffers.
+// Consumers wait on the stage's "full" mbarrier, then read weights, row slots and rows from shared memory only:
+// a feature row crosses L2 -> SM once per band instead of once per pixel group, and no consumer ever waits on a
+// global load.  Two stages: the producer fills one while the consumers drain the other.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int kTuConsumers = 8;
+constexpr int kTuProducers = 4;        // warps 8..11, one per scheduler
+constexpr int kTuThreads = 384;         // warps 0..7 consumers, warps 8..11 producers
+constexpr int kTuProducerRegs = 72;    // setmaxnreg: 12 warps start at 168 registers; the producer warpgroup drops to
+constexpr int kTuConsumerRegs = 216;   // 72 and the two consumer warpgroups grow to 216 (128 accumulators + 2 row sets)
+constexpr int kTuStages = 2;
+constexpr int kTuRows = 46;            // distinct feature rows per stage
+constexpr int kTuRecs = 32;            // records per group per stage (one per producer lane)
+constexpr int kTuHash = 512;           // >= 2 * 8 * kTuRecs
+
+struct TuDesc {
+    int32_t tile, band, flags;         // flags: 1 = first stage of the band, 2 = last stage, 4 = no more work
+    int32_t nrec[kTuConsumers];
+    float inv[kTuConsumers * kGroupPx];   // 1/(1 - T^Q) per pixel of the band, 0 where nothing is selected
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred P1;\n\tWAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+        "@P1 bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
+        ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+__device__ __forceinline__ void st_global_pred(int32_t* ptr, int32_t v, bool on)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %2, 0;\n\t@p st.global.b32 [%0], %1;\n\t}" ::"l"(ptr), "r"(v), "r"((int)on) : "memory");
+}
+__device__ __forceinline__ void st_global_pred(float* ptr, float v, bool on)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %2, 0;\n\t@p st.global.f32 [%0], %1;\n\t}" ::"l"(ptr), "f"(v), "r"((int)on) : "memory");
+}
+
+template <typename FeatT, int VW> struct SRow;
+template <> struct SRow<float, 4> {
+    static __device__ __forceinline__ void load(const unsigned char* row, int lane_vec, float (&f)[4])
+    {
+        const float4 v = *reinterpret_cast<const float4*>(row + (size_t)lane_vec * 16);
+        f[0] = v.x; f[1] = v.y; f[2] = v.z; f[3] = v.w;
+    }
+};
+template <> struct SRow<__half, 8> {
+    static __device__ __forceinline__ void load(const unsigned char* row, int lane_vec, float (&f)[8])
+    {
+        const uint4 v = *reinterpret_cast<const uint4*>(row + (size_t)lane_vec * 16);
+        const __half2* h = reinterpret_cast<const __half2*>(&v);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { const float2 t = __half22float2(h[i]); f[2 * i] = t.x; f[2 * i + 1] = t.y; }
+    }
+};
+
+struct TuSmem {            // offsets into dynamic shared memory
+    int rows, recs, rslot, desc, bars, hkey, hslot, uniq, total;
+};
+__host__ __device__ inline TuSmem tu_smem(int rowbytes)
+{
+    TuSmem L;
+    int o = 0;
+    L.rows = o;  o += kTuStages * kTuRows * rowbytes;
+    L.recs = o;  o += kTuStages * kTuConsumers * kTuRecs * kRecWords * 4;
+    L.desc = o;  o += (kTuStages * (int)sizeof(TuDesc) + 15) & ~15;
+    L.bars = o;  o += 2 * kTuStages * 8;
+    L.hkey = o;  o += kTuProducers * kTuHash * 4;
+    L.uniq = o;  o += kTuProducers * 48 * 4;
+    L.rslot = o; o += kTuStages * kTuConsumers * kTuRecs;
+    L.hslot = o; o += kTuProducers * kTuHash;
+    L.total = (o + 15) & ~15;
+    return L;
+}
+
+template <typename FeatT, int NV, int VW, bool FULL>
+__global__ void __launch_bounds__(kTuThreads, 1) blend_tu_kernel(const BlendParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int D = p.D, K = p.K;
+    const int rowbytes = D * (int)sizeof(FeatT);
+    const TuSmem L = tu_smem(rowbytes);
+    unsigned char* s_rows = smem + L.rows;
+    float* s_recs = reinterpret_cast<float*>(smem + L.recs);
+    TuDesc* s_desc = reinterpret_cast<TuDesc*>(smem + L.desc);
+    uint64_t* s_full = reinterpret_cast<uint64_t*>(smem + L.bars);
+    uint64_t* s_empty = s_full + kTuStages;
+    uint8_t* s_rslot = smem + L.rslot;
+    __shared__ int32_t s_lock, s_it, s_finished;   // producers: publish lock, next stage number, producers out of work
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) {
+        s_lock = 0; s_it = 0; s_finished = 0;
+        for (int s = 0; s < kTuStages; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], kTuConsumers); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const int num_items = p.num_tiles * 4;
+
+    if (warp >= kTuConsumers) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kTuProducerRegs));
+        // =========================================== producers ===========================================
+        // Four producer warps, one per scheduler, each building the stages of its own bands: a producer warp shares
+        // its scheduler with two consumer warps that issue FFMAs back to back, so one stage build takes ~20k cycles
+        // of wall time (measured) although it is a few hundred instructions; four bands in flight keep the stage
+        // rate above what the consumers drain.  Publishing (wait for a free buffer, descriptor, copies) is
+        // serialised by a lock so that the stages of one band stay contiguous and in order.
+        const int pw = warp - kTuConsumers;
+        int32_t* s_hkey = reinterpret_cast<int32_t*>(smem + L.hkey) + pw * kTuHash;
+        int32_t* s_uniq = reinterpret_cast<int32_t*>(smem + L.uniq) + pw * 48;
+        uint8_t* s_hslot = smem + L.hslot + pw * kTuHash;
+        volatile int32_t* v_it = &s_it;
+        // Per item (band) the producer needs the 8 list lengths and the 64 pixels' T^Q; those loads, and the ticket
+        // itself, are issued one item ahead so that their latency hides behind the stage building of the current item.
+        struct Item { int item; int n_w; float inv2[2]; };
+        auto fetch = [&](Item& t) {
+            int item = 0;
+            if (lane == 0) item = atomicAdd(p.tile_ticket, 1);
+            t.item = __shfl_sync(0xffffffffu, item, 0);
+            t.n_w = 0; t.inv2[0] = t.inv2[1] = 0.0f;
+            if (t.item >= num_items) return;
+            const int tile = t.item >> 2, band = t.item & 3;
+            const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + band * 4;
+            if (y0 >= p.cam.height) return;
+            t.n_w = __ldg(p.gcount + (int64_t)tile * kGroupsPerTile + band * 8 + (lane & 7));
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {      // lane handles pixels lane and lane + 32 of the band (group-major numbering)
+                const int gp = lane + 32 * h, w = gp >> 3, q = gp & 7;
+                const int x = x0 + (w & 3) * 4 + (q & 3), y = y0 + (w >> 2) * 2 + (q >> 2);
+                if (x < p.cam.width && y < p.cam.height) {
+                    const int64_t pix = (int64_t)y * p.cam.width + x;
+                    if (__ldg(p.n_sel + pix) > 0) t.inv2[h] = __fdiv_rn(1.0f, __fsub_rn(1.0f, __ldg(p.resid + pix)));   // line 20; R8
+                }
+            }
+        };
+        auto lock = [&]() {
+            if (lane == 0) { while (atomicCAS(&s_lock, 0, 1) != 0) { } }
+            __syncwarp();
+            __threadfence_block();
+        };
+        auto unlock = [&]() {
+            __threadfence_block();
+            __syncwarp();
+            if (lane == 0) atomicExch(&s_lock, 0);
+        };
+        Item cur_item, next_item;
+        fetch(cur_item);
+        while (true) {
+            const int item = cur_item.item;
+            if (item >= num_items) {
+                // the last producer to run out of work tells the consumers to stop
+                int last_one = 0;
+                if (lane == 0) last_one = atomicAdd(&s_finished, 1) == kTuProducers - 1;
+                if (__shfl_sync(0xffffffffu, last_one, 0)) {
+                    lock();
+                    const int it = *v_it;
+                    const int s_done = it % kTuStages;
+                    mbar_wait(&s_empty[s_done], ((it / kTuStages) & 1) ^ 1);
+                    if (lane == 0) { s_desc[s_done].flags = 4; mbar_arrive(&s_full[s_done]); }
+                    unlock();
+                }
+                break;
+            }
+            fetch(next_item);
+            const int tile = item >> 2, band = item & 3;
+            const int y0 = (tile / p.cam.tiles_x) * kTile + band * 4;
+            if (y0 >= p.cam.height) { cur_item = next_item; continue; }   // band below the image: nothing to render
+            // lane w < 8 tracks group w of the band: list length and progress
+            const int64_t gi = (int64_t)tile * kGroupsPerTile + band * 8 + (lane & 7);
+            const int n_w = cur_item.n_w;
+            int r0_w = 0;
+            const float inv2[2] = { cur_item.inv2[0], cur_item.inv2[1] };
+            bool first = true, locked = false;
+            while (true) {
+                // ---- choose the stage's records: up to R per group such that their distinct rows fit ----
+                int R = kTuRecs, cnt_w = 0, U = 0;
+                int32_t ids[kTuConsumers];
+                uint8_t slot8[kTuConsumers];
+                int hcell[kTuConsumers];
+                while (true) {
+                    cnt_w = min(R, n_w - r0_w);
+                    for (int i = lane; i < kTuHash; i += 32) s_hkey[i] = -1;
+                    __syncwarp();
+#pragma unroll
+                    for (int w = 0; w < kTuConsumers; ++w) {       // group w, record r0 + lane: 8 independent loads
+                        const int c = __shfl_sync(0xffffffffu, cnt_w, w), r0 = __shfl_sync(0xffffffffu, r0_w, w);
+                        ids[w] = -1;
+                        if (lane < c) {
+                            const int64_t g = (int64_t)tile * kGroupsPerTile + band * 8 + w;
+                            ids[w] = __float_as_int(__ldg(p.rec + (g * p.cap + r0 + lane) * kRecWords + 8));
+                        }
+                    }
+                    // insert: first probes of the 8 records are independent shared-memory CAS operations (in flight
+                    // together); only collisions walk on
+                    int32_t old[kTuConsumers];
+#pragma unroll
+                    for (int w = 0; w < kTuConsumers; ++w) {
+                        hcell[w] = (int)(((uint32_t)ids[w] * 2654435761u) >> 23);       // 9 bits
+                        old[w] = ids[w];
+                        if (ids[w] >= 0) old[w] = atomicCAS(&s_hkey[hcell[w]], -1, ids[w]);
+                    }
+#pragma unroll
+                    for (int w = 0; w < kTuConsumers; ++w) {
+                        if (ids[w] >= 0 && old[w] != -1 && old[w] != ids[w]) {
+                            int h = hcell[w];
+                            while (true) {
+                                h = (h + 1) & (kTuHash - 1);
+                                const int32_t o = atomicCAS(&s_hkey[h], -1, ids[w]);
+                                if (o == -1 || o == ids[w]) break;
+                            }
+                            hcell[w] = h;
+                        }
+                    }
+                    __syncwarp();
+                    // number the occupied cells with ballots (no atomics): cell i of lane-strided chunk c gets
+                    // base + (occupied cells before it in the chunk)
+                    U = 0;
+#pragma unroll 4
+                    for (int c = 0; c < kTuHash; c += 32) {
+                        const int32_t id = s_hkey[c + lane];
+                        const uint32_t occ = __ballot_sync(0xffffffffu, id >= 0);
+                        if (id >= 0) {
+                            const int slot = U + __popc(occ & ((1u << lane) - 1u));
+                            s_hslot[c + lane] = (uint8_t)slot;
+                            if (slot < kTuRows) s_uniq[slot] = id;
+                        }
+                        U += __popc(occ);
+                    }
+                    __syncwarp();
+                    if (U <= kTuRows) break;
+                    R = max(R >> 1, 1);                            // R = 1 always fits (<= 8 rows)
+                }
+#pragma unroll
+                for (int w = 0; w < kTuConsumers; ++w) slot8[w] = ids[w] >= 0 ? s_hslot[hcell[w]] : (uint8_t)0;
+                const bool last = __all_sync(0xffffffffu, r0_w + cnt_w >= n_w);
+
+                // ---- publish the stage ----
+                if (!locked) { lock(); locked = true; }
+                const int it = *v_it;
+                const int s = it % kTuStages;
+                mbar_wait(&s_empty[s], ((it / kTuStages) & 1) ^ 1);
+                TuDesc* d = &s_desc[s];
+                if (lane == 0) { d->tile = tile; d->band = band; d->flags = (first ? 1 : 0) | (last ? 2 : 0); }
+                if (lane < kTuConsumers) d->nrec[lane] = cnt_w;
+                d->inv[lane] = inv2[0];
+                d->inv[lane + 32] = inv2[1];
+#pragma unroll
+                for (int w = 0; w < kTuConsumers; ++w) s_rslot[(s * kTuConsumers + w) * kTuRecs + lane] = slot8[w];
+                uint32_t bytes = (lane < kTuConsumers ? (uint32_t)cnt_w * kRecWords * 4u : 0u);
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
+                bytes += (uint32_t)U * (uint32_t)rowbytes;
+                __syncwarp();
+                if (lane == 0) mbar_arrive_expect_tx(&s_full[s], bytes);
+                __syncwarp();
+                for (int u = lane; u < U; u += 32)
+                    bulk_g2s(s_rows + ((size_t)s * kTuRows + u) * rowbytes,
+                             static_cast<const unsigned char*>(p.features) + (size_t)s_uniq[u] * rowbytes,
+                             (uint32_t)rowbytes, &s_full[s]);
+                if (lane < kTuConsumers && cnt_w > 0)
+                    bulk_g2s(s_recs + ((size_t)s * kTuConsumers + lane) * kTuRecs * kRecWords,
+                             p.rec + (gi * p.cap + r0_w) * kRecWords, (uint32_t)cnt_w * kRecWords * 4u, &s_full[s]);
+                __syncwarp();                        // s_uniq / s_hkey are rewritten by the next stage
+                r0_w += cnt_w;
+                first = false;
+                if (lane == 0) *v_it = it + 1;
+                if (last) break;
+            }
+            unlock();
+            cur_item = next_item;
+        }
+    } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kTuConsumerRegs));
+        // =========================================== consumers ===========================================
+        float acc[kGroupPx][NV][VW];
+        int32_t* my_idx = nullptr;
+        float* my_w = nullptr;
+        float minv = 0.0f;
+        bool mine = false;
+        int gx0 = 0, gy0 = 0;
+        for (int it = 0;; ++it) {
+            const int s = it % kTuStages;
+            mbar_wait(&s_full[s], (it / kTuStages) & 1);
+            const TuDesc* d = &s_desc[s];
+            const int flags = d->flags;
+            if (flags & 4) break;
+            if (flags & 1) {
+                const int tile = d->tile, band = d->band;
+                gx0 = (tile % p.cam.tiles_x) * kTile + (warp & 3) * 4;
+                gy0 = (tile / p.cam.tiles_x) * kTile + band * 4 + (warp >> 2) * 2;
+                const int mx = gx0 + (lane & 3), my = gy0 + ((lane >> 2) & 1);
+                mine = lane < kGroupPx && mx < p.cam.width && my < p.cam.height;
+                const int64_t mpix = (int64_t)my * p.cam.width + mx;
+                my_idx = p.sel_idx + mpix * K;
+                my_w = p.sel_w + mpix * K;
+                minv = d->inv[warp * kGroupPx + (lane & 7)];
+#pragma unroll
+                for (int q = 0; q < kGroupPx; ++q)
+#pragma unroll
+                    for (int j = 0; j < NV; ++j)
+#pragma unroll
+                        for (int v = 0; v < VW; ++v) acc[q][j][v] = 0.0f;
+            }
+            const int n = d->nrec[warp];
+            const float* recs = s_recs + ((size_t)s * kTuConsumers + warp) * kTuRecs * kRecWords;
+            const uint8_t* rslot = s_rslot + (s * kTuConsumers + warp) * kTuRecs;
+            const unsigned char* rows = s_rows + (size_t)s * kTuRows * rowbytes;
+            // Branch-free inner loop.  Measured on B200 (profiles/): with two warps per scheduler a predicated branch
+            // costs a warp ~15-20 issue cycles, more than the 16 FFMAs it would skip, so all 8 pixels are always
+            // updated (a pixel that did not select the Gaussian has weight 0).  Software pipeline over two register
+            // sets: the weights / id / row of record i+1 are loaded from shared memory while record i is applied.
+            struct Meta { float4 w0, w1; float wm; int32_t id; };
+            auto load_meta = [&](int i) {
+                Meta m;
+                m.w0 = *reinterpret_cast<const float4*>(recs + i * kRecWords);
+                m.w1 = *reinterpret_cast<const float4*>(recs + i * kRecWords + 4);
+                m.id = __float_as_int(recs[i * kRecWords + 8]);
+                m.wm = recs[i * kRecWords + (lane & 7)];
+                return m;
+            };
+            auto load_f = [&](int i, float (&f)[NV][VW]) {
+                const unsigned char* row = rows + (size_t)rslot[i] * rowbytes;
+#pragma unroll
+                for (int j = 0; j < NV; ++j) {
+                    if (FULL || (j * 32 + lane) * VW < D) SRow<FeatT, VW>::load(row, j * 32 + lane, f[j]);
+                    else {
+#pragma unroll
+                        for (int v = 0; v < VW; ++v) f[j][v] = 0.0f;
+                    }
+                }
+            };
+            auto apply = [&](const Meta& m, const float (&f)[NV][VW]) {
+                // selection record of pixel q = lane, in list (= depth) order; predicated stores, no divergence
+                const bool on = mine && m.wm != 0.0f;
+                st_global_pred(my_idx, m.id, on);
+                st_global_pred(my_w, __fmul_rn(m.wm, minv), on);
+                my_idx += on ? 1 : 0;
+                my_w += on ? 1 : 0;
+                const float w[kGroupPx] = { m.w0.x, m.w0.y, m.w0.z, m.w0.w, m.w1.x, m.w1.y, m.w1.z, m.w1.w };
+#pragma unroll
+                for (int q = 0; q < kGroupPx; ++q)
+#pragma unroll
+                    for (int j = 0; j < NV; ++j)
+#pragma unroll
+                        for (int v = 0; v < VW; ++v) acc[q][j][v] = __fmaf_rn(w[q], f[j][v], acc[q][j][v]);   // line 9
+            };
+            if (n > 0) {
+                float fA[NV][VW], fB[NV][VW];
+                Meta mA = load_meta(0), mB;
+                load_f(0, fA);
+                int i = 0;
+                for (; i + 1 < n; i += 2) {
+                    mB = load_meta(i + 1); load_f(i + 1, fB);
+                    apply(mA, fA);
+                    if (i + 2 < n) { mA = load_meta(i + 2); load_f(i + 2, fA); }
+                    apply(mB, fB);
+                }
+                if (n & 1) apply(mA, fA);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&s_empty[s]);     // stage buffers are free; the epilogue uses registers only
+            if (flags & 2) {
+#pragma unroll
+                for (int q = 0; q < kGroupPx; ++q) {
+                    const int x = gx0 + (q & 3), y = gy0 + (q >> 2);
+                    const float inv = __shfl_sync(0xffffffffu, minv, q);
+                    if (x < p.cam.width && y < p.cam.height) {
+                        float* dst = p.out_map + ((int64_t)y * p.cam.width + x) * D;
+#pragma unroll
+                        for (int j = 0; j < NV; ++j) {
+                            const int ch = (j * 32 + lane) * VW;
+                            if (FULL || ch < D) {
+                                float o[VW];
+#pragma unroll
+                                for (int v = 0; v < VW; ++v) o[v] = __fmul_rn(acc[q][j][v], inv);
+                                store_map<VW>(dst + ch, o);
+                            }
+                        }
+                    }
+                }
+            }
+        }
+    }
+}
+
 static int sm_count()
 {
     static int n = 0;
@@ -463,6 +878,24 @@ static int sm_count()
             n = 148;
     }
     return n;
+}
+
+template <typename FeatT, int NV, int VW>
+static int launch_blend_tu(const BlendParams& p, cudaStream_t st)
+{
+    const unsigned grid = (unsigned)min(sm_count(), p.num_tiles * 4);
+    const int smem = tu_smem(p.D * (int)sizeof(FeatT)).total;
+    if (p.D == NV * 32 * VW) {
+        auto kern = blend_tu_kernel<FeatT, NV, VW, true>;
+        QR_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        kern<<<grid, kTuThreads, smem, st>>>(p);
+    } else {
+        auto kern = blend_tu_kernel<FeatT, NV, VW, false>;
+        QR_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        kern<<<grid, kTuThreads, smem, st>>>(p);
+    }
+    QR_LAUNCH_OK("blend_tu_kernel");
+    return QR_OK;
 }
 
 template <typename FeatT, int NV, int VW>
@@ -524,15 +957,15 @@ extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype f
     bp.features = features; bp.gcount = wp.gcount; bp.rec = wp.rec;
     bp.n_sel = n_sel; bp.resid = resid_TQ; bp.out_map = out_map; bp.sel_idx = sel_idx; bp.sel_w = sel_w;
     if (feat_dtype == QR_F16) {
-        if ((D + 255) / 256 == 1) return launch_blend<__half, 1, 8>(bp, st);
-        return launch_blend<__half, 2, 8>(bp, st);
+        if ((D + 255) / 256 == 1) return launch_blend_tu<__half, 1, 8>(bp, st);
+        return launch_blend_tu<__half, 2, 8>(bp, st);
     }
     if (D % 4 == 0) {
         switch ((D + 127) / 128) {
-            case 1: return launch_blend<float, 1, 4>(bp, st);
-            case 2: return launch_blend<float, 2, 4>(bp, st);
-            case 3: return launch_blend<float, 3, 4>(bp, st);
-            default: return launch_blend<float, 4, 4>(bp, st);
+            case 1: return launch_blend_tu<float, 1, 4>(bp, st);
+            case 2: return launch_blend_tu<float, 2, 4>(bp, st);
+            case 3: return launch_blend_tu<float, 3, 4>(bp, st);
+            default: return launch_blend_tu<float, 4, 4>(bp, st);
         }
     }
     switch ((D + 31) / 32) {
