@@ -758,7 +758,7 @@ __global__ void __launch_bounds__(kTuThreads, 1) blend_tu_kernel(const BlendPara
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kTuConsumerRegs));
         // =========================================== consumers ===========================================
-        float acc[kGroupPx][NV][VW];
+        float2 acc[kGroupPx][NV][VW / 2];     // packed pairs: the blend runs on FFMA2 (fma.rn.f32x2)
         int32_t* my_idx = nullptr;
         float* my_w = nullptr;
         float minv = 0.0f;
@@ -785,7 +785,7 @@ __global__ void __launch_bounds__(kTuThreads, 1) blend_tu_kernel(const BlendPara
 #pragma unroll
                     for (int j = 0; j < NV; ++j)
 #pragma unroll
-                        for (int v = 0; v < VW; ++v) acc[q][j][v] = 0.0f;
+                        for (int v = 0; v < VW / 2; ++v) acc[q][j][v] = make_float2(0.0f, 0.0f);
             }
             const int n = d->nrec[warp];
             const float* recs = s_recs + ((size_t)s * kTuConsumers + warp) * kTuRecs * kRecWords;
@@ -824,11 +824,14 @@ __global__ void __launch_bounds__(kTuThreads, 1) blend_tu_kernel(const BlendPara
                 my_w += on ? 1 : 0;
                 const float w[kGroupPx] = { m.w0.x, m.w0.y, m.w0.z, m.w0.w, m.w1.x, m.w1.y, m.w1.z, m.w1.w };
 #pragma unroll
-                for (int q = 0; q < kGroupPx; ++q)
+                for (int q = 0; q < kGroupPx; ++q) {
+                    const float2 ww = make_float2(w[q], w[q]);
 #pragma unroll
                     for (int j = 0; j < NV; ++j)
 #pragma unroll
-                        for (int v = 0; v < VW; ++v) acc[q][j][v] = __fmaf_rn(w[q], f[j][v], acc[q][j][v]);   // line 9
+                        for (int v = 0; v < VW / 2; ++v)       // line 9, two channels per instruction, each an IEEE fma
+                            acc[q][j][v] = __ffma2_rn(ww, make_float2(f[j][2 * v], f[j][2 * v + 1]), acc[q][j][v]);
+                }
             };
             if (n > 0) {
                 float fA[NV][VW], fB[NV][VW];
@@ -858,7 +861,10 @@ __global__ void __launch_bounds__(kTuThreads, 1) blend_tu_kernel(const BlendPara
                             if (FULL || ch < D) {
                                 float o[VW];
 #pragma unroll
-                                for (int v = 0; v < VW; ++v) o[v] = __fmul_rn(acc[q][j][v], inv);
+                                for (int v = 0; v < VW / 2; ++v) {
+                                    o[2 * v] = __fmul_rn(acc[q][j][v].x, inv);
+                                    o[2 * v + 1] = __fmul_rn(acc[q][j][v].y, inv);
+                                }
                                 store_map<VW>(dst + ch, o);
                             }
                         }
