@@ -1,0 +1,95 @@
+"""CPU-side (-m "not gpu") checks of the boundary: libqr.so builds/loads without a GPU, exports every symbol that
+include/qr.h declares, and rejects bad arguments with status codes before touching CUDA."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2512_20927_b200 import binding
+    return binding.load()
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "qr.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(qr_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    from paper_2512_20927_b200 import binding
+    names = _declared()
+    assert set(names) == set(binding.SYMBOLS), (names, binding.SYMBOLS)
+    for n in names:
+        assert getattr(lib, n) is not None
+
+
+def test_version_and_tiles(lib):
+    from paper_2512_20927_b200 import binding
+    from qr_inputs import make_camera
+    assert lib.qr_version() == 100
+    assert binding.qr_num_tiles(make_camera(640, 480)) == 1200
+    assert binding.qr_num_tiles(make_camera(70, 50)) == 5 * 4
+    assert lib.qr_num_tiles(None) == 0
+
+
+def test_bad_arguments_are_status_codes(lib):
+    from paper_2512_20927_b200 import binding
+    from qr_inputs import make_camera
+    cam = binding.make_camera(make_camera(64, 64))
+    p = C.c_void_p(16)      # non-NULL, never dereferenced: every check below fails before any CUDA call
+    z = C.c_void_p(0)
+    # K = 0 is a domain error, K > QR_MAX_K unsupported
+    assert lib.qr_forward(C.byref(cam), 0, 16, 0, p, p, p, p, p, p, p, p, p, p, p, 1 << 20, None) == -1
+    assert b"K = 0" in lib.qr_last_error()
+    assert lib.qr_forward(C.byref(cam), 1000, 16, 0, p, p, p, p, p, p, p, p, p, p, p, 1 << 20, None) == -3
+    # D limits and fp16 alignment
+    assert lib.qr_forward(C.byref(cam), 40, 0, 0, p, p, p, p, p, p, p, p, p, p, p, 1 << 20, None) == -1
+    assert lib.qr_forward(C.byref(cam), 40, 1024, 0, p, p, p, p, p, p, p, p, p, p, p, 1 << 20, None) == -3
+    assert lib.qr_forward(C.byref(cam), 40, 12, 1, p, p, p, p, p, p, p, p, p, p, p, 1 << 20, None) == -3
+    # NULL outputs, too-small workspace
+    assert lib.qr_forward(C.byref(cam), 40, 16, 0, p, p, p, p, p, z, p, p, p, p, p, 1 << 20, None) == -2
+    need = lib.qr_forward_workspace_bytes(C.byref(cam), 40, 16)
+    assert need > 0
+    assert lib.qr_forward(C.byref(cam), 40, 16, 0, p, p, p, p, p, p, p, p, p, p, p, need - 1, None) == -4
+    # zero-area image, NULL camera
+    bad = binding.make_camera(make_camera(64, 64)); bad.width = 0
+    assert lib.qr_preprocess(C.byref(bad), 10, p, p, p, p, p, p, p, p, p, None) == -1
+    assert lib.qr_preprocess(None, 10, p, p, p, p, p, p, p, p, p, None) == -2
+    assert lib.qr_preprocess(C.byref(cam), -1, p, p, p, p, p, p, p, p, p, None) == -1
+    assert lib.qr_preprocess(C.byref(cam), 0, z, z, z, z, z, z, z, z, z, None) == 0      # N = 0 is legal
+    assert lib.qr_dense_forward(C.byref(cam), 16, 0, C.c_float(-1.0), p, p, p, p, p, p, p, None) == -1
+    assert lib.qr_backward(C.byref(cam), 0, 16, 10, p, p, p, p, p, None, 0, None) == -1
+    assert lib.qr_bin_sort(C.byref(cam), 10, 1 << 31, p, p, p, p, p, p, 1 << 20, None) == -5
+    m = C.c_int64(-1)
+    assert lib.qr_bin_count(0, z, z, C.byref(m), z, 0, None) == 0 and m.value == 0
+    assert lib.qr_bin_workspace_bytes(1000, 5000, 16) > 5000 * 20
+
+
+def test_binding_refuses_cpu_tensors():
+    import torch
+    from paper_2512_20927_b200 import binding
+    from qr_inputs import make_camera
+    t = torch.zeros((4, 3))
+    with pytest.raises(binding.QRError):
+        binding.qr_preprocess(make_camera(32, 32), t, t, torch.zeros((4, 4)), torch.zeros(4))
+
+
+def test_product_never_imports_oracle():
+    """The CUDA package and the oracle share no code and neither imports the other."""
+    pkg = os.path.join(ROOT, "paper_2512_20927_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt and "qr_oracle" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2512" not in txt and "from paper_2512" not in txt and "libqr.so" not in txt, f
+            assert not re.search(r'#include\s+"[^"]*(csrc|qr\.h|qr_common)', txt), f
