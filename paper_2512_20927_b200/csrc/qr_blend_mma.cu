@@ -1,0 +1,513 @@
+// qr_blend_mma.cu -- the O(KC) blend of qr_forward (Algorithm 1 lines 9 and 20) as a dense
+// contraction on the 5th-generation tensor cores.
+//
+// Per 16x8-pixel half tile the blend is  out[128 px, D] = W[128 px, U] . F[U, D]  with U the union of the Gaussians
+// selected by any of the 128 pixels (mean 47, 23 % dense at config 3) and W the sparse weights w^Q.  ncu showed the
+// FFMA formulation of this product to be issue bound at 3x the time of its HBM traffic (profiles/README.md, r1_a),
+// which is the evidence north_star asks for before putting it on tensor cores.
+//
+// Precision: kind::tf32 truncates its fp32 operands to 10 explicit mantissa bits (measured on B200), so both operands
+// are split exactly, x = hi + lo with hi = x & 0xFFFFE000 and lo = x - hi, and three MMAs accumulate
+// W_hi F_hi + W_lo F_hi + W_hi F_lo in fp32 (TMEM).  The dropped W_lo F_lo term and the truncation of the lo parts
+// are <= 2^-21 relative per product, 40x below the fp32 tolerance of north_star (1e-4 relative).
+//
+// One persistent CTA per SM, 14 warps, roles by warp (no role ever waits at a block barrier):
+//   warps 0..3   epilogue: tcgen05.ld of the accumulator (thread = pixel), x 1/(1 - T^Q), swizzled st.shared into a
+//                32-pixel x 32-channel staging tile, one TMA tensor store (cp.async.bulk.tensor.3d) per tile
+//   warp  4      one thread issues tcgen05.mma (M = 128 pixels, N = 256 channels, K = 8 union rows per instruction)
+//   warp  5      loader: one bulk async copy (TMA) per feature row half (1 KB) into a raw ring, far ahead of use
+//   warps 6..13  producers: build W (K-major, no swizzle) from walk_kernel's group records, write the per-pixel
+//                selection records, and convert raw feature rows: ld.shared -> hi/lo split -> st.shared in the
+//                MN-major SWIZZLE_128B_BASE32B layout tf32 needs for a row-major (channel-contiguous) B operand
+// Work unit = (half tile, 256-channel half): two 256-column accumulators in TMEM, so the MMAs of unit i+1 overlap
+// the epilogue of unit i.  A half tile whose union exceeds 64 columns is processed in rounds of 64 columns.
+#include <cuda.h>
+
+#include "qr_blend.cuh"
+
+namespace qr {
+
+constexpr int kEpiWarps = 4;
+constexpr int kProdWarps = 8;
+constexpr int kMmaWarp = kEpiWarps;                       // warp 4
+constexpr int kLoadWarp = kEpiWarps + 1;                  // warp 5
+constexpr int kFirstProd = kEpiWarps + 2;                 // warps 6..13
+constexpr int kMmaThreads = (kEpiWarps + 2 + kProdWarps) * 32;
+constexpr int kProdThreads = kProdWarps * 32;
+constexpr int kWCols = 64;                                // union columns per round
+constexpr int kUnitN = 256;                               // channels per work unit
+constexpr int kStageRows = 8;                             // union rows per stage = one tf32 K step
+constexpr int kStages = 4;
+constexpr int kRawStages = 8;
+constexpr int kRawRow = kUnitN * 4;                       // 1 KB: one feature row half
+constexpr int kRawBytes = kStageRows * kRawRow;           // 8 KB per raw stage
+constexpr int kEpiTile = 32 * 32 * 4;                     // 4 KB: 32 pixels x 32 channels
+constexpr int kWBytes = 128 * kWCols * 4;                 // 32 KB per W buffer (hi, lo)
+constexpr int kStageHalf = kStageRows * kUnitN * 4;       // 8 KB (hi or lo)
+constexpr int kStageBytes = 2 * kStageHalf;
+
+struct MmaSmem {
+    static constexpr int w_hi = 0;
+    static constexpr int w_lo = kWBytes;
+    static constexpr int stages = 2 * kWBytes;
+    static constexpr int raw = stages + kStages * kStageBytes;
+    static constexpr int epi = raw + kRawStages * kRawBytes;              // [4 warps][2] staging tiles
+    static constexpr int uid = epi + kEpiWarps * 2 * kEpiTile;            // int32[kWCols]
+    static constexpr int bars = uid + kWCols * 4;                         // uint64[...]
+    static constexpr int n_bars = 2 * kStages + 2 * kRawStages + 2 + 4;
+    static constexpr int tmem = bars + n_bars * 8;
+    static constexpr int total = tmem + 16;
+};
+
+__device__ __forceinline__ uint32_t s_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void bar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(s_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void bar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred P1;\n\tWAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+        "@P1 bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
+        ::"r"(s_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bar_arrive_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(s_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_row(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(s_u32(dst)), "l"(src), "r"(bytes), "r"(s_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar)     // arrives when every MMA issued so far by this thread is done
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(s_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+// shared-memory matrix descriptor (sm_100): start >> 4 | LBO >> 4 << 16 | SBO >> 4 << 32 | version 1 << 46 | layout << 61
+__device__ __forceinline__ uint64_t umma_desc(uint32_t addr, uint32_t lbo, uint32_t sbo, uint32_t layout)
+{
+    return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) |
+           ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) | ((uint64_t)1 << 46) | ((uint64_t)layout << 61);
+}
+__device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t a, uint64_t b, uint32_t idesc, bool accumulate)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "l"(a), "l"(b), "r"(idesc), "r"((uint32_t)accumulate) : "memory");
+}
+
+__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
+
+// byte offset of W[m][c] in the K-major, non-swizzled canonical layout: core matrix = 8 pixels x 4 columns (128 B);
+// column chunks 128 B apart (LBO), 8-pixel groups 2 KB apart (SBO)
+__device__ __forceinline__ uint32_t w_off(int m, int c)
+{
+    return (uint32_t)((m >> 3) * (kWCols / 4 * 128) + (c >> 2) * 128 + (m & 7) * 16 + (c & 3) * 4);
+}
+
+// rounds / K steps of a half tile: both the producers and the MMA thread derive them from the union size
+__device__ __forceinline__ int rounds_of(int U) { return U <= kWCols ? 1 : (U + kWCols - 1) / kWCols; }
+__device__ __forceinline__ int cols_of(int U, int r) { return max(0, min(kWCols, U - r * kWCols)); }
+__device__ __forceinline__ int ksteps_of(int ncols) { return max(1, (ncols + kStageRows - 1) / kStageRows); }
+
+__global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tmap)
+{
+    extern __shared__ __align__(1024) unsigned char smem[];
+    float* w_hi = reinterpret_cast<float*>(smem + MmaSmem::w_hi);
+    float* w_lo = reinterpret_cast<float*>(smem + MmaSmem::w_lo);
+    unsigned char* stage_base = smem + MmaSmem::stages;
+    int32_t* uid_s = reinterpret_cast<int32_t*>(smem + MmaSmem::uid);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + MmaSmem::bars);
+    uint64_t* full = bars;                       // [kStages] producers -> MMA (8 warp arrivals)
+    uint64_t* empty = bars + kStages;            // [kStages] MMA -> producers (tcgen05.commit)
+    uint64_t* raw_full = bars + 2 * kStages;     // [kRawStages] loader (TMA complete_tx) -> producers
+    uint64_t* raw_empty = raw_full + kRawStages; // [kRawStages] producers -> loader (8 warp arrivals)
+    uint64_t* w_ready = raw_empty + kRawStages;  // producers -> MMA, loader
+    uint64_t* w_free = w_ready + 1;              // MMA -> producers (tcgen05.commit)
+    uint64_t* tmem_full = w_free + 1;            // [2] MMA -> epilogue (tcgen05.commit)
+    uint64_t* tmem_empty = tmem_full + 2;        // [2] epilogue -> MMA (4 warp arrivals)
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + MmaSmem::tmem);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int D = p.D, K = p.K;
+    const int nunits = D / kUnitN;
+    const int num_half = p.num_tiles * 2;
+
+    if (tid == 0) {
+        for (int s = 0; s < kStages; ++s) { bar_init(&full[s], kProdWarps); bar_init(&empty[s], 1); }
+        for (int s = 0; s < kRawStages; ++s) { bar_init(&raw_full[s], 1); bar_init(&raw_empty[s], kProdWarps); }
+        bar_init(w_ready, 1); bar_init(w_free, 1);
+        for (int b = 0; b < 2; ++b) { bar_init(&tmem_full[b], 1); bar_init(&tmem_empty[b], kEpiWarps); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(s_u32(tmem_slot)), "r"(512) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    auto half_origin = [&](int ht, int& x0, int& y0) {
+        const int tile = ht >> 1;
+        x0 = (tile % p.cam.tiles_x) * kTile;
+        y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
+    };
+
+    if (warp < kEpiWarps) {
+        // ================================================= epilogue =================================================
+        // thread = pixel m = 32 warp + lane of the half tile (row-major 16 x 8): TMEM lane m, 256 columns = channels.
+        // 32 channels at a time: tcgen05.ld -> scale -> 8 swizzled 16-byte st.shared into a [32 px][128 B] tile ->
+        // one TMA tensor store of the box (32 channels, 16 x, 2 y); the tensor map clips pixels outside the image.
+        unsigned char* tile_s = smem + MmaSmem::epi + warp * 2 * kEpiTile;
+        const uint32_t row_off = (uint32_t)lane * 128u;
+        const uint32_t sw = (uint32_t)(lane & 7);
+        int unit = 0, nstore = 0;
+        auto ld32 = [&](uint32_t taddr, uint32_t (&r)[32]) {
+            asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+                         : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                           "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+                           "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+                           "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+                         : "r"(taddr));
+        };
+        for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
+            int x0, y0;
+            half_origin(ht, x0, y0);
+            if (y0 >= p.cam.height) continue;
+            const int m = warp * 32 + lane;
+            const int x = x0 + (m & 15), y = y0 + (m >> 4);
+            const bool valid = x < p.cam.width && y < p.cam.height;
+            const int64_t pix = (int64_t)y * p.cam.width + x;
+            float inv = 0.0f;
+            if (valid && __ldg(p.n_sel + pix) > 0) inv = __fdiv_rn(1.0f, __fsub_rn(1.0f, __ldg(p.resid + pix)));   // line 20; R8
+            for (int c = 0; c < nunits; ++c, ++unit) {
+                const int buf = unit & 1;
+                bar_wait(&tmem_full[buf], (unit >> 1) & 1);
+                tc_fence_after();
+                const uint32_t t0 = tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(buf * kUnitN);
+                auto emit = [&](const uint32_t (&r)[32], int chunk) {
+                    unsigned char* tile = tile_s + (nstore & 1) * kEpiTile;
+                    if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the store that last read this tile is done
+                    __syncwarp();
+#pragma unroll
+                    for (int jj = 0; jj < 8; ++jj)
+                        *reinterpret_cast<float4*>(tile + row_off + (((uint32_t)jj ^ sw) << 4)) =
+                            make_float4(__fmul_rn(__uint_as_float(r[4 * jj]), inv), __fmul_rn(__uint_as_float(r[4 * jj + 1]), inv),
+                                        __fmul_rn(__uint_as_float(r[4 * jj + 2]), inv), __fmul_rn(__uint_as_float(r[4 * jj + 3]), inv));
+                    fence_async_smem();
+                    __syncwarp();
+                    if (lane == 0) {
+                        asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];"
+                                     ::"l"(reinterpret_cast<uint64_t>(&out_tmap)), "r"(s_u32(tile)),
+                                       "r"(c * kUnitN + chunk * 32), "r"(x0), "r"(y0 + warp * 2) : "memory");
+                        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                    }
+                    ++nstore;
+                };
+                uint32_t ra[32], rb[32];
+                ld32(t0, ra);
+#pragma unroll 1
+                for (int ch = 0; ch < kUnitN / 32; ch += 2) {
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    ld32(t0 + (ch + 1) * 32, rb);
+                    emit(ra, ch);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    if (ch + 2 < kUnitN / 32) ld32(t0 + (ch + 2) * 32, ra);
+                    else {                              // every tcgen05.ld of this accumulator has completed
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) bar_arrive(&tmem_empty[buf]);
+                    }
+                    emit(rb, ch + 1);
+                }
+            }
+        }
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    } else if (warp == kMmaWarp) {
+        // ================================================= MMA issuer ===============================================
+        if (lane == 0) {
+            // M = 128, N = 256, fp32 accumulate, A and B tf32, A K-major, B MN-major
+            const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 16) | ((uint32_t)(kUnitN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+            const uint32_t a_hi = s_u32(w_hi), a_lo = s_u32(w_lo), st0 = s_u32(stage_base);
+            int unit = 0, wb = 0, st = 0;
+            for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
+                int x0, y0;
+                half_origin(ht, x0, y0);
+                if (y0 >= p.cam.height) continue;
+                const int U = __ldg(p.ucount + ht);
+                const int rounds = rounds_of(U);
+                for (int c = 0; c < nunits; ++c, ++unit) {
+                    const int buf = unit & 1;
+                    bar_wait(&tmem_empty[buf], ((unit >> 1) & 1) ^ 1);
+                    tc_fence_after();
+                    const uint32_t d_tmem = tmem_base + (uint32_t)(buf * kUnitN);
+                    for (int r = 0; r < rounds; ++r) {
+                        if (c == 0 || rounds > 1) { bar_wait(w_ready, wb & 1); ++wb; }
+                        const int nk = ksteps_of(cols_of(U, r));
+                        for (int j = 0; j < nk; ++j, ++st) {
+                            const int s = st % kStages;
+                            bar_wait(&full[s], (st / kStages) & 1);
+                            tc_fence_after();
+                            const uint32_t b_hi = st0 + s * kStageBytes, b_lo = b_hi + kStageHalf;
+                            const uint64_t da_hi = umma_desc(a_hi + j * 256, 128, kWCols / 4 * 128, 0);
+                            const uint64_t da_lo = umma_desc(a_lo + j * 256, 128, kWCols / 4 * 128, 0);
+                            const uint64_t db_hi = umma_desc(b_hi, 1024, 512, 1);
+                            const uint64_t db_lo = umma_desc(b_lo, 1024, 512, 1);
+                            umma_tf32(d_tmem, da_hi, db_hi, idesc, (r | j) != 0);
+                            umma_tf32(d_tmem, da_lo, db_hi, idesc, true);
+                            umma_tf32(d_tmem, da_hi, db_lo, idesc, true);
+                            umma_commit(&empty[s]);
+                        }
+                        if (rounds > 1 || c == nunits - 1) umma_commit(w_free);     // last use of this W
+                    }
+                    umma_commit(&tmem_full[buf]);
+                }
+            }
+        }
+    } else if (warp == kLoadWarp) {
+        // ================================================= loader ===================================================
+        // lane k < 8 copies union row 8 j + k of every stage: 1 KB (256 channels) per bulk copy, kRawStages ahead
+        unsigned char* raw_base = smem + MmaSmem::raw;
+        int wb = 0, st = 0;
+        for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
+            int x0, y0;
+            half_origin(ht, x0, y0);
+            if (y0 >= p.cam.height) continue;
+            const int U = __ldg(p.ucount + ht);
+            const int rounds = rounds_of(U);
+            for (int c = 0; c < nunits; ++c) {
+                for (int r = 0; r < rounds; ++r) {
+                    if (c == 0 || rounds > 1) { bar_wait(w_ready, wb & 1); ++wb; }      // uid_s of this round is written
+                    const int ncols = cols_of(U, r);
+                    const int nk = ksteps_of(ncols);
+                    for (int j = 0; j < nk; ++j, ++st) {
+                        const int s = st % kRawStages;
+                        bar_wait(&raw_empty[s], ((st / kRawStages) & 1) ^ 1);
+                        const int rows = max(0, min(kStageRows, ncols - j * kStageRows));
+                        if (lane == 0) {
+                            if (rows > 0) bar_arrive_tx(&raw_full[s], (uint32_t)rows * kRawRow);
+                            else bar_arrive(&raw_full[s]);
+                        }
+                        __syncwarp();
+                        if (lane < rows) {
+                            const int32_t id = uid_s[j * kStageRows + lane];
+                            tma_row(raw_base + s * kRawBytes + lane * kRawRow,
+                                    static_cast<const float*>(p.features) + (int64_t)id * D + c * kUnitN, kRawRow, &raw_full[s]);
+                        }
+                    }
+                }
+            }
+        }
+    } else {
+        // ================================================= producers ================================================
+        const int pw = warp - kFirstProd;                 // 0..7
+        const int ptid = tid - kFirstProd * 32;           // 0..255
+        const uint32_t lt_mask = (1u << lane) - 1u;
+        const unsigned char* raw_base = smem + MmaSmem::raw;
+        auto prod_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kProdThreads) : "memory"); };
+        int wb = 0, st = 0;
+        for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
+            int x0, y0;
+            half_origin(ht, x0, y0);
+            if (y0 >= p.cam.height) continue;
+            const int tile = ht >> 1, half = ht & 1;
+            const int U = __ldg(p.ucount + ht);
+            const int rounds = rounds_of(U);
+            for (int c = 0; c < nunits; ++c) {
+                for (int r = 0; r < rounds; ++r) {
+                    const int ncols = cols_of(U, r);
+                    if (c == 0 || rounds > 1) {
+                        // ---------------- build W for columns [64 r, 64 r + 64) ----------------
+                        // the loads of both groups of this warp are issued before anything waits on them
+                        const bool write_sel = (c == 0 && r == 0);
+                        int n_g[2];
+                        float inv_g[2];
+                        float4 wa[2], wb4[2];
+                        float2 mt[2];
+#pragma unroll
+                        for (int gg = 0; gg < 2; ++gg) {
+                            const int g = pw * 2 + gg;
+                            const int gx = g & 3, gy = g >> 2;
+                            const int64_t group = (int64_t)tile * kGroupsPerTile + half * 16 + g;
+                            n_g[gg] = __ldg(p.gcount + group);
+                            const float* recs = p.rec + group * p.cap * kRecWords;
+                            wa[gg] = wb4[gg] = make_float4(0.f, 0.f, 0.f, 0.f);
+                            mt[gg] = make_float2(__int_as_float(-1), __int_as_float(0));
+                            if (lane < p.cap) {
+                                wa[gg] = __ldg(reinterpret_cast<const float4*>(recs + (size_t)lane * kRecWords));
+                                wb4[gg] = __ldg(reinterpret_cast<const float4*>(recs + (size_t)lane * kRecWords + 4));
+                                mt[gg] = __ldg(reinterpret_cast<const float2*>(recs + (size_t)lane * kRecWords + 8));
+                            }
+                            const int qx = x0 + gx * 4 + (lane & 3), qy = y0 + gy * 2 + ((lane >> 2) & 1);
+                            inv_g[gg] = 0.0f;
+                            if (write_sel && lane < kGroupPx && qx < p.cam.width && qy < p.cam.height) {
+                                const int64_t pix = (int64_t)qy * p.cam.width + qx;
+                                if (__ldg(p.n_sel + pix) > 0) inv_g[gg] = __fdiv_rn(1.0f, __fsub_rn(1.0f, __ldg(p.resid + pix)));
+                            }
+                        }
+                        if (wb > 0) bar_wait(w_free, (wb - 1) & 1);
+                        ++wb;
+                        {
+                            const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+                            float4* wz = reinterpret_cast<float4*>(smem);
+                            for (int i = ptid; i < 2 * kWBytes / 16; i += kProdThreads) wz[i] = z;
+                        }
+                        prod_sync();
+#pragma unroll
+                        for (int gg = 0; gg < 2; ++gg) {
+                            const int g = pw * 2 + gg;                     // group 0..15 of the half tile
+                            const int gx = g & 3, gy = g >> 2;
+                            const int64_t group = (int64_t)tile * kGroupsPerTile + half * 16 + g;
+                            const int n = n_g[gg];
+                            const float* recs = p.rec + group * p.cap * kRecWords;
+                            const float inv_l = inv_g[gg];
+                            int base[kGroupPx];
+#pragma unroll
+                            for (int q = 0; q < kGroupPx; ++q) base[q] = 0;
+                            for (int i0 = 0; i0 < n; i0 += 32) {
+                                const int i = i0 + lane;
+                                const bool have = i < n;
+                                float4 a = wa[gg], b = wb4[gg];
+                                float2 m2 = mt[gg];
+                                if (i0 > 0 && have) {
+                                    a = __ldg(reinterpret_cast<const float4*>(recs + (size_t)i * kRecWords));
+                                    b = __ldg(reinterpret_cast<const float4*>(recs + (size_t)i * kRecWords + 4));
+                                    m2 = __ldg(reinterpret_cast<const float2*>(recs + (size_t)i * kRecWords + 8));
+                                }
+                                const float w[kGroupPx] = { a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w };
+                                const int32_t id = __float_as_int(m2.x);
+                                const uint32_t nzcol = have ? (uint32_t)__float_as_int(m2.y) : 0u;
+                                const uint32_t nz = nzcol & 0xFFu;
+                                const int col = (int)(nzcol >> 8);
+                                const bool mine = have && (col / kWCols) == r;
+                                const int cl = col % kWCols;
+                                if (mine) uid_s[cl] = id;
+#pragma unroll
+                                for (int q = 0; q < kGroupPx; ++q) {
+                                    const bool bit = (nz >> q) & 1u;
+                                    if (write_sel) {
+                                        const uint32_t bal = __ballot_sync(0xffffffffu, bit);
+                                        const float inv_q = __shfl_sync(0xffffffffu, inv_l, q);
+                                        if (bit) {
+                                            const int slot = base[q] + __popc(bal & lt_mask);
+                                            const int64_t pix = (int64_t)(y0 + gy * 2 + (q >> 2)) * p.cam.width + (x0 + gx * 4 + (q & 3));
+                                            p.sel_idx[pix * K + slot] = id;
+                                            p.sel_w[pix * K + slot] = __fmul_rn(w[q], inv_q);
+                                        }
+                                        base[q] += __popc(bal);
+                                    }
+                                    if (mine && bit) {
+                                        const int m = (gy * 2 + (q >> 2)) * 16 + gx * 4 + (q & 3);
+                                        const uint32_t off = w_off(m, cl);
+                                        const float hi = tf32_hi(w[q]);
+                                        *reinterpret_cast<float*>(smem + MmaSmem::w_hi + off) = hi;
+                                        *reinterpret_cast<float*>(smem + MmaSmem::w_lo + off) = __fsub_rn(w[q], hi);
+                                    }
+                                }
+                            }
+                        }
+                        fence_async_smem();
+                        prod_sync();
+                        if (ptid == 0) bar_arrive(w_ready);
+                    }
+                    // ---------------- feature rows of this round: warp pw converts row pw of every stage ----------------
+                    const int nk = ksteps_of(ncols);
+                    // byte offset of this lane's 16 bytes inside a stage half: channels 4 lane .. 4 lane + 3 (+128)
+                    const uint32_t lane_off = (uint32_t)((lane >> 3) * 1024 + (pw >> 2) * 512 + (pw & 3) * 128 +
+                                                         ((((lane & 7) >> 1) ^ (pw & 3)) * 32) + (lane & 1) * 16);
+                    for (int j = 0; j < nk; ++j, ++st) {
+                        const int sr = st % kRawStages;
+                        bar_wait(&raw_full[sr], (st / kRawStages) & 1);
+                        float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0;
+                        if (j * kStageRows + pw < ncols) {
+                            const unsigned char* rr = raw_base + sr * kRawBytes + pw * kRawRow + lane * 16;
+                            a0 = *reinterpret_cast<const float4*>(rr);
+                            a1 = *reinterpret_cast<const float4*>(rr + 512);
+                        }
+                        const float4 h0 = make_float4(tf32_hi(a0.x), tf32_hi(a0.y), tf32_hi(a0.z), tf32_hi(a0.w));
+                        const float4 h1 = make_float4(tf32_hi(a1.x), tf32_hi(a1.y), tf32_hi(a1.z), tf32_hi(a1.w));
+                        const float4 l0 = make_float4(__fsub_rn(a0.x, h0.x), __fsub_rn(a0.y, h0.y), __fsub_rn(a0.z, h0.z), __fsub_rn(a0.w, h0.w));
+                        const float4 l1 = make_float4(__fsub_rn(a1.x, h1.x), __fsub_rn(a1.y, h1.y), __fsub_rn(a1.z, h1.z), __fsub_rn(a1.w, h1.w));
+                        __syncwarp();
+                        if (lane == 0) bar_arrive(&raw_empty[sr]);          // the raw row is in registers
+                        const int s = st % kStages;
+                        bar_wait(&empty[s], ((st / kStages) & 1) ^ 1);
+                        unsigned char* hi = stage_base + s * kStageBytes + lane_off;
+                        unsigned char* lo = hi + kStageHalf;
+                        *reinterpret_cast<float4*>(hi) = h0;
+                        *reinterpret_cast<float4*>(hi + 4 * 1024) = h1;
+                        *reinterpret_cast<float4*>(lo) = l0;
+                        *reinterpret_cast<float4*>(lo + 4 * 1024) = l1;
+                        fence_async_smem();
+                        __syncwarp();
+                        if (lane == 0) bar_arrive(&full[s]);
+                    }
+                }
+            }
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
+}
+
+bool blend_mma_supported(int32_t D, qr_dtype feat_dtype) { return feat_dtype == QR_F32 && D >= kUnitN && D % kUnitN == 0; }
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_tiled_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* sym = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(sym);
+    }
+    return fn;
+}
+
+int launch_blend_mma(const BlendParams& p, cudaStream_t st)
+{
+    static int sms = 0;
+    if (sms == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+            sms = 148;
+    }
+    // out_map [H][W][D] fp32 as a 3-D tensor (D, W, H); box = 32 channels x 16 pixels x 2 rows, 128-byte swizzle
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return fail(QR_ERR_CUDA, "qr_forward: cuTensorMapEncodeTiled is not available from the driver");
+    CUtensorMap tmap;
+    const cuuint64_t dims[3] = { (cuuint64_t)p.D, (cuuint64_t)p.cam.width, (cuuint64_t)p.cam.height };
+    const cuuint64_t strides[2] = { (cuuint64_t)p.D * 4, (cuuint64_t)p.D * 4 * (cuuint64_t)p.cam.width };
+    const cuuint32_t box[3] = { 32, 16, 2 };
+    const cuuint32_t estr[3] = { 1, 1, 1 };
+    const CUresult cr = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, p.out_map, dims, strides, box, estr,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (cr != CUDA_SUCCESS) return fail(QR_ERR_CUDA, "qr_forward: cuTensorMapEncodeTiled failed (%d)", (int)cr);
+    const unsigned grid = (unsigned)min(sms, p.num_tiles * 2);
+    QR_CUDA_OK(cudaFuncSetAttribute(blend_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MmaSmem::total));
+    blend_mma_kernel<<<grid, kMmaThreads, MmaSmem::total, st>>>(p, tmap);
+    QR_LAUNCH_OK("blend_mma_kernel");
+    return QR_OK;
+}
+
+}  // namespace qr

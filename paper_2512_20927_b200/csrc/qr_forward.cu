@@ -17,22 +17,18 @@
 //   per-pixel gather, which is what makes the blend FMA bound instead of L1/shared bound.  Epilogue: scale by
 //   1/(1 - T^Q) (Algorithm 1 line 20), 128-bit streaming stores of the HWC map; the same warp writes the per-pixel
 //   selection records (sel_idx, sel_w, -1/0 padded).
-#include "qr_common.cuh"
+#include "qr_blend.cuh"
 
 namespace qr {
 
 constexpr int kWalkThreads = 256;
 constexpr int kWalkBatch = 256;
-constexpr int kGroupPx = 8;                  // 4x2 pixels
-constexpr int kGroupsPerTile = 32;
 
-// workspace layout: tile ticket, gcount[G], rec[G][cap] (G = tiles * 32 groups, cap = 8 K + kSentinels).
-// A record is 12 words (48 B, 16-byte aligned): the 8 pixels' weights w^Q, the Gaussian id, 3 words of padding.
-// Each list ends with kSentinels records of id -1 / weight 0 so that the blend pipeline can prefetch past the end.
-constexpr int kRecWords = 12;
-constexpr int kSentinels = 3;
+// workspace layout: tile ticket, gcount[G], ucount[2 T], rec[G][cap] (G = tiles * 32 groups, cap = 8 K + kSentinels).
+// Records are described in qr_blend.cuh.  Each list ends with kSentinels records of id -1 / weight 0 so that the
+// FFMA blend pipeline can prefetch past the end.
 struct FwdLayout {
-    size_t ticket, gcount, rec, total;
+    size_t ticket, gcount, ucount, rec, total;
     int64_t G;
     int cap;
 };
@@ -45,6 +41,7 @@ static FwdLayout fwd_layout(const Cam& cam, int K)
     size_t o = 0;
     L.ticket = o; o = align_up(o + 4, 256);
     L.gcount = o; o = align_up(o + (size_t)L.G * 4, 256);
+    L.ucount = o; o = align_up(o + (size_t)(L.G / 16) * 4, 256);
     L.rec = o;    o = align_up(o + (size_t)L.G * L.cap * kRecWords * 4, 256);
     L.total = o;
     return L;
@@ -62,6 +59,7 @@ struct WalkParams {
     int32_t* sel_idx;     // only the padding (slots >= n_sel) is written here
     float* sel_w;
     int32_t* gcount;
+    int32_t* ucount;      // [2 T] union size of each 16x8 half tile
     float* rec;
     int32_t* tile_ticket; // blend_kernel's tile queue, reset here
 };
@@ -75,6 +73,8 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
     int32_t* ent_id = reinterpret_cast<int32_t*>(ent_xy + kWalkBatch);    // [256]
     float* thr = reinterpret_cast<float*>(ent_id + kWalkBatch);           // [K+1]
     __shared__ int32_t nsel_s[kTile * kTile];
+    __shared__ int32_t ent_col[2][kWalkBatch];   // column of a batch entry in its half tile's union, -1 = not selected yet
+    __shared__ int32_t ucount_s[2];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x;
@@ -97,6 +97,8 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
         thr[k] = __fsub_rn(1.0f, __fdiv_rn((float)(k + 1), (float)(K + 1)));
     const float t_break = __fdiv_rn(1.0f, (float)(K + 1));
     const int2 range = p.tile_range[tile];
+    const int half = warp >> 2;                                           // rows 0..7 / 8..15 of the tile
+    if (tid < 2) ucount_s[tid] = 0;
 
     bool done = !inside;
     float T = 1.0f, TQ = 1.0f;
@@ -126,6 +128,7 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
                 box = make_float4(xy.x - ex, xy.x + ex, xy.y - ey, xy.y + ey);
             }
             ent_id[tid] = id; ent_co[tid] = co; ent_xy[tid] = xy; ent_box[tid] = box;
+            ent_col[0][tid] = -1; ent_col[1][tid] = -1;
         }
         __syncthreads();
         if (warp_done) continue;
@@ -165,15 +168,26 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
                     }
                 }
                 const uint32_t sm = __ballot_sync(0xffffffffu, sel);
-                if (sm & gbits) {                       // some pixel of my group selected this Gaussian
-                    my_rec[gcnt * kRecWords + q] = wQ;  // 8 lanes write the record's 8 weights (32 contiguous bytes)
-                    if (q == 0) {
-                        // word 8 = Gaussian id, word 9 = which of the 8 pixels selected it (bit q)
-                        const uint32_t nz = ((sm >> (4 * gx)) & 0xFu) | (((sm >> (16 + 4 * gx)) & 0xFu) << 4);
-                        *reinterpret_cast<float2*>(my_rec + gcnt * kRecWords + 8) =
-                            make_float2(__int_as_float(ent_id[e]), __int_as_float((int)nz));
+                if (sm) {
+                    // column of this Gaussian in the half tile's union: the first warp to select it numbers it
+                    int col = 0;
+                    if (lane == 0) {
+                        volatile int32_t* slot = &ent_col[half][e];
+                        const int old = atomicCAS(&ent_col[half][e], -1, -2);
+                        if (old == -1) { col = atomicAdd(&ucount_s[half], 1); *slot = col; }
+                        else { col = old; while (col == -2) col = *slot; }
                     }
-                    ++gcnt;
+                    col = __shfl_sync(0xffffffffu, col, 0);
+                    if (sm & gbits) {                       // some pixel of my group selected this Gaussian
+                        my_rec[gcnt * kRecWords + q] = wQ;  // 8 lanes write the record's 8 weights (32 contiguous bytes)
+                        if (q == 0) {
+                            // word 8 = Gaussian id, word 9 = which of the 8 pixels selected it (bit q) | column << 8
+                            const uint32_t nz = ((sm >> (4 * gx)) & 0xFu) | (((sm >> (16 + 4 * gx)) & 0xFu) << 4);
+                            *reinterpret_cast<float2*>(my_rec + gcnt * kRecWords + 8) =
+                                make_float2(__int_as_float(ent_id[e]), __int_as_float((int)(nz | ((uint32_t)col << 8))));
+                        }
+                        ++gcnt;
+                    }
                 }
             }
             if (__all_sync(0xffffffffu, done)) { warp_done = true; break; }
@@ -195,6 +209,7 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
     // words of sel_idx / sel_w.  The used slots are written by blend_kernel (it knows 1/(1 - T^Q) by then). ----
     nsel_s[warp * 32 + lane] = ns;                      // index = (2*warp + (lane>>4))*16 + (lane&15) = y_local*16 + x_local
     __syncthreads();
+    if (tid < 2) p.ucount[tile * 2 + tid] = ucount_s[tid];
     {
         const int npx = min(kTile, p.cam.width - tile_x * kTile);
         const int row_words = npx * K;
@@ -254,19 +269,6 @@ template <> __device__ __forceinline__ void store_map<8>(float* dst, const float
 constexpr int kBlendWarps = 8;
 constexpr int kBlendSlots = 64;              // ring of tiles a CTA has claimed (only ~2 are live at any time)
 
-struct BlendParams {
-    Cam cam;
-    int32_t K, D, cap, num_tiles;
-    const void* features;
-    const int32_t* gcount;
-    const float* rec;
-    const int32_t* n_sel;
-    const float* resid;
-    float* out_map;
-    int32_t* sel_idx;
-    float* sel_w;
-    int32_t* tile_ticket;
-};
 
 // Persistent CTAs (one per SM).  Work is handed out without block barriers: a warp takes a ticket from the CTA's
 // shared counter; ticket / 32 is a slot of the CTA's tile ring, ticket % 32 the pixel group inside that tile.  The
@@ -953,6 +955,7 @@ extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype f
     wp.n_sel = n_sel; wp.resid = resid_TQ; wp.sel_idx = sel_idx; wp.sel_w = sel_w;
     wp.tile_ticket = reinterpret_cast<int32_t*>(w + L.ticket);
     wp.gcount = reinterpret_cast<int32_t*>(w + L.gcount);
+    wp.ucount = reinterpret_cast<int32_t*>(w + L.ucount);
     wp.rec = reinterpret_cast<float*>(w + L.rec);
     const size_t smem = kWalkBatch * (16 + 16 + 8 + 4) + (size_t)(K + 1) * 4;
     walk_kernel<<<(unsigned)T, kWalkThreads, smem, st>>>(wp);
@@ -960,8 +963,9 @@ extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype f
 
     BlendParams bp;
     bp.cam = c; bp.K = K; bp.D = D; bp.cap = L.cap; bp.num_tiles = T; bp.tile_ticket = wp.tile_ticket;
-    bp.features = features; bp.gcount = wp.gcount; bp.rec = wp.rec;
+    bp.features = features; bp.gcount = wp.gcount; bp.ucount = wp.ucount; bp.rec = wp.rec;
     bp.n_sel = n_sel; bp.resid = resid_TQ; bp.out_map = out_map; bp.sel_idx = sel_idx; bp.sel_w = sel_w;
+    if (blend_mma_supported(D, feat_dtype)) return launch_blend_mma(bp, st);
     if (feat_dtype == QR_F16) {
         if ((D + 255) / 256 == 1) return launch_blend_tu<__half, 1, 8>(bp, st);
         return launch_blend_tu<__half, 2, 8>(bp, st);
