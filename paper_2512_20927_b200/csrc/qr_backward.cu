@@ -13,7 +13,7 @@
 //      (band union) * D -- a 25x pre-reduction at K = 40.
 // Pixel kernel (any K): one warp per pixel, vector atomics per selected row -- the plain statement, used for
 // K > kBwdMaxK.
-#include "qr_common.cuh"
+#include "qr_backward.cuh"
 
 namespace qr {
 
@@ -22,16 +22,6 @@ constexpr int kBwdPx = 64;        // 16 x 4 pixels per CTA
 constexpr int kBwdRows = 64;      // union rows per pass (8 warps x 8 rows)
 constexpr int kBwdMaxK = 64;
 
-struct BackwardParams {
-    Cam cam;
-    int32_t K, D;
-    int64_t N;
-    const int32_t* sel_idx;
-    const float* sel_w;
-    const int32_t* n_sel;
-    const float* dL_dmap;
-    float* dL_dfeat;
-};
 
 template <int VW> __device__ __forceinline__ void load_g(const float* src, float (&g)[VW]);
 template <> __device__ __forceinline__ void load_g<4>(const float* src, float (&g)[4])
@@ -292,6 +282,7 @@ extern "C" int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N
     p.cam = make_cam(cam); p.K = K; p.D = D; p.N = N;
     p.sel_idx = sel_idx; p.sel_w = sel_w; p.n_sel = n_sel; p.dL_dmap = dL_dmap; p.dL_dfeat = dL_dfeat;
     cudaStream_t st = (cudaStream_t)stream;
+    if (backward_tile_supported(K, D)) return launch_backward_tile(p, st);
     if (D % 4 == 0) {
         switch ((D + 127) / 128) {
             case 1: return launch_backward<1, 4>(p, st);
