@@ -26,16 +26,16 @@ using namespace aq;
 constexpr int kBtConsumers = 8;
 constexpr int kBtSetupWarps = 3;
 constexpr int kBtSetupThreads = kBtSetupWarps * 32;
-constexpr int kBtThreads = 384;           // warps 0..7 consumers, 8..10 setup, 11 loader
-constexpr int kBtConsumerRegs = 216;
-constexpr int kBtProducerRegs = 72;
+constexpr int kBtThreads = 384;           // warps 0..7 consumers, 8..10 setup, 11 loader; 168 registers per thread
+                                          // hold the 128 accumulators, so no setmaxnreg re-split is needed
 constexpr int kBtPx = 128;                // half tile: 16 x 8 pixels
 constexpr int kBtStagePx = 8;
 constexpr int kBtStagesPerUnit = kBtPx / kBtStagePx;   // 16
 constexpr int kBtRows = 64;               // union rows per pass
-constexpr int kBtWStride = 72;            // words per pixel of W: 4 pixels x 8 rows fall into 32 distinct banks
+constexpr int kBtSlab = kBtPx * 8;        // W[b][warp][px][8 rows]: words per consumer warp
 constexpr int kBtHash = 4096;
-constexpr int kBtMaxRec = 2800;           // records per unit (hash load <= 0.7); 8 px x QR_MAX_K = 2048 always fits
+constexpr int kBtCap = 3072;              // staged records per unit, each pixel padded to a multiple of 4
+                                          // (hash load <= 0.75); 8 px x QR_MAX_K = 2048 always fits
 
 struct BtDesc {
     int32_t ht, j0, j1, nrows, flags;     // flags: 1 = no more work
@@ -43,18 +43,21 @@ struct BtDesc {
 };
 
 struct BtSmem {
-    int ring, W, hkey, hslot, nsel, ssum, desc, bars, total;
+    int ring, W, hkey, hslot, sid, sw, spx, nsel, E, desc, bars, total;
 };
 __host__ __device__ inline BtSmem bt_smem(int D, int stages)
 {
     BtSmem L;
     int o = 0;
     L.ring = o;  o += stages * kBtStagePx * D * 4;
-    L.W = o;     o += 2 * kBtPx * kBtWStride * 4;
+    L.W = o;     o += 2 * kBtConsumers * kBtSlab * 4;
     L.hkey = o;  o += kBtHash * 4;
+    L.sid = o;   o += 2 * kBtCap * 4;
+    L.sw = o;    o += 2 * kBtCap * 4;
+    L.spx = o;   o += 2 * kBtCap;
     L.hslot = o; o += kBtHash * 2;
-    L.nsel = o;  o += kBtPx * 4;
-    L.ssum = o;  o += kBtStagesPerUnit * 4;
+    L.nsel = o;  o += 3 * kBtPx * 4;
+    L.E = o;     o += 3 * (kBtPx + 4) * 4;
     L.desc = o;  o += 2 * (int)sizeof(BtDesc);
     o = (o + 15) & ~15;
     L.bars = o;  o += (2 * stages + 4) * 8;
@@ -72,6 +75,15 @@ __device__ __forceinline__ void bt_red4(float* dst, const float2& a, const float
 {
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y) : "memory");
 }
+__device__ __forceinline__ void bt_cp16(void* dst, const void* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void bt_cp4(void* dst, const void* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(s32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void bt_cp_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 template <int NV, bool FULL>
 __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const BackwardParams p, const int stages)
@@ -99,11 +111,11 @@ __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const Back
     __syncthreads();
 
     if (warp >= kBtConsumers) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kBtProducerRegs));
         if (warp == kBtConsumers + kBtSetupWarps) {
             // ================================================ loader ================================================
             if (lane == 0) {
-                int it = 0;
+                int s = 0;
+                uint32_t ph = 1;
                 for (int unit = 0;; ++unit) {
                     const int b = unit & 1;
                     mbar_wait(&unit_full[b], (unit >> 1) & 1);
@@ -112,9 +124,8 @@ __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const Back
                     if (flags & 1) break;
                     const int tile = ht >> 1;
                     const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
-                    for (int j = j0; j < j1; ++j, ++it) {
-                        const int s = it % stages;
-                        mbar_wait(&empty[s], ((it / stages) & 1) ^ 1);
+                    for (int j = j0; j < j1; ++j) {
+                        mbar_wait(&empty[s], ph);
                         const int x = x0 + (j & 1) * kBtStagePx, y = y0 + (j >> 1);
                         const int npx = y < p.cam.height ? max(0, min(kBtStagePx, p.cam.width - x)) : 0;
                         if (npx > 0) {
@@ -124,110 +135,208 @@ __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const Back
                         } else {
                             mbar_arrive(&full[s]);
                         }
+                        if (++s == stages) { s = 0; ph ^= 1u; }
                     }
                 }
             }
         } else {
             // ================================================ setup =================================================
+            // Software pipeline over this CTA's half tiles h_0, h_1, ...: while h_i is hashed and scattered out of
+            // shared memory, the selection records of h_(i+1) and the n_sel of h_(i+2) are in flight (cp.async), so
+            // no global-load latency sits on the path that feeds the consumers.
             const int st = tid - kBtConsumers * 32;      // 0..95
             int32_t* hkey = reinterpret_cast<int32_t*>(smem + L.hkey);
             uint16_t* hslot = reinterpret_cast<uint16_t*>(smem + L.hslot);
-            int32_t* nsel_s = reinterpret_cast<int32_t*>(smem + L.nsel);
-            int32_t* ssum = reinterpret_cast<int32_t*>(smem + L.ssum);
+            int32_t* sid_all = reinterpret_cast<int32_t*>(smem + L.sid);
+            float* sw_all = reinterpret_cast<float*>(smem + L.sw);
+            uint8_t* spx_all = smem + L.spx;
+            int32_t* nsel_all = reinterpret_cast<int32_t*>(smem + L.nsel);
+            int32_t* E_all = reinterpret_cast<int32_t*>(smem + L.E);
             __shared__ int32_t ucount;
+            const bool k4 = (K & 3) == 0;
             auto ssync = [&]() { named_sync<1, kBtSetupThreads>(); };
-            int unit = 0;
-            for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
+            auto origin = [&](int ht, int& x0, int& y0) {
                 const int tile = ht >> 1;
-                const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
-                if (y0 >= p.cam.height) continue;
-                // pixel pl of the half tile: stage j = pl >> 3 covers row j >> 1, x = 8 (j & 1) .. + 7
-                auto pix_of = [&](int pl, int64_t& pix) -> bool {
-                    const int j = pl >> 3, x = x0 + (j & 1) * kBtStagePx + (pl & 7), y = y0 + (j >> 1);
-                    pix = (int64_t)y * p.cam.width + x;
-                    return x < p.cam.width && y < p.cam.height;
-                };
+                x0 = (tile % p.cam.tiles_x) * kTile;
+                y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
+            };
+            auto next_ht = [&](int ht) {                 // next half tile of this CTA that has rows inside the image
+                while (true) {
+                    ht += gridDim.x;
+                    if (ht >= num_half) return num_half;
+                    int x0, y0;
+                    origin(ht, x0, y0);
+                    if (y0 < p.cam.height) return ht;
+                }
+            };
+            // pixel pl of a half tile: stage j = pl >> 3 covers row j >> 1, x = 8 (j & 1) .. + 7
+            auto pix_of = [&](int x0, int y0, int pl, int64_t& pix) -> bool {
+                const int j = pl >> 3, x = x0 + (j & 1) * kBtStagePx + (pl & 7), y = y0 + (j >> 1);
+                pix = (int64_t)y * p.cam.width + x;
+                return x < p.cam.width && y < p.cam.height;
+            };
+            auto issue_nsel = [&](int ht, int nb) {      // n_sel of the 128 pixels -> nsel_all[nb] (async)
+                if (ht >= num_half) return;
+                int x0, y0;
+                origin(ht, x0, y0);
                 for (int pl = st; pl < kBtPx; pl += kBtSetupThreads) {
                     int64_t pix;
-                    nsel_s[pl] = pix_of(pl, pix) ? max(0, min(K, __ldg(p.n_sel + pix))) : 0;
+                    if (pix_of(x0, y0, pl, pix)) bt_cp4(&nsel_all[nb * kBtPx + pl], p.n_sel + pix);
+                    else nsel_all[nb * kBtPx + pl] = 0;
                 }
-                ssync();
-                if (st < kBtStagesPerUnit) {
-                    int t = 0;
+            };
+            auto plan = [&](int nb) {                    // clamp n_sel, E = exclusive scan of the padded counts
+                if (st < 32) {
+                    int32_t* ns = nsel_all + nb * kBtPx + st * 4;
+                    int v[4], sum = 0;
 #pragma unroll
-                    for (int q = 0; q < kBtStagePx; ++q) t += nsel_s[st * kBtStagePx + q];
-                    ssum[st] = t;
+                    for (int k = 0; k < 4; ++k) { v[k] = max(0, min(K, ns[k])); ns[k] = v[k]; sum += (v[k] + 3) & ~3; }
+                    int inc = sum;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (st >= o) inc += t; }
+                    int e = inc - sum;
+                    int32_t* E = E_all + nb * (kBtPx + 4) + st * 4;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) { E[k] = e; e += (v[k] + 3) & ~3; }
+                    if (st == 31) E_all[nb * (kBtPx + 4) + kBtPx] = e;
                 }
                 ssync();
-                int j0 = 0;
-                while (j0 < kBtStagesPerUnit) {
-                    // ---- stage range of this unit: as many stages as fit the hash set ----
-                    int tot = 0, j1 = j0;
-                    while (j1 < kBtStagesPerUnit) {
-                        const int s = ssum[j1];
-                        if (j1 > j0 && tot + s > kBtMaxRec) break;
-                        tot += s; ++j1;
-                    }
-                    if (tot == 0) { j0 = j1; continue; }             // nothing selected: no unit
-                    int hs = 64;
-                    while (hs < 2 * tot) hs <<= 1;
-                    hs = min(hs, kBtHash);
-                    const int hmask = hs - 1;
-                    for (int i = st; i < hs; i += kBtSetupThreads) hkey[i] = -1;
-                    if (st == 0) ucount = 0;
-                    ssync();
-                    // ---- insert the ids ----
-                    for (int pl = j0 * kBtStagePx + st; pl < j1 * kBtStagePx; pl += kBtSetupThreads) {
-                        const int ns = nsel_s[pl];
-                        if (ns == 0) continue;
-                        int64_t pix;
-                        pix_of(pl, pix);
-                        const int32_t* ids = p.sel_idx + pix * K;
-                        for (int s = 0; s < ns; ++s) {
-                            const int32_t id = __ldg(ids + s);
-                            uint32_t h = bt_hash((uint32_t)id) & hmask;
-                            while (true) {
-                                const int32_t old = atomicCAS(&hkey[h], -1, id);
-                                if (old == -1 || old == id) break;
-                                h = (h + 1) & hmask;
-                            }
+            };
+            auto range_end = [&](int nb, int j0) {       // as many 8-pixel stages as fit the staging buffers
+                const int32_t* E = E_all + nb * (kBtPx + 4);
+                int j1 = j0 + 1;
+                while (j1 < kBtStagesPerUnit && E[(j1 + 1) * kBtStagePx] - E[j0 * kBtStagePx] <= kBtCap) ++j1;
+                return j1;
+            };
+            auto issue_rec = [&](int ht, int nb, int sb, int j0, int j1) {   // records of stages [j0, j1) -> staging sb
+                int x0, y0;
+                origin(ht, x0, y0);
+                const int32_t* E = E_all + nb * (kBtPx + 4);
+                const int base = E[j0 * kBtStagePx];
+                int32_t* sid = sid_all + sb * kBtCap;
+                float* sw = sw_all + sb * kBtCap;
+                uint8_t* spx = spx_all + sb * kBtCap;
+                for (int pl = j0 * kBtStagePx + st; pl < j1 * kBtStagePx; pl += kBtSetupThreads) {
+                    const int ns = nsel_all[nb * kBtPx + pl];
+                    if (ns == 0) continue;
+                    int64_t pix;
+                    pix_of(x0, y0, pl, pix);
+                    const int o = E[pl] - base;
+                    const int32_t* gi = p.sel_idx + pix * K;
+                    const float* gw = p.sel_w + pix * K;
+                    if (k4) {
+                        for (int c = 0; c < ns; c += 4) {
+                            bt_cp16(sid + o + c, gi + c);
+                            bt_cp16(sw + o + c, gw + c);
+                            *reinterpret_cast<uint32_t*>(spx + o + c) = (uint32_t)pl * 0x01010101u;
+                        }
+                    } else {
+                        for (int c = 0; c < ns; ++c) {
+                            bt_cp4(sid + o + c, gi + c);
+                            bt_cp4(sw + o + c, gw + c);
+                            spx[o + c] = (uint8_t)pl;
                         }
                     }
+                }
+            };
+            auto fixup = [&](int nb, int sb, int j0, int j1) {   // padding entries of every pixel: id -1
+                const int32_t* E = E_all + nb * (kBtPx + 4);
+                const int base = E[j0 * kBtStagePx];
+                int32_t* sid = sid_all + sb * kBtCap;
+                for (int pl = j0 * kBtStagePx + st; pl < j1 * kBtStagePx; pl += kBtSetupThreads) {
+                    const int ns = nsel_all[nb * kBtPx + pl];
+                    const int o = E[pl] - base;
+                    for (int c = ns; c < ((ns + 3) & ~3); ++c) sid[o + c] = -1;
+                }
+            };
+
+            int unit = 0;
+            int ht = blockIdx.x - (int)gridDim.x;
+            ht = next_ht(ht);
+            int ht1 = ht < num_half ? next_ht(ht) : num_half;
+            // prologue: n_sel(h_0) synchronously, records(h_0) and n_sel(h_1) in flight
+            issue_nsel(ht, 0);
+            bt_cp_wait_all();
+            ssync();
+            if (ht < num_half) {
+                plan(0);
+                issue_rec(ht, 0, 0, 0, range_end(0, 0));
+                issue_nsel(ht1, 1);
+            }
+            for (int i = 0; ht < num_half; ++i) {
+                const int nb = i % 3, sb = i & 1;
+                const int32_t* E = E_all + nb * (kBtPx + 4);
+                bt_cp_wait_all();
+                ssync();                                 // records(h_i, first range) and n_sel(h_(i+1)) have landed
+                const int ht2 = ht1 < num_half ? next_ht(ht1) : num_half;
+                if (ht1 < num_half) {
+                    const int nb1 = (i + 1) % 3;
+                    plan(nb1);
+                    issue_rec(ht1, nb1, sb ^ 1, 0, range_end(nb1, 0));
+                    issue_nsel(ht2, (i + 2) % 3);
+                }
+                int j0 = 0;
+                while (j0 < kBtStagesPerUnit) {
+                    const int j1 = range_end(nb, j0);
+                    const int R = E[j1 * kBtStagePx] - E[j0 * kBtStagePx];
+                    if (R == 0) { j0 = j1; continue; }                 // nothing selected in these stages: no unit
+                    if (j0 > 0) {                                     // later range of the same half tile (rare)
+                        ssync();
+                        issue_rec(ht, nb, sb, j0, j1);
+                        bt_cp_wait_all();
+                        ssync();
+                    }
+                    fixup(nb, sb, j0, j1);
+                    int hs = 64;
+                    while (hs < 2 * R) hs <<= 1;
+                    hs = min(hs, kBtHash);
+                    const int hmask = hs - 1;
+                    {
+                        int4* hz = reinterpret_cast<int4*>(hkey);
+                        for (int k = st; k < hs / 4; k += kBtSetupThreads) hz[k] = make_int4(-1, -1, -1, -1);
+                    }
+                    if (st == 0) ucount = 0;
                     ssync();
-                    // ---- number the occupied cells ----
-                    for (int i = st; i < hs; i += kBtSetupThreads)
-                        if (hkey[i] >= 0) hslot[i] = (uint16_t)atomicAdd(&ucount, 1);
+                    const int32_t* sid = sid_all + sb * kBtCap;
+                    const float* sw = sw_all + sb * kBtCap;
+                    const uint8_t* spx = spx_all + sb * kBtCap;
+                    // ---- insert the ids; the thread that creates a cell numbers it ----
+                    for (int k = st; k < R; k += kBtSetupThreads) {
+                        const int32_t id = sid[k];
+                        if (id < 0) continue;
+                        uint32_t h = bt_hash((uint32_t)id) & hmask;
+                        while (true) {
+                            const int32_t old = atomicCAS(&hkey[h], -1, id);
+                            if (old == -1) { hslot[h] = (uint16_t)atomicAdd(&ucount, 1); break; }
+                            if (old == id) break;
+                            h = (h + 1) & hmask;
+                        }
+                    }
                     ssync();
                     const int U = ucount;
                     const int npass = (U + kBtRows - 1) / kBtRows;
                     for (int pass = 0; pass < npass; ++pass, ++unit) {
                         const int b = unit & 1;
                         mbar_wait(&unit_empty[b], ((unit >> 1) & 1) ^ 1);
-                        float* Wb = Wbuf + b * kBtPx * kBtWStride;
+                        float* Wb = Wbuf + b * kBtConsumers * kBtSlab;
                         {
-                            float4* wz = reinterpret_cast<float4*>(Wb + j0 * kBtStagePx * kBtWStride);
-                            const int n4 = (j1 - j0) * kBtStagePx * kBtWStride / 4;
-                            for (int i = st; i < n4; i += kBtSetupThreads) wz[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+                            const int n4 = (j1 - j0) * kBtStagePx * 2;           // float4 per consumer slab
+                            for (int k = st; k < n4 * kBtConsumers; k += kBtSetupThreads) {
+                                const int w = k / n4, r = k - w * n4;
+                                reinterpret_cast<float4*>(Wb + w * kBtSlab + j0 * kBtStagePx * 8)[r] = make_float4(0.f, 0.f, 0.f, 0.f);
+                            }
                         }
                         ssync();
-                        for (int pl = j0 * kBtStagePx + st; pl < j1 * kBtStagePx; pl += kBtSetupThreads) {
-                            const int ns = nsel_s[pl];
-                            if (ns == 0) continue;
-                            int64_t pix;
-                            pix_of(pl, pix);
-                            const int32_t* ids = p.sel_idx + pix * K;
-                            const float* ws = p.sel_w + pix * K;
-                            for (int s = 0; s < ns; ++s) {
-                                const int32_t id = __ldg(ids + s);
-                                const float w = __ldg(ws + s);
-                                uint32_t h = bt_hash((uint32_t)id) & hmask;
-                                while (hkey[h] != id) h = (h + 1) & hmask;
-                                const int c = (int)hslot[h] - pass * kBtRows;
-                                if (c >= 0 && c < kBtRows) {
-                                    const int col = (c & 7) * 8 + (c >> 3);      // consumer warp c % 8, its row c / 8
-                                    Wb[pl * kBtWStride + col] = w;
-                                    desc[b].uid[col] = id;
-                                }
+                        for (int k = st; k < R; k += kBtSetupThreads) {
+                            const int32_t id = sid[k];
+                            if (id < 0) continue;
+                            uint32_t h = bt_hash((uint32_t)id) & hmask;
+                            while (hkey[h] != id) h = (h + 1) & hmask;
+                            const int c = (int)hslot[h] - pass * kBtRows;
+                            if (c >= 0 && c < kBtRows) {
+                                const int cw = c & 7, r = c >> 3;                  // consumer warp c % 8, its row c / 8
+                                Wb[cw * kBtSlab + (int)spx[k] * 8 + r] = sw[k];
+                                desc[b].uid[cw * 8 + r] = id;
                             }
                         }
                         if (st == 0) {
@@ -240,7 +349,7 @@ __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const Back
                     }
                     j0 = j1;
                 }
-                ssync();                                   // nsel_s / ssum are rewritten by the next half tile
+                ht = ht1; ht1 = ht2;
             }
             {
                 const int b = unit & 1;
@@ -249,30 +358,29 @@ __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const Back
             }
         }
     } else {
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kBtConsumerRegs));
         // ================================================== consumers ===============================================
         float2 acc[8][NV][2];
 #pragma unroll
         for (int r = 0; r < 8; ++r)
 #pragma unroll
             for (int j = 0; j < NV; ++j) acc[r][j][0] = acc[r][j][1] = make_float2(0.f, 0.f);
-        int it = 0;
+        int s = 0;
+        uint32_t ph = 0;
         for (int unit = 0;; ++unit) {
             const int b = unit & 1;
             mbar_wait(&unit_full[b], (unit >> 1) & 1);
             const BtDesc* d = &desc[b];
             if (d->flags & 1) break;
             const int j0 = d->j0, j1 = d->j1, nrows = d->nrows;
-            const float* Wb = Wbuf + b * kBtPx * kBtWStride + warp * 8 + (lane & 7) + (lane >> 3) * kBtWStride;
-            for (int j = j0; j < j1; ++j, ++it) {
-                const int s = it % stages;
-                mbar_wait(&full[s], (it / stages) & 1);
+            const float* Ws = Wbuf + (b * kBtConsumers + warp) * kBtSlab;      // this warp's [px][8 rows]
+            for (int j = j0; j < j1; ++j) {
+                mbar_wait(&full[s], ph);
                 const float* gs = ring + (size_t)s * stage_floats + lane * 4;
 #pragma unroll
                 for (int hq = 0; hq < 2; ++hq) {
                     // lane = (pixel hq*4 + (lane >> 3) of the stage, row lane & 7 of this warp)
-                    const float wl = Wb[(j * kBtStagePx + hq * 4) * kBtWStride];
-                    const uint32_t m32 = __ballot_sync(0xffffffffu, wl != 0.0f);
+                    const float* Wp = Ws + (j * kBtStagePx + hq * 4) * 8;
+                    const uint32_t m32 = __ballot_sync(0xffffffffu, Wp[lane] != 0.0f);
                     if (m32 == 0u) continue;
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
@@ -285,11 +393,13 @@ __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const Back
                             if (FULL || (jj * 32 + lane) * 4 < D) g[jj] = *reinterpret_cast<const float4*>(gp + jj * 128);
                             else g[jj] = make_float4(0.f, 0.f, 0.f, 0.f);
                         }
+                        const float4 wa = *reinterpret_cast<const float4*>(Wp + q * 8);
+                        const float4 wb = *reinterpret_cast<const float4*>(Wp + q * 8 + 4);
+                        const float w8[8] = { wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w };
 #pragma unroll
                         for (int r = 0; r < 8; ++r) {
                             if (m & (1u << r)) {
-                                const float w = __shfl_sync(0xffffffffu, wl, q * 8 + r);
-                                const float2 ww = make_float2(w, w);
+                                const float2 ww = make_float2(w8[r], w8[r]);
 #pragma unroll
                                 for (int jj = 0; jj < NV; ++jj) {
                                     acc[r][jj][0] = __ffma2_rn(ww, make_float2(g[jj].x, g[jj].y), acc[r][jj][0]);
@@ -301,6 +411,7 @@ __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const Back
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty[s]);
+                if (++s == stages) { s = 0; ph ^= 1u; }
             }
             // ---- flush: one vector reduction per (union row, 4 channels) ----
 #pragma unroll
