@@ -196,9 +196,8 @@ def run_cuda(args):
         if timers is not None:
             e3.record()
             timers.append((e0, e1, e2, e3))
-        tile_bits = max(1, int(np.ceil(np.log2(max(qr.qr_num_tiles(cam), 2)))))
-        passes = (32 + tile_bits + 7) // 8
-        launches["n"] += 1 + 3 + 1 + 3 * passes + 1 + 1 + 1
+        # preprocess 1, bin_count 3, bin_sort 5 (count, scan, scatter, 2 bucket sorts), forward 2 (walk, blend), backward 1
+        launches["n"] += 1 + 3 + 5 + 2 + 1
         return fe
 
     def barrier():

@@ -1,10 +1,10 @@
-// qr_bin.cu -- tiling stage: prefix sum of tiles touched, tile-intersection duplication, stable LSD radix sort of
-// (tile, depth) keys, per-tile ranges.  PAPER.md:80 "(1) tiling strategy", :86 "ordered sequence of indices";
-// SPEC.md:139-147, :167-168; reading R6 (ascending depth, ties by ascending Gaussian index).
+// qr_bin.cu -- tiling stage: prefix sum of tiles touched, tile-intersection duplication, sort by (tile, depth, id),
+// per-tile ranges.  PAPER.md:80 "(1) tiling strategy", :86 "ordered sequence of indices"; SPEC.md:139-147, :167-168;
+// reading R6 (ascending depth, ties by ascending Gaussian index).
 //
 // Everything is integer work: depth > znear > 0, so the IEEE bit pattern of depth orders like the float.
-// All kernels are hand-written (no CUB): scan = reduce / scan-of-sums / scan-and-add; sort = per pass
-// {block digit histograms, exclusive scan of the digit-major histogram table, stable scatter}.
+// All kernels are hand-written (no CUB): scan = reduce / scan-of-sums / scan-and-add; sort = most-significant-digit
+// radix pass over the tile field (count, scan, scatter) + a shared-memory bitonic network per tile bucket.
 #include "qr_common.cuh"
 
 namespace qr {
@@ -96,181 +96,212 @@ scan_apply_kernel(const uint32_t* __restrict__ in, int64_t N, const uint64_t* __
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// duplication: one key per (Gaussian, tile of its rectangle); value = Gaussian id.  Emitted in Gaussian-id order
-// (offsets is a scan in id order), so a stable sort breaks depth ties by ascending id (R6).
-// One warp per 32 Gaussians; lanes stride over each rectangle's tiles so a screen-filling footprint does not
-// serialise on one thread.
+// Sort by (tile, depth, id) = one most-significant-digit radix pass over the tile field (a counting sort with one
+// bucket per tile: count, exclusive scan, scatter) followed by an in-shared-memory sort of every bucket on its
+// 64-bit (depth bits << 32 | Gaussian id) keys.  Those keys are unique, so the order inside a bucket does not
+// depend on the order in which the scatter filled it: ties in depth fall to the ascending id (R6) by construction,
+// and the result is bit-identical from run to run.  6 launches per frame instead of the 20 of an 8-bit LSD sort
+// over the whole 43-bit key (ncu launch list in profiles/: the LSD passes were launch-latency bound at M = 5e5).
 // ------------------------------------------------------------------------------------------------------------
+
+// One warp per 32 Gaussians; lanes stride over each rectangle's tiles so a screen-filling footprint does not
+// serialise on one thread.  SCATTER = false: count[slot] += 1.  SCATTER = true: keys[cursor[slot]++] = key.
+// A tile has kSubBuckets counters (slot = tile * kSubBuckets + Gaussian id % kSubBuckets), contiguous in the scan, so
+// a crowded tile's atomics spread over kSubBuckets L2 addresses instead of serialising on one (a same-address
+// atomic chain of ~1,500 was the whole cost of the first version of this kernel).
+constexpr int kSubBuckets = 16;
+template <bool SCATTER>
 __global__ void __launch_bounds__(256)
-duplicate_kernel(int64_t N, int32_t tiles_x, const float* __restrict__ depth, const int4* __restrict__ tile_rect,
-                 const uint64_t* __restrict__ offsets, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals)
+tile_bucket_kernel(int64_t N, int32_t tiles_x, const float* __restrict__ depth, const int4* __restrict__ tile_rect,
+                   uint32_t* __restrict__ counter, uint64_t* __restrict__ keys)
 {
     const int lane = threadIdx.x & 31;
     const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x - lane);   // first Gaussian of this warp
     int4 r = make_int4(0, 0, 0, 0);
-    uint64_t end = 0;
     uint32_t dbits = 0;
     const int64_t i = warp0 + lane;
     if (i < N) {
         r = tile_rect[i];
-        end = offsets[i];
-        dbits = __float_as_uint(depth[i]);
+        if (SCATTER) dbits = __float_as_uint(depth[i]);
     }
     const int w = r.z - r.x, h = r.w - r.y;
     const uint32_t cnt = (uint32_t)(w * h);
-    for (int src = 0; src < 32; ++src) {
+    uint32_t todo = __ballot_sync(0xffffffffu, cnt != 0u);
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
         const uint32_t c = __shfl_sync(0xffffffffu, cnt, src);
-        if (c == 0) continue;
         const int x0 = __shfl_sync(0xffffffffu, r.x, src), y0 = __shfl_sync(0xffffffffu, r.y, src);
         const int ww = __shfl_sync(0xffffffffu, w, src);
-        const uint64_t e = __shfl_sync(0xffffffffu, end, src);
         const uint32_t db = __shfl_sync(0xffffffffu, dbits, src);
-        const uint64_t start = e - c;
+        const uint64_t key = ((uint64_t)db << 32) | (uint64_t)(uint32_t)(warp0 + src);
         for (uint32_t j = lane; j < c; j += 32) {
             const int ty = y0 + (int)(j / (uint32_t)ww), tx = x0 + (int)(j % (uint32_t)ww);
-            const uint64_t tile = (uint64_t)(ty * tiles_x + tx);
-            keys[start + j] = (tile << 32) | db;
-            vals[start + j] = (uint32_t)(warp0 + src);
+            const int slot = (ty * tiles_x + tx) * kSubBuckets + (int)((uint32_t)(warp0 + src) % kSubBuckets);
+            if (SCATTER) keys[atomicAdd(&counter[slot], 1u)] = key;
+            else atomicAdd(&counter[slot], 1u);
         }
     }
 }
 
-// ------------------------------------------------------------------------------------------------------------
-// LSD radix sort, 8-bit digits.  Block = 256 threads = 8 warps; a block owns kSortChunk consecutive keys, warp w
-// owns the 512 consecutive keys [w*512, w*512+512) of it, lane l holds keys r*32 + l, r = 0..15 (coalesced).
-// ------------------------------------------------------------------------------------------------------------
-constexpr int kSortThreads = 256;
-constexpr int kSortRounds = 16;
-constexpr int kSortWarpKeys = 32 * kSortRounds;           // 512
-constexpr int kSortChunk = (kSortThreads / 32) * kSortWarpKeys;   // 4096
-
-__global__ void __launch_bounds__(kSortThreads)
-sort_hist_kernel(const uint64_t* __restrict__ keys, int64_t M, int shift, uint32_t* __restrict__ hist, int nblocks)
-{
-    __shared__ uint32_t h[256];
-    h[threadIdx.x] = 0;
-    __syncthreads();
-    const int64_t base = (int64_t)blockIdx.x * kSortChunk;
-#pragma unroll 4
-    for (int j = 0; j < kSortChunk / kSortThreads; ++j) {
-        const int64_t i = base + (int64_t)j * kSortThreads + threadIdx.x;
-        if (i < M) atomicAdd(&h[(uint32_t)(keys[i] >> shift) & 255u], 1u);
-    }
-    __syncthreads();
-    hist[(size_t)threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];   // digit-major table
-}
-
-// one block of 1024 threads: exclusive scan of the digit-major table hist[256 * nblocks] in place
+// one block of 1024 threads, thread = tile: exclusive scan of the T * kSubBuckets slot counts -> cursors in place;
+// tile_range[t] = [cursor of the tile's first slot, end of its last slot)
 __global__ void __launch_bounds__(1024)
-sort_scan_kernel(uint32_t* __restrict__ hist, int64_t n)
+tile_scan_kernel(uint32_t* __restrict__ counter, int32_t T, int32_t* __restrict__ tile_range)
 {
+    static_assert(kSubBuckets % 4 == 0, "slots are read as uint4");
     __shared__ uint32_t warp_sums[32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint32_t carry = 0;
-    for (int64_t b0 = 0; b0 < n; b0 += 1024 * 4) {
-        const int64_t i0 = b0 + (int64_t)threadIdx.x * 4;
-        uint32_t v[4], s = 0;
+    for (int32_t t0 = 0; t0 < T; t0 += 1024) {
+        const int32_t t = t0 + (int32_t)threadIdx.x;
+        uint32_t v[kSubBuckets], s = 0;
+        uint4* slots = reinterpret_cast<uint4*>(counter + (size_t)t * kSubBuckets);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) { v[j] = (i0 + j < n) ? hist[i0 + j] : 0u; s += v[j]; }
+        for (int j = 0; j < kSubBuckets / 4; ++j) {
+            const uint4 q = t < T ? slots[j] : make_uint4(0u, 0u, 0u, 0u);
+            v[4 * j] = q.x; v[4 * j + 1] = q.y; v[4 * j + 2] = q.z; v[4 * j + 3] = q.w;
+            s += q.x + q.y + q.z + q.w;
+        }
         uint32_t inc = s;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
+            const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += u;
         }
         if (lane == 31) warp_sums[warp] = inc;
         __syncthreads();
-        uint32_t wbase = 0, tot = 0;
-        for (int w = 0; w < 32; ++w) { const uint32_t x = warp_sums[w]; if (w < warp) wbase += x; tot += x; }
+        const uint32_t ws = warp_sums[lane];
+        uint32_t winc = ws;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xffffffffu, winc, o);
+            if (lane >= o) winc += u;
+        }
+        const uint32_t wbase = __shfl_sync(0xffffffffu, winc - ws, warp);
+        const uint32_t tot = __shfl_sync(0xffffffffu, winc, 31);
         __syncthreads();
         uint32_t run = carry + wbase + inc - s;
+        if (t < T) {
+            tile_range[2 * t] = (int32_t)run;
+            tile_range[2 * t + 1] = (int32_t)(run + s);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) { if (i0 + j < n) hist[i0 + j] = run; run += v[j]; }
+            for (int j = 0; j < kSubBuckets / 4; ++j) {
+                uint4 q;
+                q.x = run; run += v[4 * j];
+                q.y = run; run += v[4 * j + 1];
+                q.z = run; run += v[4 * j + 2];
+                q.w = run; run += v[4 * j + 3];
+                slots[j] = q;
+            }
+        }
         carry += tot;
     }
 }
 
-__global__ void __launch_bounds__(kSortThreads)
-sort_scatter_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in, int64_t M, int shift,
-                    const uint32_t* __restrict__ hist_scanned, int nblocks, uint64_t* __restrict__ keys_out,
-                    uint32_t* __restrict__ vals_out)
+// bitonic network over n2 (a power of two) keys in shared memory; every thread of the block takes part
+__device__ __forceinline__ void bitonic_sort_smem(uint64_t* s, int n2)
 {
-    __shared__ uint32_t wofs[kSortThreads / 32][256];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int j = threadIdx.x; j < (kSortThreads / 32) * 256; j += kSortThreads) (&wofs[0][0])[j] = 0;
-    __syncthreads();
-
-    const int64_t wbase = (int64_t)blockIdx.x * kSortChunk + (int64_t)warp * kSortWarpKeys;
-    uint64_t k[kSortRounds];
-    uint32_t v[kSortRounds];
-#pragma unroll
-    for (int r = 0; r < kSortRounds; ++r) {
-        const int64_t i = wbase + r * 32 + lane;
-        if (i < M) { k[r] = keys_in[i]; v[r] = vals_in[i]; } else { k[r] = 0; v[r] = 0; }
-    }
-    // warp-private digit histogram
-#pragma unroll
-    for (int r = 0; r < kSortRounds; ++r)
-        if (wbase + r * 32 + lane < M) atomicAdd(&wofs[warp][(uint32_t)(k[r] >> shift) & 255u], 1u);
-    __syncthreads();
-    {   // digit d = threadIdx.x: exclusive prefix over warps + this block's global base
-        const int d = threadIdx.x;
-        uint32_t run = hist_scanned[(size_t)d * nblocks + blockIdx.x];
-#pragma unroll
-        for (int w = 0; w < kSortThreads / 32; ++w) { const uint32_t c = wofs[w][d]; wofs[w][d] = run; run += c; }
-    }
-    __syncthreads();
-    // stable placement: rounds in order, lanes in order within a round
-#pragma unroll
-    for (int r = 0; r < kSortRounds; ++r) {
-        const bool valid = wbase + r * 32 + lane < M;
-        const uint32_t d = valid ? ((uint32_t)(k[r] >> shift) & 255u) : 256u + lane;   // invalid lanes match nobody
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);
-        const uint32_t rank = __popc(peers & ((1u << lane) - 1u));
-        uint32_t pos = 0;
-        if (valid) pos = wofs[warp][d] + rank;
-        __syncwarp();
-        if (valid && rank == 0) wofs[warp][d] += __popc(peers);
-        __syncwarp();
-        if (valid) { keys_out[pos] = k[r]; vals_out[pos] = v[r]; }
+    for (int k = 2; k <= n2; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int idx = threadIdx.x; idx < (n2 >> 1); idx += blockDim.x) {
+                const int i = ((idx & ~(j - 1)) << 1) | (idx & (j - 1));
+                const int l = i | j;
+                const uint64_t a = s[i], b = s[l];
+                if ((a > b) == ((i & k) == 0)) { s[i] = b; s[l] = a; }
+            }
+            __syncthreads();
+        }
     }
 }
 
-// per-tile ranges by binary search of the sorted keys: start(t) = #keys with tile id < t
-__global__ void __launch_bounds__(256)
-tile_range_kernel(const uint64_t* __restrict__ keys, int64_t M, int32_t T, int32_t* __restrict__ tile_range)
+constexpr int kSmallBucket = 2048;          // keys sorted by tile_sort_kernel<small> (16 KB of shared memory)
+constexpr int kBigBucket = 16384;           // keys per shared-memory run of tile_sort_kernel<big> (128 KB)
+constexpr uint64_t kKeyInf = ~uint64_t(0);
+
+// One CTA per tile.  BIG = false handles buckets of <= kSmallBucket keys (several CTAs per SM), BIG = true the rest:
+// up to kBigBucket keys in one shared-memory run; beyond that, runs of kBigBucket keys are sorted one by one and every
+// key is then ranked against the other runs by binary search (keys are unique, so ranks are a permutation).
+template <bool BIG>
+__device__ __forceinline__ void tile_sort_one(const int tile, const int32_t* __restrict__ tile_range,
+                                              uint64_t* __restrict__ keys, uint64_t* __restrict__ scratch,
+                                              uint32_t* __restrict__ isect_gauss, uint64_t* skeys)
 {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t > T) return;
-    const uint64_t target = (uint64_t)t << 32;
-    int64_t lo = 0, hi = M;
-    while (lo < hi) {
-        const int64_t mid = (lo + hi) >> 1;
-        if (keys[mid] < target) lo = mid + 1; else hi = mid;
+    const int start = tile_range[2 * tile], n = tile_range[2 * tile + 1] - start;
+    if (BIG ? (n <= kSmallBucket) : (n <= 0 || n > kSmallBucket)) return;
+    constexpr int kRun = BIG ? kBigBucket : kSmallBucket;
+    if (n <= kRun) {
+        int n2 = 32;
+        while (n2 < n) n2 <<= 1;
+        for (int i = threadIdx.x; i < n2; i += blockDim.x) skeys[i] = i < n ? keys[start + i] : kKeyInf;
+        __syncthreads();
+        bitonic_sort_smem(skeys, n2);
+        for (int i = threadIdx.x; i < n; i += blockDim.x) isect_gauss[start + i] = (uint32_t)skeys[i];
+        __syncthreads();
+        return;
     }
-    if (t < T) tile_range[2 * t] = (int32_t)lo;
-    if (t > 0) tile_range[2 * (t - 1) + 1] = (int32_t)lo;
+    if (BIG) {
+        const int nruns = (n + kRun - 1) / kRun;
+        for (int r = 0; r < nruns; ++r) {                        // sort each run, back into keys
+            const int r0 = r * kRun, rn = min(kRun, n - r0);
+            for (int i = threadIdx.x; i < kRun; i += blockDim.x) skeys[i] = i < rn ? keys[start + r0 + i] : kKeyInf;
+            __syncthreads();
+            bitonic_sort_smem(skeys, kRun);
+            for (int i = threadIdx.x; i < rn; i += blockDim.x) keys[start + r0 + i] = skeys[i];
+            __syncthreads();
+        }
+        __threadfence_block();
+        __syncthreads();
+        for (int i = threadIdx.x; i < n; i += blockDim.x) {      // rank = own index in its run + keys below it elsewhere
+            const uint64_t key = keys[start + i];
+            const int own = i / kRun;
+            int rank = i - own * kRun;
+            for (int r = 0; r < nruns; ++r) {
+                if (r == own) continue;
+                const uint64_t* run = keys + start + r * kRun;
+                int lo = 0, hi = min(kRun, n - r * kRun);
+                while (lo < hi) {
+                    const int mid = (lo + hi) >> 1;
+                    if (run[mid] < key) lo = mid + 1; else hi = mid;
+                }
+                rank += lo;
+            }
+            scratch[start + rank] = key;
+        }
+        __syncthreads();
+        for (int i = threadIdx.x; i < n; i += blockDim.x) isect_gauss[start + i] = (uint32_t)scratch[start + i];
+        __syncthreads();
+    }
+}
+
+// BIG = false: one CTA per tile.  BIG = true: one CTA per SM strides over the tiles (almost all of them are small
+// and skipped, and a CTA of this kernel owns 128 KB of shared memory).
+template <bool BIG>
+__global__ void __launch_bounds__(BIG ? 1024 : 256)
+tile_sort_kernel(const int32_t* __restrict__ tile_range, int32_t T, uint64_t* __restrict__ keys,
+                 uint64_t* __restrict__ scratch, uint32_t* __restrict__ isect_gauss)
+{
+    extern __shared__ __align__(16) uint64_t skeys[];
+    for (int tile = blockIdx.x; tile < T; tile += gridDim.x) tile_sort_one<BIG>(tile, tile_range, keys, scratch, isect_gauss, skeys);
 }
 
 struct BinLayout {
-    size_t keys0, keys1, vals1, hist, sums, total;
-    int nblocks_sort;
+    size_t keys, scratch, counter, sums, total;
     int64_t nblocks_scan;
 };
 
-static BinLayout bin_layout(int64_t N, int64_t M, int32_t /*T*/)
+static BinLayout bin_layout(int64_t N, int64_t M, int32_t T)
 {
     BinLayout L;
     const size_t m = (size_t)(M > 0 ? M : 1);
-    L.nblocks_sort = (int)((m + kSortChunk - 1) / kSortChunk);
+    const size_t t = (size_t)(T > 0 ? T : 1);
     L.nblocks_scan = (N + kScanChunk - 1) / kScanChunk;
     if (L.nblocks_scan < 1) L.nblocks_scan = 1;
     size_t o = 0;
-    L.keys0 = o; o = align_up(o + m * 8, 256);
-    L.keys1 = o; o = align_up(o + m * 8, 256);
-    L.vals1 = o; o = align_up(o + m * 4, 256);
-    L.hist = o;  o = align_up(o + (size_t)256 * L.nblocks_sort * 4, 256);
-    L.sums = o;  o = align_up(o + (size_t)L.nblocks_scan * 8, 256);
+    L.sums = o;    o = align_up(o + (size_t)L.nblocks_scan * 8, 256);      // first: qr_bin_count knows neither M nor T
+    L.keys = o;    o = align_up(o + m * 8, 256);
+    L.scratch = o; o = align_up(o + m * 8, 256);
+    L.counter = o; o = align_up(o + t * kSubBuckets * 4, 256);
     L.total = o;
     return L;
 }
@@ -292,9 +323,8 @@ extern "C" int qr_bin_count(int64_t N, const uint32_t* tiles_touched, uint64_t* 
     if (N == 0) { *M_host = 0; return QR_OK; }
     if (!tiles_touched || !offsets || !ws) return fail(QR_ERR_NULL_POINTER, "qr_bin_count: NULL array");
     const BinLayout L = bin_layout(N, 0, 0);
-    if (ws_bytes < L.sums + (size_t)L.nblocks_scan * 8)
-        return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_bin_count: workspace %zu < %zu bytes", ws_bytes,
-                    L.sums + (size_t)L.nblocks_scan * 8);
+    if (ws_bytes < L.keys)
+        return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_bin_count: workspace %zu < %zu bytes", ws_bytes, L.keys);
     cudaStream_t st = (cudaStream_t)stream;
     uint64_t* sums = reinterpret_cast<uint64_t*>(static_cast<char*>(ws) + L.sums);
     const unsigned nb = (unsigned)L.nblocks_scan;
@@ -334,33 +364,34 @@ extern "C" int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M, const flo
     if (ws_bytes < L.total)
         return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_bin_sort: workspace %zu < %zu bytes", ws_bytes, L.total);
     char* w = static_cast<char*>(ws);
-    uint64_t* keys[2] = { reinterpret_cast<uint64_t*>(w + L.keys0), reinterpret_cast<uint64_t*>(w + L.keys1) };
-    uint32_t* vals[2] = { isect_gauss, reinterpret_cast<uint32_t*>(w + L.vals1) };
-    uint32_t* hist = reinterpret_cast<uint32_t*>(w + L.hist);
+    uint64_t* keys = reinterpret_cast<uint64_t*>(w + L.keys);
+    uint64_t* scratch = reinterpret_cast<uint64_t*>(w + L.scratch);
+    uint32_t* counter = reinterpret_cast<uint32_t*>(w + L.counter);
+    const int4* rects = reinterpret_cast<const int4*>(tile_rect);
+    const unsigned nbg = (unsigned)((N + 255) / 256);
 
-    int tile_bits = 0;
-    while ((int64_t(1) << tile_bits) < T) ++tile_bits;
-    const int passes = (32 + tile_bits + 7) / 8;
-    int cur = (passes % 2 == 0) ? 0 : 1;   // so that the last pass writes vals[0] = isect_gauss
-
-    duplicate_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, k.tiles_x, depth,
-                                                                 reinterpret_cast<const int4*>(tile_rect), offsets,
-                                                                 keys[cur], vals[cur]);
-    QR_LAUNCH_OK("duplicate_kernel");
-    const int nb = L.nblocks_sort;
-    for (int p = 0; p < passes; ++p) {
-        const int shift = 8 * p;
-        sort_hist_kernel<<<nb, kSortThreads, 0, st>>>(keys[cur], M, shift, hist, nb);
-        QR_LAUNCH_OK("sort_hist_kernel");
-        sort_scan_kernel<<<1, 1024, 0, st>>>(hist, (int64_t)256 * nb);
-        QR_LAUNCH_OK("sort_scan_kernel");
-        sort_scatter_kernel<<<nb, kSortThreads, 0, st>>>(keys[cur], vals[cur], M, shift, hist, nb, keys[cur ^ 1],
-                                                         vals[cur ^ 1]);
-        QR_LAUNCH_OK("sort_scatter_kernel");
-        cur ^= 1;
+    static bool attr_set = false;
+    if (!attr_set) {
+        QR_CUDA_OK(cudaFuncSetAttribute(tile_sort_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        kBigBucket * (int)sizeof(uint64_t)));
+        attr_set = true;
     }
-    // cur == 0 here: sorted ids are in isect_gauss, sorted keys in keys[0]
-    tile_range_kernel<<<(unsigned)((T + 1 + 255) / 256), 256, 0, st>>>(keys[cur], M, T, tile_range);
-    QR_LAUNCH_OK("tile_range_kernel");
+    QR_CUDA_OK(cudaMemsetAsync(counter, 0, sizeof(uint32_t) * (size_t)T * kSubBuckets, st));
+    tile_bucket_kernel<false><<<nbg, 256, 0, st>>>(N, k.tiles_x, depth, rects, counter, keys);
+    QR_LAUNCH_OK("tile_bucket_kernel<count>");
+    tile_scan_kernel<<<1, 1024, 0, st>>>(counter, T, tile_range);
+    QR_LAUNCH_OK("tile_scan_kernel");
+    tile_bucket_kernel<true><<<nbg, 256, 0, st>>>(N, k.tiles_x, depth, rects, counter, keys);
+    QR_LAUNCH_OK("tile_bucket_kernel<scatter>");
+    tile_sort_kernel<false><<<(unsigned)T, 256, kSmallBucket * sizeof(uint64_t), st>>>(tile_range, T, keys, scratch, isect_gauss);
+    QR_LAUNCH_OK("tile_sort_kernel<small>");
+    static int sms = 0;
+    if (sms == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+            sms = 148;
+    }
+    tile_sort_kernel<true><<<(unsigned)min(sms, T), 1024, kBigBucket * sizeof(uint64_t), st>>>(tile_range, T, keys, scratch, isect_gauss);
+    QR_LAUNCH_OK("tile_sort_kernel<big>");
     return QR_OK;
 }

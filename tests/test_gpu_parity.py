@@ -79,6 +79,23 @@ def test_bin_sort_depth_ties_break_by_index(qr, orc):
         assert (np.diff(ids.astype(np.int64)) > 0).all()
 
 
+@pytest.mark.parametrize("N,scale", [(12000, 1.0), (60000, 3.0)])
+def test_bin_sort_crowded_tiles(qr, orc, N, scale):
+    """Tile buckets beyond one shared-memory sort: > 2,048 keys (big-bucket kernel) and > 16,384 keys (several sorted
+    runs merged by rank) in a 48x40 image; duplicated depths keep ascending index."""
+    sc = make_scene("cfg1", seed=11, N=N, W=48, H=40)
+    sc.scales *= np.float32(scale)
+    sc.means[::7, 2] = np.float32(4.0)
+    proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
+    per_tile = (rng[:, 1] - rng[:, 0]).max()
+    assert per_tile > (16384 if scale > 1 else 2048), per_tile
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    assert fe.M == len(isect)
+    np.testing.assert_array_equal(_i32(fe.tile_range), rng)
+    np.testing.assert_array_equal(_i32(fe.isect_gauss).view(np.uint32), isect)
+
+
 def test_bin_empty_scene(qr):
     """Everything culled (behind the camera): M = 0, all ranges empty, forward renders zeros."""
     sc = make_scene("cfg1", seed=0, N=50)
