@@ -282,6 +282,7 @@ extern "C" int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N
     p.cam = make_cam(cam); p.K = K; p.D = D; p.N = N;
     p.sel_idx = sel_idx; p.sel_w = sel_w; p.n_sel = n_sel; p.dL_dmap = dL_dmap; p.dL_dfeat = dL_dfeat;
     cudaStream_t st = (cudaStream_t)stream;
+    if (backward_mma_supported(K, D)) return launch_backward_mma(p, st);
     if (backward_tile_supported(K, D)) return launch_backward_tile(p, st);
     if (D % 4 == 0) {
         switch ((D + 127) / 128) {

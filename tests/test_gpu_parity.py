@@ -217,7 +217,14 @@ def test_dense_forward(qr, orc, name, kw, t_min):
                                        ("cfg1", dict(W=70, H=50, D=3, backward=True), 40),
                                        ("cfg3", dict(N=60000, W=112, H=80, D=512), 40),
                                        ("cfg3", dict(N=40000, W=96, H=64, D=132), 8),
-                                       ("cfg2", dict(N=20000, W=64, H=64, D=64), 100)])     # K > 64: pixel kernel
+                                       ("cfg2", dict(N=20000, W=64, H=64, D=64), 100),
+                                       # tcgen05 path (D % 128 == 0): ragged image, unions > 64 rows (passes),
+                                       # K large enough to split a half tile into several stage ranges
+                                       ("cfg1", dict(W=70, H=50, D=128, backward=True), 40),
+                                       ("cfg2", dict(N=20000, W=100, H=72, D=256), 40),
+                                       ("cfg3", dict(N=60000, W=96, H=64, D=384), 10),
+                                       ("cfg3", dict(N=40000, W=64, H=48, D=128), 200),
+                                       ("cfg2", dict(N=30000, W=64, H=40, D=128), 256)])
 def test_backward_stage_isolated(qr, orc, name, kw, K):
     sc = make_scene(name, seed=9, **kw)
     proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
