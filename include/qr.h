@@ -131,6 +131,8 @@ int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype,
  *   in : sel_idx, sel_w, n_sel (from qr_forward), dL_dmap[H,W,D] fp32
  *   out: dL_dfeat[N,D] fp32, ACCUMULATED INTO (the caller zeroes it; rows never selected are left untouched).
  * Summation order over pixels is not fixed (fp32 atomics): results agree to rounding, not bit for bit.
+ * ws must hold qr_backward_workspace_bytes(cam, K, D) bytes (0 for some shapes; then ws may be NULL).  Its contents
+ * are scratch: per half tile, the numbered union of selected Gaussians and the selection as (weight, row, pixel).
  */
 size_t qr_backward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D);
 int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N,

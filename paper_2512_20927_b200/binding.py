@@ -261,10 +261,12 @@ def qr_backward(cam, N: int, sel_idx, sel_w, n_sel, dL_dmap, dL_dfeat: Optional[
     D = int(dL_dmap.shape[-1])
     if dL_dfeat is None:
         dL_dfeat = torch.zeros((int(N), D), dtype=torch.float32, device=dL_dmap.device)
+    nws = int(load().qr_backward_workspace_bytes(C.byref(c), K, D))
+    ws = torch.empty((max(nws, 16),), dtype=torch.uint8, device=dL_dmap.device)
     _check(load().qr_backward(C.byref(c), K, D, int(N), _dev(sel_idx, torch.int32, "sel_idx"),
                               _dev(sel_w, torch.float32, "sel_w"), _dev(n_sel, torch.int32, "n_sel"),
                               _dev(dL_dmap, torch.float32, "dL_dmap"), _dev(dL_dfeat, torch.float32, "dL_dfeat"),
-                              None, 0, _stream()))
+                              ws.data_ptr(), ws.numel(), _stream()))
     return dL_dfeat
 
 

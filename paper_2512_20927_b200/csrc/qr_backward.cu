@@ -257,8 +257,8 @@ static int launch_backward(const BackwardParams& p, cudaStream_t st)
 
 extern "C" size_t qr_backward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D)
 {
-    (void)cam; (void)K; (void)D;
-    return 0;
+    if (!cam || cam->width < 1 || cam->height < 1) return 0;
+    return qr::backward_mma_supported(K, D) ? qr::backward_mma_workspace_bytes(qr::make_cam(cam)) : 0;
 }
 
 extern "C" int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N, const int32_t* sel_idx,
@@ -266,7 +266,6 @@ extern "C" int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N
                            size_t ws_bytes, void* stream)
 {
     using namespace qr;
-    (void)ws; (void)ws_bytes;
     if (int rc = check_cam(cam)) return rc;
     if (K < 1) return fail(QR_ERR_INVALID_ARG, "qr_backward: K = %d < 1", K);
     if (K > QR_MAX_K) return fail(QR_ERR_UNSUPPORTED, "qr_backward: K = %d > QR_MAX_K", K);
@@ -282,7 +281,7 @@ extern "C" int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N
     p.cam = make_cam(cam); p.K = K; p.D = D; p.N = N;
     p.sel_idx = sel_idx; p.sel_w = sel_w; p.n_sel = n_sel; p.dL_dmap = dL_dmap; p.dL_dfeat = dL_dfeat;
     cudaStream_t st = (cudaStream_t)stream;
-    if (backward_mma_supported(K, D)) return launch_backward_mma(p, st);
+    if (backward_mma_supported(K, D)) return launch_backward_mma(p, ws, ws_bytes, st);
     if (backward_tile_supported(K, D)) return launch_backward_tile(p, st);
     if (D % 4 == 0) {
         switch ((D + 127) / 128) {

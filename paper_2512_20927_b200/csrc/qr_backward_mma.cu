@@ -53,35 +53,30 @@ constexpr int kBmStagesPerUnit = kBmPx / kBmStagePx;   // 16
 constexpr int kBmRows = 64;                // union rows per pass = MMA N
 constexpr int kBmHalfPx = 64;              // pixels per W half buffer
 constexpr int kBmWHalfBytes = kBmRows * kBmHalfPx * 4;           // 16 KB (hi or lo of one half)
-constexpr int kBmHash = 4096;
-constexpr int kBmCap = 2048;               // staged records per unit (each pixel padded to a multiple of 4);
-                                           // 8 px x QR_MAX_K always fits
+constexpr int kBmHash = 4096;              // backward_prep_kernel: hash cells per half tile
+constexpr int kBmEntCap = 3072;            // selection records (and distinct Gaussians) of a half tile the tcgen05 path
+                                           // takes; fuller half tiles are left to backward_tile_kernel
+constexpr int kBmEntRegs = 8;              // entries a setup thread holds in flight
+constexpr int kBmLoStages = 2;             // G_lo is produced just ahead of the MMA that reads it
 constexpr int kBmDescRing = 4;
 
 struct BmDesc {
-    int32_t ht, j0, j1, nrows, flags;      // flags: 1 = no more work
-    int32_t uid[kBmRows];                  // union row (MMA column) -> Gaussian id
+    int32_t ht, j0, j1, nrows, flags, pad; // flags: 1 = no more work
+    int64_t row[kBmRows];                  // union row (MMA column) -> offset of the Gaussian's row in dL_dfeat (floats)
 };
 
 struct BmSmem {
-    int W, stages, hkey, hslot, sid, sw, spx, nsel, E, desc, bars, misc, total;
+    int W, stages, desc, bars, misc, total;
 };
 __host__ __device__ inline BmSmem bm_smem(int D, int stages)
 {
     BmSmem L;
     int o = 0;
     L.W = o;      o += 2 * 2 * kBmWHalfBytes;                    // [half][hi, lo]
-    L.stages = o; o += stages * 2 * kBmStagePx * D * 4;          // [stage][hi, lo], 1 KB aligned
-    L.hkey = o;   o += kBmHash * 4;
-    L.sid = o;    o += 2 * kBmCap * 4;
-    L.sw = o;     o += 2 * kBmCap * 4;
-    L.hslot = o;  o += kBmHash * 2;
-    L.spx = o;    o += 2 * kBmCap;
-    L.nsel = o;   o += 3 * kBmPx * 4;
-    L.E = o;      o += 3 * (kBmPx + 4) * 4;
+    L.stages = o; o += (stages + kBmLoStages) * kBmStagePx * D * 4;   // [stages] G (= G_hi), then [kBmLoStages] G_lo; 1 KB aligned
     L.desc = o;   o += kBmDescRing * (int)sizeof(BmDesc);
     o = (o + 15) & ~15;
-    L.bars = o;   o += (3 * stages + 8) * 8;
+    L.bars = o;   o += (2 * stages + 2 * kBmLoStages + 8) * 8;
     L.misc = o;   o += 16;                                       // TMEM base, done flag
     L.total = (o + 15) & ~15;
     return L;
@@ -140,18 +135,20 @@ __global__ void __launch_bounds__(kBmThreads, 1)
 backward_mma_kernel(const BackwardParams p, const int stages, const __grid_constant__ CUtensorMap g_tmap)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
-    const int D = p.D, K = p.K;
+    const int D = p.D;
     const BmSmem L = bm_smem(D, stages);
     const int nchunks = D >> 7;                      // 128-channel MMA tiles
     const int stage_half = kBmStagePx * D * 4;       // bytes of a stage's hi (or lo) part
     unsigned char* Wsm = smem + L.W;
-    unsigned char* stage_base = smem + L.stages;
+    unsigned char* stage_base = smem + L.stages;                          // G stages (the MMA reads them as G_hi)
+    unsigned char* lo_base = stage_base + (size_t)stages * stage_half;    // G_lo stages
     BmDesc* desc = reinterpret_cast<BmDesc*>(smem + L.desc);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
     uint64_t* raw_full = bars;                       // [stages] loader (TMA complete_tx) -> converters
-    uint64_t* conv_done = raw_full + stages;         // [stages] converters (4 warp arrivals) -> MMA
-    uint64_t* stage_empty = conv_done + stages;      // [stages] MMA (tcgen05.commit) -> loader
-    uint64_t* w_ready = stage_empty + stages;        // [2] setup -> MMA, loader (half 0 also publishes the descriptor)
+    uint64_t* stage_empty = raw_full + stages;       // [stages] MMA (tcgen05.commit) -> loader
+    uint64_t* lo_ready = stage_empty + stages;       // [kBmLoStages] converters (4 warp arrivals) -> MMA
+    uint64_t* lo_empty = lo_ready + kBmLoStages;     // [kBmLoStages] MMA (tcgen05.commit) -> converters
+    uint64_t* w_ready = lo_empty + kBmLoStages;      // [2] setup -> MMA, loader (half 0 also publishes the descriptor)
     uint64_t* w_free = w_ready + 2;                  // [2] MMA (tcgen05.commit) -> setup
     uint64_t* tmem_full = w_free + 2;                // [2] MMA (tcgen05.commit) -> epilogue
     uint64_t* tmem_empty = tmem_full + 2;            // [2] epilogue (4 warp arrivals) -> MMA
@@ -162,7 +159,8 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
 
     if (tid == 0) {
-        for (int s = 0; s < stages; ++s) { mbar_init(&raw_full[s], 1); mbar_init(&conv_done[s], kBmConvWarps); mbar_init(&stage_empty[s], 1); }
+        for (int s = 0; s < stages; ++s) { mbar_init(&raw_full[s], 1); mbar_init(&stage_empty[s], 1); }
+        for (int s = 0; s < kBmLoStages; ++s) { mbar_init(&lo_ready[s], kBmConvWarps); mbar_init(&lo_empty[s], 1); }
         for (int b = 0; b < 2; ++b) {
             mbar_init(&w_ready[b], 1); mbar_init(&w_free[b], 1);
             mbar_init(&tmem_full[b], 1); mbar_init(&tmem_empty[b], kBmEpiWarps);
@@ -199,6 +197,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
             const int nrows = d->nrows;
             const uint32_t t0 = tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(buf * 256);
             float* dcol = p.dL_dfeat + warp * 32 + lane;
+            const int64_t* row = d->row;
             for (int m = 0; m < nchunks; ++m) {
                 uint32_t ra[32], rb[32];
                 ld32(t0 + m * kBmRows, ra);
@@ -209,13 +208,22 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&tmem_empty[buf]);
                 }
+                float* dm = dcol + m * 128;
 #pragma unroll
-                for (int c = 0; c < 32; ++c)
-                    if (c < nrows) bm_red(dcol + (int64_t)d->uid[c] * D + m * 128, __uint_as_float(ra[c]));
-                if (nrows > 32) {
+                for (int c0 = 0; c0 < 32; c0 += 8) {
+                    if (c0 < nrows) {                   // warp-uniform: whole groups of 8 rows are skipped
 #pragma unroll
-                    for (int c = 0; c < 32; ++c)
-                        if (32 + c < nrows) bm_red(dcol + (int64_t)d->uid[32 + c] * D + m * 128, __uint_as_float(rb[c]));
+                        for (int c = c0; c < c0 + 8; ++c)
+                            if (c < nrows) bm_red(dm + row[c], __uint_as_float(ra[c]));
+                    }
+                }
+#pragma unroll
+                for (int c0 = 0; c0 < 32; c0 += 8) {
+                    if (32 + c0 < nrows) {
+#pragma unroll
+                        for (int c = c0; c < c0 + 8; ++c)
+                            if (32 + c < nrows) bm_red(dm + row[32 + c], __uint_as_float(rb[c]));
+                    }
                 }
             }
         }
@@ -224,7 +232,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
         if (lane == 0) {
             // M = 128 channels, N = 64 rows, fp32 accumulate, A and B tf32, A MN-major, B K-major
             const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | ((uint32_t)(kBmRows >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-            const uint32_t w0 = s32(Wsm), st0 = s32(stage_base);
+            const uint32_t w0 = s32(Wsm), st0 = s32(stage_base), lo0 = s32(lo_base);
             int st = 0;
             for (int unit = 0;; ++unit) {
                 const int buf = unit & 1;
@@ -238,10 +246,10 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                 for (int j = j0; j < j1; ++j, ++st) {
                     const int h = j >> 3;
                     if (h == 1 && !have_w1) { mbar_wait(&w_ready[1], unit & 1); have_w1 = true; }
-                    const int s = st % stages;
-                    mbar_wait(&conv_done[s], (st / stages) & 1);
+                    const int s = st % stages, l = st % kBmLoStages;
+                    mbar_wait(&lo_ready[l], (st / kBmLoStages) & 1);      // implies raw_full[s]
                     bm_fence_after();
-                    const uint32_t a_hi = st0 + s * 2 * stage_half, a_lo = a_hi + stage_half;
+                    const uint32_t a_hi = st0 + s * stage_half, a_lo = lo0 + l * stage_half;
                     const uint32_t b_hi = w0 + h * 2 * kBmWHalfBytes + (j & 7) * 256, b_lo = b_hi + kBmWHalfBytes;
                     const uint64_t db_hi = bm_desc(b_hi, 128, kBmHalfPx / 4 * 128, 0);
                     const uint64_t db_lo = bm_desc(b_lo, 128, kBmHalfPx / 4 * 128, 0);
@@ -254,6 +262,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                         bm_mma(d_tmem, da_lo, db_hi, idesc, true);
                     }
                     bm_commit(&stage_empty[s]);
+                    bm_commit(&lo_empty[l]);
                     if (h == 0 && (j == 7 || j == j1 - 1)) bm_commit(&w_free[0]);     // last read of W half 0
                 }
                 if (!have_w1) mbar_wait(&w_ready[1], unit & 1);       // keep the phases of every unit in step
@@ -284,247 +293,105 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                 if (lane == 0) mbar_arrive_expect_tx(&raw_full[s], (uint32_t)stage_half);
                 __syncwarp();
                 if (lane < (D >> 5))
-                    bm_tma_box(stage_base + (size_t)s * 2 * stage_half + lane * 1024, &g_tmap, lane * 32,
+                    bm_tma_box(stage_base + (size_t)s * stage_half + lane * 1024, &g_tmap, lane * 32,
                                x0 + (j & 1) * kBmStagePx, y0 + (j >> 1), &raw_full[s]);
             }
         }
     } else if (warp < kBmFirstSetup) {
         // ================================================= converters ===============================================
         const int ct = tid - kBmFirstConv * 32;              // 0..127
-        const int n4 = stage_half >> 4;                      // float4 per stage half
+        const int n4 = stage_half >> 4;                      // float4 per stage
         for (int st = 0;; ++st) {
-            const int s = st % stages;
+            const int s = st % stages, l = st % kBmLoStages;
             mbar_wait(&raw_full[s], (st / stages) & 1);
             if (*done_flag) break;
-            const float4* hi = reinterpret_cast<const float4*>(stage_base + (size_t)s * 2 * stage_half);
-            float4* lo = reinterpret_cast<float4*>(stage_base + (size_t)s * 2 * stage_half + stage_half);
-#pragma unroll 4
-            for (int i = ct; i < n4; i += kBmConvWarps * 32) {
-                const float4 v = hi[i];
-                lo[i] = make_float4(__fsub_rn(v.x, bm_hi(v.x)), __fsub_rn(v.y, bm_hi(v.y)), __fsub_rn(v.z, bm_hi(v.z)),
-                                    __fsub_rn(v.w, bm_hi(v.w)));
+            mbar_wait(&lo_empty[l], ((st / kBmLoStages) & 1) ^ 1);       // the MMAs that read this G_lo buffer have retired
+            const float4* hi = reinterpret_cast<const float4*>(stage_base + (size_t)s * stage_half);
+            float4* lo = reinterpret_cast<float4*>(lo_base + (size_t)l * stage_half);
+            for (int i0 = ct; i0 < n4; i0 += 4 * kBmConvWarps * 32) {     // n4 is a multiple of 256 (D % 128 == 0)
+                float4 v[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    v[u] = (i0 + u * kBmConvWarps * 32 < n4) ? hi[i0 + u * kBmConvWarps * 32] : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (i0 + u * kBmConvWarps * 32 < n4)
+                        lo[i0 + u * kBmConvWarps * 32] = make_float4(__fsub_rn(v[u].x, bm_hi(v[u].x)), __fsub_rn(v[u].y, bm_hi(v[u].y)),
+                                                                    __fsub_rn(v[u].z, bm_hi(v[u].z)), __fsub_rn(v[u].w, bm_hi(v[u].w)));
             }
             fence_async_smem();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&conv_done[s]);
+            if (lane == 0) mbar_arrive(&lo_ready[l]);
         }
     } else {
         // ================================================= setup ====================================================
-        // Software pipeline over this CTA's half tiles h_0, h_1, ...: while h_i is hashed and scattered out of shared
-        // memory, the selection records of h_(i+1) and the n_sel of h_(i+2) are in flight (cp.async), so no
-        // global-load latency sits on the path that feeds the MMAs.
+        // backward_prep_kernel has numbered every half tile's selected Gaussians and left its selection as a compact
+        // list of (weight, union row, pixel) entries ordered by pixel.  What remains here is streaming: read the next
+        // unit's entries (one coalesced 8-byte load each, issued before the wait on the W half they go to), clear the
+        // half, scatter hi / lo, publish.
         const int st = tid - kBmFirstSetup * 32;          // 0..127
-        int32_t* hkey = reinterpret_cast<int32_t*>(smem + L.hkey);
-        uint16_t* hslot = reinterpret_cast<uint16_t*>(smem + L.hslot);
-        int32_t* sid_all = reinterpret_cast<int32_t*>(smem + L.sid);
-        float* sw_all = reinterpret_cast<float*>(smem + L.sw);
-        uint8_t* spx_all = smem + L.spx;
-        int32_t* nsel_all = reinterpret_cast<int32_t*>(smem + L.nsel);
-        int32_t* E_all = reinterpret_cast<int32_t*>(smem + L.E);
-        __shared__ int32_t ucount;
-        const bool k4 = (K & 3) == 0;
-        auto ssync = [&]() { named_sync<1, kBmSetupThreads>(); };
-        auto origin = [&](int ht, int& x0, int& y0) {
-            const int tile = ht >> 1;
-            x0 = (tile % p.cam.tiles_x) * kTile;
-            y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
-        };
-        auto next_ht = [&](int ht) {                      // next half tile of this CTA that has rows inside the image
-            while (true) {
-                ht += gridDim.x;
-                if (ht >= num_half) return num_half;
-                int x0, y0;
-                origin(ht, x0, y0);
-                if (y0 < p.cam.height) return ht;
-            }
-        };
-        // pixel pl of a half tile: stage j = pl >> 3 covers row j >> 1, x = 8 (j & 1) .. + 7
-        auto pix_of = [&](int x0, int y0, int pl, int64_t& pix) -> bool {
-            const int j = pl >> 3, x = x0 + (j & 1) * kBmStagePx + (pl & 7), y = y0 + (j >> 1);
-            pix = (int64_t)y * p.cam.width + x;
-            return x < p.cam.width && y < p.cam.height;
-        };
-        auto issue_nsel = [&](int ht, int nb) {           // n_sel of the 128 pixels -> nsel_all[nb] (async)
-            if (ht >= num_half) return;
-            int x0, y0;
-            origin(ht, x0, y0);
-            for (int pl = st; pl < kBmPx; pl += kBmSetupThreads) {
-                int64_t pix;
-                if (pix_of(x0, y0, pl, pix)) bm_cp4(&nsel_all[nb * kBmPx + pl], p.n_sel + pix);
-                else nsel_all[nb * kBmPx + pl] = 0;
-            }
-        };
-        auto plan = [&](int nb) {                         // clamp n_sel, E = exclusive scan of the padded counts
-            if (st < 32) {
-                int32_t* ns = nsel_all + nb * kBmPx + st * 4;
-                int v[4], sum = 0;
-#pragma unroll
-                for (int k = 0; k < 4; ++k) { v[k] = max(0, min(K, ns[k])); ns[k] = v[k]; sum += (v[k] + 3) & ~3; }
-                int inc = sum;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (st >= o) inc += t; }
-                int e = inc - sum;
-                int32_t* E = E_all + nb * (kBmPx + 4) + st * 4;
-#pragma unroll
-                for (int k = 0; k < 4; ++k) { E[k] = e; e += (v[k] + 3) & ~3; }
-                if (st == 31) E_all[nb * (kBmPx + 4) + kBmPx] = e;
-            }
-            ssync();
-        };
-        auto range_end = [&](int nb, int j0) {            // as many 8-pixel stages as fit the staging buffers
-            const int32_t* E = E_all + nb * (kBmPx + 4);
-            int j1 = j0 + 1;
-            while (j1 < kBmStagesPerUnit && E[(j1 + 1) * kBmStagePx] - E[j0 * kBmStagePx] <= kBmCap) ++j1;
-            return j1;
-        };
-        auto issue_rec = [&](int ht, int nb, int sb, int j0, int j1) {   // records of stages [j0, j1) -> staging sb
-            int x0, y0;
-            origin(ht, x0, y0);
-            const int32_t* E = E_all + nb * (kBmPx + 4);
-            const int base = E[j0 * kBmStagePx];
-            int32_t* sid = sid_all + sb * kBmCap;
-            float* sw = sw_all + sb * kBmCap;
-            uint8_t* spx = spx_all + sb * kBmCap;
-            for (int pl = j0 * kBmStagePx + st; pl < j1 * kBmStagePx; pl += kBmSetupThreads) {
-                const int ns = nsel_all[nb * kBmPx + pl];
-                if (ns == 0) continue;
-                int64_t pix;
-                pix_of(x0, y0, pl, pix);
-                const int o = E[pl] - base;
-                const int32_t* gi = p.sel_idx + pix * K;
-                const float* gw = p.sel_w + pix * K;
-                if (k4) {
-                    for (int c = 0; c < ns; c += 4) {
-                        bm_cp16(sid + o + c, gi + c);
-                        bm_cp16(sw + o + c, gw + c);
-                        *reinterpret_cast<uint32_t*>(spx + o + c) = (uint32_t)pl * 0x01010101u;
-                    }
-                } else {
-                    for (int c = 0; c < ns; ++c) {
-                        bm_cp4(sid + o + c, gi + c);
-                        bm_cp4(sw + o + c, gw + c);
-                        spx[o + c] = (uint8_t)pl;
-                    }
-                }
-            }
-        };
-        auto fixup = [&](int nb, int sb, int j0, int j1) {   // padding entries of every pixel: id -1
-            const int32_t* E = E_all + nb * (kBmPx + 4);
-            const int base = E[j0 * kBmStagePx];
-            int32_t* sid = sid_all + sb * kBmCap;
-            for (int pl = j0 * kBmStagePx + st; pl < j1 * kBmStagePx; pl += kBmSetupThreads) {
-                const int ns = nsel_all[nb * kBmPx + pl];
-                const int o = E[pl] - base;
-                for (int c = ns; c < ((ns + 3) & ~3); ++c) sid[o + c] = -1;
-            }
-        };
-
+        auto ssync_setup = [&]() { named_sync<1, kBmSetupThreads>(); };
         int unit = 0;
-        int ht = blockIdx.x - (int)gridDim.x;
-        ht = next_ht(ht);
-        int ht1 = ht < num_half ? next_ht(ht) : num_half;
-        // prologue: n_sel(h_0) synchronously, records(h_0) and n_sel(h_1) in flight
-        issue_nsel(ht, 0);
-        bm_cp_wait_all();
-        ssync();
-        if (ht < num_half) {
-            plan(0);
-            issue_rec(ht, 0, 0, 0, range_end(0, 0));
-            issue_nsel(ht1, 1);
-        }
-        for (int i = 0; ht < num_half; ++i) {
-            const int nb = i % 3, sb = i & 1;
-            const int32_t* E = E_all + nb * (kBmPx + 4);
-            bm_cp_wait_all();
-            ssync();                                      // records(h_i, first range) and n_sel(h_(i+1)) have landed
-            const int ht2 = ht1 < num_half ? next_ht(ht1) : num_half;
-            if (ht1 < num_half) {
-                const int nb1 = (i + 1) % 3;
-                plan(nb1);
-                issue_rec(ht1, nb1, sb ^ 1, 0, range_end(nb1, 0));
-                issue_nsel(ht2, (i + 2) % 3);
-            }
-            int j0 = 0;
-            while (j0 < kBmStagesPerUnit) {
-                const int j1 = range_end(nb, j0);
-                const int base = E[j0 * kBmStagePx];
-                const int R = E[j1 * kBmStagePx] - base;
-                if (R == 0) { j0 = j1; continue; }                  // nothing selected in these stages: no unit
-                if (j0 > 0) {                                      // later range of the same half tile (rare)
-                    ssync();
-                    issue_rec(ht, nb, sb, j0, j1);
-                    bm_cp_wait_all();
-                    ssync();
-                }
-                fixup(nb, sb, j0, j1);
-                int hs = 64;
-                while (hs < 2 * R) hs <<= 1;
-                hs = min(hs, kBmHash);
-                const int hmask = hs - 1;
-                {
-                    int4* hz = reinterpret_cast<int4*>(hkey);
-                    for (int k = st; k < hs / 4; k += kBmSetupThreads) hz[k] = make_int4(-1, -1, -1, -1);
-                }
-                if (st == 0) ucount = 0;
-                ssync();
-                const int32_t* sid = sid_all + sb * kBmCap;
-                const float* sw = sw_all + sb * kBmCap;
-                const uint8_t* spx = spx_all + sb * kBmCap;
-                // ---- insert the ids; the thread that creates a cell numbers it ----
-                for (int k = st; k < R; k += kBmSetupThreads) {
-                    const int32_t id = sid[k];
-                    if (id < 0) continue;
-                    uint32_t h = bm_hash((uint32_t)id) & hmask;
-                    while (true) {
-                        const int32_t old = atomicCAS(&hkey[h], -1, id);
-                        if (old == -1) { hslot[h] = (uint16_t)atomicAdd(&ucount, 1); break; }
-                        if (old == id) break;
-                        h = (h + 1) & hmask;
-                    }
-                }
-                ssync();
-                const int U = ucount;
+        auto inside = [&](int ht) {
+            const int tile = ht >> 1;
+            return (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8 < p.cam.height;
+        };
+        int ht = blockIdx.x;
+        int4 cnt = make_int4(0, 0, 0, 0);
+        if (ht < num_half && inside(ht)) cnt = __ldg(reinterpret_cast<const int4*>(p.prep_cnt) + ht);
+        while (ht < num_half) {
+            const int ht1 = ht + (int)gridDim.x;
+            int4 cnt1 = make_int4(0, 0, 0, 0);
+            if (ht1 < num_half && inside(ht1)) cnt1 = __ldg(reinterpret_cast<const int4*>(p.prep_cnt) + ht1);
+            const int R0 = cnt.x, R = cnt.y, U = cnt.z;
+            if (R > 0 && cnt.w == 0) {                    // cnt.w: left to backward_tile_kernel (too many records)
+                const uint2* ent = p.prep_ent + (size_t)ht * kBmEntCap;
+                const int32_t* uid = p.prep_uid + (size_t)ht * kBmEntCap;
                 const int npass = (U + kBmRows - 1) / kBmRows;
-                // records of W half h: pixels [max(8 j0, 64 h), min(8 j1, 64 h + 64))
-                int kb[3];
-                kb[0] = 0;
-                kb[1] = E[min(max(kBmHalfPx, j0 * kBmStagePx), j1 * kBmStagePx)] - base;
-                kb[2] = R;
                 for (int pass = 0; pass < npass; ++pass, ++unit) {
                     BmDesc* d = &desc[unit % kBmDescRing];
+                    const int c_lo = pass * kBmRows;
                     for (int h = 0; h < 2; ++h) {
-                        mbar_wait(&w_free[h], (unit & 1) ^ 1);      // the MMAs of the previous unit have read this half
-                        float4* wz = reinterpret_cast<float4*>(Wsm + h * 2 * kBmWHalfBytes);
-                        for (int k = st; k < 2 * kBmWHalfBytes / 16; k += kBmSetupThreads) wz[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-                        ssync();
+                        const int kb = h ? R0 : 0, n = (h ? R : R0) - kb;
                         unsigned char* whi = Wsm + h * 2 * kBmWHalfBytes;
-                        for (int k = kb[h] + st; k < kb[h + 1]; k += kBmSetupThreads) {
-                            const int32_t id = sid[k];
-                            if (id < 0) continue;
-                            uint32_t hh = bm_hash((uint32_t)id) & hmask;
-                            while (hkey[hh] != id) hh = (hh + 1) & hmask;
-                            const int c = (int)hslot[hh] - pass * kBmRows;
-                            if (c >= 0 && c < kBmRows) {
-                                const uint32_t off = bm_w_off(c, (int)spx[k] & (kBmHalfPx - 1));
-                                const float w = sw[k], hi = bm_hi(w);
-                                *reinterpret_cast<float*>(whi + off) = hi;
-                                *reinterpret_cast<float*>(whi + kBmWHalfBytes + off) = __fsub_rn(w, hi);
-                                d->uid[c] = id;
+                        uint2 e[kBmEntRegs];
+                        int64_t rowoff = 0;
+                        for (int base = 0; base == 0 || base < n; base += kBmEntRegs * kBmSetupThreads) {
+#pragma unroll
+                            for (int u = 0; u < kBmEntRegs; ++u) {
+                                const int k = base + u * kBmSetupThreads + st;
+                                e[u] = k < n ? __ldg(ent + kb + k) : make_uint2(0u, 0xFFFFFFFFu);
+                            }
+                            if (base == 0) {
+                                if (h == 0 && st < kBmRows && c_lo + st < U) rowoff = (int64_t)__ldg(uid + c_lo + st) * D;
+                                mbar_wait(&w_free[h], (unit & 1) ^ 1);      // the MMAs of the previous unit have read this half
+                                float4* wz = reinterpret_cast<float4*>(whi);
+                                for (int k = st; k < 2 * kBmWHalfBytes / 16; k += kBmSetupThreads) wz[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                                ssync_setup();
+                            }
+#pragma unroll
+                            for (int u = 0; u < kBmEntRegs; ++u) {
+                                const int c = (int)(e[u].y >> 8) - c_lo;
+                                if (c >= 0 && c < kBmRows) {          // padding entries have c = 2^24 - 1 - c_lo
+                                    const uint32_t off = bm_w_off(c, (int)(e[u].y & (kBmHalfPx - 1)));
+                                    const float w = __uint_as_float(e[u].x), hi = bm_hi(w);
+                                    *reinterpret_cast<float*>(whi + off) = hi;
+                                    *reinterpret_cast<float*>(whi + kBmWHalfBytes + off) = __fsub_rn(w, hi);
+                                }
                             }
                         }
-                        if (h == 0 && st == 0) {
-                            d->ht = ht; d->j0 = j0; d->j1 = j1; d->flags = 0;
-                            d->nrows = min(kBmRows, U - pass * kBmRows);
+                        if (h == 0) {
+                            if (st < kBmRows) d->row[st] = rowoff;
+                            if (st == 0) { d->ht = ht; d->j0 = 0; d->j1 = kBmStagesPerUnit; d->flags = 0; d->nrows = min(kBmRows, U - c_lo); }
                         }
-                        fence_async_smem();                        // W is read by the tensor core (async proxy)
+                        fence_async_smem();                            // W is read by the tensor core (async proxy)
                         __threadfence_block();
-                        ssync();
+                        ssync_setup();
                         if (st == 0) mbar_arrive(&w_ready[h]);
                     }
                 }
-                j0 = j1;
             }
-            ht = ht1; ht1 = ht2;
+            ht = ht1; cnt = cnt1;
         }
         {   // sentinel unit: tells the loader, the MMA thread and (through it) the epilogue to stop
             BmDesc* d = &desc[unit % kBmDescRing];
@@ -546,6 +413,138 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
 
 bool backward_mma_supported(int32_t K, int32_t D) { return D % 128 == 0 && D >= 128 && D <= 512 && K >= 1 && K <= QR_MAX_K; }
 
+// workspace: per half tile {R0, R, U, left-to-the-tile-kernel} + union ids + entries
+struct BmWorkspace { size_t cnt, uid, ent, total; };
+static BmWorkspace bm_workspace(const Cam& cam)
+{
+    const size_t nh = (size_t)cam.tiles_x * cam.tiles_y * 2;
+    BmWorkspace w;
+    size_t o = 0;
+    w.cnt = o; o = align_up(o + nh * 16, 256);
+    w.uid = o; o = align_up(o + nh * kBmEntCap * 4, 256);
+    w.ent = o; o = align_up(o + nh * kBmEntCap * 8, 256);
+    w.total = o;
+    return w;
+}
+size_t backward_mma_workspace_bytes(const Cam& cam) { return bm_workspace(cam).total; }
+
+// ------------------------------------------------------------------------------------------------------------------
+// backward_prep_kernel: one CTA per half tile, thread = pixel (the pixel order of the MMA's K dimension).  Numbers
+// the distinct selected Gaussians of the half tile (shared-memory hash set) and rewrites the selection as entries
+// {weight, union row << 8 | pixel} ordered by pixel.  This is the latency-bound, irregular part of qr_backward; run
+// here with a dozen CTAs per SM it costs a few microseconds, inside the persistent kernel it was the bottleneck
+// (profiles/README.md, r1_c).
+// ------------------------------------------------------------------------------------------------------------------
+constexpr int kBmPrepSmem = kBmHash * 4 + kBmHash * 2 + kBmEntCap * 4 + kBmEntCap * 4 + kBmEntCap + 2 * (kBmPx + 4) * 4;
+
+__global__ void __launch_bounds__(kBmPx) backward_prep_kernel(const BackwardParams p, int32_t* __restrict__ cnt,
+                                                              int32_t* __restrict__ uid, uint2* __restrict__ ent)
+{
+    extern __shared__ __align__(16) unsigned char psm[];
+    int32_t* hkey = reinterpret_cast<int32_t*>(psm);
+    int32_t* sid = hkey + kBmHash;
+    float* sw = reinterpret_cast<float*>(sid + kBmEntCap);
+    int32_t* E = reinterpret_cast<int32_t*>(sw + kBmEntCap);        // [kBmPx + 4] exclusive scan of n_sel
+    int32_t* nss = E + kBmPx + 4;                                   // [kBmPx + 4] clamped n_sel
+    uint16_t* hslot = reinterpret_cast<uint16_t*>(nss + kBmPx + 4);
+    uint8_t* spx = reinterpret_cast<uint8_t*>(hslot + kBmHash);
+    __shared__ int32_t warp_sums[kBmPx / 32];
+    __shared__ int32_t ucount;
+    const int ht = blockIdx.x, pl = threadIdx.x, lane = pl & 31, warp = pl >> 5;
+    const int K = p.K;
+    const int tile = ht >> 1;
+    const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
+    // pixel pl of the half tile: stage j = pl >> 3 covers row j >> 1, x = 8 (j & 1) .. + 7
+    auto pix_of = [&](int q, int64_t& pix) -> bool {
+        const int j = q >> 3, x = x0 + (j & 1) * kBmStagePx + (q & 7), y = y0 + (j >> 1);
+        pix = (int64_t)y * p.cam.width + x;
+        return x < p.cam.width && y < p.cam.height;
+    };
+    int64_t pix;
+    const bool valid = pix_of(pl, pix);
+    const int ns = valid ? max(0, min(K, __ldg(p.n_sel + pix))) : 0;
+    int inc = ns;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+    if (lane == 31) warp_sums[warp] = inc;
+    if (pl == 0) ucount = 0;
+    __syncthreads();
+    int e0 = inc - ns, R = 0, R0 = 0;
+#pragma unroll
+    for (int w = 0; w < kBmPx / 32; ++w) {
+        const int s = warp_sums[w];
+        if (w < warp) e0 += s;
+        if (w < 2) R0 += s;
+        R += s;
+    }
+    if (R > kBmEntCap || R == 0) {
+        if (pl == 0) reinterpret_cast<int4*>(cnt)[ht] = make_int4(R0, R, 0, R > kBmEntCap ? 1 : 0);
+        return;
+    }
+    E[pl] = e0;
+    nss[pl] = ns;
+    int hs = 64;
+    while (hs < 2 * R) hs <<= 1;
+    hs = min(hs, kBmHash);                      // R <= kBmEntCap < kBmHash: the probe loops below always terminate
+    const int hmask = hs - 1;
+    for (int k = pl; k < hs; k += kBmPx) hkey[k] = -1;
+    __syncthreads();
+    // stage the records, thread = record: every load of the half tile is in flight at once, and consecutive
+    // threads read consecutive slots of a pixel's list
+    for (int s = 0; s < ns; ++s) spx[e0 + s] = (uint8_t)pl;
+    __syncthreads();
+    for (int k0 = pl; k0 < R; k0 += 8 * kBmPx) {
+        int32_t id[8];
+        float w[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int k = k0 + u * kBmPx;
+            id[u] = -1; w[u] = 0.0f;
+            if (k < R) {
+                const int q = spx[k];
+                int64_t pq;
+                pix_of(q, pq);
+                const int64_t a = pq * K + (k - E[q]);
+                id[u] = __ldg(p.sel_idx + a);
+                w[u] = __ldg(p.sel_w + a);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int k = k0 + u * kBmPx;
+            if (k < R) { sid[k] = id[u]; sw[k] = w[u]; }
+        }
+    }
+    __syncthreads();
+    int32_t* uid_h = uid + (size_t)ht * kBmEntCap;
+#pragma unroll 4
+    for (int k = pl; k < R; k += kBmPx) {       // the thread that creates a cell numbers it
+        const int32_t id = sid[k];
+        uint32_t h = bm_hash((uint32_t)id) & hmask;
+        while (true) {
+            const int32_t old = atomicCAS(&hkey[h], -1, id);
+            if (old == -1) {
+                const int slot = atomicAdd(&ucount, 1);
+                hslot[h] = (uint16_t)slot;
+                uid_h[slot] = id;
+                break;
+            }
+            if (old == id) break;
+            h = (h + 1) & hmask;
+        }
+    }
+    __syncthreads();
+    uint2* ent_h = ent + (size_t)ht * kBmEntCap;
+#pragma unroll 4
+    for (int k = pl; k < R; k += kBmPx) {
+        const int32_t id = sid[k];
+        uint32_t h = bm_hash((uint32_t)id) & hmask;
+        while (hkey[h] != id) h = (h + 1) & hmask;
+        ent_h[k] = make_uint2(__float_as_uint(sw[k]), ((uint32_t)hslot[h] << 8) | (uint32_t)spx[k]);
+    }
+    if (pl == 0) reinterpret_cast<int4*>(cnt)[ht] = make_int4(R0, R, ucount, 0);
+}
+
 typedef CUresult (*BmEncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                     const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -563,8 +562,16 @@ static BmEncodeTiledFn bm_encode_tiled_fn()
     return fn;
 }
 
-int launch_backward_mma(const BackwardParams& p, cudaStream_t st)
+int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_t st)
 {
+    const BmWorkspace wl = bm_workspace(p.cam);
+    if (!ws) return fail(QR_ERR_NULL_POINTER, "qr_backward: workspace is NULL");
+    if (ws_bytes < wl.total) return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_backward: workspace %zu < %zu bytes", ws_bytes, wl.total);
+    if (!aligned16(ws)) return fail(QR_ERR_MISALIGNED, "qr_backward: workspace alignment");
+    int32_t* cnt = reinterpret_cast<int32_t*>(static_cast<char*>(ws) + wl.cnt);
+    int32_t* uid = reinterpret_cast<int32_t*>(static_cast<char*>(ws) + wl.uid);
+    uint2* ent = reinterpret_cast<uint2*>(static_cast<char*>(ws) + wl.ent);
+    p.prep_cnt = cnt; p.prep_uid = uid; p.prep_ent = ent;
     static int sms = 0;
     if (sms == 0) {
         int dev = 0;
@@ -587,12 +594,17 @@ int launch_backward_mma(const BackwardParams& p, cudaStream_t st)
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
     const unsigned grid = (unsigned)min(sms, num_half);
     const int fixed = bm_smem(p.D, 0).total;
-    const int stages = max(2, min(8, (232448 - fixed - 1280) / (2 * kBmStagePx * p.D * 4)));
+    const int stages = max(2, min(12, (232448 - fixed - 1280) / (kBmStagePx * p.D * 4)));
     const int smem = bm_smem(p.D, stages).total;
+    QR_CUDA_OK(cudaFuncSetAttribute(backward_prep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBmPrepSmem));
+    backward_prep_kernel<<<(unsigned)num_half, kBmPx, kBmPrepSmem, st>>>(p, cnt, uid, ent);
+    QR_LAUNCH_OK("backward_prep_kernel");
     QR_CUDA_OK(cudaFuncSetAttribute(backward_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     backward_mma_kernel<<<grid, kBmThreads, smem, st>>>(p, stages, tmap);
     QR_LAUNCH_OK("backward_mma_kernel");
-    return QR_OK;
+    // half tiles with more than kBmEntCap records (rare: a mean of more than 24 selections per pixel)
+    p.only_flagged = true;
+    return launch_backward_tile(p, st);
 }
 
 }  // namespace qr

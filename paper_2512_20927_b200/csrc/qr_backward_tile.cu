@@ -166,7 +166,9 @@ __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const Back
                     if (ht >= num_half) return num_half;
                     int x0, y0;
                     origin(ht, x0, y0);
-                    if (y0 < p.cam.height) return ht;
+                    if (y0 >= p.cam.height) continue;
+                    if (p.only_flagged && p.prep_cnt[4 * ht + 3] == 0) continue;   // the tcgen05 kernel did this one
+                    return ht;
                 }
             };
             // pixel pl of a half tile: stage j = pl >> 3 covers row j >> 1, x = 8 (j & 1) .. + 7
@@ -444,7 +446,7 @@ static int launch_bt(const BackwardParams& p, cudaStream_t st)
     }
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
     const unsigned grid = (unsigned)min(sms, num_half);
-    const int stages = p.D >= 512 ? 5 : (p.D >= 256 ? 8 : 12);
+    const int stages = max(2, min(12, (80 * 1024) / (kBtStagePx * p.D * 4)));   // ring <= 80 KB next to 146 KB of setup state
     const int smem = bt_smem(p.D, stages).total;
     if (p.D == NV * 128) {
         auto kern = backward_tile_kernel<NV, true>;
