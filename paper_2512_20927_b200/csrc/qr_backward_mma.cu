@@ -114,6 +114,14 @@ __device__ __forceinline__ void bm_mma(uint32_t d_tmem, uint64_t a, uint64_t b, 
                  "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "l"(a), "l"(b), "r"(idesc), "r"((uint32_t)accumulate) : "memory");
 }
+// one lane of a converged warp (always the same one): the warp runs the MMA loop in uniform control flow, so the
+// descriptors live in uniform registers, and only the tcgen05 instructions themselves are predicated
+__device__ __forceinline__ bool bm_elect_one()
+{
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ float bm_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
 // byte offset of W[row c][pixel k] inside a 16 KB half buffer: K-major, no swizzle; core matrix = 8 rows x 4 pixels
 // (128 B); pixel chunks 128 B apart (LBO), 8-row groups 2 KB apart (SBO)
@@ -229,34 +237,39 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
         }
     } else if (warp == kBmMmaWarp) {
         // ================================================= MMA issuer ===============================================
-        if (lane == 0) {
-            // M = 128 channels, N = 64 rows, fp32 accumulate, A and B tf32, A MN-major, B K-major
-            const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | ((uint32_t)(kBmRows >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-            const uint32_t w0 = s32(Wsm), st0 = s32(stage_base), lo0 = s32(lo_base);
-            int st = 0;
-            for (int unit = 0;; ++unit) {
-                const int buf = unit & 1;
-                mbar_wait(&w_ready[0], unit & 1);
-                const BmDesc* d = &desc[unit % kBmDescRing];
-                const int j0 = d->j0, j1 = d->j1, flags = d->flags;
-                mbar_wait(&tmem_empty[buf], ((unit >> 1) & 1) ^ 1);
+        // M = 128 channels, N = 64 rows, fp32 accumulate, A and B tf32, A MN-major, B K-major
+        const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | ((uint32_t)(kBmRows >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+        const uint32_t w0 = s32(Wsm), st0 = s32(stage_base), lo0 = s32(lo_base);
+        int st = 0;
+        for (int unit = 0;; ++unit) {
+            const int buf = unit & 1;
+            mbar_wait(&w_ready[0], unit & 1);
+            const BmDesc* d = &desc[unit % kBmDescRing];
+            const int j0 = d->j0, j1 = d->j1, flags = d->flags;
+            mbar_wait(&tmem_empty[buf], ((unit >> 1) & 1) ^ 1);
+            bm_fence_after();
+            if (flags & 1) {
+                if (bm_elect_one()) bm_commit(&tmem_full[buf]);
+                break;
+            }
+            bool have_w1 = false;
+            for (int j = j0; j < j1; ++j, ++st) {
+                const int h = j >> 3;
+                if (h == 1 && !have_w1) { mbar_wait(&w_ready[1], unit & 1); have_w1 = true; }
+                const int s = st % stages, l = st % kBmLoStages;
+                mbar_wait(&lo_ready[l], (st / kBmLoStages) & 1);      // implies raw_full[s]
                 bm_fence_after();
-                if (flags & 1) { bm_commit(&tmem_full[buf]); break; }
-                bool have_w1 = false;
-                for (int j = j0; j < j1; ++j, ++st) {
-                    const int h = j >> 3;
-                    if (h == 1 && !have_w1) { mbar_wait(&w_ready[1], unit & 1); have_w1 = true; }
-                    const int s = st % stages, l = st % kBmLoStages;
-                    mbar_wait(&lo_ready[l], (st / kBmLoStages) & 1);      // implies raw_full[s]
-                    bm_fence_after();
-                    const uint32_t a_hi = st0 + s * stage_half, a_lo = lo0 + l * stage_half;
-                    const uint32_t b_hi = w0 + h * 2 * kBmWHalfBytes + (j & 7) * 256, b_lo = b_hi + kBmWHalfBytes;
-                    const uint64_t db_hi = bm_desc(b_hi, 128, kBmHalfPx / 4 * 128, 0);
-                    const uint64_t db_lo = bm_desc(b_lo, 128, kBmHalfPx / 4 * 128, 0);
+                const uint32_t a_hi = st0 + s * stage_half, a_lo = lo0 + l * stage_half;
+                const uint32_t b_hi = w0 + h * 2 * kBmWHalfBytes + (j & 7) * 256, b_lo = b_hi + kBmWHalfBytes;
+                const uint64_t db_hi = bm_desc(b_hi, 128, kBmHalfPx / 4 * 128, 0);
+                const uint64_t db_lo = bm_desc(b_lo, 128, kBmHalfPx / 4 * 128, 0);
+                const uint64_t da_hi0 = bm_desc(a_hi, 1024, 512, 1), da_lo0 = bm_desc(a_lo, 1024, 512, 1);
+                const uint32_t d0 = tmem_base + (uint32_t)(buf * 256);
+                if (bm_elect_one()) {
+#pragma unroll 4
                     for (int m = 0; m < nchunks; ++m) {
-                        const uint64_t da_hi = bm_desc(a_hi + m * 4096, 1024, 512, 1);
-                        const uint64_t da_lo = bm_desc(a_lo + m * 4096, 1024, 512, 1);
-                        const uint32_t d_tmem = tmem_base + (uint32_t)(buf * 256 + m * kBmRows);
+                        const uint64_t da_hi = da_hi0 + (uint64_t)(m * (4096 >> 4)), da_lo = da_lo0 + (uint64_t)(m * (4096 >> 4));
+                        const uint32_t d_tmem = d0 + (uint32_t)(m * kBmRows);
                         bm_mma(d_tmem, da_hi, db_hi, idesc, j != j0);
                         bm_mma(d_tmem, da_hi, db_lo, idesc, true);
                         bm_mma(d_tmem, da_lo, db_hi, idesc, true);
@@ -265,11 +278,15 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                     bm_commit(&lo_empty[l]);
                     if (h == 0 && (j == 7 || j == j1 - 1)) bm_commit(&w_free[0]);     // last read of W half 0
                 }
-                if (!have_w1) mbar_wait(&w_ready[1], unit & 1);       // keep the phases of every unit in step
+                __syncwarp();
+            }
+            if (!have_w1) mbar_wait(&w_ready[1], unit & 1);       // keep the phases of every unit in step
+            if (bm_elect_one()) {
                 if (j0 >= 8) bm_commit(&w_free[0]);
                 bm_commit(&w_free[1]);
                 bm_commit(&tmem_full[buf]);
             }
+            __syncwarp();
         }
     } else if (warp == kBmLoadWarp) {
         // ================================================= loader ===================================================
