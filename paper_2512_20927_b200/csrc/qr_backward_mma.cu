@@ -18,13 +18,13 @@
 // accumulate G_hi W_hi + G_hi W_lo + G_lo W_hi in fp32 (TMEM).  The dropped G_lo W_lo term and the truncation of the
 // lo parts are <= 2^-21 relative per product, 40x below the fp32 tolerance of north_star (1e-4 relative).
 //
-// One persistent CTA per SM, 14 warps, roles by warp (no role ever waits at a block barrier):
+// One persistent CTA per SM, 18 warps, roles by warp (no role ever waits at a block barrier):
 //   warps 0..3    epilogue: tcgen05.ld of the accumulator (lane = channel, column = union row), one coalesced
 //                 red.global.add.f32 per (union row, 32 channels)
 //   warp  4       one thread issues tcgen05.mma
 //   warp  5       loader: TMA tensor copies of dL_dmap into a ring of stages, far ahead of use
-//   warps 6..9    converters: G_lo = G - trunc(G), elementwise over a stage (same swizzled offset in the lo buffer)
-//   warps 10..13  setup, one unit ahead: number the distinct selected Gaussians of the unit with a shared-memory hash
+//   warps 6..13   converters: G_lo = G - trunc(G), elementwise over a stage (same swizzled offset in the lo buffer)
+//   warps 14..17  setup, one unit ahead: number the distinct selected Gaussians of the unit with a shared-memory hash
 //                 set and scatter the weights into W (hi, lo).  W is double buffered by halves of the K range (pixels
 //                 0..63 / 64..127): half h of the next unit is rebuilt as soon as the MMAs that read it have retired.
 // A unit is (half tile, range of 8-pixel stages, pass): the stage range is cut so that the unit's records fit the
@@ -42,11 +42,11 @@ constexpr int kBmEpiWarps = 4;
 constexpr int kBmMmaWarp = 4;
 constexpr int kBmLoadWarp = 5;
 constexpr int kBmFirstConv = 6;
-constexpr int kBmConvWarps = 4;
-constexpr int kBmFirstSetup = kBmFirstConv + kBmConvWarps;       // 10
+constexpr int kBmConvWarps = 8;
+constexpr int kBmFirstSetup = kBmFirstConv + kBmConvWarps;       // 14
 constexpr int kBmSetupWarps = 4;
 constexpr int kBmSetupThreads = kBmSetupWarps * 32;
-constexpr int kBmThreads = (kBmFirstSetup + kBmSetupWarps) * 32;  // 448
+constexpr int kBmThreads = (kBmFirstSetup + kBmSetupWarps) * 32;  // 576
 constexpr int kBmPx = 128;                 // half tile: 16 x 8 pixels
 constexpr int kBmStagePx = 8;              // one tf32 K step
 constexpr int kBmStagesPerUnit = kBmPx / kBmStagePx;   // 16
@@ -188,14 +188,13 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
     if (warp < kBmEpiWarps) {
         // ================================================= epilogue =================================================
         // thread = channel 32 warp + lane of every 128-channel tile (TMEM lane), columns = union rows of the unit
-        auto ld32 = [&](uint32_t taddr, uint32_t (&r)[32]) {
-            asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+        auto ld16 = [&](uint32_t taddr, uint32_t (&r)[16]) {
+            asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
                          : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-                           "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
-                           "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
-                           "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+                           "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
                          : "r"(taddr));
         };
+        float* dcol = p.dL_dfeat + warp * 32 + lane;
         for (int unit = 0;; ++unit) {
             const int buf = unit & 1;
             mbar_wait(&tmem_full[buf], (unit >> 1) & 1);
@@ -203,34 +202,31 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
             const BmDesc* d = &desc[unit % kBmDescRing];
             if (d->flags & 1) break;
             const int nrows = d->nrows;
-            const uint32_t t0 = tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(buf * 256);
-            float* dcol = p.dL_dfeat + warp * 32 + lane;
             const int64_t* row = d->row;
-            for (int m = 0; m < nchunks; ++m) {
-                uint32_t ra[32], rb[32];
-                ld32(t0 + m * kBmRows, ra);
-                if (nrows > 32) ld32(t0 + m * kBmRows + 32, rb);
+            const uint32_t t0 = tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(buf * 256);
+            // 16 union rows at a time, all channel tiles of them: a row's offset is read once and serves up to four
+            // reductions 128 channels apart
+#pragma unroll 1
+            for (int c0 = 0; c0 < nrows; c0 += 16) {
+                uint32_t r0[16], r1[16], r2[16], r3[16];
+                ld16(t0 + c0, r0);
+                if (nchunks > 1) ld16(t0 + kBmRows + c0, r1);
+                if (nchunks > 2) ld16(t0 + 2 * kBmRows + c0, r2);
+                if (nchunks > 3) ld16(t0 + 3 * kBmRows + c0, r3);
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                if (m == nchunks - 1) {                 // every tcgen05.ld of this accumulator has completed
+                if (c0 + 16 >= nrows) {                 // every tcgen05.ld of this accumulator has completed
                     bm_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&tmem_empty[buf]);
                 }
-                float* dm = dcol + m * 128;
 #pragma unroll
-                for (int c0 = 0; c0 < 32; c0 += 8) {
-                    if (c0 < nrows) {                   // warp-uniform: whole groups of 8 rows are skipped
-#pragma unroll
-                        for (int c = c0; c < c0 + 8; ++c)
-                            if (c < nrows) bm_red(dm + row[c], __uint_as_float(ra[c]));
-                    }
-                }
-#pragma unroll
-                for (int c0 = 0; c0 < 32; c0 += 8) {
-                    if (32 + c0 < nrows) {
-#pragma unroll
-                        for (int c = c0; c < c0 + 8; ++c)
-                            if (32 + c < nrows) bm_red(dm + row[32 + c], __uint_as_float(rb[c]));
+                for (int c = 0; c < 16; ++c) {
+                    if (c0 + c < nrows) {
+                        float* a = dcol + row[c0 + c];
+                        bm_red(a, __uint_as_float(r0[c]));
+                        if (nchunks > 1) bm_red(a + 128, __uint_as_float(r1[c]));
+                        if (nchunks > 2) bm_red(a + 256, __uint_as_float(r2[c]));
+                        if (nchunks > 3) bm_red(a + 384, __uint_as_float(r3[c]));
                     }
                 }
             }
@@ -240,7 +236,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
         // M = 128 channels, N = 64 rows, fp32 accumulate, A and B tf32, A MN-major, B K-major
         const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | ((uint32_t)(kBmRows >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
         const uint32_t w0 = s32(Wsm), st0 = s32(stage_base), lo0 = s32(lo_base);
-        int st = 0;
+        int st = 0, s = 0;                               // st counts stages; s = st % stages without the division
         for (int unit = 0;; ++unit) {
             const int buf = unit & 1;
             mbar_wait(&w_ready[0], unit & 1);
@@ -256,7 +252,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
             for (int j = j0; j < j1; ++j, ++st) {
                 const int h = j >> 3;
                 if (h == 1 && !have_w1) { mbar_wait(&w_ready[1], unit & 1); have_w1 = true; }
-                const int s = st % stages, l = st % kBmLoStages;
+                const int l = st % kBmLoStages;
                 mbar_wait(&lo_ready[l], (st / kBmLoStages) & 1);      // implies raw_full[s]
                 bm_fence_after();
                 const uint32_t a_hi = st0 + s * stage_half, a_lo = lo0 + l * stage_half;
@@ -279,6 +275,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                     if (h == 0 && (j == 7 || j == j1 - 1)) bm_commit(&w_free[0]);     // last read of W half 0
                 }
                 __syncwarp();
+                if (++s == stages) s = 0;
             }
             if (!have_w1) mbar_wait(&w_ready[1], unit & 1);       // keep the phases of every unit in step
             if (bm_elect_one()) {
@@ -291,54 +288,55 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
     } else if (warp == kBmLoadWarp) {
         // ================================================= loader ===================================================
         // lane c < D / 32 copies channels [32 c, 32 c + 32) of the stage's 8 pixels: a [8 px][128 B] swizzled block
-        int st = 0;
+        int s = 0;
+        uint32_t ph = 1;                                 // parity to wait for on stage_empty[s]
         for (int unit = 0;; ++unit) {
             mbar_wait(&w_ready[0], unit & 1);
             const BmDesc* d = &desc[unit % kBmDescRing];
             const int ht = d->ht, j0 = d->j0, j1 = d->j1, flags = d->flags;
             if (flags & 1) {
-                const int s = st % stages;
-                mbar_wait(&stage_empty[s], ((st / stages) & 1) ^ 1);
+                mbar_wait(&stage_empty[s], ph);
                 if (lane == 0) { *done_flag = 1u; mbar_arrive(&raw_full[s]); }     // wakes the converters up to stop
                 break;
             }
             const int tile = ht >> 1;
             const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
-            for (int j = j0; j < j1; ++j, ++st) {
-                const int s = st % stages;
-                mbar_wait(&stage_empty[s], ((st / stages) & 1) ^ 1);
+            for (int j = j0; j < j1; ++j) {
+                mbar_wait(&stage_empty[s], ph);
                 if (lane == 0) mbar_arrive_expect_tx(&raw_full[s], (uint32_t)stage_half);
                 __syncwarp();
                 if (lane < (D >> 5))
                     bm_tma_box(stage_base + (size_t)s * stage_half + lane * 1024, &g_tmap, lane * 32,
                                x0 + (j & 1) * kBmStagePx, y0 + (j >> 1), &raw_full[s]);
+                if (++s == stages) { s = 0; ph ^= 1u; }
             }
         }
     } else if (warp < kBmFirstSetup) {
         // ================================================= converters ===============================================
-        const int ct = tid - kBmFirstConv * 32;              // 0..127
-        const int n4 = stage_half >> 4;                      // float4 per stage
+        // a stage is 2 D float4 = D / 128 per thread; the swizzled offset is the same in the G and the G_lo buffer
+        const int ct = tid - kBmFirstConv * 32;              // 0..255
+        int s = 0;
+        uint32_t ph = 0;                                     // parity to wait for on raw_full[s]
         for (int st = 0;; ++st) {
-            const int s = st % stages, l = st % kBmLoStages;
-            mbar_wait(&raw_full[s], (st / stages) & 1);
+            const int l = st % kBmLoStages;
+            mbar_wait(&raw_full[s], ph);
             if (*done_flag) break;
+            const float4* hi = reinterpret_cast<const float4*>(stage_base + (size_t)s * stage_half) + ct;
+            float4* lo = reinterpret_cast<float4*>(lo_base + (size_t)l * stage_half) + ct;
+            float4 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (u < nchunks) v[u] = hi[u * kBmConvWarps * 32];
             mbar_wait(&lo_empty[l], ((st / kBmLoStages) & 1) ^ 1);       // the MMAs that read this G_lo buffer have retired
-            const float4* hi = reinterpret_cast<const float4*>(stage_base + (size_t)s * stage_half);
-            float4* lo = reinterpret_cast<float4*>(lo_base + (size_t)l * stage_half);
-            for (int i0 = ct; i0 < n4; i0 += 4 * kBmConvWarps * 32) {     // n4 is a multiple of 256 (D % 128 == 0)
-                float4 v[4];
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    v[u] = (i0 + u * kBmConvWarps * 32 < n4) ? hi[i0 + u * kBmConvWarps * 32] : make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (i0 + u * kBmConvWarps * 32 < n4)
-                        lo[i0 + u * kBmConvWarps * 32] = make_float4(__fsub_rn(v[u].x, bm_hi(v[u].x)), __fsub_rn(v[u].y, bm_hi(v[u].y)),
-                                                                    __fsub_rn(v[u].z, bm_hi(v[u].z)), __fsub_rn(v[u].w, bm_hi(v[u].w)));
-            }
+            for (int u = 0; u < 4; ++u)
+                if (u < nchunks)
+                    lo[u * kBmConvWarps * 32] = make_float4(__fsub_rn(v[u].x, bm_hi(v[u].x)), __fsub_rn(v[u].y, bm_hi(v[u].y)),
+                                                           __fsub_rn(v[u].z, bm_hi(v[u].z)), __fsub_rn(v[u].w, bm_hi(v[u].w)));
             fence_async_smem();
             __syncwarp();
             if (lane == 0) mbar_arrive(&lo_ready[l]);
+            if (++s == stages) { s = 0; ph ^= 1u; }
         }
     } else {
         // ================================================= setup ====================================================
