@@ -106,6 +106,12 @@ __device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t a, uint64_t 
                  ::"r"(d_tmem), "l"(a), "l"(b), "r"(idesc), "r"((uint32_t)accumulate) : "memory");
 }
 
+__device__ __forceinline__ bool elect_one()     // one lane of a converged warp, always the same one
+{
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
 
 // byte offset of W[m][c] in the K-major, non-swizzled canonical layout: core matrix = 8 pixels x 4 columns (128 B);
@@ -237,43 +243,50 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
         if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     } else if (warp == kMmaWarp) {
         // ================================================= MMA issuer ===============================================
-        if (lane == 0) {
-            // M = 128, N = 256, fp32 accumulate, A and B tf32, A K-major, B MN-major
-            const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 16) | ((uint32_t)(kUnitN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-            const uint32_t a_hi = s_u32(w_hi), a_lo = s_u32(w_lo), st0 = s_u32(stage_base);
-            int unit = 0, wb = 0, st = 0;
-            for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
-                int x0, y0;
-                half_origin(ht, x0, y0);
-                if (y0 >= p.cam.height) continue;
-                const int U = __ldg(p.ucount + ht);
-                const int rounds = rounds_of(U);
-                for (int c = 0; c < nunits; ++c, ++unit) {
-                    const int buf = unit & 1;
-                    bar_wait(&tmem_empty[buf], ((unit >> 1) & 1) ^ 1);
-                    tc_fence_after();
-                    const uint32_t d_tmem = tmem_base + (uint32_t)(buf * kUnitN);
-                    for (int r = 0; r < rounds; ++r) {
-                        if (c == 0 || rounds > 1) { bar_wait(w_ready, wb & 1); ++wb; }
-                        const int nk = ksteps_of(cols_of(U, r));
-                        for (int j = 0; j < nk; ++j, ++st) {
-                            const int s = st % kStages;
-                            bar_wait(&full[s], (st / kStages) & 1);
-                            tc_fence_after();
-                            const uint32_t b_hi = st0 + s * kStageBytes, b_lo = b_hi + kStageHalf;
-                            const uint64_t da_hi = umma_desc(a_hi + j * 256, 128, kWCols / 4 * 128, 0);
-                            const uint64_t da_lo = umma_desc(a_lo + j * 256, 128, kWCols / 4 * 128, 0);
-                            const uint64_t db_hi = umma_desc(b_hi, 1024, 512, 1);
-                            const uint64_t db_lo = umma_desc(b_lo, 1024, 512, 1);
+        // The whole warp runs the loop in uniform control flow (descriptors stay in uniform registers); one elected
+        // lane issues the tcgen05 instructions.
+        // M = 128, N = 256, fp32 accumulate, A and B tf32, A K-major, B MN-major
+        const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 16) | ((uint32_t)(kUnitN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+        const uint32_t a_hi = s_u32(w_hi), a_lo = s_u32(w_lo), st0 = s_u32(stage_base);
+        int unit = 0, wb = 0, st = 0;
+        for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
+            int x0, y0;
+            half_origin(ht, x0, y0);
+            if (y0 >= p.cam.height) continue;
+            const int U = __ldg(p.ucount + ht);
+            const int rounds = rounds_of(U);
+            for (int c = 0; c < nunits; ++c, ++unit) {
+                const int buf = unit & 1;
+                bar_wait(&tmem_empty[buf], ((unit >> 1) & 1) ^ 1);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + (uint32_t)(buf * kUnitN);
+                for (int r = 0; r < rounds; ++r) {
+                    if (c == 0 || rounds > 1) { bar_wait(w_ready, wb & 1); ++wb; }
+                    const int nk = ksteps_of(cols_of(U, r));
+                    for (int j = 0; j < nk; ++j, ++st) {
+                        const int s = st % kStages;
+                        bar_wait(&full[s], (st / kStages) & 1);
+                        tc_fence_after();
+                        const uint32_t b_hi = st0 + s * kStageBytes, b_lo = b_hi + kStageHalf;
+                        const uint64_t da_hi = umma_desc(a_hi + j * 256, 128, kWCols / 4 * 128, 0);
+                        const uint64_t da_lo = umma_desc(a_lo + j * 256, 128, kWCols / 4 * 128, 0);
+                        const uint64_t db_hi = umma_desc(b_hi, 1024, 512, 1);
+                        const uint64_t db_lo = umma_desc(b_lo, 1024, 512, 1);
+                        if (elect_one()) {
                             umma_tf32(d_tmem, da_hi, db_hi, idesc, (r | j) != 0);
                             umma_tf32(d_tmem, da_lo, db_hi, idesc, true);
                             umma_tf32(d_tmem, da_hi, db_lo, idesc, true);
                             umma_commit(&empty[s]);
                         }
-                        if (rounds > 1 || c == nunits - 1) umma_commit(w_free);     // last use of this W
+                        __syncwarp();
                     }
-                    umma_commit(&tmem_full[buf]);
+                    if (rounds > 1 || c == nunits - 1) {                 // last use of this W
+                        if (elect_one()) umma_commit(w_free);
+                        __syncwarp();
+                    }
                 }
+                if (elect_one()) umma_commit(&tmem_full[buf]);
+                __syncwarp();
             }
         }
     } else if (warp == kLoadWarp) {
