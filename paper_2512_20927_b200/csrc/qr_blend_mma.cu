@@ -345,8 +345,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                         // ---------------- build W for columns [64 r, 64 r + 64) ----------------
                         // the loads of both groups of this warp are issued before anything waits on them
                         const bool write_sel = (c == 0 && r == 0);
-                        int n_g[2];
-                        float inv_g[2];
+                        int n_g[2], ns_g[2];
+                        float inv_g[2], res_g[2];
                         float4 wa[2], wb4[2];
                         float2 mt[2];
 #pragma unroll
@@ -364,14 +364,18 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                                 mt[gg] = __ldg(reinterpret_cast<const float2*>(recs + (size_t)lane * kRecWords + 8));
                             }
                             const int qx = x0 + gx * 4 + (lane & 3), qy = y0 + gy * 2 + ((lane >> 2) & 1);
-                            inv_g[gg] = 0.0f;
+                            ns_g[gg] = 0; res_g[gg] = 0.0f;           // both loads issued at once, used after the wait below
                             if (write_sel && lane < kGroupPx && qx < p.cam.width && qy < p.cam.height) {
                                 const int64_t pix = (int64_t)qy * p.cam.width + qx;
-                                if (__ldg(p.n_sel + pix) > 0) inv_g[gg] = __fdiv_rn(1.0f, __fsub_rn(1.0f, __ldg(p.resid + pix)));
+                                ns_g[gg] = __ldg(p.n_sel + pix);
+                                res_g[gg] = __ldg(p.resid + pix);
                             }
                         }
                         if (wb > 0) bar_wait(w_free, (wb - 1) & 1);
                         ++wb;
+#pragma unroll
+                        for (int gg = 0; gg < 2; ++gg)
+                            inv_g[gg] = ns_g[gg] > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, res_g[gg])) : 0.0f;   // line 20; R8
                         {
                             const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
                             float4* wz = reinterpret_cast<float4*>(smem);
