@@ -196,8 +196,9 @@ def run_cuda(args):
         if timers is not None:
             e3.record()
             timers.append((e0, e1, e2, e3))
-        # preprocess 1, bin_count 3, bin_sort 5 (count, scan, scatter, 2 bucket sorts), forward 2 (walk, blend), backward 1
-        launches["n"] += 1 + 3 + 5 + 2 + 1
+        # preprocess 1, bin_count 3, bin_sort 5 (count, scan, scatter, 2 bucket sorts), forward 2 (walk, blend),
+        # backward 3 (prep, tcgen05 contraction, FFMA kernel for the half tiles the prep left to it)
+        launches["n"] += 1 + 3 + 5 + 2 + 3
         return fe
 
     def barrier():
@@ -336,7 +337,7 @@ def run_cuda(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture named in profiles/ (None
 # until a capture of the current kernels is committed).
-TRAFFIC = {"qr_forward": 861.5e6, "qr_backward": 775.2e6}   # profiles/r1_a_full_metrics.csv
+TRAFFIC = {"qr_forward": 868.7e6, "qr_backward": 818.2e6}   # profiles/r1_c_full_metrics.csv (walk + blend; prep + mma)
 
 
 def main():
