@@ -12,23 +12,26 @@
 //   A = G^T, "MN-major": dL_dmap is [pixel][channel] with channels contiguous.  One TMA tensor copy per 32 channels
 //       (box = 32 channels x 8 consecutive pixels of an image row, SWIZZLE_128B_ATOM_32B) lands a stage directly in
 //       the layout the MMA reads (UMMA SWIZZLE_128B_BASE32B): no thread ever moves dL_dmap.
-//   B = W, K-major, no swizzle: built by the setup warps from the selection records.
+//   B = W, K-major, no swizzle: scattered by the setup warps from the entry lists backward_prep_kernel wrote.
 // Precision: kind::tf32 truncates fp32 operands to 10 explicit mantissa bits (measured on B200), so the raw G tile IS
 // G_hi; converter warps write G_lo = G - trunc(G) next to it, W is split exactly into W_hi + W_lo, and three MMAs
 // accumulate G_hi W_hi + G_hi W_lo + G_lo W_hi in fp32 (TMEM).  The dropped G_lo W_lo term and the truncation of the
 // lo parts are <= 2^-21 relative per product, 40x below the fp32 tolerance of north_star (1e-4 relative).
 //
-// One persistent CTA per SM, 18 warps, roles by warp (no role ever waits at a block barrier):
+// backward_prep_kernel (one CTA per half tile, high occupancy) numbers the distinct selected Gaussians of every half
+// tile and rewrites its selection as pixel-ordered entries {weight, union row << 8 | pixel}: the irregular,
+// latency-bound part of the job.  backward_mma_kernel is one persistent CTA per SM, 18 warps, roles by warp (no role
+// ever waits at a block barrier):
 //   warps 0..3    epilogue: tcgen05.ld of the accumulator (lane = channel, column = union row), one coalesced
 //                 red.global.add.f32 per (union row, 32 channels)
-//   warp  4       one thread issues tcgen05.mma
+//   warp  4       MMA issue: warp-uniform loop, one elected lane issues tcgen05.mma / tcgen05.commit
 //   warp  5       loader: TMA tensor copies of dL_dmap into a ring of stages, far ahead of use
-//   warps 6..13   converters: G_lo = G - trunc(G), elementwise over a stage (same swizzled offset in the lo buffer)
-//   warps 14..17  setup, one unit ahead: number the distinct selected Gaussians of the unit with a shared-memory hash
-//                 set and scatter the weights into W (hi, lo).  W is double buffered by halves of the K range (pixels
-//                 0..63 / 64..127): half h of the next unit is rebuilt as soon as the MMAs that read it have retired.
-// A unit is (half tile, range of 8-pixel stages, pass): the stage range is cut so that the unit's records fit the
-// hash set, and a union larger than 64 rows is processed in passes of 64 rows that re-stream the same pixels.
+//   warps 6..13   converters: G_lo = G - trunc(G), elementwise over a stage (same swizzled offset in the lo ring)
+//   warps 14..17  setup, one unit ahead: stream the unit's entries, clear W and scatter hi / lo.  W is double buffered
+//                 by halves of the K range (pixels 0..63 / 64..127): half h of the next unit is rebuilt as soon as
+//                 the MMAs that read it have retired.
+// A unit is (half tile, pass): a union larger than 64 rows is processed in passes of 64 rows that re-stream the same
+// pixels.  Half tiles with more than kBmEntCap records are left to backward_tile_kernel (qr_backward_tile.cu).
 #include <cuda.h>
 
 #include "qr_async.cuh"

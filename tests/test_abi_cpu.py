@@ -68,7 +68,7 @@ def test_bad_arguments_are_status_codes(lib):
     assert lib.qr_bin_sort(C.byref(cam), 10, 1 << 31, p, p, p, p, p, p, 1 << 20, None) == -5
     m = C.c_int64(-1)
     assert lib.qr_bin_count(0, z, z, C.byref(m), z, 0, None) == 0 and m.value == 0
-    assert lib.qr_bin_workspace_bytes(1000, 5000, 16) > 5000 * 20
+    assert lib.qr_bin_workspace_bytes(1000, 5000, 16) >= 5000 * 16 + 16 * 16 * 4      # keys + scratch + bucket cursors
 
 
 def test_binding_refuses_cpu_tensors():
