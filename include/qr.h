@@ -9,7 +9,7 @@
  *   qr_bin_count       prefix sum of tiles touched -> M = number of (Gaussian, tile) intersections
  *   qr_bin_sort        tile-intersection duplication, (tile, depth) radix sort, per-tile ranges
  *   qr_forward         per-pixel transmittance walk, quantile selection, K-sparse feature accumulation
- *   qr_backward        dL/dfeature scatter-add to the selected Gaussians
+ *   qr_backward        dL/dfeature scatter-add to the selected Gaussians (qr_backward_clear re-zeroes those rows)
  *   qr_dense_forward   Eq. 1 dense volume rendering of the same features (in-run comparator)
  *
  * Conventions the paper leaves to "[3D-GS]" are fixed in DESIGN.md ("Readings", R1-R15).
@@ -138,6 +138,20 @@ size_t qr_backward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D);
 int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N,
                 const int32_t* sel_idx, const float* sel_w, const int32_t* n_sel, const float* dL_dmap,
                 float* dL_dfeat, void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * qr_backward_clear -- zero exactly the rows of dL_dfeat that qr_backward over the same selection adds into (the
+ * distinct Gaussians selected anywhere in the frame), and nothing else.  A loop that keeps dL_dfeat zero outside
+ * those rows (zero it once, then clear after each use) writes ~|S| D floats per step instead of N D
+ * (the whole-table zero fill costs more than qr_backward's own traffic).
+ *   in : sel_idx, n_sel (from qr_forward); ws / ws_bytes = the workspace AS LEFT BY the last qr_backward call with
+ *        the same cam, K, D and selection (its per-half-tile unions are reused); when
+ *        qr_backward_workspace_bytes(cam, K, D) == 0 ws is ignored and may be NULL.
+ *   out: dL_dfeat rows of selected Gaussians = 0; other rows untouched.
+ */
+int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int64_t N,
+                      const int32_t* sel_idx, const int32_t* n_sel, float* dL_dfeat,
+                      const void* ws, size_t ws_bytes, void* stream);
 
 /*
  * qr_dense_forward -- Eq. 1: out = sum_i T_i alpha'_i f_i over the same per-pixel lists, not

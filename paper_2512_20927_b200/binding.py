@@ -27,7 +27,7 @@ STATUS = {0: "QR_OK", -1: "QR_ERR_INVALID_ARG", -2: "QR_ERR_NULL_POINTER", -3: "
 # every symbol include/qr.h declares (tests check that the library exports exactly these)
 SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_bin_workspace_bytes", "qr_bin_count",
            "qr_bin_sort", "qr_forward_workspace_bytes", "qr_forward", "qr_backward_workspace_bytes", "qr_backward",
-           "qr_dense_forward"]
+           "qr_backward_clear", "qr_dense_forward"]
 
 
 class QRError(RuntimeError):
@@ -81,6 +81,8 @@ def load() -> C.CDLL:
     lib.qr_backward_workspace_bytes.restype = sz; lib.qr_backward_workspace_bytes.argtypes = [cam, i32, i32]
     lib.qr_backward.restype = C.c_int
     lib.qr_backward.argtypes = [cam, i32, i32, i64, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.qr_backward_clear.restype = C.c_int
+    lib.qr_backward_clear.argtypes = [cam, i32, i32, i64, vp, vp, vp, vp, sz, vp]
     lib.qr_dense_forward.restype = C.c_int
     lib.qr_dense_forward.argtypes = [cam, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp]
     _lib = lib
@@ -254,19 +256,36 @@ def qr_backward_workspace_bytes(cam, K: int, D: int) -> int:
     return int(load().qr_backward_workspace_bytes(C.byref(c), int(K), int(D)))
 
 
-def qr_backward(cam, N: int, sel_idx, sel_w, n_sel, dL_dmap, dL_dfeat: Optional[torch.Tensor] = None) -> torch.Tensor:
+def qr_backward_workspace(cam, K: int, D: int, device) -> torch.Tensor:
+    """Scratch for qr_backward; keep it to pass the same tensor to qr_backward_clear afterwards."""
+    return torch.empty((max(qr_backward_workspace_bytes(cam, K, D), 16),), dtype=torch.uint8, device=device)
+
+
+def qr_backward(cam, N: int, sel_idx, sel_w, n_sel, dL_dmap, dL_dfeat: Optional[torch.Tensor] = None,
+                ws: Optional[torch.Tensor] = None) -> torch.Tensor:
     """Accumulates into dL_dfeat[N,D] (allocated zero-filled when not given)."""
     c = make_camera(cam)
     K = int(sel_idx.shape[-1])
     D = int(dL_dmap.shape[-1])
     if dL_dfeat is None:
         dL_dfeat = torch.zeros((int(N), D), dtype=torch.float32, device=dL_dmap.device)
-    nws = int(load().qr_backward_workspace_bytes(C.byref(c), K, D))
-    ws = torch.empty((max(nws, 16),), dtype=torch.uint8, device=dL_dmap.device)
+    if ws is None:
+        ws = qr_backward_workspace(cam, K, D, dL_dmap.device)
     _check(load().qr_backward(C.byref(c), K, D, int(N), _dev(sel_idx, torch.int32, "sel_idx"),
                               _dev(sel_w, torch.float32, "sel_w"), _dev(n_sel, torch.int32, "n_sel"),
                               _dev(dL_dmap, torch.float32, "dL_dmap"), _dev(dL_dfeat, torch.float32, "dL_dfeat"),
-                              ws.data_ptr(), ws.numel(), _stream()))
+                              _dev(ws, torch.uint8, "ws"), ws.numel(), _stream()))
+    return dL_dfeat
+
+
+def qr_backward_clear(cam, N: int, sel_idx, n_sel, dL_dfeat: torch.Tensor, ws: torch.Tensor) -> torch.Tensor:
+    """Zeroes the rows of dL_dfeat the last qr_backward (same selection, same ws) added into."""
+    c = make_camera(cam)
+    K = int(sel_idx.shape[-1])
+    D = int(dL_dfeat.shape[-1])
+    _check(load().qr_backward_clear(C.byref(c), K, D, int(N), _dev(sel_idx, torch.int32, "sel_idx"),
+                                    _dev(n_sel, torch.int32, "n_sel"), _dev(dL_dfeat, torch.float32, "dL_dfeat"),
+                                    _dev(ws, torch.uint8, "ws"), ws.numel(), _stream()))
     return dL_dfeat
 
 

@@ -253,7 +253,86 @@ static int launch_backward(const BackwardParams& p, cudaStream_t st)
     return QR_OK;
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// qr_backward_clear: zero exactly the rows of dL_dfeat a qr_backward over the same selection adds into, so that a
+// training loop re-zeroes ~|S| D floats per step instead of memset-ing the whole [N, D] table (1.02 GB at config 3,
+// of which 24 MB are ever non-zero).  One CTA strides over half tiles.  Where the tcgen05 path left its numbered
+// union in the workspace the rows are zeroed once per half tile; elsewhere (other D, over-full half tiles) once per
+// selection record.
+// ------------------------------------------------------------------------------------------------------------------
+constexpr int kClearThreads = 256;
+
+__device__ __forceinline__ void clear_row(float* row, int D, int lane)
+{
+    if ((D & 3) == 0) {
+        float4* r4 = reinterpret_cast<float4*>(row);
+        for (int i = lane; i < (D >> 2); i += 32) r4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    } else {
+        for (int i = lane; i < D; i += 32) row[i] = 0.0f;
+    }
+}
+
+__global__ void __launch_bounds__(kClearThreads) backward_clear_kernel(const BackwardParams p, const int uid_stride)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
+    for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
+        const int tile = ht >> 1;
+        const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
+        if (y0 >= p.cam.height) continue;
+        int4 c = make_int4(0, 1, 0, 1);
+        if (p.prep_cnt) c = __ldg(reinterpret_cast<const int4*>(p.prep_cnt) + ht);
+        if (c.y == 0) continue;                                   // nothing selected in this half tile
+        if (c.w == 0) {                                           // numbered union: one pass over its rows
+            const int32_t* uid = p.prep_uid + (size_t)ht * uid_stride;
+            for (int r = warp; r < c.z; r += kClearThreads / 32) clear_row(p.dL_dfeat + (int64_t)__ldg(uid + r) * p.D, p.D, lane);
+        } else {                                                  // every record of the 16 x 8 pixels
+            for (int q = warp; q < 128; q += kClearThreads / 32) {
+                const int x = x0 + (q & 15), y = y0 + (q >> 4);
+                if (x >= p.cam.width || y >= p.cam.height) continue;
+                const int64_t pix = (int64_t)y * p.cam.width + x;
+                const int ns = max(0, min(p.K, __ldg(p.n_sel + pix)));
+                for (int s = 0; s < ns; ++s) clear_row(p.dL_dfeat + (int64_t)__ldg(p.sel_idx + pix * p.K + s) * p.D, p.D, lane);
+            }
+        }
+    }
+}
+
 }  // namespace qr
+
+extern "C" int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int64_t N, const int32_t* sel_idx,
+                                 const int32_t* n_sel, float* dL_dfeat, const void* ws, size_t ws_bytes, void* stream)
+{
+    using namespace qr;
+    if (int rc = check_cam(cam)) return rc;
+    if (K < 1) return fail(QR_ERR_INVALID_ARG, "qr_backward_clear: K = %d < 1", K);
+    if (K > QR_MAX_K) return fail(QR_ERR_UNSUPPORTED, "qr_backward_clear: K = %d > QR_MAX_K", K);
+    if (D < 1) return fail(QR_ERR_INVALID_ARG, "qr_backward_clear: D = %d < 1", D);
+    if (D > QR_MAX_D) return fail(QR_ERR_UNSUPPORTED, "qr_backward_clear: D = %d > QR_MAX_D", D);
+    if (N < 0) return fail(QR_ERR_INVALID_ARG, "qr_backward_clear: N < 0");
+    if (!sel_idx || !n_sel) return fail(QR_ERR_NULL_POINTER, "qr_backward_clear: NULL input");
+    if (N == 0) return QR_OK;
+    if (!dL_dfeat) return fail(QR_ERR_NULL_POINTER, "qr_backward_clear: dL_dfeat is NULL");
+    if (!aligned16(dL_dfeat)) return fail(QR_ERR_MISALIGNED, "qr_backward_clear: 16-byte alignment");
+    BackwardParams p;
+    p.cam = make_cam(cam); p.K = K; p.D = D; p.N = N;
+    p.sel_idx = sel_idx; p.sel_w = nullptr; p.n_sel = n_sel; p.dL_dmap = nullptr; p.dL_dfeat = dL_dfeat;
+    int uid_stride = 0;
+    if (backward_mma_supported(K, D)) {
+        if (!ws) return fail(QR_ERR_NULL_POINTER, "qr_backward_clear: workspace is NULL");
+        if (int rc = backward_mma_workspace_view(p, ws, ws_bytes, &uid_stride)) return rc;
+    }
+    static int sms = 0;
+    if (sms == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+            sms = 148;
+    }
+    const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
+    backward_clear_kernel<<<(unsigned)min(num_half, sms * 8), kClearThreads, 0, (cudaStream_t)stream>>>(p, uid_stride);
+    QR_LAUNCH_OK("backward_clear_kernel");
+    return QR_OK;
+}
 
 extern "C" size_t qr_backward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D)
 {

@@ -26,6 +26,7 @@ bool backward_tile_supported(int32_t K, int32_t D);
 // qr_backward_mma.cu: the same contraction on tcgen05 (tf32 x 3), D a multiple of 128.
 bool backward_mma_supported(int32_t K, int32_t D);
 size_t backward_mma_workspace_bytes(const Cam& cam);
+int backward_mma_workspace_view(BackwardParams& p, const void* ws, size_t ws_bytes, int* uid_stride);
 int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_t st);
 int launch_backward_tile(const BackwardParams& p, cudaStream_t st);
 

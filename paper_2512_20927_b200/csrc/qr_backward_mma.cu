@@ -445,6 +445,19 @@ static BmWorkspace bm_workspace(const Cam& cam)
     return w;
 }
 size_t backward_mma_workspace_bytes(const Cam& cam) { return bm_workspace(cam).total; }
+// points p at the arrays a previous launch_backward_mma left in ws (for qr_backward_clear)
+int backward_mma_workspace_view(BackwardParams& p, const void* ws, size_t ws_bytes, int* uid_stride)
+{
+    const BmWorkspace wl = bm_workspace(p.cam);
+    if (ws_bytes < wl.total) return fail(QR_ERR_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", ws_bytes, wl.total);
+    if (!aligned16(ws)) return fail(QR_ERR_MISALIGNED, "workspace alignment");
+    const char* w = static_cast<const char*>(ws);
+    p.prep_cnt = reinterpret_cast<const int32_t*>(w + wl.cnt);
+    p.prep_uid = reinterpret_cast<const int32_t*>(w + wl.uid);
+    p.prep_ent = reinterpret_cast<const uint2*>(w + wl.ent);
+    *uid_stride = kBmEntCap;
+    return QR_OK;
+}
 
 // ------------------------------------------------------------------------------------------------------------------
 // backward_prep_kernel: one CTA per half tile, thread = pixel (the pixel order of the MMA's K dimension).  Numbers

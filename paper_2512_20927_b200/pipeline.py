@@ -31,8 +31,14 @@ def forward(cam, fe: Frontend, features: torch.Tensor, K: int, out: Optional[B.F
     return B.qr_forward(cam, K, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, out)
 
 
-def backward(cam, N: int, fwd: B.ForwardOut, dL_dmap: torch.Tensor, dL_dfeat: Optional[torch.Tensor] = None):
-    return B.qr_backward(cam, N, fwd.sel_idx, fwd.sel_w, fwd.n_sel, dL_dmap, dL_dfeat)
+def backward(cam, N: int, fwd: B.ForwardOut, dL_dmap: torch.Tensor, dL_dfeat: Optional[torch.Tensor] = None,
+             ws: Optional[torch.Tensor] = None):
+    return B.qr_backward(cam, N, fwd.sel_idx, fwd.sel_w, fwd.n_sel, dL_dmap, dL_dfeat, ws)
+
+
+def backward_clear(cam, N: int, fwd: B.ForwardOut, dL_dfeat: torch.Tensor, ws: torch.Tensor):
+    """Re-zero the rows the last backward(..., ws) touched (instead of zeroing the whole [N, D] table)."""
+    return B.qr_backward_clear(cam, N, fwd.sel_idx, fwd.n_sel, dL_dfeat, ws)
 
 
 def dense_forward(cam, fe: Frontend, features: torch.Tensor, t_min: float = 1e-4, out_map=None, final_T=None):

@@ -258,6 +258,36 @@ def test_backward_accumulates_and_adjoint(qr, orc):
     torch.testing.assert_close(dF2, 2.0 * dF, rtol=1e-5, atol=1e-6)
 
 
+@pytest.mark.parametrize("name,kw,K", [("cfg3", dict(N=60000, W=112, H=80, D=512), 40),      # tcgen05 path: numbered unions
+                                       ("cfg2", dict(N=20000, W=70, H=50, D=64), 40),        # no workspace: per record
+                                       ("cfg3", dict(N=40000, W=64, H=48, D=128), 200)])     # over-full half tiles
+def test_backward_clear_zeroes_exactly_the_touched_rows(qr, orc, name, kw, K):
+    """qr_backward_clear: rows of selected Gaussians become 0, every other row keeps its value (a sentinel)."""
+    sc = make_scene(name, seed=12, **kw)
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    out = qr.pipeline.forward(sc.cam, fe, g.features, K)
+    G = P.to_dev(sc.dL_dmap)
+    ws = qr.qr_backward_workspace(sc.cam, K, sc.D, G.device)
+    dF = torch.full((sc.N, sc.D), 7.0, dtype=torch.float32, device=G.device)
+    qr.pipeline.backward(sc.cam, sc.N, out, G, dF, ws)
+    qr.pipeline.backward_clear(sc.cam, sc.N, out, dF, ws)
+    sel = out.sel_idx[out.sel_idx >= 0].long()
+    touched = torch.zeros(sc.N, dtype=torch.bool, device=G.device)
+    touched[sel] = True
+    assert int(touched.sum()) > 10
+    assert (dF[touched] == 0).all()
+    assert (dF[~touched] == 7.0).all()
+    # zero once, then backward / clear / backward gives the same gradient as a fresh table
+    dF.zero_()
+    qr.pipeline.backward(sc.cam, sc.N, out, G, dF, ws)
+    first = dF.clone()
+    qr.pipeline.backward_clear(sc.cam, sc.N, out, dF, ws)
+    assert (dF == 0).all()
+    qr.pipeline.backward(sc.cam, sc.N, out, G, dF, ws)
+    torch.testing.assert_close(dF, first, rtol=1e-5, atol=1e-6)
+
+
 # ------------------------------------------------------------------------------------------------
 # full-size sampled check in the configuration bench.py times (config 3)
 # ------------------------------------------------------------------------------------------------
