@@ -28,12 +28,14 @@
 namespace qr {
 
 constexpr int kEpiWarps = 4;
-constexpr int kProdWarps = 8;
+constexpr int kProdWarps = 16;                            // 16 pixel groups of a half tile; 8 rows x 2 channel halves of a stage
 constexpr int kMmaWarp = kEpiWarps;                       // warp 4
 constexpr int kLoadWarp = kEpiWarps + 1;                  // warp 5
-constexpr int kFirstProd = kEpiWarps + 2;                 // warps 6..13
+constexpr int kFirstProd = kEpiWarps + 2;                 // warps 6..21
 constexpr int kMmaThreads = (kEpiWarps + 2 + kProdWarps) * 32;
 constexpr int kProdThreads = kProdWarps * 32;
+constexpr int kGroupsPerProd = 16 / kProdWarps;           // pixel groups of the half tile per producer warp
+static_assert(kProdWarps == 16, "the row conversion below splits a stage into 8 rows x 2 channel halves");
 constexpr int kWCols = 64;                                // union columns per round
 constexpr int kUnitN = 256;                               // channels per work unit
 constexpr int kStageRows = 8;                             // union rows per stage = one tf32 K step
@@ -325,8 +327,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
         }
     } else {
         // ================================================= producers ================================================
-        const int pw = warp - kFirstProd;                 // 0..7
-        const int ptid = tid - kFirstProd * 32;           // 0..255
+        const int pw = warp - kFirstProd;                 // 0..15
+        const int ptid = tid - kFirstProd * 32;           // 0..511
         const uint32_t lt_mask = (1u << lane) - 1u;
         const unsigned char* raw_base = smem + MmaSmem::raw;
         auto prod_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kProdThreads) : "memory"); };
@@ -350,8 +352,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                         float4 wa[2], wb4[2];
                         float2 mt[2];
 #pragma unroll
-                        for (int gg = 0; gg < 2; ++gg) {
-                            const int g = pw * 2 + gg;
+                        for (int gg = 0; gg < kGroupsPerProd; ++gg) {
+                            const int g = pw * kGroupsPerProd + gg;
                             const int gx = g & 3, gy = g >> 2;
                             const int64_t group = (int64_t)tile * kGroupsPerTile + half * 16 + g;
                             n_g[gg] = __ldg(p.gcount + group);
@@ -374,7 +376,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                         if (wb > 0) bar_wait(w_free, (wb - 1) & 1);
                         ++wb;
 #pragma unroll
-                        for (int gg = 0; gg < 2; ++gg)
+                        for (int gg = 0; gg < kGroupsPerProd; ++gg)
                             inv_g[gg] = ns_g[gg] > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, res_g[gg])) : 0.0f;   // line 20; R8
                         {
                             const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -383,8 +385,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                         }
                         prod_sync();
 #pragma unroll
-                        for (int gg = 0; gg < 2; ++gg) {
-                            const int g = pw * 2 + gg;                     // group 0..15 of the half tile
+                        for (int gg = 0; gg < kGroupsPerProd; ++gg) {
+                            const int g = pw * kGroupsPerProd + gg;                     // group 0..15 of the half tile
                             const int gx = g & 3, gy = g >> 2;
                             const int64_t group = (int64_t)tile * kGroupsPerTile + half * 16 + g;
                             const int n = n_g[gg];
@@ -439,34 +441,27 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                         prod_sync();
                         if (ptid == 0) bar_arrive(w_ready);
                     }
-                    // ---------------- feature rows of this round: warp pw converts row pw of every stage ----------------
+                    // ---------------- feature rows of this round: warp pw converts channel half pw >> 3 of row pw & 7 ----------------
                     const int nk = ksteps_of(ncols);
-                    // byte offset of this lane's 16 bytes inside a stage half: channels 4 lane .. 4 lane + 3 (+128)
-                    const uint32_t lane_off = (uint32_t)((lane >> 3) * 1024 + (pw >> 2) * 512 + (pw & 3) * 128 +
-                                                         ((((lane & 7) >> 1) ^ (pw & 3)) * 32) + (lane & 1) * 16);
+                    const int row = pw & 7, ch = pw >> 3;
+                    // byte offset of this lane's 16 bytes inside a stage half: channels 128 ch + 4 lane .. + 3
+                    const uint32_t lane_off = (uint32_t)(ch * 4 * 1024 + (lane >> 3) * 1024 + (row >> 2) * 512 + (row & 3) * 128 +
+                                                         ((((lane & 7) >> 1) ^ (row & 3)) * 32) + (lane & 1) * 16);
                     for (int j = 0; j < nk; ++j, ++st) {
                         const int sr = st % kRawStages;
                         bar_wait(&raw_full[sr], (st / kRawStages) & 1);
-                        float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0;
-                        if (j * kStageRows + pw < ncols) {
-                            const unsigned char* rr = raw_base + sr * kRawBytes + pw * kRawRow + lane * 16;
-                            a0 = *reinterpret_cast<const float4*>(rr);
-                            a1 = *reinterpret_cast<const float4*>(rr + 512);
-                        }
+                        float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (j * kStageRows + row < ncols)
+                            a0 = *reinterpret_cast<const float4*>(raw_base + sr * kRawBytes + row * kRawRow + ch * 512 + lane * 16);
                         const float4 h0 = make_float4(tf32_hi(a0.x), tf32_hi(a0.y), tf32_hi(a0.z), tf32_hi(a0.w));
-                        const float4 h1 = make_float4(tf32_hi(a1.x), tf32_hi(a1.y), tf32_hi(a1.z), tf32_hi(a1.w));
                         const float4 l0 = make_float4(__fsub_rn(a0.x, h0.x), __fsub_rn(a0.y, h0.y), __fsub_rn(a0.z, h0.z), __fsub_rn(a0.w, h0.w));
-                        const float4 l1 = make_float4(__fsub_rn(a1.x, h1.x), __fsub_rn(a1.y, h1.y), __fsub_rn(a1.z, h1.z), __fsub_rn(a1.w, h1.w));
                         __syncwarp();
                         if (lane == 0) bar_arrive(&raw_empty[sr]);          // the raw row is in registers
                         const int s = st % kStages;
                         bar_wait(&empty[s], ((st / kStages) & 1) ^ 1);
                         unsigned char* hi = stage_base + s * kStageBytes + lane_off;
-                        unsigned char* lo = hi + kStageHalf;
                         *reinterpret_cast<float4*>(hi) = h0;
-                        *reinterpret_cast<float4*>(hi + 4 * 1024) = h1;
-                        *reinterpret_cast<float4*>(lo) = l0;
-                        *reinterpret_cast<float4*>(lo + 4 * 1024) = l1;
+                        *reinterpret_cast<float4*>(hi + kStageHalf) = l0;
                         fence_async_smem();
                         __syncwarp();
                         if (lane == 0) bar_arrive(&full[s]);
