@@ -28,19 +28,20 @@
 namespace qr {
 
 constexpr int kEpiWarps = 4;
-constexpr int kProdWarps = 16;                            // 16 pixel groups of a half tile; 8 rows x 2 channel halves of a stage
+constexpr int kConvWarps = 8;                             // one union row of every stage each
+constexpr int kBuildWarps = 8;                            // two pixel groups of the half tile each
 constexpr int kMmaWarp = kEpiWarps;                       // warp 4
 constexpr int kLoadWarp = kEpiWarps + 1;                  // warp 5
-constexpr int kFirstProd = kEpiWarps + 2;                 // warps 6..21
-constexpr int kMmaThreads = (kEpiWarps + 2 + kProdWarps) * 32;
-constexpr int kProdThreads = kProdWarps * 32;
-constexpr int kGroupsPerProd = 16 / kProdWarps;           // pixel groups of the half tile per producer warp
-static_assert(kProdWarps == 16, "the row conversion below splits a stage into 8 rows x 2 channel halves");
+constexpr int kFirstConv = kEpiWarps + 2;                 // warps 6..13
+constexpr int kFirstBuild = kFirstConv + kConvWarps;      // warps 14..21
+constexpr int kMmaThreads = (kFirstBuild + kBuildWarps) * 32;
+constexpr int kBuildThreads = kBuildWarps * 32;
+constexpr int kGroupsPerBuild = 16 / kBuildWarps;         // pixel groups of the half tile per builder warp
 constexpr int kWCols = 64;                                // union columns per round
 constexpr int kUnitN = 256;                               // channels per work unit
 constexpr int kStageRows = 8;                             // union rows per stage = one tf32 K step
-constexpr int kStages = 4;
-constexpr int kRawStages = 8;
+constexpr int kStages = 2;
+constexpr int kRawStages = 4;
 constexpr int kRawRow = kUnitN * 4;                       // 1 KB: one feature row half
 constexpr int kRawBytes = kStageRows * kRawRow;           // 8 KB per raw stage
 constexpr int kEpiTile = 32 * 32 * 4;                     // 4 KB: 32 pixels x 32 channels
@@ -49,14 +50,13 @@ constexpr int kStageHalf = kStageRows * kUnitN * 4;       // 8 KB (hi or lo)
 constexpr int kStageBytes = 2 * kStageHalf;
 
 struct MmaSmem {
-    static constexpr int w_hi = 0;
-    static constexpr int w_lo = kWBytes;
-    static constexpr int stages = 2 * kWBytes;
+    static constexpr int w = 0;                                           // [2 buffers][hi, lo]
+    static constexpr int stages = 4 * kWBytes;
     static constexpr int raw = stages + kStages * kStageBytes;
     static constexpr int epi = raw + kRawStages * kRawBytes;              // [4 warps][2] staging tiles
-    static constexpr int uid = epi + kEpiWarps * 2 * kEpiTile;            // int32[kWCols]
-    static constexpr int bars = uid + kWCols * 4;                         // uint64[...]
-    static constexpr int n_bars = 2 * kStages + 2 * kRawStages + 2 + 4;
+    static constexpr int uid = epi + kEpiWarps * 2 * kEpiTile;            // int32[2 buffers][kWCols]
+    static constexpr int bars = uid + 2 * kWCols * 4;                     // uint64[...]
+    static constexpr int n_bars = 2 * kStages + 2 * kRawStages + 4 + 4;
     static constexpr int tmem = bars + n_bars * 8;
     static constexpr int total = tmem + 16;
 };
@@ -131,18 +131,16 @@ __device__ __forceinline__ int ksteps_of(int ncols) { return max(1, (ncols + kSt
 __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tmap)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
-    float* w_hi = reinterpret_cast<float*>(smem + MmaSmem::w_hi);
-    float* w_lo = reinterpret_cast<float*>(smem + MmaSmem::w_lo);
     unsigned char* stage_base = smem + MmaSmem::stages;
     int32_t* uid_s = reinterpret_cast<int32_t*>(smem + MmaSmem::uid);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + MmaSmem::bars);
-    uint64_t* full = bars;                       // [kStages] producers -> MMA (8 warp arrivals)
-    uint64_t* empty = bars + kStages;            // [kStages] MMA -> producers (tcgen05.commit)
-    uint64_t* raw_full = bars + 2 * kStages;     // [kRawStages] loader (TMA complete_tx) -> producers
-    uint64_t* raw_empty = raw_full + kRawStages; // [kRawStages] producers -> loader (8 warp arrivals)
-    uint64_t* w_ready = raw_empty + kRawStages;  // producers -> MMA, loader
-    uint64_t* w_free = w_ready + 1;              // MMA -> producers (tcgen05.commit)
-    uint64_t* tmem_full = w_free + 1;            // [2] MMA -> epilogue (tcgen05.commit)
+    uint64_t* full = bars;                       // [kStages] converters -> MMA (8 warp arrivals)
+    uint64_t* empty = bars + kStages;            // [kStages] MMA -> converters (tcgen05.commit)
+    uint64_t* raw_full = bars + 2 * kStages;     // [kRawStages] loader (TMA complete_tx) -> converters
+    uint64_t* raw_empty = raw_full + kRawStages; // [kRawStages] converters -> loader (8 warp arrivals)
+    uint64_t* w_ready = raw_empty + kRawStages;  // [2] builders -> MMA, loader: W instance i lives in buffer i & 1
+    uint64_t* w_free = w_ready + 2;              // [2] MMA -> builders (tcgen05.commit)
+    uint64_t* tmem_full = w_free + 2;            // [2] MMA -> epilogue (tcgen05.commit)
     uint64_t* tmem_empty = tmem_full + 2;        // [2] epilogue -> MMA (4 warp arrivals)
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + MmaSmem::tmem);
 
@@ -152,10 +150,12 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
     const int num_half = p.num_tiles * 2;
 
     if (tid == 0) {
-        for (int s = 0; s < kStages; ++s) { bar_init(&full[s], kProdWarps); bar_init(&empty[s], 1); }
-        for (int s = 0; s < kRawStages; ++s) { bar_init(&raw_full[s], 1); bar_init(&raw_empty[s], kProdWarps); }
-        bar_init(w_ready, 1); bar_init(w_free, 1);
-        for (int b = 0; b < 2; ++b) { bar_init(&tmem_full[b], 1); bar_init(&tmem_empty[b], kEpiWarps); }
+        for (int s = 0; s < kStages; ++s) { bar_init(&full[s], kConvWarps); bar_init(&empty[s], 1); }
+        for (int s = 0; s < kRawStages; ++s) { bar_init(&raw_full[s], 1); bar_init(&raw_empty[s], kConvWarps); }
+        for (int b = 0; b < 2; ++b) {
+            bar_init(&w_ready[b], 1); bar_init(&w_free[b], 1);
+            bar_init(&tmem_full[b], 1); bar_init(&tmem_empty[b], kEpiWarps);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 0) {
@@ -249,8 +249,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
         // lane issues the tcgen05 instructions.
         // M = 128, N = 256, fp32 accumulate, A and B tf32, A K-major, B MN-major
         const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 16) | ((uint32_t)(kUnitN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-        const uint32_t a_hi = s_u32(w_hi), a_lo = s_u32(w_lo), st0 = s_u32(stage_base);
-        int unit = 0, wb = 0, st = 0;
+        const uint32_t w0 = s_u32(smem + MmaSmem::w), st0 = s_u32(stage_base);
+        int unit = 0, wb = 0, wcur = 0, st = 0;            // wb: W instances seen so far; wcur: the one in use
         for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
             int x0, y0;
             half_origin(ht, x0, y0);
@@ -263,7 +263,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)(buf * kUnitN);
                 for (int r = 0; r < rounds; ++r) {
-                    if (c == 0 || rounds > 1) { bar_wait(w_ready, wb & 1); ++wb; }
+                    if (c == 0 || rounds > 1) { wcur = wb++; bar_wait(&w_ready[wcur & 1], (wcur >> 1) & 1); }
+                    const uint32_t a_hi = w0 + (uint32_t)(wcur & 1) * 2 * kWBytes, a_lo = a_hi + kWBytes;
                     const int nk = ksteps_of(cols_of(U, r));
                     for (int j = 0; j < nk; ++j, ++st) {
                         const int s = st % kStages;
@@ -283,7 +284,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                         __syncwarp();
                     }
                     if (rounds > 1 || c == nunits - 1) {                 // last use of this W
-                        if (elect_one()) umma_commit(w_free);
+                        if (elect_one()) umma_commit(&w_free[wcur & 1]);
                         __syncwarp();
                     }
                 }
@@ -295,7 +296,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
         // ================================================= loader ===================================================
         // lane k < 8 copies union row 8 j + k of every stage: 1 KB (256 channels) per bulk copy, kRawStages ahead
         unsigned char* raw_base = smem + MmaSmem::raw;
-        int wb = 0, st = 0;
+        int wb = 0, wcur = 0, st = 0;
         for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
             int x0, y0;
             half_origin(ht, x0, y0);
@@ -304,7 +305,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
             const int rounds = rounds_of(U);
             for (int c = 0; c < nunits; ++c) {
                 for (int r = 0; r < rounds; ++r) {
-                    if (c == 0 || rounds > 1) { bar_wait(w_ready, wb & 1); ++wb; }      // uid_s of this round is written
+                    if (c == 0 || rounds > 1) { wcur = wb++; bar_wait(&w_ready[wcur & 1], (wcur >> 1) & 1); }   // its uid_s is written
                     const int ncols = cols_of(U, r);
                     const int nk = ksteps_of(ncols);
                     for (int j = 0; j < nk; ++j, ++st) {
@@ -317,7 +318,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                         }
                         __syncwarp();
                         if (lane < rows) {
-                            const int32_t id = uid_s[j * kStageRows + lane];
+                            const int32_t id = uid_s[(wcur & 1) * kWCols + j * kStageRows + lane];
                             tma_row(raw_base + s * kRawBytes + lane * kRawRow,
                                     static_cast<const float*>(p.features) + (int64_t)id * D + c * kUnitN, kRawRow, &raw_full[s]);
                         }
@@ -325,14 +326,65 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                 }
             }
         }
-    } else {
-        // ================================================= producers ================================================
-        const int pw = warp - kFirstProd;                 // 0..15
-        const int ptid = tid - kFirstProd * 32;           // 0..511
-        const uint32_t lt_mask = (1u << lane) - 1u;
+    } else if (warp < kFirstBuild) {
+        // ================================================= converters ===============================================
+        // warp pw splits union row pw of every stage: ld.shared of the raw row -> hi / lo -> st.shared in the MN-major
+        // SWIZZLE_128B_BASE32B layout.  They only need the union sizes, never W, so they run ahead of the builders.
+        const int pw = warp - kFirstConv;                 // 0..7
         const unsigned char* raw_base = smem + MmaSmem::raw;
-        auto prod_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kProdThreads) : "memory"); };
-        int wb = 0, st = 0;
+        // byte offset of this lane's 16 bytes inside a stage half: channels 4 lane .. 4 lane + 3 (+128)
+        const uint32_t lane_off = (uint32_t)((lane >> 3) * 1024 + (pw >> 2) * 512 + (pw & 3) * 128 +
+                                             ((((lane & 7) >> 1) ^ (pw & 3)) * 32) + (lane & 1) * 16);
+        int st = 0;
+        for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
+            int x0, y0;
+            half_origin(ht, x0, y0);
+            if (y0 >= p.cam.height) continue;
+            const int U = __ldg(p.ucount + ht);
+            const int rounds = rounds_of(U);
+            for (int c = 0; c < nunits; ++c) {
+                for (int r = 0; r < rounds; ++r) {
+                    const int ncols = cols_of(U, r);
+                    const int nk = ksteps_of(ncols);
+                    for (int j = 0; j < nk; ++j, ++st) {
+                        const int sr = st % kRawStages;
+                        bar_wait(&raw_full[sr], (st / kRawStages) & 1);
+                        float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0;
+                        if (j * kStageRows + pw < ncols) {
+                            const unsigned char* rr = raw_base + sr * kRawBytes + pw * kRawRow + lane * 16;
+                            a0 = *reinterpret_cast<const float4*>(rr);
+                            a1 = *reinterpret_cast<const float4*>(rr + 512);
+                        }
+                        const float4 h0 = make_float4(tf32_hi(a0.x), tf32_hi(a0.y), tf32_hi(a0.z), tf32_hi(a0.w));
+                        const float4 h1 = make_float4(tf32_hi(a1.x), tf32_hi(a1.y), tf32_hi(a1.z), tf32_hi(a1.w));
+                        const float4 l0 = make_float4(__fsub_rn(a0.x, h0.x), __fsub_rn(a0.y, h0.y), __fsub_rn(a0.z, h0.z), __fsub_rn(a0.w, h0.w));
+                        const float4 l1 = make_float4(__fsub_rn(a1.x, h1.x), __fsub_rn(a1.y, h1.y), __fsub_rn(a1.z, h1.z), __fsub_rn(a1.w, h1.w));
+                        __syncwarp();
+                        if (lane == 0) bar_arrive(&raw_empty[sr]);          // the raw row is in registers
+                        const int s = st % kStages;
+                        bar_wait(&empty[s], ((st / kStages) & 1) ^ 1);
+                        unsigned char* hi = stage_base + s * kStageBytes + lane_off;
+                        unsigned char* lo = hi + kStageHalf;
+                        *reinterpret_cast<float4*>(hi) = h0;
+                        *reinterpret_cast<float4*>(hi + 4 * 1024) = h1;
+                        *reinterpret_cast<float4*>(lo) = l0;
+                        *reinterpret_cast<float4*>(lo + 4 * 1024) = l1;
+                        fence_async_smem();
+                        __syncwarp();
+                        if (lane == 0) bar_arrive(&full[s]);
+                    }
+                }
+            }
+        }
+    } else {
+        // ================================================= builders =================================================
+        // W instances are built one ahead of the MMAs, alternating between two buffers (hi, lo and the union's ids):
+        // the build of half tile i + 1 overlaps the feature streaming, MMAs and epilogue of half tile i.
+        const int pw = warp - kFirstBuild;                // 0..7
+        const int ptid = tid - kFirstBuild * 32;          // 0..255
+        const uint32_t lt_mask = (1u << lane) - 1u;
+        auto prod_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kBuildThreads) : "memory"); };
+        int wb = 0;
         for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
             int x0, y0;
             half_origin(ht, x0, y0);
@@ -342,7 +394,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
             const int rounds = rounds_of(U);
             for (int c = 0; c < nunits; ++c) {
                 for (int r = 0; r < rounds; ++r) {
-                    const int ncols = cols_of(U, r);
                     if (c == 0 || rounds > 1) {
                         // ---------------- build W for columns [64 r, 64 r + 64) ----------------
                         // the loads of both groups of this warp are issued before anything waits on them
@@ -352,8 +403,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                         float4 wa[2], wb4[2];
                         float2 mt[2];
 #pragma unroll
-                        for (int gg = 0; gg < kGroupsPerProd; ++gg) {
-                            const int g = pw * kGroupsPerProd + gg;
+                        for (int gg = 0; gg < kGroupsPerBuild; ++gg) {
+                            const int g = pw * kGroupsPerBuild + gg;
                             const int gx = g & 3, gy = g >> 2;
                             const int64_t group = (int64_t)tile * kGroupsPerTile + half * 16 + g;
                             n_g[gg] = __ldg(p.gcount + group);
@@ -373,20 +424,22 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                                 res_g[gg] = __ldg(p.resid + pix);
                             }
                         }
-                        if (wb > 0) bar_wait(w_free, (wb - 1) & 1);
-                        ++wb;
+                        const int wcur = wb++;                     // this W instance; it lives in buffer wcur & 1
+                        bar_wait(&w_free[wcur & 1], ((wcur >> 1) & 1) ^ 1);        // the MMAs that read the buffer have retired
+                        unsigned char* wbuf = smem + MmaSmem::w + (wcur & 1) * 2 * kWBytes;
+                        int32_t* uid_w = uid_s + (wcur & 1) * kWCols;
 #pragma unroll
-                        for (int gg = 0; gg < kGroupsPerProd; ++gg)
+                        for (int gg = 0; gg < kGroupsPerBuild; ++gg)
                             inv_g[gg] = ns_g[gg] > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, res_g[gg])) : 0.0f;   // line 20; R8
                         {
                             const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-                            float4* wz = reinterpret_cast<float4*>(smem);
-                            for (int i = ptid; i < 2 * kWBytes / 16; i += kProdThreads) wz[i] = z;
+                            float4* wz = reinterpret_cast<float4*>(wbuf);
+                            for (int i = ptid; i < 2 * kWBytes / 16; i += kBuildThreads) wz[i] = z;
                         }
                         prod_sync();
 #pragma unroll
-                        for (int gg = 0; gg < kGroupsPerProd; ++gg) {
-                            const int g = pw * kGroupsPerProd + gg;                     // group 0..15 of the half tile
+                        for (int gg = 0; gg < kGroupsPerBuild; ++gg) {
+                            const int g = pw * kGroupsPerBuild + gg;                     // group 0..15 of the half tile
                             const int gx = g & 3, gy = g >> 2;
                             const int64_t group = (int64_t)tile * kGroupsPerTile + half * 16 + g;
                             const int n = n_g[gg];
@@ -412,7 +465,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                                 const int col = (int)(nzcol >> 8);
                                 const bool mine = have && (col / kWCols) == r;
                                 const int cl = col % kWCols;
-                                if (mine) uid_s[cl] = id;
+                                if (mine) uid_w[cl] = id;
 #pragma unroll
                                 for (int q = 0; q < kGroupPx; ++q) {
                                     const bool bit = (nz >> q) & 1u;
@@ -431,40 +484,15 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                                         const int m = (gy * 2 + (q >> 2)) * 16 + gx * 4 + (q & 3);
                                         const uint32_t off = w_off(m, cl);
                                         const float hi = tf32_hi(w[q]);
-                                        *reinterpret_cast<float*>(smem + MmaSmem::w_hi + off) = hi;
-                                        *reinterpret_cast<float*>(smem + MmaSmem::w_lo + off) = __fsub_rn(w[q], hi);
+                                        *reinterpret_cast<float*>(wbuf + off) = hi;
+                                        *reinterpret_cast<float*>(wbuf + kWBytes + off) = __fsub_rn(w[q], hi);
                                     }
                                 }
                             }
                         }
                         fence_async_smem();
                         prod_sync();
-                        if (ptid == 0) bar_arrive(w_ready);
-                    }
-                    // ---------------- feature rows of this round: warp pw converts channel half pw >> 3 of row pw & 7 ----------------
-                    const int nk = ksteps_of(ncols);
-                    const int row = pw & 7, ch = pw >> 3;
-                    // byte offset of this lane's 16 bytes inside a stage half: channels 128 ch + 4 lane .. + 3
-                    const uint32_t lane_off = (uint32_t)(ch * 4 * 1024 + (lane >> 3) * 1024 + (row >> 2) * 512 + (row & 3) * 128 +
-                                                         ((((lane & 7) >> 1) ^ (row & 3)) * 32) + (lane & 1) * 16);
-                    for (int j = 0; j < nk; ++j, ++st) {
-                        const int sr = st % kRawStages;
-                        bar_wait(&raw_full[sr], (st / kRawStages) & 1);
-                        float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (j * kStageRows + row < ncols)
-                            a0 = *reinterpret_cast<const float4*>(raw_base + sr * kRawBytes + row * kRawRow + ch * 512 + lane * 16);
-                        const float4 h0 = make_float4(tf32_hi(a0.x), tf32_hi(a0.y), tf32_hi(a0.z), tf32_hi(a0.w));
-                        const float4 l0 = make_float4(__fsub_rn(a0.x, h0.x), __fsub_rn(a0.y, h0.y), __fsub_rn(a0.z, h0.z), __fsub_rn(a0.w, h0.w));
-                        __syncwarp();
-                        if (lane == 0) bar_arrive(&raw_empty[sr]);          // the raw row is in registers
-                        const int s = st % kStages;
-                        bar_wait(&empty[s], ((st / kStages) & 1) ^ 1);
-                        unsigned char* hi = stage_base + s * kStageBytes + lane_off;
-                        *reinterpret_cast<float4*>(hi) = h0;
-                        *reinterpret_cast<float4*>(hi + kStageHalf) = l0;
-                        fence_async_smem();
-                        __syncwarp();
-                        if (lane == 0) bar_arrive(&full[s]);
+                        if (ptid == 0) bar_arrive(&w_ready[wcur & 1]);
                     }
                 }
             }
