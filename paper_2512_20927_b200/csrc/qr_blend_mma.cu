@@ -11,14 +11,17 @@
 // W_hi F_hi + W_lo F_hi + W_hi F_lo in fp32 (TMEM).  The dropped W_lo F_lo term and the truncation of the lo parts
 // are <= 2^-21 relative per product, 40x below the fp32 tolerance of north_star (1e-4 relative).
 //
-// One persistent CTA per SM, 14 warps, roles by warp (no role ever waits at a block barrier):
-//   warps 0..3   epilogue: tcgen05.ld of the accumulator (thread = pixel), x 1/(1 - T^Q), swizzled st.shared into a
-//                32-pixel x 32-channel staging tile, one TMA tensor store (cp.async.bulk.tensor.3d) per tile
-//   warp  4      one thread issues tcgen05.mma (M = 128 pixels, N = 256 channels, K = 8 union rows per instruction)
-//   warp  5      loader: one bulk async copy (TMA) per feature row half (1 KB) into a raw ring, far ahead of use
-//   warps 6..13  producers: build W (K-major, no swizzle) from walk_kernel's group records, write the per-pixel
-//                selection records, and convert raw feature rows: ld.shared -> hi/lo split -> st.shared in the
-//                MN-major SWIZZLE_128B_BASE32B layout tf32 needs for a row-major (channel-contiguous) B operand
+// One persistent CTA per SM, 22 warps, roles by warp (no role ever waits at a block barrier):
+//   warps 0..3    epilogue: tcgen05.ld of the accumulator (thread = pixel), x 1/(1 - T^Q), four 256-bit st.global per
+//                 32 channels (a lane's 32 channels are 128 contiguous bytes of the map)
+//   warp  4       MMA issue: warp-uniform loop, one elected lane issues tcgen05.mma (M = 128 pixels, N = 256 channels,
+//                 K = 8 union rows per instruction) and tcgen05.commit
+//   warp  5       loader: one bulk async copy (TMA) per feature row half (1 KB) into a raw ring, ahead of use
+//   warps 6..13   converters: ld.shared of a raw row -> hi/lo split -> st.shared in the MN-major
+//                 SWIZZLE_128B_BASE32B layout tf32 needs for a row-major (channel-contiguous) B operand
+//   warps 14..21  builders: W (K-major, no swizzle; hi and lo) from walk_kernel's group records, and the per-pixel
+//                 selection records.  W and the union's ids are double buffered: the build of half tile i + 1
+//                 overlaps the feature streaming, MMAs and epilogue of half tile i.
 // Work unit = (half tile, 256-channel half): two 256-column accumulators in TMEM, so the MMAs of unit i+1 overlap
 // the epilogue of unit i.  A half tile whose union exceeds 64 columns is processed in rounds of 64 columns.
 #include <cuda.h>
@@ -40,11 +43,10 @@ constexpr int kGroupsPerBuild = 16 / kBuildWarps;         // pixel groups of the
 constexpr int kWCols = 64;                                // union columns per round
 constexpr int kUnitN = 256;                               // channels per work unit
 constexpr int kStageRows = 8;                             // union rows per stage = one tf32 K step
-constexpr int kStages = 2;
+constexpr int kStages = 4;
 constexpr int kRawStages = 4;
 constexpr int kRawRow = kUnitN * 4;                       // 1 KB: one feature row half
 constexpr int kRawBytes = kStageRows * kRawRow;           // 8 KB per raw stage
-constexpr int kEpiTile = 32 * 32 * 4;                     // 4 KB: 32 pixels x 32 channels
 constexpr int kWBytes = 128 * kWCols * 4;                 // 32 KB per W buffer (hi, lo)
 constexpr int kStageHalf = kStageRows * kUnitN * 4;       // 8 KB (hi or lo)
 constexpr int kStageBytes = 2 * kStageHalf;
@@ -53,8 +55,7 @@ struct MmaSmem {
     static constexpr int w = 0;                                           // [2 buffers][hi, lo]
     static constexpr int stages = 4 * kWBytes;
     static constexpr int raw = stages + kStages * kStageBytes;
-    static constexpr int epi = raw + kRawStages * kRawBytes;              // [4 warps][2] staging tiles
-    static constexpr int uid = epi + kEpiWarps * 2 * kEpiTile;            // int32[2 buffers][kWCols]
+    static constexpr int uid = raw + kRawStages * kRawBytes;              // int32[2 buffers][kWCols]
     static constexpr int bars = uid + 2 * kWCols * 4;                     // uint64[...]
     static constexpr int n_bars = 2 * kStages + 2 * kRawStages + 4 + 4;
     static constexpr int tmem = bars + n_bars * 8;
@@ -128,7 +129,7 @@ __device__ __forceinline__ int rounds_of(int U) { return U <= kWCols ? 1 : (U + 
 __device__ __forceinline__ int cols_of(int U, int r) { return max(0, min(kWCols, U - r * kWCols)); }
 __device__ __forceinline__ int ksteps_of(int ncols) { return max(1, (ncols + kStageRows - 1) / kStageRows); }
 
-__global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tmap)
+__global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendParams p)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char* stage_base = smem + MmaSmem::stages;
@@ -176,12 +177,11 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
     if (warp < kEpiWarps) {
         // ================================================= epilogue =================================================
         // thread = pixel m = 32 warp + lane of the half tile (row-major 16 x 8): TMEM lane m, 256 columns = channels.
-        // 32 channels at a time: tcgen05.ld -> scale -> 8 swizzled 16-byte st.shared into a [32 px][128 B] tile ->
-        // one TMA tensor store of the box (32 channels, 16 x, 2 y); the tensor map clips pixels outside the image.
-        unsigned char* tile_s = smem + MmaSmem::epi + warp * 2 * kEpiTile;
-        const uint32_t row_off = (uint32_t)lane * 128u;
-        const uint32_t sw = (uint32_t)(lane & 7);
-        int unit = 0, nstore = 0;
+        // 32 channels at a time: tcgen05.ld -> scale -> four 256-bit st.global (a lane's 32 channels are 128
+        // contiguous bytes of the map, and every store instruction writes 32 whole sectors).  The first version
+        // staged the tile in shared memory for a TMA tensor store; with two staging tiles per warp the epilogue
+        // warps spent their time in cp.async.bulk.wait_group.read and became the critical path (profiles/README.md).
+        int unit = 0;
         auto ld32 = [&](uint32_t taddr, uint32_t (&r)[32]) {
             asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
                          : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
@@ -205,24 +205,19 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                 bar_wait(&tmem_full[buf], (unit >> 1) & 1);
                 tc_fence_after();
                 const uint32_t t0 = tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(buf * kUnitN);
+                float* orow = p.out_map + pix * D + c * kUnitN;
                 auto emit = [&](const uint32_t (&r)[32], int chunk) {
-                    unsigned char* tile = tile_s + (nstore & 1) * kEpiTile;
-                    if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the store that last read this tile is done
-                    __syncwarp();
+                    if (!valid) return;
+                    float* dst = orow + chunk * 32;
 #pragma unroll
-                    for (int jj = 0; jj < 8; ++jj)
-                        *reinterpret_cast<float4*>(tile + row_off + (((uint32_t)jj ^ sw) << 4)) =
-                            make_float4(__fmul_rn(__uint_as_float(r[4 * jj]), inv), __fmul_rn(__uint_as_float(r[4 * jj + 1]), inv),
-                                        __fmul_rn(__uint_as_float(r[4 * jj + 2]), inv), __fmul_rn(__uint_as_float(r[4 * jj + 3]), inv));
-                    fence_async_smem();
-                    __syncwarp();
-                    if (lane == 0) {
-                        asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];"
-                                     ::"l"(reinterpret_cast<uint64_t>(&out_tmap)), "r"(s_u32(tile)),
-                                       "r"(c * kUnitN + chunk * 32), "r"(x0), "r"(y0 + warp * 2) : "memory");
-                        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-                    }
-                    ++nstore;
+                    for (int jj = 0; jj < 4; ++jj)
+                        asm volatile("st.global.L1::no_allocate.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                                     ::"l"(dst + 8 * jj),
+                                       "f"(__fmul_rn(__uint_as_float(r[8 * jj]), inv)), "f"(__fmul_rn(__uint_as_float(r[8 * jj + 1]), inv)),
+                                       "f"(__fmul_rn(__uint_as_float(r[8 * jj + 2]), inv)), "f"(__fmul_rn(__uint_as_float(r[8 * jj + 3]), inv)),
+                                       "f"(__fmul_rn(__uint_as_float(r[8 * jj + 4]), inv)), "f"(__fmul_rn(__uint_as_float(r[8 * jj + 5]), inv)),
+                                       "f"(__fmul_rn(__uint_as_float(r[8 * jj + 6]), inv)), "f"(__fmul_rn(__uint_as_float(r[8 * jj + 7]), inv))
+                                     : "memory");
                 };
                 uint32_t ra[32], rb[32];
                 ld32(t0, ra);
@@ -242,7 +237,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                 }
             }
         }
-        if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     } else if (warp == kMmaWarp) {
         // ================================================= MMA issuer ===============================================
         // The whole warp runs the loop in uniform control flow (descriptors stay in uniform registers); one elected
@@ -506,23 +500,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
 
 bool blend_mma_supported(int32_t D, qr_dtype feat_dtype) { return feat_dtype == QR_F32 && D >= kUnitN && D % kUnitN == 0; }
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-static EncodeTiledFn encode_tiled_fn()
-{
-    static EncodeTiledFn fn = nullptr;
-    if (!fn) {
-        void* sym = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) == cudaSuccess &&
-            qres == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeTiledFn>(sym);
-    }
-    return fn;
-}
-
 int launch_blend_mma(const BlendParams& p, cudaStream_t st)
 {
     static int sms = 0;
@@ -531,21 +508,9 @@ int launch_blend_mma(const BlendParams& p, cudaStream_t st)
         if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
             sms = 148;
     }
-    // out_map [H][W][D] fp32 as a 3-D tensor (D, W, H); box = 32 channels x 16 pixels x 2 rows, 128-byte swizzle
-    EncodeTiledFn enc = encode_tiled_fn();
-    if (!enc) return fail(QR_ERR_CUDA, "qr_forward: cuTensorMapEncodeTiled is not available from the driver");
-    CUtensorMap tmap;
-    const cuuint64_t dims[3] = { (cuuint64_t)p.D, (cuuint64_t)p.cam.width, (cuuint64_t)p.cam.height };
-    const cuuint64_t strides[2] = { (cuuint64_t)p.D * 4, (cuuint64_t)p.D * 4 * (cuuint64_t)p.cam.width };
-    const cuuint32_t box[3] = { 32, 16, 2 };
-    const cuuint32_t estr[3] = { 1, 1, 1 };
-    const CUresult cr = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, p.out_map, dims, strides, box, estr,
-                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (cr != CUDA_SUCCESS) return fail(QR_ERR_CUDA, "qr_forward: cuTensorMapEncodeTiled failed (%d)", (int)cr);
     const unsigned grid = (unsigned)min(sms, p.num_tiles * 2);
     QR_CUDA_OK(cudaFuncSetAttribute(blend_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MmaSmem::total));
-    blend_mma_kernel<<<grid, kMmaThreads, MmaSmem::total, st>>>(p, tmap);
+    blend_mma_kernel<<<grid, kMmaThreads, MmaSmem::total, st>>>(p);
     QR_LAUNCH_OK("blend_mma_kernel");
     return QR_OK;
 }
