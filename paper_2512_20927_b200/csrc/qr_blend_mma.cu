@@ -43,8 +43,8 @@ constexpr int kGroupsPerBuild = 16 / kBuildWarps;         // pixel groups of the
 constexpr int kWCols = 64;                                // union columns per round
 constexpr int kUnitN = 256;                               // channels per work unit
 constexpr int kStageRows = 8;                             // union rows per stage = one tf32 K step
-constexpr int kStages = 4;
-constexpr int kRawStages = 4;
+constexpr int kStages = 2;
+constexpr int kRawStages = 8;
 constexpr int kRawRow = kUnitN * 4;                       // 1 KB: one feature row half
 constexpr int kRawBytes = kStageRows * kRawRow;           // 8 KB per raw stage
 constexpr int kWBytes = 128 * kWCols * 4;                 // 32 KB per W buffer (hi, lo)
@@ -379,11 +379,34 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
         const uint32_t lt_mask = (1u << lane) - 1u;
         auto prod_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kBuildThreads) : "memory"); };
         int wb = 0;
+        auto prefetch_l2 = [](const void* a) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a)); };
         for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
             int x0, y0;
             half_origin(ht, x0, y0);
             if (y0 >= p.cam.height) continue;
             const int tile = ht >> 1, half = ht & 1;
+            {   // what the build of this CTA's next half tile reads (written by walk_kernel, long evicted by the map
+                // stream): fetch it into L2 now, a whole half tile ahead of its use
+                const int hn = ht + (int)gridDim.x;
+                int xn, yn;
+                half_origin(hn < num_half ? hn : ht, xn, yn);
+                if (hn < num_half && yn < p.cam.height) {
+                    if (pw == 0 && lane == 0) prefetch_l2(p.ucount + hn);
+#pragma unroll
+                    for (int gg = 0; gg < kGroupsPerBuild; ++gg) {
+                        const int g = pw * kGroupsPerBuild + gg;
+                        const int64_t group = (int64_t)(hn >> 1) * kGroupsPerTile + (hn & 1) * 16 + g;
+                        if (lane == 0) prefetch_l2(p.gcount + group);
+                        const float* recs = p.rec + group * p.cap * kRecWords;
+                        if (lane * 128 < min(p.cap, 32) * kRecWords * 4) prefetch_l2(reinterpret_cast<const char*>(recs) + lane * 128);
+                        const int qx = xn + (g & 3) * 4 + (lane & 3), qy = yn + (g >> 2) * 2 + ((lane >> 2) & 1);
+                        if (lane < kGroupPx && qx < p.cam.width && qy < p.cam.height) {
+                            prefetch_l2(p.n_sel + (int64_t)qy * p.cam.width + qx);
+                            prefetch_l2(p.resid + (int64_t)qy * p.cam.width + qx);
+                        }
+                    }
+                }
+            }
             const int U = __ldg(p.ucount + ht);
             const int rounds = rounds_of(U);
             for (int c = 0; c < nunits; ++c) {
