@@ -199,25 +199,108 @@ tile_scan_kernel(uint32_t* __restrict__ counter, int32_t T, int32_t* __restrict_
     }
 }
 
-// bitonic network over n2 (a power of two) keys in shared memory; every thread of the block takes part
+// bitonic network over n2 (a power of two, >= 32 per warp) keys in shared memory; every thread of the block takes
+// part.  Warp w owns the contiguous chunk [w n2 / W, (w + 1) n2 / W): a compare-exchange step of stride j < chunk
+// stays inside the chunk and needs only __syncwarp; block barriers remain for the log2(W) largest strides of a merge
+// (6 of the 45 steps at n2 = 512 with 8 warps) -- the network was bound by barrier stalls before (profiles/README.md).
 __device__ __forceinline__ void bitonic_sort_smem(uint64_t* s, int n2)
 {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int chunk = min(max(n2 / nwarps, 64), n2);        // keys per warp-local chunk (a power of two)
+    const int nchunks = n2 / chunk;                         // <= nwarps; warps beyond it idle in the local steps
+    bool local_before = false;
     for (int k = 2; k <= n2; k <<= 1) {
         for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int idx = threadIdx.x; idx < (n2 >> 1); idx += blockDim.x) {
-                const int i = ((idx & ~(j - 1)) << 1) | (idx & (j - 1));
-                const int l = i | j;
-                const uint64_t a = s[i], b = s[l];
-                if ((a > b) == ((i & k) == 0)) { s[i] = b; s[l] = a; }
+            if (j >= chunk) {                               // pairs span chunks: whole block, block barrier
+                if (local_before) __syncthreads();
+                for (int idx = threadIdx.x; idx < (n2 >> 1); idx += blockDim.x) {
+                    const int i = ((idx & ~(j - 1)) << 1) | (idx & (j - 1));
+                    const int l = i | j;
+                    const uint64_t a = s[i], b = s[l];
+                    if ((a > b) == ((i & k) == 0)) { s[i] = b; s[l] = a; }
+                }
+                __syncthreads();
+                local_before = false;
+            } else {
+                if (warp < nchunks) {
+                    const int base = warp * chunk;
+                    for (int idx = lane; idx < (chunk >> 1); idx += 32) {
+                        const int i = base + (((idx & ~(j - 1)) << 1) | (idx & (j - 1)));
+                        const int l = i | j;
+                        const uint64_t a = s[i], b = s[l];
+                        if ((a > b) == ((i & k) == 0)) { s[i] = b; s[l] = a; }
+                    }
+                }
+                __syncwarp();
+                local_before = true;
             }
-            __syncthreads();
         }
     }
+    __syncthreads();
 }
 
 constexpr int kSmallBucket = 2048;          // keys sorted by tile_sort_kernel<small> (16 KB of shared memory)
 constexpr int kBigBucket = 16384;           // keys per shared-memory run of tile_sort_kernel<big> (128 KB)
 constexpr uint64_t kKeyInf = ~uint64_t(0);
+
+// Register-blocked bitonic network for one bucket of 256 E keys (E = 1, 2, 4, 8) on 256 threads: thread t holds keys
+// t E .. t E + E - 1.  Strides below E are compare-exchanges inside a thread, strides below 32 E are exchanged with
+// __shfl_xor, and only the three largest strides of the last three merges (6 steps of the 36..66) go through shared
+// memory.  The all-shared-memory network (still used for the big buckets) was bound by shared-memory wavefronts.
+template <int E>
+__device__ __forceinline__ void bitonic_sort_regs(const uint64_t* __restrict__ keys, int n, uint32_t* __restrict__ out,
+                                                  uint64_t* s)
+{
+    const int t = threadIdx.x;
+    uint64_t v[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) v[e] = t * E + e < n ? keys[t * E + e] : kKeyInf;
+    constexpr int n2 = 256 * E;
+#pragma unroll 1
+    for (int k = 2; k <= n2; k <<= 1) {
+#pragma unroll 1
+        for (int j = k >> 1; j >= E; j >>= 1) {             // strides across threads
+            if (j < 32 * E) {
+                const int lm = j / E;
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    const int i = t * E + e;
+                    const uint64_t o = __shfl_xor_sync(0xffffffffu, v[e], lm);
+                    const bool keep_min = ((i & j) == 0) == ((i & k) == 0);
+                    v[e] = keep_min ? min(v[e], o) : max(v[e], o);
+                }
+            } else {
+#pragma unroll
+                for (int e = 0; e < E; ++e) s[t * E + e] = v[e];
+                __syncthreads();
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    const int i = t * E + e;
+                    const uint64_t o = s[i ^ j];
+                    const bool keep_min = ((i & j) == 0) == ((i & k) == 0);
+                    v[e] = keep_min ? min(v[e], o) : max(v[e], o);
+                }
+                __syncthreads();
+            }
+        }
+#pragma unroll
+        for (int j = E / 2; j > 0; j >>= 1) {               // strides inside a thread: compile-time register indices
+            if (j < k) {
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    if ((e & j) == 0) {
+                        const int i = t * E + e;
+                        const uint64_t a = v[e], b = v[e | j];
+                        if ((a > b) == ((i & k) == 0)) { v[e] = b; v[e | j] = a; }
+                    }
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int e = 0; e < E; ++e)
+        if (t * E + e < n) out[t * E + e] = (uint32_t)v[e];
+}
 
 // One CTA per tile.  BIG = false handles buckets of <= kSmallBucket keys (several CTAs per SM), BIG = true the rest:
 // up to kBigBucket keys in one shared-memory run; beyond that, runs of kBigBucket keys are sorted one by one and every
@@ -230,6 +313,13 @@ __device__ __forceinline__ void tile_sort_one(const int tile, const int32_t* __r
     const int start = tile_range[2 * tile], n = tile_range[2 * tile + 1] - start;
     if (BIG ? (n <= kSmallBucket) : (n <= 0 || n > kSmallBucket)) return;
     constexpr int kRun = BIG ? kBigBucket : kSmallBucket;
+    if (!BIG && n > 128) {                      // 256 threads, keys in registers
+        if (n <= 256) bitonic_sort_regs<1>(keys + start, n, isect_gauss + start, skeys);
+        else if (n <= 512) bitonic_sort_regs<2>(keys + start, n, isect_gauss + start, skeys);
+        else if (n <= 1024) bitonic_sort_regs<4>(keys + start, n, isect_gauss + start, skeys);
+        else bitonic_sort_regs<8>(keys + start, n, isect_gauss + start, skeys);
+        return;
+    }
     if (n <= kRun) {
         int n2 = 32;
         while (n2 < n) n2 <<= 1;
