@@ -19,8 +19,8 @@
 //   warp  5       loader: one bulk async copy (TMA) per feature row half (1 KB) into a raw ring, ahead of use
 //   warps 6..13   converters: ld.shared of a raw row -> hi/lo split -> st.shared in the MN-major
 //                 SWIZZLE_128B_BASE32B layout tf32 needs for a row-major (channel-contiguous) B operand
-//   warps 14..21  builders: W (K-major, no swizzle; hi and lo) from walk_kernel's group records, and the per-pixel
-//                 selection records.  W and the union's ids are double buffered: the build of half tile i + 1
+//   warps 14..21  builders: W (K-major, no swizzle; hi and lo) from walk_kernel's group records (walk_kernel also writes
+//                 the per-pixel selection records itself).  W and the union's ids are double buffered: the build of half tile i + 1
 //                 overlaps the feature streaming, MMAs and epilogue of half tile i.
 // Work unit = (half tile, 256-channel half): two 256-column accumulators in TMEM, so the MMAs of unit i+1 overlap
 // the epilogue of unit i.  A half tile whose union exceeds 64 columns is processed in rounds of 64 columns.
@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + MmaSmem::tmem);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int D = p.D, K = p.K;
+    const int D = p.D;
     const int nunits = D / kUnitN;
     const int num_half = p.num_tiles * 2;
 
@@ -376,7 +376,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
         // the build of half tile i + 1 overlaps the feature streaming, MMAs and epilogue of half tile i.
         const int pw = warp - kFirstBuild;                // 0..7
         const int ptid = tid - kFirstBuild * 32;          // 0..255
-        const uint32_t lt_mask = (1u << lane) - 1u;
         auto prod_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kBuildThreads) : "memory"); };
         int wb = 0;
         auto prefetch_l2 = [](const void* a) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a)); };
@@ -399,11 +398,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                         if (lane == 0) prefetch_l2(p.gcount + group);
                         const float* recs = p.rec + group * p.cap * kRecWords;
                         if (lane * 128 < min(p.cap, 32) * kRecWords * 4) prefetch_l2(reinterpret_cast<const char*>(recs) + lane * 128);
-                        const int qx = xn + (g & 3) * 4 + (lane & 3), qy = yn + (g >> 2) * 2 + ((lane >> 2) & 1);
-                        if (lane < kGroupPx && qx < p.cam.width && qy < p.cam.height) {
-                            prefetch_l2(p.n_sel + (int64_t)qy * p.cam.width + qx);
-                            prefetch_l2(p.resid + (int64_t)qy * p.cam.width + qx);
-                        }
                     }
                 }
             }
@@ -414,15 +408,12 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                     if (c == 0 || rounds > 1) {
                         // ---------------- build W for columns [64 r, 64 r + 64) ----------------
                         // the loads of both groups of this warp are issued before anything waits on them
-                        const bool write_sel = (c == 0 && r == 0);
-                        int n_g[2], ns_g[2];
-                        float inv_g[2], res_g[2];
+                        int n_g[2];
                         float4 wa[2], wb4[2];
                         float2 mt[2];
 #pragma unroll
                         for (int gg = 0; gg < kGroupsPerBuild; ++gg) {
                             const int g = pw * kGroupsPerBuild + gg;
-                            const int gx = g & 3, gy = g >> 2;
                             const int64_t group = (int64_t)tile * kGroupsPerTile + half * 16 + g;
                             n_g[gg] = __ldg(p.gcount + group);
                             const float* recs = p.rec + group * p.cap * kRecWords;
@@ -433,21 +424,11 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                                 wb4[gg] = __ldg(reinterpret_cast<const float4*>(recs + (size_t)lane * kRecWords + 4));
                                 mt[gg] = __ldg(reinterpret_cast<const float2*>(recs + (size_t)lane * kRecWords + 8));
                             }
-                            const int qx = x0 + gx * 4 + (lane & 3), qy = y0 + gy * 2 + ((lane >> 2) & 1);
-                            ns_g[gg] = 0; res_g[gg] = 0.0f;           // both loads issued at once, used after the wait below
-                            if (write_sel && lane < kGroupPx && qx < p.cam.width && qy < p.cam.height) {
-                                const int64_t pix = (int64_t)qy * p.cam.width + qx;
-                                ns_g[gg] = __ldg(p.n_sel + pix);
-                                res_g[gg] = __ldg(p.resid + pix);
-                            }
                         }
                         const int wcur = wb++;                     // this W instance; it lives in buffer wcur & 1
                         bar_wait(&w_free[wcur & 1], ((wcur >> 1) & 1) ^ 1);        // the MMAs that read the buffer have retired
                         unsigned char* wbuf = smem + MmaSmem::w + (wcur & 1) * 2 * kWBytes;
                         int32_t* uid_w = uid_s + (wcur & 1) * kWCols;
-#pragma unroll
-                        for (int gg = 0; gg < kGroupsPerBuild; ++gg)
-                            inv_g[gg] = ns_g[gg] > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, res_g[gg])) : 0.0f;   // line 20; R8
                         {
                             const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
                             float4* wz = reinterpret_cast<float4*>(wbuf);
@@ -461,10 +442,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                             const int64_t group = (int64_t)tile * kGroupsPerTile + half * 16 + g;
                             const int n = n_g[gg];
                             const float* recs = p.rec + group * p.cap * kRecWords;
-                            const float inv_l = inv_g[gg];
-                            int base[kGroupPx];
-#pragma unroll
-                            for (int q = 0; q < kGroupPx; ++q) base[q] = 0;
                             for (int i0 = 0; i0 < n; i0 += 32) {
                                 const int i = i0 + lane;
                                 const bool have = i < n;
@@ -486,17 +463,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
 #pragma unroll
                                 for (int q = 0; q < kGroupPx; ++q) {
                                     const bool bit = (nz >> q) & 1u;
-                                    if (write_sel) {
-                                        const uint32_t bal = __ballot_sync(0xffffffffu, bit);
-                                        const float inv_q = __shfl_sync(0xffffffffu, inv_l, q);
-                                        if (bit) {
-                                            const int slot = base[q] + __popc(bal & lt_mask);
-                                            const int64_t pix = (int64_t)(y0 + gy * 2 + (q >> 2)) * p.cam.width + (x0 + gx * 4 + (q & 3));
-                                            p.sel_idx[pix * K + slot] = id;
-                                            p.sel_w[pix * K + slot] = __fmul_rn(w[q], inv_q);
-                                        }
-                                        base[q] += __popc(bal);
-                                    }
                                     if (mine && bit) {
                                         const int m = (gy * 2 + (q >> 2)) * 16 + gx * 4 + (q & 3);
                                         const uint32_t off = w_off(m, cl);

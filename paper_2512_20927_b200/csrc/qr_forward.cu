@@ -56,7 +56,7 @@ struct WalkParams {
     const int2* tile_range;
     int32_t* n_sel;
     float* resid;
-    int32_t* sel_idx;     // only the padding (slots >= n_sel) is written here
+    int32_t* sel_idx;     // written here: used slots from the group records after the walk, then the -1 / 0 padding
     float* sel_w;
     int32_t* gcount;
     int32_t* ucount;      // [2 T] union size of each 16x8 half tile
@@ -64,7 +64,7 @@ struct WalkParams {
     int32_t* tile_ticket; // blend_kernel's tile queue, reset here
 };
 
-__global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
+__global__ void __launch_bounds__(kWalkThreads, 5) walk_kernel(const WalkParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4* ent_co = reinterpret_cast<float4*>(smem_raw);                 // [256] a, b, c, opacity
@@ -205,8 +205,53 @@ __global__ void __launch_bounds__(kWalkThreads) walk_kernel(const WalkParams p)
         p.n_sel[pix] = ns;
         p.resid[pix] = ns > 0 ? TQ : 1.0f;              // R8
     }
+    // ---- selection records of the used slots, from the four group lists this warp has just written: lane = record,
+    // a ballot per pixel ranks the records that selected it (its slot, depth order), weight x 1 / (1 - T^Q) (line 20).
+    // Done here, at full occupancy, rather than by the W builders of the persistent blend kernel, whose ~1,100
+    // dependent instructions per build were that kernel's critical path (profiles/README.md, r1_d). ----
+    {
+        const float inv = ns > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, TQ)) : 0.0f;
+        const uint32_t lt_mask = (1u << lane) - 1u;
+        __syncwarp();
+#pragma unroll 1
+        for (int g4 = 0; g4 < 4; ++g4) {
+            const int n = __shfl_sync(0xffffffffu, gcnt, g4 * 4);                   // lane g4 * 4 belongs to group g4
+            const float* recs = p.rec + ((int64_t)tile * kGroupsPerTile + warp * 4 + g4) * p.cap * kRecWords;
+            int base[kGroupPx];
+#pragma unroll
+            for (int j = 0; j < kGroupPx; ++j) base[j] = 0;
+            for (int i0 = 0; i0 < n; i0 += 32) {
+                const int i = i0 + lane;
+                const bool have = i < n;
+                float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+                float2 m2 = make_float2(0.f, 0.f);
+                if (have) {
+                    a = *reinterpret_cast<const float4*>(recs + (size_t)i * kRecWords);
+                    b = *reinterpret_cast<const float4*>(recs + (size_t)i * kRecWords + 4);
+                    m2 = *reinterpret_cast<const float2*>(recs + (size_t)i * kRecWords + 8);
+                }
+                const float w[kGroupPx] = { a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w };
+                const int32_t id = __float_as_int(m2.x);
+                const uint32_t nz = have ? ((uint32_t)__float_as_int(m2.y) & 0xFFu) : 0u;
+#pragma unroll
+                for (int j = 0; j < kGroupPx; ++j) {
+                    const bool bit = (nz >> j) & 1u;
+                    const uint32_t bal = __ballot_sync(0xffffffffu, bit);
+                    const int pl = (j >> 2) * 16 + g4 * 4 + (j & 3);                 // lane that owns pixel j of group g4
+                    const float inv_j = __shfl_sync(0xffffffffu, inv, pl);
+                    const int qx = tile_x * kTile + (pl & 15), qy = tile_y * kTile + warp * 2 + (pl >> 4);
+                    if (bit && qx < p.cam.width && qy < p.cam.height) {
+                        const int64_t o = ((int64_t)qy * p.cam.width + qx) * K + base[j] + __popc(bal & lt_mask);
+                        p.sel_idx[o] = id;
+                        p.sel_w[o] = __fmul_rn(w[j], inv_j);
+                    }
+                    base[j] += __popc(bal);
+                }
+            }
+        }
+    }
     // ---- padding of the selection records (-1 / 0 for slots >= n_sel), coalesced: a tile row is 16*K contiguous
-    // words of sel_idx / sel_w.  The used slots are written by blend_kernel (it knows 1/(1 - T^Q) by then). ----
+    // words of sel_idx / sel_w. ----
     nsel_s[warp * 32 + lane] = ns;                      // index = (2*warp + (lane>>4))*16 + (lane&15) = y_local*16 + x_local
     __syncthreads();
     if (tid < 2) p.ucount[tile * 2 + tid] = ucount_s[tid];
