@@ -342,7 +342,7 @@ def run_cuda(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture named in profiles/ (None
 # until a capture of the current kernels is committed).
-TRAFFIC = {"qr_forward": 868.7e6, "qr_backward": 818.2e6}   # profiles/r1_c_full_metrics.csv (walk + blend; prep + mma)
+TRAFFIC = {"qr_forward": 824.0e6, "qr_backward": 818.3e6}   # profiles/r1_d_full_metrics.csv (walk + blend; prep + mma)
 
 
 def main():
