@@ -324,6 +324,60 @@ def test_config3_full_size_sampled(qr, orc):
         assert (np.abs(got - ref) <= tol).all(), float((np.abs(got - ref) / tol).max())
 
 
+def _full_size_check(qr, orc, sc, Ks, n_pix=3000, n_rows=150, f16=False):
+    """Full-size frame in bench.py's launch configuration: selection parity on every pixel, features on sampled
+    pixels, gradient rows of sampled Gaussians (the oracle computes those one by one)."""
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    rect, touched = orc.tile_rects(sc.cam, proj)
+    assert fe.M == int(touched.sum())
+    lists = orc.pixel_lists(sc.cam, proj)
+    rng = np.random.default_rng(1)
+    pix = np.sort(rng.choice(sc.cam.width * sc.cam.height, size=n_pix, replace=False))
+    G = P.to_dev(sc.dL_dmap) if sc.dL_dmap is not None else None
+    for K in Ks:
+        out = qr.pipeline.forward(sc.cam, fe, g.features, K)
+        q = orc.qrender(lists, K, sc.features, pixels=pix)
+        stats = P.compare_forward(out, q, lists, K, sc.D, f16=f16, pixels=pix)
+        qa = orc.qrender(lists, K, None)
+        ex = P.exempt_mask(qa, lists)
+        same = (out.sel_idx.cpu().numpy().reshape(-1, K) == qa.sel_idx).all(1)
+        assert ((~same) & (~ex)).sum() == 0
+        print(sc.name, "K", K, "sampled:", stats, "all pixels: exempt", int(ex.sum()), "mismatching exempt", int(((~same) & ex).sum()))
+        if G is not None and K == Ks[-1]:
+            dF = qr.pipeline.backward(sc.cam, sc.N, out, G)
+            sel = qa.sel_idx[qa.sel_idx >= 0]
+            rows = np.unique(sel)
+            rows = rows[:: max(1, len(rows) // n_rows)][:n_rows].astype(np.int64)
+            ref = orc.backward(qa.sel_idx, qa.sel_w, qa.n_sel, sc.dL_dmap, sc.N, rows=rows)
+            got = dF[torch.from_numpy(rows).cuda()].cpu().numpy().astype(np.float64)
+            if same.all():
+                tol = P.ATOL + P.RTOL * np.abs(ref)
+                assert (np.abs(got - ref) <= tol).all(), float((np.abs(got - ref) / tol).max())
+            del dF
+        del out
+
+
+def test_config5_full_size_sampled(qr, orc):
+    """BASELINE.json configs[4]: 1280x720, 1,000,000 Gaussians, D = 512 fp32, K = 40, forward + backward."""
+    _full_size_check(qr, orc, make_scene("cfg5", seed=0), [40])
+
+
+def test_config5_narrow_payload_full_size(qr, orc):
+    """configs[4] D sweep, D = 64: the first 64 columns of the 512-D draw, re-normalised (FFMA blend / backward paths)."""
+    sc = make_scene("cfg5", seed=0, D=64)
+    _full_size_check(qr, orc, sc, [40], n_pix=2000, n_rows=100)
+
+
+def test_config4_full_size_sampled(qr, orc):
+    """BASELINE.json configs[3]: 1024x768, 2,000,000 Gaussians, D = 512 stored fp16 (fp32 accumulation), pose 0 of the
+    radius-3 circle, K = 4 and K = 32."""
+    sc = make_scene("cfg4", seed=0, pose=0)
+    assert sc.features.dtype == np.float16
+    _full_size_check(qr, orc, sc, [4, 32], n_pix=2000, n_rows=100, f16=True)
+
+
 # ------------------------------------------------------------------------------------------------
 # argument errors are status codes, not crashes
 # ------------------------------------------------------------------------------------------------
