@@ -93,11 +93,17 @@ int qr_bin_count(int64_t N, const uint32_t* tiles_touched, uint64_t* offsets, in
 /*
  * qr_bin_sort -- duplication + sort + ranges ("ordered sequence of indices"; SPEC.md:139-147,
  * :167-168; reading R6: order = ascending depth, ties by ascending Gaussian index).
- * Each un-culled Gaussian emits one 64-bit key (tile id << 32 | IEEE bits of depth) per tile of its rectangle;
- * keys are sorted by a stable LSD radix sort written here (8-bit digits, only the used key bits).
- *   in : depth[N], tile_rect[N,4], offsets[N] (from qr_bin_count), M (from qr_bin_count)
+ * Each un-culled Gaussian emits one entry per tile of its rectangle.  One most-significant-digit radix pass over the
+ * tile field (count, scan, scatter: a counting sort with one bucket per tile) is followed by a sort of every bucket
+ * on its 64-bit (IEEE bits of depth << 32 | Gaussian id) keys; the keys are unique, so the result does not depend on
+ * the order the buckets were filled in.
+ *   in : depth[N], tile_rect[N,4]; M = capacity of isect_gauss: the exact count from qr_bin_count, or any upper
+ *        bound (e.g. from the previous frame) when the caller wants no host synchronisation; offsets is unused by
+ *        this implementation and may be NULL.
  *   out: isect_gauss[M] Gaussian ids sorted by (tile, depth, id); tile_range[T,2] = [start, end) of tile t in
- *        isect_gauss (empty tile: start == end == number of intersections in tiles < t).
+ *        isect_gauss (empty tile: start == end == number of intersections in tiles < t);
+ *        ((int64_t*)ws)[0] = number of intersections found.  If it exceeds M the lists are truncated at M entries
+ *        (ranges clamped, nothing is written out of bounds): call again with a larger M.
  * ws must hold qr_bin_workspace_bytes(N, M, T) bytes.  M = 0 is legal (ranges are all [0,0)).
  */
 int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M,

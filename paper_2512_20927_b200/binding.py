@@ -172,9 +172,12 @@ def qr_bin_count(tiles_touched: torch.Tensor, ws: Optional[torch.Tensor] = None)
     return offsets, int(m.value)
 
 
-def qr_bin_sort(cam, M: int, depth, tile_rect, offsets, ws: Optional[torch.Tensor] = None,
-                isect_gauss: Optional[torch.Tensor] = None, tile_range: Optional[torch.Tensor] = None):
-    """Returns (isect_gauss[M] int32 bits of the uint32 ids, tile_range[T,2] int32)."""
+def qr_bin_sort(cam, M: int, depth, tile_rect, offsets=None, ws: Optional[torch.Tensor] = None,
+                isect_gauss: Optional[torch.Tensor] = None, tile_range: Optional[torch.Tensor] = None,
+                return_found: bool = False):
+    """Returns (isect_gauss[M] int32 bits of the uint32 ids, tile_range[T,2] int32).  M is the exact count from
+    qr_bin_count or an upper bound (no host synchronisation needed then); with return_found also a 1-element int64
+    DEVICE tensor = the number of intersections found (> M: the lists are truncated, call again with a larger M)."""
     c = make_camera(cam)
     n = int(depth.shape[0])
     dev = depth.device
@@ -185,9 +188,14 @@ def qr_bin_sort(cam, M: int, depth, tile_rect, offsets, ws: Optional[torch.Tenso
         tile_range = torch.empty((T, 2), dtype=torch.int32, device=dev)
     if ws is None:
         ws = torch.empty((max(qr_bin_workspace_bytes(n, M, T), 16),), dtype=torch.uint8, device=dev)
+    if M == 0:
+        ws[:8].zero_()
+    off_ptr = None if offsets is None else _dev(offsets, torch.int64, "offsets")
     _check(load().qr_bin_sort(C.byref(c), n, int(M), _dev(depth, torch.float32, "depth"),
-                              _dev(tile_rect, torch.int32, "tile_rect"), _dev(offsets, torch.int64, "offsets"),
+                              _dev(tile_rect, torch.int32, "tile_rect"), off_ptr,
                               isect_gauss.data_ptr(), tile_range.data_ptr(), ws.data_ptr(), ws.numel(), _stream()))
+    if return_found:
+        return isect_gauss[:M], tile_range, ws[:8].view(torch.int64)
     return isect_gauss[:M], tile_range
 
 

@@ -113,7 +113,7 @@ constexpr int kSubBuckets = 16;
 template <bool SCATTER>
 __global__ void __launch_bounds__(256)
 tile_bucket_kernel(int64_t N, int32_t tiles_x, const float* __restrict__ depth, const int4* __restrict__ tile_rect,
-                   uint32_t* __restrict__ counter, uint64_t* __restrict__ keys)
+                   uint32_t* __restrict__ counter, uint64_t* __restrict__ keys, uint32_t capacity)
 {
     const int lane = threadIdx.x & 31;
     const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x - lane);   // first Gaussian of this warp
@@ -138,7 +138,10 @@ tile_bucket_kernel(int64_t N, int32_t tiles_x, const float* __restrict__ depth, 
         for (uint32_t j = lane; j < c; j += 32) {
             const int ty = y0 + (int)(j / (uint32_t)ww), tx = x0 + (int)(j % (uint32_t)ww);
             const int slot = (ty * tiles_x + tx) * kSubBuckets + (int)((uint32_t)(warp0 + src) % kSubBuckets);
-            if (SCATTER) keys[atomicAdd(&counter[slot], 1u)] = key;
+            if (SCATTER) {
+                const uint32_t pos = atomicAdd(&counter[slot], 1u);
+                if (pos < capacity) keys[pos] = key;           // M was only an upper bound and it was too small: dropped
+            }
             else atomicAdd(&counter[slot], 1u);
         }
     }
@@ -147,7 +150,8 @@ tile_bucket_kernel(int64_t N, int32_t tiles_x, const float* __restrict__ depth, 
 // one block of 1024 threads, thread = tile: exclusive scan of the T * kSubBuckets slot counts -> cursors in place;
 // tile_range[t] = [cursor of the tile's first slot, end of its last slot)
 __global__ void __launch_bounds__(1024)
-tile_scan_kernel(uint32_t* __restrict__ counter, int32_t T, int32_t* __restrict__ tile_range)
+tile_scan_kernel(uint32_t* __restrict__ counter, int32_t T, int32_t* __restrict__ tile_range, uint32_t capacity,
+                 int64_t* __restrict__ found)
 {
     static_assert(kSubBuckets % 4 == 0, "slots are read as uint4");
     __shared__ uint32_t warp_sums[32];
@@ -183,8 +187,8 @@ tile_scan_kernel(uint32_t* __restrict__ counter, int32_t T, int32_t* __restrict_
         __syncthreads();
         uint32_t run = carry + wbase + inc - s;
         if (t < T) {
-            tile_range[2 * t] = (int32_t)run;
-            tile_range[2 * t + 1] = (int32_t)(run + s);
+            tile_range[2 * t] = (int32_t)min(run, capacity);            // lists are truncated at the caller's capacity
+            tile_range[2 * t + 1] = (int32_t)min(run + s, capacity);
 #pragma unroll
             for (int j = 0; j < kSubBuckets / 4; ++j) {
                 uint4 q;
@@ -197,6 +201,7 @@ tile_scan_kernel(uint32_t* __restrict__ counter, int32_t T, int32_t* __restrict_
         }
         carry += tot;
     }
+    if (threadIdx.x == 0) *found = (int64_t)carry;                       // intersections found (> capacity: truncated)
 }
 
 // bitonic network over n2 (a power of two, >= 32 per warp) keys in shared memory; every thread of the block takes
@@ -306,11 +311,12 @@ __device__ __forceinline__ void bitonic_sort_regs(const uint64_t* __restrict__ k
 // up to kBigBucket keys in one shared-memory run; beyond that, runs of kBigBucket keys are sorted one by one and every
 // key is then ranked against the other runs by binary search (keys are unique, so ranks are a permutation).
 template <bool BIG>
-__device__ __forceinline__ void tile_sort_one(const int tile, const int32_t* __restrict__ tile_range,
+__device__ __forceinline__ void tile_sort_one(const int tile, const int capacity, const int32_t* __restrict__ tile_range,
                                               uint64_t* __restrict__ keys, uint64_t* __restrict__ scratch,
                                               uint32_t* __restrict__ isect_gauss, uint64_t* skeys)
 {
-    const int start = tile_range[2 * tile], n = tile_range[2 * tile + 1] - start;
+    const int start = tile_range[2 * tile];
+    const int n = min(tile_range[2 * tile + 1], capacity) - start;      // capacity: see qr_bin_sort (M as an upper bound)
     if (BIG ? (n <= kSmallBucket) : (n <= 0 || n > kSmallBucket)) return;
     constexpr int kRun = BIG ? kBigBucket : kSmallBucket;
     if (!BIG && n > 128) {                      // 256 threads, keys in registers
@@ -368,11 +374,11 @@ __device__ __forceinline__ void tile_sort_one(const int tile, const int32_t* __r
 // and skipped, and a CTA of this kernel owns 128 KB of shared memory).
 template <bool BIG>
 __global__ void __launch_bounds__(BIG ? 1024 : 256)
-tile_sort_kernel(const int32_t* __restrict__ tile_range, int32_t T, uint64_t* __restrict__ keys,
+tile_sort_kernel(const int32_t* __restrict__ tile_range, int32_t T, int32_t capacity, uint64_t* __restrict__ keys,
                  uint64_t* __restrict__ scratch, uint32_t* __restrict__ isect_gauss)
 {
     extern __shared__ __align__(16) uint64_t skeys[];
-    for (int tile = blockIdx.x; tile < T; tile += gridDim.x) tile_sort_one<BIG>(tile, tile_range, keys, scratch, isect_gauss, skeys);
+    for (int tile = blockIdx.x; tile < T; tile += gridDim.x) tile_sort_one<BIG>(tile, capacity, tile_range, keys, scratch, isect_gauss, skeys);
 }
 
 struct BinLayout {
@@ -447,7 +453,8 @@ extern "C" int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M, const flo
         QR_CUDA_OK(cudaMemsetAsync(tile_range, 0, sizeof(int32_t) * 2 * (size_t)T, st));
         return QR_OK;
     }
-    if (!depth || !tile_rect || !offsets || !isect_gauss || !ws)
+    (void)offsets;                              // the bucketed sort finds its own offsets (kept in the ABI; may be NULL)
+    if (!depth || !tile_rect || !isect_gauss || !ws)
         return fail(QR_ERR_NULL_POINTER, "qr_bin_sort: NULL array");
     if (!aligned16(tile_rect) || !aligned16(ws)) return fail(QR_ERR_MISALIGNED, "qr_bin_sort: tile_rect / ws alignment");
     const BinLayout L = bin_layout(N, M, T);
@@ -467,13 +474,13 @@ extern "C" int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M, const flo
         attr_set = true;
     }
     QR_CUDA_OK(cudaMemsetAsync(counter, 0, sizeof(uint32_t) * (size_t)T * kSubBuckets, st));
-    tile_bucket_kernel<false><<<nbg, 256, 0, st>>>(N, k.tiles_x, depth, rects, counter, keys);
+    tile_bucket_kernel<false><<<nbg, 256, 0, st>>>(N, k.tiles_x, depth, rects, counter, keys, (uint32_t)M);
     QR_LAUNCH_OK("tile_bucket_kernel<count>");
-    tile_scan_kernel<<<1, 1024, 0, st>>>(counter, T, tile_range);
+    tile_scan_kernel<<<1, 1024, 0, st>>>(counter, T, tile_range, (uint32_t)M, reinterpret_cast<int64_t*>(w + L.sums));
     QR_LAUNCH_OK("tile_scan_kernel");
-    tile_bucket_kernel<true><<<nbg, 256, 0, st>>>(N, k.tiles_x, depth, rects, counter, keys);
+    tile_bucket_kernel<true><<<nbg, 256, 0, st>>>(N, k.tiles_x, depth, rects, counter, keys, (uint32_t)M);
     QR_LAUNCH_OK("tile_bucket_kernel<scatter>");
-    tile_sort_kernel<false><<<(unsigned)T, 256, kSmallBucket * sizeof(uint64_t), st>>>(tile_range, T, keys, scratch, isect_gauss);
+    tile_sort_kernel<false><<<(unsigned)T, 256, kSmallBucket * sizeof(uint64_t), st>>>(tile_range, T, (int32_t)M, keys, scratch, isect_gauss);
     QR_LAUNCH_OK("tile_sort_kernel<small>");
     static int sms = 0;
     if (sms == 0) {
@@ -481,7 +488,7 @@ extern "C" int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M, const flo
         if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
             sms = 148;
     }
-    tile_sort_kernel<true><<<(unsigned)min(sms, T), 1024, kBigBucket * sizeof(uint64_t), st>>>(tile_range, T, keys, scratch, isect_gauss);
+    tile_sort_kernel<true><<<(unsigned)min(sms, T), 1024, kBigBucket * sizeof(uint64_t), st>>>(tile_range, T, (int32_t)M, keys, scratch, isect_gauss);
     QR_LAUNCH_OK("tile_sort_kernel<big>");
     return QR_OK;
 }

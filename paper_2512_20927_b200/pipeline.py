@@ -13,18 +13,27 @@ from . import binding as B
 @dataclass
 class Frontend:
     proj: B.Projected
-    offsets: torch.Tensor
-    M: int
+    offsets: Optional[torch.Tensor]
+    M: int                      # entries isect_gauss holds (the exact count, or the caller's capacity)
     isect_gauss: torch.Tensor
     tile_range: torch.Tensor
+    found: Optional[torch.Tensor] = None    # capacity path: 1-element int64 device tensor, intersections found
 
 
-def frontend(cam, means, scales, quats, opac) -> Frontend:
-    """PAPER.md:80 steps (1) tiling and (2) splatting: projection, intersection count, duplication + sort."""
+def frontend(cam, means, scales, quats, opac, capacity: Optional[int] = None) -> Frontend:
+    """PAPER.md:80 steps (1) tiling and (2) splatting: projection, intersection count, duplication + sort.
+
+    capacity = None: qr_bin_count sizes the lists exactly (one device->host read of M, the only synchronisation of
+    the path).  capacity = an upper bound on the number of intersections (e.g. 1.25 x the previous frame's): nothing
+    synchronises; `found` (device) must be checked against capacity when the frame's results are read -- if it is
+    larger the lists were truncated and the frame has to be redone with a larger capacity."""
     proj = B.qr_preprocess(cam, means, scales, quats, opac)
-    offsets, M = B.qr_bin_count(proj.tiles_touched)
-    isect, rng = B.qr_bin_sort(cam, M, proj.depth, proj.tile_rect, offsets)
-    return Frontend(proj, offsets, M, isect, rng)
+    if capacity is None:
+        offsets, M = B.qr_bin_count(proj.tiles_touched)
+        isect, rng = B.qr_bin_sort(cam, M, proj.depth, proj.tile_rect, offsets)
+        return Frontend(proj, offsets, M, isect, rng)
+    isect, rng, found = B.qr_bin_sort(cam, int(capacity), proj.depth, proj.tile_rect, None, return_found=True)
+    return Frontend(proj, None, int(capacity), isect, rng, found)
 
 
 def forward(cam, fe: Frontend, features: torch.Tensor, K: int, out: Optional[B.ForwardOut] = None) -> B.ForwardOut:

@@ -96,6 +96,32 @@ def test_bin_sort_crowded_tiles(qr, orc, N, scale):
     np.testing.assert_array_equal(_i32(fe.isect_gauss).view(np.uint32), isect)
 
 
+def test_bin_sort_with_capacity_instead_of_count(qr, orc):
+    """qr_bin_sort with M = an upper bound (no qr_bin_count, no host synchronisation): same lists and ranges, the
+    found count is reported on the device; with a bound that is too small the lists are truncated, never overrun."""
+    sc = make_scene("cfg3", seed=13, N=80000, W=330, H=250, D=8)
+    proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
+    g = P.upload(sc)
+    M = len(isect)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac, capacity=M + 1000)
+    assert int(fe.found.item()) == M and fe.M == M + 1000
+    np.testing.assert_array_equal(_i32(fe.tile_range), rng)
+    np.testing.assert_array_equal(_i32(fe.isect_gauss)[:M].view(np.uint32), isect)
+    out_a = qr.pipeline.forward(sc.cam, fe, g.features, 40)
+    out_b = qr.pipeline.forward(sc.cam, qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac), g.features, 40)
+    assert torch.equal(out_a.sel_idx, out_b.sel_idx) and torch.equal(out_a.out_map, out_b.out_map)
+    # too small: truncated at the capacity, ranges clamped, the true count still reported
+    cap = M // 2
+    fe2 = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac, capacity=cap)
+    assert int(fe2.found.item()) == M
+    tr = _i32(fe2.tile_range)
+    np.testing.assert_array_equal(tr, np.minimum(rng, cap))
+    whole = int(rng[rng[:, 1] <= cap, 1].max())            # tiles that fit entirely are exact; the one cut at cap keeps
+    np.testing.assert_array_equal(_i32(fe2.isect_gauss)[:whole].view(np.uint32), isect[:whole])   # an arbitrary part
+    qr.pipeline.forward(sc.cam, fe2, g.features, 40)        # runs on the truncated lists without touching anything else
+    torch.cuda.synchronize()
+
+
 def test_bin_empty_scene(qr):
     """Everything culled (behind the camera): M = 0, all ranges empty, forward renders zeros."""
     sc = make_scene("cfg1", seed=0, N=50)
