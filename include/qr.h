@@ -151,13 +151,13 @@ int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N,
  * those rows (zero it once, then clear after each use) writes ~|S| D floats per step instead of N D
  * (the whole-table zero fill costs more than qr_backward's own traffic).
  *   in : sel_idx, n_sel (from qr_forward); ws / ws_bytes = the workspace AS LEFT BY the last qr_backward call with
- *        the same cam, K, D and selection (its per-half-tile unions are reused); when
+ *        the same cam, K, D and selection (its per-half-tile unions are reused, a scratch region of it is written); when
  *        qr_backward_workspace_bytes(cam, K, D) == 0 ws is ignored and may be NULL.
  *   out: dL_dfeat rows of selected Gaussians = 0; other rows untouched.
  */
 int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int64_t N,
                       const int32_t* sel_idx, const int32_t* n_sel, float* dL_dfeat,
-                      const void* ws, size_t ws_bytes, void* stream);
+                      void* ws, size_t ws_bytes, void* stream);
 
 /*
  * qr_dense_forward -- Eq. 1: out = sum_i T_i alpha'_i f_i over the same per-pixel lists, not

@@ -272,7 +272,17 @@ __device__ __forceinline__ void clear_row(float* row, int D, int lane)
     }
 }
 
-__global__ void __launch_bounds__(kClearThreads) backward_clear_kernel(const BackwardParams p, const int uid_stride)
+__device__ __forceinline__ uint32_t clear_hash(uint32_t x)
+{
+    x ^= x >> 16; x *= 0x7feb352dU; x ^= x >> 15; x *= 0x846ca68bU; x ^= x >> 16;
+    return x;
+}
+
+// seen[]: a direct-mapped cache of ids whose row some warp has already taken: a Gaussian is in the unions of ~10 half
+// tiles, and without it every row was zeroed ~10 times (225 MB of stores for 24 MB of rows).  A collision only costs
+// a repeated zeroing, never a missed one (the warp that finds another id in the cell zeroes its row).
+__global__ void __launch_bounds__(kClearThreads) backward_clear_kernel(const BackwardParams p, const int uid_stride,
+                                                                       int32_t* __restrict__ seen, const int seen_mask)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
@@ -285,7 +295,20 @@ __global__ void __launch_bounds__(kClearThreads) backward_clear_kernel(const Bac
         if (c.y == 0) continue;                                   // nothing selected in this half tile
         if (c.w == 0) {                                           // numbered union: one pass over its rows
             const int32_t* uid = p.prep_uid + (size_t)ht * uid_stride;
-            for (int r = warp; r < c.z; r += kClearThreads / 32) clear_row(p.dL_dfeat + (int64_t)__ldg(uid + r) * p.D, p.D, lane);
+            for (int r0 = 0; r0 < c.z; r0 += kClearThreads) {       // thread = union row: claim it, then the warp zeroes the claimed rows
+                const int r = r0 + (int)threadIdx.x;
+                int32_t id = -1;
+                if (r < c.z) {
+                    id = __ldg(uid + r);
+                    if (seen && atomicExch(&seen[clear_hash((uint32_t)id) & seen_mask], id) == id) id = -1;   // already taken
+                }
+                uint32_t todo = __ballot_sync(0xffffffffu, id >= 0);
+                while (todo) {
+                    const int src = __ffs(todo) - 1;
+                    todo &= todo - 1;
+                    clear_row(p.dL_dfeat + (int64_t)__shfl_sync(0xffffffffu, id, src) * p.D, p.D, lane);
+                }
+            }
         } else {                                                  // every record of the 16 x 8 pixels
             for (int q = warp; q < 128; q += kClearThreads / 32) {
                 const int x = x0 + (q & 15), y = y0 + (q >> 4);
@@ -301,7 +324,7 @@ __global__ void __launch_bounds__(kClearThreads) backward_clear_kernel(const Bac
 }  // namespace qr
 
 extern "C" int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int64_t N, const int32_t* sel_idx,
-                                 const int32_t* n_sel, float* dL_dfeat, const void* ws, size_t ws_bytes, void* stream)
+                                 const int32_t* n_sel, float* dL_dfeat, void* ws, size_t ws_bytes, void* stream)
 {
     using namespace qr;
     if (int rc = check_cam(cam)) return rc;
@@ -317,10 +340,12 @@ extern "C" int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int
     BackwardParams p;
     p.cam = make_cam(cam); p.K = K; p.D = D; p.N = N;
     p.sel_idx = sel_idx; p.sel_w = nullptr; p.n_sel = n_sel; p.dL_dmap = nullptr; p.dL_dfeat = dL_dfeat;
-    int uid_stride = 0;
+    int uid_stride = 0, seen_cells = 0;
+    int32_t* seen = nullptr;
     if (backward_mma_supported(K, D)) {
         if (!ws) return fail(QR_ERR_NULL_POINTER, "qr_backward_clear: workspace is NULL");
-        if (int rc = backward_mma_workspace_view(p, ws, ws_bytes, &uid_stride)) return rc;
+        if (int rc = backward_mma_workspace_view(p, ws, ws_bytes, &uid_stride, &seen, &seen_cells)) return rc;
+        QR_CUDA_OK(cudaMemsetAsync(seen, 0xFF, (size_t)seen_cells * 4, (cudaStream_t)stream));
     }
     static int sms = 0;
     if (sms == 0) {
@@ -329,7 +354,7 @@ extern "C" int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int
             sms = 148;
     }
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
-    backward_clear_kernel<<<(unsigned)min(num_half, sms * 8), kClearThreads, 0, (cudaStream_t)stream>>>(p, uid_stride);
+    backward_clear_kernel<<<(unsigned)min(num_half, sms * 8), kClearThreads, 0, (cudaStream_t)stream>>>(p, uid_stride, seen, seen_cells - 1);
     QR_LAUNCH_OK("backward_clear_kernel");
     return QR_OK;
 }

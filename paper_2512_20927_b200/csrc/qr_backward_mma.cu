@@ -62,6 +62,7 @@ constexpr int kBmEntCap = 3072;            // selection records (and distinct Ga
 constexpr int kBmEntRegs = 8;              // entries a setup thread holds in flight
 constexpr int kBmLoStages = 2;             // G_lo is produced just ahead of the MMA that reads it
 constexpr int kBmDescRing = 4;
+constexpr int kBmSeenCells = 1 << 20;      // qr_backward_clear's de-duplication table (a cache, not a set: 4 MB)
 
 struct BmDesc {
     int32_t ht, j0, j1, nrows, flags, pad; // flags: 1 = no more work
@@ -432,30 +433,34 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
 bool backward_mma_supported(int32_t K, int32_t D) { return D % 128 == 0 && D >= 128 && D <= 512 && K >= 1 && K <= QR_MAX_K; }
 
 // workspace: per half tile {R0, R, U, left-to-the-tile-kernel} + union ids + entries
-struct BmWorkspace { size_t cnt, uid, ent, total; };
+struct BmWorkspace { size_t hdr, cnt, uid, ent, seen, total; };
 static BmWorkspace bm_workspace(const Cam& cam)
 {
     const size_t nh = (size_t)cam.tiles_x * cam.tiles_y * 2;
     BmWorkspace w;
     size_t o = 0;
+    w.hdr = o; o = align_up(o + 256, 256);                      // [0] number of half tiles left to backward_tile_kernel
     w.cnt = o; o = align_up(o + nh * 16, 256);
     w.uid = o; o = align_up(o + nh * kBmEntCap * 4, 256);
     w.ent = o; o = align_up(o + nh * kBmEntCap * 8, 256);
+    w.seen = o; o = align_up(o + (size_t)kBmSeenCells * 4, 256);   // qr_backward_clear: ids whose row is already zeroed
     w.total = o;
     return w;
 }
 size_t backward_mma_workspace_bytes(const Cam& cam) { return bm_workspace(cam).total; }
 // points p at the arrays a previous launch_backward_mma left in ws (for qr_backward_clear)
-int backward_mma_workspace_view(BackwardParams& p, const void* ws, size_t ws_bytes, int* uid_stride)
+int backward_mma_workspace_view(BackwardParams& p, void* ws, size_t ws_bytes, int* uid_stride, int32_t** seen, int* seen_cells)
 {
     const BmWorkspace wl = bm_workspace(p.cam);
     if (ws_bytes < wl.total) return fail(QR_ERR_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", ws_bytes, wl.total);
     if (!aligned16(ws)) return fail(QR_ERR_MISALIGNED, "workspace alignment");
-    const char* w = static_cast<const char*>(ws);
+    char* w = static_cast<char*>(ws);
     p.prep_cnt = reinterpret_cast<const int32_t*>(w + wl.cnt);
     p.prep_uid = reinterpret_cast<const int32_t*>(w + wl.uid);
     p.prep_ent = reinterpret_cast<const uint2*>(w + wl.ent);
     *uid_stride = kBmEntCap;
+    *seen = reinterpret_cast<int32_t*>(w + wl.seen);
+    *seen_cells = kBmSeenCells;
     return QR_OK;
 }
 
@@ -469,7 +474,8 @@ int backward_mma_workspace_view(BackwardParams& p, const void* ws, size_t ws_byt
 constexpr int kBmPrepSmem = kBmHash * 4 + kBmHash * 2 + kBmEntCap * 4 + kBmEntCap * 4 + kBmEntCap + 2 * (kBmPx + 4) * 4;
 
 __global__ void __launch_bounds__(kBmPx) backward_prep_kernel(const BackwardParams p, int32_t* __restrict__ cnt,
-                                                              int32_t* __restrict__ uid, uint2* __restrict__ ent)
+                                                              int32_t* __restrict__ uid, uint2* __restrict__ ent,
+                                                              int32_t* __restrict__ nflag)
 {
     extern __shared__ __align__(16) unsigned char psm[];
     int32_t* hkey = reinterpret_cast<int32_t*>(psm);
@@ -509,7 +515,10 @@ __global__ void __launch_bounds__(kBmPx) backward_prep_kernel(const BackwardPara
         R += s;
     }
     if (R > kBmEntCap || R == 0) {
-        if (pl == 0) reinterpret_cast<int4*>(cnt)[ht] = make_int4(R0, R, 0, R > kBmEntCap ? 1 : 0);
+        if (pl == 0) {
+            reinterpret_cast<int4*>(cnt)[ht] = make_int4(R0, R, 0, R > kBmEntCap ? 1 : 0);
+            if (R > kBmEntCap) atomicAdd(nflag, 1);
+        }
         return;
     }
     E[pl] = e0;
@@ -602,7 +611,9 @@ int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_
     int32_t* cnt = reinterpret_cast<int32_t*>(static_cast<char*>(ws) + wl.cnt);
     int32_t* uid = reinterpret_cast<int32_t*>(static_cast<char*>(ws) + wl.uid);
     uint2* ent = reinterpret_cast<uint2*>(static_cast<char*>(ws) + wl.ent);
-    p.prep_cnt = cnt; p.prep_uid = uid; p.prep_ent = ent;
+    int32_t* nflag = reinterpret_cast<int32_t*>(static_cast<char*>(ws) + wl.hdr);
+    p.prep_cnt = cnt; p.prep_uid = uid; p.prep_ent = ent; p.prep_nflag = nflag;
+    QR_CUDA_OK(cudaMemsetAsync(nflag, 0, 256, st));
     static int sms = 0;
     if (sms == 0) {
         int dev = 0;
@@ -628,7 +639,7 @@ int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_
     const int stages = max(2, min(12, (232448 - fixed - 1280) / (kBmStagePx * p.D * 4)));
     const int smem = bm_smem(p.D, stages).total;
     QR_CUDA_OK(cudaFuncSetAttribute(backward_prep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBmPrepSmem));
-    backward_prep_kernel<<<(unsigned)num_half, kBmPx, kBmPrepSmem, st>>>(p, cnt, uid, ent);
+    backward_prep_kernel<<<(unsigned)num_half, kBmPx, kBmPrepSmem, st>>>(p, cnt, uid, ent, nflag);
     QR_LAUNCH_OK("backward_prep_kernel");
     QR_CUDA_OK(cudaFuncSetAttribute(backward_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     backward_mma_kernel<<<grid, kBmThreads, smem, st>>>(p, stages, tmap);

@@ -99,6 +99,7 @@ __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const Back
     uint64_t* unit_full = empty + stages;       // [2] setup -> consumers, loader
     uint64_t* unit_empty = unit_full + 2;       // [2] consumers (8) + loader (1) -> setup
 
+    if (p.only_flagged && *p.prep_nflag == 0) return;       // nothing was left to this kernel (the usual case)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
     const int stage_floats = kBtStagePx * D;
