@@ -471,9 +471,10 @@ int backward_mma_workspace_view(BackwardParams& p, void* ws, size_t ws_bytes, in
 // here with a dozen CTAs per SM it costs a few microseconds, inside the persistent kernel it was the bottleneck
 // (profiles/README.md, r1_c).
 // ------------------------------------------------------------------------------------------------------------------
+constexpr int kBmPrepThreads = 256;
 constexpr int kBmPrepSmem = kBmHash * 4 + kBmHash * 2 + kBmEntCap * 4 + kBmEntCap * 4 + kBmEntCap + 2 * (kBmPx + 4) * 4;
 
-__global__ void __launch_bounds__(kBmPx) backward_prep_kernel(const BackwardParams p, int32_t* __restrict__ cnt,
+__global__ void __launch_bounds__(kBmPrepThreads) backward_prep_kernel(const BackwardParams p, int32_t* __restrict__ cnt,
                                                               int32_t* __restrict__ uid, uint2* __restrict__ ent,
                                                               int32_t* __restrict__ nflag)
 {
@@ -487,6 +488,7 @@ __global__ void __launch_bounds__(kBmPx) backward_prep_kernel(const BackwardPara
     uint8_t* spx = reinterpret_cast<uint8_t*>(hslot + kBmHash);
     __shared__ int32_t warp_sums[kBmPx / 32];
     __shared__ int32_t ucount;
+    // threads 0..127 own a pixel each for the scan; all kBmPrepThreads share the record-parallel phases
     const int ht = blockIdx.x, pl = threadIdx.x, lane = pl & 31, warp = pl >> 5;
     const int K = p.K;
     const int tile = ht >> 1;
@@ -498,12 +500,12 @@ __global__ void __launch_bounds__(kBmPx) backward_prep_kernel(const BackwardPara
         return x < p.cam.width && y < p.cam.height;
     };
     int64_t pix;
-    const bool valid = pix_of(pl, pix);
+    const bool valid = pl < kBmPx && pix_of(pl, pix);
     const int ns = valid ? max(0, min(K, __ldg(p.n_sel + pix))) : 0;
     int inc = ns;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
-    if (lane == 31) warp_sums[warp] = inc;
+    if (lane == 31 && warp < kBmPx / 32) warp_sums[warp] = inc;
     if (pl == 0) ucount = 0;
     __syncthreads();
     int e0 = inc - ns, R = 0, R0 = 0;
@@ -521,24 +523,23 @@ __global__ void __launch_bounds__(kBmPx) backward_prep_kernel(const BackwardPara
         }
         return;
     }
-    E[pl] = e0;
-    nss[pl] = ns;
+    if (pl < kBmPx) { E[pl] = e0; nss[pl] = ns; }
     int hs = 64;
     while (hs < 2 * R) hs <<= 1;
     hs = min(hs, kBmHash);                      // R <= kBmEntCap < kBmHash: the probe loops below always terminate
     const int hmask = hs - 1;
-    for (int k = pl; k < hs; k += kBmPx) hkey[k] = -1;
+    for (int k = pl; k < hs; k += kBmPrepThreads) hkey[k] = -1;
     __syncthreads();
     // stage the records, thread = record: every load of the half tile is in flight at once, and consecutive
     // threads read consecutive slots of a pixel's list
     for (int s = 0; s < ns; ++s) spx[e0 + s] = (uint8_t)pl;
     __syncthreads();
-    for (int k0 = pl; k0 < R; k0 += 8 * kBmPx) {
+    for (int k0 = pl; k0 < R; k0 += 8 * kBmPrepThreads) {
         int32_t id[8];
         float w[8];
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            const int k = k0 + u * kBmPx;
+            const int k = k0 + u * kBmPrepThreads;
             id[u] = -1; w[u] = 0.0f;
             if (k < R) {
                 const int q = spx[k];
@@ -551,14 +552,14 @@ __global__ void __launch_bounds__(kBmPx) backward_prep_kernel(const BackwardPara
         }
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            const int k = k0 + u * kBmPx;
+            const int k = k0 + u * kBmPrepThreads;
             if (k < R) { sid[k] = id[u]; sw[k] = w[u]; }
         }
     }
     __syncthreads();
     int32_t* uid_h = uid + (size_t)ht * kBmEntCap;
 #pragma unroll 4
-    for (int k = pl; k < R; k += kBmPx) {       // the thread that creates a cell numbers it
+    for (int k = pl; k < R; k += kBmPrepThreads) {       // the thread that creates a cell numbers it
         const int32_t id = sid[k];
         uint32_t h = bm_hash((uint32_t)id) & hmask;
         while (true) {
@@ -576,7 +577,7 @@ __global__ void __launch_bounds__(kBmPx) backward_prep_kernel(const BackwardPara
     __syncthreads();
     uint2* ent_h = ent + (size_t)ht * kBmEntCap;
 #pragma unroll 4
-    for (int k = pl; k < R; k += kBmPx) {
+    for (int k = pl; k < R; k += kBmPrepThreads) {
         const int32_t id = sid[k];
         uint32_t h = bm_hash((uint32_t)id) & hmask;
         while (hkey[h] != id) h = (h + 1) & hmask;
@@ -639,7 +640,7 @@ int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_
     const int stages = max(2, min(12, (232448 - fixed - 1280) / (kBmStagePx * p.D * 4)));
     const int smem = bm_smem(p.D, stages).total;
     QR_CUDA_OK(cudaFuncSetAttribute(backward_prep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBmPrepSmem));
-    backward_prep_kernel<<<(unsigned)num_half, kBmPx, kBmPrepSmem, st>>>(p, cnt, uid, ent, nflag);
+    backward_prep_kernel<<<(unsigned)num_half, kBmPrepThreads, kBmPrepSmem, st>>>(p, cnt, uid, ent, nflag);
     QR_LAUNCH_OK("backward_prep_kernel");
     QR_CUDA_OK(cudaFuncSetAttribute(backward_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     backward_mma_kernel<<<grid, kBmThreads, smem, st>>>(p, stages, tmap);
