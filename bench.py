@@ -357,7 +357,7 @@ def run_cuda(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture named in profiles/ (None
 # until a capture of the current kernels is committed).
-TRAFFIC = {"qr_forward": 824.0e6, "qr_backward": 818.3e6}   # profiles/r1_d_full_metrics.csv (walk + blend; prep + mma)
+TRAFFIC = {"qr_forward": 825.3e6, "qr_backward": 821.4e6}   # profiles/r1_e_full_metrics.csv (walk + blend; prep + mma)
 
 
 def main():
