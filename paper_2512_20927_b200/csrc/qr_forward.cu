@@ -208,7 +208,7 @@ __global__ void __launch_bounds__(kWalkThreads, 5) walk_kernel(const WalkParams 
     // ---- selection records of the used slots, from the four group lists this warp has just written: lane = record,
     // a ballot per pixel ranks the records that selected it (its slot, depth order), weight x 1 / (1 - T^Q) (line 20).
     // Done here, at full occupancy, rather than by the W builders of the persistent blend kernel, whose ~1,100
-    // dependent instructions per build were that kernel's critical path (profiles/README.md, r1_d). ----
+    // dependent instructions per build were that kernel's critical path (profiles/README.md, r1_e). ----
     {
         const float inv = ns > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, TQ)) : 0.0f;
         const uint32_t lt_mask = (1u << lane) - 1u;
