@@ -90,9 +90,10 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def scene_for(workload: str):
+def scene_for(args):
+    """BASELINE.json's configs; --D / --K / --pose pick a point of the sweeps of configs 4 (K, pose) and 5 (D)."""
     from qr_inputs import make_scene
-    return make_scene(workload, seed=0)
+    return make_scene(args.workload, seed=0, D=args.D, K=args.K, pose=args.pose)
 
 
 # ----------------------------------------------------------------------------------------------------------------
@@ -128,7 +129,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    sc = scene_for(args.workload)
+    sc = scene_for(args)
     steps = max(1, min(args.steps, 3))          # one frame is ~10 s of CPU work: bound the run to a few minutes
     warm = min(args.warmup, 1)
     ts, cores = time_oracle(sc, steps, warm)
@@ -146,10 +147,17 @@ def run_reference(args):
 
 
 def workload_config(sc, name):
-    return {"workload": f"{name}: {sc.cam.width}x{sc.cam.height}, N={sc.N} Gaussians (64 blobs), D={sc.D} "
-                        f"{sc.feat_dtype}, K={sc.K}, forward+backward (BASELINE.json configs[2])",
+    idx = {"cfg1": 0, "cfg2": 1, "cfg3": 2, "cfg4": 3, "cfg5": 4}.get(name, -1)
+    kind = "64 blobs" if sc.meta.get("kind") == "blobs" else "uniform"
+    esz = 2 if sc.feat_dtype == "f16" else 4
+    mb = lambda n: f"{n / 1e6:.0f} MB"
+    npix = sc.cam.width * sc.cam.height
+    return {"workload": f"{name}: {sc.cam.width}x{sc.cam.height}, N={sc.N} Gaussians ({kind}), D={sc.D} "
+                        f"{sc.feat_dtype}, K={sc.K}, forward+backward (BASELINE.json configs[{idx}])",
             "K": sc.K, "D": sc.D, "N": sc.N, "width": sc.cam.width, "height": sc.cam.height,
-            "l2": "inputs larger than L2 (features 1.02 GB, dL_dmap 629 MB, map 629 MB vs 126 MB L2); no flush needed"}
+            "l2": f"inputs vs the 126 MB L2: features {mb(sc.N * sc.D * esz)}, dL_dmap {mb(npix * sc.D * 4)}, map "
+                  f"{mb(npix * sc.D * 4)}; " + ("larger than L2, no flush needed" if npix * sc.D * 4 > 2.5e8 else
+                                               "SMALLER than L2: figures at this size are L2-resident, not HBM, numbers")}
 
 
 # ----------------------------------------------------------------------------------------------------------------
@@ -171,7 +179,7 @@ def run_cuda(args):
     from paper_2512_20927_b200 import pipeline as pl
     qr.binding.load()
 
-    sc = scene_for(args.workload)
+    sc = scene_for(args)
     cam, K, D, N = sc.cam, sc.K, sc.D, sc.N
     H, W = cam.height, cam.width
     npix = H * W
@@ -367,6 +375,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--D", type=int, default=None, help="feature width (config 5 sweeps 3..512)")
+    ap.add_argument("--K", type=int, default=None, help="quantile count (config 4 sweeps 4..32)")
+    ap.add_argument("--pose", type=int, default=None, help="camera pose 0..7 of config 4's circle")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

@@ -137,8 +137,9 @@ int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype,
  *   in : sel_idx, sel_w, n_sel (from qr_forward), dL_dmap[H,W,D] fp32
  *   out: dL_dfeat[N,D] fp32, ACCUMULATED INTO (the caller zeroes it; rows never selected are left untouched).
  * Summation order over pixels is not fixed (fp32 atomics): results agree to rounding, not bit for bit.
- * ws must hold qr_backward_workspace_bytes(cam, K, D) bytes (0 for some shapes; then ws may be NULL).  Its contents
- * are scratch: per half tile, the numbered union of selected Gaussians and the selection as (weight, row, pixel).
+ * ws must hold qr_backward_workspace_bytes(cam, K, D) bytes.  Its contents are scratch: per half tile, the numbered
+ * union of selected Gaussians and the selection as (weight, row, pixel) (D % 128 == 0), and qr_backward_clear's
+ * de-duplication cache; for the other shapes qr_backward itself does not touch ws (it may be NULL there).
  */
 size_t qr_backward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D);
 int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N,
@@ -151,8 +152,7 @@ int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N,
  * those rows (zero it once, then clear after each use) writes ~|S| D floats per step instead of N D
  * (the whole-table zero fill costs more than qr_backward's own traffic).
  *   in : sel_idx, n_sel (from qr_forward); ws / ws_bytes = the workspace AS LEFT BY the last qr_backward call with
- *        the same cam, K, D and selection (its per-half-tile unions are reused, a scratch region of it is written); when
- *        qr_backward_workspace_bytes(cam, K, D) == 0 ws is ignored and may be NULL.
+ *        the same cam, K, D and selection (its per-half-tile unions are reused, a scratch region of it is written).
  *   out: dL_dfeat rows of selected Gaussians = 0; other rows untouched.
  */
 int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int64_t N,

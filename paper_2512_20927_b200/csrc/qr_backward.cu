@@ -261,6 +261,7 @@ static int launch_backward(const BackwardParams& p, cudaStream_t st)
 // selection record.
 // ------------------------------------------------------------------------------------------------------------------
 constexpr int kClearThreads = 256;
+constexpr int kClearSeenCells = 1 << 20;     // de-duplication cache when qr_backward itself needs no workspace (4 MB)
 
 __device__ __forceinline__ void clear_row(float* row, int D, int lane)
 {
@@ -310,12 +311,24 @@ __global__ void __launch_bounds__(kClearThreads) backward_clear_kernel(const Bac
                 }
             }
         } else {                                                  // every record of the 16 x 8 pixels
-            for (int q = warp; q < 128; q += kClearThreads / 32) {
+            for (int q = warp; q < 128; q += kClearThreads / 32) {      // warp = pixel, lane = record
                 const int x = x0 + (q & 15), y = y0 + (q >> 4);
                 if (x >= p.cam.width || y >= p.cam.height) continue;
                 const int64_t pix = (int64_t)y * p.cam.width + x;
                 const int ns = max(0, min(p.K, __ldg(p.n_sel + pix)));
-                for (int s = 0; s < ns; ++s) clear_row(p.dL_dfeat + (int64_t)__ldg(p.sel_idx + pix * p.K + s) * p.D, p.D, lane);
+                for (int s0 = 0; s0 < ns; s0 += 32) {
+                    int32_t id = -1;
+                    if (s0 + lane < ns) {
+                        id = __ldg(p.sel_idx + pix * p.K + s0 + lane);
+                        if (seen && atomicExch(&seen[clear_hash((uint32_t)id) & seen_mask], id) == id) id = -1;   // already taken
+                    }
+                    uint32_t todo = __ballot_sync(0xffffffffu, id >= 0);
+                    while (todo) {
+                        const int src = __ffs(todo) - 1;
+                        todo &= todo - 1;
+                        clear_row(p.dL_dfeat + (int64_t)__shfl_sync(0xffffffffu, id, src) * p.D, p.D, lane);
+                    }
+                }
             }
         }
     }
@@ -342,11 +355,16 @@ extern "C" int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int
     p.sel_idx = sel_idx; p.sel_w = nullptr; p.n_sel = n_sel; p.dL_dmap = nullptr; p.dL_dfeat = dL_dfeat;
     int uid_stride = 0, seen_cells = 0;
     int32_t* seen = nullptr;
+    if (!ws) return fail(QR_ERR_NULL_POINTER, "qr_backward_clear: workspace is NULL");
     if (backward_mma_supported(K, D)) {
-        if (!ws) return fail(QR_ERR_NULL_POINTER, "qr_backward_clear: workspace is NULL");
         if (int rc = backward_mma_workspace_view(p, ws, ws_bytes, &uid_stride, &seen, &seen_cells)) return rc;
-        QR_CUDA_OK(cudaMemsetAsync(seen, 0xFF, (size_t)seen_cells * 4, (cudaStream_t)stream));
+    } else {                                    // no numbered unions: the workspace is only the de-duplication cache
+        if (ws_bytes < (size_t)kClearSeenCells * 4) return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_backward_clear: workspace %zu < %zu bytes", ws_bytes, (size_t)kClearSeenCells * 4);
+        if (!aligned16(ws)) return fail(QR_ERR_MISALIGNED, "qr_backward_clear: workspace alignment");
+        seen = static_cast<int32_t*>(ws);
+        seen_cells = kClearSeenCells;
     }
+    QR_CUDA_OK(cudaMemsetAsync(seen, 0xFF, (size_t)seen_cells * 4, (cudaStream_t)stream));
     static int sms = 0;
     if (sms == 0) {
         int dev = 0;
@@ -362,7 +380,8 @@ extern "C" int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int
 extern "C" size_t qr_backward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D)
 {
     if (!cam || cam->width < 1 || cam->height < 1) return 0;
-    return qr::backward_mma_supported(K, D) ? qr::backward_mma_workspace_bytes(qr::make_cam(cam)) : 0;
+    return qr::backward_mma_supported(K, D) ? qr::backward_mma_workspace_bytes(qr::make_cam(cam))
+                                            : (size_t)qr::kClearSeenCells * 4;      // used by qr_backward_clear only
 }
 
 extern "C" int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N, const int32_t* sel_idx,
