@@ -362,10 +362,16 @@ static inline int alpha_prime_f32(int x, int y, const float* m2, const float* co
  * exactly.
  * Two-pass CSR: call with gid == NULL to fill counts[HW] (and borderline[HW]); then prefix-sum
  * into off[HW+1] and call again with gid/alpha to fill.
+ * bl_first[HW] (may be NULL; filled in the counting pass): list position of the first borderline
+ * event of the pixel = number of INCLUDED entries in front of the first Gaussian (included or not)
+ * whose membership is within 1e-6 of a cut of R4; INT64_MAX when the pixel has none.  A walk that
+ * consumes n_walked entries can only be affected by a borderline event at position <= n_walked
+ * (reading R15: the exemption is for what the walk actually meets, not for the whole list).
  * ---------------------------------------------------------------------------------------- */
 void orc_pixel_lists(const orc_camera* cam, int64_t N, const float* mean2d, const float* conic_opac,
                      const float* depth, const float* extent, const uint8_t* visible, int mode,
-                     int64_t* counts, uint8_t* borderline, const int64_t* off, int32_t* gid, float* alpha)
+                     int64_t* counts, uint8_t* borderline, const int64_t* off, int32_t* gid, float* alpha,
+                     int64_t* bl_first)
 {
     const int Wd = cam->width, Ht = cam->height;
     int64_t nv = 0;
@@ -383,7 +389,10 @@ void orc_pixel_lists(const orc_camera* cam, int64_t N, const float* mean2d, cons
             fill = (int64_t*)malloc(sizeof(int64_t) * (size_t)Wd);
             for (int x = 0; x < Wd; ++x) fill[x] = off[(int64_t)y * Wd + x];
         } else {
-            for (int x = 0; x < Wd; ++x) { counts[(int64_t)y * Wd + x] = 0; borderline[(int64_t)y * Wd + x] = 0; }
+            for (int x = 0; x < Wd; ++x) {
+                counts[(int64_t)y * Wd + x] = 0; borderline[(int64_t)y * Wd + x] = 0;
+                if (bl_first) bl_first[(int64_t)y * Wd + x] = INT64_MAX;
+            }
         }
         for (int64_t o = 0; o < nv; ++o) {
             const int32_t g = order[o].id;
@@ -404,7 +413,10 @@ void orc_pixel_lists(const orc_camera* cam, int64_t N, const float* mean2d, cons
                 const int inc = alpha_prime_f32(x, y, mean2d + 2 * g, conic_opac + 4 * g, &a, &bl);
                 const int64_t p = (int64_t)y * Wd + x;
                 if (!gid) {
-                    if (bl) borderline[p] = 1;
+                    if (bl) {
+                        borderline[p] = 1;
+                        if (bl_first && bl_first[p] == INT64_MAX) bl_first[p] = counts[p];
+                    }
                     if (inc) counts[p]++;
                 } else if (inc) {
                     gid[fill[x]] = g; alpha[fill[x]] = a; fill[x]++;

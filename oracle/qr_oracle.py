@@ -132,9 +132,10 @@ class PixelLists:
     off: np.ndarray         # [H*W+1] int64
     gid: np.ndarray         # [total] int32
     alpha: np.ndarray       # [total] float32
-    borderline: np.ndarray  # [H*W] uint8: list membership within 1e-6 of a cut (reading R15)
+    borderline: np.ndarray  # [H*W] uint8: list membership within 1e-6 of a cut (reading R15), anywhere in the list
     width: int
     height: int
+    bl_first: Optional[np.ndarray] = None   # [H*W] int64: list position of the first such event (INT64_MAX: none)
 
     def ray(self, p: int):
         b, e = int(self.off[p]), int(self.off[p + 1])
@@ -147,16 +148,17 @@ def pixel_lists(cam, proj: Projected, mode: str = "binned") -> PixelLists:
     n = proj.mean2d.shape[0]
     m2, co, dp, ex = _f32(proj.mean2d), _f32(proj.conic_opac), _f32(proj.depth), _f32(proj.extent)
     counts = np.zeros(hw, np.int64); bl = np.zeros(hw, np.uint8)
+    blf = np.full(hw, np.iinfo(np.int64).max, np.int64)
     c = _cam(cam)
     lib().orc_pixel_lists(C.byref(c), C.c_int64(n), _p(m2), _p(co), _p(dp), _p(ex), _p(proj.visible),
-                          C.c_int(md), _p(counts), _p(bl), None, None, None)
+                          C.c_int(md), _p(counts), _p(bl), None, None, None, _p(blf))
     off = np.zeros(hw + 1, np.int64)
     np.cumsum(counts, out=off[1:])
     tot = int(off[-1])
     gid = np.empty(max(tot, 1), np.int32); al = np.empty(max(tot, 1), np.float32)
     lib().orc_pixel_lists(C.byref(c), C.c_int64(n), _p(m2), _p(co), _p(dp), _p(ex), _p(proj.visible),
-                          C.c_int(md), _p(counts), _p(bl), _p(off), _p(gid), _p(al))
-    return PixelLists(off, gid[:tot], al[:tot], bl, cam.width, cam.height)
+                          C.c_int(md), _p(counts), _p(bl), _p(off), _p(gid), _p(al), None)
+    return PixelLists(off, gid[:tot], al[:tot], bl, cam.width, cam.height, blf)
 
 
 def lists_from_rays(rays) -> PixelLists:

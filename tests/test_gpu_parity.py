@@ -109,7 +109,9 @@ def test_bin_sort_with_capacity_instead_of_count(qr, orc):
     np.testing.assert_array_equal(_i32(fe.isect_gauss)[:M].view(np.uint32), isect)
     out_a = qr.pipeline.forward(sc.cam, fe, g.features, 40)
     out_b = qr.pipeline.forward(sc.cam, qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac), g.features, 40)
-    assert torch.equal(out_a.sel_idx, out_b.sel_idx) and torch.equal(out_a.out_map, out_b.out_map)
+    ia, wa, na = P.masked_records(out_a)
+    ib, wb, nb = P.masked_records(out_b)
+    assert (ia == ib).all() and (na == nb).all() and torch.equal(out_a.out_map, out_b.out_map)
     # too small: truncated at the capacity, ranges clamped, the true count still reported
     cap = M // 2
     fe2 = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac, capacity=cap)
@@ -132,7 +134,6 @@ def test_bin_empty_scene(qr):
     assert (fe.tile_range.cpu().numpy() == 0).all()
     out = qr.pipeline.forward(sc.cam, fe, g.features, 40)
     assert (out.out_map == 0).all() and (out.n_sel == 0).all() and (out.resid_TQ == 1).all()
-    assert (out.sel_idx == -1).all() and (out.sel_w == 0).all()
 
 
 # ------------------------------------------------------------------------------------------------
@@ -148,6 +149,8 @@ FWD_CASES = [
     ("cfg3", dict(N=60000, W=160, H=112, D=512), 40),           # blob scene, camera inside, D = 512
     ("cfg3", dict(N=60000, W=96, H=64, D=384), 10),
     ("cfg3", dict(N=40000, W=96, H=64, D=64), 200),             # K large
+    ("cfg1", dict(W=70, H=50, D=256), 40),                      # tcgen05 blend on a ragged image (store guard, skipped half tiles)
+    ("cfg3", dict(N=60000, W=100, H=72, D=512), 5),
 ]
 
 
@@ -196,8 +199,9 @@ def test_forward_invariants_full_scale(qr):
     fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
     K = 40
     out = qr.pipeline.forward(sc.cam, fe, g.features, K)
-    n_sel = out.n_sel.cpu().numpy()
-    w = out.sel_w.cpu().numpy().astype(np.float64)
+    idx, w, n_sel = P.masked_records(out)
+    n_sel = n_sel.reshape(out.n_sel.shape)
+    w = w.astype(np.float64).reshape(out.sel_w.shape)
     assert n_sel.max() <= K and n_sel.min() >= 0
     assert (w >= 0).all()
     has = n_sel > 0
@@ -206,10 +210,10 @@ def test_forward_invariants_full_scale(qr):
     const = torch.ones_like(g.features) * 0.25
     out_c = qr.pipeline.forward(sc.cam, fe, const, K)
     np.testing.assert_allclose(out_c.out_map.cpu().numpy()[has], 0.25, rtol=1e-5)
-    assert torch.equal(out_c.sel_idx, out.sel_idx)                              # selection independent of payload (G6)
+    assert (P.masked_records(out_c)[0] == idx).all()                            # selection independent of payload (G6)
     # payload width independence
     out_3 = qr.pipeline.forward(sc.cam, fe, g.features[:, :3].contiguous(), K)
-    assert torch.equal(out_3.sel_idx, out.sel_idx)
+    assert (P.masked_records(out_3)[0] == idx).all()
     np.testing.assert_allclose(out_3.out_map.cpu().numpy(), out.out_map[..., :3].cpu().numpy(), rtol=1e-6, atol=1e-7)
 
 
@@ -298,7 +302,8 @@ def test_backward_clear_zeroes_exactly_the_touched_rows(qr, orc, name, kw, K):
     dF = torch.full((sc.N, sc.D), 7.0, dtype=torch.float32, device=G.device)
     qr.pipeline.backward(sc.cam, sc.N, out, G, dF, ws)
     qr.pipeline.backward_clear(sc.cam, sc.N, out, dF, ws)
-    sel = out.sel_idx[out.sel_idx >= 0].long()
+    idx_m = torch.from_numpy(P.masked_records(out)[0]).to(G.device)
+    sel = idx_m[idx_m >= 0].long()
     touched = torch.zeros(sc.N, dtype=torch.bool, device=G.device)
     touched[sel] = True
     assert int(touched.sum()) > 10
@@ -315,42 +320,45 @@ def test_backward_clear_zeroes_exactly_the_touched_rows(qr, orc, name, kw, K):
 
 
 # ------------------------------------------------------------------------------------------------
-# full-size sampled check in the configuration bench.py times (config 3)
+# full-size checks in the configuration bench.py times
 # ------------------------------------------------------------------------------------------------
-def test_config3_full_size_sampled(qr, orc):
-    sc = make_scene("cfg3", seed=0)
-    g = P.upload(sc)
-    K = sc.K
-    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
-    out = qr.pipeline.forward(sc.cam, fe, g.features, K)
+def _backward_rows_check(qr, orc, sc, K, out, qa, same, n_rows, tag):
+    """Gradient parity on sampled dL/dF rows at full size, two ways:
+    (a) stage-isolated -- qr_backward on the ORACLE's selection records (every sampled row is comparable);
+    (b) end to end -- qr_backward on the GPU forward's own records, compared on the sampled rows that no pixel with a
+        differing selection touches (those pixels are the exempt ones; their rows legitimately differ)."""
+    H, W = sc.cam.height, sc.cam.width
     G = P.to_dev(sc.dL_dmap)
-    dF = qr.pipeline.backward(sc.cam, sc.N, out, G)
-    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
-    rect, touched = orc.tile_rects(sc.cam, proj)
-    assert fe.M == int(touched.sum())
-    lists = orc.pixel_lists(sc.cam, proj)
-    rng = np.random.default_rng(0)
-    pix = np.sort(rng.choice(sc.cam.width * sc.cam.height, size=4000, replace=False))
-    q = orc.qrender(lists, K, sc.features, pixels=pix)
-    stats = P.compare_forward(out, q, lists, K, sc.D, pixels=pix)
-    print("cfg3 sampled:", stats)
-    # selection parity on every pixel (no features needed)
-    qa = orc.qrender(lists, K, None)
-    ex = P.exempt_mask(qa, lists)
-    same = (out.sel_idx.cpu().numpy().reshape(-1, K) == qa.sel_idx).all(1)
-    assert ((~same) & (~ex)).sum() == 0
-    print("cfg3 all pixels: exempt", int(ex.sum()), "mismatching exempt", int(((~same) & ex).sum()))
-    # gradient rows of sampled Gaussians from the oracle's records
     sel = qa.sel_idx[qa.sel_idx >= 0]
-    rows = np.unique(sel)[::97][:200].astype(np.int64)
+    rows_all = np.unique(sel)
+    rows = rows_all[:: max(1, len(rows_all) // n_rows)][:n_rows].astype(np.int64)
+    assert len(rows) >= 100, len(rows)
     ref = orc.backward(qa.sel_idx, qa.sel_w, qa.n_sel, sc.dL_dmap, sc.N, rows=rows)
-    got = dF[torch.from_numpy(rows).cuda()].cpu().numpy().astype(np.float64)
-    if same.all():
-        tol = P.ATOL + P.RTOL * np.abs(ref)
-        assert (np.abs(got - ref) <= tol).all(), float((np.abs(got - ref) / tol).max())
+    ridx = torch.from_numpy(rows).cuda()
+    # (a)
+    dF = qr.qr_backward(sc.cam, sc.N, P.to_dev(qa.sel_idx.reshape(H, W, K)),
+                        P.to_dev(qa.sel_w.reshape(H, W, K).astype(np.float32)), P.to_dev(qa.n_sel.reshape(H, W)), G)
+    worst_a = P.compare_backward_rows(dF[ridx].cpu().numpy(), ref, f"{tag} stage-isolated")
+    del dF
+    # (b)
+    dF = qr.pipeline.backward(sc.cam, sc.N, out, G)
+    got = dF[ridx].cpu().numpy()
+    del dF
+    bad_px = np.flatnonzero(~same)
+    gsel = out.sel_idx.cpu().numpy().reshape(-1, K)
+    gn = out.n_sel.cpu().numpy().reshape(-1)
+    tainted = set()
+    for p in bad_px:
+        tainted.update(int(v) for v in gsel[p, :gn[p]])
+        tainted.update(int(v) for v in qa.sel_idx[p, :qa.n_sel[p]])
+    keep = np.array([int(r) not in tainted for r in rows])
+    assert keep.sum() >= 100, (int(keep.sum()), len(rows))
+    worst_b = P.compare_backward_rows(got[keep], ref[keep], f"{tag} end-to-end")
+    print(f"{tag} backward rows: stage-isolated {len(rows)} rows (worst err/tol {worst_a:.3f}); end-to-end "
+          f"{int(keep.sum())} of {len(rows)} rows (worst {worst_b:.3f}); pixels with differing selection {len(bad_px)}")
 
 
-def _full_size_check(qr, orc, sc, Ks, n_pix=3000, n_rows=150, f16=False):
+def _full_size_check(qr, orc, sc, Ks, n_pix=3000, n_rows=150, f16=False, max_exempt_frac=0.004):
     """Full-size frame in bench.py's launch configuration: selection parity on every pixel, features on sampled
     pixels, gradient rows of sampled Gaussians (the oracle computes those one by one)."""
     g = P.upload(sc)
@@ -361,28 +369,26 @@ def _full_size_check(qr, orc, sc, Ks, n_pix=3000, n_rows=150, f16=False):
     lists = orc.pixel_lists(sc.cam, proj)
     rng = np.random.default_rng(1)
     pix = np.sort(rng.choice(sc.cam.width * sc.cam.height, size=n_pix, replace=False))
-    G = P.to_dev(sc.dL_dmap) if sc.dL_dmap is not None else None
     for K in Ks:
         out = qr.pipeline.forward(sc.cam, fe, g.features, K)
         q = orc.qrender(lists, K, sc.features, pixels=pix)
         stats = P.compare_forward(out, q, lists, K, sc.D, f16=f16, pixels=pix)
         qa = orc.qrender(lists, K, None)
-        ex = P.exempt_mask(qa, lists)
-        same = (out.sel_idx.cpu().numpy().reshape(-1, K) == qa.sel_idx).all(1)
+        ex_m, ex_b = P.exempt_classes(qa, lists)
+        ex = ex_m | ex_b
+        same = P.same_selection(out.sel_idx.cpu().numpy().reshape(-1, K), out.n_sel.cpu().numpy().reshape(-1), qa)
         assert ((~same) & (~ex)).sum() == 0
-        print(sc.name, "K", K, "sampled:", stats, "all pixels: exempt", int(ex.sum()), "mismatching exempt", int(((~same) & ex).sum()))
-        if G is not None and K == Ks[-1]:
-            dF = qr.pipeline.backward(sc.cam, sc.N, out, G)
-            sel = qa.sel_idx[qa.sel_idx >= 0]
-            rows = np.unique(sel)
-            rows = rows[:: max(1, len(rows) // n_rows)][:n_rows].astype(np.int64)
-            ref = orc.backward(qa.sel_idx, qa.sel_w, qa.n_sel, sc.dL_dmap, sc.N, rows=rows)
-            got = dF[torch.from_numpy(rows).cuda()].cpu().numpy().astype(np.float64)
-            if same.all():
-                tol = P.ATOL + P.RTOL * np.abs(ref)
-                assert (np.abs(got - ref) <= tol).all(), float((np.abs(got - ref) / tol).max())
-            del dF
+        print(sc.name, "K", K, "sampled:", stats, "| all pixels:", same.size, "exempt by margin", int(ex_m.sum()),
+              "by borderline membership only", int((ex_b & ~ex_m).sum()), "differing (all exempt)", int((~same).sum()))
+        assert ex.sum() <= max_exempt_frac * same.size, (int(ex.sum()), same.size)
+        if sc.dL_dmap is not None and K == Ks[-1]:
+            _backward_rows_check(qr, orc, sc, K, out, qa, same, n_rows, f"{sc.name} K={K}")
         del out
+
+
+def test_config3_full_size_sampled(qr, orc):
+    """BASELINE.json configs[2], the headline: 640x480, 500,000 Gaussians, D = 512 fp32, K = 40, forward + backward."""
+    _full_size_check(qr, orc, make_scene("cfg3", seed=0), [40], n_pix=4000, n_rows=200)
 
 
 def test_config5_full_size_sampled(qr, orc):
@@ -396,12 +402,45 @@ def test_config5_narrow_payload_full_size(qr, orc):
     _full_size_check(qr, orc, sc, [40], n_pix=2000, n_rows=100)
 
 
-def test_config4_full_size_sampled(qr, orc):
-    """BASELINE.json configs[3]: 1024x768, 2,000,000 Gaussians, D = 512 stored fp16 (fp32 accumulation), pose 0 of the
-    radius-3 circle, K = 4 and K = 32."""
-    sc = make_scene("cfg4", seed=0, pose=0)
+@pytest.mark.parametrize("pose", [0, 5])
+def test_config4_full_size_sampled(qr, orc, pose):
+    """BASELINE.json configs[3]: 1024x768, 2,000,000 Gaussians, D = 512 stored fp16 (fp32 accumulation), two poses of
+    the radius-3 circle, K = 4 and K = 32."""
+    sc = make_scene("cfg4", seed=0, pose=pose)
     assert sc.features.dtype == np.float16
     _full_size_check(qr, orc, sc, [4, 32], n_pix=2000, n_rows=100, f16=True)
+
+
+@pytest.mark.parametrize("D", [256, 512])
+def test_midsize_every_row_many_units_per_cta(qr, orc, D):
+    """A frame with more half tiles (600) than SMs (148), so that every persistent CTA of the tcgen05 kernels runs several
+    work units (ring wrap-around, accumulator ping-pong), small enough that the oracle produces EVERY pixel and EVERY
+    gradient row: forward end to end, backward both on the oracle's records and on the forward's own."""
+    sc = make_scene("cfg3", seed=21, N=100000, W=320, H=240, D=D)
+    K = 40
+    H, W = sc.cam.height, sc.cam.width
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    out = qr.pipeline.forward(sc.cam, fe, g.features, K)
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    lists = orc.pixel_lists(sc.cam, proj)
+    q = orc.qrender(lists, K, sc.features)
+    stats = P.compare_forward(out, q, lists, K, sc.D)
+    print("mid-size forward:", stats)
+    G = P.to_dev(sc.dL_dmap)
+    ref = orc.backward(q.sel_idx, q.sel_w, q.n_sel, sc.dL_dmap, sc.N)
+    got = qr.qr_backward(sc.cam, sc.N, P.to_dev(q.sel_idx.reshape(H, W, K)), P.to_dev(q.sel_w.reshape(H, W, K).astype(np.float32)),
+                         P.to_dev(q.n_sel.reshape(H, W)), G).cpu().numpy()
+    worst = P.compare_backward_rows(got, ref, "mid-size stage-isolated")
+    same = P.same_selection(out.sel_idx.cpu().numpy().reshape(-1, K), out.n_sel.cpu().numpy().reshape(-1), q)
+    got2 = qr.pipeline.backward(sc.cam, sc.N, out, G).cpu().numpy()
+    tainted = np.zeros(sc.N, bool)
+    gsel = out.sel_idx.cpu().numpy().reshape(-1, K); gn = out.n_sel.cpu().numpy().reshape(-1)
+    for p in np.flatnonzero(~same):
+        tainted[gsel[p, :gn[p]]] = True
+        tainted[q.sel_idx[p, :q.n_sel[p]]] = True
+    worst2 = P.compare_backward_rows(got2[~tainted], ref[~tainted], "mid-size end-to-end")
+    print(f"mid-size backward: all {sc.N} rows stage-isolated (worst {worst:.3f}); {int((~tainted).sum())} rows end to end (worst {worst2:.3f})")
 
 
 # ------------------------------------------------------------------------------------------------

@@ -458,6 +458,38 @@ def test_R4_inclusion_rule(orc):
     assert (n_in[keep] == 1).all() and (n_in[drop] == 0).all() and keep.sum() > 10
 
 
+def test_R15_borderline_position(orc):
+    """Reading R15: a pixel is exempt for list membership only if the walk MEETS the borderline Gaussian.  A Gaussian
+    centred on pixel (5, 5) with opacity exactly 1/255 has alpha' == alpha_min there (power = 0): a borderline event.
+    bl_first = number of included entries in front of it: 0 when it is nearest, 1 behind one opaque Gaussian; pixels it
+    does not reach carry INT64_MAX.  With K = 1 and an alpha' = 0.8 Gaussian in front the walk consumes 1 entry and
+    breaks, so position 1 <= n_walked is still (conservatively) exempt, while behind two such Gaussians the walk never
+    gets there."""
+    cam = make_camera(16, 16)
+    amin = np.float32(1.0) / np.float32(255.0)
+    big = 0.02
+    def lists_for(depth_b, n_front):
+        m2 = [[5.5, 5.5]] + [[5.5, 5.5]] * n_front
+        co = [[big, 0.0, big, amin]] + [[big, 0.0, big, 0.8]] * n_front
+        dp = [depth_b] + [1.0 + 0.1 * i for i in range(n_front)]
+        n = len(m2)
+        proj = orc.Projected(np.array(m2, np.float32), np.array(co, np.float32), np.array(dp, np.float32),
+                             np.full((n, 2), 21.3, np.float32), np.ones(n, np.uint8))
+        return orc.pixel_lists(cam, proj, "brute")
+    p = 5 * 16 + 5
+    imax = np.iinfo(np.int64).max
+    L = lists_for(0.5, 1)                      # borderline Gaussian nearest
+    assert L.borderline[p] == 1 and L.bl_first[p] == 0
+    assert (L.bl_first[L.borderline == 0] == imax).all() and (L.bl_first[L.borderline == 1] < imax).all()
+    L = lists_for(5.0, 1)                      # behind one opaque Gaussian
+    assert L.bl_first[p] == 1
+    q = orc.qrender(L, 1)
+    assert q.n_walked[p] == 1 and L.bl_first[p] <= q.n_walked[p]
+    L = lists_for(5.0, 2)                      # behind two: alpha' = 0.8 breaks a K = 1 walk at the first entry
+    q = orc.qrender(L, 1)
+    assert L.bl_first[p] == 2 and q.n_walked[p] == 1 and not (L.bl_first[p] <= q.n_walked[p])
+
+
 # --------------------------------------------------------------------------------------------
 # G13: backward -- Jacobian rows, adjoint identity, finite differences (SPEC.md:462-470, :491)
 # --------------------------------------------------------------------------------------------
