@@ -107,7 +107,7 @@ def oracle_frame(orc, sc):
     lists = orc.pixel_lists(sc.cam, proj)
     q = orc.qrender(lists, sc.K, sc.features)
     if sc.dL_dmap is not None:
-        sel = q.sel_idx[q.sel_idx >= 0]
+        sel = q.sel_idx[q.sel_idx >= 0]            # the oracle pads its records with -1
         rows = np.unique(sel).astype(np.int64)
         orc.backward(q.sel_idx, q.sel_w, q.n_sel, sc.dL_dmap, sc.N, rows=rows)
     return q
@@ -290,7 +290,8 @@ def run_cuda(args):
 
     # workload counts for the byte model (statistics only; torch ops outside every timed region)
     n_vis = int((fe.proj.tiles_touched != 0).sum().item())
-    sel = fwd_out.sel_idx[fwd_out.sel_idx >= 0]
+    used = torch.arange(K, device=dev)[None, None, :] < fwd_out.n_sel[..., None]   # slots >= n_sel are not written
+    sel = fwd_out.sel_idx[used]
     S = int(torch.unique(sel).numel())
     nsel_mean = float(fwd_out.n_sel.float().mean().item())
     esz = 2 if sc.feat_dtype == "f16" else 4

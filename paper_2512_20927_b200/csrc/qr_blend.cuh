@@ -1,6 +1,7 @@
 // qr_blend.cuh -- what walk_kernel hands to the blend kernels of qr_forward (qr_forward.cu, qr_blend_mma.cu).
 #pragma once
 #include "qr_common.cuh"
+#include "qr_sel.cuh"
 
 namespace qr {
 
@@ -28,6 +29,8 @@ struct BlendParams {
     int32_t* sel_idx;
     float* sel_w;
     int32_t* tile_ticket;
+    SelLists sl;                 // tcgen05 blend: the walk's selection lists (qr_sel.cuh); the fields above that describe
+                                 // group records are unused there
 };
 
 // tcgen05 blend (qr_blend_mma.cu): fp32 features, D a multiple of 256.

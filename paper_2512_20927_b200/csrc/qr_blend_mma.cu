@@ -133,7 +133,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
 {
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char* stage_base = smem + MmaSmem::stages;
-    int32_t* uid_s = reinterpret_cast<int32_t*>(smem + MmaSmem::uid);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + MmaSmem::bars);
     uint64_t* full = bars;                       // [kStages] converters -> MMA (8 warp arrivals)
     uint64_t* empty = bars + kStages;            // [kStages] MMA -> converters (tcgen05.commit)
@@ -198,8 +197,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
             const int x = x0 + (m & 15), y = y0 + (m >> 4);
             const bool valid = x < p.cam.width && y < p.cam.height;
             const int64_t pix = (int64_t)y * p.cam.width + x;
-            float inv = 0.0f;
-            if (valid && __ldg(p.n_sel + pix) > 0) inv = __fdiv_rn(1.0f, __fsub_rn(1.0f, __ldg(p.resid + pix)));   // line 20; R8
             for (int c = 0; c < nunits; ++c, ++unit) {
                 const int buf = unit & 1;
                 bar_wait(&tmem_full[buf], (unit >> 1) & 1);
@@ -211,12 +208,10 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                     float* dst = orow + chunk * 32;
 #pragma unroll
                     for (int jj = 0; jj < 4; ++jj)
-                        asm volatile("st.global.L1::no_allocate.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                        asm volatile("st.global.L1::no_allocate.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
                                      ::"l"(dst + 8 * jj),
-                                       "f"(__fmul_rn(__uint_as_float(r[8 * jj]), inv)), "f"(__fmul_rn(__uint_as_float(r[8 * jj + 1]), inv)),
-                                       "f"(__fmul_rn(__uint_as_float(r[8 * jj + 2]), inv)), "f"(__fmul_rn(__uint_as_float(r[8 * jj + 3]), inv)),
-                                       "f"(__fmul_rn(__uint_as_float(r[8 * jj + 4]), inv)), "f"(__fmul_rn(__uint_as_float(r[8 * jj + 5]), inv)),
-                                       "f"(__fmul_rn(__uint_as_float(r[8 * jj + 6]), inv)), "f"(__fmul_rn(__uint_as_float(r[8 * jj + 7]), inv))
+                                       "r"(r[8 * jj]), "r"(r[8 * jj + 1]), "r"(r[8 * jj + 2]), "r"(r[8 * jj + 3]),
+                                       "r"(r[8 * jj + 4]), "r"(r[8 * jj + 5]), "r"(r[8 * jj + 6]), "r"(r[8 * jj + 7])
                                      : "memory");
                 };
                 uint32_t ra[32], rb[32];
@@ -249,7 +244,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
             int x0, y0;
             half_origin(ht, x0, y0);
             if (y0 >= p.cam.height) continue;
-            const int U = __ldg(p.ucount + ht);
+            const int U = __ldg(p.sl.hdr + (size_t)ht * kHdrWords + 4);
             const int rounds = rounds_of(U);
             for (int c = 0; c < nunits; ++c, ++unit) {
                 const int buf = unit & 1;
@@ -290,16 +285,16 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
         // ================================================= loader ===================================================
         // lane k < 8 copies union row 8 j + k of every stage: 1 KB (256 channels) per bulk copy, kRawStages ahead
         unsigned char* raw_base = smem + MmaSmem::raw;
-        int wb = 0, wcur = 0, st = 0;
+        // (the union's ids come from the walk's lists in global memory: the loader never waits for a W build)
+        int st = 0;
         for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
             int x0, y0;
             half_origin(ht, x0, y0);
             if (y0 >= p.cam.height) continue;
-            const int U = __ldg(p.ucount + ht);
+            const int U = __ldg(p.sl.hdr + (size_t)ht * kHdrWords + 4);
             const int rounds = rounds_of(U);
             for (int c = 0; c < nunits; ++c) {
                 for (int r = 0; r < rounds; ++r) {
-                    if (c == 0 || rounds > 1) { wcur = wb++; bar_wait(&w_ready[wcur & 1], (wcur >> 1) & 1); }   // its uid_s is written
                     const int ncols = cols_of(U, r);
                     const int nk = ksteps_of(ncols);
                     for (int j = 0; j < nk; ++j, ++st) {
@@ -312,7 +307,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
                         }
                         __syncwarp();
                         if (lane < rows) {
-                            const int32_t id = uid_s[(wcur & 1) * kWCols + j * kStageRows + lane];
+                            const int32_t id = __ldg(p.sl.uid + (size_t)ht * p.sl.ucap + r * kWCols + j * kStageRows + lane);
                             tma_row(raw_base + s * kRawBytes + lane * kRawRow,
                                     static_cast<const float*>(p.features) + (int64_t)id * D + c * kUnitN, kRawRow, &raw_full[s]);
                         }
@@ -334,7 +329,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
             int x0, y0;
             half_origin(ht, x0, y0);
             if (y0 >= p.cam.height) continue;
-            const int U = __ldg(p.ucount + ht);
+            const int U = __ldg(p.sl.hdr + (size_t)ht * kHdrWords + 4);
             const int rounds = rounds_of(U);
             for (int c = 0; c < nunits; ++c) {
                 for (int r = 0; r < rounds; ++r) {
@@ -372,104 +367,63 @@ __global__ void __launch_bounds__(kMmaThreads, 1) blend_mma_kernel(const BlendPa
         }
     } else {
         // ================================================= builders =================================================
-        // W instances are built one ahead of the MMAs, alternating between two buffers (hi, lo and the union's ids):
-        // the build of half tile i + 1 overlaps the feature streaming, MMAs and epilogue of half tile i.
-        const int pw = warp - kFirstBuild;                // 0..7
+        // W (K-major, no swizzle; hi and lo) from the half tile's entry lists (qr_sel.cuh): thread = entry, one coalesced
+        // 8-byte load each, issued before the wait on the buffer they go to; clear, scatter, publish.  W instances are
+        // built one ahead of the MMAs, alternating between two buffers: the build of half tile i + 1 overlaps the
+        // feature streaming, MMAs and epilogue of half tile i.
         const int ptid = tid - kFirstBuild * 32;          // 0..255
         auto prod_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kBuildThreads) : "memory"); };
+        constexpr int kEntRegs = 4;                       // entries a builder thread holds in flight
         int wb = 0;
-        auto prefetch_l2 = [](const void* a) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a)); };
         for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
             int x0, y0;
             half_origin(ht, x0, y0);
             if (y0 >= p.cam.height) continue;
-            const int tile = ht >> 1, half = ht & 1;
-            {   // what the build of this CTA's next half tile reads (written by walk_kernel, long evicted by the map
-                // stream): fetch it into L2 now, a whole half tile ahead of its use
-                const int hn = ht + (int)gridDim.x;
-                int xn, yn;
-                half_origin(hn < num_half ? hn : ht, xn, yn);
-                if (hn < num_half && yn < p.cam.height) {
-                    if (pw == 0 && lane == 0) prefetch_l2(p.ucount + hn);
-#pragma unroll
-                    for (int gg = 0; gg < kGroupsPerBuild; ++gg) {
-                        const int g = pw * kGroupsPerBuild + gg;
-                        const int64_t group = (int64_t)(hn >> 1) * kGroupsPerTile + (hn & 1) * 16 + g;
-                        if (lane == 0) prefetch_l2(p.gcount + group);
-                        const float* recs = p.rec + group * p.cap * kRecWords;
-                        if (lane * 128 < min(p.cap, 32) * kRecWords * 4) prefetch_l2(reinterpret_cast<const char*>(recs) + lane * 128);
-                    }
-                }
-            }
-            const int U = __ldg(p.ucount + ht);
+            const int4 nq = __ldg(reinterpret_cast<const int4*>(p.sl.hdr + (size_t)ht * kHdrWords));
+            const int U = __ldg(p.sl.hdr + (size_t)ht * kHdrWords + 4);
+            const int e1 = nq.x, e2 = e1 + nq.y, e3 = e2 + nq.z, total = e3 + nq.w;
+            const uint2* ent = p.sl.ent + (size_t)ht * kSelLists * p.sl.qcap;
+            auto ent_at = [&](int f) -> uint2 {            // flat index over the four lists
+                const int q = (f >= e1) + (f >= e2) + (f >= e3);
+                const int b = q == 0 ? 0 : (q == 1 ? e1 : (q == 2 ? e2 : e3));
+                return __ldg(ent + (size_t)q * p.sl.qcap + (f - b));
+            };
             const int rounds = rounds_of(U);
             for (int c = 0; c < nunits; ++c) {
                 for (int r = 0; r < rounds; ++r) {
                     if (c == 0 || rounds > 1) {
                         // ---------------- build W for columns [64 r, 64 r + 64) ----------------
-                        // the loads of both groups of this warp are issued before anything waits on them
-                        int n_g[2];
-                        float4 wa[2], wb4[2];
-                        float2 mt[2];
+                        uint2 e[kEntRegs];
 #pragma unroll
-                        for (int gg = 0; gg < kGroupsPerBuild; ++gg) {
-                            const int g = pw * kGroupsPerBuild + gg;
-                            const int64_t group = (int64_t)tile * kGroupsPerTile + half * 16 + g;
-                            n_g[gg] = __ldg(p.gcount + group);
-                            const float* recs = p.rec + group * p.cap * kRecWords;
-                            wa[gg] = wb4[gg] = make_float4(0.f, 0.f, 0.f, 0.f);
-                            mt[gg] = make_float2(__int_as_float(-1), __int_as_float(0));
-                            if (lane < p.cap) {
-                                wa[gg] = __ldg(reinterpret_cast<const float4*>(recs + (size_t)lane * kRecWords));
-                                wb4[gg] = __ldg(reinterpret_cast<const float4*>(recs + (size_t)lane * kRecWords + 4));
-                                mt[gg] = __ldg(reinterpret_cast<const float2*>(recs + (size_t)lane * kRecWords + 8));
-                            }
+                        for (int u = 0; u < kEntRegs; ++u) {
+                            const int f = u * kBuildThreads + ptid;
+                            e[u] = f < total ? ent_at(f) : make_uint2(0u, 0xFFFFFFFFu);
                         }
                         const int wcur = wb++;                     // this W instance; it lives in buffer wcur & 1
                         bar_wait(&w_free[wcur & 1], ((wcur >> 1) & 1) ^ 1);        // the MMAs that read the buffer have retired
                         unsigned char* wbuf = smem + MmaSmem::w + (wcur & 1) * 2 * kWBytes;
-                        int32_t* uid_w = uid_s + (wcur & 1) * kWCols;
                         {
                             const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
                             float4* wz = reinterpret_cast<float4*>(wbuf);
                             for (int i = ptid; i < 2 * kWBytes / 16; i += kBuildThreads) wz[i] = z;
                         }
                         prod_sync();
+                        for (int base = 0; base == 0 || base < total; base += kEntRegs * kBuildThreads) {
+                            if (base > 0) {
 #pragma unroll
-                        for (int gg = 0; gg < kGroupsPerBuild; ++gg) {
-                            const int g = pw * kGroupsPerBuild + gg;                     // group 0..15 of the half tile
-                            const int gx = g & 3, gy = g >> 2;
-                            const int64_t group = (int64_t)tile * kGroupsPerTile + half * 16 + g;
-                            const int n = n_g[gg];
-                            const float* recs = p.rec + group * p.cap * kRecWords;
-                            for (int i0 = 0; i0 < n; i0 += 32) {
-                                const int i = i0 + lane;
-                                const bool have = i < n;
-                                float4 a = wa[gg], b = wb4[gg];
-                                float2 m2 = mt[gg];
-                                if (i0 > 0 && have) {
-                                    a = __ldg(reinterpret_cast<const float4*>(recs + (size_t)i * kRecWords));
-                                    b = __ldg(reinterpret_cast<const float4*>(recs + (size_t)i * kRecWords + 4));
-                                    m2 = __ldg(reinterpret_cast<const float2*>(recs + (size_t)i * kRecWords + 8));
+                                for (int u = 0; u < kEntRegs; ++u) {
+                                    const int f = base + u * kBuildThreads + ptid;
+                                    e[u] = f < total ? ent_at(f) : make_uint2(0u, 0xFFFFFFFFu);
                                 }
-                                const float w[kGroupPx] = { a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w };
-                                const int32_t id = __float_as_int(m2.x);
-                                const uint32_t nzcol = have ? (uint32_t)__float_as_int(m2.y) : 0u;
-                                const uint32_t nz = nzcol & 0xFFu;
-                                const int col = (int)(nzcol >> 8);
-                                const bool mine = have && (col / kWCols) == r;
-                                const int cl = col % kWCols;
-                                if (mine) uid_w[cl] = id;
+                            }
 #pragma unroll
-                                for (int q = 0; q < kGroupPx; ++q) {
-                                    const bool bit = (nz >> q) & 1u;
-                                    if (mine && bit) {
-                                        const int m = (gy * 2 + (q >> 2)) * 16 + gx * 4 + (q & 3);
-                                        const uint32_t off = w_off(m, cl);
-                                        const float hi = tf32_hi(w[q]);
-                                        *reinterpret_cast<float*>(wbuf + off) = hi;
-                                        *reinterpret_cast<float*>(wbuf + kWBytes + off) = __fsub_rn(w[q], hi);
-                                    }
+                            for (int u = 0; u < kEntRegs; ++u) {
+                                const int cl = sel_col(e[u].y) - r * kWCols;       // padding entries have column 2^17 - 1
+                                if (cl >= 0 && cl < kWCols) {
+                                    const uint32_t off = w_off(sel_pixel(e[u].y), cl);
+                                    const float w = __uint_as_float(e[u].x), hi = tf32_hi(w);
+                                    *reinterpret_cast<float*>(wbuf + off) = hi;
+                                    *reinterpret_cast<float*>(wbuf + kWBytes + off) = __fsub_rn(w, hi);
                                 }
                             }
                         }

@@ -31,6 +31,7 @@ struct FwdLayout {
     size_t ticket, gcount, ucount, rec, total;
     int64_t G;
     int cap;
+    SelLayout sel;       // selection lists of the tcgen05 path (qr_sel.cuh); they share the region of the group records
 };
 
 static FwdLayout fwd_layout(const Cam& cam, int K)
@@ -43,7 +44,8 @@ static FwdLayout fwd_layout(const Cam& cam, int K)
     L.gcount = o; o = align_up(o + (size_t)L.G * 4, 256);
     L.ucount = o; o = align_up(o + (size_t)(L.G / 16) * 4, 256);
     L.rec = o;    o = align_up(o + (size_t)L.G * L.cap * kRecWords * 4, 256);
-    L.total = o;
+    L.sel = sel_layout(cam, K, L.gcount);
+    L.total = o > L.sel.total ? o : L.sel.total;
     return L;
 }
 
@@ -992,6 +994,27 @@ extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype f
     const int T = c.tiles_x * c.tiles_y;
     char* w = static_cast<char*>(ws);
 
+    if (blend_mma_supported(D, feat_dtype)) {
+        // fp32 features, D % 256 == 0: walk2_kernel -> selection lists -> tcgen05 blend
+        if (!mean2d || !conic_opac || !isect_gauss || !features)
+            return fail(QR_ERR_NULL_POINTER, "qr_forward: NULL input");
+        WalkParams2 w2;
+        w2.cam = c; w2.K = K;
+        w2.mean2d = reinterpret_cast<const float2*>(mean2d);
+        w2.conic_opac = reinterpret_cast<const float4*>(conic_opac);
+        w2.isect = isect_gauss; w2.tile_range = reinterpret_cast<const int2*>(tile_range);
+        w2.n_sel = n_sel; w2.resid = resid_TQ; w2.sel_idx = sel_idx; w2.sel_w = sel_w;
+        w2.sl = sel_view(L.sel, ws);
+        w2.ticket = reinterpret_cast<int32_t*>(w + L.ticket);
+        if (int rc = launch_walk2(w2, st)) return rc;
+        BlendParams bp;
+        bp.cam = c; bp.K = K; bp.D = D; bp.cap = 0; bp.num_tiles = T; bp.tile_ticket = w2.ticket;
+        bp.features = features; bp.gcount = nullptr; bp.ucount = nullptr; bp.rec = nullptr;
+        bp.n_sel = n_sel; bp.resid = resid_TQ; bp.out_map = out_map; bp.sel_idx = sel_idx; bp.sel_w = sel_w;
+        bp.sl = w2.sl;
+        return launch_blend_mma(bp, st);
+    }
+
     WalkParams wp;
     wp.cam = c; wp.K = K; wp.cap = L.cap;
     wp.mean2d = reinterpret_cast<const float2*>(mean2d);
@@ -1010,7 +1033,6 @@ extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype f
     bp.cam = c; bp.K = K; bp.D = D; bp.cap = L.cap; bp.num_tiles = T; bp.tile_ticket = wp.tile_ticket;
     bp.features = features; bp.gcount = wp.gcount; bp.ucount = wp.ucount; bp.rec = wp.rec;
     bp.n_sel = n_sel; bp.resid = resid_TQ; bp.out_map = out_map; bp.sel_idx = sel_idx; bp.sel_w = sel_w;
-    if (blend_mma_supported(D, feat_dtype)) return launch_blend_mma(bp, st);
     if (feat_dtype == QR_F16) {
         if ((D + 255) / 256 == 1) return launch_blend_tu<__half, 1, 8>(bp, st);
         return launch_blend_tu<__half, 2, 8>(bp, st);

@@ -1,0 +1,89 @@
+// qr_sel.cuh -- "selection lists": what the transmittance walk (qr_walk.cu) hands to the two tensor-core contractions,
+// the forward blend (qr_blend_mma.cu) and the backward scatter (qr_backward_mma.cu).
+//
+// The unit is the 16x8-pixel half tile (128 pixels = the M extent of the forward MMA and the K extent of the backward
+// one).  For every half tile the lists hold
+//   hdr[8]            n[0..3] = entries in each of the four lists, U = number of distinct selected Gaussians (the
+//                     "union": the columns of the weight matrix W[128 px, U]), flags, 0, 0
+//   uid[U]            union column -> Gaussian id (numbered in order of first selection, any order: both contractions
+//                     sum over the columns)
+//   ent[4][32 K]      one 8-byte entry per selection {weight bits, column << 15 | slot << 7 | pixel}: the NORMALISED
+//                     weight w^Q / (1 - T^Q) (Algorithm 1 lines 8 and 20), the column of the
+//                     selected Gaussian, the slot of the selection in its pixel's record (depth order) and the pixel's
+//                     row-major index inside the half tile.  List q is written by warp q of the walk CTA; lists 0, 1
+//                     only hold pixels 0..63 and lists 2, 3 pixels 64..127 (the two W half buffers of the backward).
+// Capacities are exact upper bounds (a pixel selects at most K Gaussians), so nothing here can overflow.
+#pragma once
+#include "qr_common.cuh"
+
+namespace qr {
+
+constexpr int kHalfPx = 128;
+constexpr int kSelLists = 4;
+constexpr int kHdrWords = 8;
+
+__host__ __device__ __forceinline__ uint32_t sel_pack(int col, int slot, int pixel)
+{
+    return ((uint32_t)col << 15) | ((uint32_t)slot << 7) | (uint32_t)pixel;
+}
+__host__ __device__ __forceinline__ int sel_col(uint32_t y) { return (int)(y >> 15); }
+__host__ __device__ __forceinline__ int sel_slot(uint32_t y) { return (int)((y >> 7) & 0xFFu); }
+__host__ __device__ __forceinline__ int sel_pixel(uint32_t y) { return (int)(y & 127u); }
+
+struct SelLists {
+    int32_t* hdr = nullptr;     // [half tiles][kHdrWords]
+    int32_t* uid = nullptr;     // [half tiles][ucap]
+    uint2* ent = nullptr;       // [half tiles][kSelLists][qcap]
+    int32_t ucap = 0, qcap = 0; // 128 K, 32 K
+    int32_t* stamp = nullptr;   // [8] magic, width, height, K, low / high word of the sel_idx pointer they describe
+};
+
+struct SelLayout {
+    size_t stamp, hdr, uid, ent, total;
+    int32_t ucap, qcap;
+};
+inline SelLayout sel_layout(const Cam& cam, int K, size_t base = 0)
+{
+    const size_t nh = (size_t)cam.tiles_x * cam.tiles_y * 2;
+    SelLayout L;
+    L.ucap = kHalfPx * K;
+    L.qcap = 32 * K;
+    size_t o = base;
+    L.stamp = o; o = align_up(o + 64, 256);
+    L.hdr = o;   o = align_up(o + nh * kHdrWords * 4, 256);
+    L.uid = o;   o = align_up(o + nh * (size_t)L.ucap * 4, 256);
+    L.ent = o;   o = align_up(o + nh * kSelLists * (size_t)L.qcap * 8, 256);
+    L.total = o;
+    return L;
+}
+inline SelLists sel_view(const SelLayout& L, void* ws)
+{
+    char* w = static_cast<char*>(ws);
+    SelLists s;
+    s.stamp = reinterpret_cast<int32_t*>(w + L.stamp);
+    s.hdr = reinterpret_cast<int32_t*>(w + L.hdr);
+    s.uid = reinterpret_cast<int32_t*>(w + L.uid);
+    s.ent = reinterpret_cast<uint2*>(w + L.ent);
+    s.ucap = L.ucap; s.qcap = L.qcap;
+    return s;
+}
+constexpr int32_t kSelMagic = 0x51524c31;   // "QRL1"
+
+// qr_walk.cu
+struct WalkParams2 {
+    Cam cam;
+    int32_t K;
+    const float2* mean2d;
+    const float4* conic_opac;
+    const uint32_t* isect;
+    const int2* tile_range;
+    int32_t* n_sel;
+    float* resid;
+    int32_t* sel_idx;
+    float* sel_w;
+    SelLists sl;
+    int32_t* ticket;      // work queue of the blend kernel that follows, reset here
+};
+int launch_walk2(const WalkParams2& p, cudaStream_t st);
+
+}  // namespace qr

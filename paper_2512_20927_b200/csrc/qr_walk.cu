@@ -1,0 +1,225 @@
+// qr_walk.cu -- the O(N) part of qr_forward: Algorithm 1 lines 3-19 for every pixel.
+//
+// walk2_kernel: CTA = one 16x8-pixel half tile (4 warps), thread = pixel, warp = a WX x (32 / WX) block of pixels.
+// The tile's depth-sorted list is staged 128 entries at a time in shared memory.  Per 32 staged entries a warp first
+// runs, with lane = entry, an exact conservative test "can the Gaussian's included region (rule R4: power >= -4.5 and
+// alpha' >= 1/255) reach any pixel centre of my block" -- the minimum of the conic's quadratic form over the block's
+// rectangle against a per-Gaussian bound -- and then, with lane = pixel, walks only the surviving entries, strictly in
+// list order, in the fp32 decision arithmetic of DESIGN.md (T is carried sequentially per pixel: no scan, no
+// reordering).  The inner step is branch free: a pixel that the Gaussian does not reach, or that has already stopped,
+// takes alpha' = 0, which leaves T, k and every comparison of the listing unchanged.
+//
+// A selection (line 6) is not blended here.  The warp appends one 8-byte entry {w^Q, column | slot | pixel} to its own
+// list (no atomics: a list has one writer) and the pixel's Gaussian id to sel_idx; the column is the Gaussian's number
+// in the half tile's union of selected Gaussians, handed out on first selection (one shared-memory CAS by lane 0).
+// When its pixels have all stopped (T_test < 1/(K+1), lines 15-17) the warp normalises its entries by 1/(1 - T^Q)
+// (line 20) in place and scatters them to sel_w.  qr_sel.cuh describes the lists; the forward blend and the backward
+// scatter both consume them as they are.
+#include "qr_sel.cuh"
+
+namespace qr {
+
+constexpr int kW2Threads = 128;
+constexpr int kW2Batch = 128;
+
+__device__ __forceinline__ float clampf(float v, float lo, float hi) { return fminf(fmaxf(v, lo), hi); }
+
+// min over the rectangle [X0, X1] x [Y0, Y1] of  Q(d) = a dx^2 + 2 b dx dy + c dy^2,  d = point - mean  (power = -Q/2),
+// compared with qmax.  Q is convex: if the mean is inside the rectangle the minimum is 0, otherwise it lies on one of
+// the four edges, where Q is a 1-D parabola clamped to the edge.  NaNs answer "hit" (conservative).
+__device__ __forceinline__ bool rect_hit(float mx, float my, float a, float b, float c, float ia, float ic, float qmax,
+                                         float X0, float X1, float Y0, float Y1)
+{
+    const float dx0 = X0 - mx, dx1 = X1 - mx, dy0 = Y0 - my, dy1 = Y1 - my;
+    const bool in = dx0 <= 0.0f && dx1 >= 0.0f && dy0 <= 0.0f && dy1 >= 0.0f;
+    const float b2 = b + b;
+    float t, q, qmin;
+    t = clampf(-b * dy0 * ia, dx0, dx1); qmin = __fmaf_rn(__fmaf_rn(a, t, b2 * dy0), t, c * dy0 * dy0);
+    t = clampf(-b * dy1 * ia, dx0, dx1); q = __fmaf_rn(__fmaf_rn(a, t, b2 * dy1), t, c * dy1 * dy1); qmin = fminf(qmin, q);
+    t = clampf(-b * dx0 * ic, dy0, dy1); q = __fmaf_rn(__fmaf_rn(c, t, b2 * dx0), t, a * dx0 * dx0); qmin = fminf(qmin, q);
+    t = clampf(-b * dx1 * ic, dy0, dy1); q = __fmaf_rn(__fmaf_rn(c, t, b2 * dx1), t, a * dx1 * dx1); qmin = fminf(qmin, q);
+    if (in) qmin = 0.0f;
+    return !(qmin > qmax);
+}
+
+template <int WX>
+__global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2 p)
+{
+    constexpr int WY = 32 / WX;
+    __shared__ float4 s_co[kW2Batch];      // a, b, c, opacity
+    __shared__ float4 s_cull[kW2Batch];    // 1/a, 1/c, qmax, -
+    __shared__ float2 s_xy[kW2Batch];
+    __shared__ int32_t s_id[kW2Batch];
+    __shared__ int32_t s_col[kW2Batch];    // column of a staged entry in the union, -1 = not selected yet, -2 = being numbered
+    __shared__ float thr[QR_MAX_K + 1];
+    __shared__ int32_t s_ucount, s_finished;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int ht = blockIdx.x, tile = ht >> 1;
+    const int K = p.K;
+    const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
+    int32_t* hdr = p.sl.hdr + (size_t)ht * kHdrWords;
+    if (ht == 0 && tid == 0) {
+        *p.ticket = 0;
+        p.sl.stamp[0] = kSelMagic; p.sl.stamp[1] = p.cam.width; p.sl.stamp[2] = p.cam.height; p.sl.stamp[3] = K;
+        const unsigned long long a = (unsigned long long)p.sel_idx;
+        p.sl.stamp[4] = (int32_t)(a & 0xffffffffull); p.sl.stamp[5] = (int32_t)(a >> 32);
+    }
+    if (y0 >= p.cam.height) {                         // half tile below the image: empty lists
+        if (tid < kHdrWords) hdr[tid] = 0;
+        return;
+    }
+    // block of this warp and pixel of this lane
+    const int bx0 = WX == 16 ? 0 : 8 * (warp & 1), by0 = WX == 16 ? 2 * warp : 4 * (warp >> 1);
+    const int lx = lane & (WX - 1), ly = lane / WX;
+    const int mpix = (by0 + ly) * kTile + bx0 + lx;   // row-major index inside the half tile
+    const int px = x0 + bx0 + lx, py = y0 + by0 + ly;
+    const bool inside = px < p.cam.width && py < p.cam.height;
+    const float fpx = (float)px + 0.5f, fpy = (float)py + 0.5f;          // R5
+    const float X0 = (float)(x0 + bx0) + 0.5f, X1 = X0 + (float)(WX - 1);
+    const float Y0 = (float)(y0 + by0) + 0.5f, Y1 = Y0 + (float)(WY - 1);
+    const int64_t pix = (int64_t)py * p.cam.width + px;
+    int32_t* my_idx = p.sel_idx + pix * K;
+    uint2* my_ent = p.sl.ent + ((size_t)ht * kSelLists + warp) * p.sl.qcap;
+    int32_t* uid_g = p.sl.uid + (size_t)ht * p.sl.ucap;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+
+    for (int k = tid; k <= K; k += kW2Threads)                            // thresholds as printed (R3)
+        thr[k] = __fsub_rn(1.0f, __fdiv_rn((float)(k + 1), (float)(K + 1)));
+    const float t_break = __fdiv_rn(1.0f, (float)(K + 1));
+    if (tid == 0) { s_ucount = 0; s_finished = 0; }
+    const int2 range = p.tile_range[tile];
+    __syncthreads();
+
+    bool done = !inside;
+    float T = 1.0f, TQ = 1.0f;
+    float thr_k = __fsub_rn(1.0f, __fdiv_rn(1.0f, (float)(K + 1)));      // thr[k], k = 0
+    int k = 0, ns = 0, n_ent = 0;
+    bool warp_done = __all_sync(0xffffffffu, done);
+
+    for (int b0 = range.x; b0 < range.y; b0 += kW2Batch) {
+        if (__syncthreads_and(warp_done)) break;                          // every pixel of the half tile has stopped
+        {   // ---- stage the batch ----
+            const int idx = b0 + tid;
+            int32_t id = -1;
+            float4 co = make_float4(1.f, 0.f, 1.f, 0.f), cull = make_float4(1.f, 1.f, -1.f, 0.f);   // never hit
+            float2 xy = make_float2(0.f, 0.f);
+            if (idx < range.y) {
+                id = (int32_t)p.isect[idx];
+                xy = __ldg(p.mean2d + id);
+                co = __ldg(p.conic_opac + id);
+                // included  =>  Q <= 9 (power >= -4.5)  and  opacity exp(-Q/2) >= 1/255  <=>  Q <= 2 ln(255 opacity).
+                // 1e-4 relative + 1e-3 absolute slack covers the different rounding of Q here and of `power` below.
+                float qmax = fminf(9.0f, 2.0f * __logf(255.0f * co.w)) * 1.0001f + 1e-3f;
+                const bool valid = co.x > 0.0f && co.z > 0.0f && co.x * co.z - co.y * co.y > 0.0f;
+                float ia = 0.0f, ic = 0.0f;
+                if (valid) { ia = 1.0f / co.x; ic = 1.0f / co.z; }
+                else qmax = 3.0e38f;                                      // odd conic: never culled
+                if (!(co.w > 0.0f)) qmax = -1.0f;                         // alpha' = 0 < 1/255 everywhere
+                cull = make_float4(ia, ic, qmax, 0.f);
+            }
+            s_id[tid] = id; s_co[tid] = co; s_xy[tid] = xy; s_cull[tid] = cull; s_col[tid] = -1;
+        }
+        __syncthreads();
+        if (warp_done) continue;
+        const int nb = min(kW2Batch, range.y - b0);
+
+        for (int c = 0; c < nb; c += 32) {
+            uint32_t m;
+            {   // lane = entry: which of these 32 Gaussians can reach a pixel centre of my block
+                const float4 co = s_co[c + lane], cu = s_cull[c + lane];
+                const float2 xy = s_xy[c + lane];
+                m = __ballot_sync(0xffffffffu, rect_hit(xy.x, xy.y, co.x, co.y, co.z, cu.x, cu.y, cu.z, X0, X1, Y0, Y1));
+            }
+            while (m) {                                   // lane = pixel
+                const int e = c + __ffs(m) - 1;
+                m &= m - 1;
+                const float4 co = s_co[e];
+                const float2 xy = s_xy[e];
+                // alpha' (Eq. 1) with inclusion rule R4, fp32 decision arithmetic
+                const float dx = __fsub_rn(fpx, xy.x), dy = __fsub_rn(fpy, xy.y);
+                const float q1 = __fmul_rn(__fmul_rn(co.x, dx), dx);
+                const float q2 = __fmaf_rn(__fmul_rn(co.z, dy), dy, q1);
+                const float q3 = __fmul_rn(__fmul_rn(co.y, dx), dy);
+                const float power = __fmaf_rn(-0.5f, q2, -q3);
+                float a = fminf(kAlphaMax, __fmul_rn(co.w, expf(power)));
+                if (done || power > 0.0f || power < kPowerMin || a < kAlphaMin) a = 0.0f;   // not in I for this pixel
+                const float oma = __fsub_rn(1.0f, a);
+                const float T_test = __fmul_rn(T, oma);                                  // line 5
+                const bool sel = T_test < thr_k;                                         // line 6
+                const uint32_t sm = __ballot_sync(0xffffffffu, sel);
+                if (sm) {
+                    // column of this Gaussian in the half tile's union: the first warp to select it numbers it
+                    int col = 0;
+                    if (lane == 0) {
+                        volatile int32_t* slot = &s_col[e];
+                        const int old = atomicCAS(&s_col[e], -1, -2);
+                        if (old == -1) {
+                            col = atomicAdd(&s_ucount, 1);
+                            uid_g[col] = s_id[e];
+                            *slot = col;
+                        } else {
+                            col = old;
+                            while (col == -2) col = *slot;
+                        }
+                    }
+                    col = __shfl_sync(0xffffffffu, col, 0);
+                    if (sel) {
+                        const float wQ = __fmul_rn(TQ, a);                               // line 8
+                        my_idx[ns] = s_id[e];
+                        my_ent[n_ent + __popc(sm & lt_mask)] = make_uint2(__float_as_uint(wQ), sel_pack(col, ns, mpix));
+                        ++ns;                                                            // line 9 runs in the blend
+                        k = k + 1;                                                       // line 7
+                        TQ = __fmul_rn(TQ, oma);                                         // line 10
+                        while (T_test < thr[k]) k = k + 1;                               // lines 11-13
+                        thr_k = thr[k];
+                    }
+                    n_ent += __popc(sm);
+                }
+                if (T_test < t_break) done = true;                                       // lines 15-17
+                else T = T_test;                                                         // line 18
+            }
+            if (__all_sync(0xffffffffu, done)) { warp_done = true; break; }
+        }
+    }
+
+    // ---- the warp's pixels: n_sel, T^Q; its entries: x 1/(1 - T^Q) (line 20), scattered to sel_w ----
+    const float inv = ns > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, TQ)) : 0.0f;
+    if (inside) {
+        p.n_sel[pix] = ns;
+        p.resid[pix] = ns > 0 ? TQ : 1.0f;                                               // R8
+    }
+    __syncwarp();
+    for (int i0 = 0; i0 < n_ent; i0 += 32) {
+        const int i = i0 + lane;
+        const bool have = i < n_ent;
+        uint2 en = make_uint2(0u, 0u);
+        if (have) en = __ldcg(my_ent + i);
+        const int pm = sel_pixel(en.y);
+        const int src = WX == 16 ? (pm & 31) : (((pm >> 4) & 3) * 8 + (pm & 7));         // lane that owns pixel pm
+        const float inv_p = __shfl_sync(0xffffffffu, inv, src);
+        if (have) {
+            const float w = __fmul_rn(__uint_as_float(en.x), inv_p);
+            my_ent[i].x = __float_as_uint(w);
+            const int64_t q = (int64_t)(y0 + (pm >> 4)) * p.cam.width + x0 + (pm & 15);
+            p.sel_w[q * K + sel_slot(en.y)] = w;
+        }
+    }
+    if (lane == 0) {
+        hdr[warp] = n_ent;
+        __threadfence_block();
+        if (atomicAdd(&s_finished, 1) == kSelLists - 1) {      // the last warp of the half tile publishes the union size
+            hdr[4] = s_ucount; hdr[5] = 0; hdr[6] = 0; hdr[7] = 0;
+        }
+    }
+}
+
+int launch_walk2(const WalkParams2& p, cudaStream_t st)
+{
+    const unsigned grid = (unsigned)(p.cam.tiles_x * p.cam.tiles_y * 2);
+    walk2_kernel<16><<<grid, kW2Threads, 0, st>>>(p);
+    QR_LAUNCH_OK("walk2_kernel");
+    return QR_OK;
+}
+
+}  // namespace qr
