@@ -1005,10 +1005,9 @@ extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype f
         w2.isect = isect_gauss; w2.tile_range = reinterpret_cast<const int2*>(tile_range);
         w2.n_sel = n_sel; w2.resid = resid_TQ; w2.sel_idx = sel_idx; w2.sel_w = sel_w;
         w2.sl = sel_view(L.sel, ws);
-        w2.ticket = reinterpret_cast<int32_t*>(w + L.ticket);
         if (int rc = launch_walk2(w2, st)) return rc;
         BlendParams bp;
-        bp.cam = c; bp.K = K; bp.D = D; bp.cap = 0; bp.num_tiles = T; bp.tile_ticket = w2.ticket;
+        bp.cam = c; bp.K = K; bp.D = D; bp.cap = 0; bp.num_tiles = T; bp.tile_ticket = nullptr;
         bp.features = features; bp.gcount = nullptr; bp.ucount = nullptr; bp.rec = nullptr;
         bp.n_sel = n_sel; bp.resid = resid_TQ; bp.out_map = out_map; bp.sel_idx = sel_idx; bp.sel_w = sel_w;
         bp.sl = w2.sl;

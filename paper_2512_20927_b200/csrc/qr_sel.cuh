@@ -3,8 +3,11 @@
 //
 // The unit is the 16x8-pixel half tile (128 pixels = the M extent of the forward MMA and the K extent of the backward
 // one).  For every half tile the lists hold
-//   hdr[8]            n[0..3] = entries in each of the four lists, U = number of distinct selected Gaussians (the
-//                     "union": the columns of the weight matrix W[128 px, U]), flags, 0, 0
+//   hdr[16]           n[0..3] = entries in each of the four lists, U = number of distinct selected Gaussians (the
+//                     "union": the columns of the weight matrix W[128 px, U]), flags; then the walk's work counters,
+//                     read only by bench.py's untimed statistics: [6] tile-list entries consumed before every pixel
+//                     had stopped, [7] (entry, warp) pairs that survived the culling test (x 32 = alpha' evaluations),
+//                     [8] SM clock cycles the half tile's CTA took
 //   uid[U]            union column -> Gaussian id (numbered in order of first selection, any order: both contractions
 //                     sum over the columns)
 //   ent[4][32 K]      one 8-byte entry per selection {weight bits, column << 15 | slot << 7 | pixel}: the NORMALISED
@@ -20,7 +23,7 @@ namespace qr {
 
 constexpr int kHalfPx = 128;
 constexpr int kSelLists = 4;
-constexpr int kHdrWords = 8;
+constexpr int kHdrWords = 16;
 
 __host__ __device__ __forceinline__ uint32_t sel_pack(int col, int slot, int pixel)
 {
@@ -36,10 +39,13 @@ struct SelLists {
     uint2* ent = nullptr;       // [half tiles][kSelLists][qcap]
     int32_t ucap = 0, qcap = 0; // 128 K, 32 K
     int32_t* stamp = nullptr;   // [8] magic, width, height, K, low / high word of the sel_idx pointer they describe
+    int32_t* ctrl = nullptr;    // [kCtrlWords] [0] the walk's half-tile ticket, [1] the blend's; zeroed per frame
+    int32_t* flags = nullptr;   // [half tiles] directly behind ctrl: 1 = the half tile's lists are complete (released)
 };
+constexpr int kCtrlWords = 64;
 
 struct SelLayout {
-    size_t stamp, hdr, uid, ent, total;
+    size_t stamp, ctrl, hdr, uid, ent, total;
     int32_t ucap, qcap;
 };
 inline SelLayout sel_layout(const Cam& cam, int K, size_t base = 0)
@@ -50,6 +56,7 @@ inline SelLayout sel_layout(const Cam& cam, int K, size_t base = 0)
     L.qcap = 32 * K;
     size_t o = base;
     L.stamp = o; o = align_up(o + 64, 256);
+    L.ctrl = o;  o = align_up(o + ((size_t)kCtrlWords + nh) * 4, 256);
     L.hdr = o;   o = align_up(o + nh * kHdrWords * 4, 256);
     L.uid = o;   o = align_up(o + nh * (size_t)L.ucap * 4, 256);
     L.ent = o;   o = align_up(o + nh * kSelLists * (size_t)L.qcap * 8, 256);
@@ -61,6 +68,8 @@ inline SelLists sel_view(const SelLayout& L, void* ws)
     char* w = static_cast<char*>(ws);
     SelLists s;
     s.stamp = reinterpret_cast<int32_t*>(w + L.stamp);
+    s.ctrl = reinterpret_cast<int32_t*>(w + L.ctrl);
+    s.flags = s.ctrl + kCtrlWords;
     s.hdr = reinterpret_cast<int32_t*>(w + L.hdr);
     s.uid = reinterpret_cast<int32_t*>(w + L.uid);
     s.ent = reinterpret_cast<uint2*>(w + L.ent);
@@ -82,7 +91,6 @@ struct WalkParams2 {
     int32_t* sel_idx;
     float* sel_w;
     SelLists sl;
-    int32_t* ticket;      // work queue of the blend kernel that follows, reset here
 };
 int launch_walk2(const WalkParams2& p, cudaStream_t st);
 

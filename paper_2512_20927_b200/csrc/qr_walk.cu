@@ -16,6 +16,7 @@
 // (line 20) in place and scatters them to sel_w.  qr_sel.cuh describes the lists; the forward blend and the backward
 // scatter both consume them as they are.
 #include "qr_sel.cuh"
+#include <stdlib.h>
 
 namespace qr {
 
@@ -23,6 +24,10 @@ constexpr int kW2Threads = 128;
 constexpr int kW2Batch = 128;
 
 __device__ __forceinline__ float clampf(float v, float lo, float hi) { return fminf(fmaxf(v, lo), hi); }
+__device__ __forceinline__ void st_release(int32_t* p, int32_t v)
+{
+    asm volatile("st.release.gpu.global.b32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
 
 // min over the rectangle [X0, X1] x [Y0, Y1] of  Q(d) = a dx^2 + 2 b dx dy + c dy^2,  d = point - mean  (power = -Q/2),
 // compared with qmax.  Q is convex: if the mean is inside the rectangle the minimum is 0, otherwise it lies on one of
@@ -52,22 +57,44 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
     __shared__ int32_t s_id[kW2Batch];
     __shared__ int32_t s_col[kW2Batch];    // column of a staged entry in the union, -1 = not selected yet, -2 = being numbered
     __shared__ float thr[QR_MAX_K + 1];
-    __shared__ int32_t s_ucount, s_finished;
+    __shared__ int32_t s_ucount, s_finished, s_evals, s_consumed;
 
+    __shared__ int32_t s_ht;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int ht = blockIdx.x, tile = ht >> 1;
     const int K = p.K;
-    const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
-    int32_t* hdr = p.sl.hdr + (size_t)ht * kHdrWords;
-    if (ht == 0 && tid == 0) {
-        *p.ticket = 0;
+    const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    const uint32_t s_col_addr = (uint32_t)__cvta_generic_to_shared(s_col);
+    const uint32_t s_ucount_addr = (uint32_t)__cvta_generic_to_shared(&s_ucount);
+    const uint32_t s_co_addr = (uint32_t)__cvta_generic_to_shared(s_co);
+    const uint32_t s_xy_addr = (uint32_t)__cvta_generic_to_shared(s_xy);
+    const uint32_t s_id_addr = (uint32_t)__cvta_generic_to_shared(s_id);
+    const uint32_t thr_addr = (uint32_t)__cvta_generic_to_shared(thr);
+    for (int k = tid; k <= K; k += kW2Threads)                            // thresholds as printed (R3)
+        thr[k] = __fsub_rn(1.0f, __fdiv_rn((float)(k + 1), (float)(K + 1)));
+    const float t_break = __fdiv_rn(1.0f, (float)(K + 1));
+    if (blockIdx.x == 0 && tid == 0) {
         p.sl.stamp[0] = kSelMagic; p.sl.stamp[1] = p.cam.width; p.sl.stamp[2] = p.cam.height; p.sl.stamp[3] = K;
         const unsigned long long a = (unsigned long long)p.sel_idx;
         p.sl.stamp[4] = (int32_t)(a & 0xffffffffull); p.sl.stamp[5] = (int32_t)(a >> 32);
     }
+
+  // Persistent CTAs: half tiles are handed out in index order by a global ticket (the blend kernel, which may already be
+  // running, consumes them in the same order); when a half tile's lists are complete its ready flag is released.
+  while (true) {
+    __syncthreads();                                   // everybody is through with the previous half tile's shared state
+    if (tid == 0) { s_ht = atomicAdd(p.sl.ctrl, 1); s_ucount = 0; s_finished = 0; s_evals = 0; s_consumed = 0; }
+    __syncthreads();
+    const int ht = s_ht;
+    if (ht >= num_half) break;
+    const int tile = ht >> 1;
+    const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
+    int32_t* hdr = p.sl.hdr + (size_t)ht * kHdrWords;
     if (y0 >= p.cam.height) {                         // half tile below the image: empty lists
         if (tid < kHdrWords) hdr[tid] = 0;
-        return;
+        __syncthreads();
+        if (tid == 0) { __threadfence(); st_release(p.sl.flags + ht, 1); }
+        continue;
     }
     // block of this warp and pixel of this lane
     const int bx0 = WX == 16 ? 0 : 8 * (warp & 1), by0 = WX == 16 ? 2 * warp : 4 * (warp >> 1);
@@ -82,20 +109,82 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
     int32_t* my_idx = p.sel_idx + pix * K;
     uint2* my_ent = p.sl.ent + ((size_t)ht * kSelLists + warp) * p.sl.qcap;
     int32_t* uid_g = p.sl.uid + (size_t)ht * p.sl.ucap;
-    const uint32_t lt_mask = (1u << lane) - 1u;
-
-    for (int k = tid; k <= K; k += kW2Threads)                            // thresholds as printed (R3)
-        thr[k] = __fsub_rn(1.0f, __fdiv_rn((float)(k + 1), (float)(K + 1)));
-    const float t_break = __fdiv_rn(1.0f, (float)(K + 1));
-    if (tid == 0) { s_ucount = 0; s_finished = 0; }
+    const long long t_start = clock64();
     const int2 range = p.tile_range[tile];
-    __syncthreads();
 
     bool done = !inside;
     float T = 1.0f, TQ = 1.0f;
     float thr_k = __fsub_rn(1.0f, __fdiv_rn(1.0f, (float)(K + 1)));      // thr[k], k = 0
-    int k = 0, ns = 0, n_ent = 0;
+    int k = 0, ns = 0, n_ent = 0, n_eval = 0, consumed = 0;
+    int32_t* idx_ptr = my_idx;                  // next slot of this pixel's selection record
+    uint2* ent_ptr = my_ent;                    // end of this warp's entry list (warp-uniform)
+    uint32_t slotpix = (uint32_t)mpix;          // slot << 7 | pixel of this pixel's next entry
     bool warp_done = __all_sync(0xffffffffu, done);
+
+    // alpha' of staged entry e at this pixel (Eq. 1) with inclusion rule R4, fp32 decision arithmetic;
+    // 0 = the Gaussian is not in I for this pixel
+    auto alpha_of = [&](int e) -> float {
+        float4 co; float2 xy;
+        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(co.x), "=f"(co.y), "=f"(co.z), "=f"(co.w) : "r"(s_co_addr + 16u * (uint32_t)e));
+        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(xy.x), "=f"(xy.y) : "r"(s_xy_addr + 8u * (uint32_t)e));
+        const float dx = __fsub_rn(fpx, xy.x), dy = __fsub_rn(fpy, xy.y);
+        const float q1 = __fmul_rn(__fmul_rn(co.x, dx), dx);
+        const float q2 = __fmaf_rn(__fmul_rn(co.z, dy), dy, q1);
+        const float q3 = __fmul_rn(__fmul_rn(co.y, dx), dy);
+        const float power = __fmaf_rn(-0.5f, q2, -q3);
+        float a = fminf(kAlphaMax, __fmul_rn(co.w, expf(power)));
+        if (power > 0.0f || power < kPowerMin || a < kAlphaMin) a = 0.0f;
+        return a;
+    };
+    // Algorithm 1 lines 5-18 for staged entry e with this pixel's alpha' = a (0: a no-op, T_test = T)
+    auto step = [&](int e, float a) {
+        if (done) a = 0.0f;
+        const float oma = __fsub_rn(1.0f, a);
+        const float T_test = __fmul_rn(T, oma);                                  // line 5
+        const bool sel = T_test < thr_k;                                         // line 6
+        const uint32_t sm = __ballot_sync(0xffffffffu, sel);
+        if (sm) {
+            // column of this Gaussian in the half tile's union: the first warp to select it numbers it
+            int col = 0;
+            int32_t id;
+            asm volatile("ld.shared.b32 %0, [%1];" : "=r"(id) : "r"(s_id_addr + 4u * (uint32_t)e));
+            if (lane == 0) {
+                const uint32_t slot = s_col_addr + 4u * (uint32_t)e;
+                int old;
+                asm volatile("atom.shared.cas.b32 %0, [%1], -1, -2;" : "=r"(old) : "r"(slot) : "memory");
+                if (old == -1) {
+                    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(col) : "r"(s_ucount_addr) : "memory");
+                    uid_g[col] = id;
+                    asm volatile("st.volatile.shared.b32 [%0], %1;" ::"r"(slot), "r"(col) : "memory");
+                } else {
+                    col = old;
+                    while (col == -2) asm volatile("ld.volatile.shared.b32 %0, [%1];" : "=r"(col) : "r"(slot) : "memory");
+                }
+            }
+            col = __shfl_sync(0xffffffffu, col, 0);
+            if (sel) {
+                const float wQ = __fmul_rn(TQ, a);                               // line 8
+                *idx_ptr++ = id;
+                ent_ptr[__popc(sm & lt_mask)] = make_uint2(__float_as_uint(wQ), ((uint32_t)col << 15) | slotpix);
+                slotpix += 128u;                                                 // next slot of this pixel
+                ++ns;                                                            // line 9 runs in the blend
+                k = k + 1;                                                       // line 7
+                TQ = __fmul_rn(TQ, oma);                                         // line 10
+                float tk;
+                while (true) {                                                   // lines 11-13
+                    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(tk) : "r"(thr_addr + 4u * (uint32_t)k));
+                    if (!(T_test < tk)) break;
+                    k = k + 1;
+                }
+                thr_k = tk;
+            }
+            const int ne = __popc(sm);
+            ent_ptr += ne;
+            n_ent += ne;
+        }
+        if (T_test < t_break) done = true;                                       // lines 15-17
+        else T = T_test;                                                         // line 18
+    };
 
     for (int b0 = range.x; b0 < range.y; b0 += kW2Batch) {
         if (__syncthreads_and(warp_done)) break;                          // every pixel of the half tile has stopped
@@ -123,6 +212,7 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
         __syncthreads();
         if (warp_done) continue;
         const int nb = min(kW2Batch, range.y - b0);
+        consumed = b0 + nb - range.x;
 
         for (int c = 0; c < nb; c += 32) {
             uint32_t m;
@@ -131,53 +221,19 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
                 const float2 xy = s_xy[c + lane];
                 m = __ballot_sync(0xffffffffu, rect_hit(xy.x, xy.y, co.x, co.y, co.z, cu.x, cu.y, cu.z, X0, X1, Y0, Y1));
             }
-            while (m) {                                   // lane = pixel
-                const int e = c + __ffs(m) - 1;
+            n_eval += __popc(m);
+            // lane = pixel.  Two surviving entries per iteration: their alpha' evaluations are independent and
+            // interleave; the transmittance steps (lines 5-18) then run one after the other, in list order.
+            while (m) {
+                const int e0 = c + __ffs(m) - 1;
                 m &= m - 1;
-                const float4 co = s_co[e];
-                const float2 xy = s_xy[e];
-                // alpha' (Eq. 1) with inclusion rule R4, fp32 decision arithmetic
-                const float dx = __fsub_rn(fpx, xy.x), dy = __fsub_rn(fpy, xy.y);
-                const float q1 = __fmul_rn(__fmul_rn(co.x, dx), dx);
-                const float q2 = __fmaf_rn(__fmul_rn(co.z, dy), dy, q1);
-                const float q3 = __fmul_rn(__fmul_rn(co.y, dx), dy);
-                const float power = __fmaf_rn(-0.5f, q2, -q3);
-                float a = fminf(kAlphaMax, __fmul_rn(co.w, expf(power)));
-                if (done || power > 0.0f || power < kPowerMin || a < kAlphaMin) a = 0.0f;   // not in I for this pixel
-                const float oma = __fsub_rn(1.0f, a);
-                const float T_test = __fmul_rn(T, oma);                                  // line 5
-                const bool sel = T_test < thr_k;                                         // line 6
-                const uint32_t sm = __ballot_sync(0xffffffffu, sel);
-                if (sm) {
-                    // column of this Gaussian in the half tile's union: the first warp to select it numbers it
-                    int col = 0;
-                    if (lane == 0) {
-                        volatile int32_t* slot = &s_col[e];
-                        const int old = atomicCAS(&s_col[e], -1, -2);
-                        if (old == -1) {
-                            col = atomicAdd(&s_ucount, 1);
-                            uid_g[col] = s_id[e];
-                            *slot = col;
-                        } else {
-                            col = old;
-                            while (col == -2) col = *slot;
-                        }
-                    }
-                    col = __shfl_sync(0xffffffffu, col, 0);
-                    if (sel) {
-                        const float wQ = __fmul_rn(TQ, a);                               // line 8
-                        my_idx[ns] = s_id[e];
-                        my_ent[n_ent + __popc(sm & lt_mask)] = make_uint2(__float_as_uint(wQ), sel_pack(col, ns, mpix));
-                        ++ns;                                                            // line 9 runs in the blend
-                        k = k + 1;                                                       // line 7
-                        TQ = __fmul_rn(TQ, oma);                                         // line 10
-                        while (T_test < thr[k]) k = k + 1;                               // lines 11-13
-                        thr_k = thr[k];
-                    }
-                    n_ent += __popc(sm);
-                }
-                if (T_test < t_break) done = true;                                       // lines 15-17
-                else T = T_test;                                                         // line 18
+                const bool two = m != 0;
+                const int e1 = two ? c + __ffs(m) - 1 : e0;
+                m &= m - 1;
+                float a0 = alpha_of(e0), a1 = alpha_of(e1);
+                if (!two) a1 = 0.0f;
+                step(e0, a0);
+                step(e1, a1);
             }
             if (__all_sync(0xffffffffu, done)) { warp_done = true; break; }
         }
@@ -190,33 +246,58 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
         p.resid[pix] = ns > 0 ? TQ : 1.0f;                                               // R8
     }
     __syncwarp();
-    for (int i0 = 0; i0 < n_ent; i0 += 32) {
-        const int i = i0 + lane;
-        const bool have = i < n_ent;
-        uint2 en = make_uint2(0u, 0u);
-        if (have) en = __ldcg(my_ent + i);
-        const int pm = sel_pixel(en.y);
-        const int src = WX == 16 ? (pm & 31) : (((pm >> 4) & 3) * 8 + (pm & 7));         // lane that owns pixel pm
-        const float inv_p = __shfl_sync(0xffffffffu, inv, src);
-        if (have) {
-            const float w = __fmul_rn(__uint_as_float(en.x), inv_p);
-            my_ent[i].x = __float_as_uint(w);
-            const int64_t q = (int64_t)(y0 + (pm >> 4)) * p.cam.width + x0 + (pm & 15);
-            p.sel_w[q * K + sel_slot(en.y)] = w;
+    constexpr int kPre = 8;                     // entries a lane re-reads at once: the L2 round trips overlap
+    for (int i0 = 0; i0 < n_ent; i0 += 32 * kPre) {
+        uint2 en[kPre];
+#pragma unroll
+        for (int u = 0; u < kPre; ++u) {
+            const int i = i0 + u * 32 + lane;
+            en[u] = i < n_ent ? __ldcg(my_ent + i) : make_uint2(0u, 0u);
+        }
+#pragma unroll
+        for (int u = 0; u < kPre; ++u) {
+            const int i = i0 + u * 32 + lane;
+            const int pm = sel_pixel(en[u].y);
+            const int src = WX == 16 ? (pm & 31) : (((pm >> 4) & 3) * 8 + (pm & 7));     // lane that owns pixel pm
+            const float inv_p = __shfl_sync(0xffffffffu, inv, src);
+            if (i < n_ent) {
+                const float w = __fmul_rn(__uint_as_float(en[u].x), inv_p);
+                my_ent[i].x = __float_as_uint(w);
+                const int64_t q = (int64_t)(y0 + (pm >> 4)) * p.cam.width + x0 + (pm & 15);
+                p.sel_w[q * K + sel_slot(en[u].y)] = w;
+            }
         }
     }
+    __syncwarp();
     if (lane == 0) {
         hdr[warp] = n_ent;
-        __threadfence_block();
-        if (atomicAdd(&s_finished, 1) == kSelLists - 1) {      // the last warp of the half tile publishes the union size
-            hdr[4] = s_ucount; hdr[5] = 0; hdr[6] = 0; hdr[7] = 0;
+        atomicAdd(&s_evals, n_eval);
+        atomicMax(&s_consumed, consumed);
+        __threadfence();                                       // this warp's lists, records and uid entries
+        if (atomicAdd(&s_finished, 1) == kSelLists - 1) {      // the last warp of the half tile publishes it
+            hdr[4] = s_ucount; hdr[5] = 0;
+            hdr[6] = s_consumed; hdr[7] = s_evals; hdr[8] = (int32_t)(clock64() - t_start);
+            __threadfence();
+            st_release(p.sl.flags + ht, 1);
         }
     }
+  }
 }
 
 int launch_walk2(const WalkParams2& p, cudaStream_t st)
 {
-    const unsigned grid = (unsigned)(p.cam.tiles_x * p.cam.tiles_y * 2);
+    const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
+    // tickets and ready flags of this frame
+    QR_CUDA_OK(cudaMemsetAsync(p.sl.ctrl, 0, (size_t)(kCtrlWords + num_half) * 4, st));
+    static int sms = 0, per_sm = 0;
+    if (sms == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+            sms = 148;
+        const char* e = getenv("QR_WALK_CTAS");   // EXPERIMENT
+        per_sm = e ? atoi(e) : 10;
+    }
+    const unsigned grid = (unsigned)min(num_half, sms * per_sm);
     walk2_kernel<16><<<grid, kW2Threads, 0, st>>>(p);
     QR_LAUNCH_OK("walk2_kernel");
     return QR_OK;
