@@ -20,6 +20,16 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
         "@P1 bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
         ::"r"(s32(bar)), "r"(parity) : "memory");
 }
+// the same wait with a suspend-time hint (ns): the warp sleeps in hardware until the phase completes (or the hint runs
+// out) instead of re-issuing try_wait every few hundred cycles -- for kernels that share their SM with issue-bound work
+__device__ __forceinline__ void mbar_wait_quiet(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred P1;\n\tWAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, %2;\n\t"
+        "@P1 bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
+        ::"r"(s32(bar)), "r"(parity), "r"(20000u) : "memory");
+}
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s32(bar)) : "memory");

@@ -12,20 +12,25 @@
 // W_hi F_hi + W_lo F_hi + W_hi F_lo in fp32 (TMEM).  The dropped W_lo F_lo term and the truncation of the lo parts
 // are <= 2^-21 relative per product, 40x below the fp32 tolerance of north_star (1e-4 relative).
 //
-// One persistent CTA per SM, 16 warps (512 threads, <= 64 registers: the kernel is meant to share its SM with CTAs of
-// walk2_kernel, which it follows by programmatic dependent launch), roles by warp, no role ever waits at a block barrier:
+// One persistent CTA per SM, 16 warps (512 threads, <= 64 registers, ~155 KB of shared memory: the kernel is meant to
+// share its SM with CTAs of walk2_kernel, which it follows by programmatic dependent launch), roles by warp, no role
+// ever waits at a block barrier:
 //   warps 0..3    epilogue: tcgen05.ld of the accumulator (thread = pixel), st.shared into a 128-byte-swizzled staging
 //                 tile, one TMA tensor store per (32 pixels x 32 channels): the map leaves the SM as whole 128-byte lines
-//   warp  4       MMA issue: warp-uniform loop, one elected lane issues tcgen05.mma (M = 128 pixels, N = 256 channels,
-//                 K = 8 union rows per instruction) and tcgen05.commit
-//   warp  5       loader: one bulk async copy (TMA) per feature row half (1 KB) into a raw ring, ahead of use
+//   warp  4       MMA issue: warp-uniform loop, one elected lane issues tcgen05.mma (M = 128 pixels, N = 128 channels,
+//                 K = 8 union rows per instruction; A = W from TENSOR MEMORY, B = features from shared memory)
+//   warps 5..7    loaders (stage st belongs to warp 5 + st % 3: issuing the copies was the pipeline's bottleneck with one
+//                 warp): one bulk async copy (TMA) per 512-byte feature row quarter into a 12-deep raw ring
 //   warps 8..11   converters: ld.shared of a raw row -> hi/lo split -> st.shared in the MN-major
 //                 SWIZZLE_128B_BASE32B layout tf32 needs for a row-major (channel-contiguous) B operand
 //   warps 12..15  builders: claim the next half tile (global ticket, same order as the walk), wait for its ready flag,
-//                 publish its descriptor to the other roles, then build W (K-major, no swizzle; hi and lo) from the
-//                 entry lists: thread = entry, loads issued before the wait on the buffer
-// Work unit = (half tile, 256-channel half): two 256-column accumulators in TMEM, so the MMAs of unit i+1 overlap the
-// epilogue of unit i.  A half tile whose union exceeds 64 columns is processed in rounds of 64 columns.
+//                 publish its descriptor to the other roles; scatter the entry lists into a [128 px][64 col] scratch tile
+//                 in shared memory (thread = entry), then, thread = pixel = TMEM lane, read the pixel's row back, split
+//                 it and tcgen05.st it into one of two W buffers in tensor memory.  W never sits in shared memory while
+//                 the MMAs run, and the build of half tile i + 1 overlaps all of half tile i.
+// Tensor memory: columns [0, 256) two 128-column accumulators (the MMAs of unit i+1 overlap the epilogue of unit i),
+// [256, 512) two W buffers of 64 hi + 64 lo columns.  Work unit = (half tile, 128 channels).  A half tile whose union
+// exceeds 64 columns is processed in rounds of 64 columns (two rounds keep both W instances resident).
 #include <cuda.h>
 
 #include "qr_async.cuh"
@@ -37,38 +42,45 @@ using namespace aq;
 
 constexpr int kEpiWarps = 4;
 constexpr int kMmaWarp = 4;
-constexpr int kLoadWarp = 5;
-constexpr int kFirstConv = 8;
-constexpr int kConvWarps = 4;                             // two union rows of every stage each
+constexpr int kLoadWarp = 5;                              // warps 5, 6, 7: stage st is loaded by warp 5 + st % 3
+constexpr int kLoadWarps = 3;
+constexpr int kSchedWarp = 8;
+constexpr int kFirstConv = 9;
+constexpr int kConvWarps = 3;                             // union rows pw, pw + 3, pw + 6 of every stage
 constexpr int kFirstBuild = 12;
 constexpr int kBuildWarps = 4;
 constexpr int kMmaThreads = (kFirstBuild + kBuildWarps) * 32;   // 512
 constexpr int kBuildThreads = kBuildWarps * 32;
+constexpr int kDescReaders = kEpiWarps + 1 + kLoadWarps + kConvWarps + kBuildWarps;   // warps that read a descriptor
 constexpr int kWCols = 64;                                // union columns per round
-constexpr int kUnitN = 256;                               // channels per work unit
+constexpr int kUnitN = 128;                               // channels per work unit
 constexpr int kStageRows = 8;                             // union rows per stage = one tf32 K step
-constexpr int kStages = 2;
-constexpr int kRawStages = 4;
-constexpr int kRawRow = kUnitN * 4;                       // 1 KB: one feature row half
-constexpr int kRawBytes = kStageRows * kRawRow;           // 8 KB per raw stage
-constexpr int kWBytes = 128 * kWCols * 4;                 // 32 KB (hi or lo)
-constexpr int kStageHalf = kStageRows * kUnitN * 4;       // 8 KB (hi or lo)
+constexpr int kStages = 3;
+constexpr int kRawStages = 12;
+constexpr int kRawRow = kUnitN * 4;                       // 512 B: one feature row quarter
+constexpr int kRawBytes = kStageRows * kRawRow;           // 4 KB per raw stage
+constexpr int kWsRow = kWCols + 4;                        // scratch row stride in floats: 272 B, conflict-free 16-byte row reads
+constexpr int kWsBytes = 128 * kWsRow * 4;                // 34 KB scratch tile
+constexpr int kStageHalf = kStageRows * kUnitN * 4;       // 4 KB (hi or lo)
+constexpr int kTmemW = 256;                               // first W column in tensor memory
 constexpr int kStageBytes = 2 * kStageHalf;
 constexpr int kOutBufs = 3;                               // staging tiles per epilogue warp
 constexpr int kOutTile = 32 * 128;                        // 32 pixels x 32 channels fp32
 constexpr int kDescRing = 4;
-constexpr int kEntRegs = 8;                               // entries a builder thread holds in flight
+constexpr int kUidS = 128;                                // union ids per half tile the builders hand to the loader through shared memory
+constexpr int kEntRegs = 6;                               // entries a builder lane holds per scatter round (x 2 sets in flight)
 
 struct MmaDesc { int32_t ht, U, n0, n1, n2, n3, end, pad; };
 
 struct MmaSmem {
-    static constexpr int w = 0;                                           // [hi, lo]
-    static constexpr int stages = 2 * kWBytes;
+    static constexpr int w = 0;                                           // scratch tile [128 px][kWsRow]
+    static constexpr int stages = kWsBytes;
     static constexpr int raw = stages + kStages * kStageBytes;
     static constexpr int out = raw + kRawStages * kRawBytes;              // [4 warps][kOutBufs] staging tiles, 1 KB aligned
     static constexpr int desc = out + kEpiWarps * kOutBufs * kOutTile;
-    static constexpr int bars = desc + kDescRing * (int)sizeof(MmaDesc);
-    static constexpr int n_bars = 2 * kStages + 2 * kRawStages + 2 + 4 + kDescRing;
+    static constexpr int uid = desc + kDescRing * (int)sizeof(MmaDesc);    // int32[kDescRing][kUidS]: first ids of each union
+    static constexpr int bars = uid + kDescRing * kUidS * 4;
+    static constexpr int n_bars = 2 * kStages + 2 * kRawStages + 4 + 4 + 2 * kDescRing;
     static constexpr int tmem = bars + n_bars * 8;
     static constexpr int total = tmem + 16;
 };
@@ -92,6 +104,12 @@ __device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t a, uint64_t 
                  "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "l"(a), "l"(b), "r"(idesc), "r"((uint32_t)accumulate) : "memory");
 }
+__device__ __forceinline__ void umma_tf32_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b, uint32_t idesc, bool accumulate)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "r"(a_tmem), "l"(b), "r"(idesc), "r"((uint32_t)accumulate) : "memory");
+}
 __device__ __forceinline__ bool elect_one()     // one lane of a converged warp, always the same one
 {
     uint32_t pred;
@@ -111,13 +129,6 @@ __device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, const void*
                  ::"l"(reinterpret_cast<uint64_t>(map)), "r"(s32(src)), "r"(c0), "r"(x), "r"(y) : "memory");
 }
 
-// byte offset of W[m][c] in the K-major, non-swizzled canonical layout: core matrix = 8 pixels x 4 columns (128 B);
-// column chunks 128 B apart (LBO), 8-pixel groups 2 KB apart (SBO)
-__device__ __forceinline__ uint32_t w_off(int m, int c)
-{
-    return (uint32_t)((m >> 3) * (kWCols / 4 * 128) + (c >> 2) * 128 + (m & 7) * 16 + (c & 3) * 4);
-}
-
 // rounds / K steps of a half tile: every role derives them from the union size
 __device__ __forceinline__ int rounds_of(int U) { return U <= kWCols ? 1 : (U + kWCols - 1) / kWCols; }
 __device__ __forceinline__ int cols_of(int U, int r) { return max(0, min(kWCols, U - r * kWCols)); }
@@ -129,16 +140,18 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char* stage_base = smem + MmaSmem::stages;
     MmaDesc* desc = reinterpret_cast<MmaDesc*>(smem + MmaSmem::desc);
+    int32_t* uid_s = reinterpret_cast<int32_t*>(smem + MmaSmem::uid);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + MmaSmem::bars);
     uint64_t* full = bars;                       // [kStages] converters -> MMA (4 warp arrivals)
     uint64_t* empty = bars + kStages;            // [kStages] MMA -> converters (tcgen05.commit)
     uint64_t* raw_full = bars + 2 * kStages;     // [kRawStages] loader (TMA complete_tx) -> converters
     uint64_t* raw_empty = raw_full + kRawStages; // [kRawStages] converters -> loader (4 warp arrivals)
-    uint64_t* w_ready = raw_empty + kRawStages;  // builders -> MMA
-    uint64_t* w_free = w_ready + 1;              // MMA -> builders (tcgen05.commit)
-    uint64_t* tmem_full = w_free + 1;            // [2] MMA -> epilogue (tcgen05.commit)
+    uint64_t* w_ready = raw_empty + kRawStages;  // [2] builders -> MMA: W instance i lives in tensor-memory buffer i & 1
+    uint64_t* w_free = w_ready + 2;              // [2] MMA -> builders (tcgen05.commit)
+    uint64_t* tmem_full = w_free + 2;            // [2] MMA -> epilogue (tcgen05.commit)
     uint64_t* tmem_empty = tmem_full + 2;        // [2] epilogue -> MMA (4 warp arrivals)
-    uint64_t* d_ready = tmem_empty + 2;          // [kDescRing] builders -> everybody: descriptor h is published
+    uint64_t* d_ready = tmem_empty + 2;          // [kDescRing] scheduler -> everybody: descriptor h is published
+    uint64_t* d_free = d_ready + kDescRing;      // [kDescRing] every consumer warp, once it has copied descriptor h -> scheduler
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + MmaSmem::tmem);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -147,11 +160,14 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
     const int num_half = p.num_tiles * 2;
 
     if (tid == 0) {
+        stamp_time(p.sl.ctrl, 2, true);
         for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], kConvWarps); mbar_init(&empty[s], 1); }
         for (int s = 0; s < kRawStages; ++s) { mbar_init(&raw_full[s], 1); mbar_init(&raw_empty[s], kConvWarps); }
-        mbar_init(w_ready, 1); mbar_init(w_free, 1);
-        for (int b = 0; b < 2; ++b) { mbar_init(&tmem_full[b], 1); mbar_init(&tmem_empty[b], kEpiWarps); }
-        for (int s = 0; s < kDescRing; ++s) mbar_init(&d_ready[s], 1);
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(&w_ready[b], 1); mbar_init(&w_free[b], 1);
+            mbar_init(&tmem_full[b], 1); mbar_init(&tmem_empty[b], kEpiWarps);
+        }
+        for (int s = 0; s < kDescRing; ++s) { mbar_init(&d_ready[s], 1); mbar_init(&d_free[s], kDescReaders); }
         mbar_fence_init();
     }
     if (warp == 0) {
@@ -163,9 +179,21 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    // every role walks the same sequence of descriptors h = 0, 1, ...; the builders publish them
+#ifdef QR_PROF
+    long long prof[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    const long long prof_t0 = clock64();
+#define PW(cls, bar, par) do { const long long t_ = clock64(); mbar_wait_quiet(bar, par); prof[cls] += clock64() - t_; } while (0)
+#else
+#define PW(cls, bar, par) mbar_wait_quiet(bar, par)
+#endif
+    // every role walks the same sequence of descriptors h = 0, 1, ...; the scheduler warp publishes them, and a ring slot is
+    // reused only after every consumer warp has copied what it needs out of it (desc_done)
+    auto desc_done = [&](int h) {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&d_free[h % kDescRing]);
+    };
     auto wait_desc = [&](int h) -> const MmaDesc* {
-        mbar_wait(&d_ready[h % kDescRing], (uint32_t)((h / kDescRing) & 1));
+        PW(0, &d_ready[h % kDescRing], (uint32_t)((h / kDescRing) & 1));
         return &desc[h % kDescRing];
     };
 
@@ -191,9 +219,10 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
             const int ht = d->ht;
             const int tile = ht >> 1;
             const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8 + 2 * warp;
+            desc_done(h);
             for (int c = 0; c < nunits; ++c, ++unit) {
                 const int buf = unit & 1;
-                mbar_wait(&tmem_full[buf], (unit >> 1) & 1);
+                PW(1, &tmem_full[buf], (unit >> 1) & 1);
                 tc_fence_after();
                 const uint32_t t0 = tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(buf * kUnitN);
 #pragma unroll 1
@@ -231,52 +260,56 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
         // ================================================= MMA issuer ===============================================
         // The whole warp runs the loop in uniform control flow (descriptors stay in uniform registers); one elected
         // lane issues the tcgen05 instructions.
-        // M = 128, N = 256, fp32 accumulate, A and B tf32, A K-major, B MN-major
+        // M = 128, N = 128, fp32 accumulate, A (tensor memory, K-major) and B (shared memory, MN-major) tf32
         const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 16) | ((uint32_t)(kUnitN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-        const uint32_t a_hi = s32(smem + MmaSmem::w), a_lo = a_hi + kWBytes, st0 = s32(stage_base);
-        int unit = 0, wi = 0, st = 0;                      // wi: W instances consumed so far
+        const uint32_t st0 = s32(stage_base);
+        int unit = 0, wi = 0, st = 0;                      // wi: W instances consumed so far; instance i is in buffer i & 1
         for (int h = 0;; ++h) {
             const MmaDesc* d = wait_desc(h);
             if (d->end) break;
             const int U = d->U;
+            desc_done(h);
             const int rounds = rounds_of(U);
+            const bool reuse = rounds <= 2;                // both W instances stay resident for every unit of the half tile
+            const int wi0 = wi;
             for (int c = 0; c < nunits; ++c, ++unit) {
                 const int buf = unit & 1;
-                mbar_wait(&tmem_empty[buf], ((unit >> 1) & 1) ^ 1);
+                PW(1, &tmem_empty[buf], ((unit >> 1) & 1) ^ 1);
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)(buf * kUnitN);
                 for (int r = 0; r < rounds; ++r) {
-                    if (c == 0 || rounds > 1) { mbar_wait(w_ready, wi & 1); ++wi; }
+                    const int inst = reuse ? wi0 + r : wi++;
+                    if (!reuse || c == 0) { PW(2, &w_ready[inst & 1], (inst >> 1) & 1); tc_fence_after(); }
+                    const uint32_t a_hi = tmem_base + (uint32_t)(kTmemW + (inst & 1) * 2 * kWCols), a_lo = a_hi + kWCols;
                     const int nk = ksteps_of(cols_of(U, r));
                     for (int j = 0; j < nk; ++j, ++st) {
                         const int s = st % kStages;
-                        mbar_wait(&full[s], (st / kStages) & 1);
+                        PW(3, &full[s], (st / kStages) & 1);
                         tc_fence_after();
                         const uint32_t b_hi = st0 + s * kStageBytes, b_lo = b_hi + kStageHalf;
-                        const uint64_t da_hi = umma_desc(a_hi + j * 256, 128, kWCols / 4 * 128, 0);
-                        const uint64_t da_lo = umma_desc(a_lo + j * 256, 128, kWCols / 4 * 128, 0);
                         const uint64_t db_hi = umma_desc(b_hi, 1024, 512, 1);
                         const uint64_t db_lo = umma_desc(b_lo, 1024, 512, 1);
                         if (elect_one()) {
-                            umma_tf32(d_tmem, da_hi, db_hi, idesc, (r | j) != 0);
-                            umma_tf32(d_tmem, da_lo, db_hi, idesc, true);
-                            umma_tf32(d_tmem, da_hi, db_lo, idesc, true);
+                            umma_tf32_ts(d_tmem, a_hi + j * kStageRows, db_hi, idesc, (r | j) != 0);
+                            umma_tf32_ts(d_tmem, a_lo + j * kStageRows, db_hi, idesc, true);
+                            umma_tf32_ts(d_tmem, a_hi + j * kStageRows, db_lo, idesc, true);
                             umma_commit(&empty[s]);
                         }
                         __syncwarp();
                     }
-                    if (rounds > 1 || c == nunits - 1) {                 // last use of this W
-                        if (elect_one()) umma_commit(w_free);
+                    if (!reuse || c == nunits - 1) {                     // last use of this W instance
+                        if (elect_one()) umma_commit(&w_free[inst & 1]);
                         __syncwarp();
                     }
                 }
                 if (elect_one()) umma_commit(&tmem_full[buf]);
                 __syncwarp();
             }
+            if (reuse) wi = wi0 + rounds;
         }
-    } else if (warp == kLoadWarp) {
+    } else if (warp >= kLoadWarp && warp < kLoadWarp + kLoadWarps) {
         // ================================================= loader ===================================================
-        // lane k < 8 copies union row 8 j + k of every stage: 1 KB (256 channels) per bulk copy, kRawStages ahead.  The
+        // lane k < 8 copies union row 8 j + k of every stage: 512 B (128 channels) per bulk copy, kRawStages ahead.  The
         // union's ids come from the walk's lists in global memory (L2 loads: the walk may still be running elsewhere).
         unsigned char* raw_base = smem + MmaSmem::raw;
         int st = 0;
@@ -285,17 +318,32 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
             if (d->end) break;
             const int U = d->U;
             const int32_t* uid = p.sl.uid + (size_t)d->ht * p.sl.ucap;
+            const int32_t* uid_h = uid_s + (h % kDescRing) * kUidS;
+            int32_t my_ids[kUidS / 32];                    // the shared ids of this half tile, lane-strided, copied out
+#pragma unroll
+            for (int q = 0; q < kUidS / 32; ++q) my_ids[q] = q * 32 + lane < U ? uid_h[q * 32 + lane] : 0;
+            desc_done(h);
             const int rounds = rounds_of(U);
             for (int c = 0; c < nunits; ++c) {
                 for (int r = 0; r < rounds; ++r) {
                     const int ncols = cols_of(U, r);
                     const int nk = ksteps_of(ncols);
                     for (int j = 0; j < nk; ++j, ++st) {
+                        if (st % kLoadWarps != warp - kLoadWarp) continue;
                         const int s = st % kRawStages;
                         const int rows = max(0, min(kStageRows, ncols - j * kStageRows));
                         int32_t id = 0;
-                        if (lane < rows) id = __ldcg(uid + r * kWCols + j * kStageRows + lane);
-                        mbar_wait(&raw_empty[s], ((st / kRawStages) & 1) ^ 1);
+                        {   // union id of row `lane` of the stage: from the copied ids (a shuffle), else from the lists
+                            const int col = r * kWCols + j * kStageRows + (lane & 7);
+                            int32_t v = 0;
+#pragma unroll
+                            for (int q = 0; q < kUidS / 32; ++q) {
+                                const int32_t t = __shfl_sync(0xffffffffu, my_ids[q], col & 31);
+                                if ((col >> 5) == q) v = t;
+                            }
+                            if (lane < rows) id = col < kUidS ? v : __ldcg(uid + col);
+                        }
+                        PW(1, &raw_empty[s], ((st / kRawStages) & 1) ^ 1);
                         if (lane == 0) {
                             if (rows > 0) mbar_arrive_expect_tx(&raw_full[s], (uint32_t)rows * kRawRow);
                             else mbar_arrive(&raw_full[s]);
@@ -308,22 +356,74 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                 }
             }
         }
+    } else if (warp == kSchedWarp) {
+        // ================================================= scheduler ================================================
+        // runs up to kDescRing half tiles ahead of the pipeline: claims the next half tile inside the image (global ticket,
+        // index order = the order the walk produces them), waits for its release flag, and publishes {half tile, list
+        // lengths, union size} plus the first kUidS union ids in shared memory.  Every global round trip of the hand-over
+        // (ticket, flag, header, ids) happens here, off the critical path of the builders and loaders.
+        for (int h = 0;; ++h) {
+            const int slot = h % kDescRing;
+            PW(1, &d_free[slot], (uint32_t)(((h / kDescRing) & 1) ^ 1));
+            MmaDesc* d = &desc[slot];
+            int ht = 0;
+            if (lane == 0) {
+                while (true) {
+                    ht = atomicAdd(p.sl.ctrl + 1, 1);
+                    if (ht >= num_half) break;
+                    const int y0 = ((ht >> 1) / p.cam.tiles_x) * kTile + (ht & 1) * 8;
+                    if (y0 < p.cam.height) break;
+                }
+                if (ht < num_half) {
+                    const int32_t* flag = p.sl.flags + ht;
+#ifdef QR_PROF
+                    const long long tf_ = clock64();
+#endif
+                    while (ld_acquire(flag) == 0) __nanosleep(500);
+#ifdef QR_PROF
+                    prof[2] += clock64() - tf_;
+#endif
+                }
+            }
+            ht = __shfl_sync(0xffffffffu, ht, 0);            // (also orders the other lanes' loads after the acquire)
+            const bool end = ht >= num_half;
+            int U = 0;
+            if (!end) {
+                const int32_t* hd = p.sl.hdr + (size_t)ht * kHdrWords;
+                const int32_t v = lane < 5 ? __ldcg(hd + lane) : 0;
+                U = __shfl_sync(0xffffffffu, v, 4);
+                if (lane < 4) (&d->n0)[lane] = v;
+                const int32_t* uid = p.sl.uid + (size_t)ht * p.sl.ucap;
+#pragma unroll
+                for (int q = 0; q < kUidS / 32; ++q)
+                    if (q * 32 + lane < U) uid_s[slot * kUidS + q * 32 + lane] = __ldcg(uid + q * 32 + lane);
+            }
+            if (lane == 0) { d->ht = ht; d->U = U; d->end = end ? 1 : 0; }
+            __threadfence_block();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&d_ready[slot]);
+            if (end) break;
+        }
     } else if (warp >= kFirstConv && warp < kFirstBuild) {
         // ================================================= converters ===============================================
-        // warp pw splits union rows pw and pw + 4 of every stage: ld.shared of the raw row -> hi / lo -> st.shared in the
-        // MN-major SWIZZLE_128B_BASE32B layout.
-        const int pw = warp - kFirstConv;                 // 0..3
+        // warp pw splits union rows pw, pw + 3 (and pw + 6) of every stage: ld.shared of the raw row -> hi / lo -> st.shared
+        // in the MN-major SWIZZLE_128B_BASE32B layout.
+        const int pw = warp - kFirstConv;                 // 0..2
         const unsigned char* raw_base = smem + MmaSmem::raw;
-        // byte offset of this lane's 16 bytes inside a stage half, row q of the stage: channels 4 lane .. 4 lane + 3 (+128)
+        // byte offset of this lane's 16 bytes (channels 4 lane .. 4 lane + 3) inside a stage half, row q of the stage
         auto lane_off = [&](int q) -> uint32_t {
             return (uint32_t)((lane >> 3) * 1024 + (q >> 2) * 512 + (q & 3) * 128 + ((((lane & 7) >> 1) ^ (q & 3)) * 32) + (lane & 1) * 16);
         };
-        const uint32_t off0 = lane_off(pw), off1 = lane_off(pw + 4);
+        constexpr int kRowsPerConv = (kStageRows + kConvWarps - 1) / kConvWarps;   // 3
+        uint32_t off[kRowsPerConv];
+#pragma unroll
+        for (int q = 0; q < kRowsPerConv; ++q) off[q] = lane_off(min(pw + kConvWarps * q, kStageRows - 1));
         int st = 0;
         for (int h = 0;; ++h) {
             const MmaDesc* d = wait_desc(h);
             if (d->end) break;
             const int U = d->U;
+            desc_done(h);
             const int rounds = rounds_of(U);
             for (int c = 0; c < nunits; ++c) {
                 for (int r = 0; r < rounds; ++r) {
@@ -331,31 +431,27 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                     const int nk = ksteps_of(ncols);
                     for (int j = 0; j < nk; ++j, ++st) {
                         const int sr = st % kRawStages;
-                        mbar_wait(&raw_full[sr], (st / kRawStages) & 1);
-                        float4 a[2][2];
+                        PW(1, &raw_full[sr], (st / kRawStages) & 1);
+                        float4 a[kRowsPerConv];
 #pragma unroll
-                        for (int q = 0; q < 2; ++q) {
-                            a[q][0] = a[q][1] = make_float4(0.f, 0.f, 0.f, 0.f);
-                            if (j * kStageRows + pw + 4 * q < ncols) {
-                                const unsigned char* rr = raw_base + sr * kRawBytes + (pw + 4 * q) * kRawRow + lane * 16;
-                                a[q][0] = *reinterpret_cast<const float4*>(rr);
-                                a[q][1] = *reinterpret_cast<const float4*>(rr + 512);
-                            }
+                        for (int q = 0; q < kRowsPerConv; ++q) {
+                            const int row = pw + kConvWarps * q;
+                            a[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+                            if (row < kStageRows && j * kStageRows + row < ncols)
+                                a[q] = *reinterpret_cast<const float4*>(raw_base + sr * kRawBytes + row * kRawRow + lane * 16);
                         }
                         __syncwarp();
                         if (lane == 0) mbar_arrive(&raw_empty[sr]);          // the raw rows are in registers
                         const int s = st % kStages;
-                        mbar_wait(&empty[s], ((st / kStages) & 1) ^ 1);
+                        PW(2, &empty[s], ((st / kStages) & 1) ^ 1);
 #pragma unroll
-                        for (int q = 0; q < 2; ++q) {
-                            unsigned char* hi = stage_base + s * kStageBytes + (q ? off1 : off0);
-                            unsigned char* lo = hi + kStageHalf;
-#pragma unroll
-                            for (int t = 0; t < 2; ++t) {
-                                const float4 v = a[q][t];
+                        for (int q = 0; q < kRowsPerConv; ++q) {
+                            if (pw + kConvWarps * q < kStageRows) {
+                                unsigned char* hi = stage_base + s * kStageBytes + off[q];
+                                const float4 v = a[q];
                                 const float4 hv = make_float4(tf32_hi(v.x), tf32_hi(v.y), tf32_hi(v.z), tf32_hi(v.w));
-                                *reinterpret_cast<float4*>(hi + t * 4 * 1024) = hv;
-                                *reinterpret_cast<float4*>(lo + t * 4 * 1024) =
+                                *reinterpret_cast<float4*>(hi) = hv;
+                                *reinterpret_cast<float4*>(hi + kStageHalf) =
                                     make_float4(__fsub_rn(v.x, hv.x), __fsub_rn(v.y, hv.y), __fsub_rn(v.z, hv.z), __fsub_rn(v.w, hv.w));
                             }
                         }
@@ -368,96 +464,117 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
         }
     } else if (warp >= kFirstBuild) {
         // ================================================= builders =================================================
-        const int ptid = tid - kFirstBuild * 32;          // 0..127
+        const int ptid = tid - kFirstBuild * 32;          // 0..127 = pixel of the half tile = TMEM lane (warp % 4 = lane quarter)
         auto prod_sync = [&]() { named_sync<1, kBuildThreads>(); };
-        unsigned char* wbuf = smem + MmaSmem::w;
-        int wi = 0;                                       // W instances built so far
-        for (int h = 0;; ++h) {
-            MmaDesc* d = &desc[h % kDescRing];
-            if (ptid == 0) {
-                // next half tile inside the image, in index order; its lists must be complete (the walk releases the flag)
-                int ht;
-                while (true) {
-                    ht = atomicAdd(p.sl.ctrl + 1, 1);
-                    if (ht >= num_half) break;
-                    const int y0 = ((ht >> 1) / p.cam.tiles_x) * kTile + (ht & 1) * 8;
-                    if (y0 < p.cam.height) break;
-                }
-                d->end = ht >= num_half ? 1 : 0;
-                d->ht = ht;
-                if (ht < num_half) {
-                    const int32_t* flag = p.sl.flags + ht;
-                    while (ld_acquire(flag) == 0) __nanosleep(200);
-                    const int4 nq = __ldcg(reinterpret_cast<const int4*>(p.sl.hdr + (size_t)ht * kHdrWords));
-                    d->n0 = nq.x; d->n1 = nq.y; d->n2 = nq.z; d->n3 = nq.w;
-                    d->U = __ldcg(p.sl.hdr + (size_t)ht * kHdrWords + 4);
-                }
-                __threadfence_block();
-                mbar_arrive(&d_ready[h % kDescRing]);
+        float* ws = reinterpret_cast<float*>(smem + MmaSmem::w);
+        auto st16 = [&](uint32_t taddr, const uint32_t (&r)[16]) {
+            asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+                         ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+                           "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
+        };
+        const uint32_t lane_base = ((uint32_t)((warp & 3) * 32)) << 16;
+        int wi = 0;                                       // W instances built so far; instance i goes to buffer i & 1
+        // builder warp q scatters list q (the walk's warp q wrote it): lane i takes entries i, i + 32, ...  Loads are
+        // software pipelined: while one set of kEntRegs entries is scattered the next is in flight, and the first set of
+        // what is built next is requested before the tensor-memory phase of the current instance.
+        const int bq = warp - kFirstBuild;
+        struct HT { int ht, U, n, end; };
+        auto read_desc = [&](int h) -> HT {
+            const MmaDesc* d = wait_desc(h);
+            HT t;
+            t.end = d->end; t.ht = d->ht; t.U = d->U;
+            t.n = (&d->n0)[bq];
+            if (!t.end) desc_done(h);
+            return t;
+        };
+        auto load_set = [&](const HT& t, int base, uint2 (&e)[kEntRegs]) {
+            const uint2* ent = p.sl.ent + ((size_t)t.ht * kSelLists + bq) * p.sl.qcap + base + lane;
+#pragma unroll
+            for (int u = 0; u < kEntRegs; ++u)
+                e[u] = base + u * 32 + lane < t.n ? __ldcg(ent + u * 32) : make_uint2(0u, 0xFFFFFFFFu);
+        };
+        auto scatter_set = [&](const uint2 (&e)[kEntRegs], int r) {
+#pragma unroll
+            for (int u = 0; u < kEntRegs; ++u) {
+                const int cl = sel_col(e[u].y) - r * kWCols;           // padding entries have column 2^17 - 1
+                if (cl >= 0 && cl < kWCols) ws[sel_pixel(e[u].y) * kWsRow + cl] = __uint_as_float(e[u].x);
             }
-            prod_sync();
-            if (d->end) break;
-            const int ht = d->ht, U = d->U;
-            const int e1 = d->n0, e2 = e1 + d->n1, e3 = e2 + d->n2, total = e3 + d->n3;
-            const uint2* ent = p.sl.ent + (size_t)ht * kSelLists * p.sl.qcap;
-            auto ent_at = [&](int f) -> uint2 {            // flat index over the four lists
-                const int q = (f >= e1) + (f >= e2) + (f >= e3);
-                const int b = q == 0 ? 0 : (q == 1 ? e1 : (q == 2 ? e2 : e3));
-                return __ldcg(ent + (size_t)q * p.sl.qcap + (f - b));
-            };
-            const int rounds = rounds_of(U);
-            for (int c = 0; c < nunits; ++c) {
-                for (int r = 0; r < rounds; ++r) {
-                    if (c == 0 || rounds > 1) {
-                        // ---------------- build W for columns [64 r, 64 r + 64) ----------------
-                        uint2 e[kEntRegs];
-#pragma unroll
-                        for (int u = 0; u < kEntRegs; ++u) {
-                            const int f = u * kBuildThreads + ptid;
-                            e[u] = f < total ? ent_at(f) : make_uint2(0u, 0xFFFFFFFFu);
-                        }
-                        mbar_wait(w_free, (wi & 1) ^ 1);            // the MMAs that read the previous instance have retired
-                        ++wi;
-                        {
-                            const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-                            float4* wz = reinterpret_cast<float4*>(wbuf);
-                            for (int i = ptid; i < 2 * kWBytes / 16; i += kBuildThreads) wz[i] = z;
-                        }
-                        prod_sync();
-                        for (int base = 0; base == 0 || base < total; base += kEntRegs * kBuildThreads) {
-                            if (base > 0) {
-#pragma unroll
-                                for (int u = 0; u < kEntRegs; ++u) {
-                                    const int f = base + u * kBuildThreads + ptid;
-                                    e[u] = f < total ? ent_at(f) : make_uint2(0u, 0xFFFFFFFFu);
-                                }
-                            }
-#pragma unroll
-                            for (int u = 0; u < kEntRegs; ++u) {
-                                const int cl = sel_col(e[u].y) - r * kWCols;       // padding entries have column 2^17 - 1
-                                if (cl >= 0 && cl < kWCols) {
-                                    const uint32_t off = w_off(sel_pixel(e[u].y), cl);
-                                    const float w = __uint_as_float(e[u].x), hi = tf32_hi(w);
-                                    *reinterpret_cast<float*>(wbuf + off) = hi;
-                                    *reinterpret_cast<float*>(wbuf + kWBytes + off) = __fsub_rn(w, hi);
-                                }
-                            }
-                        }
-                        fence_async_smem();
-                        prod_sync();
-                        if (ptid == 0) mbar_arrive(w_ready);
+        };
+        constexpr int kSet = kEntRegs * 32;
+        HT cur = read_desc(0);
+        uint2 ea[kEntRegs], eb[kEntRegs];
+        if (!cur.end) load_set(cur, 0, ea);
+        for (int h = 0; !cur.end; ++h) {
+            const int rounds = rounds_of(cur.U);
+            const int ninst = rounds <= 2 ? rounds : rounds * nunits;      // (the MMA warp derives the same sequence)
+            HT nxt = cur;
+            for (int ii = 0; ii < ninst; ++ii, ++wi) {
+                const int r = ii % rounds;
+                // ---------------- build W for columns [64 r, 64 r + 64) ----------------
+                {
+                    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+                    float4* wz = reinterpret_cast<float4*>(ws);
+                    for (int i = ptid; i < kWsBytes / 16; i += kBuildThreads) wz[i] = z;
+                }
+                prod_sync();
+                for (int base = 0; base < cur.n || base == 0; base += 2 * kSet) {          // ea holds [base, base + kSet)
+                    if (base + kSet < cur.n) load_set(cur, base + kSet, eb);
+                    scatter_set(ea, r);
+                    if (base + kSet < cur.n) {
+                        if (base + 2 * kSet < cur.n) load_set(cur, base + 2 * kSet, ea);
+                        scatter_set(eb, r);
                     }
                 }
+                prod_sync();
+                // the scratch tile is complete.  Request the first entries of what is built next: this half tile again
+                // (another round / instance) or the next half tile
+                if (ii + 1 < ninst) load_set(cur, 0, ea);
+                else { nxt = read_desc(h + 1); if (!nxt.end) load_set(nxt, 0, ea); }
+                // thread = pixel: its row of 64 weights -> tensor memory, hi (the raw value: kind::tf32 reads its top 19
+                // bits) and lo = w - trunc(w); the buffer is free once the MMAs of the instance two before have retired
+                PW(1, &w_free[wi & 1], ((wi >> 1) & 1) ^ 1);
+                tc_fence_after();
+                const uint32_t t_hi = tmem_base + lane_base + (uint32_t)(kTmemW + (wi & 1) * 2 * kWCols);
+                const float4* row = reinterpret_cast<const float4*>(ws + ptid * kWsRow);
+#pragma unroll
+                for (int q = 0; q < kWCols / 16; ++q) {
+                    uint32_t hi[16], lo[16];
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) {
+                        const float4 v = row[q * 4 + t];
+                        const float f[4] = { v.x, v.y, v.z, v.w };
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            hi[4 * t + i] = __float_as_uint(f[i]);
+                            lo[4 * t + i] = __float_as_uint(__fsub_rn(f[i], tf32_hi(f[i])));
+                        }
+                    }
+                    st16(t_hi + q * 16, hi);
+                    st16(t_hi + kWCols + q * 16, lo);
+                }
+                asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                tc_fence_before();
+                prod_sync();                                 // every row is in tensor memory; the scratch tile is free again
+                if (ptid == 0) mbar_arrive(&w_ready[wi & 1]);
             }
+            cur = nxt;
         }
     }
 
+#ifdef QR_PROF
+    if (lane == 0) {    // role = warp group; ctrl[16 + 8 role + class] in units of 1024 cycles, class 7 = total
+        const int role = warp < 4 ? 0 : (warp == 4 ? 1 : (warp < 8 ? 2 : (warp == 8 ? 5 : (warp < 12 ? 3 : 4))));
+        prof[7] = clock64() - prof_t0;
+        for (int c = 0; c < 8; ++c) atomicAdd(p.sl.ctrl + 16 + 8 * role + c, (int)(prof[c] >> 10));
+    }
+#endif
     tc_fence_before();
     __syncthreads();
+    if (tid == 0) stamp_time(p.sl.ctrl, 3, false);
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
 }
 
-bool blend_mma_supported(int32_t D, qr_dtype feat_dtype) { return feat_dtype == QR_F32 && D >= kUnitN && D % kUnitN == 0; }
+bool blend_mma_supported(int32_t D, qr_dtype feat_dtype) { return feat_dtype == QR_F32 && D >= kUnitN && D % kUnitN == 0; }   // 128, 256, 384, 512
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -494,7 +611,16 @@ int launch_blend_mma(const BlendParams& p, cudaStream_t st)
         sms = 148;
     const unsigned grid = (unsigned)min(sms, p.num_tiles * 2);
     QR_CUDA_OK(cudaFuncSetAttribute(blend_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MmaSmem::total));
-    blend_mma_kernel<<<grid, kMmaThreads, MmaSmem::total, st>>>(p, tmap);
+    // programmatic dependent launch: the kernel does not wait for walk2_kernel to finish (it never calls
+    // griddepcontrol.wait); it starts once every walk CTA has started and synchronises per half tile through the
+    // release flags.  If the two kernels are serialised (a profiler, a full GPU) the flags are simply all set.
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kMmaThreads); cfg.dynamicSmemBytes = MmaSmem::total; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    QR_CUDA_OK(cudaLaunchKernelEx(&cfg, blend_mma_kernel, p, tmap));
     QR_LAUNCH_OK("blend_mma_kernel");
     return QR_OK;
 }

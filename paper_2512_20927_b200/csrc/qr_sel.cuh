@@ -43,6 +43,15 @@ struct SelLists {
     int32_t* flags = nullptr;   // [half tiles] directly behind ctrl: 1 = the half tile's lists are complete (released)
 };
 constexpr int kCtrlWords = 64;
+// ctrl[8..15] as four uint64: kernel time stamps of the last frame (%globaltimer, ns), read by bench.py's untimed
+// statistics only: [0] ~first walk CTA start (stored as ~t so that atomicMax finds the minimum), [1] last walk CTA end,
+// [2] ~first blend CTA start, [3] last blend CTA end
+__device__ __forceinline__ void stamp_time(int32_t* ctrl, int slot, bool is_start)
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    atomicMax(reinterpret_cast<unsigned long long*>(ctrl + 8) + slot, is_start ? ~t : t);
+}
 
 struct SelLayout {
     size_t stamp, ctrl, hdr, uid, ent, total;

@@ -73,6 +73,10 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
     for (int k = tid; k <= K; k += kW2Threads)                            // thresholds as printed (R3)
         thr[k] = __fsub_rn(1.0f, __fdiv_rn((float)(k + 1), (float)(K + 1)));
     const float t_break = __fdiv_rn(1.0f, (float)(K + 1));
+    // the blend kernel (launched with programmatic stream serialization) may start as soon as every walk CTA is resident:
+    // it consumes half tiles as their flags are released and shares the SMs with this kernel
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (tid == 0) stamp_time(p.sl.ctrl, 0, true);
     if (blockIdx.x == 0 && tid == 0) {
         p.sl.stamp[0] = kSelMagic; p.sl.stamp[1] = p.cam.width; p.sl.stamp[2] = p.cam.height; p.sl.stamp[3] = K;
         const unsigned long long a = (unsigned long long)p.sel_idx;
@@ -86,7 +90,7 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
     if (tid == 0) { s_ht = atomicAdd(p.sl.ctrl, 1); s_ucount = 0; s_finished = 0; s_evals = 0; s_consumed = 0; }
     __syncthreads();
     const int ht = s_ht;
-    if (ht >= num_half) break;
+    if (ht >= num_half) { if (tid == 0) stamp_time(p.sl.ctrl, 1, false); break; }
     const int tile = ht >> 1;
     const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
     int32_t* hdr = p.sl.hdr + (size_t)ht * kHdrWords;
@@ -295,8 +299,11 @@ int launch_walk2(const WalkParams2& p, cudaStream_t st)
         if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
             sms = 148;
         const char* e = getenv("QR_WALK_CTAS");   // EXPERIMENT
-        per_sm = e ? atoi(e) : 10;
+        per_sm = e ? atoi(e) : 5;
     }
+    // the blend kernel joins these CTAs on the same SMs and needs ~157 KB of shared memory there: an SM only changes its
+    // L1 / shared split when it is idle, so this kernel asks for the largest shared-memory carve-out although it uses 8 KB
+    QR_CUDA_OK(cudaFuncSetAttribute(walk2_kernel<16>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     const unsigned grid = (unsigned)min(num_half, sms * per_sm);
     walk2_kernel<16><<<grid, kW2Threads, 0, st>>>(p);
     QR_LAUNCH_OK("walk2_kernel");

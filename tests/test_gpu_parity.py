@@ -214,7 +214,7 @@ def test_forward_invariants_full_scale(qr):
     # payload width independence
     out_3 = qr.pipeline.forward(sc.cam, fe, g.features[:, :3].contiguous(), K)
     assert (P.masked_records(out_3)[0] == idx).all()
-    np.testing.assert_allclose(out_3.out_map.cpu().numpy(), out.out_map[..., :3].cpu().numpy(), rtol=1e-6, atol=1e-7)
+    np.testing.assert_allclose(out_3.out_map.cpu().numpy(), out.out_map[..., :3].cpu().numpy(), rtol=2e-5, atol=1e-6)   # FFMA vs tcgen05 path
 
 
 # ------------------------------------------------------------------------------------------------
