@@ -211,12 +211,12 @@ def run_cuda(args):
         fwd_out = pl.forward(cam, fe, d["features"], K, fwd_out)
         if timers is not None:
             e1.record()
-        pl.backward(cam, N, fwd_out, d["dL_dmap"], dF, bws)
+        pl.backward(cam, N, fwd_out, d["dL_dmap"], dF, None if fwd_out.has_lists else bws)
         if timers is not None:
             e2.record()
         # dL_dfeat would be consumed here (the 3D network's backward); then the rows this step touched are re-zeroed,
         # so that the table is all-zero again for the next step without a 1.02 GB memset
-        pl.backward_clear(cam, N, fwd_out, dF, bws)
+        pl.backward_clear(cam, N, fwd_out, dF, None if fwd_out.has_lists else bws)
         if timers is not None:
             e3.record()
             timers.append((e0, e1, e2, e3))
@@ -321,10 +321,10 @@ def run_cuda(args):
                 dd[k].copy_(host[k], non_blocking=True)
             fe2 = pl.frontend(cam, dd["means"], dd["scales"], dd["quats"], dd["opac"], state["capacity"])
             o = pl.forward(cam, fe2, dd["features"], K, fwd_out)
-            pl.backward(cam, N, o, dd["dL_dmap"], dF, bws)
+            pl.backward(cam, N, o, dd["dL_dmap"], dF, None if o.has_lists else bws)
             out_host.copy_(o.out_map, non_blocking=True)
             dF_host.copy_(dF, non_blocking=True)
-            pl.backward_clear(cam, N, o, dF, bws)
+            pl.backward_clear(cam, N, o, dF, None if o.has_lists else bws)
 
         e2e_step()
         barrier()

@@ -33,7 +33,7 @@
 extern "C" {
 #endif
 
-#define QR_VERSION 100       /* major*10000 + minor*100 + patch */
+#define QR_VERSION 200       /* major*10000 + minor*100 + patch */
 #define QR_TILE 16           /* tile edge in pixels (3D-GS convention) */
 #define QR_MAX_K 256         /* largest K qr_forward / qr_backward accept */
 #define QR_MAX_D 512         /* largest feature width ("up to 512-D") */
@@ -117,11 +117,15 @@ int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M,
  *   in : mean2d, conic_opac (qr_preprocess); isect_gauss, tile_range (qr_bin_sort);
  *        features[N,D] row-major, fp32 or fp16 (feat_dtype); fp16 is widened exactly, accumulation is fp32.
  *   out: out_map[H,W,D] fp32 (HWC; 0 where nothing is selected, R8)
- *        sel_idx[H,W,K] int32 selected Gaussian ids in depth order, -1 padded
- *        sel_w[H,W,K]   fp32 normalised weights w^Q / (1 - T^Q), 0 padded
- *        n_sel[H,W]     int32 number selected (<= K)
- *        resid_TQ[H,W]  fp32 T^Q after the walk (1 where nothing is selected)
+ *        sel_idx[H,W,K] int32 selected Gaussian ids in depth order; only slots s < n_sel[p] are part of the result:
+ *        sel_w[H,W,K]   fp32 normalised weights w^Q / (1 - T^Q)       the others are left as the caller passed them
+ *        n_sel[H,W]     int32 number selected (<= K)                  (writing -1 / 0 there would be two thirds of the
+ *        resid_TQ[H,W]  fp32 T^Q after the walk (1 where nothing is selected)     records' traffic, for no reader)
  * K in [1, QR_MAX_K]; D in [1, QR_MAX_D]; D % 4 == 0 unless D <= 128; fp16 needs D % 8 == 0.
+ * ws must hold qr_forward_workspace_bytes(cam, K, D) bytes; every pointer must be non-NULL.  For fp32 features with
+ * D % 128 == 0 (the tcgen05 path) the call leaves in ws, per 16x8-pixel half tile, the numbered union of selected
+ * Gaussians and the selection as (weight, column, pixel) entries; qr_backward_lists and qr_backward_clear accept that
+ * workspace as it is, until the next call that writes it.
  */
 size_t qr_forward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D);
 int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype,
@@ -147,12 +151,24 @@ int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N,
                 float* dL_dfeat, void* ws, size_t ws_bytes, void* stream);
 
 /*
+ * qr_backward_lists -- the same gradient as qr_backward, computed from the per-half-tile selection lists that the last
+ * qr_forward(cam, K, D, QR_F32, ...) left in ITS workspace fwd_ws (see qr_forward), instead of re-deriving the unions
+ * from sel_idx / sel_w: one kernel instead of two.  fp32, D % 128 == 0, D <= 512 only (QR_ERR_UNSUPPORTED otherwise).
+ * The lists carry a stamp (image size, K) that the kernel checks on the device: a workspace that does not hold the
+ * lists of this camera and K makes the call a no-op (dL_dfeat untouched).  fwd_ws is only read.
+ */
+int qr_backward_lists(const qr_camera* cam, int32_t K, int32_t D, int64_t N, void* fwd_ws, size_t fwd_ws_bytes,
+                      const float* dL_dmap, float* dL_dfeat, void* stream);
+
+/*
  * qr_backward_clear -- zero exactly the rows of dL_dfeat that qr_backward over the same selection adds into (the
  * distinct Gaussians selected anywhere in the frame), and nothing else.  A loop that keeps dL_dfeat zero outside
  * those rows (zero it once, then clear after each use) writes ~|S| D floats per step instead of N D
  * (the whole-table zero fill costs more than qr_backward's own traffic).
  *   in : sel_idx, n_sel (from qr_forward); ws / ws_bytes = the workspace AS LEFT BY the last qr_backward call with
- *        the same cam, K, D and selection (its per-half-tile unions are reused, a scratch region of it is written).
+ *        the same cam, K, D and selection, or -- after qr_backward_lists -- the forward's workspace (its per-half-tile
+ *        unions are reused, a scratch region of it is written).  A workspace whose stamp does not match cam and K is
+ *        not trusted: the rows are then found from sel_idx / n_sel.  Ids outside [0, N) are ignored.
  *   out: dL_dfeat rows of selected Gaussians = 0; other rows untouched.
  */
 int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int64_t N,

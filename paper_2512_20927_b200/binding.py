@@ -27,7 +27,7 @@ STATUS = {0: "QR_OK", -1: "QR_ERR_INVALID_ARG", -2: "QR_ERR_NULL_POINTER", -3: "
 # every symbol include/qr.h declares (tests check that the library exports exactly these)
 SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_bin_workspace_bytes", "qr_bin_count",
            "qr_bin_sort", "qr_forward_workspace_bytes", "qr_forward", "qr_backward_workspace_bytes", "qr_backward",
-           "qr_backward_clear", "qr_dense_forward"]
+           "qr_backward_lists", "qr_backward_clear", "qr_dense_forward"]
 
 
 class QRError(RuntimeError):
@@ -81,6 +81,8 @@ def load() -> C.CDLL:
     lib.qr_backward_workspace_bytes.restype = sz; lib.qr_backward_workspace_bytes.argtypes = [cam, i32, i32]
     lib.qr_backward.restype = C.c_int
     lib.qr_backward.argtypes = [cam, i32, i32, i64, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.qr_backward_lists.restype = C.c_int
+    lib.qr_backward_lists.argtypes = [cam, i32, i32, i64, vp, sz, vp, vp, vp]
     lib.qr_backward_clear.restype = C.c_int
     lib.qr_backward_clear.argtypes = [cam, i32, i32, i64, vp, vp, vp, vp, sz, vp]
     lib.qr_dense_forward.restype = C.c_int
@@ -206,6 +208,9 @@ class ForwardOut:
     sel_w: torch.Tensor     # [H,W,K] f32
     n_sel: torch.Tensor     # [H,W] i32
     resid_TQ: torch.Tensor  # [H,W] f32
+    ws: Optional[torch.Tensor] = None   # the workspace the call used: for fp32 D % 128 == 0 it holds the selection lists
+                                        # qr_backward_lists / qr_backward_clear read, until the next call that writes it
+    has_lists: bool = False
 
 
 def _feat_dtype(features: torch.Tensor) -> int:
@@ -243,6 +248,12 @@ def qr_forward(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, feature
     dt = _feat_dtype(features)
     if ws is None:
         ws = _workspace(qr_forward_workspace_bytes(c, K, D), dev)
+    if out is not None:
+        kk = max(int(K), 1)
+        want = {"out_map": (H, W, D), "sel_idx": (H, W, kk), "sel_w": (H, W, kk), "n_sel": (H, W), "resid_TQ": (H, W)}
+        for name, shape in want.items():
+            if tuple(getattr(out, name).shape) != shape:
+                raise QRError(-1, f"out.{name} has shape {tuple(getattr(out, name).shape)}, expected {shape}")
     if out is None:
         kk = max(int(K), 1)
         out = ForwardOut(torch.empty((H, W, D), dtype=torch.float32, device=dev),
@@ -256,7 +267,14 @@ def qr_forward(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, feature
                              _dev(features, features.dtype, "features"), out.out_map.data_ptr(), out.sel_idx.data_ptr(),
                              out.sel_w.data_ptr(), out.n_sel.data_ptr(), out.resid_TQ.data_ptr(),
                              ws.data_ptr(), ws.numel(), _stream()))
+    out.ws = ws
+    out.has_lists = lists_supported(features.dtype, D)
     return out
+
+
+def lists_supported(features_dtype, D: int) -> bool:
+    """qr_forward leaves selection lists in its workspace for fp32 features with D % 128 == 0 (include/qr.h)."""
+    return features_dtype == torch.float32 and D % 128 == 0 and 128 <= D <= QR_MAX_D
 
 
 def qr_backward_workspace_bytes(cam, K: int, D: int) -> int:
@@ -283,6 +301,18 @@ def qr_backward(cam, N: int, sel_idx, sel_w, n_sel, dL_dmap, dL_dfeat: Optional[
                               _dev(sel_w, torch.float32, "sel_w"), _dev(n_sel, torch.int32, "n_sel"),
                               _dev(dL_dmap, torch.float32, "dL_dmap"), _dev(dL_dfeat, torch.float32, "dL_dfeat"),
                               _dev(ws, torch.uint8, "ws"), ws.numel(), _stream()))
+    return dL_dfeat
+
+
+def qr_backward_lists(cam, K: int, N: int, fwd_ws: torch.Tensor, dL_dmap, dL_dfeat: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """qr_backward from the selection lists the last qr_forward left in its workspace fwd_ws (ForwardOut.ws)."""
+    c = make_camera(cam)
+    D = int(dL_dmap.shape[-1])
+    if dL_dfeat is None:
+        dL_dfeat = torch.zeros((int(N), D), dtype=torch.float32, device=dL_dmap.device)
+    _check(load().qr_backward_lists(C.byref(c), int(K), D, int(N), _dev(fwd_ws, torch.uint8, "fwd_ws"), fwd_ws.numel(),
+                                    _dev(dL_dmap, torch.float32, "dL_dmap"), _dev(dL_dfeat, torch.float32, "dL_dfeat"),
+                                    _stream()))
     return dL_dfeat
 
 

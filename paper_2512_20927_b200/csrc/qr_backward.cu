@@ -282,26 +282,33 @@ __device__ __forceinline__ uint32_t clear_hash(uint32_t x)
 // seen[]: a direct-mapped cache of ids whose row some warp has already taken: a Gaussian is in the unions of ~10 half
 // tiles, and without it every row was zeroed ~10 times (225 MB of stores for 24 MB of rows).  A collision only costs
 // a repeated zeroing, never a missed one (the warp that finds another id in the cell zeroes its row).
-__global__ void __launch_bounds__(kClearThreads) backward_clear_kernel(const BackwardParams p, const int uid_stride,
+__global__ void __launch_bounds__(kClearThreads) backward_clear_kernel(const BackwardParams p, const bool have_lists,
                                                                        int32_t* __restrict__ seen, const int seen_mask)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
+    // a workspace that does not hold the lists of this camera and K (fresh memory, another frame size) is not trusted:
+    // fall back to the selection records, which are this call's own arguments
+    const bool lists = have_lists && sel_stamp_ok(p.sl.stamp, p.cam, p.K);
     for (int ht = blockIdx.x; ht < num_half; ht += gridDim.x) {
         const int tile = ht >> 1;
         const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
         if (y0 >= p.cam.height) continue;
-        int4 c = make_int4(0, 1, 0, 1);
-        if (p.prep_cnt) c = __ldg(reinterpret_cast<const int4*>(p.prep_cnt) + ht);
-        if (c.y == 0) continue;                                   // nothing selected in this half tile
-        if (c.w == 0) {                                           // numbered union: one pass over its rows
-            const int32_t* uid = p.prep_uid + (size_t)ht * uid_stride;
-            for (int r0 = 0; r0 < c.z; r0 += kClearThreads) {       // thread = union row: claim it, then the warp zeroes the claimed rows
+        int U = 0, flagged = 1;
+        if (lists) {
+            const int32_t* hd = p.sl.hdr + (size_t)ht * kHdrWords;
+            U = hd[4]; flagged = hd[5];
+            if (flagged == 0 && U == 0) continue;                 // nothing selected in this half tile
+        }
+        if (flagged == 0) {                                       // numbered union: one pass over its rows
+            const int32_t* uid = p.sl.uid + (size_t)ht * p.sl.ucap;
+            for (int r0 = 0; r0 < U; r0 += kClearThreads) {         // thread = union row: claim it, then the warp zeroes the claimed rows
                 const int r = r0 + (int)threadIdx.x;
                 int32_t id = -1;
-                if (r < c.z) {
-                    id = __ldg(uid + r);
-                    if (seen && atomicExch(&seen[clear_hash((uint32_t)id) & seen_mask], id) == id) id = -1;   // already taken
+                if (r < U) {
+                    id = uid[r];
+                    if ((uint32_t)id >= (uint32_t)p.N) id = -1;    // never write outside the table
+                    else if (seen && atomicExch(&seen[clear_hash((uint32_t)id) & seen_mask], id) == id) id = -1;   // already taken
                 }
                 uint32_t todo = __ballot_sync(0xffffffffu, id >= 0);
                 while (todo) {
@@ -320,7 +327,8 @@ __global__ void __launch_bounds__(kClearThreads) backward_clear_kernel(const Bac
                     int32_t id = -1;
                     if (s0 + lane < ns) {
                         id = __ldg(p.sel_idx + pix * p.K + s0 + lane);
-                        if (seen && atomicExch(&seen[clear_hash((uint32_t)id) & seen_mask], id) == id) id = -1;   // already taken
+                        if ((uint32_t)id >= (uint32_t)p.N) id = -1;    // never write outside the table
+                        else if (seen && atomicExch(&seen[clear_hash((uint32_t)id) & seen_mask], id) == id) id = -1;   // already taken
                     }
                     uint32_t todo = __ballot_sync(0xffffffffu, id >= 0);
                     while (todo) {
@@ -353,11 +361,13 @@ extern "C" int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int
     BackwardParams p;
     p.cam = make_cam(cam); p.K = K; p.D = D; p.N = N;
     p.sel_idx = sel_idx; p.sel_w = nullptr; p.n_sel = n_sel; p.dL_dmap = nullptr; p.dL_dfeat = dL_dfeat;
-    int uid_stride = 0, seen_cells = 0;
+    int seen_cells = 0;
     int32_t* seen = nullptr;
+    bool have_lists = false;
     if (!ws) return fail(QR_ERR_NULL_POINTER, "qr_backward_clear: workspace is NULL");
     if (backward_mma_supported(K, D)) {
-        if (int rc = backward_mma_workspace_view(p, ws, ws_bytes, &uid_stride, &seen, &seen_cells)) return rc;
+        if (int rc = backward_mma_workspace_view(p, ws, ws_bytes, &seen, &seen_cells)) return rc;
+        have_lists = true;
     } else {                                    // no numbered unions: the workspace is only the de-duplication cache
         if (ws_bytes < (size_t)kClearSeenCells * 4) return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_backward_clear: workspace %zu < %zu bytes", ws_bytes, (size_t)kClearSeenCells * 4);
         if (!aligned16(ws)) return fail(QR_ERR_MISALIGNED, "qr_backward_clear: workspace alignment");
@@ -372,7 +382,7 @@ extern "C" int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int
             sms = 148;
     }
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
-    backward_clear_kernel<<<(unsigned)min(num_half, sms * 8), kClearThreads, 0, (cudaStream_t)stream>>>(p, uid_stride, seen, seen_cells - 1);
+    backward_clear_kernel<<<(unsigned)min(num_half, sms * 8), kClearThreads, 0, (cudaStream_t)stream>>>(p, have_lists, seen, seen_cells - 1);
     QR_LAUNCH_OK("backward_clear_kernel");
     return QR_OK;
 }
@@ -380,7 +390,7 @@ extern "C" int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int
 extern "C" size_t qr_backward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D)
 {
     if (!cam || cam->width < 1 || cam->height < 1) return 0;
-    return qr::backward_mma_supported(K, D) ? qr::backward_mma_workspace_bytes(qr::make_cam(cam))
+    return qr::backward_mma_supported(K, D) ? qr::backward_mma_workspace_bytes(qr::make_cam(cam), K)
                                             : (size_t)qr::kClearSeenCells * 4;      // used by qr_backward_clear only
 }
 
@@ -404,7 +414,7 @@ extern "C" int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N
     p.cam = make_cam(cam); p.K = K; p.D = D; p.N = N;
     p.sel_idx = sel_idx; p.sel_w = sel_w; p.n_sel = n_sel; p.dL_dmap = dL_dmap; p.dL_dfeat = dL_dfeat;
     cudaStream_t st = (cudaStream_t)stream;
-    if (backward_mma_supported(K, D)) return launch_backward_mma(p, ws, ws_bytes, st);
+    if (backward_mma_supported(K, D)) return launch_backward_mma(p, ws, ws_bytes, st, false);
     if (backward_tile_supported(K, D)) return launch_backward_tile(p, st);
     if (D % 4 == 0) {
         switch ((D + 127) / 128) {
@@ -420,4 +430,24 @@ extern "C" int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N
         case 3: return launch_backward<3, 1>(p, st);
         default: return launch_backward<4, 1>(p, st);
     }
+}
+
+extern "C" int qr_backward_lists(const qr_camera* cam, int32_t K, int32_t D, int64_t N, void* fwd_ws, size_t fwd_ws_bytes,
+                                 const float* dL_dmap, float* dL_dfeat, void* stream)
+{
+    using namespace qr;
+    if (int rc = check_cam(cam)) return rc;
+    if (K < 1) return fail(QR_ERR_INVALID_ARG, "qr_backward_lists: K = %d < 1", K);
+    if (K > QR_MAX_K) return fail(QR_ERR_UNSUPPORTED, "qr_backward_lists: K = %d > QR_MAX_K", K);
+    if (!backward_mma_supported(K, D))
+        return fail(QR_ERR_UNSUPPORTED, "qr_backward_lists: needs D %% 128 == 0, D <= 512 (D = %d): use qr_backward", D);
+    if (N < 0) return fail(QR_ERR_INVALID_ARG, "qr_backward_lists: N < 0");
+    if (!fwd_ws || !dL_dmap) return fail(QR_ERR_NULL_POINTER, "qr_backward_lists: NULL input");
+    if (N == 0) return QR_OK;
+    if (!dL_dfeat) return fail(QR_ERR_NULL_POINTER, "qr_backward_lists: dL_dfeat is NULL");
+    if (!aligned16(dL_dmap) || !aligned16(dL_dfeat)) return fail(QR_ERR_MISALIGNED, "qr_backward_lists: 16-byte alignment");
+    BackwardParams p;
+    p.cam = make_cam(cam); p.K = K; p.D = D; p.N = N;
+    p.sel_idx = nullptr; p.sel_w = nullptr; p.n_sel = nullptr; p.dL_dmap = dL_dmap; p.dL_dfeat = dL_dfeat;
+    return launch_backward_mma(p, fwd_ws, fwd_ws_bytes, (cudaStream_t)stream, true);
 }

@@ -1,6 +1,7 @@
 // qr_backward.cuh -- parameters shared by the qr_backward kernels (qr_backward.cu, qr_backward_tile.cu).
 #pragma once
 #include "qr_common.cuh"
+#include "qr_sel.cuh"
 
 namespace qr {
 
@@ -13,11 +14,10 @@ struct BackwardParams {
     const int32_t* n_sel;
     const float* dL_dmap;
     float* dL_dfeat;
-    // written by backward_prep_kernel (qr_backward_mma.cu) into the caller's workspace; NULL on the FFMA-only paths
-    const int32_t* prep_cnt = nullptr;     // [half tiles][4]: records in pixels 0..63, records, distinct Gaussians,
-                                           // 1 = this half tile is left to backward_tile_kernel
-    const int32_t* prep_uid = nullptr;     // [half tiles][kBmEntCap] union row -> Gaussian id
-    const uint2* prep_ent = nullptr;       // [half tiles][kBmEntCap] {weight bits, union row << 8 | pixel}, pixel order
+    // tcgen05 path: the selection lists (qr_sel.cuh) -- written by backward_prep_kernel into the caller's workspace, or left
+    // there by qr_forward (qr_backward_lists); hdr[5] == 1 marks a half tile left to backward_tile_kernel.  Unset on the
+    // FFMA-only paths.
+    SelLists sl;
     const int32_t* prep_nflag = nullptr;   // [1] how many half tiles carry that flag
     bool only_flagged = false;             // backward_tile_kernel: process only half tiles with prep_cnt[..][3] == 1
 };
@@ -26,9 +26,10 @@ struct BackwardParams {
 bool backward_tile_supported(int32_t K, int32_t D);
 // qr_backward_mma.cu: the same contraction on tcgen05 (tf32 x 3), D a multiple of 128.
 bool backward_mma_supported(int32_t K, int32_t D);
-size_t backward_mma_workspace_bytes(const Cam& cam);
-int backward_mma_workspace_view(BackwardParams& p, void* ws, size_t ws_bytes, int* uid_stride, int32_t** seen, int* seen_cells);
-int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_t st);
+size_t backward_mma_workspace_bytes(const Cam& cam, int K);
+int backward_mma_workspace_view(BackwardParams& p, void* ws, size_t ws_bytes, int32_t** seen, int* seen_cells);
+// from_lists: ws is a workspace whose selection lists are already complete (qr_forward's): no numbering pass
+int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_t st, bool from_lists);
 int launch_backward_tile(const BackwardParams& p, cudaStream_t st);
 
 }  // namespace qr

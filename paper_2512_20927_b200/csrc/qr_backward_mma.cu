@@ -62,7 +62,6 @@ constexpr int kBmEntCap = 3072;            // selection records (and distinct Ga
 constexpr int kBmEntRegs = 8;              // entries a setup thread holds in flight
 constexpr int kBmLoStages = 2;             // G_lo is produced just ahead of the MMA that reads it
 constexpr int kBmDescRing = 4;
-constexpr int kBmSeenCells = 1 << 20;      // qr_backward_clear's de-duplication table (a cache, not a set: 4 MB)
 
 struct BmDesc {
     int32_t ht, j0, j1, nrows, flags, pad; // flags: 1 = no more work
@@ -169,6 +168,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
+    if (!sel_stamp_ok(p.sl.stamp, p.cam, p.K)) return;      // not the lists of this camera / K: touch nothing
 
     if (tid == 0) {
         for (int s = 0; s < stages; ++s) { mbar_init(&raw_full[s], 1); mbar_init(&stage_empty[s], 1); }
@@ -225,7 +225,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                 }
 #pragma unroll
                 for (int c = 0; c < 16; ++c) {
-                    if (c0 + c < nrows) {
+                    if (c0 + c < nrows && row[c0 + c] >= 0) {
                         float* a = dcol + row[c0 + c];
                         bm_red(a, __uint_as_float(r0[c]));
                         if (nchunks > 1) bm_red(a + 128, __uint_as_float(r1[c]));
@@ -355,23 +355,37 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
             const int tile = ht >> 1;
             return (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8 < p.cam.height;
         };
+        struct Hd { int n[4], U, flag; };
+        auto load_hd = [&](int ht) -> Hd {
+            Hd t;
+            t.n[0] = t.n[1] = t.n[2] = t.n[3] = 0; t.U = 0; t.flag = 0;
+            if (ht < num_half && inside(ht)) {
+                const int32_t* hd = p.sl.hdr + (size_t)ht * kHdrWords;
+                const int4 v = __ldg(reinterpret_cast<const int4*>(hd));
+                const int2 w = __ldg(reinterpret_cast<const int2*>(hd + 4));
+                t.n[0] = v.x; t.n[1] = v.y; t.n[2] = v.z; t.n[3] = v.w; t.U = w.x; t.flag = w.y;
+            }
+            return t;
+        };
         int ht = blockIdx.x;
-        int4 cnt = make_int4(0, 0, 0, 0);
-        if (ht < num_half && inside(ht)) cnt = __ldg(reinterpret_cast<const int4*>(p.prep_cnt) + ht);
+        Hd cnt = load_hd(ht);
         while (ht < num_half) {
             const int ht1 = ht + (int)gridDim.x;
-            int4 cnt1 = make_int4(0, 0, 0, 0);
-            if (ht1 < num_half && inside(ht1)) cnt1 = __ldg(reinterpret_cast<const int4*>(p.prep_cnt) + ht1);
-            const int R0 = cnt.x, R = cnt.y, U = cnt.z;
-            if (R > 0 && cnt.w == 0) {                    // cnt.w: left to backward_tile_kernel (too many records)
-                const uint2* ent = p.prep_ent + (size_t)ht * kBmEntCap;
-                const int32_t* uid = p.prep_uid + (size_t)ht * kBmEntCap;
+            const Hd cnt1 = load_hd(ht1);
+            const int U = cnt.U;
+            const int R = cnt.n[0] + cnt.n[1] + cnt.n[2] + cnt.n[3];
+            if (R > 0 && cnt.flag == 0) {                 // flag: left to backward_tile_kernel (too many records for the prep)
+                const uint2* ent = p.sl.ent + (size_t)ht * kSelLists * p.sl.qcap;
+                const int32_t* uid = p.sl.uid + (size_t)ht * p.sl.ucap;
                 const int npass = (U + kBmRows - 1) / kBmRows;
                 for (int pass = 0; pass < npass; ++pass, ++unit) {
                     BmDesc* d = &desc[unit % kBmDescRing];
                     const int c_lo = pass * kBmRows;
                     for (int h = 0; h < 2; ++h) {
-                        const int kb = h ? R0 : 0, n = (h ? R : R0) - kb;
+                        // W half h = pixels 64 h .. 64 h + 63 = lists 2 h and 2 h + 1, read as one flat sequence
+                        const int na = cnt.n[2 * h], n = na + cnt.n[2 * h + 1];
+                        const uint2* la = ent + (size_t)(2 * h) * p.sl.qcap;
+                        const uint2* lb = la + p.sl.qcap;
                         unsigned char* whi = Wsm + h * 2 * kBmWHalfBytes;
                         uint2 e[kBmEntRegs];
                         int64_t rowoff = 0;
@@ -379,10 +393,13 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
 #pragma unroll
                             for (int u = 0; u < kBmEntRegs; ++u) {
                                 const int k = base + u * kBmSetupThreads + st;
-                                e[u] = k < n ? __ldg(ent + kb + k) : make_uint2(0u, 0xFFFFFFFFu);
+                                e[u] = k < n ? __ldg(k < na ? la + k : lb + (k - na)) : make_uint2(0u, 0xFFFFFFFFu);
                             }
                             if (base == 0) {
-                                if (h == 0 && st < kBmRows && c_lo + st < U) rowoff = (int64_t)__ldg(uid + c_lo + st) * D;
+                                if (h == 0 && st < kBmRows && c_lo + st < U) {
+                                    const int32_t id = __ldg(uid + c_lo + st);
+                                    rowoff = (uint32_t)id < (uint32_t)p.N ? (int64_t)id * D : -1;   // never add outside the table
+                                }
                                 mbar_wait(&w_free[h], (unit & 1) ^ 1);      // the MMAs of the previous unit have read this half
                                 float4* wz = reinterpret_cast<float4*>(whi);
                                 for (int k = st; k < 2 * kBmWHalfBytes / 16; k += kBmSetupThreads) wz[k] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -390,9 +407,9 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                             }
 #pragma unroll
                             for (int u = 0; u < kBmEntRegs; ++u) {
-                                const int c = (int)(e[u].y >> 8) - c_lo;
-                                if (c >= 0 && c < kBmRows) {          // padding entries have c = 2^24 - 1 - c_lo
-                                    const uint32_t off = bm_w_off(c, (int)(e[u].y & (kBmHalfPx - 1)));
+                                const int c = sel_col(e[u].y) - c_lo;
+                                if (c >= 0 && c < kBmRows) {          // padding entries have column 2^17 - 1
+                                    const uint32_t off = bm_w_off(c, sel_pixel(e[u].y) & (kBmHalfPx - 1));
                                     const float w = __uint_as_float(e[u].x), hi = bm_hi(w);
                                     *reinterpret_cast<float*>(whi + off) = hi;
                                     *reinterpret_cast<float*>(whi + kBmWHalfBytes + off) = __fsub_rn(w, hi);
@@ -432,35 +449,18 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
 
 bool backward_mma_supported(int32_t K, int32_t D) { return D % 128 == 0 && D >= 128 && D <= 512 && K >= 1 && K <= QR_MAX_K; }
 
-// workspace: per half tile {R0, R, U, left-to-the-tile-kernel} + union ids + entries
-struct BmWorkspace { size_t hdr, cnt, uid, ent, seen, total; };
-static BmWorkspace bm_workspace(const Cam& cam)
+// workspace = the common layout of qr_sel.cuh (the forward's workspace has the same one)
+size_t backward_mma_workspace_bytes(const Cam& cam, int K) { return ws_layout(cam, K).total; }
+// points p at the lists and the clear cache inside ws
+int backward_mma_workspace_view(BackwardParams& p, void* ws, size_t ws_bytes, int32_t** seen, int* seen_cells)
 {
-    const size_t nh = (size_t)cam.tiles_x * cam.tiles_y * 2;
-    BmWorkspace w;
-    size_t o = 0;
-    w.hdr = o; o = align_up(o + 256, 256);                      // [0] number of half tiles left to backward_tile_kernel
-    w.cnt = o; o = align_up(o + nh * 16, 256);
-    w.uid = o; o = align_up(o + nh * kBmEntCap * 4, 256);
-    w.ent = o; o = align_up(o + nh * kBmEntCap * 8, 256);
-    w.seen = o; o = align_up(o + (size_t)kBmSeenCells * 4, 256);   // qr_backward_clear: ids whose row is already zeroed
-    w.total = o;
-    return w;
-}
-size_t backward_mma_workspace_bytes(const Cam& cam) { return bm_workspace(cam).total; }
-// points p at the arrays a previous launch_backward_mma left in ws (for qr_backward_clear)
-int backward_mma_workspace_view(BackwardParams& p, void* ws, size_t ws_bytes, int* uid_stride, int32_t** seen, int* seen_cells)
-{
-    const BmWorkspace wl = bm_workspace(p.cam);
+    const WsLayout wl = ws_layout(p.cam, p.K);
     if (ws_bytes < wl.total) return fail(QR_ERR_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", ws_bytes, wl.total);
     if (!aligned16(ws)) return fail(QR_ERR_MISALIGNED, "workspace alignment");
-    char* w = static_cast<char*>(ws);
-    p.prep_cnt = reinterpret_cast<const int32_t*>(w + wl.cnt);
-    p.prep_uid = reinterpret_cast<const int32_t*>(w + wl.uid);
-    p.prep_ent = reinterpret_cast<const uint2*>(w + wl.ent);
-    *uid_stride = kBmEntCap;
-    *seen = reinterpret_cast<int32_t*>(w + wl.seen);
-    *seen_cells = kBmSeenCells;
+    p.sl = sel_view(wl.sel, ws);
+    p.prep_nflag = reinterpret_cast<const int32_t*>(ws);
+    *seen = reinterpret_cast<int32_t*>(static_cast<char*>(ws) + wl.seen);
+    *seen_cells = kSeenCells;
     return QR_OK;
 }
 
@@ -474,9 +474,7 @@ int backward_mma_workspace_view(BackwardParams& p, void* ws, size_t ws_bytes, in
 constexpr int kBmPrepThreads = 256;
 constexpr int kBmPrepSmem = kBmHash * 4 + kBmHash * 2 + kBmEntCap * 4 + kBmEntCap * 4 + kBmEntCap + 2 * (kBmPx + 4) * 4;
 
-__global__ void __launch_bounds__(kBmPrepThreads) backward_prep_kernel(const BackwardParams p, int32_t* __restrict__ cnt,
-                                                              int32_t* __restrict__ uid, uint2* __restrict__ ent,
-                                                              int32_t* __restrict__ nflag)
+__global__ void __launch_bounds__(kBmPrepThreads) backward_prep_kernel(const BackwardParams p, int32_t* __restrict__ nflag)
 {
     extern __shared__ __align__(16) unsigned char psm[];
     int32_t* hkey = reinterpret_cast<int32_t*>(psm);
@@ -491,6 +489,12 @@ __global__ void __launch_bounds__(kBmPrepThreads) backward_prep_kernel(const Bac
     // threads 0..127 own a pixel each for the scan; all kBmPrepThreads share the record-parallel phases
     const int ht = blockIdx.x, pl = threadIdx.x, lane = pl & 31, warp = pl >> 5;
     const int K = p.K;
+    int32_t* hdr = p.sl.hdr + (size_t)ht * kHdrWords;
+    if (ht == 0 && pl == 0) {
+        p.sl.stamp[0] = kSelMagic; p.sl.stamp[1] = p.cam.width; p.sl.stamp[2] = p.cam.height; p.sl.stamp[3] = K;
+        const unsigned long long a = (unsigned long long)p.sel_idx;
+        p.sl.stamp[4] = (int32_t)(a & 0xffffffffull); p.sl.stamp[5] = (int32_t)(a >> 32);
+    }
     const int tile = ht >> 1;
     const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
     // pixel pl of the half tile: stage j = pl >> 3 covers row j >> 1, x = 8 (j & 1) .. + 7
@@ -517,10 +521,8 @@ __global__ void __launch_bounds__(kBmPrepThreads) backward_prep_kernel(const Bac
         R += s;
     }
     if (R > kBmEntCap || R == 0) {
-        if (pl == 0) {
-            reinterpret_cast<int4*>(cnt)[ht] = make_int4(R0, R, 0, R > kBmEntCap ? 1 : 0);
-            if (R > kBmEntCap) atomicAdd(nflag, 1);
-        }
+        if (pl < kHdrWords) hdr[pl] = (pl == 5 && R > kBmEntCap) ? 1 : 0;      // empty lists; [5]: left to the FFMA kernel
+        if (pl == 0 && R > kBmEntCap) atomicAdd(nflag, 1);
         return;
     }
     if (pl < kBmPx) { E[pl] = e0; nss[pl] = ns; }
@@ -557,7 +559,7 @@ __global__ void __launch_bounds__(kBmPrepThreads) backward_prep_kernel(const Bac
         }
     }
     __syncthreads();
-    int32_t* uid_h = uid + (size_t)ht * kBmEntCap;
+    int32_t* uid_h = p.sl.uid + (size_t)ht * p.sl.ucap;
 #pragma unroll 4
     for (int k = pl; k < R; k += kBmPrepThreads) {       // the thread that creates a cell numbers it
         const int32_t id = sid[k];
@@ -575,15 +577,24 @@ __global__ void __launch_bounds__(kBmPrepThreads) backward_prep_kernel(const Bac
         }
     }
     __syncthreads();
-    uint2* ent_h = ent + (size_t)ht * kBmEntCap;
+    // the records are ordered by pixel: list q (pixels 32 q .. 32 q + 31) is records [E[32 q], E[32 q + 32])
+    uint2* ent_h = p.sl.ent + (size_t)ht * kSelLists * p.sl.qcap;
 #pragma unroll 4
     for (int k = pl; k < R; k += kBmPrepThreads) {
         const int32_t id = sid[k];
         uint32_t h = bm_hash((uint32_t)id) & hmask;
         while (hkey[h] != id) h = (h + 1) & hmask;
-        ent_h[k] = make_uint2(__float_as_uint(sw[k]), ((uint32_t)hslot[h] << 8) | (uint32_t)spx[k]);
+        const int q = spx[k], list = q >> 5;
+        ent_h[(size_t)list * p.sl.qcap + (k - E[32 * list])] =
+            make_uint2(__float_as_uint(sw[k]), sel_pack((int)hslot[h], k - E[q], q));
     }
-    if (pl == 0) reinterpret_cast<int4*>(cnt)[ht] = make_int4(R0, R, ucount, 0);
+    if (pl < kHdrWords) {
+        int v = 0;
+        if (pl < 3) v = E[32 * (pl + 1)] - E[32 * pl];
+        else if (pl == 3) v = R - E[96];
+        else if (pl == 4) v = ucount;
+        hdr[pl] = v;
+    }
 }
 
 typedef CUresult (*BmEncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -603,18 +614,16 @@ static BmEncodeTiledFn bm_encode_tiled_fn()
     return fn;
 }
 
-int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_t st)
+int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_t st, bool from_lists)
 {
-    const BmWorkspace wl = bm_workspace(p.cam);
+    const WsLayout wl = ws_layout(p.cam, p.K);
     if (!ws) return fail(QR_ERR_NULL_POINTER, "qr_backward: workspace is NULL");
     if (ws_bytes < wl.total) return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_backward: workspace %zu < %zu bytes", ws_bytes, wl.total);
     if (!aligned16(ws)) return fail(QR_ERR_MISALIGNED, "qr_backward: workspace alignment");
-    int32_t* cnt = reinterpret_cast<int32_t*>(static_cast<char*>(ws) + wl.cnt);
-    int32_t* uid = reinterpret_cast<int32_t*>(static_cast<char*>(ws) + wl.uid);
-    uint2* ent = reinterpret_cast<uint2*>(static_cast<char*>(ws) + wl.ent);
-    int32_t* nflag = reinterpret_cast<int32_t*>(static_cast<char*>(ws) + wl.hdr);
-    p.prep_cnt = cnt; p.prep_uid = uid; p.prep_ent = ent; p.prep_nflag = nflag;
-    QR_CUDA_OK(cudaMemsetAsync(nflag, 0, 256, st));
+    p.sl = sel_view(wl.sel, ws);
+    int32_t* nflag = reinterpret_cast<int32_t*>(ws);
+    p.prep_nflag = nflag;
+    if (!from_lists) QR_CUDA_OK(cudaMemsetAsync(nflag, 0, 256, st));
     static int sms = 0;
     if (sms == 0) {
         int dev = 0;
@@ -639,12 +648,15 @@ int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_
     const int fixed = bm_smem(p.D, 0).total;
     const int stages = max(2, min(12, (232448 - fixed - 1280) / (kBmStagePx * p.D * 4)));
     const int smem = bm_smem(p.D, stages).total;
-    QR_CUDA_OK(cudaFuncSetAttribute(backward_prep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBmPrepSmem));
-    backward_prep_kernel<<<(unsigned)num_half, kBmPrepThreads, kBmPrepSmem, st>>>(p, cnt, uid, ent, nflag);
-    QR_LAUNCH_OK("backward_prep_kernel");
+    if (!from_lists) {
+        QR_CUDA_OK(cudaFuncSetAttribute(backward_prep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBmPrepSmem));
+        backward_prep_kernel<<<(unsigned)num_half, kBmPrepThreads, kBmPrepSmem, st>>>(p, nflag);
+        QR_LAUNCH_OK("backward_prep_kernel");
+    }
     QR_CUDA_OK(cudaFuncSetAttribute(backward_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     backward_mma_kernel<<<grid, kBmThreads, smem, st>>>(p, stages, tmap);
     QR_LAUNCH_OK("backward_mma_kernel");
+    if (from_lists) return QR_OK;       // the walk's lists have exact capacities: no half tile is left over
     // half tiles with more than kBmEntCap records (rare: a mean of more than 24 selections per pixel)
     p.only_flagged = true;
     return launch_backward_tile(p, st);

@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const Back
                     int x0, y0;
                     origin(ht, x0, y0);
                     if (y0 >= p.cam.height) continue;
-                    if (p.only_flagged && p.prep_cnt[4 * ht + 3] == 0) continue;   // the tcgen05 kernel did this one
+                    if (p.only_flagged && p.sl.hdr[(size_t)ht * kHdrWords + 5] == 0) continue;   // the tcgen05 kernel did this one
                     return ht;
                 }
             };

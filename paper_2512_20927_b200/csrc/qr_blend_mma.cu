@@ -32,6 +32,7 @@
 // [256, 512) two W buffers of 64 hi + 64 lo columns.  Work unit = (half tile, 128 channels).  A half tile whose union
 // exceeds 64 columns is processed in rounds of 64 columns (two rounds keep both W instances resident).
 #include <cuda.h>
+#include <stdlib.h>
 
 #include "qr_async.cuh"
 #include "qr_blend.cuh"
@@ -184,10 +185,11 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
     const long long prof_t0 = clock64();
 #define PW(cls, bar, par) do { const long long t_ = clock64(); mbar_wait_quiet(bar, par); prof[cls] += clock64() - t_; } while (0)
 #else
-#define PW(cls, bar, par) mbar_wait_quiet(bar, par)
+#define PW(cls, bar, par) mbar_wait(bar, par)
 #endif
     // every role walks the same sequence of descriptors h = 0, 1, ...; the scheduler warp publishes them, and a ring slot is
-    // reused only after every consumer warp has copied what it needs out of it (desc_done)
+    // reused only after every consumer warp is through with that half tile (desc_done: what it read from the slot has
+    // long been used by then -- an mbarrier arrive does not wait for the warp's outstanding shared-memory loads)
     auto desc_done = [&](int h) {
         __syncwarp();
         if (lane == 0) mbar_arrive(&d_free[h % kDescRing]);
@@ -219,7 +221,6 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
             const int ht = d->ht;
             const int tile = ht >> 1;
             const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8 + 2 * warp;
-            desc_done(h);
             for (int c = 0; c < nunits; ++c, ++unit) {
                 const int buf = unit & 1;
                 PW(1, &tmem_full[buf], (unit >> 1) & 1);
@@ -254,6 +255,7 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                     }
                 }
             }
+            desc_done(h);
         }
         if (lane == 0) bulk_wait<0>();
     } else if (warp == kMmaWarp) {
@@ -268,7 +270,6 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
             const MmaDesc* d = wait_desc(h);
             if (d->end) break;
             const int U = d->U;
-            desc_done(h);
             const int rounds = rounds_of(U);
             const bool reuse = rounds <= 2;                // both W instances stay resident for every unit of the half tile
             const int wi0 = wi;
@@ -306,6 +307,7 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                 __syncwarp();
             }
             if (reuse) wi = wi0 + rounds;
+            desc_done(h);
         }
     } else if (warp >= kLoadWarp && warp < kLoadWarp + kLoadWarps) {
         // ================================================= loader ===================================================
@@ -322,7 +324,6 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
             int32_t my_ids[kUidS / 32];                    // the shared ids of this half tile, lane-strided, copied out
 #pragma unroll
             for (int q = 0; q < kUidS / 32; ++q) my_ids[q] = q * 32 + lane < U ? uid_h[q * 32 + lane] : 0;
-            desc_done(h);
             const int rounds = rounds_of(U);
             for (int c = 0; c < nunits; ++c) {
                 for (int r = 0; r < rounds; ++r) {
@@ -355,6 +356,7 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                     }
                 }
             }
+            desc_done(h);
         }
     } else if (warp == kSchedWarp) {
         // ================================================= scheduler ================================================
@@ -380,6 +382,9 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                     const long long tf_ = clock64();
 #endif
                     while (ld_acquire(flag) == 0) __nanosleep(500);
+#ifdef QR_LAG
+                    { const int32_t* f2 = p.sl.flags + min(ht + QR_LAG, num_half - 1); while (ld_acquire(f2) == 0) __nanosleep(500); }
+#endif
 #ifdef QR_PROF
                     prof[2] += clock64() - tf_;
 #endif
@@ -423,7 +428,6 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
             const MmaDesc* d = wait_desc(h);
             if (d->end) break;
             const int U = d->U;
-            desc_done(h);
             const int rounds = rounds_of(U);
             for (int c = 0; c < nunits; ++c) {
                 for (int r = 0; r < rounds; ++r) {
@@ -440,8 +444,6 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                             if (row < kStageRows && j * kStageRows + row < ncols)
                                 a[q] = *reinterpret_cast<const float4*>(raw_base + sr * kRawBytes + row * kRawRow + lane * 16);
                         }
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(&raw_empty[sr]);          // the raw rows are in registers
                         const int s = st % kStages;
                         PW(2, &empty[s], ((st / kStages) & 1) ^ 1);
 #pragma unroll
@@ -457,10 +459,13 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                         }
                         fence_async_smem();
                         __syncwarp();
-                        if (lane == 0) mbar_arrive(&full[s]);
+                        // the raw slot is released only now: the loads above have provably completed (their values were
+                        // stored), so the loader's next TMA write cannot overtake a read still queued in the LSU
+                        if (lane == 0) { mbar_arrive(&raw_empty[sr]); mbar_arrive(&full[s]); }
                     }
                 }
             }
+            desc_done(h);
         }
     } else if (warp >= kFirstBuild) {
         // ================================================= builders =================================================
@@ -484,7 +489,6 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
             HT t;
             t.end = d->end; t.ht = d->ht; t.U = d->U;
             t.n = (&d->n0)[bq];
-            if (!t.end) desc_done(h);
             return t;
         };
         auto load_set = [&](const HT& t, int base, uint2 (&e)[kEntRegs]) {
@@ -557,6 +561,7 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                 prod_sync();                                 // every row is in tensor memory; the scratch tile is free again
                 if (ptid == 0) mbar_arrive(&w_ready[wi & 1]);
             }
+            desc_done(h);                                    // (the fields of descriptor h + 1 were copied out after a barrier)
             cur = nxt;
         }
     }
@@ -619,7 +624,7 @@ int launch_blend_mma(const BlendParams& p, cudaStream_t st)
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
+    cfg.attrs = attr; cfg.numAttrs = getenv("QR_NO_PDL") ? 0 : 1;   // EXPERIMENT
     QR_CUDA_OK(cudaLaunchKernelEx(&cfg, blend_mma_kernel, p, tmap));
     QR_LAUNCH_OK("blend_mma_kernel");
     return QR_OK;

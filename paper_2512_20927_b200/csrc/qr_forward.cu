@@ -44,8 +44,9 @@ static FwdLayout fwd_layout(const Cam& cam, int K)
     L.gcount = o; o = align_up(o + (size_t)L.G * 4, 256);
     L.ucount = o; o = align_up(o + (size_t)(L.G / 16) * 4, 256);
     L.rec = o;    o = align_up(o + (size_t)L.G * L.cap * kRecWords * 4, 256);
-    L.sel = sel_layout(cam, K, L.gcount);
-    L.total = o > L.sel.total ? o : L.sel.total;
+    const WsLayout wl = ws_layout(cam, K);      // tcgen05 path: the layout qr_backward_lists / qr_backward_clear also read
+    L.sel = wl.sel;
+    L.total = o > wl.total ? o : wl.total;
     return L;
 }
 

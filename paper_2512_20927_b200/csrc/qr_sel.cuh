@@ -87,6 +87,27 @@ inline SelLists sel_view(const SelLayout& L, void* ws)
 }
 constexpr int32_t kSelMagic = 0x51524c31;   // "QRL1"
 
+// Common layout of the qr_forward and the qr_backward workspace (fp32 features, D % 128 == 0: the tcgen05 paths), so that
+// qr_backward_lists and qr_backward_clear can be handed either one:
+//   [0, 256)      scratch words of the owning call (qr_backward: [0] half tiles left to the FFMA kernel)
+//   [256, ...)    selection lists: stamp, tickets + release flags, headers, union ids, entries
+//   then          qr_backward_clear's de-duplication cache (kSeenCells ints)
+constexpr int kSeenCells = 1 << 20;
+struct WsLayout { SelLayout sel; size_t seen, total; };
+inline WsLayout ws_layout(const Cam& cam, int K)
+{
+    WsLayout L;
+    L.sel = sel_layout(cam, K, 256);
+    L.seen = L.sel.total;
+    L.total = align_up(L.seen + (size_t)kSeenCells * 4, 256);
+    return L;
+}
+// device-side check that lists belong to this camera and K (anything else: the kernel leaves without touching memory)
+__device__ __forceinline__ bool sel_stamp_ok(const int32_t* stamp, const Cam& cam, int K)
+{
+    return stamp[0] == kSelMagic && stamp[1] == cam.width && stamp[2] == cam.height && stamp[3] == K;
+}
+
 // qr_walk.cu
 struct WalkParams2 {
     Cam cam;

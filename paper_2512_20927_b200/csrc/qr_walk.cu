@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
     const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
     int32_t* hdr = p.sl.hdr + (size_t)ht * kHdrWords;
     if (y0 >= p.cam.height) {                         // half tile below the image: empty lists
-        if (tid < kHdrWords) hdr[tid] = 0;
+        if (tid < kHdrWords) { hdr[tid] = 0; __threadfence(); }
         __syncthreads();
         if (tid == 0) { __threadfence(); st_release(p.sl.flags + ht, 1); }
         continue;
@@ -272,12 +272,13 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
             }
         }
     }
+    __threadfence();                                           // every lane: its entries, records (and lane 0's uid entries)
     __syncwarp();
     if (lane == 0) {
         hdr[warp] = n_ent;
         atomicAdd(&s_evals, n_eval);
         atomicMax(&s_consumed, consumed);
-        __threadfence();                                       // this warp's lists, records and uid entries
+        __threadfence();
         if (atomicAdd(&s_finished, 1) == kSelLists - 1) {      // the last warp of the half tile publishes it
             hdr[4] = s_ucount; hdr[5] = 0;
             hdr[6] = s_consumed; hdr[7] = s_evals; hdr[8] = (int32_t)(clock64() - t_start);

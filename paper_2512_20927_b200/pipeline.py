@@ -42,12 +42,19 @@ def forward(cam, fe: Frontend, features: torch.Tensor, K: int, out: Optional[B.F
 
 def backward(cam, N: int, fwd: B.ForwardOut, dL_dmap: torch.Tensor, dL_dfeat: Optional[torch.Tensor] = None,
              ws: Optional[torch.Tensor] = None):
+    """dL/dF of the frame `fwd`.  Without a workspace of its own the call goes through qr_backward_lists where the
+    forward left its selection lists (fp32 features, D % 128 == 0: no second numbering pass); with `ws`, or for the
+    other shapes, through qr_backward on the selection records."""
+    D = int(dL_dmap.shape[-1])
+    if ws is None and fwd.ws is not None and fwd.has_lists and fwd.out_map.shape[-1] == D:
+        return B.qr_backward_lists(cam, int(fwd.sel_idx.shape[-1]), N, fwd.ws, dL_dmap, dL_dfeat)
     return B.qr_backward(cam, N, fwd.sel_idx, fwd.sel_w, fwd.n_sel, dL_dmap, dL_dfeat, ws)
 
 
-def backward_clear(cam, N: int, fwd: B.ForwardOut, dL_dfeat: torch.Tensor, ws: torch.Tensor):
-    """Re-zero the rows the last backward(..., ws) touched (instead of zeroing the whole [N, D] table)."""
-    return B.qr_backward_clear(cam, N, fwd.sel_idx, fwd.n_sel, dL_dfeat, ws)
+def backward_clear(cam, N: int, fwd: B.ForwardOut, dL_dfeat: torch.Tensor, ws: Optional[torch.Tensor] = None):
+    """Re-zero the rows the last backward touched (instead of zeroing the whole [N, D] table).  ws = the workspace that
+    backward used: its own, or (default) the forward's."""
+    return B.qr_backward_clear(cam, N, fwd.sel_idx, fwd.n_sel, dL_dfeat, fwd.ws if ws is None else ws)
 
 
 def dense_forward(cam, fe: Frontend, features: torch.Tensor, t_min: float = 1e-4, out_map=None, final_T=None):

@@ -32,7 +32,7 @@ def test_every_declared_symbol_is_exported(lib):
 def test_version_and_tiles(lib):
     from paper_2512_20927_b200 import binding
     from qr_inputs import make_camera
-    assert lib.qr_version() == 100
+    assert lib.qr_version() == 200
     assert binding.qr_num_tiles(make_camera(640, 480)) == 1200
     assert binding.qr_num_tiles(make_camera(70, 50)) == 5 * 4
     assert lib.qr_num_tiles(None) == 0
