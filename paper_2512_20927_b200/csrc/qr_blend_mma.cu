@@ -47,7 +47,7 @@ constexpr int kLoadWarp = 5;                              // warps 5, 6, 7: stag
 constexpr int kLoadWarps = 3;
 constexpr int kSchedWarp = 8;
 constexpr int kFirstConv = 9;
-constexpr int kConvWarps = 3;                             // union rows pw, pw + 3, pw + 6 of every stage
+constexpr int kConvWarps = 3;                             // stage st is converted by warp 9 + st % 3
 constexpr int kFirstBuild = 12;
 constexpr int kBuildWarps = 4;
 constexpr int kMmaThreads = (kFirstBuild + kBuildWarps) * 32;   // 512
@@ -56,7 +56,7 @@ constexpr int kDescReaders = kEpiWarps + 1 + kLoadWarps + kConvWarps + kBuildWar
 constexpr int kWCols = 64;                                // union columns per round
 constexpr int kUnitN = 128;                               // channels per work unit
 constexpr int kStageRows = 8;                             // union rows per stage = one tf32 K step
-constexpr int kStages = 3;
+constexpr int kStages = 6;
 constexpr int kRawStages = 12;
 constexpr int kRawRow = kUnitN * 4;                       // 512 B: one feature row quarter
 constexpr int kRawBytes = kStageRows * kRawRow;           // 4 KB per raw stage
@@ -69,7 +69,7 @@ constexpr int kOutBufs = 3;                               // staging tiles per e
 constexpr int kOutTile = 32 * 128;                        // 32 pixels x 32 channels fp32
 constexpr int kDescRing = 4;
 constexpr int kUidS = 128;                                // union ids per half tile the builders hand to the loader through shared memory
-constexpr int kEntRegs = 6;                               // entries a builder lane holds per scatter round (x 2 sets in flight)
+constexpr int kEbuf = 512;                                // entries of each list staged in shared memory (cp.async)
 
 struct MmaDesc { int32_t ht, U, n0, n1, n2, n3, end, pad; };
 
@@ -78,7 +78,8 @@ struct MmaSmem {
     static constexpr int stages = kWsBytes;
     static constexpr int raw = stages + kStages * kStageBytes;
     static constexpr int out = raw + kRawStages * kRawBytes;              // [4 warps][kOutBufs] staging tiles, 1 KB aligned
-    static constexpr int desc = out + kEpiWarps * kOutBufs * kOutTile;
+    static constexpr int ebuf = out + kEpiWarps * kOutBufs * kOutTile;     // uint2[4 lists][kEbuf] staged entries
+    static constexpr int desc = ebuf + kSelLists * kEbuf * 8;
     static constexpr int uid = desc + kDescRing * (int)sizeof(MmaDesc);    // int32[kDescRing][kUidS]: first ids of each union
     static constexpr int bars = uid + kDescRing * kUidS * 4;
     static constexpr int n_bars = 2 * kStages + 2 * kRawStages + 4 + 4 + 2 * kDescRing;
@@ -124,6 +125,12 @@ __device__ __forceinline__ int32_t ld_acquire(const int32_t* p)
     asm volatile("ld.acquire.gpu.global.b32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+// four rows of the [N, D] feature table, any four, 128 channels each, in one TMA instruction: they land as [4][512 B]
+__device__ __forceinline__ void tma_gather4(void* dst, const CUtensorMap* map, int c0, int r0, int r1, int r2, int r3, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cta.global.tile::gather4.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+                 ::"r"(s32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(s32(bar)), "r"(c0), "r"(r0), "r"(r1), "r"(r2), "r"(r3) : "memory");
+}
 __device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, const void* src, int c0, int x, int y)
 {
     asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];"
@@ -136,17 +143,17 @@ __device__ __forceinline__ int cols_of(int U, int r) { return max(0, min(kWCols,
 __device__ __forceinline__ int ksteps_of(int ncols) { return max(1, (ncols + kStageRows - 1) / kStageRows); }
 
 __global__ void __launch_bounds__(kMmaThreads, 2)       // "2" only caps the registers at 64; shared memory allows one CTA
-blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tmap)
+blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tmap, const __grid_constant__ CUtensorMap feat_tmap)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char* stage_base = smem + MmaSmem::stages;
     MmaDesc* desc = reinterpret_cast<MmaDesc*>(smem + MmaSmem::desc);
     int32_t* uid_s = reinterpret_cast<int32_t*>(smem + MmaSmem::uid);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + MmaSmem::bars);
-    uint64_t* full = bars;                       // [kStages] converters -> MMA (4 warp arrivals)
+    uint64_t* full = bars;                       // [kStages] converter warp of the stage -> MMA
     uint64_t* empty = bars + kStages;            // [kStages] MMA -> converters (tcgen05.commit)
     uint64_t* raw_full = bars + 2 * kStages;     // [kRawStages] loader (TMA complete_tx) -> converters
-    uint64_t* raw_empty = raw_full + kRawStages; // [kRawStages] converters -> loader (4 warp arrivals)
+    uint64_t* raw_empty = raw_full + kRawStages; // [kRawStages] converter warp of the stage -> loader
     uint64_t* w_ready = raw_empty + kRawStages;  // [2] builders -> MMA: W instance i lives in tensor-memory buffer i & 1
     uint64_t* w_free = w_ready + 2;              // [2] MMA -> builders (tcgen05.commit)
     uint64_t* tmem_full = w_free + 2;            // [2] MMA -> epilogue (tcgen05.commit)
@@ -162,8 +169,8 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
 
     if (tid == 0) {
         stamp_time(p.sl.ctrl, 2, true);
-        for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], kConvWarps); mbar_init(&empty[s], 1); }
-        for (int s = 0; s < kRawStages; ++s) { mbar_init(&raw_full[s], 1); mbar_init(&raw_empty[s], kConvWarps); }
+        for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < kRawStages; ++s) { mbar_init(&raw_full[s], 1); mbar_init(&raw_empty[s], 1); }
         for (int b = 0; b < 2; ++b) {
             mbar_init(&w_ready[b], 1); mbar_init(&w_free[b], 1);
             mbar_init(&tmem_full[b], 1); mbar_init(&tmem_empty[b], kEpiWarps);
@@ -344,15 +351,24 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                             }
                             if (lane < rows) id = col < kUidS ? v : __ldcg(uid + col);
                         }
+                        // lane g < 2 gathers rows 4 g .. 4 g + 3 with one instruction; rows past the union repeat a valid id
+                        // (the converters zero them)
+                        const int ngrp = (rows + 3) >> 2;
+                        int ids4[4];
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const int src = min(4 * (lane & 1) + k, max(rows - 1, 0));
+                            ids4[k] = __shfl_sync(0xffffffffu, id, src);
+                        }
                         PW(1, &raw_empty[s], ((st / kRawStages) & 1) ^ 1);
                         if (lane == 0) {
-                            if (rows > 0) mbar_arrive_expect_tx(&raw_full[s], (uint32_t)rows * kRawRow);
+                            if (ngrp > 0) mbar_arrive_expect_tx(&raw_full[s], (uint32_t)ngrp * 4 * kRawRow);
                             else mbar_arrive(&raw_full[s]);
                         }
                         __syncwarp();
-                        if (lane < rows)
-                            bulk_g2s(raw_base + s * kRawBytes + lane * kRawRow,
-                                     static_cast<const float*>(p.features) + (int64_t)id * D + c * kUnitN, kRawRow, &raw_full[s]);
+                        if (lane < ngrp)
+                            tma_gather4(raw_base + s * kRawBytes + lane * 4 * kRawRow, &feat_tmap, c * kUnitN,
+                                        ids4[0], ids4[1], ids4[2], ids4[3], &raw_full[s]);
                     }
                 }
             }
@@ -411,18 +427,16 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
         }
     } else if (warp >= kFirstConv && warp < kFirstBuild) {
         // ================================================= converters ===============================================
-        // warp pw splits union rows pw, pw + 3 (and pw + 6) of every stage: ld.shared of the raw row -> hi / lo -> st.shared
-        // in the MN-major SWIZZLE_128B_BASE32B layout.
+        // converter warp pw owns the stages st with st % 3 == pw (all 8 union rows of the stage): ld.shared of the raw rows ->
+        // hi / lo -> st.shared in the MN-major SWIZZLE_128B_BASE32B layout.  One warp per stage, three stages in flight:
+        // with the rows of ONE stage spread over the warps every hand-over latency (barrier wake-up, ld.shared,
+        // fence.proxy.async) was paid 24 times in series per half tile and the MMA warp starved.
         const int pw = warp - kFirstConv;                 // 0..2
         const unsigned char* raw_base = smem + MmaSmem::raw;
         // byte offset of this lane's 16 bytes (channels 4 lane .. 4 lane + 3) inside a stage half, row q of the stage
         auto lane_off = [&](int q) -> uint32_t {
             return (uint32_t)((lane >> 3) * 1024 + (q >> 2) * 512 + (q & 3) * 128 + ((((lane & 7) >> 1) ^ (q & 3)) * 32) + (lane & 1) * 16);
         };
-        constexpr int kRowsPerConv = (kStageRows + kConvWarps - 1) / kConvWarps;   // 3
-        uint32_t off[kRowsPerConv];
-#pragma unroll
-        for (int q = 0; q < kRowsPerConv; ++q) off[q] = lane_off(min(pw + kConvWarps * q, kStageRows - 1));
         int st = 0;
         for (int h = 0;; ++h) {
             const MmaDesc* d = wait_desc(h);
@@ -434,28 +448,27 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                     const int ncols = cols_of(U, r);
                     const int nk = ksteps_of(ncols);
                     for (int j = 0; j < nk; ++j, ++st) {
+                        if (st % kConvWarps != pw) continue;
                         const int sr = st % kRawStages;
                         PW(1, &raw_full[sr], (st / kRawStages) & 1);
-                        float4 a[kRowsPerConv];
+                        const int rows = max(0, min(kStageRows, ncols - j * kStageRows));
+                        float4 a[kStageRows];
 #pragma unroll
-                        for (int q = 0; q < kRowsPerConv; ++q) {
-                            const int row = pw + kConvWarps * q;
+                        for (int q = 0; q < kStageRows; ++q) {
                             a[q] = make_float4(0.f, 0.f, 0.f, 0.f);
-                            if (row < kStageRows && j * kStageRows + row < ncols)
-                                a[q] = *reinterpret_cast<const float4*>(raw_base + sr * kRawBytes + row * kRawRow + lane * 16);
+                            if (q < rows) a[q] = *reinterpret_cast<const float4*>(raw_base + sr * kRawBytes + q * kRawRow + lane * 16);
                         }
                         const int s = st % kStages;
                         PW(2, &empty[s], ((st / kStages) & 1) ^ 1);
+                        unsigned char* stg = stage_base + s * kStageBytes;
 #pragma unroll
-                        for (int q = 0; q < kRowsPerConv; ++q) {
-                            if (pw + kConvWarps * q < kStageRows) {
-                                unsigned char* hi = stage_base + s * kStageBytes + off[q];
-                                const float4 v = a[q];
-                                const float4 hv = make_float4(tf32_hi(v.x), tf32_hi(v.y), tf32_hi(v.z), tf32_hi(v.w));
-                                *reinterpret_cast<float4*>(hi) = hv;
-                                *reinterpret_cast<float4*>(hi + kStageHalf) =
-                                    make_float4(__fsub_rn(v.x, hv.x), __fsub_rn(v.y, hv.y), __fsub_rn(v.z, hv.z), __fsub_rn(v.w, hv.w));
-                            }
+                        for (int q = 0; q < kStageRows; ++q) {
+                            unsigned char* hi = stg + lane_off(q);
+                            const float4 v = a[q];
+                            const float4 hv = make_float4(tf32_hi(v.x), tf32_hi(v.y), tf32_hi(v.z), tf32_hi(v.w));
+                            *reinterpret_cast<float4*>(hi) = hv;
+                            *reinterpret_cast<float4*>(hi + kStageHalf) =
+                                make_float4(__fsub_rn(v.x, hv.x), __fsub_rn(v.y, hv.y), __fsub_rn(v.z, hv.z), __fsub_rn(v.w, hv.w));
                         }
                         fence_async_smem();
                         __syncwarp();
@@ -472,17 +485,17 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
         const int ptid = tid - kFirstBuild * 32;          // 0..127 = pixel of the half tile = TMEM lane (warp % 4 = lane quarter)
         auto prod_sync = [&]() { named_sync<1, kBuildThreads>(); };
         float* ws = reinterpret_cast<float*>(smem + MmaSmem::w);
-        auto st16 = [&](uint32_t taddr, const uint32_t (&r)[16]) {
-            asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-                         ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
-                           "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
+        auto st8 = [&](uint32_t taddr, const uint32_t (&r)[8]) {
+            asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                         ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]) : "memory");
         };
         const uint32_t lane_base = ((uint32_t)((warp & 3) * 32)) << 16;
         int wi = 0;                                       // W instances built so far; instance i goes to buffer i & 1
-        // builder warp q scatters list q (the walk's warp q wrote it): lane i takes entries i, i + 32, ...  Loads are
-        // software pipelined: while one set of kEntRegs entries is scattered the next is in flight, and the first set of
-        // what is built next is requested before the tensor-memory phase of the current instance.
+        // builder warp q scatters list q (the walk's warp q wrote it).  The first kEbuf entries of the list are staged in
+        // shared memory by cp.async while the PREVIOUS instance is stored to tensor memory, so the scatter never waits for
+        // an L2 round trip; the rare longer lists read their tail straight from global memory.
         const int bq = warp - kFirstBuild;
+        uint2* ebuf = reinterpret_cast<uint2*>(smem + MmaSmem::ebuf) + bq * kEbuf;
         struct HT { int ht, U, n, end; };
         auto read_desc = [&](int h) -> HT {
             const MmaDesc* d = wait_desc(h);
@@ -491,74 +504,72 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
             t.n = (&d->n0)[bq];
             return t;
         };
-        auto load_set = [&](const HT& t, int base, uint2 (&e)[kEntRegs]) {
-            const uint2* ent = p.sl.ent + ((size_t)t.ht * kSelLists + bq) * p.sl.qcap + base + lane;
-#pragma unroll
-            for (int u = 0; u < kEntRegs; ++u)
-                e[u] = base + u * 32 + lane < t.n ? __ldcg(ent + u * 32) : make_uint2(0u, 0xFFFFFFFFu);
+        auto stage_entries = [&](const HT& t) {             // 16 bytes = 2 entries per cp.async
+            const uint2* src = p.sl.ent + ((size_t)t.ht * kSelLists + bq) * p.sl.qcap;
+            const int n2 = (min(t.n, kEbuf) + 1) >> 1;
+            for (int i = lane; i < n2; i += 32)
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s32(ebuf + 2 * i)), "l"(src + 2 * i) : "memory");
+            asm volatile("cp.async.commit_group;" ::: "memory");
         };
-        auto scatter_set = [&](const uint2 (&e)[kEntRegs], int r) {
-#pragma unroll
-            for (int u = 0; u < kEntRegs; ++u) {
-                const int cl = sel_col(e[u].y) - r * kWCols;           // padding entries have column 2^17 - 1
-                if (cl >= 0 && cl < kWCols) ws[sel_pixel(e[u].y) * kWsRow + cl] = __uint_as_float(e[u].x);
-            }
-        };
-        constexpr int kSet = kEntRegs * 32;
         HT cur = read_desc(0);
-        uint2 ea[kEntRegs], eb[kEntRegs];
-        if (!cur.end) load_set(cur, 0, ea);
+        if (!cur.end) stage_entries(cur);
         for (int h = 0; !cur.end; ++h) {
             const int rounds = rounds_of(cur.U);
             const int ninst = rounds <= 2 ? rounds : rounds * nunits;      // (the MMA warp derives the same sequence)
+            const uint2* tail = p.sl.ent + ((size_t)cur.ht * kSelLists + bq) * p.sl.qcap;
             HT nxt = cur;
             for (int ii = 0; ii < ninst; ++ii, ++wi) {
                 const int r = ii % rounds;
                 // ---------------- build W for columns [64 r, 64 r + 64) ----------------
+#ifdef QR_PROF
+                const long long tb0_ = clock64();
+#endif
                 {
                     const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
                     float4* wz = reinterpret_cast<float4*>(ws);
                     for (int i = ptid; i < kWsBytes / 16; i += kBuildThreads) wz[i] = z;
                 }
+                asm volatile("cp.async.wait_all;" ::: "memory");     // this warp's staged entries have landed
                 prod_sync();
-                for (int base = 0; base < cur.n || base == 0; base += 2 * kSet) {          // ea holds [base, base + kSet)
-                    if (base + kSet < cur.n) load_set(cur, base + kSet, eb);
-                    scatter_set(ea, r);
-                    if (base + kSet < cur.n) {
-                        if (base + 2 * kSet < cur.n) load_set(cur, base + 2 * kSet, ea);
-                        scatter_set(eb, r);
-                    }
+                const int c_lo = r * kWCols;
+                for (int i = lane; i < cur.n; i += 32) {
+                    const uint2 e = i < kEbuf ? ebuf[i] : __ldcg(tail + i);
+                    const int cl = sel_col(e.y) - c_lo;
+                    if (cl >= 0 && cl < kWCols) ws[sel_pixel(e.y) * kWsRow + cl] = __uint_as_float(e.x);
                 }
                 prod_sync();
-                // the scratch tile is complete.  Request the first entries of what is built next: this half tile again
-                // (another round / instance) or the next half tile
-                if (ii + 1 < ninst) load_set(cur, 0, ea);
-                else { nxt = read_desc(h + 1); if (!nxt.end) load_set(nxt, 0, ea); }
+#ifdef QR_PROF
+                const long long tb1_ = clock64();
+                prof[2] += tb1_ - tb0_;
+#endif
+                // the scratch tile is complete; after the last instance of this half tile the staging buffer is free:
+                // request the next half tile's entries now, they land during the tensor-memory phase below
+                if (ii + 1 == ninst) { nxt = read_desc(h + 1); if (!nxt.end) stage_entries(nxt); }
                 // thread = pixel: its row of 64 weights -> tensor memory, hi (the raw value: kind::tf32 reads its top 19
                 // bits) and lo = w - trunc(w); the buffer is free once the MMAs of the instance two before have retired
                 PW(1, &w_free[wi & 1], ((wi >> 1) & 1) ^ 1);
                 tc_fence_after();
                 const uint32_t t_hi = tmem_base + lane_base + (uint32_t)(kTmemW + (wi & 1) * 2 * kWCols);
                 const float4* row = reinterpret_cast<const float4*>(ws + ptid * kWsRow);
+#pragma unroll 2
+                for (int q = 0; q < kWCols / 8; ++q) {
+                    const float4 v0 = row[2 * q], v1 = row[2 * q + 1];
+                    const float f[8] = { v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w };
+                    uint32_t hi[8], lo[8];
 #pragma unroll
-                for (int q = 0; q < kWCols / 16; ++q) {
-                    uint32_t hi[16], lo[16];
-#pragma unroll
-                    for (int t = 0; t < 4; ++t) {
-                        const float4 v = row[q * 4 + t];
-                        const float f[4] = { v.x, v.y, v.z, v.w };
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            hi[4 * t + i] = __float_as_uint(f[i]);
-                            lo[4 * t + i] = __float_as_uint(__fsub_rn(f[i], tf32_hi(f[i])));
-                        }
+                    for (int i = 0; i < 8; ++i) {
+                        hi[i] = __float_as_uint(f[i]);
+                        lo[i] = __float_as_uint(__fsub_rn(f[i], tf32_hi(f[i])));
                     }
-                    st16(t_hi + q * 16, hi);
-                    st16(t_hi + kWCols + q * 16, lo);
+                    st8(t_hi + q * 8, hi);
+                    st8(t_hi + kWCols + q * 8, lo);
                 }
                 asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                 tc_fence_before();
                 prod_sync();                                 // every row is in tensor memory; the scratch tile is free again
+#ifdef QR_PROF
+                prof[3] += clock64() - tb1_;
+#endif
                 if (ptid == 0) mbar_arrive(&w_ready[wi & 1]);
             }
             desc_done(h);                                    // (the fields of descriptor h + 1 were copied out after a barrier)
@@ -611,6 +622,19 @@ int launch_blend_mma(const BlendParams& p, cudaStream_t st)
                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (cr != CUDA_SUCCESS) return fail(QR_ERR_CUDA, "qr_forward: cuTensorMapEncodeTiled failed (%d)", (int)cr);
+    // features [N][D] fp32 as a 2-D tensor (D, N) for tile::gather4: box = 128 channels x 1 row, no swizzle
+    CUtensorMap fmap;
+    {
+        // (qr_forward is not told N: the row bound is left open, ids come from the caller's own intersection lists)
+        const cuuint64_t fdims[2] = { (cuuint64_t)p.D, (cuuint64_t)0x7fffffff };
+        const cuuint64_t fstr[1] = { (cuuint64_t)p.D * 4 };
+        const cuuint32_t fbox[2] = { (cuuint32_t)kUnitN, 1 };
+        const cuuint32_t fes[2] = { 1, 1 };
+        const CUresult fr = enc(&fmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(p.features), fdims, fstr, fbox, fes,
+                                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (fr != CUDA_SUCCESS) return fail(QR_ERR_CUDA, "qr_forward: cuTensorMapEncodeTiled (features) failed (%d)", (int)fr);
+    }
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
         sms = 148;
@@ -625,7 +649,7 @@ int launch_blend_mma(const BlendParams& p, cudaStream_t st)
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = getenv("QR_NO_PDL") ? 0 : 1;   // EXPERIMENT
-    QR_CUDA_OK(cudaLaunchKernelEx(&cfg, blend_mma_kernel, p, tmap));
+    QR_CUDA_OK(cudaLaunchKernelEx(&cfg, blend_mma_kernel, p, tmap, fmap));
     QR_LAUNCH_OK("blend_mma_kernel");
     return QR_OK;
 }
