@@ -18,7 +18,8 @@ LIB = os.path.join(HERE, "libqr.so")
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"] + \
     (["-DQR_PROF"] if os.environ.get("QR_PROF") == "1" else []) + \
-    (["-DQR_LAG=" + os.environ["QR_LAG"]] if os.environ.get("QR_LAG") else [])     # per-role wait counters in the blend kernel
+    (["-DQR_LAG=" + os.environ["QR_LAG"]] if os.environ.get("QR_LAG") else []) + \
+    os.environ.get("QR_DEFS", "").split()       # QR_PROF: per-role wait counters in the blend kernel; QR_DEFS: extra -D flags for experiments
 
 
 def sources():

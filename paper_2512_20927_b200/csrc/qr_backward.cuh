@@ -19,6 +19,7 @@ struct BackwardParams {
     // FFMA-only paths.
     SelLists sl;
     const int32_t* prep_nflag = nullptr;   // [1] how many half tiles carry that flag
+    int32_t* ticket = nullptr;             // tcgen05 contraction: half-tile ticket (zeroed by the launcher)
     bool only_flagged = false;             // backward_tile_kernel: process only half tiles with prep_cnt[..][3] == 1
 };
 

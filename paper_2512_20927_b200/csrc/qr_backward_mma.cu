@@ -60,7 +60,10 @@ constexpr int kBmHash = 4096;              // backward_prep_kernel: hash cells p
 constexpr int kBmEntCap = 3072;            // selection records (and distinct Gaussians) of a half tile the tcgen05 path
                                            // takes; fuller half tiles are left to backward_tile_kernel
 constexpr int kBmEntRegs = 8;              // entries a setup thread holds in flight
-constexpr int kBmLoStages = 2;             // G_lo is produced just ahead of the MMA that reads it
+#ifndef KBM_LO
+#define KBM_LO 2
+#endif
+constexpr int kBmLoStages = KBM_LO;             // G_lo is produced just ahead of the MMA that reads it
 constexpr int kBmDescRing = 4;
 
 struct BmDesc {
@@ -80,7 +83,7 @@ __host__ __device__ inline BmSmem bm_smem(int D, int stages)
     L.desc = o;   o += kBmDescRing * (int)sizeof(BmDesc);
     o = (o + 15) & ~15;
     L.bars = o;   o += (2 * stages + 2 * kBmLoStages + 8) * 8;
-    L.misc = o;   o += 16;                                       // TMEM base, done flag
+    L.misc = o;   o += 16;                                       // TMEM base, done flag, two half-tile ticket slots
     L.total = (o + 15) & ~15;
     return L;
 }
@@ -367,11 +370,19 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
             }
             return t;
         };
-        int ht = blockIdx.x;
+        // half tiles are handed out by a global ticket (their cost varies with the union size: a static stride left the
+        // slowest CTA ~8 % behind the mean); the ticket after next is requested one half tile early and passed to the other
+        // setup threads through two alternating shared-memory slots
+        volatile int32_t* tslot = reinterpret_cast<volatile int32_t*>(smem + L.misc + 8);
+        int32_t* ticket = p.ticket;
+        if (st == 0) { tslot[0] = atomicAdd(ticket, 1); tslot[1] = atomicAdd(ticket, 1); }
+        ssync_setup();
+        int ht = tslot[0], ht1 = tslot[1];
+        ssync_setup();
         Hd cnt = load_hd(ht);
-        while (ht < num_half) {
-            const int ht1 = ht + (int)gridDim.x;
+        for (int it = 0; ht < num_half; ++it) {
             const Hd cnt1 = load_hd(ht1);
+            if (st == 0) tslot[it & 1] = atomicAdd(ticket, 1);
             const int U = cnt.U;
             const int R = cnt.n[0] + cnt.n[1] + cnt.n[2] + cnt.n[3];
             if (R > 0 && cnt.flag == 0) {                 // flag: left to backward_tile_kernel (too many records for the prep)
@@ -427,7 +438,8 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                     }
                 }
             }
-            ht = ht1; cnt = cnt1;
+            ssync_setup();
+            ht = ht1; cnt = cnt1; ht1 = tslot[it & 1];
         }
         {   // sentinel unit: tells the loader, the MMA thread and (through it) the epilogue to stop
             BmDesc* d = &desc[unit % kBmDescRing];
@@ -623,7 +635,8 @@ int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_
     p.sl = sel_view(wl.sel, ws);
     int32_t* nflag = reinterpret_cast<int32_t*>(ws);
     p.prep_nflag = nflag;
-    if (!from_lists) QR_CUDA_OK(cudaMemsetAsync(nflag, 0, 256, st));
+    QR_CUDA_OK(cudaMemsetAsync(nflag, 0, 256, st));      // [0] half tiles left to the FFMA kernel, [1] the contraction's half-tile ticket
+    p.ticket = nflag + 1;
     static int sms = 0;
     if (sms == 0) {
         int dev = 0;
