@@ -57,7 +57,10 @@ constexpr int kWCols = 64;                                // union columns per r
 constexpr int kUnitN = 128;                               // channels per work unit
 constexpr int kStageRows = 8;                             // union rows per stage = one tf32 K step
 constexpr int kStages = 6;
-constexpr int kRawStages = 12;
+#ifndef KRAW
+#define KRAW 12
+#endif
+constexpr int kRawStages = KRAW;
 constexpr int kRawRow = kUnitN * 4;                       // 512 B: one feature row quarter
 constexpr int kRawBytes = kStageRows * kRawRow;           // 4 KB per raw stage
 constexpr int kWsRow = kWCols + 4;                        // scratch row stride in floats: 272 B, conflict-free 16-byte row reads
@@ -65,11 +68,17 @@ constexpr int kWsBytes = 128 * kWsRow * 4;                // 34 KB scratch tile
 constexpr int kStageHalf = kStageRows * kUnitN * 4;       // 4 KB (hi or lo)
 constexpr int kTmemW = 256;                               // first W column in tensor memory
 constexpr int kStageBytes = 2 * kStageHalf;
-constexpr int kOutBufs = 3;                               // staging tiles per epilogue warp
+#ifndef KOUTBUFS
+#define KOUTBUFS 3
+#endif
+#ifndef KEBUF
+#define KEBUF 512
+#endif
+constexpr int kOutBufs = KOUTBUFS;                               // staging tiles per epilogue warp
 constexpr int kOutTile = 32 * 128;                        // 32 pixels x 32 channels fp32
 constexpr int kDescRing = 4;
 constexpr int kUidS = 128;                                // union ids per half tile the builders hand to the loader through shared memory
-constexpr int kEbuf = 512;                                // entries of each list staged in shared memory (cp.async)
+constexpr int kEbuf = KEBUF;                                // entries of each list staged in shared memory (cp.async)
 
 struct MmaDesc { int32_t ht, U, n0, n1, n2, n3, end, pad; };
 
@@ -192,7 +201,11 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
     const long long prof_t0 = clock64();
 #define PW(cls, bar, par) do { const long long t_ = clock64(); mbar_wait_quiet(bar, par); prof[cls] += clock64() - t_; } while (0)
 #else
+#ifdef QR_QUIET
+#define PW(cls, bar, par) mbar_wait_quiet(bar, par)
+#else
 #define PW(cls, bar, par) mbar_wait(bar, par)
+#endif
 #endif
     // every role walks the same sequence of descriptors h = 0, 1, ...; the scheduler warp publishes them, and a ring slot is
     // reused only after every consumer warp is through with that half tile (desc_done: what it read from the slot has

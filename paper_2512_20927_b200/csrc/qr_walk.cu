@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
     __shared__ int32_t s_id[kW2Batch];
     __shared__ int32_t s_col[kW2Batch];    // column of a staged entry in the union, -1 = not selected yet, -2 = being numbered
     __shared__ float thr[QR_MAX_K + 1];
-    __shared__ int32_t s_ucount, s_finished, s_evals, s_consumed;
+    __shared__ int32_t s_ucount, s_evals, s_consumed;
 
     __shared__ int32_t s_ht;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -85,12 +85,25 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
 
   // Persistent CTAs: half tiles are handed out in index order by a global ticket (the blend kernel, which may already be
   // running, consumes them in the same order); when a half tile's lists are complete its ready flag is released.
+  int prev_ht = -1;
+  long long prev_start = 0;
   while (true) {
-    __syncthreads();                                   // everybody is through with the previous half tile's shared state
-    if (tid == 0) { s_ht = atomicAdd(p.sl.ctrl, 1); s_ucount = 0; s_finished = 0; s_evals = 0; s_consumed = 0; }
+    __syncthreads();                                   // everybody is through with the previous half tile: its lists are written
+    if (tid == 0) {
+        // publish the previous half tile.  One release per CTA: the block barrier orders every thread's list, record and
+        // header stores before this thread's st.release, which is cumulative (no per-warp __threadfence: with the blend
+        // streaming the map through the same memory system a fence costs microseconds)
+        if (prev_ht >= 0) {
+            int32_t* h = p.sl.hdr + (size_t)prev_ht * kHdrWords;
+            h[4] = s_ucount; h[5] = 0; h[6] = s_consumed; h[7] = s_evals; h[8] = (int32_t)(clock64() - prev_start);
+            st_release(p.sl.flags + prev_ht, 1);
+        }
+        s_ht = atomicAdd(p.sl.ctrl, 1); s_ucount = 0; s_evals = 0; s_consumed = 0;
+    }
     __syncthreads();
     const int ht = s_ht;
     if (ht >= num_half) { if (tid == 0) stamp_time(p.sl.ctrl, 1, false); break; }
+    prev_ht = -1;
     const int tile = ht >> 1;
     const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
     int32_t* hdr = p.sl.hdr + (size_t)ht * kHdrWords;
@@ -272,20 +285,12 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
             }
         }
     }
-    __threadfence();                                           // every lane: its entries, records (and lane 0's uid entries)
-    __syncwarp();
     if (lane == 0) {
         hdr[warp] = n_ent;
         atomicAdd(&s_evals, n_eval);
         atomicMax(&s_consumed, consumed);
-        __threadfence();
-        if (atomicAdd(&s_finished, 1) == kSelLists - 1) {      // the last warp of the half tile publishes it
-            hdr[4] = s_ucount; hdr[5] = 0;
-            hdr[6] = s_consumed; hdr[7] = s_evals; hdr[8] = (int32_t)(clock64() - t_start);
-            __threadfence();
-            st_release(p.sl.flags + ht, 1);
-        }
     }
+    prev_ht = ht; prev_start = t_start;                        // published by thread 0 after the barrier at the loop top
   }
 }
 
