@@ -13,6 +13,7 @@
  *   - PAPER.md:81-86    Eq. 1 (V-Render)
  *   - PAPER.md:129-158  Algorithm 1 (QuantileRender), executed literally, line by line
  *   - SPEC.md:462-470   backward: d f~ / d f_i = w^Q_i / (1 - T^Q) * I  (selection is piecewise constant)
+ *   - PAPER.md:167,:187 top-K comparator, as reconstructed in SPEC.md:221-229 (reading R17)
  * No blocking, fusion or reordering beyond those passages.
  *
  * Precision.  Everything is fp64 EXCEPT the quantities that decide an integer (which
@@ -27,7 +28,8 @@
  * V-Render micro-rays SPEC.md:208-209, telescoping identities, closed-form projections
  * SPEC.md:58-60,:136-138,:154-156, brute-force lists == binned lists, Q -> V limiting case,
  * Appendix-C bound PAPER.md:672-678 on discretised 1-D models, adjoint identity and finite
- * differences for the backward.  No function here is "parity unpinned".
+ * differences for the backward; top-K: SPEC.md:227-229 examples, K >= n equals V-Render / (1 - T), brute-force
+ * argsort restatement, permutation of equal weights.  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -556,6 +558,118 @@ void orc_vrender(int64_t npix, const int64_t* pix, const int64_t* off, const int
             for (int d = 0; d < D; ++d) out_map[j * D + d] = (float)acc[d];
         }
         free(acc);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O6: top-K render, the paper's other comparator ("Unlike top-K sampling proposed by a
+ * concurrent study, which requires additional complexity to sort values, O(N log K + KC)"; complexity
+ * table; speed / accuracy figure PAPER.md:306-310, :332 "top-K sorts and selects K
+ * Gaussians").  The paper gives no procedure; this is the reconstruction SPEC.md:221-229, :268 fixes
+ * (reading R17), step by step:
+ *   1. dense weights of Eq. 1, w_s = T_s alpha'_s, T_s = prod_{j<s} (1 - alpha'_j), over the ray's list,
+ *      with V-Render's early stop R7 (stop before entry s when T_s (1 - alpha'_s) < t_min; t_min = 0: whole list);
+ *   2. keep the K largest w_s, ties -> the smaller list position;
+ *   3. re-blend the kept entries in depth order with a fresh transmittance:
+ *      w^top = T^top alpha',  T^top <- T^top (1 - alpha');
+ *   4. normalise by (1 - T^top) exactly as Algorithm 1 line 20; nothing kept -> zero vector, resid 1 (R8).
+ * Steps 1-2 decide integers, so T_s and w_s are fp32 in the kernel's operation order (T_test = T * (1 - a),
+ * w = T * a); steps 3-4 are fp64.  The selection is a plain O(n K) scan: for each of the K picks, the largest
+ * weight not picked yet (strict >, so the first of equals wins).
+ * gap = w_(K) - w_(K+1) (fp64 of the fp32 weights; inf when every weighted entry is kept): a pixel with
+ * gap <= 1e-6 may legitimately select differently under a 1-ulp expf difference.  stop_margin as in O3.
+ * ---------------------------------------------------------------------------------------- */
+static void topk_ray(int64_t n, const int32_t* I, const float* alpha, int K, int D, const float* F, int64_t fstride,
+                     float t_min, double* acc, int32_t* sel_idx, double* sel_w, int32_t* n_sel_out, double* resid,
+                     double* gap_out, double* stop_margin, int32_t* n_dense_out, float* wbuf, uint8_t* taken)
+{
+    /* step 1: dense weights */
+    float T = 1.0f;
+    int64_t nd = 0;
+    double marg = INFINITY;
+    for (int64_t s = 0; s < n; ++s) {
+        const float a = alpha[s];
+        const float T_test = T * (1.0f - a);
+        if (t_min > 0.0f) {
+            const double m = fabs((double)T_test - (double)t_min) / (double)t_min;
+            if (m < marg) marg = m;
+        }
+        if (T_test < t_min) break;
+        wbuf[s] = T * a;
+        taken[s] = 0;
+        T = T_test;
+        ++nd;
+    }
+    /* step 2: K largest, ties -> smaller position */
+    int32_t ns = 0;
+    double last_kept = INFINITY;
+    for (int pick = 0; pick < K && pick < nd; ++pick) {
+        int64_t best = -1;
+        for (int64_t s = 0; s < nd; ++s)
+            if (!taken[s] && (best < 0 || wbuf[s] > wbuf[best])) best = s;
+        taken[best] = 1;
+        last_kept = (double)wbuf[best];
+        ++ns;
+    }
+    double gap = INFINITY;
+    if (nd > K) {
+        int64_t best = -1;
+        for (int64_t s = 0; s < nd; ++s)
+            if (!taken[s] && (best < 0 || wbuf[s] > wbuf[best])) best = s;
+        gap = last_kept - (double)wbuf[best];
+    }
+    /* steps 3, 4: re-blend in depth order, normalise */
+    if (acc) for (int d = 0; d < D; ++d) acc[d] = 0.0;
+    for (int s = 0; s < K; ++s) { sel_idx[s] = -1; sel_w[s] = 0.0; }
+    double Tt = 1.0;
+    int32_t j = 0;
+    for (int64_t s = 0; s < nd; ++s) {
+        if (!taken[s]) continue;
+        const double a = (double)alpha[s];
+        const double w = Tt * a;
+        if (acc) {
+            const float* f = F + (int64_t)I[s] * fstride;
+            for (int d = 0; d < D; ++d) acc[d] += w * (double)f[d];
+        }
+        sel_idx[j] = I[s]; sel_w[j] = w; ++j;
+        Tt = Tt * (1.0 - a);
+    }
+    if (ns > 0) {
+        const double norm = 1.0 - Tt;
+        if (acc) for (int d = 0; d < D; ++d) acc[d] = acc[d] / norm;
+        for (int s = 0; s < ns; ++s) sel_w[s] = sel_w[s] / norm;
+    } else {
+        Tt = 1.0;
+    }
+    *n_sel_out = ns; *resid = Tt; *gap_out = gap; *stop_margin = marg; *n_dense_out = (int32_t)nd;
+}
+
+void orc_topk(int64_t npix, const int64_t* pix, const int64_t* off, const int32_t* gid, const float* alpha,
+              int K, int D, const float* features, int64_t fstride, float t_min, float* out_map, int32_t* sel_idx,
+              double* sel_w, int32_t* n_sel, double* resid, double* gap, double* stop_margin, int32_t* n_dense)
+{
+#pragma omp parallel
+    {
+        double* acc = (double*)malloc(sizeof(double) * (size_t)(D > 0 ? D : 1));
+        int64_t cap = 0;
+        float* wbuf = NULL;
+        uint8_t* taken = NULL;
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t j = 0; j < npix; ++j) {
+            const int64_t p = pix ? pix[j] : j;
+            const int64_t b = off[p], e = off[p + 1];
+            if (e - b > cap) {
+                cap = (e - b) * 2;
+                free(wbuf); free(taken);
+                wbuf = (float*)malloc(sizeof(float) * (size_t)cap);
+                taken = (uint8_t*)malloc((size_t)cap);
+            }
+            topk_ray(e - b, gid + b, alpha + b, K, D, features, fstride, t_min, features ? acc : NULL, sel_idx + j * K,
+                     sel_w + j * K, n_sel + j, resid + j, gap + j, stop_margin + j, n_dense + j, wbuf, taken);
+            if (features && out_map)
+                for (int d = 0; d < D; ++d) out_map[j * D + d] = (float)acc[d];
+        }
+        free(acc); free(wbuf); free(taken);
     }
 }
 

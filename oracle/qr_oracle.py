@@ -225,6 +225,39 @@ def vrender(lists: PixelLists, features: np.ndarray, t_min: float = 1e-4,
     return VOut(out, ft, sm, nb)
 
 
+@dataclass
+class TopKOut:
+    out_map: Optional[np.ndarray]  # [P,D] float32
+    sel_idx: np.ndarray            # [P,K] int32, -1 padded, depth order
+    sel_w: np.ndarray              # [P,K] float64 normalised weights w^top/(1-T^top), 0 padded
+    n_sel: np.ndarray              # [P] int32 = min(K, n_dense)
+    resid: np.ndarray              # [P] float64 T^top (1 where nothing kept)
+    gap: np.ndarray                # [P] float64 w_(K) - w_(K+1), inf when everything is kept
+    stop_margin: np.ndarray        # [P] float64 as VOut.stop_margin
+    n_dense: np.ndarray            # [P] int32 entries that received a dense weight
+
+
+def topk(lists: PixelLists, K: int, features: Optional[np.ndarray] = None, t_min: float = 1e-4,
+         pixels: Optional[np.ndarray] = None) -> TopKOut:
+    """Top-K render: K largest dense weights, re-blended in depth order."""
+    if K < 1:
+        raise ValueError("K must be >= 1")
+    npix = (len(lists.off) - 1) if pixels is None else len(pixels)
+    pix = None if pixels is None else np.ascontiguousarray(pixels, dtype=np.int64)
+    D = 0; feats = None; out = None; fstride = 0
+    if features is not None:
+        feats = _f32(features)
+        D = feats.shape[1]; fstride = feats.shape[1]
+        out = np.empty((npix, D), np.float32)
+    sel_idx = np.empty((npix, K), np.int32); sel_w = np.empty((npix, K), np.float64)
+    n_sel = np.empty(npix, np.int32); rs = np.empty(npix, np.float64)
+    gap = np.empty(npix, np.float64); sm = np.empty(npix, np.float64); nd = np.empty(npix, np.int32)
+    lib().orc_topk(C.c_int64(npix), _p(pix), _p(lists.off), _p(lists.gid), _p(lists.alpha), C.c_int(K), C.c_int(D),
+                   _p(feats), C.c_int64(fstride), C.c_float(t_min), _p(out), _p(sel_idx), _p(sel_w), _p(n_sel), _p(rs),
+                   _p(gap), _p(sm), _p(nd))
+    return TopKOut(out, sel_idx, sel_w, n_sel, rs, gap, sm, nd)
+
+
 def backward(sel_idx, sel_w, n_sel, dL_dmap, N: int, rows: Optional[np.ndarray] = None) -> np.ndarray:
     """dL/dF rows (all N, or only `rows`) in fp64 from the selection records of every pixel."""
     sel_idx = np.ascontiguousarray(sel_idx, dtype=np.int32)

@@ -557,3 +557,98 @@ def test_fp16_features_are_widened_exactly(orc, tiny):
     a = orc.qrender(lists, 10, f16).out_map
     b = orc.qrender(lists, 10, f16.astype(np.float32)).out_map
     assert np.array_equal(a, b)
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-1: top-K render (reading R17)
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ray", _gold("topk_rays.json")["rays"], ids=lambda r: r["name"][:2])
+def test_topk_hand_worked(orc, ray):
+    n = len(ray["alphas"])
+    feats = np.eye(n, dtype=np.float32)
+    lists = orc.lists_from_rays([(range(n), ray["alphas"])])
+    t = orc.topk(lists, ray["K"], feats, t_min=ray["t_min"])
+    ns = len(ray["selected"])
+    assert t.n_sel[0] == ns and t.n_dense[0] == len(ray["dense_w"])
+    assert t.sel_idx[0, :ns].tolist() == ray["selected"] and (t.sel_idx[0, ns:] == -1).all()
+    np.testing.assert_allclose(t.sel_w[0, :ns], ray["w_hat"], rtol=2e-6)
+    np.testing.assert_allclose(t.resid[0], ray["T_top"], rtol=2e-5)     # products of fp32-rounded alphas
+    np.testing.assert_allclose(t.sel_w[0, :ns] * (1.0 - t.resid[0]), ray["w_top"], rtol=2e-6)
+    expect = np.zeros(n)
+    expect[ray["selected"]] = ray["w_hat"]
+    np.testing.assert_allclose(t.out_map[0], expect, rtol=2e-6, atol=1e-12)
+
+
+def _topk_numpy(alphas, K, t_min):
+    """Independent restatement with library routines: cumprod for Eq. 1, a stable argsort for the selection."""
+    a = np.asarray(alphas, np.float32)
+    T = np.float32(1.0); w = []
+    for x in a:                                   # the fp32 decision arithmetic of DESIGN.md: T_test = T * (1 - a), w = T * a
+        Tt = np.float32(T * np.float32(np.float32(1.0) - x))
+        if Tt < np.float32(t_min):
+            break
+        w.append(np.float32(T * x)); T = Tt
+    w = np.asarray(w, np.float32)
+    keep = np.sort(np.argsort(-w, kind="stable")[:K])
+    ad = a[keep].astype(np.float64)
+    Tex = np.concatenate([[1.0], np.cumprod(1.0 - ad)])
+    wt = Tex[:-1] * ad
+    resid = Tex[-1] if len(keep) else 1.0
+    return keep, (wt / (1.0 - resid) if len(keep) else wt), resid, len(w)
+
+
+def test_topk_matches_numpy_restatement_on_random_rays(orc):
+    rng = np.random.default_rng(11)
+    rays = []
+    for _ in range(400):
+        n = int(rng.integers(0, 70))
+        al = np.minimum(0.99, rng.beta(0.7, 2.0, n)).astype(np.float32)
+        al[rng.random(n) < 0.15] = np.float32(0.25)            # repeated values: exercises the tie rule
+        rays.append((np.arange(n), al))
+    lists = orc.lists_from_rays(rays)
+    for K, t_min in [(1, 0.0), (4, 1e-4), (10, 1e-4), (40, 0.0), (64, 1e-4)]:
+        t = orc.topk(lists, K, None, t_min=t_min)
+        for p, (_, al) in enumerate(rays):
+            keep, w, resid, nd = _topk_numpy(al, K, t_min)
+            assert t.n_dense[p] == nd and t.n_sel[p] == len(keep) == min(K, nd)
+            assert t.sel_idx[p, :len(keep)].tolist() == keep.tolist()
+            np.testing.assert_allclose(t.sel_w[p, :len(keep)], w, rtol=1e-12)
+            np.testing.assert_allclose(t.resid[p], resid, rtol=1e-12)
+
+
+def test_topk_keeps_the_heaviest_subset_brute_force(orc):
+    """Among all K-subsets of the weighted entries the kept one has the largest total dense weight (definition of
+    'K largest'), checked by enumeration on tiny rays."""
+    import itertools
+    rng = np.random.default_rng(12)
+    for _ in range(60):
+        n = int(rng.integers(1, 9)); K = int(rng.integers(1, 5))
+        al = rng.uniform(0.02, 0.9, n).astype(np.float32)
+        t = orc.topk(orc.lists_from_rays([(np.arange(n), al)]), K, None, t_min=0.0)
+        T = np.concatenate([[1.0], np.cumprod(1.0 - al.astype(np.float64))])[:-1]
+        w = T * al
+        best = max(itertools.combinations(range(n), min(K, n)), key=lambda c: sum(w[list(c)]))
+        assert sorted(t.sel_idx[0, :t.n_sel[0]].tolist()) == sorted(best)
+
+
+def test_topk_limits_and_invariants(orc):
+    sc = make_scene("cfg1", seed=3)
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    lists = orc.pixel_lists(sc.cam, proj)
+    v = orc.vrender(lists, sc.features, t_min=0.0)
+    big = orc.topk(lists, 4096, sc.features, t_min=0.0)          # K >= every list: V-Render / (1 - T) (SPEC.md:227)
+    has = big.n_sel > 0
+    np.testing.assert_allclose(big.out_map[has], v.out_map[has] / (1.0 - v.final_T[has, None]), rtol=2e-6, atol=1e-7)
+    np.testing.assert_allclose(big.resid[has], v.final_T[has], rtol=1e-12)
+    t = orc.topk(lists, 8, sc.features, t_min=1e-4)
+    assert (t.n_sel == np.minimum(8, t.n_dense)).all()
+    np.testing.assert_allclose(t.sel_w.sum(1)[t.n_sel > 0], 1.0, rtol=1e-12)      # same normalisation as Algorithm 1 line 20
+    assert (t.sel_w >= 0).all() and ((t.resid >= 0) & (t.resid <= 1)).all()
+    assert (t.out_map[t.n_sel == 0] == 0).all() and (t.resid[t.n_sel == 0] == 1).all()        # R8
+    # kept entries come back in depth order: positions inside the pixel's list strictly increase
+    for p in np.flatnonzero(t.n_sel > 1)[:300]:
+        ids, _ = lists.ray(p)
+        pos = [int(np.flatnonzero(ids == g)[0]) for g in t.sel_idx[p, :t.n_sel[p]]]
+        assert pos == sorted(pos)
+    with pytest.raises(ValueError):
+        orc.topk(lists, 0, None)                                                  # SPEC.md:226: K = 0 is a domain error
