@@ -36,6 +36,7 @@ extern "C" {
 #define QR_VERSION 200       /* major*10000 + minor*100 + patch */
 #define QR_TILE 16           /* tile edge in pixels (3D-GS convention) */
 #define QR_MAX_K 256         /* largest K qr_forward / qr_backward accept */
+#define QR_TOPK_MAX_K 64      /* largest K qr_topk_forward accepts (the paper sweeps 5..50) */
 #define QR_MAX_D 512         /* largest feature width ("up to 512-D") */
 
 typedef enum {
@@ -185,6 +186,26 @@ int qr_dense_forward(const qr_camera* cam, int32_t D, qr_dtype feat_dtype, float
                      const float* mean2d, const float* conic_opac,
                      const uint32_t* isect_gauss, const int32_t* tile_range, const void* features,
                      float* out_map, float* final_T, void* stream);
+
+/*
+ * qr_topk_forward -- the paper's second comparator, top-K render ("top-K sampling ... requires additional
+ * complexity to sort values, O(N log K + KC)"; complexity table; "top-K sorts and selects K
+ * Gaussians").  The paper gives no procedure; this is the reconstruction of SPEC.md:221-229 (reading R17):
+ * dense weights w_i = T_i alpha'_i of Eq. 1 over the pixel's list (same inclusion rule R4 and early stop R7 / t_min as
+ * qr_dense_forward), the K largest kept (ties -> the earlier list position), re-blended in depth order with a fresh
+ * transmittance T^top, normalised by 1 - T^top like Algorithm 1 line 20; nothing kept -> zero vector, resid = 1.
+ *   in : as qr_forward, plus t_min (>= 0; 1e-4 by convention, 0 = weights over the whole list)
+ *   out: out_map[H,W,D] fp32; sel_idx / sel_w / n_sel / resid in qr_forward's record format (slots s < n_sel[p] are
+ *        written; n_sel[p] = min(K, weighted entries)), so qr_backward accepts them as they are.
+ * K in [1, QR_TOPK_MAX_K].  ws must hold qr_topk_workspace_bytes(cam, K, D) bytes (scratch; used for fp32, D % 128 == 0,
+ * where the blend is the same tcgen05 contraction as qr_forward's; may be NULL otherwise).
+ */
+size_t qr_topk_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D);
+int qr_topk_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype, float t_min,
+                    const float* mean2d, const float* conic_opac,
+                    const uint32_t* isect_gauss, const int32_t* tile_range, const void* features,
+                    float* out_map, int32_t* sel_idx, float* sel_w, int32_t* n_sel, float* resid,
+                    void* ws, size_t ws_bytes, void* stream);
 
 #ifdef __cplusplus
 }

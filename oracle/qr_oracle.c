@@ -576,8 +576,9 @@ void orc_vrender(int64_t npix, const int64_t* pix, const int64_t* off, const int
  * Steps 1-2 decide integers, so T_s and w_s are fp32 in the kernel's operation order (T_test = T * (1 - a),
  * w = T * a); steps 3-4 are fp64.  The selection is a plain O(n K) scan: for each of the K picks, the largest
  * weight not picked yet (strict >, so the first of equals wins).
- * gap = w_(K) - w_(K+1) (fp64 of the fp32 weights; inf when every weighted entry is kept): a pixel with
- * gap <= 1e-6 may legitimately select differently under a 1-ulp expf difference.  stop_margin as in O3.
+ * gap = (w_(K) - w_(K+1)) / w_(K) (fp64 of the fp32 weights; inf when every weighted entry is kept): a 1-ulp expf
+ * difference moves alpha' by ~1e-7 relative and the dense T by up to a few 1e-6 relative (sum of d alpha / (1 - alpha)),
+ * so a pixel with gap <= 1e-5 may legitimately keep the other entry.  stop_margin as in O3.
  * ---------------------------------------------------------------------------------------- */
 static void topk_ray(int64_t n, const int32_t* I, const float* alpha, int K, int D, const float* F, int64_t fstride,
                      float t_min, double* acc, int32_t* sel_idx, double* sel_w, int32_t* n_sel_out, double* resid,
@@ -616,7 +617,7 @@ static void topk_ray(int64_t n, const int32_t* I, const float* alpha, int K, int
         int64_t best = -1;
         for (int64_t s = 0; s < nd; ++s)
             if (!taken[s] && (best < 0 || wbuf[s] > wbuf[best])) best = s;
-        gap = last_kept - (double)wbuf[best];
+        gap = (last_kept - (double)wbuf[best]) / last_kept;
     }
     /* steps 3, 4: re-blend in depth order, normalise */
     if (acc) for (int d = 0; d < D; ++d) acc[d] = 0.0;

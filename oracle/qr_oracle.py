@@ -232,7 +232,7 @@ class TopKOut:
     sel_w: np.ndarray              # [P,K] float64 normalised weights w^top/(1-T^top), 0 padded
     n_sel: np.ndarray              # [P] int32 = min(K, n_dense)
     resid: np.ndarray              # [P] float64 T^top (1 where nothing kept)
-    gap: np.ndarray                # [P] float64 w_(K) - w_(K+1), inf when everything is kept
+    gap: np.ndarray                # [P] float64 (w_(K) - w_(K+1)) / w_(K), inf when everything is kept
     stop_margin: np.ndarray        # [P] float64 as VOut.stop_margin
     n_dense: np.ndarray            # [P] int32 entries that received a dense weight
 

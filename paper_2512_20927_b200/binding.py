@@ -27,7 +27,7 @@ STATUS = {0: "QR_OK", -1: "QR_ERR_INVALID_ARG", -2: "QR_ERR_NULL_POINTER", -3: "
 # every symbol include/qr.h declares (tests check that the library exports exactly these)
 SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_bin_workspace_bytes", "qr_bin_count",
            "qr_bin_sort", "qr_forward_workspace_bytes", "qr_forward", "qr_backward_workspace_bytes", "qr_backward",
-           "qr_backward_lists", "qr_backward_clear", "qr_dense_forward"]
+           "qr_backward_lists", "qr_backward_clear", "qr_dense_forward", "qr_topk_workspace_bytes", "qr_topk_forward"]
 
 
 class QRError(RuntimeError):
@@ -87,6 +87,9 @@ def load() -> C.CDLL:
     lib.qr_backward_clear.argtypes = [cam, i32, i32, i64, vp, vp, vp, vp, sz, vp]
     lib.qr_dense_forward.restype = C.c_int
     lib.qr_dense_forward.argtypes = [cam, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.qr_topk_workspace_bytes.restype = sz; lib.qr_topk_workspace_bytes.argtypes = [cam, i32, i32]
+    lib.qr_topk_forward.restype = C.c_int
+    lib.qr_topk_forward.argtypes = [cam, i32, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     _lib = lib
     return lib
 
@@ -229,9 +232,9 @@ def qr_forward_workspace_bytes(cam, K: int, D: int) -> int:
 _ws_cache = {}
 
 
-def _workspace(nbytes: int, dev) -> torch.Tensor:
-    """One cached scratch tensor per device, grown on demand (device memory only; contents are scratch)."""
-    key = str(dev)
+def _workspace(nbytes: int, dev, tag: str = "") -> torch.Tensor:
+    """One cached scratch tensor per device (and tag), grown on demand (device memory only; contents are scratch)."""
+    key = str(dev) + tag
     t = _ws_cache.get(key)
     if t is None or t.numel() < nbytes:
         t = torch.empty((max(int(nbytes), 256),), dtype=torch.uint8, device=dev)
@@ -344,3 +347,37 @@ def qr_dense_forward(cam, mean2d, conic_opac, isect_gauss, tile_range, features,
                                    _dev(features, features.dtype, "features"), out_map.data_ptr(), final_T.data_ptr(),
                                    _stream()))
     return out_map, final_T
+
+
+def qr_topk_forward(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, features, t_min: float = 1e-4,
+                    out: Optional[ForwardOut] = None, ws: Optional[torch.Tensor] = None) -> ForwardOut:
+    """Top-K render comparator (include/qr.h qr_topk_forward).  Returns records in qr_forward's format; its workspace
+    is its own (the forward's selection lists are left alone)."""
+    c = make_camera(cam)
+    H, W = c.height, c.width
+    D = int(features.shape[1])
+    dev = features.device
+    dt = _feat_dtype(features)
+    if ws is None:
+        ws = _workspace(int(load().qr_topk_workspace_bytes(C.byref(c), int(K), D)), dev, "topk")
+    kk = max(int(K), 1)
+    if out is None:
+        out = ForwardOut(torch.empty((H, W, D), dtype=torch.float32, device=dev),
+                         torch.empty((H, W, kk), dtype=torch.int32, device=dev),
+                         torch.empty((H, W, kk), dtype=torch.float32, device=dev),
+                         torch.empty((H, W), dtype=torch.int32, device=dev),
+                         torch.empty((H, W), dtype=torch.float32, device=dev))
+    else:
+        want = {"out_map": (H, W, D), "sel_idx": (H, W, kk), "sel_w": (H, W, kk), "n_sel": (H, W), "resid_TQ": (H, W)}
+        for name, shape in want.items():
+            if tuple(getattr(out, name).shape) != shape:
+                raise QRError(-1, f"out.{name} has shape {tuple(getattr(out, name).shape)}, expected {shape}")
+    _check(load().qr_topk_forward(C.byref(c), int(K), D, dt, float(t_min), _dev(mean2d, torch.float32, "mean2d"),
+                                  _dev(conic_opac, torch.float32, "conic_opac"),
+                                  _dev(isect_gauss, torch.int32, "isect_gauss"), _dev(tile_range, torch.int32, "tile_range"),
+                                  _dev(features, features.dtype, "features"), out.out_map.data_ptr(), out.sel_idx.data_ptr(),
+                                  out.sel_w.data_ptr(), out.n_sel.data_ptr(), out.resid_TQ.data_ptr(),
+                                  ws.data_ptr(), ws.numel(), _stream()))
+    out.ws = None
+    out.has_lists = False
+    return out

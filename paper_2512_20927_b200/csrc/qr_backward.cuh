@@ -32,5 +32,9 @@ int backward_mma_workspace_view(BackwardParams& p, void* ws, size_t ws_bytes, in
 // from_lists: ws is a workspace whose selection lists are already complete (qr_forward's): no numbering pass
 int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_t st, bool from_lists);
 int launch_backward_tile(const BackwardParams& p, cudaStream_t st);
+// backward_prep_kernel alone: numbers each half tile's union of selected Gaussians and writes its entry lists (p.sl) from the
+// selection records; *nflag counts the half tiles it left out (more than 5,120 records; their hdr[5] == 1).  qr_topk_forward
+// feeds the tcgen05 blend with it.
+int launch_backward_prep(const BackwardParams& p, int32_t* nflag, cudaStream_t st);
 
 }  // namespace qr

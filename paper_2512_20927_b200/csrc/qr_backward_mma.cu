@@ -56,8 +56,8 @@ constexpr int kBmStagesPerUnit = kBmPx / kBmStagePx;   // 16
 constexpr int kBmRows = 64;                // union rows per pass = MMA N
 constexpr int kBmHalfPx = 64;              // pixels per W half buffer
 constexpr int kBmWHalfBytes = kBmRows * kBmHalfPx * 4;           // 16 KB (hi or lo of one half)
-constexpr int kBmHash = 4096;              // backward_prep_kernel: hash cells per half tile
-constexpr int kBmEntCap = 3072;            // selection records (and distinct Gaussians) of a half tile the tcgen05 path
+constexpr int kBmHash = 8192;              // backward_prep_kernel: hash cells per half tile
+constexpr int kBmEntCap = 5120;            // selection records (and distinct Gaussians) of a half tile the tcgen05 path
                                            // takes; fuller half tiles are left to backward_tile_kernel
 constexpr int kBmEntRegs = 8;              // entries a setup thread holds in flight
 #ifndef KBM_LO
@@ -626,6 +626,15 @@ static BmEncodeTiledFn bm_encode_tiled_fn()
     return fn;
 }
 
+int launch_backward_prep(const BackwardParams& p, int32_t* nflag, cudaStream_t st)
+{
+    const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
+    QR_CUDA_OK(cudaFuncSetAttribute(backward_prep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBmPrepSmem));
+    backward_prep_kernel<<<(unsigned)num_half, kBmPrepThreads, kBmPrepSmem, st>>>(p, nflag);
+    QR_LAUNCH_OK("backward_prep_kernel");
+    return QR_OK;
+}
+
 int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_t st, bool from_lists)
 {
     const WsLayout wl = ws_layout(p.cam, p.K);
@@ -661,11 +670,8 @@ int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_
     const int fixed = bm_smem(p.D, 0).total;
     const int stages = max(2, min(12, (232448 - fixed - 1280) / (kBmStagePx * p.D * 4)));
     const int smem = bm_smem(p.D, stages).total;
-    if (!from_lists) {
-        QR_CUDA_OK(cudaFuncSetAttribute(backward_prep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBmPrepSmem));
-        backward_prep_kernel<<<(unsigned)num_half, kBmPrepThreads, kBmPrepSmem, st>>>(p, nflag);
-        QR_LAUNCH_OK("backward_prep_kernel");
-    }
+    if (!from_lists)
+        if (int rc = launch_backward_prep(p, nflag, st)) return rc;
     QR_CUDA_OK(cudaFuncSetAttribute(backward_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     backward_mma_kernel<<<grid, kBmThreads, smem, st>>>(p, stages, tmap);
     QR_LAUNCH_OK("backward_mma_kernel");

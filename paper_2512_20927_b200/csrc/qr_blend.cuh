@@ -35,6 +35,8 @@ struct BlendParams {
 
 // tcgen05 blend (qr_blend_mma.cu): fp32 features, D a multiple of 256.
 bool blend_mma_supported(int32_t D, qr_dtype feat_dtype);
-int launch_blend_mma(const BlendParams& p, cudaStream_t st);
+// pdl: launch with programmatic stream serialization behind walk2_kernel (the half tiles' release flags synchronise the
+// two); false: a plain launch behind whatever wrote the lists
+int launch_blend_mma(const BlendParams& p, cudaStream_t st, bool pdl = true);
 
 }  // namespace qr

@@ -621,7 +621,7 @@ static EncodeTiledFn encode_tiled_fn()
     return fn;
 }
 
-int launch_blend_mma(const BlendParams& p, cudaStream_t st)
+int launch_blend_mma(const BlendParams& p, cudaStream_t st, bool pdl)
 {
     // out_map [H][W][D] fp32 as a 3-D tensor (D, W, H); box = 32 channels x 16 pixels x 2 rows, 128-byte swizzle
     EncodeTiledFn enc = encode_tiled_fn();
@@ -661,7 +661,7 @@ int launch_blend_mma(const BlendParams& p, cudaStream_t st)
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = getenv("QR_NO_PDL") ? 0 : 1;   // EXPERIMENT
+    cfg.attrs = attr; cfg.numAttrs = (pdl && !getenv("QR_NO_PDL")) ? 1 : 0;     // QR_NO_PDL: serialise the two kernels (profiling)
     QR_CUDA_OK(cudaLaunchKernelEx(&cfg, blend_mma_kernel, p, tmap, fmap));
     QR_LAUNCH_OK("blend_mma_kernel");
     return QR_OK;

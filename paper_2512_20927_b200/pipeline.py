@@ -60,3 +60,8 @@ def backward_clear(cam, N: int, fwd: B.ForwardOut, dL_dfeat: torch.Tensor, ws: O
 def dense_forward(cam, fe: Frontend, features: torch.Tensor, t_min: float = 1e-4, out_map=None, final_T=None):
     return B.qr_dense_forward(cam, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, t_min,
                               out_map, final_T)
+
+
+def topk_forward(cam, fe: Frontend, features: torch.Tensor, K: int, t_min: float = 1e-4, out: Optional[B.ForwardOut] = None):
+    """The top-K comparator on the same front end."""
+    return B.qr_topk_forward(cam, K, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, t_min, out)

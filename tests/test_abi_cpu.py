@@ -65,6 +65,13 @@ def test_bad_arguments_are_status_codes(lib):
     assert lib.qr_preprocess(C.byref(cam), 0, z, z, z, z, z, z, z, z, z, None) == 0      # N = 0 is legal
     assert lib.qr_dense_forward(C.byref(cam), 16, 0, C.c_float(-1.0), p, p, p, p, p, p, p, None) == -1
     assert lib.qr_backward(C.byref(cam), 0, 16, 10, p, p, p, p, p, None, 0, None) == -1
+    # top-K comparator: K = 0 domain error, K > QR_TOPK_MAX_K unsupported, t_min < 0, NULL, small workspace
+    tk = lambda K, D, t, out, wsb: lib.qr_topk_forward(C.byref(cam), K, D, 0, C.c_float(t), p, p, p, p, p, out, p, p, p, p, p, wsb, None)
+    assert tk(0, 16, 1e-4, p, 1 << 20) == -1
+    assert tk(65, 16, 1e-4, p, 1 << 20) == -3
+    assert tk(8, 16, -1.0, p, 1 << 20) == -1
+    assert tk(8, 16, 1e-4, z, 1 << 20) == -2
+    assert lib.qr_topk_workspace_bytes(C.byref(cam), 8, 16) > 0 and lib.qr_topk_workspace_bytes(C.byref(cam), 0, 16) == 0
     assert lib.qr_bin_sort(C.byref(cam), 10, 1 << 31, p, p, p, p, p, p, 1 << 20, None) == -5
     m = C.c_int64(-1)
     assert lib.qr_bin_count(0, z, z, C.byref(m), z, 0, None) == 0 and m.value == 0

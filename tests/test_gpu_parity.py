@@ -450,6 +450,69 @@ def test_midsize_every_row_many_units_per_cta(qr, orc, D):
 # ------------------------------------------------------------------------------------------------
 # argument errors are status codes, not crashes
 # ------------------------------------------------------------------------------------------------
+# ------------------------------------------------------------------------------------------------
+# qr_topk_forward (NEXT-1; reading R17)
+# ------------------------------------------------------------------------------------------------
+TOPK_CASES = [
+    ("cfg1", dict(), 8, 1e-4),                                   # FFMA-free plain path (D = 16)
+    ("cfg1", dict(W=70, H=50, D=3), 40, 0.0),                    # ragged image, odd D, whole-list weights
+    ("cfg2", dict(N=20000, W=128, H=96), 5, 1e-4),
+    ("cfg3", dict(N=60000, W=160, H=112, D=512), 40, 1e-4),      # tcgen05 blend, R = 5,120 records per full half tile
+    ("cfg3", dict(N=60000, W=100, H=72, D=256), 10, 1e-4),       # tcgen05 blend, ragged image
+    ("cfg3", dict(N=60000, W=96, H=64, D=128), 64, 1e-4),        # K = QR_TOPK_MAX_K: half tiles over the prep's capacity
+    ("cfg1", dict(D=64), 1, 1e-4),                               # K = 1
+]
+
+
+@pytest.mark.parametrize("name,kw,K,t_min", TOPK_CASES)
+def test_topk_forward_stage_isolated(qr, orc, name, kw, K, t_min):
+    sc = make_scene(name, seed=21, **kw)
+    proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
+    lists = orc.pixel_lists(sc.cam, proj)
+    t = orc.topk(lists, K, sc.features, t_min=t_min)
+    out = qr.qr_topk_forward(sc.cam, K, P.to_dev(proj.mean2d), P.to_dev(proj.conic_opac), P.to_dev(isect.view(np.int32)),
+                             P.to_dev(rng), P.to_dev(sc.features), t_min)
+    stats = P.compare_topk(out, t, lists, K, sc.D)
+    assert stats["exempt"] < 0.02 * stats["pixels"] + 5, stats
+    print(name, kw, K, stats)
+
+
+def test_topk_fp16_and_backward_accepts_its_records(qr, orc):
+    """fp16 features through the plain blend; qr_backward on top-K's records equals the oracle's backward of them."""
+    sc = make_scene("cfg4", seed=22, N=60000, W=96, H=64, D=128, pose=1, backward=True)
+    proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
+    lists = orc.pixel_lists(sc.cam, proj)
+    K = 12
+    t = orc.topk(lists, K, sc.features, t_min=1e-4)
+    args = (P.to_dev(proj.mean2d), P.to_dev(proj.conic_opac), P.to_dev(isect.view(np.int32)), P.to_dev(rng))
+    out = qr.qr_topk_forward(sc.cam, K, *args, P.to_dev(sc.features), 1e-4)
+    P.compare_topk(out, t, lists, K, sc.D, f16=True)
+    H, W = sc.cam.height, sc.cam.width
+    dF = qr.qr_backward(sc.cam, sc.N, P.to_dev(t.sel_idx.reshape(H, W, K)), P.to_dev(t.sel_w.reshape(H, W, K).astype(np.float32)),
+                        P.to_dev(t.n_sel.reshape(H, W)), P.to_dev(sc.dL_dmap))
+    ref = orc.backward(t.sel_idx, t.sel_w, t.n_sel, sc.dL_dmap, sc.N)
+    P.compare_backward_rows(dF.cpu().numpy(), ref, "top-K records")
+
+
+def test_topk_full_size_config3_sampled(qr, orc):
+    """BASELINE config 3 at full size, K = 40: selection on every pixel, features on sampled pixels."""
+    sc = make_scene("cfg3", seed=0)
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    out = qr.pipeline.topk_forward(sc.cam, fe, g.features, sc.K, 1e-4)
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    lists = orc.pixel_lists(sc.cam, proj)
+    t = orc.topk(lists, sc.K, None, t_min=1e-4)
+    stats = P.compare_topk(out, t, lists, sc.K, sc.D)
+    rng = np.random.default_rng(5)
+    pix = np.sort(rng.choice(sc.cam.width * sc.cam.height, 1500, replace=False))
+    tp = orc.topk(lists, sc.K, sc.features, t_min=1e-4, pixels=pix)
+    sub = type("L", (), dict(borderline=lists.borderline))()
+    s2 = P.compare_topk(out, tp, sub, sc.K, sc.D, pixels=pix)
+    assert stats["exempt"] < 0.02 * stats["pixels"], stats
+    print("top-K cfg3 full size:", stats, "sampled:", s2)
+
+
 def test_error_codes(qr):
     sc = make_scene("cfg1", seed=0, N=100)
     g = P.upload(sc)
