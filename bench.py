@@ -3,17 +3,22 @@
 
 A step = one pass of the whole Q-Render hot path over one synthetic frame, through the C ABI:
     qr_preprocess -> qr_bin_sort -> qr_forward -> qr_backward -> qr_backward_clear
-(qr_bin_count sizes the intersection lists once, before the timed region; the timed steps pass that size + 25 % as
-the lists' capacity, so no step synchronises with the host, and the count found is verified afterwards)
-(dL/dF is zeroed once before the loop; qr_backward_clear re-zeroes exactly the rows the step's qr_backward touched,
-which is what a training loop does after consuming the gradient, instead of a 1.02 GB memset per step)
-`value` = Mpix/s of that step with inputs resident in HBM (CUDA events, max over ranks).  The dense comparator
-(qr_dense_forward) is timed beside it in the same run and reported under "dense"; it is not part
-of the step.  `roofline` describes the dominant kernel (the longer of qr_forward / qr_backward), timed with CUDA
-events around each call inside the timed steps.  `e2e` repeats the step with HOST (pinned) inputs and outputs, the
-copies inside the timed region.  `cpu_baseline` times the CPU oracle on one full frame on the box's host cores.
+Two things a naive loop pays every step are NOT in the step, and `config.step` says so next to the number:
+  * qr_bin_count and its device->host read of M: the lists are sized once, by the untimed first step; the timed steps pass
+    that size + 25 % as the lists' capacity, nothing synchronises with the host, and the count found is verified afterwards;
+  * the zero fill of the whole [N, D] dL_dfeat table (1.02 GB): it is zeroed once before the loop and qr_backward_clear
+    re-zeroes exactly the rows the step's qr_backward touched, which is what a training loop does after consuming the
+    gradient.  `kernels_ms.zero_fill_ms` reports what the whole-table fill would cost.
+`value` = Mpix/s of that step with inputs resident in HBM (CUDA events, max over ranks).  The comparators -- dense V-Render
+(qr_dense_forward) and top-K (qr_topk_forward, 8(f) NEXT-1) -- are timed beside it in the same run; they
+are not part of the step.  `roofline` describes the dominant call (the longer of qr_forward / qr_backward), timed with CUDA
+events around each call inside the timed steps; `traffic` is the DRAM traffic of an ncu capture of exactly this workload,
+D and K if profiles/traffic.json has one, else null.  `gpu_launches` is counted by the library.  `e2e` repeats the step
+with HOST (pinned) inputs and outputs, the copies inside the timed region.  `cpu_baseline` times the CPU oracle on one full
+frame on the box's host cores (plus its V-Render / top-K and a 1-thread figure on configs 1 and 2).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg3] [--D d] [--K k] [--pose j]
+    python bench.py --sweep cfg4|cfg5 [--out file.json] [--no-parity]     every point of BASELINE.json configs[3] / [4]
 N > 1: launched by torch.distributed.run, one rank per GPU, independent replicas of the same frame (weak scaling,
 no data-path collective: SURVEY 8(e)); rank 0 prints the one JSON line.
 """
@@ -160,9 +165,177 @@ def workload_config(sc, name):
                                                "SMALLER than L2: figures at this size are L2-resident, not HBM, numbers")}
 
 
+
+
 # ----------------------------------------------------------------------------------------------------------------
 # CUDA arm
 # ----------------------------------------------------------------------------------------------------------------
+def _traffic(workload, D, K):
+    """dram__bytes_read.sum + dram__bytes_write.sum per call from the committed ncu --set full capture of exactly this
+    (workload, D, K) -- profiles/traffic.json names the capture -- else None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return {}
+    with open(p) as f:
+        return json.load(f).get(f"{workload}:D{D}:K{K}", {})
+
+
+class Frame:
+    """One scene resident on the device and the step over it (all through the C ABI binding)."""
+
+    def __init__(self, sc, dev, qr):
+        import torch
+        self.torch, self.qr, self.pl = torch, qr, qr.pipeline
+        self.sc, self.dev = sc, dev
+        self.cam, self.K, self.D, self.N = sc.cam, sc.K, sc.D, sc.N
+        self.host = {k: torch.from_numpy(np.ascontiguousarray(getattr(sc, k))).pin_memory()
+                     for k in ("means", "scales", "quats", "opac", "features", "dL_dmap")}
+        self.d = {k: v.to(dev, non_blocking=True) for k, v in self.host.items()}
+        self.dF = torch.zeros((self.N, self.D), dtype=torch.float32, device=dev)   # zeroed ONCE; each step re-zeroes what it touched
+        self.bws = qr.qr_backward_workspace(self.cam, self.K, self.D, dev)
+        self.fwd_out = None
+        self.capacity = None          # of the intersection lists: sized by the first (untimed) step's qr_bin_count
+        self.found = None
+        self.fe = None
+
+    def reset(self, cam=None, K=None):
+        """Another camera pose and / or K over the same Gaussians (config 4's sweep)."""
+        if cam is not None:
+            self.cam = cam
+            self.capacity = None
+        if K is not None and K != self.K:
+            self.K = K
+            self.fwd_out = None
+        self.bws = self.qr.qr_backward_workspace(self.cam, self.K, self.D, self.dev)
+
+    def step(self, timers=None):
+        t, pl, d = self.torch, self.pl, self.d
+        fe = pl.frontend(self.cam, d["means"], d["scales"], d["quats"], d["opac"], self.capacity)
+        if self.capacity is None:
+            self.capacity = int(fe.M * 1.25) + 1024
+        else:
+            self.found = fe.found            # device scalar; only the latest is kept
+        if timers is not None:
+            ev = [t.cuda.Event(enable_timing=True) for _ in range(4)]
+            ev[0].record()
+        self.fwd_out = pl.forward(self.cam, fe, d["features"], self.K, self.fwd_out)
+        if timers is not None:
+            ev[1].record()
+        ws = None if self.fwd_out.has_lists else self.bws
+        pl.backward(self.cam, self.N, self.fwd_out, d["dL_dmap"], self.dF, ws)
+        if timers is not None:
+            ev[2].record()
+        # dL_dfeat would be consumed here (the 3D network's backward); then the rows this step touched are re-zeroed,
+        # so that the table is all-zero again for the next step without a 1.02 GB memset
+        pl.backward_clear(self.cam, self.N, self.fwd_out, self.dF, ws)
+        if timers is not None:
+            ev[3].record()
+            timers.append(ev)
+        self.fe = fe
+        return fe
+
+    def timed(self, steps, warmup, barrier, world=1, dist=None):
+        t = self.torch
+        for _ in range(max(warmup, 3)):
+            self.step()
+        barrier()
+        timers = []
+        s0, s1 = t.cuda.Event(enable_timing=True), t.cuda.Event(enable_timing=True)
+        n0 = self.qr.binding.qr_launch_count()
+        barrier()
+        s0.record()
+        for _ in range(steps):
+            self.step(timers)
+        s1.record()
+        barrier()
+        launches = self.qr.binding.qr_launch_count() - n0
+        total_ms = s0.elapsed_time(s1)
+        found = int(self.found.item()) if self.found is not None else self.fe.M
+        if found > self.capacity:
+            raise RuntimeError(f"intersection lists overflowed their capacity ({found} > {self.capacity}): invalid run")
+        tt = t.tensor([total_ms], dtype=t.float64, device=self.dev)
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        mean = lambda i, j: statistics.mean(e[i].elapsed_time(e[j]) for e in timers)
+        return {"ms_step": float(tt.item()) / steps, "fwd_ms": mean(0, 1), "bwd_ms": mean(1, 2), "clear_ms": mean(2, 3),
+                "launches": int(launches), "M_found": found}
+
+    def time_call(self, fn, n=5, warm=2):
+        t = self.torch
+        for _ in range(warm):
+            fn()
+        t.cuda.synchronize()
+        a, b = t.cuda.Event(enable_timing=True), t.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(n):
+            fn()
+        b.record()
+        t.cuda.synchronize()
+        return a.elapsed_time(b) / n
+
+    def counts(self):
+        """Workload counts for the byte model and SURVEY 8(d)'s work counters (statistics only, outside every timed region)."""
+        t, K = self.torch, self.K
+        fo = self.fwd_out
+        npix = self.cam.width * self.cam.height
+        n_vis = int((self.fe.proj.tiles_touched != 0).sum().item())
+        used = t.arange(K, device=self.dev)[None, None, :] < fo.n_sel[..., None]      # slots >= n_sel are not written
+        S = int(t.unique(fo.sel_idx[used]).numel())
+        hist = t.bincount(fo.n_sel.reshape(-1).to(t.int64), minlength=K + 1).cpu().tolist()
+        out = {"N_visible": n_vis, "n_sel_mean": float(fo.n_sel.float().mean().item()), "n_sel_max": int(fo.n_sel.max().item()),
+               "S_distinct_selected": S, "zero_selection_pixels": int(hist[0]), "selection_record_bytes": npix * (8 * K + 4),
+               "n_sel_histogram": hist}
+        if fo.has_lists:
+            st = self.qr.binding.qr_forward_stats(self.cam, K, fo)
+            nh = 2 * self.qr.binding.qr_num_tiles(self.cam)
+            out.update({"sum_U_half_tiles": st["sum_U_half_tiles"], "U_half_tile_mean": st["sum_U_half_tiles"] / nh,
+                        "half_tiles_U_gt_64": st["half_tiles_U_gt_64"],
+                        "walk_list_entries_consumed": st["list_entries_consumed"],
+                        "walk_entry_pixel_evaluations": st["entry_pixel_evaluations"],
+                        "walk_evaluations_per_pixel": st["entry_pixel_evaluations"] / npix})
+        return out
+
+
+def cpu_baseline_record(sc, workload):
+    """The oracle, as it stands, on the box's host cores: one full frame of the workload (all threads), the oracle's
+    own work counts for the byte model (N-bar = mean walk length), its V-Render and top-K on the same lists, and a
+    1-thread figure on configs 1 and 2 (SURVEY 8(d) "Oracle timing beside it")."""
+    from oracle import qr_oracle as orc
+    from qr_inputs import make_scene
+    npix = sc.cam.width * sc.cam.height
+    t0 = time.perf_counter()
+    q = oracle_frame(orc, sc)
+    sec = time.perf_counter() - t0
+    cores = orc.num_threads()
+    rec = {"value": npix / sec / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": sec,
+           "sample": f"1 full frame of {workload} ({npix} px; O1 projection, O2b lists, O4 Algorithm 1 with D={sc.D} "
+                     f"features, O5 backward of the selected rows)",
+           "N_bar_mean_walk_length": float(q.n_walked.mean()), "n_sel_mean": float(q.n_sel.mean())}
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    lists = orc.pixel_lists(sc.cam, proj)
+    rec["mean_list_length"] = float(len(lists.gid)) / npix
+    t0 = time.perf_counter()
+    v = orc.vrender(lists, sc.features, t_min=1e-4)
+    rec["vrender_seconds"] = time.perf_counter() - t0
+    rec["dense_walk_mean"] = float(v.n_blended.mean())
+    if sc.K <= 64:
+        t0 = time.perf_counter()
+        orc.topk(lists, sc.K, sc.features, t_min=1e-4)
+        rec["topk_seconds"] = time.perf_counter() - t0
+    one = {}
+    orc.set_num_threads(1)
+    try:
+        for name in ("cfg1", "cfg2"):
+            s1 = make_scene(name, seed=0)
+            t0 = time.perf_counter()
+            oracle_frame(orc, s1)
+            one[name] = {"seconds": time.perf_counter() - t0, "mpix_s": s1.cam.width * s1.cam.height / (time.perf_counter() - t0) / 1e6}
+    finally:
+        orc.set_num_threads(cores)
+    rec["one_thread"] = one
+    return rec
+
+
 def run_cuda(args):
     import torch
     import torch.distributed as dist
@@ -176,160 +349,107 @@ def run_cuda(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     import paper_2512_20927_b200 as qr
-    from paper_2512_20927_b200 import pipeline as pl
     qr.binding.load()
-
-    sc = scene_for(args)
-    cam, K, D, N = sc.cam, sc.K, sc.D, sc.N
-    H, W = cam.height, cam.width
-    npix = H * W
+    pl = qr.pipeline
     dev = torch.device("cuda", local)
-    host = {k: torch.from_numpy(np.ascontiguousarray(getattr(sc, k))).pin_memory()
-            for k in ("means", "scales", "quats", "opac", "features", "dL_dmap")}
-    d = {k: v.to(dev, non_blocking=True) for k, v in host.items()}
-    dF = torch.zeros((N, D), dtype=torch.float32, device=dev)      # zeroed ONCE; every step re-zeroes the rows it touched
-    bws = qr.qr_backward_workspace(cam, K, D, dev)
-    fwd_out = None
-    ev = lambda: torch.cuda.Event(enable_timing=True)
-    launches = {"n": 0}
-
-    # Front end: the first (untimed) step sizes the intersection lists exactly with qr_bin_count (one device->host
-    # read); every later step passes 1.25 x that count as the capacity of the lists, so nothing in the timed region
-    # synchronises with the host.  The count found on the device is checked against the capacity after the loop.
-    state = {"capacity": None, "found": []}
-
-    def step(timers=None):
-        nonlocal fwd_out
-        fe = pl.frontend(cam, d["means"], d["scales"], d["quats"], d["opac"], state["capacity"])
-        if state["capacity"] is None:
-            state["capacity"] = int(fe.M * 1.25) + 1024
-        else:
-            state["found"] = [fe.found]          # device scalar; only the latest is kept (holding all would pin every workspace)
-        if timers is not None:
-            e0, e1, e2, e3 = ev(), ev(), ev(), ev()
-            e0.record()
-        fwd_out = pl.forward(cam, fe, d["features"], K, fwd_out)
-        if timers is not None:
-            e1.record()
-        pl.backward(cam, N, fwd_out, d["dL_dmap"], dF, None if fwd_out.has_lists else bws)
-        if timers is not None:
-            e2.record()
-        # dL_dfeat would be consumed here (the 3D network's backward); then the rows this step touched are re-zeroed,
-        # so that the table is all-zero again for the next step without a 1.02 GB memset
-        pl.backward_clear(cam, N, fwd_out, dF, None if fwd_out.has_lists else bws)
-        if timers is not None:
-            e3.record()
-            timers.append((e0, e1, e2, e3))
-        # preprocess 1, bin_sort 5 (count, scan, scatter, 2 bucket sorts), forward 2 (walk, blend),
-        # backward 3 (prep, tcgen05 contraction, FFMA kernel for the half tiles the prep left to it), clear 1
-        launches["n"] += 1 + 5 + 2 + 3 + 1
-        return fe
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        fe = step()
-    barrier()
+    if args.sweep:
+        rc = run_sweep(args, qr, dev, barrier) if rank == 0 else 0
+        if world > 1:
+            dist.destroy_process_group()
+        return rc
+
+    sc = scene_for(args)
+    fr = Frame(sc, dev, qr)
+    cam, K, D, N = fr.cam, fr.K, fr.D, fr.N
+    H, W = cam.height, cam.width
+    npix = H * W
     sampler = ClockSampler(local)
+    for _ in range(max(args.warmup, 3)):
+        fr.step()
+    barrier()
     if rank == 0:
         sampler.start()
-    launches["n"] = 0
-    timers = []
-    s0, s1 = ev(), ev()
-    barrier()
-    s0.record()
-    for _ in range(args.steps):
-        fe = step(timers)
-    s1.record()
-    barrier()
-    total_ms = s0.elapsed_time(s1)
-    found = [int(f.item()) for f in state["found"]]
-    if found and max(found) > state["capacity"]:
-        raise RuntimeError(f"intersection lists overflowed their capacity ({max(found)} > {state['capacity']}): invalid run")
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
-    ms_step = total_ms / args.steps
+    r = fr.timed(args.steps, args.warmup, barrier, world, dist)
+    ms_step, fwd_ms, bwd_ms, zero_ms = r["ms_step"], r["fwd_ms"], r["bwd_ms"], r["clear_ms"]
     value = world * npix / (ms_step * 1e-3) / 1e6
-    fwd_ms = statistics.mean(a.elapsed_time(b) for a, b, _, _ in timers)
-    bwd_ms = statistics.mean(b.elapsed_time(c) for _, b, c, _ in timers)
-    zero_ms = statistics.mean(c.elapsed_time(e) for _, _, c, e in timers)
+    fe = fr.fe
 
-    # dense comparator, same frame, same front end (not part of the step)
+    # comparators on the same frame and front end (not part of the step): dense V-Render (Eq. 1) and top-K
     dense_map = torch.empty((H, W, D), dtype=torch.float32, device=dev)
     dense_T = torch.empty((H, W), dtype=torch.float32, device=dev)
-    for _ in range(2):
-        pl.dense_forward(cam, fe, d["features"], 1e-4, dense_map, dense_T)
-    torch.cuda.synchronize()
-    a, b = ev(), ev()
-    nd = 5
-    a.record()
-    for _ in range(nd):
-        pl.dense_forward(cam, fe, d["features"], 1e-4, dense_map, dense_T)
-    b.record()
-    torch.cuda.synchronize()
-    dense_ms = a.elapsed_time(b) / nd
+    dense_ms = fr.time_call(lambda: pl.dense_forward(cam, fe, fr.d["features"], 1e-4, dense_map, dense_T))
     del dense_map
-    # The timed region is ~15 ms at 20 steps, shorter than nvidia-smi's 100 ms sampling period: keep the SAME step
+    topk_ms = None
+    if K <= 64:
+        tk = {"out": None}
+
+        def topk_call():
+            tk["out"] = pl.topk_forward(cam, fe, fr.d["features"], K, 1e-4, tk["out"])
+        topk_ms = fr.time_call(topk_call)
+        topk_nsel = float(tk["out"].n_sel.float().mean().item())
+        del tk
+    # zero fill of the whole dL_dfeat table: what a caller without qr_backward_clear pays per step (reported, not in the step)
+    fill_ms = fr.time_call(lambda: fr.dF.zero_())
+    # The timed region is ~12 ms at 20 steps, shorter than nvidia-smi's 100 ms sampling period: keep the SAME step
     # running (untimed, not counted anywhere) for ~0.4 s so that the clock / throttle samples are taken under this load.
     if rank == 0:
         hold_until = time.perf_counter() + 0.4
-        n_before = launches["n"]
         while time.perf_counter() < hold_until:
             for _ in range(20):
-                step()
+                fr.step()
             torch.cuda.synchronize()
-        launches["n"] = n_before
     clocks = sampler.stop() if rank == 0 else None
     if clocks is not None:
-        clocks["note"] = "sampled every 100 ms over the timed steps, the dense comparator and ~0.4 s of the same step kept running"
+        clocks["note"] = "sampled every 100 ms over the timed steps, the comparators and ~0.4 s of the same step kept running"
 
-    # workload counts for the byte model (statistics only; torch ops outside every timed region)
-    n_vis = int((fe.proj.tiles_touched != 0).sum().item())
-    used = torch.arange(K, device=dev)[None, None, :] < fwd_out.n_sel[..., None]   # slots >= n_sel are not written
-    sel = fwd_out.sel_idx[used]
-    S = int(torch.unique(sel).numel())
-    nsel_mean = float(fwd_out.n_sel.float().mean().item())
+    counts = fr.counts()
+    S, n_vis, M_found = counts["S_distinct_selected"], counts["N_visible"], r["M_found"]
     esz = 2 if sc.feat_dtype == "f16" else 4
-    M_found = found[-1] if found else fe.M
     fwd_bytes = M_found * 4 + n_vis * 32 + S * D * esz + npix * D * 4 + npix * 4
     rec_bytes = npix * (8 * K + 4)
     bwd_bytes = npix * D * 4 + S * D * 4 + rec_bytes
     peak, peak_src = _peaks()
-    dom = "qr_forward" if fwd_ms >= bwd_ms else "qr_backward"
-    dom_bytes, dom_ms = (fwd_bytes, fwd_ms) if dom == "qr_forward" else (bwd_bytes, bwd_ms)
+    traffic = _traffic(args.workload, D, K)
 
-    def roof(nbytes, ms, kernel, traffic=None):
+    def roof(nbytes, ms, kernel):
         ach = nbytes / (ms * 1e-3) / 1e9
+        tr = traffic.get(kernel)
         return {"kernel": kernel, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "peak_source": peak_src, "frac_of_nominal_8TBs": ach / NOMINAL_HBM_GBS, "algorithmic_bytes": nbytes,
-                "ms_per_launch": ms, "traffic": traffic}
+                "ms_per_launch": ms, "traffic": tr, "traffic_source": traffic.get("source") if tr else None,
+                "traffic_over_algorithmic": (tr / nbytes) if tr else None}
+
+    dom = "qr_forward" if fwd_ms >= bwd_ms else "qr_backward"
+    dom_bytes, dom_ms = (fwd_bytes, fwd_ms) if dom == "qr_forward" else (bwd_bytes, bwd_ms)
 
     # ---- e2e: host buffers in, host buffers out, copies inside the timed region ----
     e2e = None
     if not args.no_e2e:
         out_host = torch.empty((H, W, D), dtype=torch.float32).pin_memory()
         dF_host = torch.empty((N, D), dtype=torch.float32).pin_memory()
-        dd = {k: torch.empty_like(v) for k, v in d.items()}
+        dd = {k: torch.empty_like(v) for k, v in fr.d.items()}
 
         def e2e_step():
             for k in dd:
-                dd[k].copy_(host[k], non_blocking=True)
-            fe2 = pl.frontend(cam, dd["means"], dd["scales"], dd["quats"], dd["opac"], state["capacity"])
-            o = pl.forward(cam, fe2, dd["features"], K, fwd_out)
-            pl.backward(cam, N, o, dd["dL_dmap"], dF, None if o.has_lists else bws)
+                dd[k].copy_(fr.host[k], non_blocking=True)
+            fe2 = pl.frontend(cam, dd["means"], dd["scales"], dd["quats"], dd["opac"], fr.capacity)
+            o = pl.forward(cam, fe2, dd["features"], K, fr.fwd_out)
+            ws = None if o.has_lists else fr.bws
+            pl.backward(cam, N, o, dd["dL_dmap"], fr.dF, ws)
             out_host.copy_(o.out_map, non_blocking=True)
-            dF_host.copy_(dF, non_blocking=True)
-            pl.backward_clear(cam, N, o, dF, None if o.has_lists else bws)
+            dF_host.copy_(fr.dF, non_blocking=True)
+            pl.backward_clear(cam, N, o, fr.dF, ws)
 
         e2e_step()
         barrier()
         ne = max(2, min(args.steps, 4))
-        a, b = ev(), ev()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
         for _ in range(ne):
             e2e_step()
@@ -339,46 +459,152 @@ def run_cuda(args):
         if world > 1:
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e_ms = float(t.item()) / ne
-        h2d = sum(v.numel() * v.element_size() for v in host.values())
+        h2d = sum(v.numel() * v.element_size() for v in fr.host.values())
         d2h = out_host.numel() * 4 + dF_host.numel() * 4
         e2e = {"value": world * npix / (e_ms * 1e-3) / 1e6, "unit": UNIT, "ms_per_step": e_ms, "steps": ne,
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-               "note": "inputs (Gaussians, features, dL_dmap) from pinned host memory; out_map and dL_dfeat read back"}
+               "note": "inputs (Gaussians, features, dL_dmap) from pinned host memory; out_map and the whole dL_dfeat table "
+                       "read back: PCIe-bound by construction"}
         del out_host, dF_host, dd
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        ts, cores = time_oracle(sc, 1, 0)
-        cpu_baseline = {"value": npix / ts[0] / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle",
-                        "seconds": ts[0],
-                        "sample": f"1 full frame of {args.workload} ({npix} px; O1 projection, O2b lists, O4 Algorithm 1 "
-                                  f"with D={D} features, O5 backward of the selected rows)"}
+        cpu_baseline = cpu_baseline_record(sc, args.workload)
 
     if rank == 0:
+        cfg = workload_config(sc, args.workload)
+        cfg["step"] = ("qr_preprocess, qr_bin_sort (list capacity from an untimed first step: qr_bin_count and its host read "
+                       "are NOT in the step), qr_forward, qr_backward, qr_backward_clear (re-zeroes the touched rows; the "
+                       "zero fill of the whole dL_dfeat table is NOT in the step, see zero_fill_ms)")
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(sc, args.workload),
-                "clocks": clocks, "e2e": e2e, "gpu_launches": launches["n"],
-                "roofline": roof(dom_bytes, dom_ms, dom, TRAFFIC.get(dom)),
-                "roofline_fwd": roof(fwd_bytes, fwd_ms, "qr_forward", TRAFFIC.get("qr_forward")),
-                "roofline_bwd": roof(bwd_bytes, bwd_ms, "qr_backward", TRAFFIC.get("qr_backward")),
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
+                "clocks": clocks, "e2e": e2e, "gpu_launches": r["launches"],
+                "gpu_launches_note": "counted by the library at every kernel launch it issues (qr_launch_count) over the timed steps",
+                "roofline": roof(dom_bytes, dom_ms, dom),
+                "roofline_fwd": roof(fwd_bytes, fwd_ms, "qr_forward"),
+                "roofline_bwd": roof(bwd_bytes, bwd_ms, "qr_backward"),
                 "cpu_baseline": cpu_baseline,
                 "kernels_ms": {"qr_forward": fwd_ms, "qr_backward": bwd_ms, "qr_backward_clear": zero_ms,
-                               "frontend_and_rest": ms_step - fwd_ms - bwd_ms - zero_ms},
+                               "frontend_and_rest": ms_step - fwd_ms - bwd_ms - zero_ms, "zero_fill_ms": fill_ms},
                 "mpix_s": {"fwd_kernel": npix / fwd_ms / 1e3, "fwd_bwd_kernels": npix / (fwd_ms + bwd_ms) / 1e3,
-                           "dense_fwd_kernel": npix / dense_ms / 1e3},
-                "dense": {"ms": dense_ms, "speedup_qr_forward_over_dense": dense_ms / fwd_ms, "t_min": 1e-4},
-                "workload_counts": {"M": M_found, "M_capacity": state["capacity"], "N_visible": n_vis, "n_sel_mean": nsel_mean, "S_distinct_selected": S,
-                                    "selection_record_bytes": rec_bytes}}
+                           "dense_fwd_kernel": npix / dense_ms / 1e3,
+                           "topk_fwd_kernel": (npix / topk_ms / 1e3) if topk_ms else None},
+                "dense": {"ms": dense_ms, "speedup_qr_forward_over_dense": dense_ms / fwd_ms, "t_min": 1e-4,
+                          "note": "render_kernel<1>: FFMA formulation without the tensor-core blend (DESIGN.md 5.5); the ratio "
+                                  "compares a tuned kernel with an untuned one"},
+                "topk": ({"ms": topk_ms, "K": K, "n_sel_mean": topk_nsel, "qr_forward_over_topk": topk_ms / fwd_ms,
+                          "note": "same tcgen05 blend as Q-Render; selection by a per-pixel heap (O(N log K), PAPER.md:187)"}
+                         if topk_ms else None),
+                "workload_counts": dict(counts, M=M_found, M_capacity=fr.capacity)}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture named in profiles/ (None
-# until a capture of the current kernels is committed).
-TRAFFIC = {"qr_forward": 825.3e6, "qr_backward": 821.4e6}   # profiles/r1_e_full_metrics.csv (walk + blend; prep + mma)
+def _parity_counts(orc, lists, K, fwd_out):
+    """Selection parity of a frame against the oracle on EVERY pixel (indices bit-exact off the exemption set of
+    DESIGN.md reading R15); returns counts, never raises: the sweep records them next to the timings."""
+    q = orc.qrender(lists, K, None)
+    sel = fwd_out.sel_idx.cpu().numpy().reshape(-1, K)
+    n = fwd_out.n_sel.cpu().numpy().reshape(-1)
+    used = np.arange(K)[None, :] < q.n_sel[:, None]
+    same = (n == q.n_sel) & ((sel == q.sel_idx) | ~used).all(axis=1)
+    ex_m = q.margin <= 1e-6
+    ex_b = lists.bl_first <= q.n_walked.astype(np.int64)
+    ex = ex_m | ex_b
+    return {"pixels": int(same.size), "exempt_margin": int(ex_m.sum()), "exempt_borderline": int((ex_b & ~ex_m).sum()),
+            "mismatch_exempt": int(((~same) & ex).sum()), "mismatch_nonexempt": int(((~same) & ~ex).sum())}
+
+
+def run_sweep(args, qr, dev, barrier):
+    """BASELINE.json configs[3] (cfg4: K in {4, 8, 16, 32} x 8 camera poses, fp16 features) or configs[4] (cfg5: D in
+    {3, 16, 64, 128, 256, 512}, Q-Render vs dense): every point timed like the headline step, with its clocks, work
+    counts and (unless --no-parity) its selection parity against the oracle on every pixel.  Writes --out (JSON)."""
+    import torch
+    from qr_inputs import make_scene
+    from qr_inputs.scenes import pose_on_circle
+    pl = qr.pipeline
+    orc = None
+    if not args.no_parity:
+        from oracle import qr_oracle as orc
+    points = []
+    steps = max(3, min(args.steps, 10))
+    sampler = ClockSampler(dev.index or 0)
+
+    def measure(fr, tag, lists):
+        sampler.lines = []
+        sampler.start()
+        r = fr.timed(steps, 3, barrier)
+        cam, K, D = fr.cam, fr.K, fr.D
+        npix = cam.width * cam.height
+        fe = fr.fe
+        rec = dict(tag, ms_step=r["ms_step"], qr_forward_ms=r["fwd_ms"], qr_backward_ms=r["bwd_ms"], clear_ms=r["clear_ms"],
+                   frontend_ms=r["ms_step"] - r["fwd_ms"] - r["bwd_ms"] - r["clear_ms"], gpu_launches=r["launches"], steps=steps,
+                   mpix_s_step=npix / r["ms_step"] / 1e3, M=r["M_found"])
+        if args.sweep == "cfg5":
+            dm = torch.empty((cam.height, cam.width, D), dtype=torch.float32, device=dev)
+            dT = torch.empty((cam.height, cam.width), dtype=torch.float32, device=dev)
+            rec["dense_ms"] = fr.time_call(lambda: pl.dense_forward(cam, fe, fr.d["features"], 1e-4, dm, dT), n=3, warm=1)
+            rec["dense_over_qr_forward"] = rec["dense_ms"] / r["fwd_ms"]
+            del dm
+        if K <= 64:
+            tk = {"out": None}
+
+            def topk_call():
+                tk["out"] = pl.topk_forward(cam, fe, fr.d["features"], K, 1e-4, tk["out"])
+            rec["topk_ms"] = fr.time_call(topk_call, n=3, warm=1)
+            del tk
+        hold = time.perf_counter() + 0.25           # keep the step running so that nvidia-smi samples it under load
+        while time.perf_counter() < hold:
+            for _ in range(10):
+                fr.step()
+            torch.cuda.synchronize()
+        rec["clocks"] = sampler.stop()
+        c = fr.counts()
+        c.pop("n_sel_histogram", None)
+        rec["counts"] = c
+        if lists is not None:
+            rec["parity"] = _parity_counts(orc, lists, K, fr.fwd_out)
+        print(json.dumps(rec), file=sys.stderr, flush=True)
+        points.append(rec)
+
+    if args.sweep == "cfg5":
+        for D in (3, 16, 64, 128, 256, 512):
+            sc = make_scene("cfg5", seed=0, D=D)
+            fr = Frame(sc, dev, qr)
+            lists = None
+            if orc is not None:
+                proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+                lists = orc.pixel_lists(sc.cam, proj)
+            measure(fr, {"workload": "cfg5", "D": D, "K": sc.K, "dtype": sc.feat_dtype}, lists)
+            del fr, sc
+            torch.cuda.empty_cache()
+    elif args.sweep == "cfg4":
+        sc = make_scene("cfg4", seed=0, pose=0)
+        fr = Frame(sc, dev, qr)
+        for pose in range(8):
+            cam = sc.cam.copy()
+            cam.world_to_cam = pose_on_circle(pose, 8)
+            lists = None
+            if orc is not None:
+                proj = orc.project(cam, sc.means, sc.scales, sc.quats, sc.opac)
+                lists = orc.pixel_lists(cam, proj)
+            for K in (4, 8, 16, 32):
+                fr.reset(cam=cam, K=K)
+                measure(fr, {"workload": "cfg4", "pose": pose, "K": K, "D": sc.D, "dtype": sc.feat_dtype}, lists)
+    else:
+        raise SystemExit(f"unknown sweep {args.sweep}")
+    out = {"sweep": args.sweep, "command": "python bench.py --sweep " + args.sweep + (" --no-parity" if args.no_parity else ""),
+           "peak_hbm_gbs": _peaks()[0], "points": points}
+    path = args.out or os.path.join(ROOT, "gpurun_out", f"sweep_{args.sweep}.json")
+    os.makedirs(os.path.dirname(path), exist_ok=True)
+    with open(path, "w") as f:
+        json.dump(out, f, indent=1)
+    bad = sum(p.get("parity", {}).get("mismatch_nonexempt", 0) for p in points)
+    print(json.dumps({"sweep": args.sweep, "points": len(points), "written": path, "mismatch_nonexempt_total": bad}))
+    return 0 if bad == 0 else 1
 
 
 def main():
@@ -393,6 +619,10 @@ def main():
     ap.add_argument("--pose", type=int, default=None, help="camera pose 0..7 of config 4's circle")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--sweep", default=None, choices=["cfg4", "cfg5"],
+                    help="run every point of BASELINE.json's config 4 (4 K x 8 poses) or config 5 (6 D) and write a JSON file")
+    ap.add_argument("--out", default=None, help="where --sweep writes (default gpurun_out/sweep_<cfg>.json)")
+    ap.add_argument("--no-parity", action="store_true", help="--sweep: skip the oracle's selection parity of every point")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -63,6 +63,10 @@ typedef struct {
 int qr_version(void);
 const char* qr_last_error(void);   /* HOST string, thread-local, valid until the next failing call on this thread */
 
+/* Kernels this process has launched through the library so far (every launch is counted where it is issued;
+ * memsets are not kernels and are not counted).  bench.py reports the difference over its timed region. */
+long long qr_launch_count(void);
+
 /* Number of tiles of a camera: ceil(width/16) * ceil(height/16).  Returns 0 for a NULL or zero-area camera. */
 int32_t qr_num_tiles(const qr_camera* cam);
 
@@ -134,6 +138,17 @@ int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype,
                const uint32_t* isect_gauss, const int32_t* tile_range, const void* features,
                float* out_map, int32_t* sel_idx, float* sel_w, int32_t* n_sel, float* resid_TQ,
                void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * qr_forward_stats -- work counters of the last qr_forward that took the tcgen05 path (fp32, D % 128 == 0), summed over
+ * the half-tile headers it left in its workspace ("the bench must report this count"):
+ *   stats[0] selections (sum of n_sel)            stats[1] sum over half tiles of U_ht (distinct Gaussians selected)
+ *   stats[2] tile-list entries consumed before every pixel of the half tile had stopped
+ *   stats[3] (entry, pixel) alpha' evaluations of the walk (32 x the (entry, warp) pairs that survived the culling test)
+ *   stats[4] SM clock cycles summed over the walk's half tiles      stats[5] half tiles with U_ht > 64 (two+ MMA rounds)
+ * stats is a DEVICE array of 8 int64; the call enqueues a memset and one small kernel on `stream`.
+ */
+int qr_forward_stats(const qr_camera* cam, int32_t K, const void* fwd_ws, size_t fwd_ws_bytes, int64_t* stats, void* stream);
 
 /*
  * qr_backward -- PAPER.md:37, :210.  The selection is piecewise constant in alpha' and the

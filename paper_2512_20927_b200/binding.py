@@ -27,7 +27,8 @@ STATUS = {0: "QR_OK", -1: "QR_ERR_INVALID_ARG", -2: "QR_ERR_NULL_POINTER", -3: "
 # every symbol include/qr.h declares (tests check that the library exports exactly these)
 SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_bin_workspace_bytes", "qr_bin_count",
            "qr_bin_sort", "qr_forward_workspace_bytes", "qr_forward", "qr_backward_workspace_bytes", "qr_backward",
-           "qr_backward_lists", "qr_backward_clear", "qr_dense_forward", "qr_topk_workspace_bytes", "qr_topk_forward"]
+           "qr_backward_lists", "qr_backward_clear", "qr_dense_forward", "qr_topk_workspace_bytes", "qr_topk_forward",
+           "qr_launch_count", "qr_forward_stats"]
 
 
 class QRError(RuntimeError):
@@ -87,6 +88,8 @@ def load() -> C.CDLL:
     lib.qr_backward_clear.argtypes = [cam, i32, i32, i64, vp, vp, vp, vp, sz, vp]
     lib.qr_dense_forward.restype = C.c_int
     lib.qr_dense_forward.argtypes = [cam, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.qr_launch_count.restype = C.c_longlong; lib.qr_launch_count.argtypes = []
+    lib.qr_forward_stats.restype = C.c_int; lib.qr_forward_stats.argtypes = [cam, i32, vp, sz, vp, vp]
     lib.qr_topk_workspace_bytes.restype = sz; lib.qr_topk_workspace_bytes.argtypes = [cam, i32, i32]
     lib.qr_topk_forward.restype = C.c_int
     lib.qr_topk_forward.argtypes = [cam, i32, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -381,3 +384,22 @@ def qr_topk_forward(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, fe
     out.ws = None
     out.has_lists = False
     return out
+
+
+def qr_launch_count() -> int:
+    return int(load().qr_launch_count())
+
+
+FORWARD_STATS = ("selections", "sum_U_half_tiles", "list_entries_consumed", "entry_pixel_evaluations", "walk_cycles",
+                 "half_tiles_U_gt_64")
+
+
+def qr_forward_stats(cam, K: int, fwd: ForwardOut) -> dict:
+    """Work counters of the forward that produced `fwd` (tcgen05 path only); synchronises to read eight integers."""
+    if not fwd.has_lists or fwd.ws is None:
+        raise QRError(-3, "qr_forward_stats needs the workspace of a forward on the tcgen05 path")
+    c = make_camera(cam)
+    st = torch.empty((8,), dtype=torch.int64, device=fwd.ws.device)
+    _check(load().qr_forward_stats(C.byref(c), int(K), fwd.ws.data_ptr(), fwd.ws.numel(), st.data_ptr(), _stream()))
+    v = st.cpu().tolist()
+    return dict(zip(FORWARD_STATS, v[:len(FORWARD_STATS)]))

@@ -1,5 +1,8 @@
 // qr_api.cu -- version, error string and argument checks shared by every C-ABI entry point (include/qr.h).
 #include "qr_common.cuh"
+#include "qr_sel.cuh"
+
+#include <atomic>
 
 namespace qr {
 
@@ -8,6 +11,9 @@ char* err_buf()
     static thread_local char buf[512] = {0};
     return buf;
 }
+
+static std::atomic<long long> g_launches{0};
+void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 
 int fail(int code, const char* fmt, ...)
 {
@@ -41,7 +47,44 @@ int check_feat(int32_t D, qr_dtype dt, const char* who)
     return QR_OK;
 }
 
+// sums over the half-tile headers the walk left in a forward workspace (qr_sel.cuh)
+__global__ void forward_stats_kernel(const int32_t* __restrict__ hdr, int num_half, long long* __restrict__ out)
+{
+    long long ent = 0, uni = 0, cons = 0, ev = 0, cyc = 0, big = 0;
+    for (int h = blockIdx.x * blockDim.x + threadIdx.x; h < num_half; h += gridDim.x * blockDim.x) {
+        const int32_t* d = hdr + (size_t)h * kHdrWords;
+        ent += (long long)d[0] + d[1] + d[2] + d[3];
+        uni += d[4]; cons += d[6]; ev += d[7]; cyc += d[8]; big += d[4] > 64 ? 1 : 0;
+    }
+    atomicAdd(reinterpret_cast<unsigned long long*>(out + 0), (unsigned long long)ent);
+    atomicAdd(reinterpret_cast<unsigned long long*>(out + 1), (unsigned long long)uni);
+    atomicAdd(reinterpret_cast<unsigned long long*>(out + 2), (unsigned long long)cons);
+    atomicAdd(reinterpret_cast<unsigned long long*>(out + 3), (unsigned long long)ev * 32ull);
+    atomicAdd(reinterpret_cast<unsigned long long*>(out + 4), (unsigned long long)cyc);
+    atomicAdd(reinterpret_cast<unsigned long long*>(out + 5), (unsigned long long)big);
+}
+
 }  // namespace qr
+
+extern "C" long long qr_launch_count(void) { return qr::g_launches.load(std::memory_order_relaxed); }
+
+extern "C" int qr_forward_stats(const qr_camera* cam, int32_t K, const void* fwd_ws, size_t fwd_ws_bytes, int64_t* stats, void* stream)
+{
+    using namespace qr;
+    if (int rc = check_cam(cam)) return rc;
+    if (K < 1 || K > QR_MAX_K) return fail(QR_ERR_INVALID_ARG, "qr_forward_stats: K out of range");
+    if (!fwd_ws || !stats) return fail(QR_ERR_NULL_POINTER, "qr_forward_stats: NULL argument");
+    const Cam c = make_cam(cam);
+    const WsLayout wl = ws_layout(c, K);
+    if (fwd_ws_bytes < wl.total) return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_forward_stats: workspace %zu < %zu bytes", fwd_ws_bytes, wl.total);
+    const SelLists sl = sel_view(wl.sel, const_cast<void*>(fwd_ws));
+    cudaStream_t st = (cudaStream_t)stream;
+    QR_CUDA_OK(cudaMemsetAsync(stats, 0, 8 * sizeof(int64_t), st));
+    const int nh = c.tiles_x * c.tiles_y * 2;
+    forward_stats_kernel<<<(nh + 255) / 256, 256, 0, st>>>(sl.hdr, nh, reinterpret_cast<long long*>(stats));
+    QR_LAUNCH_OK("forward_stats_kernel");
+    return QR_OK;
+}
 
 extern "C" int qr_version(void) { return QR_VERSION; }
 

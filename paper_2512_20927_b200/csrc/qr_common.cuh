@@ -50,8 +50,12 @@ int check_feat(int32_t D, qr_dtype dt, const char* who);
             return qr::fail(QR_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(e__));     \
     } while (0)
 
+// every kernel launch of the library passes through QR_LAUNCH_OK: qr_launch_count() reports how many there were
+void count_launch();
+
 #define QR_LAUNCH_OK(name)                                                                     \
     do {                                                                                       \
+        qr::count_launch();                                                                    \
         cudaError_t e__ = cudaGetLastError();                                                  \
         if (e__ != cudaSuccess)                                                                \
             return qr::fail(QR_ERR_CUDA, "launch of %s failed: %s", name, cudaGetErrorString(e__)); \
