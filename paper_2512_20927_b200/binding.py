@@ -196,8 +196,6 @@ def qr_bin_sort(cam, M: int, depth, tile_rect, offsets=None, ws: Optional[torch.
         tile_range = torch.empty((T, 2), dtype=torch.int32, device=dev)
     if ws is None:
         ws = torch.empty((max(qr_bin_workspace_bytes(n, M, T), 16),), dtype=torch.uint8, device=dev)
-    if M == 0:
-        ws[:8].zero_()
     off_ptr = None if offsets is None else _dev(offsets, torch.int64, "offsets")
     _check(load().qr_bin_sort(C.byref(c), n, int(M), _dev(depth, torch.float32, "depth"),
                               _dev(tile_rect, torch.int32, "tile_rect"), off_ptr,

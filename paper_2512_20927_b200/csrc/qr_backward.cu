@@ -39,11 +39,6 @@ template <> __device__ __forceinline__ void red_add<4>(float* dst, const float (
 }
 template <> __device__ __forceinline__ void red_add<1>(float* dst, const float (&a)[1]) { atomicAdd(dst, a[0]); }
 
-__device__ __forceinline__ uint32_t hash_id(uint32_t x)
-{
-    x ^= x >> 16; x *= 0x7feb352dU; x ^= x >> 15; x *= 0x846ca68bU; x ^= x >> 16;
-    return x;
-}
 
 template <int NV, int VW>
 __global__ void __launch_bounds__(kBwdThreads, 1) backward_band_kernel(const BackwardParams p, const int hs_max /*pow2*/)
@@ -96,7 +91,7 @@ __global__ void __launch_bounds__(kBwdThreads, 1) backward_band_kernel(const Bac
         const int lp = i / K, s = i - lp * K;
         if (s < nsel_s[lp]) {
             const int32_t id = rec_slot[i];
-            uint32_t h = hash_id((uint32_t)id) & hmask;
+            uint32_t h = hash32((uint32_t)id) & hmask;
             while (true) {
                 const int32_t old = atomicCAS(&hkey[h], -1, id);
                 if (old == -1 || old == id) break;
@@ -120,7 +115,7 @@ __global__ void __launch_bounds__(kBwdThreads, 1) backward_band_kernel(const Bac
         const int lp = i / K, s = i - lp * K;
         if (s < nsel_s[lp]) {
             const int32_t id = rec_slot[i];
-            uint32_t h = hash_id((uint32_t)id) & hmask;
+            uint32_t h = hash32((uint32_t)id) & hmask;
             while (hkey[h] != id) h = (h + 1) & hmask;
             rec_slot[i] = hslot[h];
         }
@@ -273,11 +268,6 @@ __device__ __forceinline__ void clear_row(float* row, int D, int lane)
     }
 }
 
-__device__ __forceinline__ uint32_t clear_hash(uint32_t x)
-{
-    x ^= x >> 16; x *= 0x7feb352dU; x ^= x >> 15; x *= 0x846ca68bU; x ^= x >> 16;
-    return x;
-}
 
 // seen[]: a direct-mapped cache of ids whose row some warp has already taken: a Gaussian is in the unions of ~10 half
 // tiles, and without it every row was zeroed ~10 times (225 MB of stores for 24 MB of rows).  A collision only costs
@@ -308,7 +298,7 @@ __global__ void __launch_bounds__(kClearThreads) backward_clear_kernel(const Bac
                 if (r < U) {
                     id = uid[r];
                     if ((uint32_t)id >= (uint32_t)p.N) id = -1;    // never write outside the table
-                    else if (seen && atomicExch(&seen[clear_hash((uint32_t)id) & seen_mask], id) == id) id = -1;   // already taken
+                    else if (seen && atomicExch(&seen[hash32((uint32_t)id) & seen_mask], id) == id) id = -1;   // already taken
                 }
                 uint32_t todo = __ballot_sync(0xffffffffu, id >= 0);
                 while (todo) {
@@ -328,7 +318,7 @@ __global__ void __launch_bounds__(kClearThreads) backward_clear_kernel(const Bac
                     if (s0 + lane < ns) {
                         id = __ldg(p.sel_idx + pix * p.K + s0 + lane);
                         if ((uint32_t)id >= (uint32_t)p.N) id = -1;    // never write outside the table
-                        else if (seen && atomicExch(&seen[clear_hash((uint32_t)id) & seen_mask], id) == id) id = -1;   // already taken
+                        else if (seen && atomicExch(&seen[hash32((uint32_t)id) & seen_mask], id) == id) id = -1;   // already taken
                     }
                     uint32_t todo = __ballot_sync(0xffffffffu, id >= 0);
                     while (todo) {
@@ -375,12 +365,7 @@ extern "C" int qr_backward_clear(const qr_camera* cam, int32_t K, int32_t D, int
         seen_cells = kClearSeenCells;
     }
     QR_CUDA_OK(cudaMemsetAsync(seen, 0xFF, (size_t)seen_cells * 4, (cudaStream_t)stream));
-    static int sms = 0;
-    if (sms == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-            sms = 148;
-    }
+    const int sms = sm_count();
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
     backward_clear_kernel<<<(unsigned)min(num_half, sms * 8), kClearThreads, 0, (cudaStream_t)stream>>>(p, have_lists, seen, seen_cells - 1);
     QR_LAUNCH_OK("backward_clear_kernel");
@@ -416,14 +401,7 @@ extern "C" int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N
     cudaStream_t st = (cudaStream_t)stream;
     if (backward_mma_supported(K, D)) return launch_backward_mma(p, ws, ws_bytes, st, false);
     if (backward_tile_supported(K, D)) return launch_backward_tile(p, st);
-    if (D % 4 == 0) {
-        switch ((D + 127) / 128) {
-            case 1: return launch_backward<1, 4>(p, st);
-            case 2: return launch_backward<2, 4>(p, st);
-            case 3: return launch_backward<3, 4>(p, st);
-            default: return launch_backward<4, 4>(p, st);
-        }
-    }
+    // D % 4 == 0 never reaches this point (backward_tile_supported takes it): what is left is D % 4 != 0, D <= 128
     switch ((D + 31) / 32) {
         case 1: return launch_backward<1, 1>(p, st);
         case 2: return launch_backward<2, 1>(p, st);

@@ -34,8 +34,8 @@
 // pixels.  Half tiles with more than kBmEntCap records are left to backward_tile_kernel (qr_backward_tile.cu).
 #include <cuda.h>
 
-#include "qr_async.cuh"
 #include "qr_backward.cuh"
+#include "qr_umma.cuh"
 
 namespace qr {
 
@@ -88,11 +88,6 @@ __host__ __device__ inline BmSmem bm_smem(int D, int stages)
     return L;
 }
 
-__device__ __forceinline__ uint32_t bm_hash(uint32_t x)
-{
-    x ^= x >> 16; x *= 0x7feb352dU; x ^= x >> 15; x *= 0x846ca68bU; x ^= x >> 16;
-    return x;
-}
 __device__ __forceinline__ void bm_cp16(void* dst, const void* src)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s32(dst)), "l"(src) : "memory");
@@ -102,33 +97,6 @@ __device__ __forceinline__ void bm_cp4(void* dst, const void* src)
     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(s32(dst)), "l"(src) : "memory");
 }
 __device__ __forceinline__ void bm_cp_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-__device__ __forceinline__ void bm_commit(uint64_t* bar)    // arrives when every MMA issued so far by this thread is done
-{
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(s32(bar)) : "memory");
-}
-__device__ __forceinline__ void bm_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void bm_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-// shared-memory matrix descriptor (sm_100): start >> 4 | LBO >> 4 << 16 | SBO >> 4 << 32 | version 1 << 46 | layout << 61
-__device__ __forceinline__ uint64_t bm_desc(uint32_t addr, uint32_t lbo, uint32_t sbo, uint32_t layout)
-{
-    return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) |
-           ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) | ((uint64_t)1 << 46) | ((uint64_t)layout << 61);
-}
-__device__ __forceinline__ void bm_mma(uint32_t d_tmem, uint64_t a, uint64_t b, uint32_t idesc, bool accumulate)
-{
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
-                 ::"r"(d_tmem), "l"(a), "l"(b), "r"(idesc), "r"((uint32_t)accumulate) : "memory");
-}
-// one lane of a converged warp (always the same one): the warp runs the MMA loop in uniform control flow, so the
-// descriptors live in uniform registers, and only the tcgen05 instructions themselves are predicated
-__device__ __forceinline__ bool bm_elect_one()
-{
-    uint32_t pred;
-    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
-    return pred != 0;
-}
-__device__ __forceinline__ float bm_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
 // byte offset of W[row c][pixel k] inside a 16 KB half buffer: K-major, no swizzle; core matrix = 8 rows x 4 pixels
 // (128 B); pixel chunks 128 B apart (LBO), 8-row groups 2 KB apart (SBO)
 __device__ __forceinline__ uint32_t bm_w_off(int c, int k)
@@ -187,9 +155,9 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(s32(tmem_slot)), "r"(512) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
-    bm_fence_before();
+    tc_fence_before();
     __syncthreads();
-    bm_fence_after();
+    tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
     if (warp < kBmEpiWarps) {
@@ -205,7 +173,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
         for (int unit = 0;; ++unit) {
             const int buf = unit & 1;
             mbar_wait(&tmem_full[buf], (unit >> 1) & 1);
-            bm_fence_after();
+            tc_fence_after();
             const BmDesc* d = &desc[unit % kBmDescRing];
             if (d->flags & 1) break;
             const int nrows = d->nrows;
@@ -222,7 +190,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                 if (nchunks > 3) ld16(t0 + 3 * kBmRows + c0, r3);
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
                 if (c0 + 16 >= nrows) {                 // every tcgen05.ld of this accumulator has completed
-                    bm_fence_before();
+                    tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&tmem_empty[buf]);
                 }
@@ -250,9 +218,9 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
             const BmDesc* d = &desc[unit % kBmDescRing];
             const int j0 = d->j0, j1 = d->j1, flags = d->flags;
             mbar_wait(&tmem_empty[buf], ((unit >> 1) & 1) ^ 1);
-            bm_fence_after();
+            tc_fence_after();
             if (flags & 1) {
-                if (bm_elect_one()) bm_commit(&tmem_full[buf]);
+                if (elect_one()) umma_commit(&tmem_full[buf]);
                 break;
             }
             bool have_w1 = false;
@@ -261,34 +229,34 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                 if (h == 1 && !have_w1) { mbar_wait(&w_ready[1], unit & 1); have_w1 = true; }
                 const int l = st % kBmLoStages;
                 mbar_wait(&lo_ready[l], (st / kBmLoStages) & 1);      // implies raw_full[s]
-                bm_fence_after();
+                tc_fence_after();
                 const uint32_t a_hi = st0 + s * stage_half, a_lo = lo0 + l * stage_half;
                 const uint32_t b_hi = w0 + h * 2 * kBmWHalfBytes + (j & 7) * 256, b_lo = b_hi + kBmWHalfBytes;
-                const uint64_t db_hi = bm_desc(b_hi, 128, kBmHalfPx / 4 * 128, 0);
-                const uint64_t db_lo = bm_desc(b_lo, 128, kBmHalfPx / 4 * 128, 0);
-                const uint64_t da_hi0 = bm_desc(a_hi, 1024, 512, 1), da_lo0 = bm_desc(a_lo, 1024, 512, 1);
+                const uint64_t db_hi = umma_desc(b_hi, 128, kBmHalfPx / 4 * 128, 0);
+                const uint64_t db_lo = umma_desc(b_lo, 128, kBmHalfPx / 4 * 128, 0);
+                const uint64_t da_hi0 = umma_desc(a_hi, 1024, 512, 1), da_lo0 = umma_desc(a_lo, 1024, 512, 1);
                 const uint32_t d0 = tmem_base + (uint32_t)(buf * 256);
-                if (bm_elect_one()) {
+                if (elect_one()) {
 #pragma unroll 4
                     for (int m = 0; m < nchunks; ++m) {
                         const uint64_t da_hi = da_hi0 + (uint64_t)(m * (4096 >> 4)), da_lo = da_lo0 + (uint64_t)(m * (4096 >> 4));
                         const uint32_t d_tmem = d0 + (uint32_t)(m * kBmRows);
-                        bm_mma(d_tmem, da_hi, db_hi, idesc, j != j0);
-                        bm_mma(d_tmem, da_hi, db_lo, idesc, true);
-                        bm_mma(d_tmem, da_lo, db_hi, idesc, true);
+                        umma_tf32(d_tmem, da_hi, db_hi, idesc, j != j0);
+                        umma_tf32(d_tmem, da_hi, db_lo, idesc, true);
+                        umma_tf32(d_tmem, da_lo, db_hi, idesc, true);
                     }
-                    bm_commit(&stage_empty[s]);
-                    bm_commit(&lo_empty[l]);
-                    if (h == 0 && (j == 7 || j == j1 - 1)) bm_commit(&w_free[0]);     // last read of W half 0
+                    umma_commit(&stage_empty[s]);
+                    umma_commit(&lo_empty[l]);
+                    if (h == 0 && (j == 7 || j == j1 - 1)) umma_commit(&w_free[0]);     // last read of W half 0
                 }
                 __syncwarp();
                 if (++s == stages) s = 0;
             }
             if (!have_w1) mbar_wait(&w_ready[1], unit & 1);       // keep the phases of every unit in step
-            if (bm_elect_one()) {
-                if (j0 >= 8) bm_commit(&w_free[0]);
-                bm_commit(&w_free[1]);
-                bm_commit(&tmem_full[buf]);
+            if (elect_one()) {
+                if (j0 >= 8) umma_commit(&w_free[0]);
+                umma_commit(&w_free[1]);
+                umma_commit(&tmem_full[buf]);
             }
             __syncwarp();
         }
@@ -338,8 +306,8 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
 #pragma unroll
             for (int u = 0; u < 4; ++u)
                 if (u < nchunks)
-                    lo[u * kBmConvWarps * 32] = make_float4(__fsub_rn(v[u].x, bm_hi(v[u].x)), __fsub_rn(v[u].y, bm_hi(v[u].y)),
-                                                           __fsub_rn(v[u].z, bm_hi(v[u].z)), __fsub_rn(v[u].w, bm_hi(v[u].w)));
+                    lo[u * kBmConvWarps * 32] = make_float4(__fsub_rn(v[u].x, tf32_hi(v[u].x)), __fsub_rn(v[u].y, tf32_hi(v[u].y)),
+                                                           __fsub_rn(v[u].z, tf32_hi(v[u].z)), __fsub_rn(v[u].w, tf32_hi(v[u].w)));
             fence_async_smem();
             __syncwarp();
             if (lane == 0) mbar_arrive(&lo_ready[l]);
@@ -421,7 +389,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                                 const int c = sel_col(e[u].y) - c_lo;
                                 if (c >= 0 && c < kBmRows) {          // padding entries have column 2^17 - 1
                                     const uint32_t off = bm_w_off(c, sel_pixel(e[u].y) & (kBmHalfPx - 1));
-                                    const float w = __uint_as_float(e[u].x), hi = bm_hi(w);
+                                    const float w = __uint_as_float(e[u].x), hi = tf32_hi(w);
                                     *reinterpret_cast<float*>(whi + off) = hi;
                                     *reinterpret_cast<float*>(whi + kBmWHalfBytes + off) = __fsub_rn(w, hi);
                                 }
@@ -454,7 +422,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
         }
     }
 
-    bm_fence_before();
+    tc_fence_before();
     __syncthreads();
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
 }
@@ -575,7 +543,7 @@ __global__ void __launch_bounds__(kBmPrepThreads) backward_prep_kernel(const Bac
 #pragma unroll 4
     for (int k = pl; k < R; k += kBmPrepThreads) {       // the thread that creates a cell numbers it
         const int32_t id = sid[k];
-        uint32_t h = bm_hash((uint32_t)id) & hmask;
+        uint32_t h = hash32((uint32_t)id) & hmask;
         while (true) {
             const int32_t old = atomicCAS(&hkey[h], -1, id);
             if (old == -1) {
@@ -594,7 +562,7 @@ __global__ void __launch_bounds__(kBmPrepThreads) backward_prep_kernel(const Bac
 #pragma unroll 4
     for (int k = pl; k < R; k += kBmPrepThreads) {
         const int32_t id = sid[k];
-        uint32_t h = bm_hash((uint32_t)id) & hmask;
+        uint32_t h = hash32((uint32_t)id) & hmask;
         while (hkey[h] != id) h = (h + 1) & hmask;
         const int q = spx[k], list = q >> 5;
         ent_h[(size_t)list * p.sl.qcap + (k - E[32 * list])] =
@@ -607,23 +575,6 @@ __global__ void __launch_bounds__(kBmPrepThreads) backward_prep_kernel(const Bac
         else if (pl == 4) v = ucount;
         hdr[pl] = v;
     }
-}
-
-typedef CUresult (*BmEncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-static BmEncodeTiledFn bm_encode_tiled_fn()
-{
-    static BmEncodeTiledFn fn = nullptr;
-    if (!fn) {
-        void* sym = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) == cudaSuccess &&
-            qres == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<BmEncodeTiledFn>(sym);
-    }
-    return fn;
 }
 
 int launch_backward_prep(const BackwardParams& p, int32_t* nflag, cudaStream_t st)
@@ -646,15 +597,10 @@ int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_
     p.prep_nflag = nflag;
     QR_CUDA_OK(cudaMemsetAsync(nflag, 0, 256, st));      // [0] half tiles left to the FFMA kernel, [1] the contraction's half-tile ticket
     p.ticket = nflag + 1;
-    static int sms = 0;
-    if (sms == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-            sms = 148;
-    }
+    const int sms = sm_count();
     // dL_dmap [H][W][D] fp32 as a 3-D tensor (D, W, H); box = 32 channels x 8 pixels x 1 row, 32-byte-atom 128-byte
     // swizzle (what UMMA calls SWIZZLE_128B_BASE32B); pixels outside the image are filled with zeros
-    BmEncodeTiledFn enc = bm_encode_tiled_fn();
+    EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return fail(QR_ERR_CUDA, "qr_backward: cuTensorMapEncodeTiled is not available from the driver");
     CUtensorMap tmap;
     const cuuint64_t dims[3] = { (cuuint64_t)p.D, (cuuint64_t)p.cam.width, (cuuint64_t)p.cam.height };

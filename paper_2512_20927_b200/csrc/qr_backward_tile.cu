@@ -65,11 +65,6 @@ __host__ __device__ inline BtSmem bt_smem(int D, int stages)
     return L;
 }
 
-__device__ __forceinline__ uint32_t bt_hash(uint32_t x)
-{
-    x ^= x >> 16; x *= 0x7feb352dU; x ^= x >> 15; x *= 0x846ca68bU; x ^= x >> 16;
-    return x;
-}
 
 __device__ __forceinline__ void bt_red4(float* dst, const float2& a, const float2& b)
 {
@@ -307,7 +302,7 @@ __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const Back
                     for (int k = st; k < R; k += kBtSetupThreads) {
                         const int32_t id = sid[k];
                         if (id < 0) continue;
-                        uint32_t h = bt_hash((uint32_t)id) & hmask;
+                        uint32_t h = hash32((uint32_t)id) & hmask;
                         while (true) {
                             const int32_t old = atomicCAS(&hkey[h], -1, id);
                             if (old == -1) { hslot[h] = (uint16_t)atomicAdd(&ucount, 1); break; }
@@ -333,7 +328,7 @@ __global__ void __launch_bounds__(kBtThreads, 1) backward_tile_kernel(const Back
                         for (int k = st; k < R; k += kBtSetupThreads) {
                             const int32_t id = sid[k];
                             if (id < 0) continue;
-                            uint32_t h = bt_hash((uint32_t)id) & hmask;
+                            uint32_t h = hash32((uint32_t)id) & hmask;
                             while (hkey[h] != id) h = (h + 1) & hmask;
                             const int c = (int)hslot[h] - pass * kBtRows;
                             if (c >= 0 && c < kBtRows) {
@@ -439,12 +434,7 @@ bool backward_tile_supported(int32_t K, int32_t D) { return D % 4 == 0 && D >= 4
 template <int NV>
 static int launch_bt(const BackwardParams& p, cudaStream_t st)
 {
-    static int sms = 0;
-    if (sms == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-            sms = 148;
-    }
+    const int sms = sm_count();
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
     const unsigned grid = (unsigned)min(sms, num_half);
     const int stages = max(2, min(12, (80 * 1024) / (kBtStagePx * p.D * 4)));   // ring <= 80 KB next to 146 KB of setup state

@@ -451,6 +451,7 @@ extern "C" int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M, const flo
     cudaStream_t st = (cudaStream_t)stream;
     if (M == 0 || N == 0) {
         QR_CUDA_OK(cudaMemsetAsync(tile_range, 0, sizeof(int32_t) * 2 * (size_t)T, st));
+        if (ws && ws_bytes >= 8) QR_CUDA_OK(cudaMemsetAsync(ws, 0, 8, st));      // intersections found (N == 0: none; M == 0: not counted)
         return QR_OK;
     }
     (void)offsets;                              // the bucketed sort finds its own offsets (kept in the ABI; may be NULL)
@@ -482,12 +483,7 @@ extern "C" int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M, const flo
     QR_LAUNCH_OK("tile_bucket_kernel<scatter>");
     tile_sort_kernel<false><<<(unsigned)T, 256, kSmallBucket * sizeof(uint64_t), st>>>(tile_range, T, (int32_t)M, keys, scratch, isect_gauss);
     QR_LAUNCH_OK("tile_sort_kernel<small>");
-    static int sms = 0;
-    if (sms == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-            sms = 148;
-    }
+    const int sms = sm_count();
     tile_sort_kernel<true><<<(unsigned)min(sms, T), 1024, kBigBucket * sizeof(uint64_t), st>>>(tile_range, T, (int32_t)M, keys, scratch, isect_gauss);
     QR_LAUNCH_OK("tile_sort_kernel<big>");
     return QR_OK;

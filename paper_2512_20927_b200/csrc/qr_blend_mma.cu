@@ -34,8 +34,8 @@
 #include <cuda.h>
 #include <stdlib.h>
 
-#include "qr_async.cuh"
 #include "qr_blend.cuh"
+#include "qr_umma.cuh"
 
 namespace qr {
 
@@ -96,38 +96,6 @@ struct MmaSmem {
     static constexpr int total = tmem + 16;
 };
 
-__device__ __forceinline__ void umma_commit(uint64_t* bar)     // arrives when every MMA issued so far by this thread is done
-{
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(s32(bar)) : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-
-// shared-memory matrix descriptor (sm_100): start >> 4 | LBO >> 4 << 16 | SBO >> 4 << 32 | version 1 << 46 | layout << 61
-__device__ __forceinline__ uint64_t umma_desc(uint32_t addr, uint32_t lbo, uint32_t sbo, uint32_t layout)
-{
-    return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) |
-           ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) | ((uint64_t)1 << 46) | ((uint64_t)layout << 61);
-}
-__device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t a, uint64_t b, uint32_t idesc, bool accumulate)
-{
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
-                 ::"r"(d_tmem), "l"(a), "l"(b), "r"(idesc), "r"((uint32_t)accumulate) : "memory");
-}
-__device__ __forceinline__ void umma_tf32_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b, uint32_t idesc, bool accumulate)
-{
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}"
-                 ::"r"(d_tmem), "r"(a_tmem), "l"(b), "r"(idesc), "r"((uint32_t)accumulate) : "memory");
-}
-__device__ __forceinline__ bool elect_one()     // one lane of a converged warp, always the same one
-{
-    uint32_t pred;
-    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
-    return pred != 0;
-}
-__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
 __device__ __forceinline__ int32_t ld_acquire(const int32_t* p)
 {
     int32_t v;
@@ -605,22 +573,6 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
 
 bool blend_mma_supported(int32_t D, qr_dtype feat_dtype) { return feat_dtype == QR_F32 && D >= kUnitN && D % kUnitN == 0; }   // 128, 256, 384, 512
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-static EncodeTiledFn encode_tiled_fn()
-{
-    static EncodeTiledFn fn = nullptr;
-    if (!fn) {
-        void* sym = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) == cudaSuccess &&
-            qres == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeTiledFn>(sym);
-    }
-    return fn;
-}
-
 int launch_blend_mma(const BlendParams& p, cudaStream_t st, bool pdl)
 {
     // out_map [H][W][D] fp32 as a 3-D tensor (D, W, H); box = 32 channels x 16 pixels x 2 rows, 128-byte swizzle
@@ -648,9 +600,7 @@ int launch_blend_mma(const BlendParams& p, cudaStream_t st, bool pdl)
                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (fr != CUDA_SUCCESS) return fail(QR_ERR_CUDA, "qr_forward: cuTensorMapEncodeTiled (features) failed (%d)", (int)fr);
     }
-    int dev = 0, sms = 148;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-        sms = 148;
+    const int sms = sm_count();
     const unsigned grid = (unsigned)min(sms, p.num_tiles * 2);
     QR_CUDA_OK(cudaFuncSetAttribute(blend_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MmaSmem::total));
     // programmatic dependent launch: the kernel does not wait for walk2_kernel to finish (it never calls

@@ -61,6 +61,16 @@ void count_launch();
             return qr::fail(QR_ERR_CUDA, "launch of %s failed: %s", name, cudaGetErrorString(e__)); \
     } while (0)
 
+// SMs of the current device (148 on B200)
+int sm_count();
+
+// 32-bit integer mixer (the public-domain "lowbias32" constants): shared-memory hash sets of Gaussian ids
+__host__ __device__ __forceinline__ uint32_t hash32(uint32_t x)
+{
+    x ^= x >> 16; x *= 0x7feb352dU; x ^= x >> 15; x *= 0x846ca68bU; x ^= x >> 16;
+    return x;
+}
+
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 

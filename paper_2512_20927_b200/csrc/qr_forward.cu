@@ -1,22 +1,23 @@
 // qr_forward.cu -- qr_forward: Algorithm 1 for every pixel, then f~^Q = f^Q / (1 - T^Q).
 //
-// Two kernels, split where the method itself splits ("O(N) transmittance walk" / "O(KC) blend"):
-//
-// walk_kernel   -- the O(N) part, ALU bound.  CTA = one 16x16 tile, thread = pixel, warp = 16x2 pixels = four
-//   4x2-pixel groups.  The tile's depth-sorted list is staged 256 entries at a time in shared memory; each warp
-//   first intersects the batch with its own pixel rectangle (lane-parallel box test + ballot), then runs
-//   Algorithm 1 lines 3-19 sequentially per pixel over the surviving entries only, in the paper's order and in the
-//   fp32 decision arithmetic of DESIGN.md.  A selected Gaussian is not blended here: per 4x2 pixel group the kernel
-//   appends one record (Gaussian id, the 8 pixels' weights w^Q, 0 where a pixel did not select it) to the group's
-//   list in the workspace -- the group's union of selected Gaussians, in depth order.
-//
-// blend_kernel  -- the O(KC) part.  CTA = one tile, warp = one pixel group at a time; a lane owns 4 consecutive
-//   channels of every 128-channel slab for all 8 pixels (128 fp32 accumulators at D = 512).  For every record of the
-//   group's list the feature row is loaded ONCE (128-bit coalesced, one row = one 2 KB burst at D = 512; rows shared
-//   by the groups of a tile stay in L1) and applied to the 8 pixels from registers -- 8x fewer row loads than a
-//   per-pixel gather, which is what makes the blend FMA bound instead of L1/shared bound.  Epilogue: scale by
-//   1/(1 - T^Q) (Algorithm 1 line 20), 128-bit streaming stores of the HWC map; the same warp writes the per-pixel
-//   selection records (sel_idx, sel_w, -1/0 padded).
+// The call is split where the method itself splits (the O(N) transmittance walk, the O(KC) blend):
+//   fp32 features, D % 128 == 0   walk2_kernel (qr_walk.cu: selection lists per 16x8 half tile) -> blend_mma_kernel
+//                                 (qr_blend_mma.cu: the blend as a tcgen05 contraction); the dispatcher is at the end of
+//                                 this file
+//   every other shape             the kernels of THIS file:
+// walk_kernel     -- CTA = one 16x16 tile, thread = pixel, warp = 16x2 pixels = four 4x2-pixel groups.  The tile's
+//   depth-sorted list is staged 256 entries at a time in shared memory; each warp first intersects the batch with its own
+//   pixel rectangle (lane-parallel box test + ballot), then runs Algorithm 1 lines 3-19 sequentially per pixel over the
+//   surviving entries only, in the paper's order and in the fp32 decision arithmetic of DESIGN.md.  A selected Gaussian is
+//   not blended here: per 4x2 pixel group the kernel appends one record (Gaussian id, the 8 pixels' weights w^Q, 0 where
+//   a pixel did not select it) to the group's list in the workspace -- the group's union of selected Gaussians, in depth
+//   order.  After the walk the same warp writes n_sel, T^Q and the used slots of the per-pixel selection records
+//   sel_idx / sel_w from the group lists it has just written.
+// blend_tu_kernel -- D % 4 == 0 (fp16 features, or fp32 with D % 128 != 0): persistent, warp-specialised, TMA-staged FFMA2
+//   blend of the group records (described at the kernel).
+// blend_kernel    -- D % 4 != 0 (D <= 128): CTA = one tile, warp = one pixel group at a time, feature rows loaded once per
+//   record and applied to the 8 pixels of the group from registers; epilogue x 1/(1 - T^Q) (line 20), streaming stores.
+#include "qr_async.cuh"
 #include "qr_blend.cuh"
 
 namespace qr {
@@ -330,7 +331,7 @@ __global__ void __launch_bounds__(kBlendWarps * 32, 1) blend_kernel(const BlendP
     __shared__ unsigned long long s_slot[kBlendSlots];   // ((slot + 1) << 32) | tile, 0 = never written
     __shared__ int32_t s_reads[kBlendSlots];             // how many of the slot's 31 other groups have read it
     const int lane = threadIdx.x & 31;
-    const int D = p.D, K = p.K;
+    const int D = p.D;
     if (threadIdx.x == 0) s_ticket = 0;
     if (threadIdx.x < kBlendSlots) { s_slot[threadIdx.x] = 0ull; s_reads[threadIdx.x] = 0; }
     __syncthreads();
@@ -399,13 +400,8 @@ __global__ void __launch_bounds__(kBlendWarps * 32, 1) blend_kernel(const BlendP
         const float4* rec4 = reinterpret_cast<const float4*>(recf);
         const float* recw = recf + (lane & 7);                               // lane q < 8: its own pixel's weight
 
-        // lanes 0..7 own the bookkeeping of pixel q = lane: 1/(1 - T^Q) and the record cursor
-        const int mx = gx0 + (lane & 3), my = gy0 + ((lane >> 2) & 1);
-        const bool mine = lane < kGroupPx && mx < p.cam.width && my < p.cam.height;
-        const int64_t mpix = (int64_t)my * p.cam.width + mx;
+        // lanes 0..7 carry 1/(1 - T^Q) of pixel q = lane
         const float minv = cur.inv;
-        int32_t* my_idx = p.sel_idx + mpix * K;
-        float* my_w = p.sel_w + mpix * K;
 
         float acc[kGroupPx][NV][VW];
 #pragma unroll
@@ -446,11 +442,6 @@ __global__ void __launch_bounds__(kBlendWarps * 32, 1) blend_kernel(const BlendP
             }
         };
         auto apply = [&](const Meta& m, int32_t id, const float (&f)[NV][VW]) {
-            // selection record of pixel q = lane, in list (= depth) order
-            if (mine && m.wm != 0.0f) {
-                *my_idx++ = id;
-                *my_w++ = __fmul_rn(m.wm, minv);
-            }
             // which of the 8 pixels selected this Gaussian: a ballot, so the branches below are provably uniform
             const uint32_t nz = __ballot_sync(0xffffffffu, m.wm != 0.0f) & 0xFFu;
             const float w[kGroupPx] = { m.w0.x, m.w0.y, m.w0.z, m.w0.w, m.w1.x, m.w1.y, m.w1.z, m.w1.w };
@@ -536,41 +527,8 @@ struct TuDesc {
     float inv[kTuConsumers * kGroupPx];   // 1/(1 - T^Q) per pixel of the band, 0 where nothing is selected
 };
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n\t.reg .pred P1;\n\tWAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
-        "@P1 bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
-        ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-
-__device__ __forceinline__ void st_global_pred(int32_t* ptr, int32_t v, bool on)
-{
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %2, 0;\n\t@p st.global.b32 [%0], %1;\n\t}" ::"l"(ptr), "r"(v), "r"((int)on) : "memory");
-}
-__device__ __forceinline__ void st_global_pred(float* ptr, float v, bool on)
-{
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %2, 0;\n\t@p st.global.f32 [%0], %1;\n\t}" ::"l"(ptr), "f"(v), "r"((int)on) : "memory");
-}
+using namespace aq;     // mbarrier / bulk-copy helpers (qr_async.cuh)
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return s32(p); }
 
 template <typename FeatT, int VW> struct SRow;
 template <> struct SRow<float, 4> {
@@ -613,7 +571,7 @@ template <typename FeatT, int NV, int VW, bool FULL>
 __global__ void __launch_bounds__(kTuThreads, 1) blend_tu_kernel(const BlendParams p)
 {
     extern __shared__ __align__(128) unsigned char smem[];
-    const int D = p.D, K = p.K;
+    const int D = p.D;
     const int rowbytes = D * (int)sizeof(FeatT);
     const TuSmem L = tu_smem(rowbytes);
     unsigned char* s_rows = smem + L.rows;
@@ -809,10 +767,7 @@ __global__ void __launch_bounds__(kTuThreads, 1) blend_tu_kernel(const BlendPara
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kTuConsumerRegs));
         // =========================================== consumers ===========================================
         float2 acc[kGroupPx][NV][VW / 2];     // packed pairs: the blend runs on FFMA2 (fma.rn.f32x2)
-        int32_t* my_idx = nullptr;
-        float* my_w = nullptr;
         float minv = 0.0f;
-        bool mine = false;
         int gx0 = 0, gy0 = 0;
         for (int it = 0;; ++it) {
             const int s = it % kTuStages;
@@ -824,11 +779,6 @@ __global__ void __launch_bounds__(kTuThreads, 1) blend_tu_kernel(const BlendPara
                 const int tile = d->tile, band = d->band;
                 gx0 = (tile % p.cam.tiles_x) * kTile + (warp & 3) * 4;
                 gy0 = (tile / p.cam.tiles_x) * kTile + band * 4 + (warp >> 2) * 2;
-                const int mx = gx0 + (lane & 3), my = gy0 + ((lane >> 2) & 1);
-                mine = lane < kGroupPx && mx < p.cam.width && my < p.cam.height;
-                const int64_t mpix = (int64_t)my * p.cam.width + mx;
-                my_idx = p.sel_idx + mpix * K;
-                my_w = p.sel_w + mpix * K;
                 minv = d->inv[warp * kGroupPx + (lane & 7)];
 #pragma unroll
                 for (int q = 0; q < kGroupPx; ++q)
@@ -866,12 +816,6 @@ __global__ void __launch_bounds__(kTuThreads, 1) blend_tu_kernel(const BlendPara
                 }
             };
             auto apply = [&](const Meta& m, const float (&f)[NV][VW]) {
-                // selection record of pixel q = lane, in list (= depth) order; predicated stores, no divergence
-                const bool on = mine && m.wm != 0.0f;
-                st_global_pred(my_idx, m.id, on);
-                st_global_pred(my_w, __fmul_rn(m.wm, minv), on);
-                my_idx += on ? 1 : 0;
-                my_w += on ? 1 : 0;
                 const float w[kGroupPx] = { m.w0.x, m.w0.y, m.w0.z, m.w0.w, m.w1.x, m.w1.y, m.w1.z, m.w1.w };
 #pragma unroll
                 for (int q = 0; q < kGroupPx; ++q) {
@@ -923,17 +867,6 @@ __global__ void __launch_bounds__(kTuThreads, 1) blend_tu_kernel(const BlendPara
             }
         }
     }
-}
-
-static int sm_count()
-{
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
-            n = 148;
-    }
-    return n;
 }
 
 template <typename FeatT, int NV, int VW>

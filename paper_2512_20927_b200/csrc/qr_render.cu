@@ -1,11 +1,8 @@
-// qr_render.cu -- qr_dense_forward (Eq. 1), the in-run dense comparator, as a fused band kernel.
-// (MODE 0 of the template is the first fused Q-Render kernel of this build; qr_forward now lives in qr_forward.cu
-// and MODE 0 is no longer instantiated.)
+// qr_render.cu -- qr_dense_forward (Eq. 1), the in-run dense comparator, as a fused band kernel (the FFMA
+// formulation: the first fused design of this build, kept for the comparator; Q-Render itself lives in qr_walk.cu,
+// qr_blend_mma.cu and qr_forward.cu).
 //
-// One kernel template serves both: the only difference is the rule that turns an included Gaussian into a blending
-// weight (Q-Render: only at a quantile crossing, weight T^Q alpha'; V-Render: always, weight T alpha').
-//
-// Work decomposition (DESIGN.md "qr_forward"):
+// Work decomposition:
 //   CTA  = one 16x4-pixel band of a 16x16 tile (4 CTAs share a tile's depth-sorted list), 256 threads = 8 warps.
 //   The tile list is consumed in batches of 32 entries:
 //     load     32 threads gather (id, mean2d, conic, opacity) of the batch into shared memory and derive a
@@ -13,16 +10,16 @@
 //     evaluate all 8 warps: warp (h, j) tests entries j, j+4, ... against the 32 pixels of half-band h; entries whose
 //              box misses the warp's pixels are skipped with one uniform branch; alpha' goes to shared memory, the
 //              per-entry inclusion ballot to pmask;
-//     resolve  2 warps, one thread per pixel: the sequential part of Algorithm 1 (T, T_test, k, T^Q) in the paper's
-//              order over the included entries only; selections are recorded, their weights go to Wb, and a per
-//              pixel-group bit mask of "entries some pixel of the group selected" is built with ballots;
+//     resolve  2 warps, one thread per pixel: the sequential part of Eq. 1 (T, T_test, the early stop R7) in list order
+//              over the included entries only; the weights T alpha' go to Wb, and a per pixel-group bit mask of
+//              "entries some pixel of the group blends" is built with ballots;
 //     blend    all 8 warps: warp g owns the 4x2-pixel group g and all D channels (lane = 4 consecutive channels per
 //              128-channel slab): for every entry of its mask it loads the feature row once (128-bit coalesced,
 //              L1-resident across the groups of a tile) and applies it to the 8 pixels from registers.
-//   Epilogue: normalise by 1/(1 - T^Q), 128-bit streaming stores of the HWC map, coalesced flush of the records.
+//   Epilogue: 128-bit streaming stores of the HWC map (no normalisation), final T per pixel.
 //
-// fp32 decision arithmetic (power, alpha', T, thresholds) uses explicit rounding intrinsics in the order fixed in
-// DESIGN.md so that the selected indices are reproducible; the library is also compiled with -fmad=false.
+// fp32 decision arithmetic (power, alpha', T) uses explicit rounding intrinsics in the order fixed in DESIGN.md; the
+// library is also compiled with -fmad=false.
 #include "qr_common.cuh"
 
 namespace qr {
@@ -35,7 +32,7 @@ constexpr int kRenderThreads = 256;
 
 struct RenderParams {
     Cam cam;
-    int32_t K, D;
+    int32_t D;
     float t_min;
     const float2* mean2d;
     const float4* conic_opac;
@@ -43,10 +40,7 @@ struct RenderParams {
     const int2* tile_range;
     const void* features;
     float* out_map;
-    int32_t* sel_idx;
-    float* sel_w;
-    int32_t* n_sel;
-    float* resid;     // resid_TQ (Q) or final_T (dense)
+    float* final_T;
 };
 
 template <typename FeatT, int VW> struct RowLoad;
@@ -85,8 +79,7 @@ template <> __device__ __forceinline__ void store_out<8>(float* dst, const float
     __stcs(reinterpret_cast<float4*>(dst) + 1, make_float4(v[4], v[5], v[6], v[7]));
 }
 
-// MODE 0 = Q-Render (Algorithm 1), MODE 1 = dense V-Render (Eq. 1)
-template <int MODE, typename FeatT, int NV, int VW>
+template <typename FeatT, int NV, int VW>
 __global__ void __launch_bounds__(kRenderThreads, 1) render_kernel(const RenderParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -98,15 +91,9 @@ __global__ void __launch_bounds__(kRenderThreads, 1) render_kernel(const RenderP
     uint32_t* pmask = reinterpret_cast<uint32_t*>(ent_id + kBatch);             // [32][2]
     uint32_t* gmask = pmask + 2 * kBatch;                                       // [8]
     uint32_t* done_mask = gmask + kGroups;                                      // [2]
-    float* inv_s = reinterpret_cast<float*>(done_mask + 2);                     // [64] 1/(1-T^Q) (Q) or 1 (dense)
-    int32_t* nsel_s = reinterpret_cast<int32_t*>(inv_s + kBandPx);              // [64]
-    float* A = reinterpret_cast<float*>(nsel_s + kBandPx + 2);                  // [32][64] alpha' (16-byte aligned)
+    float* A = reinterpret_cast<float*>(done_mask + 4);                         // [32][64] alpha' (2 + 2 pad words: 16-byte aligned)
     float* Wb = A + kBatch * kBandPx;                                           // [32][64] blending weights
-    float* thr = Wb + kBatch * kBandPx;                                         // [K+1] (Q only)
-    const int K = p.K, D = p.D;
-    const int rstride = K + 1;                                                  // odd-ish stride: fewer conflicts
-    int32_t* rec_id = reinterpret_cast<int32_t*>(thr + ((K + 1 + 3) & ~3));     // [64][K+1] (Q only)
-    float* rec_w = reinterpret_cast<float*>(rec_id + kBandPx * rstride);        // [64][K+1]
+    const int D = p.D;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x >> 2, band = blockIdx.x & 3;
@@ -116,20 +103,14 @@ __global__ void __launch_bounds__(kRenderThreads, 1) render_kernel(const RenderP
 
     // ---- init ----
     for (int i = tid; i < kBatch * kBandPx; i += kRenderThreads) Wb[i] = 0.0f;
-    if (MODE == 0) {
-        // thresholds 1 - (k+1)/(K+1), k = 0..K, computed as printed (R3); thr[K] == 0 is never crossed
-        for (int k = tid; k <= K; k += kRenderThreads)
-            thr[k] = __fsub_rn(1.0f, __fdiv_rn((float)(k + 1), (float)(K + 1)));
-    }
     const int2 range = p.tile_range[tile];
 
     // resolve state (meaningful in warps 0, 1 only: thread = pixel)
     const int rp = tid;                                  // local pixel index when tid < 64
     const int rpx = x0 + (rp & 15), rpy = y0 + ((rp >> 4) & 3);
     bool done = !(tid < kBandPx && rpx < p.cam.width && rpy < p.cam.height);
-    float T = 1.0f, TQ = 1.0f;
-    int k = 0, ns = 0;
-    const float t_break = (MODE == 0) ? __fdiv_rn(1.0f, (float)(K + 1)) : p.t_min;
+    float T = 1.0f;
+    const float t_break = p.t_min;
     if (tid < kBandPx) {
         const uint32_t dm = __ballot_sync(0xffffffffu, done);
         if (lane == 0) done_mask[warp] = dm;
@@ -221,28 +202,12 @@ __global__ void __launch_bounds__(kRenderThreads, 1) render_kernel(const RenderP
                 if (((pm >> lane) & 1u) && !done) {
                     const float a = A[e * kBandPx + rp];
                     const float T_test = __fmul_rn(T, __fsub_rn(1.0f, a));          // line 5
-                    if (MODE == 0) {
-                        if (T_test < thr[k]) {                                      // line 6
-                            k = k + 1;                                              // line 7
-                            const float wQ = __fmul_rn(TQ, a);                      // line 8
-                            rec_id[rp * rstride + ns] = ent_id[e];
-                            rec_w[rp * rstride + ns] = wQ;
-                            ++ns;
-                            Wb[e * kBandPx + rp] = wQ;                              // line 9 happens in "blend"
-                            sel = true;
-                            TQ = __fmul_rn(TQ, __fsub_rn(1.0f, a));                 // line 10
-                            while (T_test < thr[k]) k = k + 1;                      // lines 11-13
-                        }
-                        if (T_test < t_break) done = true;                          // lines 15-17
-                        else T = T_test;                                            // line 18
+                    if (T_test < t_break) {
+                        done = true;                                            // R7: stop without blending
                     } else {
-                        if (T_test < t_break) {
-                            done = true;                                            // R7: stop without blending
-                        } else {
-                            Wb[e * kBandPx + rp] = __fmul_rn(T, a);                 // w_i = T_i alpha'_i
-                            sel = true;
-                            T = T_test;
-                        }
+                        Wb[e * kBandPx + rp] = __fmul_rn(T, a);                 // w_i = T_i alpha'_i
+                        sel = true;
+                        T = T_test;
                     }
                 }
                 const uint32_t sm = __ballot_sync(0xffffffffu, sel);
@@ -296,21 +261,8 @@ __global__ void __launch_bounds__(kRenderThreads, 1) render_kernel(const RenderP
 
     // ---------------- epilogue ----------------
     if (tid < kBandPx) {
-        float inv = 1.0f;
-        if (MODE == 0) inv = ns > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, TQ)) : 0.0f;   // line 20; R8
-        inv_s[rp] = inv;
-        nsel_s[rp] = ns;
-        if (rpx < p.cam.width && rpy < p.cam.height) {
-            const int64_t pix = (int64_t)rpy * p.cam.width + rpx;
-            if (MODE == 0) {
-                p.n_sel[pix] = ns;
-                p.resid[pix] = ns > 0 ? TQ : 1.0f;
-            } else {
-                p.resid[pix] = T;
-            }
-        }
+        if (rpx < p.cam.width && rpy < p.cam.height) p.final_T[(int64_t)rpy * p.cam.width + rpx] = T;
     }
-    __syncthreads();
 
     // map: warp g writes its 8 pixels, 512 contiguous bytes per store instruction
 #pragma unroll
@@ -318,7 +270,6 @@ __global__ void __launch_bounds__(kRenderThreads, 1) render_kernel(const RenderP
         const int lp = gy * 32 + (q >> 2) * 16 + gx * 4 + (q & 3);
         const int px = x0 + (lp & 15), py = y0 + (lp >> 4);
         if (px < p.cam.width && py < p.cam.height) {
-            const float inv = inv_s[lp];
             float* dst = p.out_map + ((int64_t)py * p.cam.width + px) * D;
 #pragma unroll
             for (int j = 0; j < NV; ++j) {
@@ -326,83 +277,58 @@ __global__ void __launch_bounds__(kRenderThreads, 1) render_kernel(const RenderP
                 if (ch < D) {
                     float o[VW];
 #pragma unroll
-                    for (int v = 0; v < VW; ++v) o[v] = __fmul_rn(acc[q][j][v], inv);
+                    for (int v = 0; v < VW; ++v) o[v] = acc[q][j][v];
                     store_out<VW>(dst + ch, o);
                 }
             }
         }
     }
-
-    // selection records: each band row is 16*K contiguous words of sel_idx / sel_w
-    if (MODE == 0) {
-        const int npx = min(kTile, p.cam.width - x0);
-        for (int r = 0; r < kBandH; ++r) {
-            const int py = y0 + r;
-            if (py >= p.cam.height) break;
-            const int64_t gbase = ((int64_t)py * p.cam.width + x0) * K;
-            for (int i = tid; i < npx * K; i += kRenderThreads) {
-                const int pxl = i / K, s = i - pxl * K;
-                const int lp = r * 16 + pxl;
-                const bool used = s < nsel_s[lp];
-                p.sel_idx[gbase + i] = used ? rec_id[lp * rstride + s] : -1;
-                p.sel_w[gbase + i] = used ? __fmul_rn(rec_w[lp * rstride + s], inv_s[lp]) : 0.0f;
-            }
-        }
-    }
 }
 
-static size_t render_smem_bytes(int mode, int K)
+static size_t render_smem_bytes()
 {
     size_t b = 0;
     b += kBatch * (16 + 16 + 8 + 4);             // ent_co, ent_box, ent_xy, ent_id
-    b += (2 * kBatch + kGroups + 2) * 4;         // pmask, gmask, done_mask
-    b += kBandPx * 4 + (kBandPx + 2) * 4;        // inv_s, nsel_s (+2 pad keeps A 16-byte aligned)
+    b += (2 * kBatch + kGroups + 4) * 4;         // pmask, gmask, done_mask (+ 2 pad words)
     b += 2 * kBatch * kBandPx * 4;               // A, Wb
-    if (mode == 0) {
-        b += ((K + 1 + 3) & ~3) * 4;             // thr
-        b += 2 * (size_t)kBandPx * (K + 1) * 4;  // rec_id, rec_w
-    } else {
-        b += 16;
-    }
-    return b + 16;
+    return b + 32;
 }
 
-template <int MODE, typename FeatT, int NV, int VW>
+template <typename FeatT, int NV, int VW>
 static int launch_one(const RenderParams& p, int T, cudaStream_t st)
 {
-    const size_t smem = render_smem_bytes(MODE, p.K);
-    auto kern = render_kernel<MODE, FeatT, NV, VW>;
+    const size_t smem = render_smem_bytes();
+    auto kern = render_kernel<FeatT, NV, VW>;
     QR_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<(unsigned)T * 4u, kRenderThreads, smem, st>>>(p);
     QR_LAUNCH_OK("render_kernel");
     return QR_OK;
 }
 
-template <int MODE>
 static int launch_render(const RenderParams& p, qr_dtype dt, cudaStream_t st)
 {
     const int T = p.cam.tiles_x * p.cam.tiles_y;
     const int D = p.D;
     if (dt == QR_F16) {
         const int nv = (D + 255) / 256;
-        if (nv == 1) return launch_one<MODE, __half, 1, 8>(p, T, st);
-        return launch_one<MODE, __half, 2, 8>(p, T, st);
+        if (nv == 1) return launch_one<__half, 1, 8>(p, T, st);
+        return launch_one<__half, 2, 8>(p, T, st);
     }
     if (D % 4 == 0) {
         const int nv = (D + 127) / 128;
         switch (nv) {
-            case 1: return launch_one<MODE, float, 1, 4>(p, T, st);
-            case 2: return launch_one<MODE, float, 2, 4>(p, T, st);
-            case 3: return launch_one<MODE, float, 3, 4>(p, T, st);
-            default: return launch_one<MODE, float, 4, 4>(p, T, st);
+            case 1: return launch_one<float, 1, 4>(p, T, st);
+            case 2: return launch_one<float, 2, 4>(p, T, st);
+            case 3: return launch_one<float, 3, 4>(p, T, st);
+            default: return launch_one<float, 4, 4>(p, T, st);
         }
     }
     const int nv = (D + 31) / 32;
     switch (nv) {
-        case 1: return launch_one<MODE, float, 1, 1>(p, T, st);
-        case 2: return launch_one<MODE, float, 2, 1>(p, T, st);
-        case 3: return launch_one<MODE, float, 3, 1>(p, T, st);
-        default: return launch_one<MODE, float, 4, 1>(p, T, st);
+        case 1: return launch_one<float, 1, 1>(p, T, st);
+        case 2: return launch_one<float, 2, 1>(p, T, st);
+        case 3: return launch_one<float, 3, 1>(p, T, st);
+        default: return launch_one<float, 4, 1>(p, T, st);
     }
 }
 
@@ -420,10 +346,10 @@ extern "C" int qr_dense_forward(const qr_camera* cam, int32_t D, qr_dtype feat_d
     if (!aligned16(out_map) || !aligned16(features) || !aligned16(conic_opac) || !aligned16(mean2d))
         return fail(QR_ERR_MISALIGNED, "qr_dense_forward: 16-byte alignment");
     RenderParams p;
-    p.cam = make_cam(cam); p.K = 1; p.D = D; p.t_min = t_min;
+    p.cam = make_cam(cam); p.D = D; p.t_min = t_min;
     p.mean2d = reinterpret_cast<const float2*>(mean2d);
     p.conic_opac = reinterpret_cast<const float4*>(conic_opac);
     p.isect = isect_gauss; p.tile_range = reinterpret_cast<const int2*>(tile_range); p.features = features;
-    p.out_map = out_map; p.sel_idx = nullptr; p.sel_w = nullptr; p.n_sel = nullptr; p.resid = final_T;
-    return launch_render<1>(p, feat_dtype, (cudaStream_t)stream);
+    p.out_map = out_map; p.final_T = final_T;
+    return launch_render(p, feat_dtype, (cudaStream_t)stream);
 }

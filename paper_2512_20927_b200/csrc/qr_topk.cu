@@ -216,9 +216,7 @@ extern "C" int qr_topk_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dt
     topk_select_kernel<<<(unsigned)T, kTkThreads, 0, st>>>(tp);
     QR_LAUNCH_OK("topk_select_kernel");
 
-    int dev = 0, sms = 148;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-        sms = 148;
+    const int sms = sm_count();
     const unsigned rgrid = (unsigned)(sms * 8);
     const bool mma = blend_mma_supported(D, feat_dtype);
     if (mma) {

@@ -299,16 +299,12 @@ int launch_walk2(const WalkParams2& p, cudaStream_t st)
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
     // tickets and ready flags of this frame
     QR_CUDA_OK(cudaMemsetAsync(p.sl.ctrl, 0, (size_t)(kCtrlWords + num_half) * 4, st));
-    static int sms = 0, per_sm = 0;
-    if (sms == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-            sms = 148;
-        const char* e = getenv("QR_WALK_CTAS");   // EXPERIMENT
-        per_sm = e ? atoi(e) : 5;
-    }
-    // the blend kernel joins these CTAs on the same SMs and needs ~157 KB of shared memory there: an SM only changes its
-    // L1 / shared split when it is idle, so this kernel asks for the largest shared-memory carve-out although it uses 8 KB
+    const int sms = sm_count();
+    const char* e = getenv("QR_WALK_CTAS");           // profiling knob: walk CTAs per SM
+    const int per_sm = e ? atoi(e) : 5;
+    // the blend kernel takes over the SMs as these CTAs drain (programmatic dependent launch) and needs ~200 KB of shared
+    // memory there: an SM only changes its L1 / shared split when it is idle, so this kernel asks for the largest
+    // shared-memory carve-out although it uses 8 KB
     QR_CUDA_OK(cudaFuncSetAttribute(walk2_kernel<16>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     const unsigned grid = (unsigned)min(num_half, sms * per_sm);
     walk2_kernel<16><<<grid, kW2Threads, 0, st>>>(p);
