@@ -47,8 +47,11 @@ constexpr int kLoadWarp = 5;                              // warps 5, 6, 7: stag
 constexpr int kLoadWarps = 3;
 constexpr int kSchedWarp = 8;
 constexpr int kFirstConv = 9;
-constexpr int kConvWarps = 3;                             // stage st is converted by warp 9 + st % 3
-constexpr int kFirstBuild = 12;
+#ifndef KCONV
+#define KCONV 3
+#endif
+constexpr int kConvWarps = KCONV;                         // stage st is converted by warp 9 + st % kConvWarps
+constexpr int kFirstBuild = kFirstConv + kConvWarps;
 constexpr int kBuildWarps = 4;
 constexpr int kMmaThreads = (kFirstBuild + kBuildWarps) * 32;   // 512
 constexpr int kBuildThreads = kBuildWarps * 32;
@@ -56,7 +59,10 @@ constexpr int kDescReaders = kEpiWarps + 1 + kLoadWarps + kConvWarps + kBuildWar
 constexpr int kWCols = 64;                                // union columns per round
 constexpr int kUnitN = 128;                               // channels per work unit
 constexpr int kStageRows = 8;                             // union rows per stage = one tf32 K step
-constexpr int kStages = 6;
+#ifndef KSTAGES
+#define KSTAGES 6
+#endif
+constexpr int kStages = KSTAGES;
 #ifndef KRAW
 #define KRAW 12
 #endif
@@ -119,7 +125,10 @@ __device__ __forceinline__ int rounds_of(int U) { return U <= kWCols ? 1 : (U + 
 __device__ __forceinline__ int cols_of(int U, int r) { return max(0, min(kWCols, U - r * kWCols)); }
 __device__ __forceinline__ int ksteps_of(int ncols) { return max(1, (ncols + kStageRows - 1) / kStageRows); }
 
-__global__ void __launch_bounds__(kMmaThreads, 2)       // "2" only caps the registers at 64; shared memory allows one CTA
+#ifndef KMINB
+#define KMINB 2
+#endif
+__global__ void __launch_bounds__(kMmaThreads, KMINB)   // "2" only caps the registers at 64; shared memory allows one CTA
 blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tmap, const __grid_constant__ CUtensorMap feat_tmap)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -463,7 +472,7 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
         }
     } else if (warp >= kFirstBuild) {
         // ================================================= builders =================================================
-        const int ptid = tid - kFirstBuild * 32;          // 0..127 = pixel of the half tile = TMEM lane (warp % 4 = lane quarter)
+        const int ptid = (warp & 3) * 32 + lane;          // 0..127 = pixel of the half tile = TMEM lane (a warp reaches the lane quarter warp % 4)
         auto prod_sync = [&]() { named_sync<1, kBuildThreads>(); };
         float* ws = reinterpret_cast<float*>(smem + MmaSmem::w);
         auto st8 = [&](uint32_t taddr, const uint32_t (&r)[8]) {
