@@ -594,6 +594,62 @@ def run_sweep(args, qr, dev, barrier):
             for K in (4, 8, 16, 32):
                 fr.reset(cam=cam, K=K)
                 measure(fr, {"workload": "cfg4", "pose": pose, "K": K, "D": sc.D, "dtype": sc.feat_dtype}, lists)
+        # the same poses as ONE batch (include/qr.h "Multi-camera batching": B views stacked as one tall tile grid, one set of
+        # launches, one backward into one dL_dfeat), against the sum of the single-view steps above
+        ev = lambda: torch.cuda.Event(enable_timing=True)
+        N, D = sc.N, sc.D
+        for nb in (4, 8):
+            cams = []
+            for pose in range(nb):
+                cam = sc.cam.copy()
+                cam.world_to_cam = pose_on_circle(pose, 8)
+                cams.append(cam)
+            H, W = sc.cam.height, sc.cam.width
+            G = torch.randn((nb * H, W, D), dtype=torch.float32, device=dev)      # dL_dmap of the tall image, drawn on the device
+            for K in (4, 8, 16, 32):
+                st = {"cap": None, "out": None}
+                tall = qr.binding.qr_batch_camera(cams)
+                bws = qr.qr_backward_workspace(tall, K, D, dev)
+
+                def bstep(tm=None):
+                    e = [ev() for _ in range(4)] if tm is not None else None
+                    if e: e[0].record()
+                    t_, fe = pl.frontend_batch(cams, fr.d["means"], fr.d["scales"], fr.d["quats"], fr.d["opac"], st["cap"])
+                    if st["cap"] is None:
+                        st["cap"] = int(fe.M * 1.1) + 1024
+                    if e: e[1].record()
+                    st["out"] = pl.forward_batch(t_, nb, N, fe, fr.d["features"], K, st["out"])
+                    if e: e[2].record()
+                    ws = None if st["out"].has_lists else bws
+                    pl.backward(t_, N, st["out"], G, fr.dF, ws)
+                    pl.backward_clear(t_, N, st["out"], fr.dF, ws)
+                    if e:
+                        e[3].record(); tm.append(e)
+                    return fe
+                for _ in range(3):
+                    fe = bstep()
+                torch.cuda.synchronize()
+                tm = []
+                n0 = qr.binding.qr_launch_count()
+                a, b = ev(), ev()
+                a.record()
+                for _ in range(steps):
+                    fe = bstep(tm)
+                b.record()
+                torch.cuda.synchronize()
+                found = int(fe.found.item())
+                assert found <= st["cap"], "batched intersection lists overflowed"
+                mean = lambda i, j: statistics.mean(e[i].elapsed_time(e[j]) for e in tm)
+                single = sum(p["ms_step"] for p in points if p.get("K") == K and p.get("pose", 99) < nb and "views" not in p)
+                rec = {"workload": "cfg4", "views": nb, "K": K, "D": D, "dtype": sc.feat_dtype, "ms_step": a.elapsed_time(b) / steps,
+                       "frontend_ms": mean(0, 1), "qr_forward_ms": mean(1, 2), "qr_backward_and_clear_ms": mean(2, 3),
+                       "gpu_launches": qr.binding.qr_launch_count() - n0, "steps": steps, "M": found,
+                       "sum_of_single_view_steps_ms": single, "mpix_s_step": nb * H * W / (a.elapsed_time(b) / steps) / 1e3}
+                print(json.dumps(rec), file=sys.stderr, flush=True)
+                points.append(rec)
+                del st, bws
+            del G
+            torch.cuda.empty_cache()
     else:
         raise SystemExit(f"unknown sweep {args.sweep}")
     out = {"sweep": args.sweep, "command": "python bench.py --sweep " + args.sweep + (" --no-parity" if args.no_parity else ""),

@@ -37,6 +37,7 @@ extern "C" {
 #define QR_TILE 16           /* tile edge in pixels (3D-GS convention) */
 #define QR_MAX_K 256         /* largest K qr_forward / qr_backward accept */
 #define QR_TOPK_MAX_K 64      /* largest K qr_topk_forward accepts (the paper sweeps 5..50) */
+#define QR_MAX_BATCH 16       /* views per batched call (the paper trains on 4 viewpoints per step) */
 #define QR_MAX_D 512         /* largest feature width ("up to 512-D") */
 
 typedef enum {
@@ -221,6 +222,33 @@ int qr_topk_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dt
                     const uint32_t* isect_gauss, const int32_t* tile_range, const void* features,
                     float* out_map, int32_t* sel_idx, float* sel_w, int32_t* n_sel, float* resid,
                     void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * Multi-camera batching ("rendering loss from 4 randomly chosen training viewpoints"): B views
+ * of the same Gaussians, same image size (height % 16 == 0), rendered by ONE set of launches and back-propagated into ONE
+ * dL_dfeat.  The B tile grids are stacked into one tall grid of B * tiles_y tile rows; everything after the projection works on
+ * that tall image as on any other, with two indirections inside the walk: a list entry v = b * N + i ("virtual Gaussian") is
+ * looked up in the projected arrays as v and reported (sel_idx, union ids, feature / gradient rows) as i, and alpha' is evaluated
+ * in the view's own pixel coordinates -- so every per-view result is what the single-view calls give for that camera.
+ *
+ *   qr_batch_camera      tall = cams[0] with height B * H: the camera to pass to qr_bin_sort, qr_forward_batch,
+ *                        qr_backward / qr_backward_lists / qr_backward_clear and the workspace-size calls.
+ *   qr_preprocess_batch  qr_preprocess for cams[0..B) (HOST array) in one launch; every output array has B * N entries, view b
+ *                        in [b N, (b+1) N); mean2d / conic_opac / depth are bit-identical to qr_preprocess(cams[b]); tile_rect
+ *                        rows are offset by b * tiles_y.  qr_bin_count / qr_bin_sort then take B * N as their N.
+ *   qr_forward_batch     qr_forward on the tall image: out_map [B*H, W, D], records [B*H, W, ...]; N = Gaussians per view.
+ * Errors as the single-view calls; B outside [1, QR_MAX_BATCH], unequal image sizes or height % 16 != 0: QR_ERR_INVALID_ARG.
+ */
+int qr_batch_camera(const qr_camera* cams, int32_t B, qr_camera* tall);
+int qr_preprocess_batch(const qr_camera* cams, int32_t B, int64_t N,
+                        const float* means, const float* scales, const float* quats, const float* opac,
+                        float* mean2d, float* conic_opac, float* depth,
+                        int32_t* tile_rect, uint32_t* tiles_touched, void* stream);
+int qr_forward_batch(const qr_camera* tall, int32_t B, int64_t N, int32_t K, int32_t D, qr_dtype feat_dtype,
+                     const float* mean2d, const float* conic_opac,
+                     const uint32_t* isect_gauss, const int32_t* tile_range, const void* features,
+                     float* out_map, int32_t* sel_idx, float* sel_w, int32_t* n_sel, float* resid_TQ,
+                     void* ws, size_t ws_bytes, void* stream);
 
 #ifdef __cplusplus
 }

@@ -28,7 +28,7 @@ STATUS = {0: "QR_OK", -1: "QR_ERR_INVALID_ARG", -2: "QR_ERR_NULL_POINTER", -3: "
 SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_bin_workspace_bytes", "qr_bin_count",
            "qr_bin_sort", "qr_forward_workspace_bytes", "qr_forward", "qr_backward_workspace_bytes", "qr_backward",
            "qr_backward_lists", "qr_backward_clear", "qr_dense_forward", "qr_topk_workspace_bytes", "qr_topk_forward",
-           "qr_launch_count", "qr_forward_stats"]
+           "qr_launch_count", "qr_forward_stats", "qr_batch_camera", "qr_preprocess_batch", "qr_forward_batch"]
 
 
 class QRError(RuntimeError):
@@ -90,6 +90,11 @@ def load() -> C.CDLL:
     lib.qr_dense_forward.argtypes = [cam, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.qr_launch_count.restype = C.c_longlong; lib.qr_launch_count.argtypes = []
     lib.qr_forward_stats.restype = C.c_int; lib.qr_forward_stats.argtypes = [cam, i32, vp, sz, vp, vp]
+    lib.qr_batch_camera.restype = C.c_int; lib.qr_batch_camera.argtypes = [cam, i32, cam]
+    lib.qr_preprocess_batch.restype = C.c_int
+    lib.qr_preprocess_batch.argtypes = [cam, i32, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.qr_forward_batch.restype = C.c_int
+    lib.qr_forward_batch.argtypes = [cam, i32, i64, i32, i32, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.qr_topk_workspace_bytes.restype = sz; lib.qr_topk_workspace_bytes.argtypes = [cam, i32, i32]
     lib.qr_topk_forward.restype = C.c_int
     lib.qr_topk_forward.argtypes = [cam, i32, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -401,3 +406,67 @@ def qr_forward_stats(cam, K: int, fwd: ForwardOut) -> dict:
     _check(load().qr_forward_stats(C.byref(c), int(K), fwd.ws.data_ptr(), fwd.ws.numel(), st.data_ptr(), _stream()))
     v = st.cpu().tolist()
     return dict(zip(FORWARD_STATS, v[:len(FORWARD_STATS)]))
+
+
+def _cam_array(cams):
+    arr = (qr_camera * len(cams))()
+    for i, c in enumerate(cams):
+        arr[i] = make_camera(c)
+    return arr
+
+
+def qr_batch_camera(cams) -> qr_camera:
+    """The camera of the tall image that stacks the views of `cams` (include/qr.h, multi-camera batching)."""
+    arr = _cam_array(cams)
+    tall = qr_camera()
+    _check(load().qr_batch_camera(arr, len(cams), C.byref(tall)))
+    return tall
+
+
+def qr_preprocess_batch(cams, means, scales, quats, opac) -> Projected:
+    """qr_preprocess for every camera of `cams` in one launch; arrays have B * N entries (view b in [b N, (b+1) N))."""
+    arr = _cam_array(cams)
+    B = len(cams)
+    n = int(means.shape[0])
+    dev = means.device
+    out = Projected(torch.empty((B * n, 2), dtype=torch.float32, device=dev), torch.empty((B * n, 4), dtype=torch.float32, device=dev),
+                    torch.empty((B * n,), dtype=torch.float32, device=dev), torch.empty((B * n, 4), dtype=torch.int32, device=dev),
+                    torch.empty((B * n,), dtype=torch.int32, device=dev))
+    _check(load().qr_preprocess_batch(arr, B, n, _dev(means, torch.float32, "means"), _dev(scales, torch.float32, "scales"),
+                                      _dev(quats, torch.float32, "quats"), _dev(opac, torch.float32, "opac"),
+                                      out.mean2d.data_ptr(), out.conic_opac.data_ptr(), out.depth.data_ptr(),
+                                      out.tile_rect.data_ptr(), out.tiles_touched.data_ptr(), _stream()))
+    return out
+
+
+def qr_forward_batch(tall, B: int, N: int, K: int, mean2d, conic_opac, isect_gauss, tile_range, features,
+                     out: Optional[ForwardOut] = None, ws: Optional[torch.Tensor] = None) -> ForwardOut:
+    """qr_forward on the tall image of a batch of B views (N Gaussians per view).  Outputs are [B*H, W, ...]."""
+    c = make_camera(tall)
+    H, W = c.height, c.width
+    D = int(features.shape[1])
+    dev = features.device
+    dt = _feat_dtype(features)
+    if ws is None:
+        ws = _workspace(qr_forward_workspace_bytes(c, K, D), dev)
+    kk = max(int(K), 1)
+    if out is None:
+        out = ForwardOut(torch.empty((H, W, D), dtype=torch.float32, device=dev),
+                         torch.empty((H, W, kk), dtype=torch.int32, device=dev),
+                         torch.empty((H, W, kk), dtype=torch.float32, device=dev),
+                         torch.empty((H, W), dtype=torch.int32, device=dev),
+                         torch.empty((H, W), dtype=torch.float32, device=dev))
+    else:
+        want = {"out_map": (H, W, D), "sel_idx": (H, W, kk), "sel_w": (H, W, kk), "n_sel": (H, W), "resid_TQ": (H, W)}
+        for name, shape in want.items():
+            if tuple(getattr(out, name).shape) != shape:
+                raise QRError(-1, f"out.{name} has shape {tuple(getattr(out, name).shape)}, expected {shape}")
+    _check(load().qr_forward_batch(C.byref(c), int(B), int(N), int(K), D, dt, _dev(mean2d, torch.float32, "mean2d"),
+                                   _dev(conic_opac, torch.float32, "conic_opac"),
+                                   _dev(isect_gauss, torch.int32, "isect_gauss"), _dev(tile_range, torch.int32, "tile_range"),
+                                   _dev(features, features.dtype, "features"), out.out_map.data_ptr(), out.sel_idx.data_ptr(),
+                                   out.sel_w.data_ptr(), out.n_sel.data_ptr(), out.resid_TQ.data_ptr(),
+                                   ws.data_ptr(), ws.numel(), _stream()))
+    out.ws = ws
+    out.has_lists = lists_supported(features.dtype, D)
+    return out

@@ -66,6 +66,7 @@ struct WalkParams {
     int32_t* ucount;      // [2 T] union size of each 16x8 half tile
     float* rec;
     int32_t* tile_ticket; // blend_kernel's tile queue, reset here
+    int32_t batch_n = 0, view_h = 0;   // qr_forward_batch (see WalkParams2)
 };
 
 __global__ void __launch_bounds__(kWalkThreads, 5) walk_kernel(const WalkParams p)
@@ -88,9 +89,11 @@ __global__ void __launch_bounds__(kWalkThreads, 5) walk_kernel(const WalkParams 
     // warp = pixel rows 2*warp, 2*warp+1 of the tile; lane -> (x = lane & 15, y = lane >> 4)
     const int px = tile_x * kTile + (lane & 15), py = tile_y * kTile + warp * 2 + (lane >> 4);
     const bool inside = px < p.cam.width && py < p.cam.height;
-    const float fpx = (float)px + 0.5f, fpy = (float)py + 0.5f;          // R5
+    // batch of views stacked as one tall tile grid (qr_forward_batch): alpha' in the view's own pixel coordinates
+    const int yoff = p.view_h > 0 ? (tile_y * kTile / p.view_h) * p.view_h : 0;
+    const float fpx = (float)px + 0.5f, fpy = (float)(py - yoff) + 0.5f;          // R5
     const float wx_lo = (float)(tile_x * kTile), wx_hi = wx_lo + (float)kTile;
-    const float wy_lo = (float)(tile_y * kTile + warp * 2), wy_hi = wy_lo + 2.0f;
+    const float wy_lo = (float)(tile_y * kTile - yoff + warp * 2), wy_hi = wy_lo + 2.0f;
     // group of this lane: gx = (lane & 15) >> 2 ; slot of the pixel inside its group q = (lane >> 4) * 4 + (lane & 3)
     const int gx = (lane & 15) >> 2, q = (lane >> 4) * 4 + (lane & 3);
     const uint32_t gbits = (0xFu << (4 * gx)) | (0xFu << (16 + 4 * gx));  // lanes of my group
@@ -131,6 +134,7 @@ __global__ void __launch_bounds__(kWalkThreads, 5) walk_kernel(const WalkParams 
                 }
                 box = make_float4(xy.x - ex, xy.x + ex, xy.y - ey, xy.y + ey);
             }
+            if (p.batch_n > 0 && id >= 0) id = (int32_t)((uint32_t)id % (uint32_t)p.batch_n);     // virtual Gaussian b N + i -> i
             ent_id[tid] = id; ent_co[tid] = co; ent_xy[tid] = xy; ent_box[tid] = box;
             ent_col[0][tid] = -1; ent_col[1][tid] = -1;
         }
@@ -906,10 +910,11 @@ extern "C" size_t qr_forward_workspace_bytes(const qr_camera* cam, int32_t K, in
     return qr::fwd_layout(qr::make_cam(cam), K).total;
 }
 
-extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype, const float* mean2d,
-                          const float* conic_opac, const uint32_t* isect_gauss, const int32_t* tile_range,
-                          const void* features, float* out_map, int32_t* sel_idx, float* sel_w, int32_t* n_sel,
-                          float* resid_TQ, void* ws, size_t ws_bytes, void* stream)
+// batch_n / view_h: 0 for a single view; qr_forward_batch passes the Gaussians per view and the rows per view
+static int forward_impl(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype, const float* mean2d,
+                        const float* conic_opac, const uint32_t* isect_gauss, const int32_t* tile_range,
+                        const void* features, float* out_map, int32_t* sel_idx, float* sel_w, int32_t* n_sel,
+                        float* resid_TQ, void* ws, size_t ws_bytes, void* stream, int32_t batch_n, int32_t view_h)
 {
     using namespace qr;
     if (int rc = check_cam(cam)) return rc;
@@ -939,6 +944,7 @@ extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype f
         w2.isect = isect_gauss; w2.tile_range = reinterpret_cast<const int2*>(tile_range);
         w2.n_sel = n_sel; w2.resid = resid_TQ; w2.sel_idx = sel_idx; w2.sel_w = sel_w;
         w2.sl = sel_view(L.sel, ws);
+        w2.batch_n = batch_n; w2.view_h = view_h;
         if (int rc = launch_walk2(w2, st)) return rc;
         BlendParams bp;
         bp.cam = c; bp.K = K; bp.D = D; bp.cap = 0; bp.num_tiles = T; bp.tile_ticket = nullptr;
@@ -958,6 +964,7 @@ extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype f
     wp.gcount = reinterpret_cast<int32_t*>(w + L.gcount);
     wp.ucount = reinterpret_cast<int32_t*>(w + L.ucount);
     wp.rec = reinterpret_cast<float*>(w + L.rec);
+    wp.batch_n = batch_n; wp.view_h = view_h;
     const size_t smem = kWalkBatch * (16 + 16 + 8 + 4) + (size_t)(K + 1) * 4;
     walk_kernel<<<(unsigned)T, kWalkThreads, smem, st>>>(wp);
     QR_LAUNCH_OK("walk_kernel");
@@ -984,4 +991,28 @@ extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype f
         case 3: return launch_blend<float, 3, 1>(bp, st);
         default: return launch_blend<float, 4, 1>(bp, st);
     }
+}
+
+extern "C" int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype, const float* mean2d,
+                          const float* conic_opac, const uint32_t* isect_gauss, const int32_t* tile_range,
+                          const void* features, float* out_map, int32_t* sel_idx, float* sel_w, int32_t* n_sel,
+                          float* resid_TQ, void* ws, size_t ws_bytes, void* stream)
+{
+    return forward_impl(cam, K, D, feat_dtype, mean2d, conic_opac, isect_gauss, tile_range, features, out_map, sel_idx, sel_w,
+                        n_sel, resid_TQ, ws, ws_bytes, stream, 0, 0);
+}
+
+extern "C" int qr_forward_batch(const qr_camera* tall, int32_t B, int64_t N, int32_t K, int32_t D, qr_dtype feat_dtype,
+                                const float* mean2d, const float* conic_opac, const uint32_t* isect_gauss,
+                                const int32_t* tile_range, const void* features, float* out_map, int32_t* sel_idx,
+                                float* sel_w, int32_t* n_sel, float* resid_TQ, void* ws, size_t ws_bytes, void* stream)
+{
+    using namespace qr;
+    if (int rc = check_cam(tall)) return rc;
+    if (B < 1 || B > QR_MAX_BATCH) return fail(QR_ERR_INVALID_ARG, "qr_forward_batch: B = %d outside [1, QR_MAX_BATCH]", B);
+    if (tall->height % B != 0 || (tall->height / B) % kTile != 0)
+        return fail(QR_ERR_INVALID_ARG, "qr_forward_batch: height %d is not B = %d views of a multiple of 16 rows", tall->height, B);
+    if (N < 1 || N * (int64_t)B >= (int64_t(1) << 31)) return fail(QR_ERR_INVALID_ARG, "qr_forward_batch: N outside [1, 2^31 / B)");
+    return forward_impl(tall, K, D, feat_dtype, mean2d, conic_opac, isect_gauss, tile_range, features, out_map, sel_idx, sel_w,
+                        n_sel, resid_TQ, ws, ws_bytes, stream, (int32_t)N, tall->height / B);
 }

@@ -16,14 +16,14 @@ __device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b);
 __device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b); }
 __device__ __forceinline__ float fdiv(float a, float b) { return __fdiv_rn(a, b); }
 
-__global__ void __launch_bounds__(256)
-preprocess_kernel(const Cam cam, const int64_t N, const float* __restrict__ means, const float* __restrict__ scales,
-                  const float* __restrict__ quats, const float* __restrict__ opac, float2* __restrict__ mean2d,
-                  float4* __restrict__ conic_opac, float* __restrict__ depth, int4* __restrict__ tile_rect,
-                  uint32_t* __restrict__ tiles_touched)
+// Gaussian i seen by `cam`; results go to slot `o` of the output arrays; the tile rectangle's rows are shifted by `ty_off`
+// tiles (0 for a single view; view b of a batch sits b * tiles_y rows down the tall tile grid)
+__device__ __forceinline__ void project_one(const Cam& cam, const int64_t i, const int64_t o, const int ty_off,
+                                            const float* __restrict__ means, const float* __restrict__ scales,
+                                            const float* __restrict__ quats, const float* __restrict__ opac,
+                                            float2* __restrict__ mean2d, float4* __restrict__ conic_opac, float* __restrict__ depth,
+                                            int4* __restrict__ tile_rect, uint32_t* __restrict__ tiles_touched)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
 
     const float mx = means[3 * i], my = means[3 * i + 1], mz = means[3 * i + 2];
     const float* W = cam.w;
@@ -34,7 +34,7 @@ preprocess_kernel(const Cam cam, const int64_t N, const float* __restrict__ mean
         t[r] = __fmaf_rn(W[4 * r + 2], mz, __fmaf_rn(W[4 * r + 1], my, __fmaf_rn(W[4 * r], mx, W[4 * r + 3])));
 
     const float tz = t[2];
-    depth[i] = tz;
+    depth[o] = tz;
     float2 m2 = make_float2(0.f, 0.f);
     float4 co = make_float4(0.f, 0.f, 0.f, 0.f);
     int4 rect = make_int4(0, 0, 0, 0);
@@ -109,15 +109,42 @@ preprocess_kernel(const Cam cam, const int64_t N, const float* __restrict__ mean
             const int y0 = min(max((int)fminf(fmaxf(fy0, -big), big), 0), cam.tiles_y);
             const int y1 = min(max((int)fminf(fmaxf(fy1, -big), big) + 1, 0), cam.tiles_y);
             if (x1 > x0 && y1 > y0) {
-                rect = make_int4(x0, y0, x1, y1);
+                rect = make_int4(x0, y0 + ty_off, x1, y1 + ty_off);
                 touched = (uint32_t)((x1 - x0) * (y1 - y0));
             }
         }
     }
-    mean2d[i] = m2;
-    conic_opac[i] = co;
-    tile_rect[i] = rect;
-    tiles_touched[i] = touched;
+    mean2d[o] = m2;
+    conic_opac[o] = co;
+    tile_rect[o] = rect;
+    tiles_touched[o] = touched;
+}
+
+__global__ void __launch_bounds__(256)
+preprocess_kernel(const Cam cam, const int64_t N, const float* __restrict__ means, const float* __restrict__ scales,
+                  const float* __restrict__ quats, const float* __restrict__ opac, float2* __restrict__ mean2d,
+                  float4* __restrict__ conic_opac, float* __restrict__ depth, int4* __restrict__ tile_rect,
+                  uint32_t* __restrict__ tiles_touched)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    project_one(cam, i, i, 0, means, scales, quats, opac, mean2d, conic_opac, depth, tile_rect, tiles_touched);
+}
+
+// B views in one launch (blockIdx.y = view): virtual Gaussian v = b N + i
+struct CamBatch { Cam c[QR_MAX_BATCH]; };
+__global__ void __launch_bounds__(256)
+preprocess_batch_kernel(const __grid_constant__ CamBatch cams, const int64_t N, const float* __restrict__ means,
+                        const float* __restrict__ scales, const float* __restrict__ quats, const float* __restrict__ opac,
+                        float2* __restrict__ mean2d, float4* __restrict__ conic_opac, float* __restrict__ depth,
+                        int4* __restrict__ tile_rect, uint32_t* __restrict__ tiles_touched)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int b = blockIdx.y;
+    const Cam& cam = cams.c[b];
+    project_one(cam, i, (int64_t)b * N + i, b * cam.tiles_y, means, scales, quats, opac, mean2d, conic_opac, depth, tile_rect,
+                tiles_touched);
 }
 
 }  // namespace qr
@@ -141,5 +168,53 @@ extern "C" int qr_preprocess(const qr_camera* cam, int64_t N, const float* means
         k, N, means, scales, quats, opac, reinterpret_cast<float2*>(mean2d), reinterpret_cast<float4*>(conic_opac),
         depth, reinterpret_cast<int4*>(tile_rect), tiles_touched);
     QR_LAUNCH_OK("preprocess_kernel");
+    return QR_OK;
+}
+
+static int check_batch(const qr_camera* cams, int32_t B)
+{
+    using namespace qr;
+    if (!cams) return fail(QR_ERR_NULL_POINTER, "cameras are NULL");
+    if (B < 1 || B > QR_MAX_BATCH) return fail(QR_ERR_INVALID_ARG, "B = %d outside [1, QR_MAX_BATCH]", B);
+    for (int b = 0; b < B; ++b) {
+        if (int rc = check_cam(cams + b)) return rc;
+        if (cams[b].width != cams[0].width || cams[b].height != cams[0].height)
+            return fail(QR_ERR_INVALID_ARG, "the views of a batch must have the same image size");
+    }
+    if (cams[0].height % kTile != 0)
+        return fail(QR_ERR_INVALID_ARG, "batched views need height %% 16 == 0 (height = %d)", cams[0].height);
+    return QR_OK;
+}
+
+extern "C" int qr_batch_camera(const qr_camera* cams, int32_t B, qr_camera* tall)
+{
+    using namespace qr;
+    if (int rc = check_batch(cams, B)) return rc;
+    if (!tall) return fail(QR_ERR_NULL_POINTER, "qr_batch_camera: tall is NULL");
+    *tall = cams[0];
+    tall->height = cams[0].height * B;
+    return check_cam(tall);
+}
+
+extern "C" int qr_preprocess_batch(const qr_camera* cams, int32_t B, int64_t N, const float* means, const float* scales,
+                                   const float* quats, const float* opac, float* mean2d, float* conic_opac, float* depth,
+                                   int32_t* tile_rect, uint32_t* tiles_touched, void* stream)
+{
+    using namespace qr;
+    if (int rc = check_batch(cams, B)) return rc;
+    if (N < 0) return fail(QR_ERR_INVALID_ARG, "N = %lld < 0", (long long)N);
+    if (N * (int64_t)B >= (int64_t(1) << 31)) return fail(QR_ERR_UNSUPPORTED, "B N >= 2^31");
+    if (N == 0) return QR_OK;
+    if (!means || !scales || !quats || !opac || !mean2d || !conic_opac || !depth || !tile_rect || !tiles_touched)
+        return fail(QR_ERR_NULL_POINTER, "qr_preprocess_batch: NULL array");
+    if (!aligned16(quats) || !aligned16(conic_opac) || !aligned16(tile_rect) || !aligned16(mean2d))
+        return fail(QR_ERR_MISALIGNED, "qr_preprocess_batch: quats / mean2d / conic_opac / tile_rect must be 16-byte aligned");
+    CamBatch cb;
+    for (int b = 0; b < QR_MAX_BATCH; ++b) cb.c[b] = make_cam(cams + (b < B ? b : 0));
+    const dim3 grid((unsigned)((N + 255) / 256), (unsigned)B);
+    preprocess_batch_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(
+        cb, N, means, scales, quats, opac, reinterpret_cast<float2*>(mean2d), reinterpret_cast<float4*>(conic_opac),
+        depth, reinterpret_cast<int4*>(tile_rect), tiles_touched);
+    QR_LAUNCH_OK("preprocess_batch_kernel");
     return QR_OK;
 }

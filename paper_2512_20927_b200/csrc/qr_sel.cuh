@@ -121,6 +121,8 @@ struct WalkParams2 {
     int32_t* sel_idx;
     float* sel_w;
     SelLists sl;
+    int32_t batch_n = 0;    // qr_forward_batch: ids in isect are virtual (view * N + Gaussian); 0 = single view
+    int32_t view_h = 0;     //                   rows per view of the tall image; 0 = single view
 };
 int launch_walk2(const WalkParams2& p, cudaStream_t st);
 

@@ -22,6 +22,9 @@ namespace qr {
 
 constexpr int kW2Threads = 128;
 constexpr int kW2Batch = 128;
+#ifndef QR_WX
+#define QR_WX 16
+#endif
 
 __device__ __forceinline__ float clampf(float v, float lo, float hi) { return fminf(fmaxf(v, lo), hi); }
 __device__ __forceinline__ void st_release(int32_t* p, int32_t v)
@@ -119,9 +122,12 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
     const int mpix = (by0 + ly) * kTile + bx0 + lx;   // row-major index inside the half tile
     const int px = x0 + bx0 + lx, py = y0 + by0 + ly;
     const bool inside = px < p.cam.width && py < p.cam.height;
-    const float fpx = (float)px + 0.5f, fpy = (float)py + 0.5f;          // R5
+    // batch of views stacked as one tall tile grid (qr_forward_batch): alpha' is evaluated in the view's own pixel
+    // coordinates, exactly as a single-view call would; only the output index uses the tall row
+    const int yoff = p.view_h > 0 ? (y0 / p.view_h) * p.view_h : 0;
+    const float fpx = (float)px + 0.5f, fpy = (float)(py - yoff) + 0.5f;          // R5
     const float X0 = (float)(x0 + bx0) + 0.5f, X1 = X0 + (float)(WX - 1);
-    const float Y0 = (float)(y0 + by0) + 0.5f, Y1 = Y0 + (float)(WY - 1);
+    const float Y0 = (float)(y0 - yoff + by0) + 0.5f, Y1 = Y0 + (float)(WY - 1);
     const int64_t pix = (int64_t)py * p.cam.width + px;
     int32_t* my_idx = p.sel_idx + pix * K;
     uint2* my_ent = p.sl.ent + ((size_t)ht * kSelLists + warp) * p.sl.qcap;
@@ -224,6 +230,7 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
                 if (!(co.w > 0.0f)) qmax = -1.0f;                         // alpha' = 0 < 1/255 everywhere
                 cull = make_float4(ia, ic, qmax, 0.f);
             }
+            if (p.batch_n > 0 && id >= 0) id = (int32_t)((uint32_t)id % (uint32_t)p.batch_n);     // virtual Gaussian b N + i -> i
             s_id[tid] = id; s_co[tid] = co; s_xy[tid] = xy; s_cull[tid] = cull; s_col[tid] = -1;
         }
         __syncthreads();
@@ -305,9 +312,9 @@ int launch_walk2(const WalkParams2& p, cudaStream_t st)
     // the blend kernel takes over the SMs as these CTAs drain (programmatic dependent launch) and needs ~200 KB of shared
     // memory there: an SM only changes its L1 / shared split when it is idle, so this kernel asks for the largest
     // shared-memory carve-out although it uses 8 KB
-    QR_CUDA_OK(cudaFuncSetAttribute(walk2_kernel<16>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    QR_CUDA_OK(cudaFuncSetAttribute(walk2_kernel<QR_WX>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     const unsigned grid = (unsigned)min(num_half, sms * per_sm);
-    walk2_kernel<16><<<grid, kW2Threads, 0, st>>>(p);
+    walk2_kernel<QR_WX><<<grid, kW2Threads, 0, st>>>(p);
     QR_LAUNCH_OK("walk2_kernel");
     return QR_OK;
 }

@@ -65,3 +65,22 @@ def dense_forward(cam, fe: Frontend, features: torch.Tensor, t_min: float = 1e-4
 def topk_forward(cam, fe: Frontend, features: torch.Tensor, K: int, t_min: float = 1e-4, out: Optional[B.ForwardOut] = None):
     """The top-K comparator on the same front end."""
     return B.qr_topk_forward(cam, K, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, t_min, out)
+
+
+def frontend_batch(cams, means, scales, quats, opac, capacity: Optional[int] = None):
+    """Front end of a batch of views (include/qr.h, multi-camera batching): one projection launch for all cameras, one
+    sort over the tall tile grid.  Returns (tall camera, Frontend); arrays have B * N entries."""
+    tall = B.qr_batch_camera(cams)
+    proj = B.qr_preprocess_batch(cams, means, scales, quats, opac)
+    if capacity is None:
+        offsets, M = B.qr_bin_count(proj.tiles_touched)
+        isect, rng = B.qr_bin_sort(tall, M, proj.depth, proj.tile_rect, offsets)
+        return tall, Frontend(proj, offsets, M, isect, rng)
+    isect, rng, found = B.qr_bin_sort(tall, int(capacity), proj.depth, proj.tile_rect, None, return_found=True)
+    return tall, Frontend(proj, None, int(capacity), isect, rng, found)
+
+
+def forward_batch(tall, n_views: int, N: int, fe: Frontend, features: torch.Tensor, K: int, out: Optional[B.ForwardOut] = None):
+    """Q-Render of every view of the batch in one walk + one blend; outputs are [B*H, W, ...].  backward / backward_clear
+    take `tall` and N as they are and accumulate every view into one dL_dfeat."""
+    return B.qr_forward_batch(tall, n_views, N, K, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, out)

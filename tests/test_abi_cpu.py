@@ -71,6 +71,13 @@ def test_bad_arguments_are_status_codes(lib):
     assert tk(65, 16, 1e-4, p, 1 << 20) == -3
     assert tk(8, 16, -1.0, p, 1 << 20) == -1
     assert tk(8, 16, 1e-4, z, 1 << 20) == -2
+    # batching: B out of range, unequal sizes, height % 16 != 0
+    two = (binding.qr_camera * 2)(binding.make_camera(make_camera(64, 64)), binding.make_camera(make_camera(64, 48)))
+    tall = binding.qr_camera()
+    assert lib.qr_batch_camera(two, 0, C.byref(tall)) == -1 and lib.qr_batch_camera(two, 2, C.byref(tall)) == -1
+    odd = (binding.qr_camera * 1)(binding.make_camera(make_camera(64, 50)))
+    assert lib.qr_batch_camera(odd, 1, C.byref(tall)) == -1
+    assert lib.qr_batch_camera(two, 1, C.byref(tall)) == 0 and tall.height == 64
     assert lib.qr_topk_workspace_bytes(C.byref(cam), 8, 16) > 0 and lib.qr_topk_workspace_bytes(C.byref(cam), 0, 16) == 0
     assert lib.qr_bin_sort(C.byref(cam), 10, 1 << 31, p, p, p, p, p, p, 1 << 20, None) == -5
     m = C.c_int64(-1)

@@ -513,6 +513,59 @@ def test_topk_full_size_config3_sampled(qr, orc):
     print("top-K cfg3 full size:", stats, "sampled:", s2)
 
 
+# ------------------------------------------------------------------------------------------------
+# multi-camera batching (NEXT-4; include/qr.h "Multi-camera batching")
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("D,K,n_views", [(128, 16, 3), (16, 40, 4), (512, 8, 2)])
+def test_batch_of_views_equals_the_oracle_per_view(qr, orc, D, K, n_views):
+    """B poses of config 4's circle rendered by ONE set of launches (tall tile grid): every view's slice is compared with
+    the oracle run on that camera alone, the projection is bit-identical to the single-view call, and the gradient of
+    all views, accumulated into one dL_dfeat by one backward, equals the sum of the oracle's per-view gradients."""
+    from qr_inputs.scenes import pose_on_circle
+    sc = make_scene("cfg4", seed=23, N=40000, W=96, H=64, D=D, pose=0, backward=True)
+    feats = sc.features.astype(np.float32)
+    cams = []
+    for j in range(n_views):
+        c = sc.cam.copy()
+        c.world_to_cam = pose_on_circle(2 * j + 1, 8)
+        cams.append(c)
+    H, W, N = sc.cam.height, sc.cam.width, sc.N
+    g = P.upload(sc)
+    gf = P.to_dev(feats)
+    tall, fe = qr.pipeline.frontend_batch(cams, g.means, g.scales, g.quats, g.opac)
+    assert tall.height == n_views * H and tall.width == W
+    out = qr.pipeline.forward_batch(tall, n_views, N, fe, gf, K)
+    rng = np.random.default_rng(3)
+    G = rng.standard_normal((n_views * H, W, D), dtype=np.float32)
+    dF = qr.pipeline.backward(tall, N, out, P.to_dev(G))
+    gref = np.zeros((N, D))
+    A = np.zeros((N, D))                         # sum |w g| per element: the fan-in term of the gradient tolerance
+    tainted = np.zeros(N, bool)
+    for j, cam in enumerate(cams):
+        single = qr.qr_preprocess(cam, g.means, g.scales, g.quats, g.opac)
+        for name in ("mean2d", "conic_opac", "depth", "tiles_touched"):
+            assert torch.equal(getattr(fe.proj, name)[j * N:(j + 1) * N], getattr(single, name)), name
+        proj = orc.project(cam, sc.means, sc.scales, sc.quats, sc.opac)
+        lists = orc.pixel_lists(cam, proj)
+        q = orc.qrender(lists, K, feats)
+        view = qr.binding.ForwardOut(out.out_map[j * H:(j + 1) * H], out.sel_idx[j * H:(j + 1) * H], out.sel_w[j * H:(j + 1) * H],
+                                     out.n_sel[j * H:(j + 1) * H], out.resid_TQ[j * H:(j + 1) * H])
+        stats = P.compare_forward(view, q, lists, K, D)
+        print("view", j, stats)
+        gref += orc.backward(q.sel_idx, q.sel_w, q.n_sel, G[j * H:(j + 1) * H].reshape(H * W, D), N)
+        A += orc.backward(q.sel_idx, q.sel_w, q.n_sel, np.abs(G[j * H:(j + 1) * H]).reshape(H * W, D), N)
+        sel, _, n = P.masked_records(view)
+        same = P.same_selection(sel, n, q)
+        for pth in np.flatnonzero(~same):
+            tainted[sel[pth, :n[pth]]] = True
+            tainted[q.sel_idx[pth, :q.n_sel[pth]]] = True
+    assert (~tainted).sum() > 0.5 * N
+    worst, over = P.compare_backward_rows(dF.cpu().numpy()[~tainted], gref[~tainted], "batched backward", A[~tainted])
+    print("gradient rows compared", int((~tainted).sum()), "worst err/tol", worst, "elements over the plain bar", over)
+    qr.pipeline.backward_clear(tall, N, out, dF)
+    assert float(dF.abs().max()) == 0.0
+
+
 def test_error_codes(qr):
     sc = make_scene("cfg1", seed=0, N=100)
     g = P.upload(sc)
