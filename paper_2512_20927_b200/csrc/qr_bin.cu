@@ -248,11 +248,11 @@ constexpr int kSmallBucket = 2048;          // keys sorted by tile_sort_kernel<s
 constexpr int kBigBucket = 16384;           // keys per shared-memory run of tile_sort_kernel<big> (128 KB)
 constexpr uint64_t kKeyInf = ~uint64_t(0);
 
-// Register-blocked bitonic network for one bucket of 256 E keys (E = 1, 2, 4, 8) on 256 threads: thread t holds keys
+// Register-blocked bitonic network for one bucket of THREADS x E keys: thread t holds keys
 // t E .. t E + E - 1.  Strides below E are compare-exchanges inside a thread, strides below 32 E are exchanged with
 // __shfl_xor, and only the three largest strides of the last three merges (6 steps of the 36..66) go through shared
 // memory.  The all-shared-memory network (still used for the big buckets) was bound by shared-memory wavefronts.
-template <int E>
+template <int E, int THREADS = 256>
 __device__ __forceinline__ void bitonic_sort_regs(const uint64_t* __restrict__ keys, int n, uint32_t* __restrict__ out,
                                                   uint64_t* s)
 {
@@ -260,7 +260,7 @@ __device__ __forceinline__ void bitonic_sort_regs(const uint64_t* __restrict__ k
     uint64_t v[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) v[e] = t * E + e < n ? keys[t * E + e] : kKeyInf;
-    constexpr int n2 = 256 * E;
+    constexpr int n2 = THREADS * E;
 #pragma unroll 1
     for (int k = 2; k <= n2; k <<= 1) {
 #pragma unroll 1
@@ -275,13 +275,16 @@ __device__ __forceinline__ void bitonic_sort_regs(const uint64_t* __restrict__ k
                     v[e] = keep_min ? min(v[e], o) : max(v[e], o);
                 }
             } else {
+                // key i = t E + e sits at s[e THREADS + t]: a warp's stores are contiguous, and so are its loads of the
+                // partners i ^ j = (t ^ j / E) E + e (j / E >= 32 flips a bit above the lane index): no bank conflicts
 #pragma unroll
-                for (int e = 0; e < E; ++e) s[t * E + e] = v[e];
+                for (int e = 0; e < E; ++e) s[e * THREADS + t] = v[e];
                 __syncthreads();
+                const int tp = t ^ (j / E);
 #pragma unroll
                 for (int e = 0; e < E; ++e) {
                     const int i = t * E + e;
-                    const uint64_t o = s[i ^ j];
+                    const uint64_t o = s[e * THREADS + tp];
                     const bool keep_min = ((i & j) == 0) == ((i & k) == 0);
                     v[e] = keep_min ? min(v[e], o) : max(v[e], o);
                 }
@@ -324,6 +327,13 @@ __device__ __forceinline__ void tile_sort_one(const int tile, const int capacity
         else if (n <= 512) bitonic_sort_regs<2>(keys + start, n, isect_gauss + start, skeys);
         else if (n <= 1024) bitonic_sort_regs<4>(keys + start, n, isect_gauss + start, skeys);
         else bitonic_sort_regs<8>(keys + start, n, isect_gauss + start, skeys);
+        return;
+    }
+    if (BIG && n <= kRun) {                     // 1,024 threads, 4 / 8 / 16 keys per thread in registers (was the all-shared-memory
+        if (n <= 4096) bitonic_sort_regs<4, 1024>(keys + start, n, isect_gauss + start, skeys);          // network: 0.64 ms of config 4's
+        else if (n <= 8192) bitonic_sort_regs<8, 1024>(keys + start, n, isect_gauss + start, skeys);     // 0.87 ms front end)
+        else bitonic_sort_regs<16, 1024>(keys + start, n, isect_gauss + start, skeys);
+        __syncthreads();
         return;
     }
     if (n <= kRun) {
