@@ -14,6 +14,7 @@
  *   - PAPER.md:129-158  Algorithm 1 (QuantileRender), executed literally, line by line
  *   - SPEC.md:462-470   backward: d f~ / d f_i = w^Q_i / (1 - T^Q) * I  (selection is piecewise constant)
  *   - PAPER.md:167,:187 top-K comparator, as reconstructed in SPEC.md:221-229 (reading R17)
+ *   - PAPER.md:760-769  stratified-K variant (reading R18)
  * No blocking, fusion or reordering beyond those passages.
  *
  * Precision.  Everything is fp64 EXCEPT the quantities that decide an integer (which
@@ -671,6 +672,124 @@ void orc_topk(int64_t npix, const int64_t* pix, const int64_t* off, const int32_
                 for (int d = 0; d < D; ++d) out_map[j * D + d] = (float)acc[d];
         }
         free(acc); free(wbuf); free(taken);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O7: stratified-K, the paper's adaptive variant ("we compute the mean and standard deviation of the
+ * transmittance values along the depth dimension ... uniformly partition the transmittance interval in the z-score space
+ * and then map the samples back to the original transmittance domain"; "two passes along each ray").  The
+ * paper gives the idea, not the constants; reading R18 fixes them (z_max = 2 as SPEC.md:272):
+ *   pass 1  dense transmittance T_i = prod_{j<=i} (1 - alpha'_j) over the ray's list with V-Render's early stop R7
+ *           (entries before the first T_test < t_min); mu = mean(T_i), sigma = population std(T_i) over those n entries;
+ *   pass 2  Algorithm 1 with the K boundaries  b_k = clamp(mu + sigma z_k, 0, 1),  z_k = z_max (1 - 2 (k+1) / (K+1)),
+ *           k = 0..K-1 (b_K = 0 is never crossed), in place of 1 - (k+1)/(K+1); the walk breaks once every boundary is
+ *           crossed (T_test < b_{K-1}) or the dense stop is reached (T_test < t_min), after the selection test as in
+ *           lines 15-17; weights, sparse T^Q and the normalisation are Algorithm 1's.
+ *   sigma == 0 (n <= 1, or all T_i equal): Q-Render's uniform boundaries ("fall back to Q-Render partition").
+ * Everything that decides an integer is fp32 in this order: S1 += T_i; S2 = fmaf(T_i, T_i, S2); mu = S1 / n;
+ * var = S2 / n - mu * mu; sigma = sqrtf(max(var, 0)); z_k = z_max * (1 - (float)(2 (k+1)) / (float)(K+1));
+ * b_k = fminf(fmaxf(fmaf(sigma, z_k, mu), 0), 1).
+ * margin = min |T_test - b_k| over walked steps and open boundaries (fp64), stop_margin as O3 for pass 1.
+ * ---------------------------------------------------------------------------------------- */
+static inline float strat_boundary(int k, int K, float mu, float sigma, float z_max)
+{
+    if (k >= K) return 0.0f;
+    if (!(sigma > 0.0f)) return q_threshold(k, K);
+    const float z = z_max * (1.0f - (float)(2 * (k + 1)) / (float)(K + 1));
+    return fminf(fmaxf(fmaf(sigma, z, mu), 0.0f), 1.0f);
+}
+
+static void stratified_ray(int64_t n, const int32_t* I, const float* alpha, int K, int D, const float* F, int64_t fstride,
+                           float t_min, float z_max, double* fQ, int32_t* sel_idx, double* sel_w, int32_t* n_sel_out,
+                           double* TQ_out, int32_t* n_walked, double* margin_out, double* stop_margin, float* mu_out,
+                           float* sigma_out, int32_t* n_dense_out)
+{
+    /* pass 1: statistics of the dense transmittance */
+    float T = 1.0f, S1 = 0.0f, S2 = 0.0f;
+    int32_t nd = 0;
+    double smarg = INFINITY;
+    for (int64_t s = 0; s < n; ++s) {
+        const float T_test = T * (1.0f - alpha[s]);
+        if (t_min > 0.0f) {
+            const double m = fabs((double)T_test - (double)t_min) / (double)t_min;
+            if (m < smarg) smarg = m;
+        }
+        if (T_test < t_min) break;
+        T = T_test;
+        S1 = S1 + T;
+        S2 = fmaf(T, T, S2);
+        ++nd;
+    }
+    float mu = 0.0f, sigma = 0.0f;
+    if (nd > 0) {
+        mu = S1 / (float)nd;
+        const float var = S2 / (float)nd - mu * mu;
+        sigma = sqrtf(fmaxf(var, 0.0f));
+    }
+    /* pass 2: Algorithm 1 with the stratified boundaries */
+    T = 1.0f;
+    double TQ = 1.0;
+    int k = 0;
+    if (fQ) for (int d = 0; d < D; ++d) fQ[d] = 0.0;
+    for (int s = 0; s < K; ++s) { sel_idx[s] = -1; sel_w[s] = 0.0; }
+    int32_t ns = 0, walked = 0;
+    double marg = INFINITY;
+    const float b_last = strat_boundary(K - 1, K, mu, sigma, z_max);
+    for (int64_t s = 0; s < n; ++s) {
+        const int32_t i = I[s];
+        const float a = alpha[s];
+        const float T_test = T * (1.0f - a);
+        ++walked;
+        for (int kk = k; kk < K; ++kk) {
+            const double m = fabs((double)T_test - (double)strat_boundary(kk, K, mu, sigma, z_max));
+            if (m < marg) marg = m;
+        }
+        { const double m = fabs((double)T_test - (double)t_min); if (m < marg) marg = m; }
+        if (T_test < strat_boundary(k, K, mu, sigma, z_max)) {
+            k = k + 1;
+            const double wQ = TQ * (double)a;
+            if (fQ) {
+                const float* f = F + (int64_t)i * fstride;
+                for (int d = 0; d < D; ++d) fQ[d] += wQ * (double)f[d];
+            }
+            sel_idx[ns] = i; sel_w[ns] = wQ; ++ns;
+            TQ = TQ * (1.0 - (double)a);
+            while (T_test < strat_boundary(k, K, mu, sigma, z_max)) k = k + 1;
+        }
+        if (T_test < b_last || T_test < t_min) break;
+        T = T_test;
+    }
+    if (ns > 0) {
+        const double norm = 1.0 - TQ;
+        if (fQ) for (int d = 0; d < D; ++d) fQ[d] = fQ[d] / norm;
+        for (int s = 0; s < ns; ++s) sel_w[s] = sel_w[s] / norm;
+    } else {
+        TQ = 1.0;
+    }
+    *n_sel_out = ns; *TQ_out = TQ; *n_walked = walked; *margin_out = marg; *stop_margin = smarg;
+    *mu_out = mu; *sigma_out = sigma; *n_dense_out = nd;
+}
+
+void orc_stratified(int64_t npix, const int64_t* pix, const int64_t* off, const int32_t* gid, const float* alpha,
+                    int K, int D, const float* features, int64_t fstride, float t_min, float z_max, float* out_map,
+                    int32_t* sel_idx, double* sel_w, int32_t* n_sel, double* resid_TQ, int32_t* n_walked, double* margin,
+                    double* stop_margin, float* mu, float* sigma, int32_t* n_dense)
+{
+#pragma omp parallel
+    {
+        double* acc = (double*)malloc(sizeof(double) * (size_t)(D > 0 ? D : 1));
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t j = 0; j < npix; ++j) {
+            const int64_t p = pix ? pix[j] : j;
+            const int64_t b = off[p], e = off[p + 1];
+            stratified_ray(e - b, gid + b, alpha + b, K, D, features, fstride, t_min, z_max, features ? acc : NULL,
+                           sel_idx + j * K, sel_w + j * K, n_sel + j, resid_TQ + j, n_walked + j, margin + j, stop_margin + j,
+                           mu + j, sigma + j, n_dense + j);
+            if (features && out_map)
+                for (int d = 0; d < D; ++d) out_map[j * D + d] = (float)acc[d];
+        }
+        free(acc);
     }
 }
 

@@ -258,6 +258,43 @@ def topk(lists: PixelLists, K: int, features: Optional[np.ndarray] = None, t_min
     return TopKOut(out, sel_idx, sel_w, n_sel, rs, gap, sm, nd)
 
 
+@dataclass
+class StratOut:
+    out_map: Optional[np.ndarray]
+    sel_idx: np.ndarray
+    sel_w: np.ndarray
+    n_sel: np.ndarray
+    resid_TQ: np.ndarray
+    n_walked: np.ndarray
+    margin: np.ndarray          # [P] float64 min |T_test - boundary| over the walk
+    stop_margin: np.ndarray     # [P] float64 pass 1: relative distance of the nearest T_test to t_min
+    mu: np.ndarray              # [P] float32 mean of the dense transmittance values
+    sigma: np.ndarray           # [P] float32 their population standard deviation (0: uniform boundaries)
+    n_dense: np.ndarray         # [P] int32 entries the statistics cover
+
+
+def stratified(lists: PixelLists, K: int, features: Optional[np.ndarray] = None, t_min: float = 1e-4, z_max: float = 2.0,
+               pixels: Optional[np.ndarray] = None) -> StratOut:
+    """Stratified-K (reading R18): Algorithm 1 with boundaries mu + sigma z_k."""
+    if K < 1:
+        raise ValueError("K must be >= 1")
+    npix = (len(lists.off) - 1) if pixels is None else len(pixels)
+    pix = None if pixels is None else np.ascontiguousarray(pixels, dtype=np.int64)
+    D = 0; feats = None; out = None; fstride = 0
+    if features is not None:
+        feats = _f32(features)
+        D = feats.shape[1]; fstride = feats.shape[1]
+        out = np.empty((npix, D), np.float32)
+    sel_idx = np.empty((npix, K), np.int32); sel_w = np.empty((npix, K), np.float64)
+    n_sel = np.empty(npix, np.int32); tq = np.empty(npix, np.float64)
+    nw = np.empty(npix, np.int32); mg = np.empty(npix, np.float64); sm = np.empty(npix, np.float64)
+    mu = np.empty(npix, np.float32); sg = np.empty(npix, np.float32); nd = np.empty(npix, np.int32)
+    lib().orc_stratified(C.c_int64(npix), _p(pix), _p(lists.off), _p(lists.gid), _p(lists.alpha), C.c_int(K), C.c_int(D),
+                         _p(feats), C.c_int64(fstride), C.c_float(t_min), C.c_float(z_max), _p(out), _p(sel_idx), _p(sel_w),
+                         _p(n_sel), _p(tq), _p(nw), _p(mg), _p(sm), _p(mu), _p(sg), _p(nd))
+    return StratOut(out, sel_idx, sel_w, n_sel, tq, nw, mg, sm, mu, sg, nd)
+
+
 def backward(sel_idx, sel_w, n_sel, dL_dmap, N: int, rows: Optional[np.ndarray] = None) -> np.ndarray:
     """dL/dF rows (all N, or only `rows`) in fp64 from the selection records of every pixel."""
     sel_idx = np.ascontiguousarray(sel_idx, dtype=np.int32)

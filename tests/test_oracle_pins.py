@@ -652,3 +652,113 @@ def test_topk_limits_and_invariants(orc):
         assert pos == sorted(pos)
     with pytest.raises(ValueError):
         orc.topk(lists, 0, None)                                                  # K = 0 is a domain error
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-3: stratified-K (reading R18)
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ray", _gold("stratified_rays.json")["rays"], ids=lambda r: r["name"][:2])
+def test_stratified_hand_worked(orc, ray):
+    n = len(ray["alphas"])
+    feats = np.eye(n, dtype=np.float32)
+    lists = orc.lists_from_rays([(range(n), ray["alphas"])])
+    t = orc.stratified(lists, ray["K"], feats, t_min=ray["t_min"])
+    ns = len(ray["selected"])
+    assert t.n_dense[0] == len(ray["T"])
+    np.testing.assert_allclose(t.mu[0], ray["mu"], rtol=1e-6)
+    np.testing.assert_allclose(t.sigma[0], ray["sigma"], rtol=2e-5, atol=1e-7)
+    assert t.n_sel[0] == ns and t.sel_idx[0, :ns].tolist() == ray["selected"] and (t.sel_idx[0, ns:] == -1).all()
+    np.testing.assert_allclose(t.sel_w[0, :ns], ray["w_hat"], rtol=1e-6)
+    np.testing.assert_allclose(t.resid_TQ[0], ray["TQ"], rtol=1e-6)
+    np.testing.assert_allclose(t.sel_w[0, :ns] * (1.0 - t.resid_TQ[0]), ray["wQ"], rtol=1e-6)
+    expect = np.zeros(n)
+    expect[ray["selected"]] = ray["w_hat"]
+    np.testing.assert_allclose(t.out_map[0], expect, rtol=1e-6, atol=1e-12)
+
+
+def _stratified_numpy(alphas, K, t_min, z_max=2.0):
+    """Independent restatement: library cumprod / mean / std for the statistics (fp64, then compared through the
+    boundaries' effect), and the level characterisation of Algorithm 1 (selected <=> the number of
+    boundaries below which T lies grows) instead of the sequential listing."""
+    f32 = np.float32
+    a = np.asarray(alphas, f32)
+    T = f32(1.0); Ts = []
+    for x in a:                                   # fp32 decision arithmetic: T_test = T * (1 - a)
+        Tt = f32(T * f32(f32(1.0) - x))
+        if Tt < f32(t_min):
+            break
+        T = Tt; Ts.append(T)
+    nd = len(Ts)
+    S1 = f32(0.0); S2 = f32(0.0)
+    for v in Ts:
+        S1 = f32(S1 + v)
+        S2 = f32(np.float64(v) * np.float64(v) + np.float64(S2))       # fmaf: one rounding
+    if nd:
+        mu = f32(S1 / f32(nd)); var = f32(f32(S2 / f32(nd)) - f32(mu * mu)); sg = f32(np.sqrt(max(var, f32(0.0))))
+    else:
+        mu = sg = f32(0.0)
+    if sg > 0:
+        b = []
+        for k in range(K):
+            z = f32(f32(z_max) * f32(f32(1.0) - f32(f32(2 * (k + 1)) / f32(K + 1))))
+            b.append(min(max(f32(np.float64(sg) * np.float64(z) + np.float64(mu)), f32(0.0)), f32(1.0)))
+        b = np.asarray(b, f32)
+    else:
+        b = np.asarray([f32(1.0) - f32(k + 1) / f32(K + 1) for k in range(K)], f32)
+    level = lambda t: int((t < b).sum())          # boundaries are non-increasing in k
+    sel = []; T = f32(1.0)
+    for s, x in enumerate(a):
+        Tt = f32(T * f32(f32(1.0) - x))
+        if level(Tt) > level(T) if s else level(Tt) > 0:
+            sel.append(s)
+        if Tt < b[-1] or Tt < f32(t_min):
+            break
+        T = Tt
+    return sel, float(mu), float(sg), nd, b
+
+
+def test_stratified_matches_numpy_restatement_on_random_rays(orc):
+    rng = np.random.default_rng(13)
+    rays = []
+    for _ in range(300):
+        n = int(rng.integers(0, 60))
+        rays.append((np.arange(n), np.minimum(0.99, rng.beta(0.7, 2.5, n)).astype(np.float32)))
+    lists = orc.lists_from_rays(rays)
+    for K, t_min in [(1, 0.0), (4, 1e-4), (10, 1e-4), (40, 1e-4), (40, 0.0)]:
+        t = orc.stratified(lists, K, None, t_min=t_min)
+        for p, (_, al) in enumerate(rays):
+            sel, mu, sg, nd, b = _stratified_numpy(al, K, t_min)
+            assert t.n_dense[p] == nd
+            assert t.mu[p] == np.float32(mu) and t.sigma[p] == np.float32(sg), (p, t.mu[p], mu, t.sigma[p], sg)
+            assert t.sel_idx[p, :t.n_sel[p]].tolist() == sel, (K, p)
+            assert (np.diff(b) <= 0).all()                            # boundaries descend with k
+            if sg > 0:
+                assert (b >= max(mu - 2 * sg, 0) - 1e-6).all() and (b <= min(mu + 2 * sg, 1) + 1e-6).all()
+
+
+def test_stratified_statistics_against_library_routines(orc):
+    """mu and sigma are the mean and population standard deviation of the dense transmittance (np.cumprod / mean / std)."""
+    rng = np.random.default_rng(14)
+    rays = [(np.arange(n), rng.uniform(0.02, 0.6, n).astype(np.float32)) for n in rng.integers(2, 40, 100)]
+    t = orc.stratified(orc.lists_from_rays(rays), 8, None, t_min=0.0)
+    for p, (_, al) in enumerate(rays):
+        T = np.cumprod(1.0 - al.astype(np.float64))
+        np.testing.assert_allclose(t.mu[p], T.mean(), rtol=2e-6)
+        np.testing.assert_allclose(t.sigma[p], T.std(), rtol=1e-3, atol=2e-6)     # fp32 E[T^2] - mu^2 cancels
+
+
+def test_stratified_fallback_invariants_and_domain(orc):
+    sc = make_scene("cfg1", seed=3)
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    lists = orc.pixel_lists(sc.cam, proj)
+    t = orc.stratified(lists, 8, sc.features, t_min=1e-4)
+    q = orc.qrender(lists, 8, sc.features)
+    flat = t.sigma == 0                                          # sigma = 0 -> Q-Render's partition (SPEC.md:233), except that the
+    one = flat & (t.n_dense == 1)                                # walk also ends at the dense stop; single-entry rays cannot reach it
+    assert one.sum() > 0
+    assert (t.sel_idx[one] == q.sel_idx[one]).all() and np.allclose(t.out_map[one], q.out_map[one])
+    assert (t.n_sel <= 8).all() and (t.n_sel >= 0).all()
+    np.testing.assert_allclose(t.sel_w.sum(1)[t.n_sel > 0], 1.0, rtol=1e-12)          # Algorithm 1 line 20
+    assert (t.out_map[t.n_sel == 0] == 0).all() and (t.resid_TQ[t.n_sel == 0] == 1).all()     # R8
+    with pytest.raises(ValueError):
+        orc.stratified(lists, 0, None)
