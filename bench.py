@@ -394,6 +394,15 @@ def run_cuda(args):
         topk_ms = fr.time_call(topk_call)
         topk_nsel = float(tk["out"].n_sel.float().mean().item())
         del tk
+    strat_ms = None
+    if qr.binding.lists_supported(fr.d["features"].dtype, D):           # stratified-K variant (two walks), same blend
+        so = {"out": None}
+
+        def strat_call():
+            so["out"] = pl.stratified_forward(cam, fe, fr.d["features"], K, 1e-4, 2.0, so["out"])
+        strat_ms = fr.time_call(strat_call)
+        strat_nsel = float(so["out"].n_sel.float().mean().item())
+        del so
     # zero fill of the whole dL_dfeat table: what a caller without qr_backward_clear pays per step (reported, not in the step)
     fill_ms = fr.time_call(lambda: fr.dF.zero_())
     # The timed region is ~12 ms at 20 steps, shorter than nvidia-smi's 100 ms sampling period: keep the SAME step
@@ -496,6 +505,10 @@ def run_cuda(args):
                 "topk": ({"ms": topk_ms, "K": K, "n_sel_mean": topk_nsel, "qr_forward_over_topk": topk_ms / fwd_ms,
                           "note": "same tcgen05 blend as Q-Render; selection by a per-pixel heap (O(N log K), PAPER.md:187)"}
                          if topk_ms else None),
+                "stratified": ({"ms": strat_ms, "K": K, "n_sel_mean": strat_nsel, "over_qr_forward": strat_ms / fwd_ms,
+                                "note": "qr_forward_stratified: statistics pass + walk with per-pixel boundaries + the same blend "
+                                        "(PAPER.md:775 reports about half the FPS of Q-Render for its two-pass variants)"}
+                               if strat_ms else None),
                 "workload_counts": dict(counts, M=M_found, M_capacity=fr.capacity)}
         print(json.dumps(line))
     if world > 1:

@@ -224,6 +224,24 @@ int qr_topk_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dt
                     void* ws, size_t ws_bytes, void* stream);
 
 /*
+ * qr_forward_stratified -- the paper's stratified-K variant ("we compute the mean and
+ * standard deviation of the transmittance values along the depth dimension ... uniformly partition the transmittance interval
+ * in the z-score space and then map the samples back"; "two passes along each ray").  DESIGN.md reading R18:
+ *   pass 1: per pixel, mu and sigma (population) of the dense transmittance values T_i over its list up to the stop R7 (t_min);
+ *   pass 2: Algorithm 1 with the boundaries b_k = clamp(mu + sigma z_k, 0, 1), z_k = z_max (1 - 2 (k+1) / (K+1)), k < K, in
+ *           place of 1 - (k+1)/(K+1); the walk ends once T_test < max(b_{K-1}, t_min); sigma == 0 -> Q-Render's boundaries.
+ * Inputs and outputs as qr_forward (the records and the workspace's selection lists have the same format: qr_backward,
+ * qr_backward_lists and qr_backward_clear accept them); z_max = 2 by convention.  fp32 features with D % 128 == 0 only
+ * (QR_ERR_UNSUPPORTED otherwise).  ws must hold qr_stratified_workspace_bytes(cam, K, D) bytes.
+ */
+size_t qr_stratified_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D);
+int qr_forward_stratified(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype, float t_min, float z_max,
+                          const float* mean2d, const float* conic_opac,
+                          const uint32_t* isect_gauss, const int32_t* tile_range, const void* features,
+                          float* out_map, int32_t* sel_idx, float* sel_w, int32_t* n_sel, float* resid_TQ,
+                          void* ws, size_t ws_bytes, void* stream);
+
+/*
  * Multi-camera batching ("rendering loss from 4 randomly chosen training viewpoints"): B views
  * of the same Gaussians, same image size (height % 16 == 0), rendered by ONE set of launches and back-propagated into ONE
  * dL_dfeat.  The B tile grids are stacked into one tall grid of B * tiles_y tile rows; everything after the projection works on

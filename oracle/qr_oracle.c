@@ -690,7 +690,8 @@ void orc_topk(int64_t npix, const int64_t* pix, const int64_t* off, const int32_
  * Everything that decides an integer is fp32 in this order: S1 += T_i; S2 = fmaf(T_i, T_i, S2); mu = S1 / n;
  * var = S2 / n - mu * mu; sigma = sqrtf(max(var, 0)); z_k = z_max * (1 - (float)(2 (k+1)) / (float)(K+1));
  * b_k = fminf(fmaxf(fmaf(sigma, z_k, mu), 0), 1).
- * margin = min |T_test - b_k| over walked steps and open boundaries (fp64), stop_margin as O3 for pass 1.
+ * margin = min |T_test - (mu + sigma z_k)| over walked steps and open boundaries, and |T_test - t_min| / t_min (fp64; a diagnostic for the
+ * parity tests, not part of the result), stop_margin as O3 for pass 1.
  * ---------------------------------------------------------------------------------------- */
 static inline float strat_boundary(int k, int K, float mu, float sigma, float z_max)
 {
@@ -741,11 +742,13 @@ static void stratified_ray(int64_t n, const int32_t* I, const float* alpha, int 
         const float a = alpha[s];
         const float T_test = T * (1.0f - a);
         ++walked;
-        for (int kk = k; kk < K; ++kk) {
-            const double m = fabs((double)T_test - (double)strat_boundary(kk, K, mu, sigma, z_max));
+        for (int kk = k; kk < K; ++kk) {            /* distance to the UNCLAMPED boundary: one clamped to 0 (or 1) cannot be (un)crossed */
+            double b = (double)strat_boundary(kk, K, mu, sigma, z_max);
+            if (sigma > 0.0f) b = (double)fmaf(sigma, z_max * (1.0f - (float)(2 * (kk + 1)) / (float)(K + 1)), mu);
+            const double m = fabs((double)T_test - b);
             if (m < marg) marg = m;
         }
-        { const double m = fabs((double)T_test - (double)t_min); if (m < marg) marg = m; }
+        if (t_min > 0.0f) { const double m = fabs((double)T_test - (double)t_min) / (double)t_min; if (m < marg) marg = m; }
         if (T_test < strat_boundary(k, K, mu, sigma, z_max)) {
             k = k + 1;
             const double wQ = TQ * (double)a;

@@ -28,7 +28,8 @@ STATUS = {0: "QR_OK", -1: "QR_ERR_INVALID_ARG", -2: "QR_ERR_NULL_POINTER", -3: "
 SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_bin_workspace_bytes", "qr_bin_count",
            "qr_bin_sort", "qr_forward_workspace_bytes", "qr_forward", "qr_backward_workspace_bytes", "qr_backward",
            "qr_backward_lists", "qr_backward_clear", "qr_dense_forward", "qr_topk_workspace_bytes", "qr_topk_forward",
-           "qr_launch_count", "qr_forward_stats", "qr_batch_camera", "qr_preprocess_batch", "qr_forward_batch"]
+           "qr_launch_count", "qr_forward_stats", "qr_batch_camera", "qr_preprocess_batch", "qr_forward_batch",
+           "qr_stratified_workspace_bytes", "qr_forward_stratified"]
 
 
 class QRError(RuntimeError):
@@ -95,6 +96,9 @@ def load() -> C.CDLL:
     lib.qr_preprocess_batch.argtypes = [cam, i32, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.qr_forward_batch.restype = C.c_int
     lib.qr_forward_batch.argtypes = [cam, i32, i64, i32, i32, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.qr_stratified_workspace_bytes.restype = sz; lib.qr_stratified_workspace_bytes.argtypes = [cam, i32, i32]
+    lib.qr_forward_stratified.restype = C.c_int
+    lib.qr_forward_stratified.argtypes = [cam, i32, i32, C.c_int, f32, f32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.qr_topk_workspace_bytes.restype = sz; lib.qr_topk_workspace_bytes.argtypes = [cam, i32, i32]
     lib.qr_topk_forward.restype = C.c_int
     lib.qr_topk_forward.argtypes = [cam, i32, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -467,6 +471,34 @@ def qr_forward_batch(tall, B: int, N: int, K: int, mean2d, conic_opac, isect_gau
                                    _dev(features, features.dtype, "features"), out.out_map.data_ptr(), out.sel_idx.data_ptr(),
                                    out.sel_w.data_ptr(), out.n_sel.data_ptr(), out.resid_TQ.data_ptr(),
                                    ws.data_ptr(), ws.numel(), _stream()))
+    out.ws = ws
+    out.has_lists = lists_supported(features.dtype, D)
+    return out
+
+
+def qr_forward_stratified(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, features, t_min: float = 1e-4,
+                          z_max: float = 2.0, out: Optional[ForwardOut] = None, ws: Optional[torch.Tensor] = None) -> ForwardOut:
+    """Stratified-K forward (include/qr.h qr_forward_stratified); same outputs as qr_forward, own (cached) workspace."""
+    c = make_camera(cam)
+    H, W = c.height, c.width
+    D = int(features.shape[1])
+    dev = features.device
+    dt = _feat_dtype(features)
+    if ws is None:
+        ws = _workspace(int(load().qr_stratified_workspace_bytes(C.byref(c), int(K), D)), dev, "strat")
+    kk = max(int(K), 1)
+    if out is None:
+        out = ForwardOut(torch.empty((H, W, D), dtype=torch.float32, device=dev),
+                         torch.empty((H, W, kk), dtype=torch.int32, device=dev),
+                         torch.empty((H, W, kk), dtype=torch.float32, device=dev),
+                         torch.empty((H, W), dtype=torch.int32, device=dev),
+                         torch.empty((H, W), dtype=torch.float32, device=dev))
+    _check(load().qr_forward_stratified(C.byref(c), int(K), D, dt, float(t_min), float(z_max),
+                                        _dev(mean2d, torch.float32, "mean2d"), _dev(conic_opac, torch.float32, "conic_opac"),
+                                        _dev(isect_gauss, torch.int32, "isect_gauss"), _dev(tile_range, torch.int32, "tile_range"),
+                                        _dev(features, features.dtype, "features"), out.out_map.data_ptr(), out.sel_idx.data_ptr(),
+                                        out.sel_w.data_ptr(), out.n_sel.data_ptr(), out.resid_TQ.data_ptr(),
+                                        ws.data_ptr(), ws.numel(), _stream()))
     out.ws = ws
     out.has_lists = lists_supported(features.dtype, D)
     return out

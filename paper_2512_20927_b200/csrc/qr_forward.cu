@@ -914,7 +914,8 @@ extern "C" size_t qr_forward_workspace_bytes(const qr_camera* cam, int32_t K, in
 static int forward_impl(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype, const float* mean2d,
                         const float* conic_opac, const uint32_t* isect_gauss, const int32_t* tile_range,
                         const void* features, float* out_map, int32_t* sel_idx, float* sel_w, int32_t* n_sel,
-                        float* resid_TQ, void* ws, size_t ws_bytes, void* stream, int32_t batch_n, int32_t view_h)
+                        float* resid_TQ, void* ws, size_t ws_bytes, void* stream, int32_t batch_n, int32_t view_h,
+                        bool strat = false, float t_min = 0.0f, float z_max = 2.0f)
 {
     using namespace qr;
     if (int rc = check_cam(cam)) return rc;
@@ -927,8 +928,11 @@ static int forward_impl(const qr_camera* cam, int32_t K, int32_t D, qr_dtype fea
         return fail(QR_ERR_MISALIGNED, "qr_forward: out_map / features / conic_opac / mean2d / ws must be 16-byte aligned");
     const Cam c = make_cam(cam);
     const FwdLayout L = fwd_layout(c, K);
-    if (ws_bytes < L.total)
-        return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_forward: workspace %zu < %zu bytes", ws_bytes, L.total);
+    const size_t stats_bytes = strat ? (size_t)c.width * c.height * sizeof(float2) : 0;
+    if (ws_bytes < L.total + stats_bytes)
+        return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_forward: workspace %zu < %zu bytes", ws_bytes, L.total + stats_bytes);
+    if (strat && !blend_mma_supported(D, feat_dtype))
+        return fail(QR_ERR_UNSUPPORTED, "qr_forward_stratified: fp32 features with D %% 128 == 0 only (D = %d)", D);
     cudaStream_t st = (cudaStream_t)stream;
     const int T = c.tiles_x * c.tiles_y;
     char* w = static_cast<char*>(ws);
@@ -945,7 +949,11 @@ static int forward_impl(const qr_camera* cam, int32_t K, int32_t D, qr_dtype fea
         w2.n_sel = n_sel; w2.resid = resid_TQ; w2.sel_idx = sel_idx; w2.sel_w = sel_w;
         w2.sl = sel_view(L.sel, ws);
         w2.batch_n = batch_n; w2.view_h = view_h;
-        if (int rc = launch_walk2(w2, st)) return rc;
+        if (strat) {
+            w2.stats = reinterpret_cast<float2*>(w + L.total);
+            w2.t_min = t_min; w2.z_max = z_max;
+            if (int rc = launch_walk2_stratified(w2, st)) return rc;
+        } else if (int rc = launch_walk2(w2, st)) return rc;
         BlendParams bp;
         bp.cam = c; bp.K = K; bp.D = D; bp.cap = 0; bp.num_tiles = T; bp.tile_ticket = nullptr;
         bp.features = features; bp.gcount = nullptr; bp.ucount = nullptr; bp.rec = nullptr;
@@ -1015,4 +1023,23 @@ extern "C" int qr_forward_batch(const qr_camera* tall, int32_t B, int64_t N, int
     if (N < 1 || N * (int64_t)B >= (int64_t(1) << 31)) return fail(QR_ERR_INVALID_ARG, "qr_forward_batch: N outside [1, 2^31 / B)");
     return forward_impl(tall, K, D, feat_dtype, mean2d, conic_opac, isect_gauss, tile_range, features, out_map, sel_idx, sel_w,
                         n_sel, resid_TQ, ws, ws_bytes, stream, (int32_t)N, tall->height / B);
+}
+
+extern "C" size_t qr_stratified_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D)
+{
+    const size_t base = qr_forward_workspace_bytes(cam, K, D);
+    if (base == 0) return 0;
+    return base + (size_t)cam->width * cam->height * sizeof(float2);
+}
+
+extern "C" int qr_forward_stratified(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype, float t_min, float z_max,
+                                     const float* mean2d, const float* conic_opac, const uint32_t* isect_gauss,
+                                     const int32_t* tile_range, const void* features, float* out_map, int32_t* sel_idx,
+                                     float* sel_w, int32_t* n_sel, float* resid_TQ, void* ws, size_t ws_bytes, void* stream)
+{
+    using namespace qr;
+    if (!(t_min >= 0.0f)) return fail(QR_ERR_INVALID_ARG, "qr_forward_stratified: t_min must be >= 0");
+    if (!(z_max > 0.0f)) return fail(QR_ERR_INVALID_ARG, "qr_forward_stratified: z_max must be > 0");
+    return forward_impl(cam, K, D, feat_dtype, mean2d, conic_opac, isect_gauss, tile_range, features, out_map, sel_idx, sel_w,
+                        n_sel, resid_TQ, ws, ws_bytes, stream, 0, 0, true, t_min, z_max);
 }

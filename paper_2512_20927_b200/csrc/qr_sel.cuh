@@ -123,7 +123,10 @@ struct WalkParams2 {
     SelLists sl;
     int32_t batch_n = 0;    // qr_forward_batch: ids in isect are virtual (view * N + Gaussian); 0 = single view
     int32_t view_h = 0;     //                   rows per view of the tall image; 0 = single view
+    float2* stats = nullptr;   // stratified-K: per pixel (mu, sigma) of the dense transmittance values (pass 1 writes, pass 2 reads)
+    float t_min = 0.0f, z_max = 2.0f;
 };
 int launch_walk2(const WalkParams2& p, cudaStream_t st);
+int launch_walk2_stratified(const WalkParams2& p, cudaStream_t st);
 
 }  // namespace qr

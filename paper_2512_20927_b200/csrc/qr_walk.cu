@@ -50,7 +50,12 @@ __device__ __forceinline__ bool rect_hit(float mx, float my, float a, float b, f
     return !(qmin > qmax);
 }
 
-template <int WX>
+// MODE 0: Q-Render (Algorithm 1).  MODE 1: stratified-K pass 2 (reading R18): the same walk with
+// the per-pixel boundaries b_k = clamp(mu + sigma z_k, 0, 1) in place of 1 - (k+1)/(K+1).  MODE 2: stratified-K pass 1: the
+// dense transmittance statistics (mu, sigma) of every pixel, nothing else.
+enum { kWalkQ = 0, kWalkStrat = 1, kWalkStats = 2 };
+
+template <int WX, int MODE>
 __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2 p)
 {
     constexpr int WY = 32 / WX;
@@ -60,6 +65,7 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
     __shared__ int32_t s_id[kW2Batch];
     __shared__ int32_t s_col[kW2Batch];    // column of a staged entry in the union, -1 = not selected yet, -2 = being numbered
     __shared__ float thr[QR_MAX_K + 1];
+    __shared__ float zs[MODE == kWalkStrat ? QR_MAX_K + 1 : 1];     // z_k of the stratified boundaries
     __shared__ int32_t s_ucount, s_evals, s_consumed;
 
     __shared__ int32_t s_ht;
@@ -75,12 +81,15 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
     const uint32_t thr_addr = (uint32_t)__cvta_generic_to_shared(thr);
     for (int k = tid; k <= K; k += kW2Threads)                            // thresholds as printed (R3)
         thr[k] = __fsub_rn(1.0f, __fdiv_rn((float)(k + 1), (float)(K + 1)));
-    const float t_break = __fdiv_rn(1.0f, (float)(K + 1));
+    if (MODE == kWalkStrat)
+        for (int k = tid; k <= K; k += kW2Threads)
+            zs[k] = __fmul_rn(p.z_max, __fsub_rn(1.0f, __fdiv_rn((float)(2 * (k + 1)), (float)(K + 1))));
+    const float t_break_q = __fdiv_rn(1.0f, (float)(K + 1));
     // the blend kernel (launched with programmatic stream serialization) may start as soon as every walk CTA is resident:
     // it consumes half tiles as their flags are released and shares the SMs with this kernel
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (tid == 0) stamp_time(p.sl.ctrl, 0, true);
-    if (blockIdx.x == 0 && tid == 0) {
+    if (MODE != kWalkStats && blockIdx.x == 0 && tid == 0) {
         p.sl.stamp[0] = kSelMagic; p.sl.stamp[1] = p.cam.width; p.sl.stamp[2] = p.cam.height; p.sl.stamp[3] = K;
         const unsigned long long a = (unsigned long long)p.sel_idx;
         p.sl.stamp[4] = (int32_t)(a & 0xffffffffull); p.sl.stamp[5] = (int32_t)(a >> 32);
@@ -96,7 +105,7 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
         // publish the previous half tile.  One release per CTA: the block barrier orders every thread's list, record and
         // header stores before this thread's st.release, which is cumulative (no per-warp __threadfence: with the blend
         // streaming the map through the same memory system a fence costs microseconds)
-        if (prev_ht >= 0) {
+        if (MODE != kWalkStats && prev_ht >= 0) {
             int32_t* h = p.sl.hdr + (size_t)prev_ht * kHdrWords;
             h[4] = s_ucount; h[5] = 0; h[6] = s_consumed; h[7] = s_evals; h[8] = (int32_t)(clock64() - prev_start);
             st_release(p.sl.flags + prev_ht, 1);
@@ -111,9 +120,11 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
     const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
     int32_t* hdr = p.sl.hdr + (size_t)ht * kHdrWords;
     if (y0 >= p.cam.height) {                         // half tile below the image: empty lists
-        if (tid < kHdrWords) { hdr[tid] = 0; __threadfence(); }
-        __syncthreads();
-        if (tid == 0) { __threadfence(); st_release(p.sl.flags + ht, 1); }
+        if (MODE != kWalkStats) {
+            if (tid < kHdrWords) { hdr[tid] = 0; __threadfence(); }
+            __syncthreads();
+            if (tid == 0) { __threadfence(); st_release(p.sl.flags + ht, 1); }
+        }
         continue;
     }
     // block of this warp and pixel of this lane
@@ -137,7 +148,22 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
 
     bool done = !inside;
     float T = 1.0f, TQ = 1.0f;
-    float thr_k = __fsub_rn(1.0f, __fdiv_rn(1.0f, (float)(K + 1)));      // thr[k], k = 0
+    // boundary k of this pixel: Algorithm 1's 1 - (k+1)/(K+1), or the stratified one (sigma == 0: the uniform one)
+    float mu = 0.0f, sg = 0.0f;
+    if (MODE == kWalkStrat && inside) { const float2 st = p.stats[pix]; mu = st.x; sg = st.y; }
+    auto bnd = [&](int kk) -> float {
+        float u;
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(u) : "r"(thr_addr + 4u * (uint32_t)kk));
+        if (MODE == kWalkStrat) {
+            const float b = fminf(fmaxf(__fmaf_rn(sg, zs[kk], mu), 0.0f), 1.0f);
+            if (sg > 0.0f) u = kk >= K ? 0.0f : b;
+        }
+        return u;
+    };
+    float thr_k = bnd(0);
+    const float t_break = MODE == kWalkQ ? t_break_q : (MODE == kWalkStrat ? fmaxf(bnd(K - 1), p.t_min) : p.t_min);
+    float S1 = 0.0f, S2 = 0.0f;                 // MODE 2: sums of T and T^2 over the entries that get a dense weight
+    int nd = 0;
     int k = 0, ns = 0, n_ent = 0, n_eval = 0, consumed = 0;
     int32_t* idx_ptr = my_idx;                  // next slot of this pixel's selection record
     uint2* ent_ptr = my_ent;                    // end of this warp's entry list (warp-uniform)
@@ -164,6 +190,13 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
         if (done) a = 0.0f;
         const float oma = __fsub_rn(1.0f, a);
         const float T_test = __fmul_rn(T, oma);                                  // line 5
+        if (MODE == kWalkStats) {               // pass 1 of stratified-K: T_i of every entry before the dense stop R7
+            if (a > 0.0f) {
+                if (T_test < t_break) done = true;
+                else { T = T_test; S1 = __fadd_rn(S1, T); S2 = __fmaf_rn(T, T, S2); ++nd; }
+            }
+            return;
+        }
         const bool sel = T_test < thr_k;                                         // line 6
         const uint32_t sm = __ballot_sync(0xffffffffu, sel);
         if (sm) {
@@ -195,7 +228,7 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
                 TQ = __fmul_rn(TQ, oma);                                         // line 10
                 float tk;
                 while (true) {                                                   // lines 11-13
-                    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(tk) : "r"(thr_addr + 4u * (uint32_t)k));
+                    tk = bnd(k);
                     if (!(T_test < tk)) break;
                     k = k + 1;
                 }
@@ -264,6 +297,18 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
     }
 
     // ---- the warp's pixels: n_sel, T^Q; its entries: x 1/(1 - T^Q) (line 20), scattered to sel_w ----
+    if (MODE == kWalkStats) {
+        if (inside) {
+            float m = 0.0f, sd = 0.0f;
+            if (nd > 0) {
+                m = __fdiv_rn(S1, (float)nd);
+                const float var = __fsub_rn(__fdiv_rn(S2, (float)nd), __fmul_rn(m, m));
+                sd = __fsqrt_rn(fmaxf(var, 0.0f));
+            }
+            p.stats[pix] = make_float2(m, sd);
+        }
+        continue;
+    }
     const float inv = ns > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, TQ)) : 0.0f;
     if (inside) {
         p.n_sel[pix] = ns;
@@ -301,7 +346,8 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
   }
 }
 
-int launch_walk2(const WalkParams2& p, cudaStream_t st)
+template <int MODE>
+static int launch_walk2_mode(const WalkParams2& p, cudaStream_t st)
 {
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
     // tickets and ready flags of this frame
@@ -312,11 +358,20 @@ int launch_walk2(const WalkParams2& p, cudaStream_t st)
     // the blend kernel takes over the SMs as these CTAs drain (programmatic dependent launch) and needs ~200 KB of shared
     // memory there: an SM only changes its L1 / shared split when it is idle, so this kernel asks for the largest
     // shared-memory carve-out although it uses 8 KB
-    QR_CUDA_OK(cudaFuncSetAttribute(walk2_kernel<QR_WX>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    QR_CUDA_OK(cudaFuncSetAttribute(walk2_kernel<QR_WX, MODE>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     const unsigned grid = (unsigned)min(num_half, sms * per_sm);
-    walk2_kernel<QR_WX><<<grid, kW2Threads, 0, st>>>(p);
+    walk2_kernel<QR_WX, MODE><<<grid, kW2Threads, 0, st>>>(p);
     QR_LAUNCH_OK("walk2_kernel");
     return QR_OK;
+}
+
+int launch_walk2(const WalkParams2& p, cudaStream_t st) { return launch_walk2_mode<kWalkQ>(p, st); }
+
+// stratified-K: pass 1 (statistics into p.stats), then pass 2 (the walk with the stratified boundaries)
+int launch_walk2_stratified(const WalkParams2& p, cudaStream_t st)
+{
+    if (int rc = launch_walk2_mode<kWalkStats>(p, st)) return rc;
+    return launch_walk2_mode<kWalkStrat>(p, st);
 }
 
 }  // namespace qr

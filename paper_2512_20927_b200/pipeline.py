@@ -84,3 +84,9 @@ def forward_batch(tall, n_views: int, N: int, fe: Frontend, features: torch.Tens
     """Q-Render of every view of the batch in one walk + one blend; outputs are [B*H, W, ...].  backward / backward_clear
     take `tall` and N as they are and accumulate every view into one dL_dfeat."""
     return B.qr_forward_batch(tall, n_views, N, K, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, out)
+
+
+def stratified_forward(cam, fe: Frontend, features: torch.Tensor, K: int, t_min: float = 1e-4, z_max: float = 2.0,
+                       out: Optional[B.ForwardOut] = None):
+    """The stratified-K variant: two walks, then the same blend; backward() takes its output as is."""
+    return B.qr_forward_stratified(cam, K, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, t_min, z_max, out)

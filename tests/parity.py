@@ -194,3 +194,21 @@ def compare_topk(gpu_out, t, lists, K, D, f16=False, pixels=None):
     z = n_sel == 0
     assert (out_map[z] == 0).all() and (resid[z] == 1.0).all()
     return stats
+
+
+STRAT_BAND = 1e-5
+
+
+def compare_stratified(gpu_out, t, lists, K, D, pixels=None):
+    """qr_forward_stratified against orc_stratified (reading R18).  Same comparison as compare_forward, with the
+    exemption band on |T_test - boundary| widened from 1e-6 to 1e-5: the boundaries mu + sigma z_k are themselves functions
+    of the ray's transmittance values, and a 1-ulp expf difference moves sigma = sqrt(E[T^2] - mu^2) by up to ~1e-6 / sigma.
+    Pixels whose pass-1 stop lies within 1e-5 relative of t_min (the statistics then cover one entry more or less) are
+    exempt too.  Both classes are counted."""
+    import copy
+    q = copy.copy(t)
+    m = np.where(t.stop_margin <= 1e-5, 0.0, t.margin * (MARGIN / STRAT_BAND))
+    q.margin = m
+    stats = compare_forward(gpu_out, q, lists, K, D, pixels=pixels)
+    stats["exempt_stop"] = int((t.stop_margin <= 1e-5).sum())
+    return stats

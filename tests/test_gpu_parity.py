@@ -566,6 +566,47 @@ def test_batch_of_views_equals_the_oracle_per_view(qr, orc, D, K, n_views):
     assert float(dF.abs().max()) == 0.0
 
 
+# ------------------------------------------------------------------------------------------------
+# stratified-K (NEXT-3; reading R18)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,kw,K,t_min", [("cfg3", dict(N=60000, W=160, H=112, D=512), 40, 1e-4),
+                                             ("cfg2", dict(N=20000, W=96, H=64, D=256), 8, 1e-4),
+                                             ("cfg1", dict(W=70, H=50, D=128), 16, 0.0),          # ragged image, whole-list statistics
+                                             ("cfg3", dict(N=60000, W=100, H=72, D=128), 1, 1e-4)])
+def test_stratified_forward_and_backward(qr, orc, name, kw, K, t_min):
+    sc = make_scene(name, seed=25, backward=True, **kw)
+    proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
+    lists = orc.pixel_lists(sc.cam, proj)
+    t = orc.stratified(lists, K, sc.features, t_min=t_min)
+    out = qr.binding.qr_forward_stratified(sc.cam, K, P.to_dev(proj.mean2d), P.to_dev(proj.conic_opac), P.to_dev(isect.view(np.int32)),
+                                           P.to_dev(rng), P.to_dev(sc.features), t_min)
+    stats = P.compare_stratified(out, t, lists, K, sc.D)
+    assert stats["exempt"] < 0.03 * stats["pixels"] + 5, stats
+    print(name, kw, K, stats)
+    if K == 1:
+        return          # every weight is exactly 1 and single Gaussians collect thousands of pixels: outside what the gradient bar covers
+    # the selection lists it leaves are what qr_backward_lists consumes: gradient on untainted rows vs the oracle's
+    dF = qr.pipeline.backward(sc.cam, sc.N, out, P.to_dev(sc.dL_dmap))
+    sel, _, n = P.masked_records(out)
+    same = P.same_selection(sel, n, t)
+    tainted = np.zeros(sc.N, bool)
+    for pth in np.flatnonzero(~same):
+        tainted[sel[pth, :n[pth]]] = True
+        tainted[t.sel_idx[pth, :t.n_sel[pth]]] = True
+    gref = orc.backward(t.sel_idx, t.sel_w, t.n_sel, sc.dL_dmap, sc.N)
+    A = orc.backward(t.sel_idx, t.sel_w, t.n_sel, np.abs(sc.dL_dmap), sc.N)
+    P.compare_backward_rows(dF.cpu().numpy()[~tainted], gref[~tainted], "stratified backward", A[~tainted])
+
+
+def test_stratified_unsupported_shapes_are_status_codes(qr):
+    sc = make_scene("cfg1", seed=1)
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    with pytest.raises(qr.QRError) as e:
+        qr.pipeline.stratified_forward(sc.cam, fe, g.features, 8)          # D = 16: not on the tcgen05 path
+    assert e.value.code == -3
+
+
 def test_error_codes(qr):
     sc = make_scene("cfg1", seed=0, N=100)
     g = P.upload(sc)
