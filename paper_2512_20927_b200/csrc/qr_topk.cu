@@ -6,9 +6,9 @@
 //   2. keep the K largest (ties -> the earlier list position);
 //   3. re-blend the kept entries in depth order with a fresh transmittance;  4. normalise by 1 - T^top (line 20).
 //
-// topk_select_kernel is the O(N log K) part: CTA = 16x16 tile, thread = pixel.  The tile's list is staged 256 entries at
+// topk_select_kernel is the O(N log K) part: CTA = 16x8 half tile, thread = pixel.  The tile's list is staged 128 entries at
 // a time; every thread evaluates alpha' (rule R4, the fp32 decision arithmetic of DESIGN.md), carries the dense T and
-// keeps the K largest weights in a binary min-heap in local memory, ordered by (weight, later position first) so that
+// keeps the K largest weights in a binary min-heap in shared memory, ordered by (weight, later position first) so that
 // the root is always the entry to drop.  After the walk the heap is sorted by list position (depth order), re-blended
 // and written as selection records (sel_idx, sel_w, n_sel, resid) in qr_forward's format: qr_backward accepts them.
 //
@@ -21,8 +21,8 @@
 
 namespace qr {
 
-constexpr int kTkThreads = 256;
-constexpr int kTkBatch = 256;
+constexpr int kTkThreads = 128;          // CTA = one 16x8-pixel half tile, thread = pixel
+constexpr int kTkBatch = 128;
 
 struct TopkParams {
     Cam cam;
@@ -41,22 +41,40 @@ struct TopkParams {
 // (w1, pos1) is dropped before (w2, pos2): the smaller weight; among equal weights the later list position
 __device__ __forceinline__ bool tk_less(float w1, int p1, float w2, int p2) { return w1 < w2 || (w1 == w2 && p1 > p2); }
 
+// alpha' of a Gaussian at a pixel centre with inclusion rule R4 (0 = not in the pixel's list), the operation order of DESIGN.md 2
+__device__ __forceinline__ float tk_alpha(float fpx, float fpy, float2 xy, float4 co)
+{
+    const float dx = __fsub_rn(fpx, xy.x), dy = __fsub_rn(fpy, xy.y);
+    const float q1 = __fmul_rn(__fmul_rn(co.x, dx), dx);
+    const float q2 = __fmaf_rn(__fmul_rn(co.z, dy), dy, q1);
+    const float q3 = __fmul_rn(__fmul_rn(co.y, dx), dy);
+    const float power = __fmaf_rn(-0.5f, q2, -q3);
+    if (power > 0.0f || power < kPowerMin) return 0.0f;
+    const float a = fminf(kAlphaMax, __fmul_rn(co.w, expf(power)));
+    return a < kAlphaMin ? 0.0f : a;
+}
+
+// The heap lives in SHARED memory, slot-major ([slot][thread]: conflict free), and holds only (weight, list position): 8 K
+// bytes per pixel.  (The first version kept {w, alpha', id, pos} per thread in local memory: 1 KB x 256 threads x 8 CTAs per SM
+// thrashed L1 and the kernel took 1.8 ms at config 3.)  alpha' and the id of the kept entries are recomputed from their list
+// positions after the walk -- the same arithmetic on the same inputs, so the same bits.
 __global__ void __launch_bounds__(kTkThreads) topk_select_kernel(const TopkParams p)
 {
+    extern __shared__ __align__(16) unsigned char tk_smem[];
     __shared__ float4 s_co[kTkBatch];
     __shared__ float2 s_xy[kTkBatch];
-    __shared__ int32_t s_id[kTkBatch];
     const int tid = threadIdx.x;
-    const int tile = blockIdx.x;
-    const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile;
+    const int K = p.K;
+    float* hw = reinterpret_cast<float*>(tk_smem) + tid;                  // hw[i * kTkThreads]
+    int32_t* hp = reinterpret_cast<int32_t*>(tk_smem) + K * kTkThreads + tid;
+    const int ht = blockIdx.x, tile = ht >> 1;
+    const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
     const int px = x0 + (tid & 15), py = y0 + (tid >> 4);
     const bool inside = px < p.cam.width && py < p.cam.height;
     const float fpx = (float)px + 0.5f, fpy = (float)py + 0.5f;          // R5
-    const int K = p.K;
     const int2 range = p.tile_range[tile];
-
-    float hw[QR_TOPK_MAX_K], ha[QR_TOPK_MAX_K];
-    int32_t hid[QR_TOPK_MAX_K], hpos[QR_TOPK_MAX_K];
+#define HW(i) hw[(i) * kTkThreads]
+#define HP(i) hp[(i) * kTkThreads]
     int nh = 0;
     float T = 1.0f;
     bool done = !inside;
@@ -65,27 +83,17 @@ __global__ void __launch_bounds__(kTkThreads) topk_select_kernel(const TopkParam
         if (__syncthreads_and(done)) break;
         {
             const int idx = b0 + tid;
-            int32_t id = -1;
             float4 co = make_float4(0.f, 0.f, 0.f, 0.f);
             float2 xy = make_float2(0.f, 0.f);
-            if (idx < range.y) { id = (int32_t)p.isect[idx]; xy = __ldg(p.mean2d + id); co = __ldg(p.conic_opac + id); }
-            s_id[tid] = id; s_xy[tid] = xy; s_co[tid] = co;
+            if (idx < range.y) { const int32_t id = (int32_t)p.isect[idx]; xy = __ldg(p.mean2d + id); co = __ldg(p.conic_opac + id); }
+            s_xy[tid] = xy; s_co[tid] = co;
         }
         __syncthreads();
         if (done) continue;
         const int nb = min(kTkBatch, range.y - b0);
         for (int e = 0; e < nb; ++e) {
-            const float4 co = s_co[e];
-            const float2 xy = s_xy[e];
-            // alpha' with inclusion rule R4, the operation order of DESIGN.md section 2
-            const float dx = __fsub_rn(fpx, xy.x), dy = __fsub_rn(fpy, xy.y);
-            const float q1 = __fmul_rn(__fmul_rn(co.x, dx), dx);
-            const float q2 = __fmaf_rn(__fmul_rn(co.z, dy), dy, q1);
-            const float q3 = __fmul_rn(__fmul_rn(co.y, dx), dy);
-            const float power = __fmaf_rn(-0.5f, q2, -q3);
-            if (power > 0.0f || power < kPowerMin) continue;
-            const float a = fminf(kAlphaMax, __fmul_rn(co.w, expf(power)));
-            if (a < kAlphaMin) continue;
+            const float a = tk_alpha(fpx, fpy, s_xy[e], s_co[e]);
+            if (a == 0.0f) continue;
             const float T_test = __fmul_rn(T, __fsub_rn(1.0f, a));
             if (T_test < p.t_min) { done = true; break; }                 // R7: stop WITHOUT this entry
             const float w = __fmul_rn(T, a);                              // Eq. 1 weight (step 1)
@@ -94,45 +102,55 @@ __global__ void __launch_bounds__(kTkThreads) topk_select_kernel(const TopkParam
                 int i = nh++;
                 while (i > 0) {
                     const int par = (i - 1) >> 1;
-                    if (!tk_less(w, pos, hw[par], hpos[par])) break;
-                    hw[i] = hw[par]; ha[i] = ha[par]; hid[i] = hid[par]; hpos[i] = hpos[par];
+                    const float pw = HW(par); const int pp = HP(par);
+                    if (!tk_less(w, pos, pw, pp)) break;
+                    HW(i) = pw; HP(i) = pp;
                     i = par;
                 }
-                hw[i] = w; ha[i] = a; hid[i] = s_id[e]; hpos[i] = pos;
-            } else if (w > hw[0]) {                                       // equal to the smallest kept: the earlier one stays
+                HW(i) = w; HP(i) = pos;
+            } else if (w > HW(0)) {                                       // equal to the smallest kept: the earlier one stays
                 int i = 0;
                 while (true) {
                     int c = 2 * i + 1;
                     if (c >= nh) break;
-                    if (c + 1 < nh && tk_less(hw[c + 1], hpos[c + 1], hw[c], hpos[c])) ++c;
-                    if (!tk_less(hw[c], hpos[c], w, pos)) break;
-                    hw[i] = hw[c]; ha[i] = ha[c]; hid[i] = hid[c]; hpos[i] = hpos[c];
+                    float cw = HW(c); int cp = HP(c);
+                    if (c + 1 < nh) {
+                        const float cw2 = HW(c + 1); const int cp2 = HP(c + 1);
+                        if (tk_less(cw2, cp2, cw, cp)) { ++c; cw = cw2; cp = cp2; }
+                    }
+                    if (!tk_less(cw, cp, w, pos)) break;
+                    HW(i) = cw; HP(i) = cp;
                     i = c;
                 }
-                hw[i] = w; ha[i] = a; hid[i] = s_id[e]; hpos[i] = pos;
+                HW(i) = w; HP(i) = pos;
             }
             T = T_test;
         }
     }
     if (!inside) return;
-    // depth order = list position (insertion sort; K <= 64)
+    // depth order = list position (insertion sort on the positions; K <= 64)
     for (int i = 1; i < nh; ++i) {
-        const float a = ha[i]; const int32_t id = hid[i]; const int pos = hpos[i];
+        const int pos = HP(i);
         int j = i - 1;
-        while (j >= 0 && hpos[j] > pos) { ha[j + 1] = ha[j]; hid[j + 1] = hid[j]; hpos[j + 1] = hpos[j]; --j; }
-        ha[j + 1] = a; hid[j + 1] = id; hpos[j + 1] = pos;
+        while (j >= 0 && HP(j) > pos) { HP(j + 1) = HP(j); --j; }
+        HP(j + 1) = pos;
     }
-    // steps 3, 4: fresh transmittance, normalise
-    float Tt = 1.0f;
-    for (int i = 0; i < nh; ++i) { hw[i] = __fmul_rn(Tt, ha[i]); Tt = __fmul_rn(Tt, __fsub_rn(1.0f, ha[i])); }
+    // steps 3, 4: fresh transmittance over the kept entries in depth order, then normalise
     const int64_t pix = (int64_t)py * p.cam.width + px;
-    const float inv = nh > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, Tt)) : 0.0f;
+    float Tt = 1.0f;
     for (int i = 0; i < nh; ++i) {
-        p.sel_idx[pix * K + i] = hid[i];
-        p.sel_w[pix * K + i] = __fmul_rn(hw[i], inv);
+        const int32_t id = (int32_t)p.isect[range.x + HP(i)];
+        const float a = tk_alpha(fpx, fpy, __ldg(p.mean2d + id), __ldg(p.conic_opac + id));
+        HW(i) = __fmul_rn(Tt, a);
+        Tt = __fmul_rn(Tt, __fsub_rn(1.0f, a));
+        p.sel_idx[pix * K + i] = id;
     }
+    const float inv = nh > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, Tt)) : 0.0f;
+    for (int i = 0; i < nh; ++i) p.sel_w[pix * K + i] = __fmul_rn(HW(i), inv);
     p.n_sel[pix] = nh;
     p.resid[pix] = nh > 0 ? Tt : 1.0f;                                    // R8
+#undef HW
+#undef HP
 }
 
 __device__ __forceinline__ float tk_f32(float v) { return v; }
@@ -213,7 +231,9 @@ extern "C" int qr_topk_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dt
     tp.conic_opac = reinterpret_cast<const float4*>(conic_opac);
     tp.isect = isect_gauss; tp.tile_range = reinterpret_cast<const int2*>(tile_range);
     tp.n_sel = n_sel; tp.resid = resid; tp.sel_idx = sel_idx; tp.sel_w = sel_w;
-    topk_select_kernel<<<(unsigned)T, kTkThreads, 0, st>>>(tp);
+    const size_t heap_bytes = (size_t)K * kTkThreads * 8;                  // <= 64 KB at K = 64
+    QR_CUDA_OK(cudaFuncSetAttribute(topk_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)heap_bytes));
+    topk_select_kernel<<<(unsigned)T * 2u, kTkThreads, heap_bytes, st>>>(tp);
     QR_LAUNCH_OK("topk_select_kernel");
 
     const int sms = sm_count();
