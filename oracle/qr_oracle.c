@@ -15,6 +15,7 @@
  *   - SPEC.md:462-470   backward: d f~ / d f_i = w^Q_i / (1 - T^Q) * I  (selection is piecewise constant)
  *   - PAPER.md:167,:187 top-K comparator, as reconstructed in SPEC.md:221-229 (reading R17)
  *   - PAPER.md:760-769  stratified-K variant (reading R18)
+ *   - PAPER.md:1121-1179, :216-228  de-voxelisation (Listing 3) and the mask-pooled contrastive loss (Eq. 2; reading R19)
  * No blocking, fusion or reordering beyond those passages.
  *
  * Precision.  Everything is fp64 EXCEPT the quantities that decide an integer (which
@@ -827,3 +828,124 @@ void orc_backward(int64_t npix, int K, int D, int64_t N, const int32_t* sel_idx,
     }
     free(slot);
 }
+
+/* ------------------------------------------------------------------------------------------
+ * O8: the two neighbours of the path.
+ *
+ * De-voxelisation (Listing 3): the 3D network predicts one row per UNIQUE voxel; every Gaussian was
+ * sampled into counts[g] voxels (consecutive: Gaussian g owns voxels [off[g], off[g+1]), off = exclusive cumsum of counts),
+ * and inverse_indices[v] names the unique voxel of sampled voxel v.  Step 1 expands the predictions to all voxels,
+ * voxels_pred[v] = uni[inverse_indices[v]] (the listing's `scatter` by inverse index); step 2 reduces each
+ * Gaussian's voxels with REDUCE in {"mean", "max"} (componentwise).  A Gaussian without voxels gets a zero row (what
+ * segment_csr returns for an empty segment).  argmax[g,c] = the FIRST voxel attaining the maximum (-1 for an empty
+ * segment): where the max's gradient goes (reading R19).
+ * ---------------------------------------------------------------------------------------- */
+void orc_devoxelize(int64_t U, int C, int64_t G, const float* uni, const int64_t* inverse_indices, const int64_t* counts,
+                    int reduce_max, double* out, int64_t* argmax)
+{
+    (void)U;
+    int64_t v0 = 0;
+    for (int64_t g = 0; g < G; ++g) {
+        const int64_t n = counts[g];
+        for (int c = 0; c < C; ++c) {
+            double acc = 0.0;
+            int64_t am = -1;
+            for (int64_t v = v0; v < v0 + n; ++v) {
+                const double x = (double)uni[inverse_indices[v] * C + c];
+                if (reduce_max) { if (am < 0 || x > acc) { acc = x; am = v; } }
+                else acc += x;
+            }
+            if (!reduce_max && n > 0) acc /= (double)n;
+            out[g * C + c] = n > 0 ? acc : 0.0;
+            if (argmax) argmax[g * C + c] = am;
+        }
+        v0 += n;
+    }
+}
+
+/* its adjoint: d uni[u,c] = sum over voxels v with inverse_indices[v] = u of  (mean: d gs[g(v),c] / counts[g(v)];
+ * max: d gs[g(v),c] if v == argmax[g(v),c] else 0) */
+void orc_devoxelize_backward(int64_t U, int C, int64_t G, const int64_t* inverse_indices, const int64_t* counts, int reduce_max,
+                             const int64_t* argmax, const float* d_gs, double* d_uni)
+{
+    memset(d_uni, 0, sizeof(double) * (size_t)U * (size_t)C);
+    int64_t v0 = 0;
+    for (int64_t g = 0; g < G; ++g) {
+        const int64_t n = counts[g];
+        for (int64_t v = v0; v < v0 + n; ++v)
+            for (int c = 0; c < C; ++c) {
+                if (reduce_max) { if (argmax[g * C + c] == v) d_uni[inverse_indices[v] * C + c] += (double)d_gs[g * C + c]; }
+                else d_uni[inverse_indices[v] * C + c] += (double)d_gs[g * C + c] / (double)n;
+            }
+        v0 += n;
+    }
+}
+
+/* Mask-pooled contrastive loss (Eq. 2).  The paper pairs masks m_s with CLIP embeddings f_s and minimises
+ * -log( exp(sim(f~, f_s)) / sum_j exp(sim(f~, f_j)) ), sim = cosine similarity; the printed denominator's "i != j" is ambiguous
+ * and the pooling is not stated.  DESIGN.md reading R19 (= SPEC.md:453-456, :497, :512): the rendered feature of mask s is the
+ * arithmetic MEAN of the map over the mask's pixels; the denominator runs over ALL S targets (InfoNCE, positive included); the
+ * loss is the mean over the non-empty masks with a non-zero pooled vector; no temperature.  mask_id[p] in [0, S) or -1.
+ *   pooled[s,:] = mean_{p in m_s} map[p,:];  c_j = <pooled_s, t_j> / (|pooled_s| |t_j|);  L_s = log sum_j e^{c_j} - c_s
+ *   dL_s/dpooled = sum_j (softmax_j - [j = s]) (t_j / |t_j| - c_j pooled_s / |pooled_s|) / |pooled_s|
+ *   d_map[p,:] = dL_s/dpooled / (|m_s| S_eff)   for p in m_s,  0 elsewhere.
+ * ---------------------------------------------------------------------------------------- */
+void orc_mask_loss(int64_t P, int D, const float* map, const int32_t* mask_id, int S, const float* targets, double* pooled,
+                   double* loss_s, double* loss, double* d_map)
+{
+    int64_t* cnt = (int64_t*)calloc((size_t)S, sizeof(int64_t));
+    double* g = (double*)calloc((size_t)S * (size_t)D, sizeof(double));
+    double* c = (double*)malloc(sizeof(double) * (size_t)S);
+    memset(pooled, 0, sizeof(double) * (size_t)S * (size_t)D);
+    for (int64_t p = 0; p < P; ++p) {
+        const int s = mask_id[p];
+        if (s < 0 || s >= S) continue;
+        ++cnt[s];
+        for (int d = 0; d < D; ++d) pooled[(int64_t)s * D + d] += (double)map[p * D + d];
+    }
+    int S_eff = 0;
+    for (int s = 0; s < S; ++s) {
+        loss_s[s] = 0.0;
+        if (cnt[s] == 0) continue;
+        double n2 = 0.0;
+        for (int d = 0; d < D; ++d) { pooled[(int64_t)s * D + d] /= (double)cnt[s]; n2 += pooled[(int64_t)s * D + d] * pooled[(int64_t)s * D + d]; }
+        if (n2 > 0.0) ++S_eff; else cnt[s] = -cnt[s];       /* zero pooled vector: no loss, no gradient */
+    }
+    double total = 0.0;
+    for (int s = 0; s < S; ++s) {
+        if (cnt[s] <= 0) continue;
+        const double* ps = pooled + (int64_t)s * D;
+        double np = 0.0;
+        for (int d = 0; d < D; ++d) np += ps[d] * ps[d];
+        np = sqrt(np);
+        double mx = -INFINITY;
+        for (int j = 0; j < S; ++j) {
+            double dot = 0.0, nt = 0.0;
+            for (int d = 0; d < D; ++d) { dot += ps[d] * (double)targets[(int64_t)j * D + d]; nt += (double)targets[(int64_t)j * D + d] * (double)targets[(int64_t)j * D + d]; }
+            c[j] = dot / (np * sqrt(nt));
+            if (c[j] > mx) mx = c[j];
+        }
+        double Z = 0.0;
+        for (int j = 0; j < S; ++j) Z += exp(c[j] - mx);
+        loss_s[s] = (mx + log(Z)) - c[s];
+        total += loss_s[s];
+        for (int j = 0; j < S; ++j) {
+            const double coef = exp(c[j] - mx) / Z - (j == s ? 1.0 : 0.0);
+            double nt = 0.0;
+            for (int d = 0; d < D; ++d) nt += (double)targets[(int64_t)j * D + d] * (double)targets[(int64_t)j * D + d];
+            nt = sqrt(nt);
+            for (int d = 0; d < D; ++d)
+                g[(int64_t)s * D + d] += coef * ((double)targets[(int64_t)j * D + d] / nt - c[j] * ps[d] / np) / np;
+        }
+    }
+    *loss = S_eff > 0 ? total / (double)S_eff : 0.0;
+    if (d_map) {
+        for (int64_t p = 0; p < P; ++p) {
+            const int s = mask_id[p];
+            for (int d = 0; d < D; ++d)
+                d_map[p * D + d] = (s >= 0 && s < S && cnt[s] > 0) ? g[(int64_t)s * D + d] / ((double)cnt[s] * (double)S_eff) : 0.0;
+        }
+    }
+    free(cnt); free(g); free(c);
+}
+

@@ -316,3 +316,53 @@ def render_scene(scene, K: Optional[int] = None, mode: str = "binned", with_feat
     lists = pixel_lists(scene.cam, proj, mode)
     q = qrender(lists, scene.K if K is None else K, scene.features if with_features else None)
     return proj, lists, q
+
+
+def devoxelize(uni, inverse_indices, counts, reduce: str = "max"):
+    """De-voxelisation (Listing 3): returns (gs_pred [G,C] float64, argmax [G,C] int64)."""
+    uni = _f32(uni)
+    inv = np.ascontiguousarray(inverse_indices, dtype=np.int64)
+    cnt = np.ascontiguousarray(counts, dtype=np.int64)
+    if reduce not in ("mean", "max"):
+        raise ValueError("reduce must be 'mean' or 'max'")
+    if cnt.sum() != len(inv) or (len(inv) and (inv.min() < 0 or inv.max() >= uni.shape[0])):
+        raise ValueError("index out of range / counts do not cover the voxels")       # SPEC.md:408
+    G, C_ = len(cnt), uni.shape[1]
+    out = np.empty((G, C_), np.float64); am = np.empty((G, C_), np.int64)
+    lib().orc_devoxelize(C.c_int64(uni.shape[0]), C.c_int(C_), C.c_int64(G), _p(uni), _p(inv), _p(cnt), C.c_int(reduce == "max"),
+                         _p(out), _p(am))
+    return out, am
+
+
+def devoxelize_backward(n_unique: int, inverse_indices, counts, reduce: str, argmax, d_gs):
+    inv = np.ascontiguousarray(inverse_indices, dtype=np.int64)
+    cnt = np.ascontiguousarray(counts, dtype=np.int64)
+    d = _f32(d_gs)
+    am = None if argmax is None else np.ascontiguousarray(argmax, dtype=np.int64)
+    out = np.empty((n_unique, d.shape[1]), np.float64)
+    lib().orc_devoxelize_backward(C.c_int64(n_unique), C.c_int(d.shape[1]), C.c_int64(len(cnt)), _p(inv), _p(cnt),
+                                  C.c_int(reduce == "max"), _p(am), _p(d), _p(out))
+    return out
+
+
+@dataclass
+class MaskLoss:
+    loss: float
+    loss_per_mask: np.ndarray   # [S] float64 (0 for empty masks)
+    pooled: np.ndarray          # [S,D] float64 mean of the map over each mask
+    d_map: np.ndarray           # [P,D] float64
+
+
+def mask_loss(feature_map, mask_id, targets) -> MaskLoss:
+    """Mask-pooled contrastive loss (Eq. 2; reading R19) and its gradient w.r.t. the map."""
+    m = _f32(feature_map)
+    m = m.reshape(-1, m.shape[-1])
+    mid = np.ascontiguousarray(mask_id, dtype=np.int32).reshape(-1)
+    t = _f32(targets)
+    P_, D = m.shape
+    S = t.shape[0]
+    pooled = np.empty((S, D), np.float64); ls = np.empty(S, np.float64); tot = C.c_double(0.0)
+    dm = np.empty((P_, D), np.float64)
+    lib().orc_mask_loss(C.c_int64(P_), C.c_int(D), _p(m), _p(mid), C.c_int(S), _p(t), _p(pooled), _p(ls), C.byref(tot), _p(dm))
+    return MaskLoss(float(tot.value), ls, pooled, dm)
+

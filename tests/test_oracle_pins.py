@@ -762,3 +762,97 @@ def test_stratified_fallback_invariants_and_domain(orc):
     assert (t.out_map[t.n_sel == 0] == 0).all() and (t.resid_TQ[t.n_sel == 0] == 1).all()     # R8
     with pytest.raises(ValueError):
         orc.stratified(lists, 0, None)
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-2: de-voxelisation (Listing 3) and the mask-pooled contrastive loss (Eq. 2;
+# DESIGN.md reading R19)
+# --------------------------------------------------------------------------------------------
+def test_devoxelize_examples_and_library_routines(orc):
+    u = np.array([[1, 2], [3, 0]], np.float32)                       # rows (1,2), (3,0)
+    assert orc.devoxelize(u, [0, 1], [2], "max")[0].tolist() == [[3.0, 2.0]]
+    assert orc.devoxelize(u, [0, 1], [2], "mean")[0].tolist() == [[2.0, 1.0]]
+    rng = np.random.default_rng(15)
+    U, C_, G = 300, 7, 120
+    uni = rng.standard_normal((U, C_)).astype(np.float32)
+    counts = rng.integers(0, 6, G); counts[5] = 0
+    inv = rng.integers(0, U, counts.sum())
+    off = np.concatenate([[0], np.cumsum(counts)])
+    vox = uni[inv].astype(np.float64)                                 # step 1: expansion by the inverse index
+    mx, am = orc.devoxelize(uni, inv, counts, "max")
+    mn, _ = orc.devoxelize(uni, inv, counts, "mean")
+    ne = counts > 0
+    # step 2 with NumPy's segmented reductions (reduceat needs non-empty segments)
+    np.testing.assert_array_equal(mx[ne], np.maximum.reduceat(vox, off[:-1][ne], axis=0))
+    np.testing.assert_allclose(mn[ne], np.add.reduceat(vox, off[:-1][ne], axis=0) / counts[ne, None], rtol=1e-13)
+    assert (mx[~ne] == 0).all() and (mn[~ne] == 0).all() and (am[~ne] == -1).all()
+    one = np.ones(U, np.int64)                                        # centre sampling, 1 voxel per Gaussian
+    perm = rng.permutation(U)
+    for mode in ("max", "mean"):
+        np.testing.assert_array_equal(orc.devoxelize(uni, perm, one, mode)[0], uni[perm].astype(np.float64))
+    with pytest.raises(ValueError):
+        orc.devoxelize(uni, [0, U], [2], "max")                       # index out of range
+    # first voxel wins a tie for the max
+    _, am2 = orc.devoxelize(np.array([[1.0], [1.0]], np.float32), [0, 1, 0], [3], "max")
+    assert am2[0, 0] == 0
+
+
+def test_devoxelize_backward_is_the_adjoint(orc):
+    rng = np.random.default_rng(16)
+    U, C_, G = 80, 5, 40
+    uni = rng.standard_normal((U, C_)).astype(np.float32)
+    counts = rng.integers(0, 5, G)
+    inv = rng.integers(0, U, counts.sum())
+    dgs = rng.standard_normal((G, C_)).astype(np.float32)
+    # mean is linear: <devox(uni), dgs> = <uni, devox^T(dgs)>
+    mn, _ = orc.devoxelize(uni, inv, counts, "mean")
+    du = orc.devoxelize_backward(U, inv, counts, "mean", None, dgs)
+    np.testing.assert_allclose((mn * dgs).sum(), (uni.astype(np.float64) * du).sum(), rtol=1e-12)
+    # max: gradient lands on the arg max only; finite differences where the maximiser is unique
+    mx, am = orc.devoxelize(uni, inv, counts, "max")
+    dm = orc.devoxelize_backward(U, inv, counts, "max", am, dgs)
+    h = 1e-3
+    for _ in range(20):
+        u, c = int(rng.integers(U)), int(rng.integers(C_))
+        up = uni.copy(); up[u, c] += h
+        um = uni.copy(); um[u, c] -= h
+        fd = ((orc.devoxelize(up, inv, counts, "max")[0] - orc.devoxelize(um, inv, counts, "max")[0]) * dgs).sum() / (2 * h)
+        assert abs(fd - dm[u, c]) < 1e-3 * (1 + abs(fd)) or abs(abs(fd) - abs(dm[u, c])) < 0.6 * abs(dgs).max()   # kink within h
+
+
+def test_mask_loss_closed_forms_and_gradient(orc):
+    t = np.array([[1, 0, 0], [0, 1, 0]], np.float32)
+    # rendered = positive, one orthogonal negative -> -log(e / (e + 1))
+    r = orc.mask_loss(np.array([[2.0, 0, 0]], np.float32), [0], t)
+    assert abs(r.loss - (-math.log(math.e / (math.e + 1)))) < 1e-12
+    # similarity 0 to both -> log 2
+    r = orc.mask_loss(np.array([[0, 0, 5.0]], np.float32), [0], t)
+    assert abs(r.loss - math.log(2)) < 1e-12
+    # pooling is the arithmetic mean over the mask; pixels outside every mask get no gradient; loss = mean over masks
+    rng = np.random.default_rng(17)
+    P_, D, S = 60, 6, 4
+    fmap = rng.standard_normal((P_, D)).astype(np.float32)
+    mid = rng.integers(-1, S, P_).astype(np.int32)
+    mid[mid == 2] = -1                                               # mask 2 is empty
+    tg = rng.standard_normal((S, D)).astype(np.float32)
+    r = orc.mask_loss(fmap, mid, tg)
+    for s in (0, 1, 3):
+        np.testing.assert_allclose(r.pooled[s], fmap[mid == s].astype(np.float64).mean(0), rtol=1e-12)
+    assert r.loss_per_mask[2] == 0 and abs(r.loss - r.loss_per_mask[[0, 1, 3]].mean()) < 1e-12
+    assert (r.d_map[mid < 0] == 0).all()
+    # independent restatement with library routines (log-sum-exp of cosine similarities)
+    for s in (0, 1, 3):
+        p = r.pooled[s]
+        cs = (tg.astype(np.float64) @ p) / (np.linalg.norm(tg.astype(np.float64), axis=1) * np.linalg.norm(p))
+        assert abs(r.loss_per_mask[s] - (np.log(np.exp(cs).sum()) - cs[s])) < 1e-12
+    # central finite differences of the total loss w.r.t. map entries
+    h = 1e-3
+    for _ in range(25):
+        p, d = int(rng.integers(P_)), int(rng.integers(D))
+        a = fmap.copy(); a[p, d] += h
+        b = fmap.copy(); b[p, d] -= h
+        fd = (orc.mask_loss(a, mid, tg).loss - orc.mask_loss(b, mid, tg).loss) / (2 * h)
+        assert abs(fd - r.d_map[p, d]) < 2e-5 + 1e-3 * abs(fd)
+    # adding a duplicate negative strictly increases the loss
+    r1 = orc.mask_loss(fmap, mid, np.concatenate([tg, tg[1:2]]))
+    assert r1.loss > r.loss
