@@ -403,6 +403,38 @@ def run_cuda(args):
         strat_ms = fr.time_call(strat_call)
         strat_nsel = float(so["out"].n_sel.float().mean().item())
         del so
+    # the path's neighbours, on synthetic stand-ins of this frame's size: de-voxelisation producing the
+    # [N, D] feature table from ~N unique voxels (2 voxels per Gaussian on average) and the mask-pooled loss over the map
+    nb = None
+    if D % 4 == 0 and sc.feat_dtype == "f32":
+        g = torch.Generator(device=dev).manual_seed(0)
+        U = N
+        uni = torch.randn((U, D), device=dev, generator=g)
+        cnts = torch.randint(0, 5, (N,), device=dev, generator=g, dtype=torch.int32)
+        Mv = int(cnts.sum().item())
+        inv = torch.randint(0, U, (Mv,), device=dev, generator=g, dtype=torch.int64)
+        st_ = {}
+
+        def devox():
+            st_["gs"], st_["am"], st_["ws"] = qr.binding.qr_devoxelize(uni, inv, cnts, "max", st_.get("ws"))
+        devox_ms = fr.time_call(devox)
+        dgs = torch.randn((N, D), device=dev, generator=g)
+        duni = torch.zeros((U, D), device=dev)
+        devox_bwd_ms = fr.time_call(lambda: qr.binding.qr_devoxelize_backward(U, inv, "max", st_["am"], dgs, st_["ws"], duni))
+        S_m = 32
+        ys = torch.arange(H, device=dev)[:, None] // max(H // 4, 1)
+        xs = torch.arange(W, device=dev)[None, :] // max(W // 8, 1)
+        mid = (ys * 8 + xs).clamp(max=S_m - 1).to(torch.int32).contiguous()
+        tg = torch.randn((S_m, D), device=dev, generator=g)
+        dm = torch.empty((H, W, D), dtype=torch.float32, device=dev)
+        loss_ms = fr.time_call(lambda: qr.binding.qr_mask_loss(cam, fr.fwd_out.out_map, mid, tg, dm))
+        devox_bytes = Mv * (D * 4 + 8) + N * D * 4 * 2            # voxel rows gathered + indices, table + argmax written
+        loss_bytes = 2 * npix * D * 4 + npix * 8
+        nb = {"devoxelize_max": {"ms": devox_ms, "voxels": Mv, "unique_voxels": U, "gb_s": devox_bytes / devox_ms / 1e6},
+              "devoxelize_backward_max": {"ms": devox_bwd_ms},
+              "mask_loss": {"ms": loss_ms, "masks": S_m, "gb_s": loss_bytes / loss_ms / 1e6,
+                            "note": "one read of the map + one write of dL/dmap"}}
+        del uni, inv, dgs, duni, dm, st_
     # zero fill of the whole dL_dfeat table: what a caller without qr_backward_clear pays per step (reported, not in the step)
     fill_ms = fr.time_call(lambda: fr.dF.zero_())
     # The timed region is ~12 ms at 20 steps, shorter than nvidia-smi's 100 ms sampling period: keep the SAME step
@@ -509,6 +541,7 @@ def run_cuda(args):
                                 "note": "qr_forward_stratified: statistics pass + walk with per-pixel boundaries + the same blend "
                                         "(PAPER.md:775 reports about half the FPS of Q-Render for its two-pass variants)"}
                                if strat_ms else None),
+                "neighbours": nb,
                 "workload_counts": dict(counts, M=M_found, M_capacity=fr.capacity)}
         print(json.dumps(line))
     if world > 1:

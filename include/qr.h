@@ -38,6 +38,9 @@ extern "C" {
 #define QR_MAX_K 256         /* largest K qr_forward / qr_backward accept */
 #define QR_TOPK_MAX_K 64      /* largest K qr_topk_forward accepts (the paper sweeps 5..50) */
 #define QR_MAX_BATCH 16       /* views per batched call (the paper trains on 4 viewpoints per step) */
+#define QR_MAX_MASKS 2048     /* masks per frame qr_mask_loss accepts */
+#define QR_REDUCE_MEAN 0
+#define QR_REDUCE_MAX 1
 #define QR_MAX_D 512         /* largest feature width ("up to 512-D") */
 
 typedef enum {
@@ -267,6 +270,41 @@ int qr_forward_batch(const qr_camera* tall, int32_t B, int64_t N, int32_t K, int
                      const uint32_t* isect_gauss, const int32_t* tile_range, const void* features,
                      float* out_map, int32_t* sel_idx, float* sel_w, int32_t* n_sel, float* resid_TQ,
                      void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * The two neighbours of the path.
+ *
+ * qr_devoxelize -- PAPER.md:1121-1179 (Listing 3): the 3D network predicts uni_pred[U,C], one row per UNIQUE voxel; Gaussian g
+ * was sampled into num_voxels_per_g[g] consecutive voxels, and inverse_indices[v] names the unique voxel of sampled voxel v.
+ *   gs_pred[g,:] = REDUCE over the voxels v of g of uni_pred[inverse_indices[v],:],  REDUCE = mean or componentwise max
+ * (a Gaussian without voxels gets a zero row).  This is F, the feature table qr_forward reads.  For max, argmax[g,c] receives
+ * the first voxel attaining the maximum (-1: none), which qr_devoxelize_backward needs.  The call also leaves the cumulative
+ * voxel offsets in ws; qr_devoxelize_backward reads them from the same ws.  C <= 512.  Indices are trusted (out of
+ * range is a contract violation).
+ * qr_devoxelize_backward -- the adjoint: d_uni[u,:] += sum over voxels v with inverse_indices[v] == u of d_gs[g(v),:] / count
+ * (mean) or of d_gs[g(v),c] where v == argmax[g(v),c] (max).  d_gs is dL/dF as qr_backward produces it; d_uni is ACCUMULATED INTO.
+ */
+size_t qr_devoxelize_workspace_bytes(int64_t G);
+int qr_devoxelize(int64_t U, int32_t C, int64_t G, const float* uni_pred, const int64_t* inverse_indices,
+                  const uint32_t* num_voxels_per_g, int32_t reduce, float* gs_pred, int32_t* argmax,
+                  void* ws, size_t ws_bytes, void* stream);
+int qr_devoxelize_backward(int64_t U, int32_t C, int64_t G, const int64_t* inverse_indices, int32_t reduce,
+                           const int32_t* argmax, const float* d_gs, float* d_uni,
+                           const void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * qr_mask_loss -- the training loss of PAPER.md:216-228 (Eq. 2) on a rendered map, and its gradient dL/dmap (the input of
+ * qr_backward).  DESIGN.md reading R19 (the printed denominator and the pooling are ambiguous):
+ *   pooled_s = mean of map over the pixels p with mask_id[p] == s;  c_j = cos(pooled_s, targets[j]);
+ *   L_s = log sum_j exp(c_j) - c_s  (all S targets in the denominator);  L = mean of L_s over masks with pixels and pooled_s != 0.
+ *   in : map[H,W,D] fp32, mask_id[H,W] int32 in [0, S) or -1, targets[S,D] fp32 (any non-zero norm)
+ *   out: loss[1] (device), loss_per_mask[S] (0 for skipped masks), d_map[H,W,D] = dL/dmap (0 outside every mask)
+ * D % 4 == 0, D <= 512, S <= QR_MAX_MASKS.  ws must hold qr_mask_loss_workspace_bytes(S, D) bytes.
+ */
+size_t qr_mask_loss_workspace_bytes(int32_t S, int32_t D);
+int qr_mask_loss(const qr_camera* cam, int32_t D, int32_t S, const float* map, const int32_t* mask_id,
+                 const float* targets, float* loss, float* loss_per_mask, float* d_map,
+                 void* ws, size_t ws_bytes, void* stream);
 
 #ifdef __cplusplus
 }

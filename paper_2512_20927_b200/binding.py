@@ -29,7 +29,8 @@ SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_b
            "qr_bin_sort", "qr_forward_workspace_bytes", "qr_forward", "qr_backward_workspace_bytes", "qr_backward",
            "qr_backward_lists", "qr_backward_clear", "qr_dense_forward", "qr_topk_workspace_bytes", "qr_topk_forward",
            "qr_launch_count", "qr_forward_stats", "qr_batch_camera", "qr_preprocess_batch", "qr_forward_batch",
-           "qr_stratified_workspace_bytes", "qr_forward_stratified"]
+           "qr_stratified_workspace_bytes", "qr_forward_stratified", "qr_devoxelize_workspace_bytes", "qr_devoxelize",
+           "qr_devoxelize_backward", "qr_mask_loss_workspace_bytes", "qr_mask_loss"]
 
 
 class QRError(RuntimeError):
@@ -99,6 +100,12 @@ def load() -> C.CDLL:
     lib.qr_stratified_workspace_bytes.restype = sz; lib.qr_stratified_workspace_bytes.argtypes = [cam, i32, i32]
     lib.qr_forward_stratified.restype = C.c_int
     lib.qr_forward_stratified.argtypes = [cam, i32, i32, C.c_int, f32, f32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.qr_devoxelize_workspace_bytes.restype = sz; lib.qr_devoxelize_workspace_bytes.argtypes = [i64]
+    lib.qr_devoxelize.restype = C.c_int; lib.qr_devoxelize.argtypes = [i64, i32, i64, vp, vp, vp, i32, vp, vp, vp, sz, vp]
+    lib.qr_devoxelize_backward.restype = C.c_int
+    lib.qr_devoxelize_backward.argtypes = [i64, i32, i64, vp, i32, vp, vp, vp, vp, sz, vp]
+    lib.qr_mask_loss_workspace_bytes.restype = sz; lib.qr_mask_loss_workspace_bytes.argtypes = [i32, i32]
+    lib.qr_mask_loss.restype = C.c_int; lib.qr_mask_loss.argtypes = [cam, i32, i32, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.qr_topk_workspace_bytes.restype = sz; lib.qr_topk_workspace_bytes.argtypes = [cam, i32, i32]
     lib.qr_topk_forward.restype = C.c_int
     lib.qr_topk_forward.argtypes = [cam, i32, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -502,3 +509,51 @@ def qr_forward_stratified(cam, K: int, mean2d, conic_opac, isect_gauss, tile_ran
     out.ws = ws
     out.has_lists = lists_supported(features.dtype, D)
     return out
+
+
+REDUCE = {"mean": 0, "max": 1}
+
+
+def qr_devoxelize(uni_pred, inverse_indices, num_voxels_per_g, reduce: str = "max", ws: Optional[torch.Tensor] = None):
+    """De-voxelisation (include/qr.h qr_devoxelize; PAPER.md Listing 3).  Returns (gs_pred [G,C], argmax [G,C] or None, ws);
+    pass argmax and ws to qr_devoxelize_backward."""
+    U, Cn = int(uni_pred.shape[0]), int(uni_pred.shape[1])
+    G = int(num_voxels_per_g.shape[0])
+    dev = uni_pred.device
+    if ws is None:
+        ws = torch.empty((max(int(load().qr_devoxelize_workspace_bytes(G)), 256),), dtype=torch.uint8, device=dev)
+    gs = torch.empty((G, Cn), dtype=torch.float32, device=dev)
+    am = torch.empty((G, Cn), dtype=torch.int32, device=dev) if reduce == "max" else None
+    _check(load().qr_devoxelize(U, Cn, G, _dev(uni_pred, torch.float32, "uni_pred"), _dev(inverse_indices, torch.int64, "inverse_indices"),
+                                _dev(num_voxels_per_g, torch.int32, "num_voxels_per_g"), REDUCE[reduce], gs.data_ptr(),
+                                None if am is None else am.data_ptr(), ws.data_ptr(), ws.numel(), _stream()))
+    return gs, am, ws
+
+
+def qr_devoxelize_backward(n_unique: int, inverse_indices, reduce: str, argmax, d_gs, ws: torch.Tensor,
+                           d_uni: Optional[torch.Tensor] = None) -> torch.Tensor:
+    G, Cn = int(d_gs.shape[0]), int(d_gs.shape[1])
+    if d_uni is None:
+        d_uni = torch.zeros((n_unique, Cn), dtype=torch.float32, device=d_gs.device)
+    _check(load().qr_devoxelize_backward(int(n_unique), Cn, G, _dev(inverse_indices, torch.int64, "inverse_indices"), REDUCE[reduce],
+                                         None if argmax is None else _dev(argmax, torch.int32, "argmax"),
+                                         _dev(d_gs, torch.float32, "d_gs"), _dev(d_uni, torch.float32, "d_uni"),
+                                         _dev(ws, torch.uint8, "ws"), ws.numel(), _stream()))
+    return d_uni
+
+
+def qr_mask_loss(cam, feature_map, mask_id, targets, d_map: Optional[torch.Tensor] = None):
+    """Mask-pooled contrastive loss and dL/dmap (include/qr.h qr_mask_loss).  Returns (loss [1], loss_per_mask [S], d_map)."""
+    c = make_camera(cam)
+    D = int(feature_map.shape[-1])
+    S = int(targets.shape[0])
+    dev = feature_map.device
+    ws = _workspace(int(load().qr_mask_loss_workspace_bytes(S, D)), dev, "maskloss")
+    loss = torch.empty((1,), dtype=torch.float32, device=dev)
+    per = torch.empty((S,), dtype=torch.float32, device=dev)
+    if d_map is None:
+        d_map = torch.empty((c.height, c.width, D), dtype=torch.float32, device=dev)
+    _check(load().qr_mask_loss(C.byref(c), D, S, _dev(feature_map, torch.float32, "map"), _dev(mask_id, torch.int32, "mask_id"),
+                               _dev(targets, torch.float32, "targets"), loss.data_ptr(), per.data_ptr(), d_map.data_ptr(),
+                               ws.data_ptr(), ws.numel(), _stream()))
+    return loss, per, d_map

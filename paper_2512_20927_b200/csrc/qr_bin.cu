@@ -391,6 +391,20 @@ tile_sort_kernel(const int32_t* __restrict__ tile_range, int32_t T, int32_t capa
     for (int tile = blockIdx.x; tile < T; tile += gridDim.x) tile_sort_one<BIG>(tile, capacity, tile_range, keys, scratch, isect_gauss, skeys);
 }
 
+// inclusive prefix sum of N uint32 counts into uint64 (used by qr_bin_count and by qr_devoxelize); sums: scan_blocks(N) uint64
+int64_t scan_blocks(int64_t N) { return N > 0 ? (N + kScanChunk - 1) / kScanChunk : 1; }
+int launch_inclusive_scan_u32(const uint32_t* in, int64_t N, uint64_t* out, uint64_t* sums, cudaStream_t st)
+{
+    const unsigned nb = (unsigned)scan_blocks(N);
+    scan_reduce_kernel<<<nb, kScanThreads, 0, st>>>(in, N, sums);
+    QR_LAUNCH_OK("scan_reduce_kernel");
+    scan_sums_kernel<<<1, kScanThreads, 0, st>>>(sums, (int64_t)nb);
+    QR_LAUNCH_OK("scan_sums_kernel");
+    scan_apply_kernel<<<nb, kScanThreads, 0, st>>>(in, N, sums, out);
+    QR_LAUNCH_OK("scan_apply_kernel");
+    return QR_OK;
+}
+
 struct BinLayout {
     size_t keys, scratch, counter, sums, total;
     int64_t nblocks_scan;
@@ -433,13 +447,7 @@ extern "C" int qr_bin_count(int64_t N, const uint32_t* tiles_touched, uint64_t* 
         return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_bin_count: workspace %zu < %zu bytes", ws_bytes, L.keys);
     cudaStream_t st = (cudaStream_t)stream;
     uint64_t* sums = reinterpret_cast<uint64_t*>(static_cast<char*>(ws) + L.sums);
-    const unsigned nb = (unsigned)L.nblocks_scan;
-    scan_reduce_kernel<<<nb, kScanThreads, 0, st>>>(tiles_touched, N, sums);
-    QR_LAUNCH_OK("scan_reduce_kernel");
-    scan_sums_kernel<<<1, kScanThreads, 0, st>>>(sums, L.nblocks_scan);
-    QR_LAUNCH_OK("scan_sums_kernel");
-    scan_apply_kernel<<<nb, kScanThreads, 0, st>>>(tiles_touched, N, sums, offsets);
-    QR_LAUNCH_OK("scan_apply_kernel");
+    if (int rc = launch_inclusive_scan_u32(tiles_touched, N, offsets, sums, st)) return rc;
     uint64_t m = 0;
     QR_CUDA_OK(cudaMemcpyAsync(&m, offsets + (N - 1), sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
     QR_CUDA_OK(cudaStreamSynchronize(st));

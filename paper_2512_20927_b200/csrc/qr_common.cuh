@@ -71,6 +71,10 @@ __host__ __device__ __forceinline__ uint32_t hash32(uint32_t x)
     return x;
 }
 
+// qr_bin.cu: inclusive prefix sum of uint32 counts (three launches); sums = scan_blocks(N) uint64 of scratch
+int64_t scan_blocks(int64_t N);
+int launch_inclusive_scan_u32(const uint32_t* in, int64_t N, uint64_t* out, uint64_t* sums, cudaStream_t st);
+
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 

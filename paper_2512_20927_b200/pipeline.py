@@ -90,3 +90,13 @@ def stratified_forward(cam, fe: Frontend, features: torch.Tensor, K: int, t_min:
                        out: Optional[B.ForwardOut] = None):
     """The stratified-K variant: two walks, then the same blend; backward() takes its output as is."""
     return B.qr_forward_stratified(cam, K, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, t_min, z_max, out)
+
+
+def devoxelize(uni_pred, inverse_indices, num_voxels_per_g, reduce: str = "max"):
+    """Per-unique-voxel predictions -> per-Gaussian feature table (Listing 3); see binding.qr_devoxelize."""
+    return B.qr_devoxelize(uni_pred, inverse_indices, num_voxels_per_g, reduce)
+
+
+def mask_loss(cam, feature_map, mask_id, targets):
+    """Mask-pooled contrastive loss of PAPER.md Eq. 2 and dL/dmap for backward(); see binding.qr_mask_loss."""
+    return B.qr_mask_loss(cam, feature_map, mask_id, targets)

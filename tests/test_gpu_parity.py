@@ -607,6 +607,52 @@ def test_stratified_unsupported_shapes_are_status_codes(qr):
     assert e.value.code == -3
 
 
+# ------------------------------------------------------------------------------------------------
+# the path's neighbours (NEXT-2): de-voxelisation (Listing 3) and the mask-pooled loss (Eq. 2, reading R19)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("U,Cn,G,reduce", [(5000, 512, 3000, "max"), (5000, 512, 3000, "mean"), (300, 7, 1000, "max"), (1, 64, 1, "mean")])
+def test_devoxelize_forward_and_backward(qr, orc, U, Cn, G, reduce):
+    rng = np.random.default_rng(41)
+    uni = rng.standard_normal((U, Cn)).astype(np.float32)
+    counts = rng.integers(0, 9, G).astype(np.int32)
+    counts[G // 2] = 0 if G > 1 else 3
+    inv = rng.integers(0, U, int(counts.sum())).astype(np.int64)
+    ref, am_ref = orc.devoxelize(uni, inv, counts, reduce)
+    gs, am, ws = qr.binding.qr_devoxelize(P.to_dev(uni), P.to_dev(inv), P.to_dev(counts), reduce)
+    got = gs.cpu().numpy()
+    if reduce == "max":
+        assert np.array_equal(got.astype(np.float64), ref)                       # a maximum is exact
+        assert np.array_equal(am.cpu().numpy().astype(np.int64), am_ref)
+    else:
+        assert (np.abs(got - ref) <= P.ATOL + P.RTOL * np.abs(ref)).all()
+    dgs = rng.standard_normal((G, Cn)).astype(np.float32)
+    dref = orc.devoxelize_backward(U, inv, counts, reduce, am_ref if reduce == "max" else None, dgs)
+    du = qr.binding.qr_devoxelize_backward(U, P.to_dev(inv), reduce, am, P.to_dev(dgs), ws).cpu().numpy()
+    assert (np.abs(du - dref) <= P.ATOL + P.RTOL * np.abs(dref)).all()
+
+
+@pytest.mark.parametrize("W,H,D,S", [(96, 64, 128, 12), (70, 50, 512, 5), (64, 64, 16, 40)])
+def test_mask_loss_and_gradient(qr, orc, W, H, D, S):
+    from qr_inputs import make_camera
+    rng = np.random.default_rng(43)
+    cam = make_camera(W, H)
+    fmap = rng.standard_normal((H, W, D)).astype(np.float32)
+    # blocky masks (spatially coherent, as segmentation masks are), some pixels outside every mask, one mask empty
+    mid = ((np.arange(H)[:, None] // 9) * 7 + (np.arange(W)[None, :] // 11)) % (S + 2) - 1
+    mid[mid >= S] = -1
+    mid[mid == 1] = -1
+    mid = mid.astype(np.int32)
+    tg = rng.standard_normal((S, D)).astype(np.float32)
+    ref = orc.mask_loss(fmap, mid, tg)
+    loss, per, dmap = qr.binding.qr_mask_loss(cam, P.to_dev(fmap), P.to_dev(mid), P.to_dev(tg))
+    assert abs(float(loss.item()) - ref.loss) <= 1e-5 + 1e-4 * abs(ref.loss)
+    np.testing.assert_allclose(per.cpu().numpy(), ref.loss_per_mask, rtol=1e-4, atol=1e-5)
+    got = dmap.cpu().numpy().reshape(-1, D).astype(np.float64)
+    scale = np.abs(ref.d_map).max()                                  # entries are O(1 / (pixels per mask x masks)): compare relative to the map's scale
+    assert (np.abs(got - ref.d_map) <= 1e-4 * scale + 1e-4 * np.abs(ref.d_map)).all()
+    assert (got[mid.reshape(-1) < 0] == 0).all()
+
+
 def test_error_codes(qr):
     sc = make_scene("cfg1", seed=0, N=100)
     g = P.upload(sc)
