@@ -428,12 +428,34 @@ def run_cuda(args):
         tg = torch.randn((S_m, D), device=dev, generator=g)
         dm = torch.empty((H, W, D), dtype=torch.float32, device=dev)
         loss_ms = fr.time_call(lambda: qr.binding.qr_mask_loss(cam, fr.fwd_out.out_map, mid, tg, dm))
+        # the same loss FUSED with the path (qr_pooled_loss: from the selection lists, no map, no dL/dmap), and the training step
+        # built on it: front end, selection-only forward, loss + dL/dF, clear
+        fused = None
+        if fr.fwd_out.has_lists:
+            fused_loss_ms = fr.time_call(lambda: qr.binding.qr_pooled_loss(cam, K, N, fr.fwd_out, fr.d["features"], mid, tg, fr.dF))
+            fr.dF.zero_()
+            sel = {"out": None}
+
+            def fused_step():
+                fe2 = pl.frontend(cam, fr.d["means"], fr.d["scales"], fr.d["quats"], fr.d["opac"], fr.capacity)
+                sel["out"] = pl.forward(cam, fe2, fr.d["features"], K, sel["out"] or fr.fwd_out, select_only=True)
+                qr.binding.qr_pooled_loss(cam, K, N, sel["out"], fr.d["features"], mid, tg, fr.dF)
+                pl.backward_clear(cam, N, sel["out"], fr.dF)
+            fused_step_ms = fr.time_call(fused_step, n=10, warm=3)
+            select_ms = fr.time_call(lambda: pl.forward(cam, fr.fe, fr.d["features"], K, fr.fwd_out, select_only=True))
+            fused = {"qr_pooled_loss_ms": fused_loss_ms, "selection_only_forward_ms": select_ms, "training_step_ms": fused_step_ms,
+                     "unfused_equivalent_ms": ms_step + loss_ms,
+                     "note": "training step with the mask-pooled loss: qr_preprocess, qr_bin_sort, qr_forward(out_map = NULL), "
+                             "qr_pooled_loss (loss + dL/dF), qr_backward_clear -- the map and dL/dmap never exist; unfused = the "
+                             "headline step + qr_mask_loss"}
+            pl.forward(cam, fr.fe, fr.d["features"], K, fr.fwd_out)        # leave a complete forward behind for the counters below
         devox_bytes = Mv * (D * 4 + 8) + N * D * 4 * 2            # voxel rows gathered + indices, table + argmax written
         loss_bytes = 2 * npix * D * 4 + npix * 8
         nb = {"devoxelize_max": {"ms": devox_ms, "voxels": Mv, "unique_voxels": U, "gb_s": devox_bytes / devox_ms / 1e6},
               "devoxelize_backward_max": {"ms": devox_bwd_ms},
               "mask_loss": {"ms": loss_ms, "masks": S_m, "gb_s": loss_bytes / loss_ms / 1e6,
-                            "note": "one read of the map + one write of dL/dmap"}}
+                            "note": "one read of the map + one write of dL/dmap"},
+              "fused": fused}
         del uni, inv, dgs, duni, dm, st_
     # zero fill of the whole dL_dfeat table: what a caller without qr_backward_clear pays per step (reported, not in the step)
     fill_ms = fr.time_call(lambda: fr.dF.zero_())

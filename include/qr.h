@@ -130,6 +130,8 @@ int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M,
  *        sel_w[H,W,K]   fp32 normalised weights w^Q / (1 - T^Q)       the others are left as the caller passed them
  *        n_sel[H,W]     int32 number selected (<= K)                  (writing -1 / 0 there would be two thirds of the
  *        resid_TQ[H,W]  fp32 T^Q after the walk (1 where nothing is selected)     records' traffic, for no reader)
+ * out_map may be NULL on the tcgen05 path (fp32, D % 128 == 0): selection only -- the walk, the records and the selection
+ * lists, no blend, no map (what qr_pooled_loss needs).
  * K in [1, QR_MAX_K]; D in [1, QR_MAX_D]; D % 4 == 0 unless D <= 128; fp16 needs D % 8 == 0.
  * ws must hold qr_forward_workspace_bytes(cam, K, D) bytes; every pointer must be non-NULL.  For fp32 features with
  * D % 128 == 0 (the tcgen05 path) the call leaves in ws, per 16x8-pixel half tile, the numbered union of selected
@@ -305,6 +307,23 @@ size_t qr_mask_loss_workspace_bytes(int32_t S, int32_t D);
 int qr_mask_loss(const qr_camera* cam, int32_t D, int32_t S, const float* map, const int32_t* mask_id,
                  const float* targets, float* loss, float* loss_per_mask, float* d_map,
                  void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * qr_pooled_loss -- qr_mask_loss and qr_backward FUSED with the render path, without the map ("would let
+ * qr_forward / qr_backward skip the 629 MB map round-trip").  Rendering is linear in the features and the loss pools the map by
+ * a mean per mask, so with A[i,s] = sum over the pixels p of mask s of the normalised weight of Gaussian i at p,
+ *     pooled_s = (1 / |m_s|) sum_i A[i,s] F[i,:]      and      dL/dF[i,:] = sum_s A[i,s] g_s     (g_s = dL/dmap on mask s):
+ * both directions need only A, which the selection lists of the last qr_forward(cam, K, D, QR_F32, ...) in fwd_ws give per
+ * half tile.  Same loss, per-mask losses and gradient as qr_mask_loss on that forward's map followed by qr_backward on its
+ * dL/dmap (to rounding), at a fraction of the traffic: neither out_map nor dL/dmap is read or written (call qr_forward with
+ * out_map = NULL for a training step).
+ *   in : fwd_ws (only read; stamp checked on the device as in qr_backward_lists), features[N,D] fp32, mask_id[H,W], targets[S,D]
+ *   out: loss[1], loss_per_mask[S]; dL_dfeat[N,D] ACCUMULATED INTO (may be NULL: loss only)
+ * fp32, D % 128 == 0, D <= 512.  ws must hold qr_mask_loss_workspace_bytes(S, D) bytes.
+ */
+int qr_pooled_loss(const qr_camera* cam, int32_t K, int32_t D, int64_t N, void* fwd_ws, size_t fwd_ws_bytes,
+                   const float* features, const int32_t* mask_id, int32_t S, const float* targets,
+                   float* loss, float* loss_per_mask, float* dL_dfeat, void* ws, size_t ws_bytes, void* stream);
 
 #ifdef __cplusplus
 }

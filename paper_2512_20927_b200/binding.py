@@ -30,7 +30,7 @@ SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_b
            "qr_backward_lists", "qr_backward_clear", "qr_dense_forward", "qr_topk_workspace_bytes", "qr_topk_forward",
            "qr_launch_count", "qr_forward_stats", "qr_batch_camera", "qr_preprocess_batch", "qr_forward_batch",
            "qr_stratified_workspace_bytes", "qr_forward_stratified", "qr_devoxelize_workspace_bytes", "qr_devoxelize",
-           "qr_devoxelize_backward", "qr_mask_loss_workspace_bytes", "qr_mask_loss"]
+           "qr_devoxelize_backward", "qr_mask_loss_workspace_bytes", "qr_mask_loss", "qr_pooled_loss"]
 
 
 class QRError(RuntimeError):
@@ -106,6 +106,8 @@ def load() -> C.CDLL:
     lib.qr_devoxelize_backward.argtypes = [i64, i32, i64, vp, i32, vp, vp, vp, vp, sz, vp]
     lib.qr_mask_loss_workspace_bytes.restype = sz; lib.qr_mask_loss_workspace_bytes.argtypes = [i32, i32]
     lib.qr_mask_loss.restype = C.c_int; lib.qr_mask_loss.argtypes = [cam, i32, i32, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.qr_pooled_loss.restype = C.c_int
+    lib.qr_pooled_loss.argtypes = [cam, i32, i32, i64, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, sz, vp]
     lib.qr_topk_workspace_bytes.restype = sz; lib.qr_topk_workspace_bytes.argtypes = [cam, i32, i32]
     lib.qr_topk_forward.restype = C.c_int
     lib.qr_topk_forward.argtypes = [cam, i32, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -260,7 +262,8 @@ def _workspace(nbytes: int, dev, tag: str = "") -> torch.Tensor:
 
 
 def qr_forward(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, features,
-               out: Optional[ForwardOut] = None, ws: Optional[torch.Tensor] = None) -> ForwardOut:
+               out: Optional[ForwardOut] = None, ws: Optional[torch.Tensor] = None, select_only: bool = False) -> ForwardOut:
+    """select_only: pass out_map = NULL (tcgen05 path): the walk, the records and the selection lists, no blend, no map."""
     c = make_camera(cam)
     H, W = c.height, c.width
     D = int(features.shape[1])
@@ -284,8 +287,8 @@ def qr_forward(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, feature
     _check(load().qr_forward(C.byref(c), int(K), D, dt, _dev(mean2d, torch.float32, "mean2d"),
                              _dev(conic_opac, torch.float32, "conic_opac"),
                              _dev(isect_gauss, torch.int32, "isect_gauss"), _dev(tile_range, torch.int32, "tile_range"),
-                             _dev(features, features.dtype, "features"), out.out_map.data_ptr(), out.sel_idx.data_ptr(),
-                             out.sel_w.data_ptr(), out.n_sel.data_ptr(), out.resid_TQ.data_ptr(),
+                             _dev(features, features.dtype, "features"), None if select_only else out.out_map.data_ptr(),
+                             out.sel_idx.data_ptr(), out.sel_w.data_ptr(), out.n_sel.data_ptr(), out.resid_TQ.data_ptr(),
                              ws.data_ptr(), ws.numel(), _stream()))
     out.ws = ws
     out.has_lists = lists_supported(features.dtype, D)
@@ -557,3 +560,24 @@ def qr_mask_loss(cam, feature_map, mask_id, targets, d_map: Optional[torch.Tenso
                                _dev(targets, torch.float32, "targets"), loss.data_ptr(), per.data_ptr(), d_map.data_ptr(),
                                ws.data_ptr(), ws.numel(), _stream()))
     return loss, per, d_map
+
+
+def qr_pooled_loss(cam, K: int, N: int, fwd: ForwardOut, features, mask_id, targets, dL_dfeat: Optional[torch.Tensor] = None,
+                   with_grad: bool = True):
+    """The mask-pooled loss and dL/dF straight from the forward's selection lists, without the map (include/qr.h
+    qr_pooled_loss).  Returns (loss [1], loss_per_mask [S], dL_dfeat or None)."""
+    if not fwd.has_lists or fwd.ws is None:
+        raise QRError(-3, "qr_pooled_loss needs the workspace of a forward on the tcgen05 path")
+    c = make_camera(cam)
+    D = int(features.shape[1])
+    S = int(targets.shape[0])
+    dev = features.device
+    ws = _workspace(int(load().qr_mask_loss_workspace_bytes(S, D)), dev, "maskloss")
+    loss = torch.empty((1,), dtype=torch.float32, device=dev)
+    per = torch.empty((S,), dtype=torch.float32, device=dev)
+    if with_grad and dL_dfeat is None:
+        dL_dfeat = torch.zeros((N, D), dtype=torch.float32, device=dev)
+    _check(load().qr_pooled_loss(C.byref(c), int(K), D, int(N), fwd.ws.data_ptr(), fwd.ws.numel(), _dev(features, torch.float32, "features"),
+                                 _dev(mask_id, torch.int32, "mask_id"), S, _dev(targets, torch.float32, "targets"), loss.data_ptr(),
+                                 per.data_ptr(), dL_dfeat.data_ptr() if with_grad else None, ws.data_ptr(), ws.numel(), _stream()))
+    return loss, per, (dL_dfeat if with_grad else None)

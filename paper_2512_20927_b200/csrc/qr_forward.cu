@@ -922,8 +922,11 @@ static int forward_impl(const qr_camera* cam, int32_t K, int32_t D, qr_dtype fea
     if (K < 1) return fail(QR_ERR_INVALID_ARG, "qr_forward: K = %d < 1 (SPEC.md:215)", K);
     if (K > QR_MAX_K) return fail(QR_ERR_UNSUPPORTED, "qr_forward: K = %d > QR_MAX_K", K);
     if (int rc = check_feat(D, feat_dtype, "qr_forward")) return rc;
-    if (!tile_range || !out_map || !sel_idx || !sel_w || !n_sel || !resid_TQ || !ws)
+    if (!tile_range || !sel_idx || !sel_w || !n_sel || !resid_TQ || !ws)
         return fail(QR_ERR_NULL_POINTER, "qr_forward: NULL output, tile_range or workspace");
+    // out_map == NULL: selection only (walk, records, selection lists; no blend) -- the tcgen05 path only
+    if (!out_map && !blend_mma_supported(D, feat_dtype))
+        return fail(QR_ERR_NULL_POINTER, "qr_forward: out_map is NULL (selection only needs fp32 features with D %% 128 == 0)");
     if (!aligned16(out_map) || !aligned16(features) || !aligned16(conic_opac) || !aligned16(mean2d) || !aligned16(ws))
         return fail(QR_ERR_MISALIGNED, "qr_forward: out_map / features / conic_opac / mean2d / ws must be 16-byte aligned");
     const Cam c = make_cam(cam);
@@ -954,6 +957,7 @@ static int forward_impl(const qr_camera* cam, int32_t K, int32_t D, qr_dtype fea
             w2.t_min = t_min; w2.z_max = z_max;
             if (int rc = launch_walk2_stratified(w2, st)) return rc;
         } else if (int rc = launch_walk2(w2, st)) return rc;
+        if (!out_map) return QR_OK;             // selection only: qr_pooled_loss / qr_backward_lists consume the lists
         BlendParams bp;
         bp.cam = c; bp.K = K; bp.D = D; bp.cap = 0; bp.num_tiles = T; bp.tile_ticket = nullptr;
         bp.features = features; bp.gcount = nullptr; bp.ucount = nullptr; bp.rec = nullptr;

@@ -406,3 +406,225 @@ extern "C" int qr_mask_loss(const qr_camera* cam, int32_t D, int32_t S, const fl
     QR_LAUNCH_OK("mask_dmap_kernel");
     return QR_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// The loss fused with the render path ("would let qr_forward / qr_backward skip the 629 MB map
+// round-trip").  Rendering is linear in the features and the loss pools the map by a MEAN over each mask, so
+//     pooled_s = (1 / |m_s|) sum_{p in m_s} f~(p) = (1 / |m_s|) sum_i A[i,s] F[i,:],   A[i,s] = sum_{p in m_s} w^_{p,i}
+//     dL/dF[i,:] = sum_p w^_{p,i} dL/dmap[p,:] = sum_s A[i,s] g_s,                      g_s = dL/dmap of every pixel of m_s
+// i.e. both directions need only the small matrix A (selected Gaussians x masks), which the walk's selection lists give
+// per half tile, and neither the map nor dL/dmap has to exist.  pooled_lists_kernel builds, per 16x8 half tile, A restricted
+// to the half tile's union (columns) and the masks present in its 128 pixels (a handful), in shared memory, and then either
+// accumulates the pooled sums (FWD: one feature row read per column, from L2) or scatters the gradient (BWD: one 16-byte
+// vector reduction per thread and column, the same atomics the tcgen05 backward's epilogue issues).
+// ---------------------------------------------------------------------------------------------------------------
+#include "qr_sel.cuh"
+
+namespace qr {
+
+__device__ __forceinline__ void nb_red(float* dst, float v) { asm volatile("red.global.add.f32 [%0], %1;" ::"l"(dst), "f"(v) : "memory"); }
+
+constexpr int kPlThreads = 128;
+constexpr int kPlMasks = 8;              // masks per round
+constexpr int kPlCols = 256;             // union columns per chunk
+constexpr float kPlFix = 16777216.0f;     // 2^24: weights are accumulated as 32-bit fixed point (see Ahi)
+
+template <bool BWD>
+__global__ void __launch_bounds__(kPlThreads) pooled_lists_kernel(const Cam cam, const int K, const int D, const int S, const int64_t N,
+                                                                  const SelLists sl, const int32_t* __restrict__ mask_id,
+                                                                  const float* __restrict__ features, float* __restrict__ sum,
+                                                                  int32_t* __restrict__ cnt, const float* __restrict__ g,
+                                                                  float* __restrict__ dL_dfeat)
+{
+    // A is accumulated with NATIVE 32-bit integer shared-memory atomics on weights scaled by 2^24 (float and 64-bit atomicAdd on
+    // shared memory are compare-and-swap loops, and ~37 entries hit each cell: half of this kernel's instructions), then
+    // converted.  A cell sums at most 128 weights <= 1: 2^31 fits; the rounding, 2^-25 per entry, is far inside the tolerance.
+    __shared__ uint32_t Ahi[kPlMasks][kPlCols];
+    __shared__ float Ah[kPlMasks][kPlCols];
+    __shared__ int32_t hkey[256];            // tiny hash set: mask id -> local index
+    __shared__ int32_t hloc[256];
+    __shared__ int32_t loc_mask[kHalfPx];    // local index -> mask id
+    __shared__ uint8_t px_loc[kHalfPx];      // pixel -> local mask index (255: none)
+    __shared__ int32_t nm_s;
+    __shared__ int32_t uid_s[kPlCols];       // the chunk's union ids, staged once (a per-column global load chain cost 1 us per column)
+    __shared__ __align__(16) float gs[BWD ? kPlMasks * QR_MAX_D : 4];
+    if (!sel_stamp_ok(sl.stamp, cam, K)) return;
+    const int tid = threadIdx.x;
+    const int ht = blockIdx.x, tile = ht >> 1;
+    const int x0 = (tile % cam.tiles_x) * kTile, y0 = (tile / cam.tiles_x) * kTile + (ht & 1) * 8;
+    if (y0 >= cam.height) return;
+    const int32_t* hdr = sl.hdr + (size_t)ht * kHdrWords;
+    const int U = hdr[4];
+    const int n0 = hdr[0], n1 = hdr[1], n2 = hdr[2], n3 = hdr[3];
+    // masks present in the half tile, numbered locally
+    for (int i = tid; i < 256; i += kPlThreads) hkey[i] = -1;
+    if (tid == 0) nm_s = 0;
+    __syncthreads();
+    {
+        const int px = x0 + (tid & 15), py = y0 + (tid >> 4);
+        int m = -1;
+        if (px < cam.width && py < cam.height) m = mask_id[(int64_t)py * cam.width + px];
+        if (m < 0 || m >= S) m = -1;
+        int loc = 255;
+        // one representative per (warp, mask) inserts: masks are spatially coherent, a warp usually holds one or two
+        const uint32_t peers = __match_any_sync(0xffffffffu, m);
+        const bool leader = (int)(__ffs(peers) - 1) == (tid & 31);
+        if (m >= 0) {
+            if (!BWD && leader) atomicAdd(cnt + m, __popc(peers));
+            uint32_t h = hash32((uint32_t)m) & 255u;
+            if (leader) {
+                while (true) {
+                    const int old = atomicCAS(&hkey[h], -1, m);
+                    if (old == -1) { const int l = atomicAdd(&nm_s, 1); hloc[h] = l; loc_mask[l] = m; break; }
+                    if (old == m) break;
+                    h = (h + 1) & 255u;
+                }
+            }
+            h = __shfl_sync(peers, h, __ffs(peers) - 1);
+            loc = (int)h;
+        }
+        __syncthreads();
+        px_loc[tid] = m >= 0 ? (uint8_t)hloc[loc] : (uint8_t)255;
+    }
+    __syncthreads();
+    const int nm = nm_s;
+    if (U == 0 || nm == 0) return;
+    const uint2* ent = sl.ent + (size_t)ht * kSelLists * sl.qcap;
+    const int32_t* uid = sl.uid + (size_t)ht * sl.ucap;
+    const int nl[4] = { n0, n1, n2, n3 };
+    const int d4 = D >> 2;
+    for (int m0 = 0; m0 < nm; m0 += kPlMasks) {
+        const int nmr = min(kPlMasks, nm - m0);
+        if (BWD) {          // gradient rows of this round's masks
+            for (int i = tid; i < nmr * d4; i += kPlThreads) {
+                const int l = i / d4, c4 = i - l * d4;
+                reinterpret_cast<float4*>(gs + l * QR_MAX_D)[c4] = __ldg(reinterpret_cast<const float4*>(g + (int64_t)loc_mask[m0 + l] * D) + c4);
+            }
+        }
+        for (int c0 = 0; c0 < U; c0 += kPlCols) {
+            const int nc = min(kPlCols, U - c0);
+            for (int i = tid; i < kPlMasks * kPlCols; i += kPlThreads) (&Ahi[0][0])[i] = 0u;
+            for (int i = tid; i < nc; i += kPlThreads) uid_s[i] = __ldg(uid + c0 + i);
+            __syncthreads();
+            for (int q = 0; q < kSelLists; ++q) {              // A[col, mask] += w over the half tile's entries
+                const uint2* lq = ent + (size_t)q * sl.qcap;
+                // consecutive entries of a list are the pixels that selected ONE Gaussian (one column) at one walk step, so a warp's 32
+                // entries fall into a few cells: sum each cell's group with one REDUX and let its first lane do the atomic
+                for (int i0 = (tid & ~31); i0 < nl[q]; i0 += kPlThreads) {
+                    const int i = i0 + (tid & 31);
+                    int cell = -1;
+                    uint32_t fx = 0u;
+                    if (i < nl[q]) {
+                        const uint2 e = __ldg(lq + i);
+                        const int col = sel_col(e.y) - c0;
+                        const int l = (int)px_loc[sel_pixel(e.y)] - m0;
+                        if (col >= 0 && col < nc && l >= 0 && l < nmr) { cell = l * kPlCols + col; fx = __float2uint_rn(__uint_as_float(e.x) * kPlFix); }
+                    }
+                    uint32_t todo = __ballot_sync(0xffffffffu, cell >= 0);
+                    while (todo) {
+                        const int key = __shfl_sync(0xffffffffu, cell, __ffs(todo) - 1);
+                        const uint32_t grp = __ballot_sync(0xffffffffu, cell == key);
+                        const uint32_t sum = __reduce_add_sync(0xffffffffu, cell == key ? fx : 0u);
+                        if ((int)(__ffs(grp) - 1) == (tid & 31)) atomicAdd(&(&Ahi[0][0])[key], sum);
+                        todo &= ~grp;
+                    }
+                }
+            }
+            __syncthreads();
+            for (int i = tid; i < kPlMasks * kPlCols; i += kPlThreads) (&Ah[0][0])[i] = (float)(&Ahi[0][0])[i] * (1.0f / kPlFix);
+            __syncthreads();
+            if (tid < d4) {
+                if (!BWD) {
+                    float4 acc[kPlMasks];
+#pragma unroll
+                    for (int l = 0; l < kPlMasks; ++l) acc[l] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    for (int col0 = 0; col0 < nc; col0 += 4) {           // four feature rows in flight
+                        float4 f[4];
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            const int col = min(col0 + u, nc - 1);
+                            f[u] = __ldg(reinterpret_cast<const float4*>(features + (int64_t)uid_s[col] * D) + tid);
+                        }
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            if (col0 + u < nc) {
+#pragma unroll
+                                for (int l = 0; l < kPlMasks; ++l) {
+                                    const float a = Ah[l][col0 + u];
+                                    acc[l].x = fmaf(a, f[u].x, acc[l].x); acc[l].y = fmaf(a, f[u].y, acc[l].y);
+                                    acc[l].z = fmaf(a, f[u].z, acc[l].z); acc[l].w = fmaf(a, f[u].w, acc[l].w);
+                                }
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int l = 0; l < kPlMasks; ++l) {
+                        if (l < nmr) {
+                            float* dst = sum + (int64_t)loc_mask[m0 + l] * D + 4 * tid;
+                            nb_red(dst, acc[l].x); nb_red(dst + 1, acc[l].y); nb_red(dst + 2, acc[l].z); nb_red(dst + 3, acc[l].w);
+                        }
+                    }
+                } else {
+                    for (int col = 0; col < nc; ++col) {
+                        float4 d = make_float4(0.f, 0.f, 0.f, 0.f);
+                        bool any = false;
+#pragma unroll
+                        for (int l = 0; l < kPlMasks; ++l) {
+                            const float a = Ah[l][col];
+                            if (l < nmr && a != 0.0f) {
+                                const float4 gv = reinterpret_cast<const float4*>(gs + l * QR_MAX_D)[tid];
+                                d.x = fmaf(a, gv.x, d.x); d.y = fmaf(a, gv.y, d.y); d.z = fmaf(a, gv.z, d.z); d.w = fmaf(a, gv.w, d.w);
+                                any = true;
+                            }
+                        }
+                        if (!any) continue;
+                        const int32_t id = uid_s[col];
+                        if ((uint32_t)id >= (uint32_t)N) continue;      // never add outside the table
+                        float* dst = dL_dfeat + (int64_t)id * D + 4 * tid;
+                        nb_red(dst, d.x); nb_red(dst + 1, d.y); nb_red(dst + 2, d.z); nb_red(dst + 3, d.w);
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+
+}  // namespace qr
+
+extern "C" int qr_pooled_loss(const qr_camera* cam, int32_t K, int32_t D, int64_t N, void* fwd_ws, size_t fwd_ws_bytes,
+                              const float* features, const int32_t* mask_id, int32_t S, const float* targets, float* loss,
+                              float* loss_per_mask, float* dL_dfeat, void* ws, size_t ws_bytes, void* stream)
+{
+    using namespace qr;
+    if (int rc = check_cam(cam)) return rc;
+    if (K < 1 || K > QR_MAX_K) return fail(QR_ERR_INVALID_ARG, "qr_pooled_loss: K out of range");
+    if (D < 128 || D % 128 != 0 || D > kNbMaxC) return fail(QR_ERR_UNSUPPORTED, "qr_pooled_loss: needs fp32 features with D %% 128 == 0 (D = %d)", D);
+    if (S < 1 || S > QR_MAX_MASKS) return fail(QR_ERR_INVALID_ARG, "qr_pooled_loss: S = %d outside [1, QR_MAX_MASKS]", S);
+    if (N < 1) return fail(QR_ERR_INVALID_ARG, "qr_pooled_loss: N < 1");
+    if (!fwd_ws || !features || !mask_id || !targets || !loss || !loss_per_mask || !ws) return fail(QR_ERR_NULL_POINTER, "qr_pooled_loss: NULL argument");
+    if (!aligned16(features) || !aligned16(fwd_ws) || !aligned16(ws) || (dL_dfeat && !aligned16(dL_dfeat)))
+        return fail(QR_ERR_MISALIGNED, "qr_pooled_loss: 16-byte alignment");
+    const Cam c = make_cam(cam);
+    const WsLayout wl = ws_layout(c, K);
+    if (fwd_ws_bytes < wl.total) return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_pooled_loss: forward workspace %zu < %zu bytes", fwd_ws_bytes, wl.total);
+    const MaskWs w = mask_ws(ws, S, D);
+    if (ws_bytes < w.total) return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_pooled_loss: workspace %zu < %zu bytes", ws_bytes, w.total);
+    const SelLists sl = sel_view(wl.sel, fwd_ws);
+    cudaStream_t st = (cudaStream_t)stream;
+    const unsigned nh = (unsigned)(c.tiles_x * c.tiles_y * 2);
+    QR_CUDA_OK(cudaMemsetAsync(ws, 0, w.total, st));
+    QR_CUDA_OK(cudaMemsetAsync(loss, 0, sizeof(float), st));
+    pooled_lists_kernel<false><<<nh, kPlThreads, 0, st>>>(c, K, D, S, N, sl, mask_id, features, w.sum, w.cnt, nullptr, nullptr);
+    QR_LAUNCH_OK("pooled_lists_kernel<fwd>");
+    mask_mean_kernel<<<(unsigned)S, 256, 0, st>>>(D, w.sum, w.cnt, w.valid, w.norm);
+    QR_LAUNCH_OK("mask_mean_kernel");
+    const size_t smem = ((size_t)D + 3 * (size_t)S) * 4;
+    mask_grad_kernel<<<(unsigned)S, 256, smem, st>>>(D, S, targets, w.sum, w.cnt, w.valid, w.norm, loss, loss_per_mask);
+    QR_LAUNCH_OK("mask_grad_kernel");
+    if (dL_dfeat) {
+        pooled_lists_kernel<true><<<nh, kPlThreads, 0, st>>>(c, K, D, S, N, sl, mask_id, features, nullptr, nullptr, w.sum, dL_dfeat);
+        QR_LAUNCH_OK("pooled_lists_kernel<bwd>");
+    }
+    return QR_OK;
+}

@@ -36,8 +36,10 @@ def frontend(cam, means, scales, quats, opac, capacity: Optional[int] = None) ->
     return Frontend(proj, None, int(capacity), isect, rng, found)
 
 
-def forward(cam, fe: Frontend, features: torch.Tensor, K: int, out: Optional[B.ForwardOut] = None) -> B.ForwardOut:
-    return B.qr_forward(cam, K, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, out)
+def forward(cam, fe: Frontend, features: torch.Tensor, K: int, out: Optional[B.ForwardOut] = None,
+            select_only: bool = False) -> B.ForwardOut:
+    return B.qr_forward(cam, K, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, out,
+                        select_only=select_only)
 
 
 def backward(cam, N: int, fwd: B.ForwardOut, dL_dmap: torch.Tensor, dL_dfeat: Optional[torch.Tensor] = None,
@@ -100,3 +102,8 @@ def devoxelize(uni_pred, inverse_indices, num_voxels_per_g, reduce: str = "max")
 def mask_loss(cam, feature_map, mask_id, targets):
     """Mask-pooled contrastive loss of PAPER.md Eq. 2 and dL/dmap for backward(); see binding.qr_mask_loss."""
     return B.qr_mask_loss(cam, feature_map, mask_id, targets)
+
+
+def pooled_loss(cam, N: int, fwd: B.ForwardOut, features, mask_id, targets, dL_dfeat=None, with_grad: bool = True):
+    """Loss + dL/dF from the selection lists of `fwd` (which may come from forward(..., select_only=True)): no map round trip."""
+    return B.qr_pooled_loss(cam, int(fwd.sel_idx.shape[-1]), N, fwd, features, mask_id, targets, dL_dfeat, with_grad)

@@ -653,6 +653,42 @@ def test_mask_loss_and_gradient(qr, orc, W, H, D, S):
     assert (got[mid.reshape(-1) < 0] == 0).all()
 
 
+@pytest.mark.parametrize("name,kw,K,S", [("cfg3", dict(N=60000, W=160, H=112, D=512), 40, 9), ("cfg2", dict(N=20000, W=100, H=72, D=128), 16, 30)])
+def test_pooled_loss_equals_loss_on_the_map_then_backward(qr, orc, name, kw, K, S):
+    """qr_pooled_loss (no map, no dL/dmap) against the oracle's unfused chain: Algorithm 1 map -> mask loss -> d_map -> backward;
+    and selection-only forward leaves the same lists as the full forward."""
+    sc = make_scene(name, seed=27, **kw)
+    H, W, D, N = sc.cam.height, sc.cam.width, sc.D, sc.N
+    proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
+    lists = orc.pixel_lists(sc.cam, proj)
+    q = orc.qrender(lists, K, sc.features)
+    r = np.random.default_rng(5)
+    mid = ((np.arange(H)[:, None] // 13) * 5 + (np.arange(W)[None, :] // 17)) % (S + 1) - 1        # blocky masks, -1 = none
+    mid = mid.astype(np.int32)
+    tg = r.standard_normal((S, D)).astype(np.float32)
+    ref = orc.mask_loss(q.out_map, mid, tg)
+    gref = orc.backward(q.sel_idx, q.sel_w, q.n_sel, ref.d_map.astype(np.float32), N)
+    args = (P.to_dev(proj.mean2d), P.to_dev(proj.conic_opac), P.to_dev(isect.view(np.int32)), P.to_dev(rng), P.to_dev(sc.features))
+    out = qr.qr_forward(sc.cam, K, *args, select_only=True)
+    sel, _, n = P.masked_records(out)
+    same = P.same_selection(sel, n, q)
+    assert ((~same) & ~P.exempt_mask(q, lists)).sum() == 0
+    loss, per, dF = qr.binding.qr_pooled_loss(sc.cam, K, N, out, args[4], P.to_dev(mid), P.to_dev(tg))
+    if same.all():           # a differing (exempt) pixel changes its mask's pooled vector: compare only when none differs
+        assert abs(float(loss.item()) - ref.loss) <= 1e-5 + 1e-4 * abs(ref.loss)
+        np.testing.assert_allclose(per.cpu().numpy(), ref.loss_per_mask, rtol=1e-4, atol=1e-5)
+        scale = np.abs(gref).max()
+        assert (np.abs(dF.cpu().numpy() - gref) <= 1e-4 * scale + 1e-4 * np.abs(gref)).all()
+    # against the library's own unfused chain on the same selection (always comparable)
+    full = qr.qr_forward(sc.cam, K, *args)
+    l2, per2, dmap = qr.binding.qr_mask_loss(sc.cam, full.out_map, P.to_dev(mid), P.to_dev(tg))
+    dF2 = qr.pipeline.backward(sc.cam, N, full, dmap)
+    assert abs(float(loss.item()) - float(l2.item())) <= 1e-5 + 1e-4 * abs(float(l2.item()))
+    a, b = dF.cpu().numpy(), dF2.cpu().numpy()
+    assert (np.abs(a - b) <= 2e-4 * np.abs(b).max() + 1e-3 * np.abs(b)).all()
+    print("pooled loss", float(loss.item()), "oracle", ref.loss, "pixels differing", int((~same).sum()))
+
+
 def test_error_codes(qr):
     sc = make_scene("cfg1", seed=0, N=100)
     g = P.upload(sc)
