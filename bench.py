@@ -234,10 +234,66 @@ class Frame:
         self.fe = fe
         return fe
 
-    def timed(self, steps, warmup, barrier, world=1, dist=None):
+    def capture(self):
+        """The step as four CUDA graphs (front end | qr_forward | qr_backward | qr_backward_clear): the same library calls, captured
+        once on a side stream and replayed, so that the ~12 launches and memsets of a step cost four graph launches.  Events are
+        recorded between the replays, so the per-call timings stay live.  Returns False (and the step stays eager) if capture
+        is not possible."""
+        t, pl, d = self.torch, self.pl, self.d
+        try:
+            if self.capacity is None:
+                self.step()
+            t.cuda.synchronize()
+            n0 = self.qr.binding.qr_launch_count()
+            g = [t.cuda.CUDAGraph() for _ in range(4)]
+            pool = t.cuda.graph_pool_handle()
+            with t.cuda.graph(g[0], pool=pool):
+                fe = pl.frontend(self.cam, d["means"], d["scales"], d["quats"], d["opac"], self.capacity)
+            with t.cuda.graph(g[1], pool=pool):
+                self.fwd_out = pl.forward(self.cam, fe, d["features"], self.K, self.fwd_out)
+            ws = None if self.fwd_out.has_lists else self.bws
+            with t.cuda.graph(g[2], pool=pool):
+                pl.backward(self.cam, self.N, self.fwd_out, d["dL_dmap"], self.dF, ws)
+            with t.cuda.graph(g[3], pool=pool):
+                pl.backward_clear(self.cam, self.N, self.fwd_out, self.dF, ws)
+            self.graph_launches = self.qr.binding.qr_launch_count() - n0       # kernels one replayed step launches
+            self.graphs, self.fe, self.found = g, fe, fe.found
+            for _ in range(2):
+                self.step_graph()
+            t.cuda.synchronize()
+            return True
+        except Exception as e:           # noqa: BLE001 -- any failure: stay eager, say why
+            self.graphs = None
+            self.graph_error = repr(e)[:200]
+            t.cuda.synchronize()
+            return False
+
+    def step_graph(self, timers=None):
+        t, g = self.torch, self.graphs
+        g[0].replay()
+        if timers is not None:
+            ev = [t.cuda.Event(enable_timing=True) for _ in range(4)]
+            ev[0].record()
+        g[1].replay()
+        if timers is not None:
+            ev[1].record()
+        g[2].replay()
+        if timers is not None:
+            ev[2].record()
+        g[3].replay()
+        if timers is not None:
+            ev[3].record()
+            timers.append(ev)
+
+    def timed(self, steps, warmup, barrier, world=1, dist=None, graph=False):
         t = self.torch
         for _ in range(max(warmup, 3)):
             self.step()
+        barrier()
+        use_graph = bool(graph) and self.capture()
+        run = self.step_graph if use_graph else self.step
+        for _ in range(3 if use_graph else 0):
+            run()
         barrier()
         timers = []
         s0, s1 = t.cuda.Event(enable_timing=True), t.cuda.Event(enable_timing=True)
@@ -245,10 +301,10 @@ class Frame:
         barrier()
         s0.record()
         for _ in range(steps):
-            self.step(timers)
+            run(timers)
         s1.record()
         barrier()
-        launches = self.qr.binding.qr_launch_count() - n0
+        launches = (self.graph_launches * steps) if use_graph else (self.qr.binding.qr_launch_count() - n0)
         total_ms = s0.elapsed_time(s1)
         found = int(self.found.item()) if self.found is not None else self.fe.M
         if found > self.capacity:
@@ -258,7 +314,8 @@ class Frame:
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         mean = lambda i, j: statistics.mean(e[i].elapsed_time(e[j]) for e in timers)
         return {"ms_step": float(tt.item()) / steps, "fwd_ms": mean(0, 1), "bwd_ms": mean(1, 2), "clear_ms": mean(2, 3),
-                "launches": int(launches), "M_found": found}
+                "launches": int(launches), "M_found": found, "cuda_graph": use_graph,
+                "cuda_graph_error": getattr(self, "graph_error", None)}
 
     def time_call(self, fn, n=5, warm=2):
         t = self.torch
@@ -375,7 +432,7 @@ def run_cuda(args):
     barrier()
     if rank == 0:
         sampler.start()
-    r = fr.timed(args.steps, args.warmup, barrier, world, dist)
+    r = fr.timed(args.steps, args.warmup, barrier, world, dist, graph=not args.no_graph)
     ms_step, fwd_ms, bwd_ms, zero_ms = r["ms_step"], r["fwd_ms"], r["bwd_ms"], r["clear_ms"]
     value = world * npix / (ms_step * 1e-3) / 1e6
     fe = fr.fe
@@ -536,6 +593,9 @@ def run_cuda(args):
 
     if rank == 0:
         cfg = workload_config(sc, args.workload)
+        cfg["cuda_graph"] = ("the step is replayed as four CUDA graphs (front end | qr_forward | qr_backward | qr_backward_clear), captured "
+                             "from the same library calls; events between the replays time each call" if r["cuda_graph"] else
+                             "eager launches" + (f" (graph capture failed: {r['cuda_graph_error']})" if r["cuda_graph_error"] else ""))
         cfg["step"] = ("qr_preprocess, qr_bin_sort (list capacity from an untimed first step: qr_bin_count and its host read "
                        "are NOT in the step), qr_forward, qr_backward, qr_backward_clear (re-zeroes the touched rows; the "
                        "zero fill of the whole dL_dfeat table is NOT in the step, see zero_fill_ms)")
@@ -743,6 +803,7 @@ def main():
     ap.add_argument("--pose", type=int, default=None, help="camera pose 0..7 of config 4's circle")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="launch the step's kernels eagerly instead of replaying CUDA graphs")
     ap.add_argument("--sweep", default=None, choices=["cfg4", "cfg5"],
                     help="run every point of BASELINE.json's config 4 (4 K x 8 poses) or config 5 (6 D) and write a JSON file")
     ap.add_argument("--out", default=None, help="where --sweep writes (default gpurun_out/sweep_<cfg>.json)")
