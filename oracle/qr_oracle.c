@@ -263,10 +263,15 @@ void orc_tile_rects(const orc_camera* cam, int64_t N, const float* mean2d, const
         tiles_touched[i] = 0;
         if (!visible[i]) continue;
         const float inv = 1.0f / (float)ORC_TILE;
-        const float fx0 = floorf((mean2d[2 * i] - extent[2 * i]) * inv);
-        const float fx1 = floorf((mean2d[2 * i] + extent[2 * i]) * inv);
-        const float fy0 = floorf((mean2d[2 * i + 1] - extent[2 * i + 1]) * inv);
-        const float fy1 = floorf((mean2d[2 * i + 1] + extent[2 * i + 1]) * inv);
+        /* The rectangle is cut from the 3-sigma AABB of cov2d, membership (R4) from the fp32-INVERTED conic: for an elongated,
+         * ill-conditioned cov2d the conic's 3-sigma ellipse can reach ~0.01 px past that AABB, and a pixel centre on a tile edge
+         * could pass R4 yet miss the tile's list.  Any superset is correct (R4 is per pixel), so the extent is inflated by
+         * 0.1 % + 0.01 px here (reading R4, note on the rectangle). */
+        const float ex = extent[2 * i] * 1.001f + 0.01f, ey = extent[2 * i + 1] * 1.001f + 0.01f;
+        const float fx0 = floorf((mean2d[2 * i] - ex) * inv);
+        const float fx1 = floorf((mean2d[2 * i] + ex) * inv);
+        const float fy0 = floorf((mean2d[2 * i + 1] - ey) * inv);
+        const float fy1 = floorf((mean2d[2 * i + 1] + ey) * inv);
         /* clamp in float first so that huge footprints cannot overflow the int conversion */
         const float big = 1.0e6f;
         int x0 = clampi((int)fminf(fmaxf(fx0, -big), big), 0, TX);

@@ -98,7 +98,9 @@ __device__ __forceinline__ void project_one(const Cam& cam, const int64_t i, con
         if (det > 0.0f) {
             co = make_float4(fdiv(cyy, det), fdiv(-cxy, det), fdiv(cxx, det), opac[i]);
             m2 = make_float2(__fmaf_rn(cam.fx, txz, cam.cx), __fmaf_rn(cam.fy, tyz, cam.cy));
-            const float ex = mul(3.0f, __fsqrt_rn(cxx)), ey = mul(3.0f, __fsqrt_rn(cyy));
+            // 3-sigma AABB, inflated by 0.1 % + 0.01 px: the conic that decides membership is an fp32 inverse and its ellipse can
+            // reach that far past the AABB of an ill-conditioned cov2d (any superset is correct: rule R4 is per pixel)
+            const float ex = add(mul(mul(3.0f, __fsqrt_rn(cxx)), 1.001f), 0.01f), ey = add(mul(mul(3.0f, __fsqrt_rn(cyy)), 1.001f), 0.01f);
             // tile rectangle of the 3-sigma AABB, half-open, clamped to the grid
             const float inv = 1.0f / (float)kTile;   // exact power of two
             const float big = 1.0e6f;

@@ -856,3 +856,29 @@ def test_mask_loss_closed_forms_and_gradient(orc):
     # adding a duplicate negative strictly increases the loss
     r1 = orc.mask_loss(fmap, mid, np.concatenate([tg, tg[1:2]]))
     assert r1.loss > r.loss
+
+
+def test_tile_rectangles_cover_every_included_pixel_of_elongated_gaussians(orc):
+    """Rule R4 is per pixel; the tile rectangle must be a superset of it.  Needle-like Gaussians (scale ratio 1000:1, random
+    orientation: ill-conditioned cov2d, where the fp32-inverted conic's ellipse and the AABB of cov2d drift apart) placed so that
+    they straddle tile edges: every (pixel, Gaussian) pair of the brute-force per-pixel lists lies inside that Gaussian's tile
+    rectangle, and the binned lists equal the brute-force ones."""
+    rng = np.random.default_rng(19)
+    cam = make_camera(96, 64)
+    n = 400
+    means = np.stack([rng.uniform(-1.2, 1.2, n), rng.uniform(-0.8, 0.8, n), rng.uniform(1.5, 3.0, n)], 1).astype(np.float32)
+    scales = np.stack([rng.uniform(0.2, 0.6, n), rng.uniform(2e-4, 6e-4, n), rng.uniform(2e-4, 6e-4, n)], 1).astype(np.float32)
+    q = rng.standard_normal((n, 4)).astype(np.float32)
+    q /= np.linalg.norm(q, axis=1, keepdims=True)
+    opac = rng.uniform(0.3, 0.99, n).astype(np.float32)
+    proj = orc.project(cam, means, scales, q, opac)
+    rect, touched = orc.tile_rects(cam, proj)
+    brute = orc.pixel_lists(cam, proj, "brute")
+    binned = orc.pixel_lists(cam, proj, "binned")
+    assert np.array_equal(brute.off, binned.off) and np.array_equal(brute.gid, binned.gid)
+    assert len(brute.gid) > 2000
+    pix = np.repeat(np.arange(cam.width * cam.height), np.diff(brute.off))
+    tx, ty = (pix % cam.width) // 16, (pix // cam.width) // 16
+    r = rect[brute.gid]
+    assert ((tx >= r[:, 0]) & (tx < r[:, 2]) & (ty >= r[:, 1]) & (ty < r[:, 3])).all()
+    assert (touched[np.unique(brute.gid)] > 0).all()
