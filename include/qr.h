@@ -130,10 +130,10 @@ int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M,
  *        sel_w[H,W,K]   fp32 normalised weights w^Q / (1 - T^Q)       the others are left as the caller passed them
  *        n_sel[H,W]     int32 number selected (<= K)                  (writing -1 / 0 there would be two thirds of the
  *        resid_TQ[H,W]  fp32 T^Q after the walk (1 where nothing is selected)     records' traffic, for no reader)
- * out_map may be NULL on the tcgen05 path (fp32, D % 128 == 0): selection only -- the walk, the records and the selection
+ * out_map may be NULL on the tcgen05 path (D % 128 == 0): selection only -- the walk, the records and the selection
  * lists, no blend, no map (what qr_pooled_loss needs).
  * K in [1, QR_MAX_K]; D in [1, QR_MAX_D]; D % 4 == 0 unless D <= 128; fp16 needs D % 8 == 0.
- * ws must hold qr_forward_workspace_bytes(cam, K, D) bytes; every pointer must be non-NULL.  For fp32 features with
+ * ws must hold qr_forward_workspace_bytes(cam, K, D) bytes; every pointer must be non-NULL.  For fp32 or fp16 features with
  * D % 128 == 0 (the tcgen05 path) the call leaves in ws, per 16x8-pixel half tile, the numbered union of selected
  * Gaussians and the selection as (weight, column, pixel) entries; qr_backward_lists and qr_backward_clear accept that
  * workspace as it is, until the next call that writes it.
@@ -174,8 +174,8 @@ int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N,
 
 /*
  * qr_backward_lists -- the same gradient as qr_backward, computed from the per-half-tile selection lists that the last
- * qr_forward(cam, K, D, QR_F32, ...) left in ITS workspace fwd_ws (see qr_forward), instead of re-deriving the unions
- * from sel_idx / sel_w: one kernel instead of two.  fp32, D % 128 == 0, D <= 512 only (QR_ERR_UNSUPPORTED otherwise).
+ * qr_forward(cam, K, D, ...) left in ITS workspace fwd_ws (see qr_forward), instead of re-deriving the unions
+ * from sel_idx / sel_w: one kernel instead of two.  D % 128 == 0, D <= 512 only (QR_ERR_UNSUPPORTED otherwise).
  * The lists carry a stamp (image size, K) that the kernel checks on the device: a workspace that does not hold the
  * lists of this camera and K makes the call a no-op (dL_dfeat untouched).  fwd_ws is only read.
  */
@@ -236,7 +236,7 @@ int qr_topk_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dt
  *   pass 2: Algorithm 1 with the boundaries b_k = clamp(mu + sigma z_k, 0, 1), z_k = z_max (1 - 2 (k+1) / (K+1)), k < K, in
  *           place of 1 - (k+1)/(K+1); the walk ends once T_test < max(b_{K-1}, t_min); sigma == 0 -> Q-Render's boundaries.
  * Inputs and outputs as qr_forward (the records and the workspace's selection lists have the same format: qr_backward,
- * qr_backward_lists and qr_backward_clear accept them); z_max = 2 by convention.  fp32 features with D % 128 == 0 only
+ * qr_backward_lists and qr_backward_clear accept them); z_max = 2 by convention.  Features with D % 128 == 0 only
  * (QR_ERR_UNSUPPORTED otherwise).  ws must hold qr_stratified_workspace_bytes(cam, K, D) bytes.
  */
 size_t qr_stratified_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D);

@@ -296,8 +296,8 @@ def qr_forward(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, feature
 
 
 def lists_supported(features_dtype, D: int) -> bool:
-    """qr_forward leaves selection lists in its workspace for fp32 features with D % 128 == 0 (include/qr.h)."""
-    return features_dtype == torch.float32 and D % 128 == 0 and 128 <= D <= QR_MAX_D
+    """qr_forward leaves selection lists in its workspace for fp32 / fp16 features with D % 128 == 0 (include/qr.h)."""
+    return features_dtype in (torch.float32, torch.float16) and D % 128 == 0 and 128 <= D <= QR_MAX_D
 
 
 def qr_backward_workspace_bytes(cam, K: int, D: int) -> int:

@@ -19,6 +19,7 @@ constexpr int kSentinels = 3;
 struct BlendParams {
     Cam cam;
     int32_t K, D, cap, num_tiles;
+    int32_t feat_f16 = 0;        // tcgen05 blend: features are fp16 (widened exactly, R14)
     const void* features;
     const int32_t* gcount;       // [tiles * 32] records per group
     const int32_t* ucount;       // [tiles * 2] size of each half tile's union

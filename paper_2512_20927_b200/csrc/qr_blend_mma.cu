@@ -150,6 +150,10 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int D = p.D;
+    // fp16 features (R14: widened exactly): a raw row quarter is 256 bytes, the widened value IS the tf32 operand (10 explicit mantissa
+    // bits: nothing to split off), so the F_lo buffer is never written and the third MMA is skipped
+    const bool f16 = p.feat_f16 != 0;
+    const int raw_row = f16 ? kRawRow / 2 : kRawRow;
     const int nunits = D / kUnitN;
     const int num_half = p.num_tiles * 2;
 
@@ -290,7 +294,7 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                         if (elect_one()) {
                             umma_tf32_ts(d_tmem, a_hi + j * kStageRows, db_hi, idesc, (r | j) != 0);
                             umma_tf32_ts(d_tmem, a_lo + j * kStageRows, db_hi, idesc, true);
-                            umma_tf32_ts(d_tmem, a_hi + j * kStageRows, db_lo, idesc, true);
+                            if (!f16) umma_tf32_ts(d_tmem, a_hi + j * kStageRows, db_lo, idesc, true);
                             umma_commit(&empty[s]);
                         }
                         __syncwarp();
@@ -352,12 +356,12 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                         }
                         PW(1, &raw_empty[s], ((st / kRawStages) & 1) ^ 1);
                         if (lane == 0) {
-                            if (ngrp > 0) mbar_arrive_expect_tx(&raw_full[s], (uint32_t)ngrp * 4 * kRawRow);
+                            if (ngrp > 0) mbar_arrive_expect_tx(&raw_full[s], (uint32_t)(ngrp * 4 * raw_row));
                             else mbar_arrive(&raw_full[s]);
                         }
                         __syncwarp();
                         if (lane < ngrp)
-                            tma_gather4(raw_base + s * kRawBytes + lane * 4 * kRawRow, &feat_tmap, c * kUnitN,
+                            tma_gather4(raw_base + s * kRawBytes + lane * 4 * raw_row, &feat_tmap, c * kUnitN,
                                         ids4[0], ids4[1], ids4[2], ids4[3], &raw_full[s]);
                     }
                 }
@@ -446,7 +450,16 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
 #pragma unroll
                         for (int q = 0; q < kStageRows; ++q) {
                             a[q] = make_float4(0.f, 0.f, 0.f, 0.f);
-                            if (q < rows) a[q] = *reinterpret_cast<const float4*>(raw_base + sr * kRawBytes + q * kRawRow + lane * 16);
+                            if (q < rows) {
+                                if (f16) {
+                                    const uint2 h = *reinterpret_cast<const uint2*>(raw_base + sr * kRawBytes + q * raw_row + lane * 8);
+                                    const float2 f0 = __half22float2(*reinterpret_cast<const __half2*>(&h.x));
+                                    const float2 f1 = __half22float2(*reinterpret_cast<const __half2*>(&h.y));
+                                    a[q] = make_float4(f0.x, f0.y, f1.x, f1.y);
+                                } else {
+                                    a[q] = *reinterpret_cast<const float4*>(raw_base + sr * kRawBytes + q * kRawRow + lane * 16);
+                                }
+                            }
                         }
                         const int s = st % kStages;
                         PW(2, &empty[s], ((st / kStages) & 1) ^ 1);
@@ -457,8 +470,9 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                             const float4 v = a[q];
                             const float4 hv = make_float4(tf32_hi(v.x), tf32_hi(v.y), tf32_hi(v.z), tf32_hi(v.w));
                             *reinterpret_cast<float4*>(hi) = hv;
-                            *reinterpret_cast<float4*>(hi + kStageHalf) =
-                                make_float4(__fsub_rn(v.x, hv.x), __fsub_rn(v.y, hv.y), __fsub_rn(v.z, hv.z), __fsub_rn(v.w, hv.w));
+                            if (!f16)
+                                *reinterpret_cast<float4*>(hi + kStageHalf) =
+                                    make_float4(__fsub_rn(v.x, hv.x), __fsub_rn(v.y, hv.y), __fsub_rn(v.z, hv.z), __fsub_rn(v.w, hv.w));
                         }
                         fence_async_smem();
                         __syncwarp();
@@ -580,7 +594,7 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
 }
 
-bool blend_mma_supported(int32_t D, qr_dtype feat_dtype) { return feat_dtype == QR_F32 && D >= kUnitN && D % kUnitN == 0; }   // 128, 256, 384, 512
+bool blend_mma_supported(int32_t D, qr_dtype feat_dtype) { return (feat_dtype == QR_F32 || feat_dtype == QR_F16) && D >= kUnitN && D % kUnitN == 0; }   // 128, 256, 384, 512
 
 int launch_blend_mma(const BlendParams& p, cudaStream_t st, bool pdl)
 {
@@ -601,10 +615,10 @@ int launch_blend_mma(const BlendParams& p, cudaStream_t st, bool pdl)
     {
         // (qr_forward is not told N: the row bound is left open, ids come from the caller's own intersection lists)
         const cuuint64_t fdims[2] = { (cuuint64_t)p.D, (cuuint64_t)0x7fffffff };
-        const cuuint64_t fstr[1] = { (cuuint64_t)p.D * 4 };
+        const cuuint64_t fstr[1] = { (cuuint64_t)p.D * (p.feat_f16 ? 2 : 4) };
         const cuuint32_t fbox[2] = { (cuuint32_t)kUnitN, 1 };
         const cuuint32_t fes[2] = { 1, 1 };
-        const CUresult fr = enc(&fmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(p.features), fdims, fstr, fbox, fes,
+        const CUresult fr = enc(&fmap, p.feat_f16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(p.features), fdims, fstr, fbox, fes,
                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (fr != CUDA_SUCCESS) return fail(QR_ERR_CUDA, "qr_forward: cuTensorMapEncodeTiled (features) failed (%d)", (int)fr);

@@ -963,6 +963,7 @@ static int forward_impl(const qr_camera* cam, int32_t K, int32_t D, qr_dtype fea
         bp.features = features; bp.gcount = nullptr; bp.ucount = nullptr; bp.rec = nullptr;
         bp.n_sel = n_sel; bp.resid = resid_TQ; bp.out_map = out_map; bp.sel_idx = sel_idx; bp.sel_w = sel_w;
         bp.sl = w2.sl;
+        bp.feat_f16 = feat_dtype == QR_F16 ? 1 : 0;
         return launch_blend_mma(bp, st);
     }
 

@@ -259,9 +259,14 @@ extern "C" int qr_topk_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dt
         bl.features = features; bl.gcount = nullptr; bl.ucount = nullptr; bl.rec = nullptr;
         bl.n_sel = n_sel; bl.resid = resid; bl.out_map = out_map; bl.sel_idx = sel_idx; bl.sel_w = sel_w;
         bl.sl = bp.sl;
+        bl.feat_f16 = feat_dtype == QR_F16 ? 1 : 0;
         if (int rc = launch_blend_mma(bl, st, false)) return rc;
-        records_blend_kernel<float><<<rgrid, 256, 0, st>>>(c, K, D, static_cast<const float*>(features), sel_idx, sel_w, n_sel,
-                                                           out_map, bp.sl.hdr, nflag);
+        if (feat_dtype == QR_F16)
+            records_blend_kernel<__half><<<rgrid, 256, 0, st>>>(c, K, D, static_cast<const __half*>(features), sel_idx, sel_w, n_sel,
+                                                                out_map, bp.sl.hdr, nflag);
+        else
+            records_blend_kernel<float><<<rgrid, 256, 0, st>>>(c, K, D, static_cast<const float*>(features), sel_idx, sel_w, n_sel,
+                                                               out_map, bp.sl.hdr, nflag);
         QR_LAUNCH_OK("records_blend_kernel");
         return QR_OK;
     }
