@@ -689,6 +689,28 @@ def test_pooled_loss_equals_loss_on_the_map_then_backward(qr, orc, name, kw, K, 
     print("pooled loss", float(loss.item()), "oracle", ref.loss, "pixels differing", int((~same).sum()))
 
 
+@pytest.mark.parametrize("W,H,D,N,K", [(1, 1, 128, 50, 4), (17, 3, 128, 300, 40), (16, 16, 512, 1, 1), (5, 40, 256, 2000, 7), (33, 9, 16, 500, 3)])
+def test_degenerate_image_sizes_through_every_forward(qr, orc, W, H, D, N, K):
+    """One-pixel, one-Gaussian, sliver-shaped images: front end, Q-Render forward + backward, stratified-K and top-K against the
+    oracle (TMA boxes larger than the image, half tiles below it, unions of one column)."""
+    sc = make_scene("cfg1", seed=3, W=W, H=H, D=D, N=N, backward=True)
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    out = qr.pipeline.forward(sc.cam, fe, g.features, K)
+    dF = qr.pipeline.backward(sc.cam, N, out, P.to_dev(sc.dL_dmap))
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    lists = orc.pixel_lists(sc.cam, proj)
+    q = orc.qrender(lists, K, sc.features)
+    st = P.compare_forward(out, q, lists, K, D)
+    if st["mismatch_exempt"] == 0:
+        P.compare_backward_rows(dF.cpu().numpy(), orc.backward(q.sel_idx, q.sel_w, q.n_sel, sc.dL_dmap, N), "tiny image")
+    if D % 128 == 0:
+        so = qr.pipeline.stratified_forward(sc.cam, fe, g.features, K)
+        P.compare_stratified(so, orc.stratified(lists, K, sc.features, t_min=1e-4), lists, K, D)
+    tk = qr.pipeline.topk_forward(sc.cam, fe, g.features, K, 1e-4)
+    P.compare_topk(tk, orc.topk(lists, K, sc.features, t_min=1e-4), lists, K, D)
+
+
 def test_error_codes(qr):
     sc = make_scene("cfg1", seed=0, N=100)
     g = P.upload(sc)
