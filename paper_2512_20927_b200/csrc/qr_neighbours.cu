@@ -423,6 +423,11 @@ extern "C" int qr_mask_loss(const qr_camera* cam, int32_t D, int32_t S, const fl
 namespace qr {
 
 __device__ __forceinline__ void nb_red(float* dst, float v) { asm volatile("red.global.add.f32 [%0], %1;" ::"l"(dst), "f"(v) : "memory"); }
+// four consecutive floats in one vector reduction (16-byte aligned destination)
+__device__ __forceinline__ void nb_red4(float* dst, float4 v)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
 
 constexpr int kPlThreads = 128;
 constexpr int kPlMasks = 8;              // masks per round
@@ -561,7 +566,7 @@ __global__ void __launch_bounds__(kPlThreads) pooled_lists_kernel(const Cam cam,
                     for (int l = 0; l < kPlMasks; ++l) {
                         if (l < nmr) {
                             float* dst = sum + (int64_t)loc_mask[m0 + l] * D + 4 * tid;
-                            nb_red(dst, acc[l].x); nb_red(dst + 1, acc[l].y); nb_red(dst + 2, acc[l].z); nb_red(dst + 3, acc[l].w);
+                            nb_red4(dst, acc[l]);
                         }
                     }
                 } else {
@@ -581,7 +586,7 @@ __global__ void __launch_bounds__(kPlThreads) pooled_lists_kernel(const Cam cam,
                         const int32_t id = uid_s[col];
                         if ((uint32_t)id >= (uint32_t)N) continue;      // never add outside the table
                         float* dst = dL_dfeat + (int64_t)id * D + 4 * tid;
-                        nb_red(dst, d.x); nb_red(dst + 1, d.y); nb_red(dst + 2, d.z); nb_red(dst + 3, d.w);
+                        nb_red4(dst, d);
                     }
                 }
             }
