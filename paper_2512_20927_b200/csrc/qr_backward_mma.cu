@@ -108,11 +108,23 @@ __device__ __forceinline__ void bm_tma_box(void* dst, const CUtensorMap* map, in
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
                  ::"r"(s32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(s32(bar)), "r"(c0), "r"(x), "r"(y) : "memory");
 }
+__device__ __forceinline__ void bm_tma_box4(void* dst, const CUtensorMap* map, int c0, int x, int g, int y, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+                 ::"r"(s32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(s32(bar)), "r"(c0), "r"(x), "r"(g), "r"(y) : "memory");
+}
 __device__ __forceinline__ void bm_red(float* dst, float v)
 {
     asm volatile("red.global.add.f32 [%0], %1;" ::"l"(dst), "f"(v) : "memory");
 }
 
+// QR_PROF builds: cycles every role spends waiting on each barrier class, summed over the CTAs into ctrl[16..27] (in
+// units of 1,024 cycles; [27] = the CTAs' lifetimes); profiles/README.md, experiment 13
+#ifdef QR_PROF
+#define BPW(cls, bar, par) do { const long long t_ = clock64(); mbar_wait(bar, par); bpw[cls] += clock64() - t_; } while (0)
+#else
+#define BPW(cls, bar, par) mbar_wait(bar, par)
+#endif
 __global__ void __launch_bounds__(kBmThreads, 1)
 backward_mma_kernel(const BackwardParams p, const int stages, const __grid_constant__ CUtensorMap g_tmap)
 {
@@ -139,6 +151,10 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
+#ifdef QR_PROF
+    const long long t_start = clock64();
+    long long bpw[11] = { 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0 };
+#endif
     if (!sel_stamp_ok(p.sl.stamp, p.cam, p.K)) return;      // not the lists of this camera / K: touch nothing
 
     if (tid == 0) {
@@ -172,7 +188,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
         float* dcol = p.dL_dfeat + warp * 32 + lane;
         for (int unit = 0;; ++unit) {
             const int buf = unit & 1;
-            mbar_wait(&tmem_full[buf], (unit >> 1) & 1);
+            BPW(0, &tmem_full[buf], (unit >> 1) & 1);
             tc_fence_after();
             const BmDesc* d = &desc[unit % kBmDescRing];
             if (d->flags & 1) break;
@@ -214,10 +230,10 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
         int st = 0, s = 0;                               // st counts stages; s = st % stages without the division
         for (int unit = 0;; ++unit) {
             const int buf = unit & 1;
-            mbar_wait(&w_ready[0], unit & 1);
+            BPW(1, &w_ready[0], unit & 1);
             const BmDesc* d = &desc[unit % kBmDescRing];
             const int j0 = d->j0, j1 = d->j1, flags = d->flags;
-            mbar_wait(&tmem_empty[buf], ((unit >> 1) & 1) ^ 1);
+            BPW(2, &tmem_empty[buf], ((unit >> 1) & 1) ^ 1);
             tc_fence_after();
             if (flags & 1) {
                 if (elect_one()) umma_commit(&tmem_full[buf]);
@@ -226,9 +242,9 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
             bool have_w1 = false;
             for (int j = j0; j < j1; ++j, ++st) {
                 const int h = j >> 3;
-                if (h == 1 && !have_w1) { mbar_wait(&w_ready[1], unit & 1); have_w1 = true; }
+                if (h == 1 && !have_w1) { BPW(3, &w_ready[1], unit & 1); have_w1 = true; }
                 const int l = st % kBmLoStages;
-                mbar_wait(&lo_ready[l], (st / kBmLoStages) & 1);      // implies raw_full[s]
+                BPW(4, &lo_ready[l], (st / kBmLoStages) & 1);      // implies raw_full[s]
                 tc_fence_after();
                 const uint32_t a_hi = st0 + s * stage_half, a_lo = lo0 + l * stage_half;
                 const uint32_t b_hi = w0 + h * 2 * kBmWHalfBytes + (j & 7) * 256, b_lo = b_hi + kBmWHalfBytes;
@@ -236,6 +252,9 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                 const uint64_t db_lo = umma_desc(b_lo, 128, kBmHalfPx / 4 * 128, 0);
                 const uint64_t da_hi0 = umma_desc(a_hi, 1024, 512, 1), da_lo0 = umma_desc(a_lo, 1024, 512, 1);
                 const uint32_t d0 = tmem_base + (uint32_t)(buf * 256);
+#ifdef QR_PROF
+                const long long t_issue = clock64();
+#endif
                 if (elect_one()) {
 #pragma unroll 4
                     for (int m = 0; m < nchunks; ++m) {
@@ -250,6 +269,9 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                     if (h == 0 && (j == 7 || j == j1 - 1)) umma_commit(&w_free[0]);     // last read of W half 0
                 }
                 __syncwarp();
+#ifdef QR_PROF
+                bpw[10] += clock64() - t_issue;           // issuing the stage's MMAs and commits
+#endif
                 if (++s == stages) s = 0;
             }
             if (!have_w1) mbar_wait(&w_ready[1], unit & 1);       // keep the phases of every unit in step
@@ -262,7 +284,10 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
         }
     } else if (warp == kBmLoadWarp) {
         // ================================================= loader ===================================================
-        // lane c < D / 32 copies channels [32 c, 32 c + 32) of the stage's 8 pixels: a [8 px][128 B] swizzled block
+        // a stage is D / 32 blocks of [8 px][128 B] (32 channels, swizzled), one behind the other.  The tensor map has the
+        // 32-channel group as a dimension of its own BEHIND the pixel dimension, so ONE box {32 ch, 8 px, D / 32 groups, 1 row}
+        // lands in exactly that layout: one TMA instruction per stage (issued per 1 KB block, the warp's loop over the lanes'
+        // boxes kept the loader busy 95 % of the kernel; profiles/README.md, experiment 13)
         int s = 0;
         uint32_t ph = 1;                                 // parity to wait for on stage_empty[s]
         for (int unit = 0;; ++unit) {
@@ -277,12 +302,12 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
             const int tile = ht >> 1;
             const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
             for (int j = j0; j < j1; ++j) {
-                mbar_wait(&stage_empty[s], ph);
-                if (lane == 0) mbar_arrive_expect_tx(&raw_full[s], (uint32_t)stage_half);
+                BPW(5, &stage_empty[s], ph);
+                if (lane == 0) {
+                    mbar_arrive_expect_tx(&raw_full[s], (uint32_t)stage_half);
+                    bm_tma_box4(stage_base + (size_t)s * stage_half, &g_tmap, 0, x0 + (j & 1) * kBmStagePx, 0, y0 + (j >> 1), &raw_full[s]);
+                }
                 __syncwarp();
-                if (lane < (D >> 5))
-                    bm_tma_box(stage_base + (size_t)s * stage_half + lane * 1024, &g_tmap, lane * 32,
-                               x0 + (j & 1) * kBmStagePx, y0 + (j >> 1), &raw_full[s]);
                 if (++s == stages) { s = 0; ph ^= 1u; }
             }
         }
@@ -294,7 +319,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
         uint32_t ph = 0;                                     // parity to wait for on raw_full[s]
         for (int st = 0;; ++st) {
             const int l = st % kBmLoStages;
-            mbar_wait(&raw_full[s], ph);
+            BPW(6, &raw_full[s], ph);
             if (*done_flag) break;
             const float4* hi = reinterpret_cast<const float4*>(stage_base + (size_t)s * stage_half) + ct;
             float4* lo = reinterpret_cast<float4*>(lo_base + (size_t)l * stage_half) + ct;
@@ -302,7 +327,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
 #pragma unroll
             for (int u = 0; u < 4; ++u)
                 if (u < nchunks) v[u] = hi[u * kBmConvWarps * 32];
-            mbar_wait(&lo_empty[l], ((st / kBmLoStages) & 1) ^ 1);       // the MMAs that read this G_lo buffer have retired
+            BPW(7, &lo_empty[l], ((st / kBmLoStages) & 1) ^ 1);       // the MMAs that read this G_lo buffer have retired
 #pragma unroll
             for (int u = 0; u < 4; ++u)
                 if (u < nchunks)
@@ -379,7 +404,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                                     const int32_t id = __ldg(uid + c_lo + st);
                                     rowoff = (uint32_t)id < (uint32_t)p.N ? (int64_t)id * D : -1;   // never add outside the table
                                 }
-                                mbar_wait(&w_free[h], (unit & 1) ^ 1);      // the MMAs of the previous unit have read this half
+                                BPW(8, &w_free[h], (unit & 1) ^ 1);      // the MMAs of the previous unit have read this half
                                 float4* wz = reinterpret_cast<float4*>(whi);
                                 for (int k = st; k < 2 * kBmWHalfBytes / 16; k += kBmSetupThreads) wz[k] = make_float4(0.f, 0.f, 0.f, 0.f);
                                 ssync_setup();
@@ -422,6 +447,12 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
         }
     }
 
+#ifdef QR_PROF
+    if (tid == 0) atomicAdd(&p.sl.ctrl[27], (int)((clock64() - t_start) >> 10));
+    if (lane == 0)
+        for (int c = 0; c < 11; ++c)
+            if (bpw[c]) atomicAdd(&p.sl.ctrl[16 + c], (int)(bpw[c] >> 10));
+#endif
     tc_fence_before();
     __syncthreads();
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
@@ -598,16 +629,17 @@ int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_
     QR_CUDA_OK(cudaMemsetAsync(nflag, 0, 256, st));      // [0] half tiles left to the FFMA kernel, [1] the contraction's half-tile ticket
     p.ticket = nflag + 1;
     const int sms = sm_count();
-    // dL_dmap [H][W][D] fp32 as a 3-D tensor (D, W, H); box = 32 channels x 8 pixels x 1 row, 32-byte-atom 128-byte
-    // swizzle (what UMMA calls SWIZZLE_128B_BASE32B); pixels outside the image are filled with zeros
+    // dL_dmap [H][W][D] fp32 as a 4-D tensor (32 channels, W, D / 32 channel groups, H); box = 32 channels x 8 pixels x
+    // all groups x 1 row, 32-byte-atom 128-byte swizzle (what UMMA calls SWIZZLE_128B_BASE32B); pixels outside the image
+    // are filled with zeros
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return fail(QR_ERR_CUDA, "qr_backward: cuTensorMapEncodeTiled is not available from the driver");
     CUtensorMap tmap;
-    const cuuint64_t dims[3] = { (cuuint64_t)p.D, (cuuint64_t)p.cam.width, (cuuint64_t)p.cam.height };
-    const cuuint64_t strides[2] = { (cuuint64_t)p.D * 4, (cuuint64_t)p.D * 4 * (cuuint64_t)p.cam.width };
-    const cuuint32_t box[3] = { 32, kBmStagePx, 1 };
-    const cuuint32_t estr[3] = { 1, 1, 1 };
-    const CUresult cr = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(p.dL_dmap), dims, strides, box, estr,
+    const cuuint64_t dims[4] = { 32, (cuuint64_t)p.cam.width, (cuuint64_t)(p.D / 32), (cuuint64_t)p.cam.height };
+    const cuuint64_t strides[3] = { (cuuint64_t)p.D * 4, 128, (cuuint64_t)p.D * 4 * (cuuint64_t)p.cam.width };
+    const cuuint32_t box[4] = { 32, kBmStagePx, (cuuint32_t)(p.D / 32), 1 };
+    const cuuint32_t estr[4] = { 1, 1, 1, 1 };
+    const CUresult cr = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float*>(p.dL_dmap), dims, strides, box, estr,
                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (cr != CUDA_SUCCESS) return fail(QR_ERR_CUDA, "qr_backward: cuTensorMapEncodeTiled failed (%d)", (int)cr);
