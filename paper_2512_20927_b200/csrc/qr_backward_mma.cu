@@ -225,7 +225,8 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
     } else if (warp == kBmMmaWarp) {
         // ================================================= MMA issuer ===============================================
         // M = 128 channels, N = 64 rows, fp32 accumulate, A and B tf32, A MN-major, B K-major
-        const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | ((uint32_t)(kBmRows >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+        // N = the unit's union rows rounded up to 16: the tensor core's time per MMA grows with N
+        const uint32_t idesc0 = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | ((uint32_t)(128 >> 4) << 24);
         const uint32_t w0 = s32(Wsm), st0 = s32(stage_base), lo0 = s32(lo_base);
         int st = 0, s = 0;                               // st counts stages; s = st % stages without the division
         for (int unit = 0;; ++unit) {
@@ -233,6 +234,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
             BPW(1, &w_ready[0], unit & 1);
             const BmDesc* d = &desc[unit % kBmDescRing];
             const int j0 = d->j0, j1 = d->j1, flags = d->flags;
+            const uint32_t idesc = idesc0 | ((uint32_t)(max(16, (d->nrows + 15) & ~15) >> 3) << 17);
             BPW(2, &tmem_empty[buf], ((unit >> 1) & 1) ^ 1);
             tc_fence_after();
             if (flags & 1) {
