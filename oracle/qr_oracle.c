@@ -954,3 +954,69 @@ void orc_mask_loss(int64_t P, int D, const float* map, const int32_t* mask_id, i
     free(cnt); free(g); free(c);
 }
 
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * View-dependent colour of a Gaussian from spherical-harmonics coefficients: the RGB payload of PAPER.md:940-947
+ * (App. E.6, "directly apply Q-Render to pre-trained 3D-GS models"; 3D-GS itself is PAPER.md:79-80's [3D-GS]).
+ * The paper gives no formula; reading R20: the real spherical harmonics of degree <= 3 with the
+ * Condon-Shortley phase KEPT,
+ *     Y_{l,0} = Y_l^0,   Y_{l,m} = sqrt(2) Re Y_l^m  (m > 0),   Y_{l,-m} = sqrt(2) Im Y_l^m  (m > 0),
+ * ordered (l, m = -l..l), evaluated at the unit vector from the camera centre to the Gaussian's mean;
+ *     colour = max(0, 1/2 + sum_k Y_k(dir) sh[k])   per channel.
+ * Written out as polynomials in the unit vector (x, y, z) = (sin t cos p, sin t sin p, cos t); every constant is
+ * spelled as its closed form.  Pins (tests/test_oracle_pins.py): scipy's complex Y_l^m, orthonormality by quadrature,
+ * hand values at the poles.
+ * ------------------------------------------------------------------------------------------------------------------ */
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
+void orc_sh_basis(int degree, const double d[3], double* Y)
+{
+    const double x = d[0], y = d[1], z = d[2];
+    Y[0] = 0.5 * sqrt(1.0 / M_PI);
+    if (degree < 1) return;
+    const double c1 = sqrt(3.0 / (4.0 * M_PI));
+    Y[1] = -c1 * y;
+    Y[2] = c1 * z;
+    Y[3] = -c1 * x;
+    if (degree < 2) return;
+    const double xx = x * x, yy = y * y, zz = z * z;
+    Y[4] = 0.5 * sqrt(15.0 / M_PI) * x * y;
+    Y[5] = -0.5 * sqrt(15.0 / M_PI) * y * z;
+    Y[6] = 0.25 * sqrt(5.0 / M_PI) * (2.0 * zz - xx - yy);
+    Y[7] = -0.5 * sqrt(15.0 / M_PI) * x * z;
+    Y[8] = 0.25 * sqrt(15.0 / M_PI) * (xx - yy);
+    if (degree < 3) return;
+    Y[9] = -0.25 * sqrt(35.0 / (2.0 * M_PI)) * y * (3.0 * xx - yy);
+    Y[10] = 0.5 * sqrt(105.0 / M_PI) * x * y * z;
+    Y[11] = -0.25 * sqrt(21.0 / (2.0 * M_PI)) * y * (4.0 * zz - xx - yy);
+    Y[12] = 0.25 * sqrt(7.0 / M_PI) * z * (2.0 * zz - 3.0 * xx - 3.0 * yy);
+    Y[13] = -0.25 * sqrt(21.0 / (2.0 * M_PI)) * x * (4.0 * zz - xx - yy);
+    Y[14] = 0.25 * sqrt(105.0 / M_PI) * z * (xx - yy);
+    Y[15] = -0.25 * sqrt(35.0 / (2.0 * M_PI)) * x * (xx - 3.0 * yy);
+}
+
+/* sh[N][(degree+1)^2][3] -> colors[N][3] (fp64); the camera centre is -R^T t of the world-to-camera [R|t].
+ * A Gaussian AT the camera centre has no direction: its colour is the degree-0 term alone. */
+void orc_sh_colors(const orc_camera* cam, int64_t N, int degree, const float* means, const float* sh, double* colors)
+{
+    const float* w = cam->w2c;
+    double c[3];
+    for (int j = 0; j < 3; ++j) c[j] = -((double)w[0 + j] * (double)w[3] + (double)w[4 + j] * (double)w[7] + (double)w[8 + j] * (double)w[11]);
+    const int nb = (degree + 1) * (degree + 1);
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < N; ++i) {
+        double d[3] = { (double)means[3 * i] - c[0], (double)means[3 * i + 1] - c[1], (double)means[3 * i + 2] - c[2] };
+        const double n = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        double Y[16];
+        int deg = degree;
+        if (n > 0.0) { d[0] /= n; d[1] /= n; d[2] /= n; } else deg = 0;
+        orc_sh_basis(deg, d, Y);
+        const int nbi = (deg + 1) * (deg + 1);
+        for (int ch = 0; ch < 3; ++ch) {
+            double s = 0.5;
+            for (int k = 0; k < nbi; ++k) s += Y[k] * (double)sh[((int64_t)i * nb + k) * 3 + ch];
+            colors[3 * i + ch] = s > 0.0 ? s : 0.0;
+        }
+    }
+}

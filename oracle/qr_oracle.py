@@ -366,3 +366,23 @@ def mask_loss(feature_map, mask_id, targets) -> MaskLoss:
     lib().orc_mask_loss(C.c_int64(P_), C.c_int(D), _p(m), _p(mid), C.c_int(S), _p(t), _p(pooled), _p(ls), C.byref(tot), _p(dm))
     return MaskLoss(float(tot.value), ls, pooled, dm)
 
+
+
+def sh_basis(degree: int, direction) -> np.ndarray:
+    """The (degree+1)^2 real spherical harmonics of DESIGN.md reading R20 at a unit vector (float64)."""
+    d = np.ascontiguousarray(direction, dtype=np.float64).reshape(3)
+    Y = np.zeros(16, np.float64)
+    lib().orc_sh_basis(C.c_int(int(degree)), _p(d), _p(Y))
+    return Y[:(degree + 1) ** 2]
+
+
+def sh_colors(cam, means, sh, degree: int) -> np.ndarray:
+    """View-dependent RGB of every Gaussian (reading R20): [N,3] float64."""
+    m = _f32(means)
+    s = _f32(sh)
+    N = m.shape[0]
+    assert 0 <= degree <= 3 and s.shape == (N, (degree + 1) ** 2, 3), s.shape
+    out = np.empty((N, 3), np.float64)
+    c = _cam(cam)
+    lib().orc_sh_colors(C.byref(c), C.c_int64(N), C.c_int(int(degree)), _p(m), _p(s), _p(out))
+    return out

@@ -882,3 +882,95 @@ def test_tile_rectangles_cover_every_included_pixel_of_elongated_gaussians(orc):
     r = rect[brute.gid]
     assert ((tx >= r[:, 0]) & (tx < r[:, 2]) & (ty >= r[:, 1]) & (ty < r[:, 3])).all()
     assert (touched[np.unique(brute.gid)] > 0).all()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# spherical-harmonics colour (reading R20)
+# ---------------------------------------------------------------------------------------------------------------
+def test_sh_basis_equals_scipys_complex_harmonics(orc):
+    """R20 defines the basis through the complex Y_l^m: Y_{l,0} = Y_l^0, Y_{l,m} = sqrt2 Re Y_l^m, Y_{l,-m} = sqrt2 Im Y_l^m
+    (phase kept).  scipy.special evaluates Y_l^m from its own recurrences; the oracle's polynomials must agree at random
+    directions, for every degree (a wrong constant, sign, or swapped pair of indices fails)."""
+    from scipy.special import sph_harm_y
+    rng = np.random.default_rng(3)
+    for _ in range(200):
+        d = rng.standard_normal(3)
+        d /= np.linalg.norm(d)
+        theta, phi = math.acos(d[2]), math.atan2(d[1], d[0])
+        want = []
+        for l in range(4):
+            for m in range(-l, l + 1):
+                y = complex(sph_harm_y(l, abs(m), theta, phi))
+                want.append(y.real if m == 0 else math.sqrt(2) * (y.real if m > 0 else y.imag))
+        got = orc.sh_basis(3, d)
+        np.testing.assert_allclose(got, want, rtol=0, atol=1e-13)
+        for deg in range(3):
+            np.testing.assert_allclose(orc.sh_basis(deg, d), want[:(deg + 1) ** 2], rtol=0, atol=1e-13)
+
+
+def test_sh_basis_is_orthonormal_on_the_sphere(orc):
+    """Integral over the sphere of Y_i Y_j = delta_ij: Gauss-Legendre in cos(theta) x uniform phi integrates products of
+    degree <= 6 polynomials exactly."""
+    xs, ws = np.polynomial.legendre.leggauss(8)
+    nphi = 16
+    G = np.zeros((16, 16))
+    for z, w in zip(xs, ws):
+        s = math.sqrt(1 - z * z)
+        for k in range(nphi):
+            p = 2 * math.pi * k / nphi
+            Y = orc.sh_basis(3, [s * math.cos(p), s * math.sin(p), z])
+            G += w * (2 * math.pi / nphi) * np.outer(Y, Y)
+    np.testing.assert_allclose(G, np.eye(16), rtol=0, atol=1e-12)
+
+
+def test_sh_basis_hand_values(orc):
+    """Values anyone can check by hand: Y_0 = 1/(2 sqrt(pi)); at the north pole only the m = 0 terms survive,
+    Y_{l,0}(z = 1) = sqrt((2 l + 1) / (4 pi)); along +x the degree-1 terms are (0, 0, -sqrt(3 / (4 pi)))."""
+    Y = orc.sh_basis(3, [0.0, 0.0, 1.0])
+    want = np.zeros(16)
+    for l, k in ((0, 0), (1, 2), (2, 6), (3, 12)):
+        want[k] = math.sqrt((2 * l + 1) / (4 * math.pi))
+    np.testing.assert_allclose(Y, want, rtol=0, atol=1e-15)
+    assert abs(Y[0] - 0.28209479177387814) < 1e-16
+    Yx = orc.sh_basis(1, [1.0, 0.0, 0.0])
+    np.testing.assert_allclose(Yx, [0.28209479177387814, 0.0, 0.0, -math.sqrt(3 / (4 * math.pi))], rtol=0, atol=1e-15)
+
+
+def test_sh_colors_definition_and_special_cases(orc):
+    """colour = max(0, 1/2 + sum_k Y_k(dir) sh_k) with dir from the camera CENTRE (-R^T t) to the mean: restated in NumPy on
+    the pinned basis with a rotated, translated camera; degree 0 is view independent; a Gaussian at the camera centre keeps
+    only the constant term; negative sums clamp to 0."""
+    rng = np.random.default_rng(5)
+    cam = make_camera(64, 48)
+    # a non-trivial pose: rotate about y by 0.4 rad, about x by -0.2 rad, translate
+    cy, sy, cx, sx = math.cos(0.4), math.sin(0.4), math.cos(-0.2), math.sin(-0.2)
+    R = np.array([[1, 0, 0], [0, cx, -sx], [0, sx, cx]]) @ np.array([[cy, 0, sy], [0, 1, 0], [-sy, 0, cy]])
+    t = np.array([0.3, -0.2, 1.5])
+    cam.world_to_cam = np.concatenate([R, t[:, None]], 1).astype(np.float32)
+    Rf, tf = cam.world_to_cam[:, :3].astype(np.float64), cam.world_to_cam[:, 3].astype(np.float64)
+    centre = -Rf.T @ tf
+    N = 300
+    means = rng.uniform(-2, 2, (N, 3)).astype(np.float32)
+    means[7] = centre.astype(np.float32)
+    for deg in range(4):
+        nb = (deg + 1) ** 2
+        sh = (rng.standard_normal((N, nb, 3)) * 0.8).astype(np.float32)
+        got = orc.sh_colors(cam, means, sh, deg)
+        for i in range(N):
+            d = means[i].astype(np.float64) - centre
+            n = np.linalg.norm(d)
+            if n == 0 or i == 7 and n < 1e-6:
+                continue
+            Y = orc.sh_basis(deg, d / n)
+            want = np.maximum(0.0, 0.5 + Y @ sh[i].astype(np.float64))
+            np.testing.assert_allclose(got[i], want, rtol=0, atol=1e-12)
+        assert (got >= 0).all() and (got == 0).any()
+        if deg == 0:
+            cam2 = make_camera(64, 48)
+            np.testing.assert_array_equal(got, orc.sh_colors(cam2, means, sh, 0))
+    # exactly at the centre (float32 centre may differ from the float64 one: build the camera so that it is exact)
+    cam3 = make_camera(64, 48)
+    cam3.world_to_cam = np.concatenate([np.eye(3), np.array([[0.5], [0.25], [-1.0]])], 1).astype(np.float32)
+    m3 = np.array([[-0.5, -0.25, 1.0]], np.float32)
+    sh3 = rng.standard_normal((1, 16, 3)).astype(np.float32)
+    np.testing.assert_allclose(orc.sh_colors(cam3, m3, sh3, 3)[0], np.maximum(0, 0.5 + 0.28209479177387814 * sh3[0, 0].astype(np.float64)), atol=1e-15)
