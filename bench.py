@@ -506,12 +506,18 @@ def run_cuda(args):
                              "qr_pooled_loss (loss + dL/dF), qr_backward_clear -- the map and dL/dmap never exist; unfused = the "
                              "headline step + qr_mask_loss"}
             pl.forward(cam, fr.fe, fr.d["features"], K, fr.fwd_out)        # leave a complete forward behind for the counters below
+        # RGB payload (NEXT-4): this view's colours from degree-3 spherical harmonics, N Gaussians
+        shc = torch.randn((N, 16, 3), device=dev, generator=g) * 0.5
+        col = torch.empty((N, 3), device=dev)
+        sh_ms = fr.time_call(lambda: qr.binding.qr_sh_colors(cam, fr.d["means"], shc, 3, col))
+        del shc, col
         devox_bytes = Mv * (D * 4 + 8) + N * D * 4 * 2            # voxel rows gathered + indices, table + argmax written
         loss_bytes = 2 * npix * D * 4 + npix * 8
         nb = {"devoxelize_max": {"ms": devox_ms, "voxels": Mv, "unique_voxels": U, "gb_s": devox_bytes / devox_ms / 1e6},
               "devoxelize_backward_max": {"ms": devox_bwd_ms},
               "mask_loss": {"ms": loss_ms, "masks": S_m, "gb_s": loss_bytes / loss_ms / 1e6,
                             "note": "one read of the map + one write of dL/dmap"},
+              "sh_colors_degree3": {"ms": sh_ms, "gb_s": N * 216 / sh_ms / 1e6, "note": "12 + 192 + 12 bytes per Gaussian"},
               "fused": fused}
         del uni, inv, dgs, duni, dm, st_
     # zero fill of the whole dL_dfeat table: what a caller without qr_backward_clear pays per step (reported, not in the step)

@@ -325,6 +325,19 @@ int qr_pooled_loss(const qr_camera* cam, int32_t K, int32_t D, int64_t N, void* 
                    const float* features, const int32_t* mask_id, int32_t S, const float* targets,
                    float* loss, float* loss_per_mask, float* dL_dfeat, void* ws, size_t ws_bytes, void* stream);
 
+/*
+ * qr_sh_colors -- the RGB payload of PAPER.md:940-947 (App. E.6: Q-Render applied to pre-trained 3D-GS models; SURVEY.md 8(f)
+ * NEXT-4), reading R20: the view-dependent colour of every Gaussian from its spherical-harmonics coefficients,
+ *     colors[i,c] = max(0, 1/2 + sum_k Y_k(dir_i) sh[i,k,c]),   dir_i = unit vector from the camera centre (-R^T t) to means[i],
+ * Y_k the real harmonics of degree <= `degree` ordered (l, m = -l..l) with the Condon-Shortley phase kept (degree-1 terms
+ * (-y, z, -x) sqrt(3 / (4 pi))).  A Gaussian at the camera centre keeps the constant term only.  colors[N,3] is then the
+ * D = 3 fp32 feature table of qr_forward / qr_dense_forward for that view.
+ *   in : means[N,3], sh[N, (degree+1)^2, 3] fp32        out: colors[N,3] fp32
+ * degree outside [0, 3]: QR_ERR_INVALID_ARG.  N = 0 is legal.  No alignment requirement.
+ */
+int qr_sh_colors(const qr_camera* cam, int64_t N, int32_t degree, const float* means, const float* sh, float* colors,
+                 void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -30,7 +30,7 @@ SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_b
            "qr_backward_lists", "qr_backward_clear", "qr_dense_forward", "qr_topk_workspace_bytes", "qr_topk_forward",
            "qr_launch_count", "qr_forward_stats", "qr_batch_camera", "qr_preprocess_batch", "qr_forward_batch",
            "qr_stratified_workspace_bytes", "qr_forward_stratified", "qr_devoxelize_workspace_bytes", "qr_devoxelize",
-           "qr_devoxelize_backward", "qr_mask_loss_workspace_bytes", "qr_mask_loss", "qr_pooled_loss"]
+           "qr_devoxelize_backward", "qr_mask_loss_workspace_bytes", "qr_mask_loss", "qr_pooled_loss", "qr_sh_colors"]
 
 
 class QRError(RuntimeError):
@@ -108,6 +108,8 @@ def load() -> C.CDLL:
     lib.qr_mask_loss.restype = C.c_int; lib.qr_mask_loss.argtypes = [cam, i32, i32, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.qr_pooled_loss.restype = C.c_int
     lib.qr_pooled_loss.argtypes = [cam, i32, i32, i64, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, sz, vp]
+    lib.qr_sh_colors.restype = C.c_int
+    lib.qr_sh_colors.argtypes = [cam, i64, i32, vp, vp, vp, vp]
     lib.qr_topk_workspace_bytes.restype = sz; lib.qr_topk_workspace_bytes.argtypes = [cam, i32, i32]
     lib.qr_topk_forward.restype = C.c_int
     lib.qr_topk_forward.argtypes = [cam, i32, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -581,3 +583,18 @@ def qr_pooled_loss(cam, K: int, N: int, fwd: ForwardOut, features, mask_id, targ
                                  _dev(mask_id, torch.int32, "mask_id"), S, _dev(targets, torch.float32, "targets"), loss.data_ptr(),
                                  per.data_ptr(), dL_dfeat.data_ptr() if with_grad else None, ws.data_ptr(), ws.numel(), _stream()))
     return loss, per, (dL_dfeat if with_grad else None)
+
+
+def qr_sh_colors(cam, means, sh, degree: int, colors: Optional[torch.Tensor] = None):
+    """View-dependent RGB of every Gaussian from its spherical-harmonics coefficients (include/qr.h qr_sh_colors;
+    PAPER.md:940-947, reading R20).  sh [N, (degree+1)^2, 3] fp32 -> colors [N, 3] fp32, the D = 3 feature table
+    of qr_forward for this view."""
+    c = make_camera(cam)
+    N = int(means.shape[0])
+    if tuple(sh.shape) != (N, (int(degree) + 1) ** 2, 3):
+        raise QRError(-1, f"sh has shape {tuple(sh.shape)}, expected {(N, (int(degree) + 1) ** 2, 3)}")
+    if colors is None:
+        colors = torch.empty((N, 3), dtype=torch.float32, device=means.device)
+    _check(load().qr_sh_colors(C.byref(c), N, int(degree), _dev(means, torch.float32, "means"), _dev(sh, torch.float32, "sh"),
+                               _dev(colors, torch.float32, "colors"), _stream()))
+    return colors

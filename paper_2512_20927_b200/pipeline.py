@@ -107,3 +107,9 @@ def mask_loss(cam, feature_map, mask_id, targets):
 def pooled_loss(cam, N: int, fwd: B.ForwardOut, features, mask_id, targets, dL_dfeat=None, with_grad: bool = True):
     """Loss + dL/dF from the selection lists of `fwd` (which may come from forward(..., select_only=True)): no map round trip."""
     return B.qr_pooled_loss(cam, int(fwd.sel_idx.shape[-1]), N, fwd, features, mask_id, targets, dL_dfeat, with_grad)
+
+
+def sh_colors(cam, means, sh, degree: int, colors=None):
+    """RGB payload: per-view colours from spherical harmonics; feed the result to forward() as the
+    D = 3 feature table.  See binding.qr_sh_colors."""
+    return B.qr_sh_colors(cam, means, sh, degree, colors)

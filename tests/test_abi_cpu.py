@@ -83,6 +83,10 @@ def test_bad_arguments_are_status_codes(lib):
     assert lib.qr_batch_camera(two, 1, C.byref(tall)) == 0 and tall.height == 64
     assert lib.qr_topk_workspace_bytes(C.byref(cam), 8, 16) > 0 and lib.qr_topk_workspace_bytes(C.byref(cam), 0, 16) == 0
     assert lib.qr_bin_sort(C.byref(cam), 10, 1 << 31, p, p, p, p, p, p, 1 << 20, None) == -5
+    # spherical-harmonics colour: degree outside [0, 3], NULL arrays, N = 0
+    assert lib.qr_sh_colors(C.byref(cam), 10, 4, p, p, p, None) == -1 and lib.qr_sh_colors(C.byref(cam), 10, -1, p, p, p, None) == -1
+    assert lib.qr_sh_colors(C.byref(cam), 10, 3, p, z, p, None) == -2 and lib.qr_sh_colors(None, 10, 3, p, p, p, None) == -2
+    assert lib.qr_sh_colors(C.byref(cam), 0, 3, z, z, z, None) == 0
     m = C.c_int64(-1)
     assert lib.qr_bin_count(0, z, z, C.byref(m), z, 0, None) == 0 and m.value == 0
     assert lib.qr_bin_workspace_bytes(1000, 5000, 16) >= 5000 * 16 + 16 * 16 * 4      # keys + scratch + bucket cursors

@@ -3,6 +3,8 @@
 Stage-isolated (each GPU stage fed the oracle's upstream outputs) and end to end, at sizes the oracle finishes in
 seconds that still span several tiles and ragged tails, plus sampled checks at BASELINE.json's config-3 size.
 """
+import math
+
 import numpy as np
 import pytest
 import torch
@@ -727,3 +729,43 @@ def test_error_codes(qr):
     with pytest.raises(qr.QRError) as e:
         qr.qr_preprocess(bad, g.means, g.scales, g.quats, g.opac)
     assert e.value.code == -1
+
+
+# ------------------------------------------------------------------------------------------------
+# RGB payload (NEXT-4): spherical-harmonics colours (reading R20), then Q-Render / V-Render with D = 3
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,degree", [(50000, 3), (1000, 2), (129, 1), (77, 0), (1, 3)])
+def test_sh_colors_against_the_oracle(qr, orc, N, degree):
+    from qr_inputs import make_camera
+    rng = np.random.default_rng(47 + degree)
+    cam = make_camera(96, 64)
+    cy, sy = math.cos(0.3), math.sin(0.3)
+    cam.world_to_cam = np.array([[cy, 0, sy, 0.2], [0, 1, 0, -0.1], [-sy, 0, cy, 0.7]], np.float32)
+    means = rng.uniform(-3, 3, (N, 3)).astype(np.float32)
+    sh = (rng.standard_normal((N, (degree + 1) ** 2, 3)) * 0.6).astype(np.float32)
+    ref = orc.sh_colors(cam, means, sh, degree)
+    got = qr.pipeline.sh_colors(cam, P.to_dev(means), P.to_dev(sh), degree).cpu().numpy()
+    assert got.shape == (N, 3) and (got >= 0).all()
+    # the basis is a cubic in a unit vector normalised in fp32 and the sum has up to 16 terms of either sign
+    A = 0.5 + np.abs(sh.astype(np.float64)).sum(1)
+    assert (np.abs(got - ref) <= P.ATOL + P.RTOL * np.abs(ref) + 8 * 2.0 ** -24 * A).all()
+    if N >= 1000:
+        assert (ref == 0).any() and ((got == 0) == (ref == 0)).mean() > 0.999      # the clamp is exercised
+
+
+def test_rgb_render_from_sh_colors(qr, orc):
+    """The whole RGB path: colours of this view from degree-3 coefficients, then Q-Render with D = 3 -- selection as for
+    any payload, the image within the fp32 feature tolerance of the oracle run on the ORACLE's colours."""
+    sc = make_scene("cfg1", seed=9, D=3)
+    rng = np.random.default_rng(9)
+    sh = (rng.standard_normal((sc.N, 16, 3)) * 0.5).astype(np.float32)
+    g = P.upload(sc)
+    colors = qr.pipeline.sh_colors(sc.cam, g.means, P.to_dev(sh), 3)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    out = qr.pipeline.forward(sc.cam, fe, colors, sc.K)
+    cref = orc.sh_colors(sc.cam, sc.means, sh, 3).astype(np.float32)
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    lists = orc.pixel_lists(sc.cam, proj)
+    q = orc.qrender(lists, sc.K, cref)
+    stats = P.compare_forward(out, q, lists, sc.K, 3)
+    assert stats["mismatch_nonexempt"] == 0

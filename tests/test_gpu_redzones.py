@@ -125,5 +125,14 @@ def test_no_call_writes_outside_its_arrays(qr, name, kw, K):
     B._check(lib.qr_topk_forward(C.byref(c), kt, D, 0, C.c_float(1e-4), ptr(mean2d), ptr(conic), ptr(isect), ptr(rng),
                                  ptr(inputs["features"]), ptr(t_map), ptr(t_idx), ptr(t_w), ptr(t_n), ptr(t_r), ptr(tws), tws.numel(), st))
     z.check("qr_topk_forward")
+    # qr_sh_colors (every degree: the staging loops have a different row length each)
+    for deg in range(4):
+        shc = z.alloc((N, (deg + 1) ** 2, 3), torch.float32)
+        shc.normal_()
+        keep = shc.clone()
+        col = z.alloc((N, 3), torch.float32)
+        B._check(lib.qr_sh_colors(C.byref(c), N, deg, ptr(inputs["means"]), ptr(shc), ptr(col), st))
+        z.check(f"qr_sh_colors(degree {deg})")
+        assert torch.equal(shc, keep), "sh was modified"
     for k, v in inputs.items():
         assert torch.equal(v, before[k]), f"input {k} was modified"
