@@ -226,6 +226,71 @@ __global__ void __launch_bounds__(256) backward_pixel_kernel(const BackwardParam
     }
 }
 
+// backward_small_kernel -- D <= 8 with D % 4 != 0 (the RGB payload, D = 3): CTA = one 16x16 tile, thread = pixel.  With so
+// few channels the band kernel's lane = channel layout leaves the warp idle; here every thread walks its own selection record
+// and adds w g[c] into a shared-memory hash table keyed by the Gaussian id (the tile's union is a few hundred rows), which is
+// flushed with one red.global.add per (cell, channel).  An id that finds no free cell within kSmallProbe steps goes straight
+// to global memory.
+constexpr int kSmallCells = 2048;
+constexpr int kSmallProbe = 16;
+__global__ void __launch_bounds__(256) backward_small_kernel(const BackwardParams p)
+{
+    __shared__ int32_t s_key[kSmallCells];
+    extern __shared__ __align__(16) unsigned char small_raw[];
+    float* s_val = reinterpret_cast<float*>(small_raw);                  // [kSmallCells][D]
+    const int tid = threadIdx.x, D = p.D, K = p.K;
+    const int tile_x = blockIdx.x % p.cam.tiles_x, tile_y = blockIdx.x / p.cam.tiles_x;
+    const int x = tile_x * kTile + (tid & 15), y = tile_y * kTile + (tid >> 4);
+    for (int i = tid; i < kSmallCells; i += 256) s_key[i] = -1;
+    for (int i = tid; i < kSmallCells * D; i += 256) s_val[i] = 0.0f;
+    __syncthreads();
+    if (x < p.cam.width && y < p.cam.height) {
+        const int64_t pix = (int64_t)y * p.cam.width + x;
+        const int ns = min(max(__ldg(p.n_sel + pix), 0), K);
+        float g[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) g[c] = c < D ? __ldg(p.dL_dmap + pix * D + c) : 0.0f;
+        for (int s = 0; s < ns; ++s) {
+            const int32_t id = __ldg(p.sel_idx + pix * K + s);
+            const float w = __ldg(p.sel_w + pix * K + s);
+            if ((uint32_t)id >= (uint32_t)p.N) continue;                 // never add outside the table
+            uint32_t h = hash32((uint32_t)id) & (kSmallCells - 1);
+            int cell = -1;
+            for (int t = 0; t < kSmallProbe; ++t) {
+                const int32_t old = atomicCAS(&s_key[h], -1, id);
+                if (old == -1 || old == id) { cell = (int)h; break; }
+                h = (h + 1) & (kSmallCells - 1);
+            }
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                if (c < D) {
+                    const float a = __fmul_rn(w, g[c]);
+                    if (cell >= 0) atomicAdd(&s_val[cell * D + c], a);
+                    else atomicAdd(p.dL_dfeat + (int64_t)id * D + c, a);
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (int i = tid; i < kSmallCells * D; i += 256) {
+        const int cell = i / D;
+        const int32_t id = s_key[cell];
+        if (id >= 0) {
+            const float v = s_val[i];
+            if (v != 0.0f) asm volatile("red.global.add.f32 [%0], %1;" ::"l"(p.dL_dfeat + (int64_t)id * D + (i - cell * D)), "f"(v) : "memory");
+        }
+    }
+}
+
+static int launch_backward_small(const BackwardParams& p, cudaStream_t st)
+{
+    const int T = p.cam.tiles_x * p.cam.tiles_y;
+    QR_CUDA_OK(cudaFuncSetAttribute(backward_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmallCells * 8 * 4));
+    backward_small_kernel<<<(unsigned)T, 256, (size_t)kSmallCells * p.D * 4, st>>>(p);
+    QR_LAUNCH_OK("backward_small_kernel");
+    return QR_OK;
+}
+
 static int next_pow2(int v) { int p = 1; while (p < v) p <<= 1; return p; }
 
 template <int NV, int VW>
@@ -402,6 +467,7 @@ extern "C" int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N
     if (backward_mma_supported(K, D)) return launch_backward_mma(p, ws, ws_bytes, st, false);
     if (backward_tile_supported(K, D)) return launch_backward_tile(p, st);
     // D % 4 == 0 never reaches this point (backward_tile_supported takes it): what is left is D % 4 != 0, D <= 128
+    if (D <= 8) return launch_backward_small(p, st);
     switch ((D + 31) / 32) {
         case 1: return launch_backward<1, 1>(p, st);
         case 2: return launch_backward<2, 1>(p, st);

@@ -901,6 +901,44 @@ static int launch_blend(const BlendParams& p, cudaStream_t st)
     return QR_OK;
 }
 
+// blend_pixel_kernel -- D <= 8 with D % 4 != 0 (the RGB payload, D = 3): thread = pixel.  With so few channels a lane per
+// channel (blend_kernel) leaves 29 of 32 lanes idle; here a thread walks its own selection record,
+//     out[p,:] = sum_s sel_w[p,s] F[sel_idx[p,s],:]        (sel_w is already normalised by 1 - T^Q: line 20),
+// the feature table (12 bytes per Gaussian) stays in L2, and a warp's 32 results leave as one contiguous 32 D-float block.
+constexpr int kPixThreads = 256;
+__global__ void __launch_bounds__(kPixThreads) blend_pixel_kernel(const BlendParams p)
+{
+    const int64_t pix = (int64_t)blockIdx.x * kPixThreads + threadIdx.x;
+    if (pix >= (int64_t)p.cam.width * p.cam.height) return;
+    const int D = p.D, K = p.K;
+    const float* F = static_cast<const float*>(p.features);
+    const int n = min(max(__ldg(p.n_sel + pix), 0), K);
+    float acc[8];
+#pragma unroll
+    for (int c = 0; c < 8; ++c) acc[c] = 0.0f;
+    const int32_t* ids = p.sel_idx + pix * K;
+    const float* ws = p.sel_w + pix * K;
+    for (int s = 0; s < n; ++s) {
+        const float w = ws[s];
+        const float* f = F + (int64_t)ids[s] * D;
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+            if (c < D) acc[c] = __fadd_rn(acc[c], __fmul_rn(w, __ldg(f + c)));
+    }
+    float* o = p.out_map + pix * D;
+#pragma unroll
+    for (int c = 0; c < 8; ++c)
+        if (c < D) o[c] = acc[c];
+}
+
+static int launch_blend_pixel(const BlendParams& p, cudaStream_t st)
+{
+    const int64_t npix = (int64_t)p.cam.width * p.cam.height;
+    blend_pixel_kernel<<<(unsigned)((npix + kPixThreads - 1) / kPixThreads), kPixThreads, 0, st>>>(p);
+    QR_LAUNCH_OK("blend_pixel_kernel");
+    return QR_OK;
+}
+
 }  // namespace qr
 
 extern "C" size_t qr_forward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D)
@@ -998,6 +1036,7 @@ static int forward_impl(const qr_camera* cam, int32_t K, int32_t D, qr_dtype fea
             default: return launch_blend_tu<float, 4, 4>(bp, st);
         }
     }
+    if (D <= 8) return launch_blend_pixel(bp, st);
     switch ((D + 31) / 32) {
         case 1: return launch_blend<float, 1, 1>(bp, st);
         case 2: return launch_blend<float, 2, 1>(bp, st);

@@ -153,6 +153,9 @@ FWD_CASES = [
     ("cfg3", dict(N=40000, W=96, H=64, D=64), 200),             # K large
     ("cfg1", dict(W=70, H=50, D=256), 40),                      # tcgen05 blend on a ragged image (store guard, skipped half tiles)
     ("cfg3", dict(N=60000, W=100, H=72, D=512), 5),
+    ("cfg3", dict(N=40000, W=100, H=72, D=3), 40),              # thread = pixel blend (D <= 8, D % 4 != 0)
+    ("cfg2", dict(N=20000, W=64, H=48, D=7), 12),
+    ("cfg1", dict(W=33, H=17, D=1), 3),
 ]
 
 
@@ -256,7 +259,13 @@ def test_dense_forward(qr, orc, name, kw, t_min):
                                        ("cfg2", dict(N=20000, W=100, H=72, D=256), 40),
                                        ("cfg3", dict(N=60000, W=96, H=64, D=384), 10),
                                        ("cfg3", dict(N=40000, W=64, H=48, D=128), 200),
-                                       ("cfg2", dict(N=30000, W=64, H=40, D=128), 256)])
+                                       ("cfg2", dict(N=30000, W=64, H=40, D=128), 256),
+                                       # thread = pixel backward (D <= 8, D % 4 != 0); K = 200 on the blob scene overflows
+                                       # the tile's shared-memory hash table (direct global atomics for the rest)
+                                       ("cfg3", dict(N=40000, W=100, H=72, D=3), 40),
+                                       ("cfg3", dict(N=40000, W=64, H=48, D=3), 200),
+                                       ("cfg2", dict(N=20000, W=64, H=48, D=7), 12),
+                                       ("cfg1", dict(W=33, H=17, D=1, backward=True), 3)])
 def test_backward_stage_isolated(qr, orc, name, kw, K):
     sc = make_scene(name, seed=9, **kw)
     proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
