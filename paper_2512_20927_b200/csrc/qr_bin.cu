@@ -245,8 +245,9 @@ __device__ __forceinline__ void bitonic_sort_smem(uint64_t* s, int n2)
 }
 
 constexpr int kSmallBucket = 2048;          // keys sorted by tile_sort_kernel<small> (16 KB of shared memory)
-constexpr int kBigBucket = 16384;           // keys per shared-memory run of tile_sort_kernel<big> (128 KB)
+constexpr int kBigBucket = 8192;            // keys per shared-memory run of tile_sort_kernel<big> (64 KB: two CTAs per SM)
 constexpr uint64_t kKeyInf = ~uint64_t(0);
+constexpr int kBigSmem = kBigBucket * 8 + 32 * 256 * 4;      // a run of keys + the radix sort's per-warp digit counters
 
 // Register-blocked bitonic network for one bucket of THREADS x E keys: thread t holds keys
 // t E .. t E + E - 1.  Strides below E are compare-exchanges inside a thread, strides below 32 E are exchanged with
@@ -310,6 +311,103 @@ __device__ __forceinline__ void bitonic_sort_regs(const uint64_t* __restrict__ k
         if (t * E + e < n) out[t * E + e] = (uint32_t)v[e];
 }
 
+// LSD radix sort of one bucket of up to 1,024 x E keys in shared memory (1,024 threads), for the buckets above kSmallBucket keys:
+// a bitonic network does O(n log^2 n) 64-bit compare-exchanges (config 4: 0.51 ms for 1,689 buckets of 2,049..6,518 keys),
+// four 8-bit passes over the DEPTH half of the key do O(n).  Warp w owns the keys [32 E w, 32 E (w + 1)), key (round e, lane)
+// at 32 E w + 32 e + lane, so "earlier" means (warp, round, lane) and a stable rank is
+//     keys of smaller digits  +  same digit in earlier warps  +  same digit earlier in this warp,
+// the last from per-warp digit counters advanced round by round (__match_any_sync groups the lanes of a digit), the second
+// from a column scan of those counters, the first from a scan over the 256 digit totals.  A pass in which every real key
+// has the same digit is skipped (the sign / exponent byte of the depths of one tile, usually).  Equal depths are then ordered
+// by Gaussian id (the low half of the key) in a last step: each key of a run of equal depths counts the smaller ids of its run.
+constexpr int kRadixWarps = 32;
+template <int E>
+__device__ __forceinline__ void radix_sort_bucket(const uint64_t* __restrict__ keys, const int n, uint32_t* __restrict__ out,
+                                                  uint64_t* s, uint32_t* cnt)
+{
+    __shared__ uint32_t base[256], wsum[8];
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    const uint32_t lt = (1u << lane) - 1u;
+    constexpr int n2 = kRadixWarps * 32 * E;
+    const int pad = n2 - n;
+    uint32_t* wc = cnt + w * 256;
+    uint64_t v[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int i = w * 32 * E + e * 32 + lane;
+        v[e] = i < n ? keys[i] : kKeyInf;
+    }
+#pragma unroll 1
+    for (int shift = 32; shift < 64; shift += 8) {
+        for (int i = t; i < kRadixWarps * 256; i += kRadixWarps * 32) cnt[i] = 0u;
+        __syncthreads();
+        uint32_t rank[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const uint32_t d = (uint32_t)(v[e] >> shift) & 255u;
+            const uint32_t peers = __match_any_sync(0xffffffffu, d);
+            const uint32_t pre = wc[d];
+            __syncwarp();
+            if (lane == __ffs(peers) - 1) wc[d] = pre + __popc(peers);
+            __syncwarp();
+            rank[e] = pre + __popc(peers & lt);
+        }
+        __syncthreads();
+        // column scan over the warps (thread = digit), then the scan over the digits
+        uint32_t tot = 0u, incl = 0u;
+        if (t < 256) {
+#pragma unroll 4
+            for (int ww = 0; ww < kRadixWarps; ++ww) {
+                const uint32_t x = cnt[ww * 256 + t];
+                cnt[ww * 256 + t] = tot;
+                tot += x;
+            }
+            incl = tot;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += y; }
+            if (lane == 31) wsum[w] = incl;
+        }
+        const int same = __syncthreads_or(t < 256 && (int)tot - (t == 255 ? pad : 0) == n);
+        if (same) continue;                     // every real key has this digit: the pass would move nothing
+        if (t < 256) {
+            uint32_t off = 0u;
+            for (int ww = 0; ww < w; ++ww) off += wsum[ww];
+            base[t] = off + incl - tot;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const uint32_t d = (uint32_t)(v[e] >> shift) & 255u;
+            s[base[d] + wc[d] + rank[e]] = v[e];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < E; ++e) v[e] = s[w * 32 * E + e * 32 + lane];
+        __syncthreads();
+    }
+#pragma unroll
+    for (int e = 0; e < E; ++e) s[w * 32 * E + e * 32 + lane] = v[e];
+    __syncthreads();
+    // equal depths by ascending id
+#pragma unroll 1
+    for (int e = 0; e < E; ++e) {
+        const int i = w * 32 * E + e * 32 + lane;
+        if (i >= n) continue;
+        const uint64_t key = v[e];
+        const uint32_t dep = (uint32_t)(key >> 32), id = (uint32_t)key;
+        const bool tl = i > 0 && (uint32_t)(s[i - 1] >> 32) == dep, tr = i + 1 < n && (uint32_t)(s[i + 1] >> 32) == dep;
+        int pos = i;
+        if (tl || tr) {
+            int a = i;
+            while (a > 0 && (uint32_t)(s[a - 1] >> 32) == dep) --a;
+            int r = 0;
+            for (int j = a; j < n && (uint32_t)(s[j] >> 32) == dep; ++j) r += (uint32_t)s[j] < id;
+            pos = a + r;
+        }
+        out[pos] = id;
+    }
+}
+
 // One CTA per tile.  BIG = false handles buckets of <= kSmallBucket keys (several CTAs per SM), BIG = true the rest:
 // up to kBigBucket keys in one shared-memory run; beyond that, runs of kBigBucket keys are sorted one by one and every
 // key is then ranked against the other runs by binary search (keys are unique, so ranks are a permutation).
@@ -329,10 +427,10 @@ __device__ __forceinline__ void tile_sort_one(const int tile, const int capacity
         else bitonic_sort_regs<8>(keys + start, n, isect_gauss + start, skeys);
         return;
     }
-    if (BIG && n <= kRun) {                     // 1,024 threads, 4 / 8 / 16 keys per thread in registers (was the all-shared-memory
-        if (n <= 4096) bitonic_sort_regs<4, 1024>(keys + start, n, isect_gauss + start, skeys);          // network: 0.64 ms of config 4's
-        else if (n <= 8192) bitonic_sort_regs<8, 1024>(keys + start, n, isect_gauss + start, skeys);     // 0.87 ms front end)
-        else bitonic_sort_regs<16, 1024>(keys + start, n, isect_gauss + start, skeys);
+    if (BIG && n <= kRun) {                     // 1,024 threads, 4 / 8 / 16 keys per thread: radix sort in shared memory
+        uint32_t* cnt = reinterpret_cast<uint32_t*>(skeys + kBigBucket);
+        if (n <= 4096) radix_sort_bucket<4>(keys + start, n, isect_gauss + start, skeys, cnt);
+        else radix_sort_bucket<8>(keys + start, n, isect_gauss + start, skeys, cnt);
         __syncthreads();
         return;
     }
@@ -380,8 +478,8 @@ __device__ __forceinline__ void tile_sort_one(const int tile, const int capacity
     }
 }
 
-// BIG = false: one CTA per tile.  BIG = true: one CTA per SM strides over the tiles (almost all of them are small
-// and skipped, and a CTA of this kernel owns 128 KB of shared memory).
+// One CTA per tile in both kernels (a CTA whose bucket belongs to the other kernel returns at once); two CTAs of the
+// big kernel (96 KB of shared memory each) fit an SM.
 template <bool BIG>
 __global__ void __launch_bounds__(BIG ? 1024 : 256)
 tile_sort_kernel(const int32_t* __restrict__ tile_range, int32_t T, int32_t capacity, uint64_t* __restrict__ keys,
@@ -488,8 +586,7 @@ extern "C" int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M, const flo
 
     static bool attr_set = false;
     if (!attr_set) {
-        QR_CUDA_OK(cudaFuncSetAttribute(tile_sort_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        kBigBucket * (int)sizeof(uint64_t)));
+        QR_CUDA_OK(cudaFuncSetAttribute(tile_sort_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kBigSmem));
         attr_set = true;
     }
     QR_CUDA_OK(cudaMemsetAsync(counter, 0, sizeof(uint32_t) * (size_t)T * kSubBuckets, st));
@@ -502,7 +599,8 @@ extern "C" int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M, const flo
     tile_sort_kernel<false><<<(unsigned)T, 256, kSmallBucket * sizeof(uint64_t), st>>>(tile_range, T, (int32_t)M, keys, scratch, isect_gauss);
     QR_LAUNCH_OK("tile_sort_kernel<small>");
     const int sms = sm_count();
-    tile_sort_kernel<true><<<(unsigned)min(sms, T), 1024, kBigBucket * sizeof(uint64_t), st>>>(tile_range, T, (int32_t)M, keys, scratch, isect_gauss);
+    (void)sms;
+    tile_sort_kernel<true><<<(unsigned)T, 1024, kBigSmem, st>>>(tile_range, T, (int32_t)M, keys, scratch, isect_gauss);
     QR_LAUNCH_OK("tile_sort_kernel<big>");
     return QR_OK;
 }
