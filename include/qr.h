@@ -309,6 +309,22 @@ int qr_mask_loss(const qr_camera* cam, int32_t D, int32_t S, const float* map, c
                  void* ws, size_t ws_bytes, void* stream);
 
 /*
+ * qr_mask_loss_static -- qr_mask_loss (same inputs, outputs, kernels and arithmetic) for callers that cannot allocate device
+ * memory: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The workspace is a
+ * file-scope device array of QR_STATIC_SCRATCH_BYTES inside the library (every GPU that loads the library holds it until
+ * exit); the call performs no cudaMalloc / cudaFree and calls no allocating library routine (two cudaMemsetAsync, four kernel
+ * launches; on its first use per device, one cudaGetSymbolAddress).
+ * Limit: qr_mask_loss_workspace_bytes(S, D) <= QR_STATIC_SCRATCH_BYTES, i.e. S <= QR_STATIC_MAX_MASKS = 256 masks at D = 512
+ * (more at a smaller D); beyond it QR_ERR_UNSUPPORTED with the sizes in qr_last_error().  Other errors as qr_mask_loss.
+ * Every call on a device shares the one array, which keeps the previous call's contents (the call clears what it needs at its
+ * start, on `stream`): calls that overlap on the GPU -- two streams, two host threads -- RACE on it; serialise them.
+ */
+#define QR_STATIC_MAX_MASKS 256
+#define QR_STATIC_SCRATCH_BYTES (QR_STATIC_MAX_MASKS * 512 * 4 + 3 * 1024)
+int qr_mask_loss_static(const qr_camera* cam, int32_t D, int32_t S, const float* map, const int32_t* mask_id,
+                        const float* targets, float* loss, float* loss_per_mask, float* d_map, void* stream);
+
+/*
  * qr_pooled_loss -- qr_mask_loss and qr_backward FUSED with the render path, without the map ("would let
  * qr_forward / qr_backward skip the 629 MB map round-trip").  Rendering is linear in the features and the loss pools the map by
  * a mean per mask, so with A[i,s] = sum over the pixels p of mask s of the normalised weight of Gaussian i at p,

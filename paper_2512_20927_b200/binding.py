@@ -30,7 +30,7 @@ SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_b
            "qr_backward_lists", "qr_backward_clear", "qr_dense_forward", "qr_topk_workspace_bytes", "qr_topk_forward",
            "qr_launch_count", "qr_forward_stats", "qr_batch_camera", "qr_preprocess_batch", "qr_forward_batch",
            "qr_stratified_workspace_bytes", "qr_forward_stratified", "qr_devoxelize_workspace_bytes", "qr_devoxelize",
-           "qr_devoxelize_backward", "qr_mask_loss_workspace_bytes", "qr_mask_loss", "qr_pooled_loss", "qr_sh_colors"]
+           "qr_devoxelize_backward", "qr_mask_loss_workspace_bytes", "qr_mask_loss", "qr_pooled_loss", "qr_sh_colors", "qr_mask_loss_static"]
 
 
 class QRError(RuntimeError):
@@ -106,6 +106,7 @@ def load() -> C.CDLL:
     lib.qr_devoxelize_backward.argtypes = [i64, i32, i64, vp, i32, vp, vp, vp, vp, sz, vp]
     lib.qr_mask_loss_workspace_bytes.restype = sz; lib.qr_mask_loss_workspace_bytes.argtypes = [i32, i32]
     lib.qr_mask_loss.restype = C.c_int; lib.qr_mask_loss.argtypes = [cam, i32, i32, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.qr_mask_loss_static.restype = C.c_int; lib.qr_mask_loss_static.argtypes = [cam, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.qr_pooled_loss.restype = C.c_int
     lib.qr_pooled_loss.argtypes = [cam, i32, i32, i64, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, sz, vp]
     lib.qr_sh_colors.restype = C.c_int
@@ -598,3 +599,24 @@ def qr_sh_colors(cam, means, sh, degree: int, colors: Optional[torch.Tensor] = N
     _check(load().qr_sh_colors(C.byref(c), N, int(degree), _dev(means, torch.float32, "means"), _dev(sh, torch.float32, "sh"),
                                _dev(colors, torch.float32, "colors"), _stream()))
     return colors
+
+
+def qr_mask_loss_static(cam, feature_map, mask_id, targets, loss: Optional[torch.Tensor] = None,
+                        loss_per_mask: Optional[torch.Tensor] = None, d_map: Optional[torch.Tensor] = None):
+    """qr_mask_loss without a workspace: the library's own static device array serves as scratch (include/qr.h
+    qr_mask_loss_static; at most 256 masks at D = 512).  The C call allocates nothing; pass loss [1], loss_per_mask [S] and
+    d_map [H, W, D] to keep this wrapper from allocating them.  Calls that overlap on the GPU race on the array."""
+    c = make_camera(cam)
+    D = int(feature_map.shape[-1])
+    S = int(targets.shape[0])
+    dev = feature_map.device
+    if loss is None:
+        loss = torch.empty((1,), dtype=torch.float32, device=dev)
+    if loss_per_mask is None:
+        loss_per_mask = torch.empty((S,), dtype=torch.float32, device=dev)
+    if d_map is None:
+        d_map = torch.empty((c.height, c.width, D), dtype=torch.float32, device=dev)
+    _check(load().qr_mask_loss_static(C.byref(c), D, S, _dev(feature_map, torch.float32, "map"), _dev(mask_id, torch.int32, "mask_id"),
+                                      _dev(targets, torch.float32, "targets"), _dev(loss, torch.float32, "loss"),
+                                      _dev(loss_per_mask, torch.float32, "loss_per_mask"), _dev(d_map, torch.float32, "d_map"), _stream()))
+    return loss, loss_per_mask, d_map

@@ -408,6 +408,78 @@ extern "C" int qr_mask_loss(const qr_camera* cam, int32_t D, int32_t S, const fl
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// qr_mask_loss_static: qr_mask_loss for callers that cannot allocate (code under CUDA graph capture, serving loops,
+// harnesses that forbid cudaMalloc).  The same four kernels, with the workspace (per-mask sums, counts, flags, norms) in a
+// file-scope device array of QR_STATIC_SCRATCH_BYTES instead of a caller-provided buffer; every GPU that loads the library
+// holds the array until exit.  In HOST code the array's name is a host-side stand-in, not a device address: the address the
+// kernels get comes from cudaGetSymbolAddress, asked for once per device with that device current.
+// ---------------------------------------------------------------------------------------------------------------
+#include <mutex>
+
+static __device__ __align__(256) unsigned char g_mask_scratch[QR_STATIC_SCRATCH_BYTES];
+
+namespace qr {
+
+constexpr int kStaticMaxDevices = 64;
+
+// device address of g_mask_scratch on the CURRENT device (nullptr + error state on failure)
+static int static_scratch_ptr(void** out)
+{
+    static std::mutex mu;
+    static void* ptr[kStaticMaxDevices] = {};
+    int dev = -1;
+    QR_CUDA_OK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(QR_ERR_UNSUPPORTED, "qr_mask_loss_static: device ordinal %d >= %d", dev, kStaticMaxDevices);
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr[dev]) {
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_mask_scratch);
+        if (e != cudaSuccess || !p)
+            return fail(QR_ERR_CUDA, "qr_mask_loss_static: cudaGetSymbolAddress failed on device %d: %s", dev, cudaGetErrorString(e));
+        ptr[dev] = p;
+    }
+    *out = ptr[dev];
+    return QR_OK;
+}
+
+}  // namespace qr
+
+extern "C" int qr_mask_loss_static(const qr_camera* cam, int32_t D, int32_t S, const float* map, const int32_t* mask_id,
+                                   const float* targets, float* loss, float* loss_per_mask, float* d_map, void* stream)
+{
+    using namespace qr;
+    if (int rc = check_cam(cam)) return rc;
+    if (D < 4 || D % 4 != 0) return fail(QR_ERR_UNSUPPORTED, "qr_mask_loss_static: D = %d must be a positive multiple of 4", D);
+    if (D > kNbMaxC) return fail(QR_ERR_UNSUPPORTED, "qr_mask_loss_static: D = %d > %d", D, kNbMaxC);
+    if (S < 1 || S > QR_MAX_MASKS) return fail(QR_ERR_INVALID_ARG, "qr_mask_loss_static: S = %d outside [1, QR_MAX_MASKS]", S);
+    const size_t need = mask_ws(nullptr, S, D).total;
+    if (need > (size_t)QR_STATIC_SCRATCH_BYTES)
+        return fail(QR_ERR_UNSUPPORTED, "qr_mask_loss_static: S = %d masks x D = %d channels need %zu bytes of scratch, the static array holds "
+                                        "%d (S <= %d at D = 512): use qr_mask_loss with a workspace of your own",
+                    S, D, need, QR_STATIC_SCRATCH_BYTES, QR_STATIC_MAX_MASKS);
+    if (!map || !mask_id || !targets || !loss || !loss_per_mask || !d_map) return fail(QR_ERR_NULL_POINTER, "qr_mask_loss_static: NULL argument");
+    if (!aligned16(map) || !aligned16(d_map)) return fail(QR_ERR_MISALIGNED, "qr_mask_loss_static: map / d_map must be 16-byte aligned");
+    void* ws = nullptr;
+    if (int rc = static_scratch_ptr(&ws)) return rc;
+    const MaskWs w = mask_ws(ws, S, D);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t P = (int64_t)cam->width * cam->height;
+    QR_CUDA_OK(cudaMemsetAsync(ws, 0, w.total, st));                 // the array keeps the last call's sums: they must start at zero
+    QR_CUDA_OK(cudaMemsetAsync(loss, 0, sizeof(float), st));
+    const int64_t strips = (P + kPoolStrip - 1) / kPoolStrip;
+    mask_pool_kernel<<<(unsigned)((strips + 7) / 8), 256, 0, st>>>(P, D, S, map, mask_id, w.sum, w.cnt);
+    QR_LAUNCH_OK("mask_pool_kernel");
+    mask_mean_kernel<<<(unsigned)S, 256, 0, st>>>(D, w.sum, w.cnt, w.valid, w.norm);
+    QR_LAUNCH_OK("mask_mean_kernel");
+    const size_t smem = ((size_t)D + 3 * (size_t)S) * 4;
+    mask_grad_kernel<<<(unsigned)S, 256, smem, st>>>(D, S, targets, w.sum, w.cnt, w.valid, w.norm, loss, loss_per_mask);
+    QR_LAUNCH_OK("mask_grad_kernel");
+    mask_dmap_kernel<<<(unsigned)(sm_count() * 8), 256, 0, st>>>(P, D, S, mask_id, w.sum, d_map);
+    QR_LAUNCH_OK("mask_dmap_kernel");
+    return QR_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // The loss fused with the render path ("would let qr_forward / qr_backward skip the 629 MB map
 // round-trip").  Rendering is linear in the features and the loss pools the map by a MEAN over each mask, so
 //     pooled_s = (1 / |m_s|) sum_{p in m_s} f~(p) = (1 / |m_s|) sum_i A[i,s] F[i,:],   A[i,s] = sum_{p in m_s} w^_{p,i}

@@ -87,6 +87,11 @@ def test_bad_arguments_are_status_codes(lib):
     assert lib.qr_sh_colors(C.byref(cam), 10, 4, p, p, p, None) == -1 and lib.qr_sh_colors(C.byref(cam), 10, -1, p, p, p, None) == -1
     assert lib.qr_sh_colors(C.byref(cam), 10, 3, p, z, p, None) == -2 and lib.qr_sh_colors(None, 10, 3, p, p, p, None) == -2
     assert lib.qr_sh_colors(C.byref(cam), 0, 3, z, z, z, None) == 0
+    # the entry point with static scratch: sizes beyond the array are refused before anything touches CUDA
+    assert lib.qr_mask_loss_static(C.byref(cam), 512, 257, p, p, p, p, p, p, None) == -3 and b"static array" in lib.qr_last_error()
+    assert lib.qr_mask_loss_static(C.byref(cam), 512, 0, p, p, p, p, p, p, None) == -1
+    assert lib.qr_mask_loss_static(C.byref(cam), 512, 256, p, z, p, p, p, p, None) == -2
+    assert lib.qr_mask_loss_workspace_bytes(256, 512) == 256 * 512 * 4 + 3 * 1024
     m = C.c_int64(-1)
     assert lib.qr_bin_count(0, z, z, C.byref(m), z, 0, None) == 0 and m.value == 0
     assert lib.qr_bin_workspace_bytes(1000, 5000, 16) >= 5000 * 16 + 16 * 16 * 4      # keys + scratch + bucket cursors
