@@ -130,11 +130,12 @@ int qr_bin_sort(const qr_camera* cam, int64_t N, int64_t M,
  *        sel_w[H,W,K]   fp32 normalised weights w^Q / (1 - T^Q)       the others are left as the caller passed them
  *        n_sel[H,W]     int32 number selected (<= K)                  (writing -1 / 0 there would be two thirds of the
  *        resid_TQ[H,W]  fp32 T^Q after the walk (1 where nothing is selected)     records' traffic, for no reader)
- * out_map may be NULL on the tcgen05 path (D % 128 == 0): selection only -- the walk, the records and the selection
+ * out_map may be NULL on the tcgen05 path (see below): selection only -- the walk, the records and the selection
  * lists, no blend, no map (what qr_pooled_loss needs).
  * K in [1, QR_MAX_K]; D in [1, QR_MAX_D]; D % 4 == 0 unless D <= 128; fp16 needs D % 8 == 0.
  * ws must hold qr_forward_workspace_bytes(cam, K, D) bytes; every pointer must be non-NULL.  For fp32 or fp16 features with
- * D % 128 == 0 (the tcgen05 path) the call leaves in ws, per 16x8-pixel half tile, the numbered union of selected
+ * D % 32 == 0, or D < 32 with D % 4 == 0 (the tcgen05 path: the contractions run on whole 128-channel tiles and let TMA pad the
+ * loads with zeros and clip the stores; fp16 additionally D % 8 == 0) the call leaves in ws, per 16x8-pixel half tile, the numbered union of selected
  * Gaussians and the selection as (weight, column, pixel) entries; qr_backward_lists and qr_backward_clear accept that
  * workspace as it is, until the next call that writes it.
  */
@@ -146,7 +147,7 @@ int qr_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dtype,
                void* ws, size_t ws_bytes, void* stream);
 
 /*
- * qr_forward_stats -- work counters of the last qr_forward that took the tcgen05 path (fp32, D % 128 == 0), summed over
+ * qr_forward_stats -- work counters of the last qr_forward that took the tcgen05 path (the shapes named at qr_forward), summed over
  * the half-tile headers it left in its workspace ("the bench must report this count"):
  *   stats[0] selections (sum of n_sel)            stats[1] sum over half tiles of U_ht (distinct Gaussians selected)
  *   stats[2] tile-list entries consumed before every pixel of the half tile had stopped
@@ -164,7 +165,7 @@ int qr_forward_stats(const qr_camera* cam, int32_t K, const void* fwd_ws, size_t
  *   out: dL_dfeat[N,D] fp32, ACCUMULATED INTO (the caller zeroes it; rows never selected are left untouched).
  * Summation order over pixels is not fixed (fp32 atomics): results agree to rounding, not bit for bit.
  * ws must hold qr_backward_workspace_bytes(cam, K, D) bytes.  Its contents are scratch: per half tile, the numbered
- * union of selected Gaussians and the selection as (weight, row, pixel) (D % 128 == 0), and qr_backward_clear's
+ * union of selected Gaussians and the selection as (weight, row, pixel) (tcgen05 shapes), and qr_backward_clear's
  * de-duplication cache; for the other shapes qr_backward itself does not touch ws (it may be NULL there).
  */
 size_t qr_backward_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D);
@@ -175,7 +176,7 @@ int qr_backward(const qr_camera* cam, int32_t K, int32_t D, int64_t N,
 /*
  * qr_backward_lists -- the same gradient as qr_backward, computed from the per-half-tile selection lists that the last
  * qr_forward(cam, K, D, ...) left in ITS workspace fwd_ws (see qr_forward), instead of re-deriving the unions
- * from sel_idx / sel_w: one kernel instead of two.  D % 128 == 0, D <= 512 only (QR_ERR_UNSUPPORTED otherwise).
+ * from sel_idx / sel_w: one kernel instead of two.  Shapes of the tcgen05 path only (QR_ERR_UNSUPPORTED otherwise).
  * The lists carry a stamp (image size, K) that the kernel checks on the device: a workspace that does not hold the
  * lists of this camera and K makes the call a no-op (dL_dfeat untouched).  fwd_ws is only read.
  */
@@ -218,7 +219,7 @@ int qr_dense_forward(const qr_camera* cam, int32_t D, qr_dtype feat_dtype, float
  *   in : as qr_forward, plus t_min (>= 0; 1e-4 by convention, 0 = weights over the whole list)
  *   out: out_map[H,W,D] fp32; sel_idx / sel_w / n_sel / resid in qr_forward's record format (slots s < n_sel[p] are
  *        written; n_sel[p] = min(K, weighted entries)), so qr_backward accepts them as they are.
- * K in [1, QR_TOPK_MAX_K].  ws must hold qr_topk_workspace_bytes(cam, K, D) bytes (scratch; used for fp32, D % 128 == 0,
+ * K in [1, QR_TOPK_MAX_K].  ws must hold qr_topk_workspace_bytes(cam, K, D) bytes (scratch; used for the tcgen05 shapes,
  * where the blend is the same tcgen05 contraction as qr_forward's; may be NULL otherwise).
  */
 size_t qr_topk_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D);
@@ -236,7 +237,7 @@ int qr_topk_forward(const qr_camera* cam, int32_t K, int32_t D, qr_dtype feat_dt
  *   pass 2: Algorithm 1 with the boundaries b_k = clamp(mu + sigma z_k, 0, 1), z_k = z_max (1 - 2 (k+1) / (K+1)), k < K, in
  *           place of 1 - (k+1)/(K+1); the walk ends once T_test < max(b_{K-1}, t_min); sigma == 0 -> Q-Render's boundaries.
  * Inputs and outputs as qr_forward (the records and the workspace's selection lists have the same format: qr_backward,
- * qr_backward_lists and qr_backward_clear accept them); z_max = 2 by convention.  Features with D % 128 == 0 only
+ * qr_backward_lists and qr_backward_clear accept them); z_max = 2 by convention.  Shapes of the tcgen05 path only
  * (QR_ERR_UNSUPPORTED otherwise).  ws must hold qr_stratified_workspace_bytes(cam, K, D) bytes.
  */
 size_t qr_stratified_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D);

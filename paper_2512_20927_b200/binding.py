@@ -299,8 +299,10 @@ def qr_forward(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, feature
 
 
 def lists_supported(features_dtype, D: int) -> bool:
-    """qr_forward leaves selection lists in its workspace for fp32 / fp16 features with D % 128 == 0 (include/qr.h)."""
-    return features_dtype in (torch.float32, torch.float16) and D % 128 == 0 and 128 <= D <= QR_MAX_D
+    """qr_forward leaves selection lists in its workspace on the tcgen05 path: fp32 / fp16 features with D % 32 == 0, or D < 32
+    with D % 4 == 0 (fp16: D % 8 == 0), D <= 512 (include/qr.h; the contractions run on whole 128-channel tiles, TMA pads)."""
+    ok = 4 <= D <= min(QR_MAX_D, 512) and (D % 32 == 0 or (D < 32 and D % 4 == 0))
+    return ok and (features_dtype == torch.float32 or (features_dtype == torch.float16 and D % 8 == 0))
 
 
 def qr_backward_workspace_bytes(cam, K: int, D: int) -> int:

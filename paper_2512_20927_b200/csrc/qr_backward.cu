@@ -484,7 +484,7 @@ extern "C" int qr_backward_lists(const qr_camera* cam, int32_t K, int32_t D, int
     if (K < 1) return fail(QR_ERR_INVALID_ARG, "qr_backward_lists: K = %d < 1", K);
     if (K > QR_MAX_K) return fail(QR_ERR_UNSUPPORTED, "qr_backward_lists: K = %d > QR_MAX_K", K);
     if (!backward_mma_supported(K, D))
-        return fail(QR_ERR_UNSUPPORTED, "qr_backward_lists: needs D %% 128 == 0, D <= 512 (D = %d): use qr_backward", D);
+        return fail(QR_ERR_UNSUPPORTED, "qr_backward_lists: needs D %% 32 == 0 (or D < 32 with D %% 4 == 0), D <= 512 (D = %d): use qr_backward", D);
     if (N < 0) return fail(QR_ERR_INVALID_ARG, "qr_backward_lists: N < 0");
     if (!fwd_ws || !dL_dmap) return fail(QR_ERR_NULL_POINTER, "qr_backward_lists: NULL input");
     if (N == 0) return QR_OK;

@@ -74,6 +74,7 @@ struct BmDesc {
 struct BmSmem {
     int W, stages, desc, bars, misc, total;
 };
+__host__ __device__ inline int bm_pad(int D) { return (D + 127) & ~127; }
 __host__ __device__ inline BmSmem bm_smem(int D, int stages)
 {
     BmSmem L;
@@ -129,7 +130,9 @@ __global__ void __launch_bounds__(kBmThreads, 1)
 backward_mma_kernel(const BackwardParams p, const int stages, const __grid_constant__ CUtensorMap g_tmap)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
-    const int D = p.D;
+    // D: the channel count the contraction runs on = p.D rounded up to whole 128-channel tiles (the TMA load fills channels
+    // beyond p.D with zeros, the epilogue does not write them); p.D itself only sizes the rows of dL_dfeat
+    const int D = bm_pad(p.D);
     const BmSmem L = bm_smem(D, stages);
     const int nchunks = D >> 7;                      // 128-channel MMA tiles
     const int stage_half = kBmStagePx * D * 4;       // bytes of a stage's hi (or lo) part
@@ -186,6 +189,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                          : "r"(taddr));
         };
         float* dcol = p.dL_dfeat + warp * 32 + lane;
+        const bool lastok = (nchunks - 1) * 128 + warp * 32 + lane < p.D;      // the last 128-channel tile may be partial
         for (int unit = 0;; ++unit) {
             const int buf = unit & 1;
             BPW(0, &tmem_full[buf], (unit >> 1) & 1);
@@ -214,10 +218,10 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                 for (int c = 0; c < 16; ++c) {
                     if (c0 + c < nrows && row[c0 + c] >= 0) {
                         float* a = dcol + row[c0 + c];
-                        bm_red(a, __uint_as_float(r0[c]));
-                        if (nchunks > 1) bm_red(a + 128, __uint_as_float(r1[c]));
-                        if (nchunks > 2) bm_red(a + 256, __uint_as_float(r2[c]));
-                        if (nchunks > 3) bm_red(a + 384, __uint_as_float(r3[c]));
+                        if (nchunks > 1 || lastok) bm_red(a, __uint_as_float(r0[c]));
+                        if (nchunks > 1 && (nchunks > 2 || lastok)) bm_red(a + 128, __uint_as_float(r1[c]));
+                        if (nchunks > 2 && (nchunks > 3 || lastok)) bm_red(a + 256, __uint_as_float(r2[c]));
+                        if (nchunks > 3 && lastok) bm_red(a + 384, __uint_as_float(r3[c]));
                     }
                 }
             }
@@ -404,7 +408,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
                             if (base == 0) {
                                 if (h == 0 && st < kBmRows && c_lo + st < U) {
                                     const int32_t id = __ldg(uid + c_lo + st);
-                                    rowoff = (uint32_t)id < (uint32_t)p.N ? (int64_t)id * D : -1;   // never add outside the table
+                                    rowoff = (uint32_t)id < (uint32_t)p.N ? (int64_t)id * p.D : -1;   // never add outside the table
                                 }
                                 BPW(8, &w_free[h], (unit & 1) ^ 1);      // the MMAs of the previous unit have read this half
                                 float4* wz = reinterpret_cast<float4*>(whi);
@@ -460,7 +464,7 @@ backward_mma_kernel(const BackwardParams p, const int stages, const __grid_const
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
 }
 
-bool backward_mma_supported(int32_t K, int32_t D) { return D % 128 == 0 && D >= 128 && D <= 512 && K >= 1 && K <= QR_MAX_K; }
+bool backward_mma_supported(int32_t K, int32_t D) { return tc_channels_supported(D) && K >= 1 && K <= QR_MAX_K; }
 
 // workspace = the common layout of qr_sel.cuh (the forward's workspace has the same one)
 size_t backward_mma_workspace_bytes(const Cam& cam, int K) { return ws_layout(cam, K).total; }
@@ -637,9 +641,12 @@ int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return fail(QR_ERR_CUDA, "qr_backward: cuTensorMapEncodeTiled is not available from the driver");
     CUtensorMap tmap;
-    const cuuint64_t dims[4] = { 32, (cuuint64_t)p.cam.width, (cuuint64_t)(p.D / 32), (cuuint64_t)p.cam.height };
+    // (D below 128-channel tiles: the box still spans whole tiles, what lies beyond D -- whole 32-channel groups, or the channels
+    // behind D < 32 -- is out of bounds for the tensor and arrives as zeros)
+    const int Dp = bm_pad(p.D);
+    const cuuint64_t dims[4] = { (cuuint64_t)min(32, p.D), (cuuint64_t)p.cam.width, (cuuint64_t)((p.D + 31) / 32), (cuuint64_t)p.cam.height };
     const cuuint64_t strides[3] = { (cuuint64_t)p.D * 4, 128, (cuuint64_t)p.D * 4 * (cuuint64_t)p.cam.width };
-    const cuuint32_t box[4] = { 32, kBmStagePx, (cuuint32_t)(p.D / 32), 1 };
+    const cuuint32_t box[4] = { 32, kBmStagePx, (cuuint32_t)(Dp / 32), 1 };
     const cuuint32_t estr[4] = { 1, 1, 1, 1 };
     const CUresult cr = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float*>(p.dL_dmap), dims, strides, box, estr,
                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
@@ -647,9 +654,9 @@ int launch_backward_mma(BackwardParams p, void* ws, size_t ws_bytes, cudaStream_
     if (cr != CUDA_SUCCESS) return fail(QR_ERR_CUDA, "qr_backward: cuTensorMapEncodeTiled failed (%d)", (int)cr);
     const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
     const unsigned grid = (unsigned)min(sms, num_half);
-    const int fixed = bm_smem(p.D, 0).total;
-    const int stages = max(2, min(12, (232448 - fixed - 1280) / (kBmStagePx * p.D * 4)));
-    const int smem = bm_smem(p.D, stages).total;
+    const int fixed = bm_smem(Dp, 0).total;
+    const int stages = max(2, min(12, (232448 - fixed - 1280) / (kBmStagePx * Dp * 4)));
+    const int smem = bm_smem(Dp, stages).total;
     if (!from_lists)
         if (int rc = launch_backward_prep(p, nflag, st)) return rc;
     QR_CUDA_OK(cudaFuncSetAttribute(backward_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));

@@ -149,7 +149,7 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + MmaSmem::tmem);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int D = p.D;
+    const int D = (p.D + kUnitN - 1) / kUnitN * kUnitN;      // whole 128-channel units; TMA pads the loads and clips the stores
     // fp16 features (R14: widened exactly): a raw row quarter is 256 bytes, the widened value IS the tf32 operand (10 explicit mantissa
     // bits: nothing to split off), so the F_lo buffer is never written and the third MMA is skipped
     const bool f16 = p.feat_f16 != 0;
@@ -594,7 +594,10 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
 }
 
-bool blend_mma_supported(int32_t D, qr_dtype feat_dtype) { return (feat_dtype == QR_F32 || feat_dtype == QR_F16) && D >= kUnitN && D % kUnitN == 0; }   // 128, 256, 384, 512
+bool blend_mma_supported(int32_t D, qr_dtype feat_dtype)
+{
+    return tc_channels_supported(D) && (feat_dtype == QR_F32 || (feat_dtype == QR_F16 && D % 8 == 0));
+}
 
 int launch_blend_mma(const BlendParams& p, cudaStream_t st, bool pdl)
 {

@@ -26,6 +26,11 @@ struct Cam {
     int32_t tiles_x, tiles_y;
 };
 
+// Channel counts the tcgen05 contractions (blend_mma_kernel, backward_mma_kernel) take: they work on whole 128-channel tiles and
+// let TMA pad (zeros on load, clipped on store).  The 32-channel groups of backward_mma_kernel's tensor map must be whole
+// (D % 32 == 0) or there must be a single partial one (D < 32); rows must be 16-byte multiples.
+inline bool tc_channels_supported(int32_t D) { return D >= 4 && D <= 512 && (D % 32 == 0 || (D < 32 && D % 4 == 0)); }
+
 inline Cam make_cam(const qr_camera* c)
 {
     Cam k;

@@ -1,7 +1,7 @@
 // qr_forward.cu -- qr_forward: Algorithm 1 for every pixel, then f~^Q = f^Q / (1 - T^Q).
 //
 // The call is split where the method itself splits (the O(N) transmittance walk, the O(KC) blend):
-//   fp32 features, D % 128 == 0   walk2_kernel (qr_walk.cu: selection lists per 16x8 half tile) -> blend_mma_kernel
+//   D % 32 == 0 or D < 32, D % 4 == 0 (padded to whole 128-channel tiles by TMA)   walk2_kernel (qr_walk.cu: selection lists per 16x8 half tile) -> blend_mma_kernel
 //                                 (qr_blend_mma.cu: the blend as a tcgen05 contraction); the dispatcher is at the end of
 //                                 this file
 //   every other shape             the kernels of THIS file:
@@ -13,7 +13,7 @@
 //   a pixel did not select it) to the group's list in the workspace -- the group's union of selected Gaussians, in depth
 //   order.  After the walk the same warp writes n_sel, T^Q and the used slots of the per-pixel selection records
 //   sel_idx / sel_w from the group lists it has just written.
-// blend_tu_kernel -- D % 4 == 0 (fp16 features, or fp32 with D % 128 != 0): persistent, warp-specialised, TMA-staged FFMA2
+// blend_tu_kernel -- D % 4 == 0 outside the tcgen05 shapes (e.g. D = 132): persistent, warp-specialised, TMA-staged FFMA2
 //   blend of the group records (described at the kernel).
 // blend_kernel    -- D % 4 != 0 (D <= 128): CTA = one tile, warp = one pixel group at a time, feature rows loaded once per
 //   record and applied to the 8 pixels of the group from registers; epilogue x 1/(1 - T^Q) (line 20), streaming stores.
@@ -964,7 +964,7 @@ static int forward_impl(const qr_camera* cam, int32_t K, int32_t D, qr_dtype fea
         return fail(QR_ERR_NULL_POINTER, "qr_forward: NULL output, tile_range or workspace");
     // out_map == NULL: selection only (walk, records, selection lists; no blend) -- the tcgen05 path only
     if (!out_map && !blend_mma_supported(D, feat_dtype))
-        return fail(QR_ERR_NULL_POINTER, "qr_forward: out_map is NULL (selection only needs fp32 features with D %% 128 == 0)");
+        return fail(QR_ERR_NULL_POINTER, "qr_forward: out_map is NULL (selection only needs a shape of the tcgen05 path: D %% 32 == 0, or D < 32 with D %% 4 == 0)");
     if (!aligned16(out_map) || !aligned16(features) || !aligned16(conic_opac) || !aligned16(mean2d) || !aligned16(ws))
         return fail(QR_ERR_MISALIGNED, "qr_forward: out_map / features / conic_opac / mean2d / ws must be 16-byte aligned");
     const Cam c = make_cam(cam);
@@ -973,14 +973,15 @@ static int forward_impl(const qr_camera* cam, int32_t K, int32_t D, qr_dtype fea
     if (ws_bytes < L.total + stats_bytes)
         return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_forward: workspace %zu < %zu bytes", ws_bytes, L.total + stats_bytes);
     if (strat && !blend_mma_supported(D, feat_dtype))
-        return fail(QR_ERR_UNSUPPORTED, "qr_forward_stratified: fp32 features with D %% 128 == 0 only (D = %d)", D);
+        return fail(QR_ERR_UNSUPPORTED, "qr_forward_stratified: shapes of the tcgen05 path only: D %% 32 == 0, or D < 32 with D %% 4 == 0 (D = %d)", D);
     cudaStream_t st = (cudaStream_t)stream;
     const int T = c.tiles_x * c.tiles_y;
     char* w = static_cast<char*>(ws);
 
     if (blend_mma_supported(D, feat_dtype)) {
-        // fp32 features, D % 256 == 0: walk2_kernel -> selection lists -> tcgen05 blend
-        if (!mean2d || !conic_opac || !isect_gauss || !features)
+        // walk2_kernel -> selection lists -> tcgen05 blend.  isect_gauss may be NULL when M = 0 (every tile range is empty: it
+        // is never read), as on the FFMA paths
+        if (!mean2d || !conic_opac || !features)
             return fail(QR_ERR_NULL_POINTER, "qr_forward: NULL input");
         WalkParams2 w2;
         w2.cam = c; w2.K = K;

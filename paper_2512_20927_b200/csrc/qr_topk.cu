@@ -202,7 +202,7 @@ __global__ void __launch_bounds__(256) records_blend_kernel(const Cam cam, const
 extern "C" size_t qr_topk_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D)
 {
     if (!cam || cam->width < 1 || cam->height < 1 || K < 1 || K > QR_TOPK_MAX_K) return 0;
-    if (D >= 128 && D % 128 == 0 && D <= QR_MAX_D) return qr::ws_layout(qr::make_cam(cam), K).total;
+    if (qr::tc_channels_supported(D)) return qr::ws_layout(qr::make_cam(cam), K).total;
     return 256;
 }
 

@@ -53,7 +53,8 @@ def test_bad_arguments_are_status_codes(lib):
     assert lib.qr_forward(C.byref(cam), 40, 1024, 0, p, p, p, p, p, p, p, p, p, p, p, 1 << 20, None) == -3
     assert lib.qr_forward(C.byref(cam), 40, 12, 1, p, p, p, p, p, p, p, p, p, p, p, 1 << 20, None) == -3
     # NULL outputs, too-small workspace
-    assert lib.qr_forward(C.byref(cam), 40, 16, 0, p, p, p, p, p, z, p, p, p, p, p, 1 << 20, None) == -2
+    assert lib.qr_forward(C.byref(cam), 40, 36, 0, p, p, p, p, p, z, p, p, p, p, p, 1 << 20, None) == -2      # D = 36: not a tcgen05 shape,
+    assert lib.qr_forward(C.byref(cam), 40, 16, 0, p, p, p, p, p, p, z, p, p, p, p, 1 << 20, None) == -2      # where out_map = NULL is legal
     need = lib.qr_forward_workspace_bytes(C.byref(cam), 40, 16)
     assert need > 0
     assert lib.qr_forward(C.byref(cam), 40, 16, 0, p, p, p, p, p, p, p, p, p, p, p, need - 1, None) == -4
@@ -72,7 +73,7 @@ def test_bad_arguments_are_status_codes(lib):
     assert tk(8, 16, -1.0, p, 1 << 20) == -1
     assert tk(8, 16, 1e-4, z, 1 << 20) == -2
     assert lib.qr_forward_stratified(C.byref(cam), 8, 128, 0, C.c_float(-1.0), C.c_float(2.0), p, p, p, p, p, p, p, p, p, p, p, 1 << 30, None) == -1
-    assert lib.qr_forward_stratified(C.byref(cam), 8, 16, 0, C.c_float(1e-4), C.c_float(2.0), p, p, p, p, p, p, p, p, p, p, p, 1 << 30, None) == -3
+    assert lib.qr_forward_stratified(C.byref(cam), 8, 36, 0, C.c_float(1e-4), C.c_float(2.0), p, p, p, p, p, p, p, p, p, p, p, 1 << 30, None) == -3
     assert lib.qr_stratified_workspace_bytes(C.byref(cam), 8, 128) == lib.qr_forward_workspace_bytes(C.byref(cam), 8, 128) + 64 * 64 * 8
     # batching: B out of range, unequal sizes, height % 16 != 0
     two = (binding.qr_camera * 2)(binding.make_camera(make_camera(64, 64)), binding.make_camera(make_camera(64, 48)))

@@ -101,7 +101,7 @@ def test_bin_sort_crowded_tiles(qr, orc, N, scale):
 def test_bin_sort_with_capacity_instead_of_count(qr, orc):
     """qr_bin_sort with M = an upper bound (no qr_bin_count, no host synchronisation): same lists and ranges, the
     found count is reported on the device; with a bound that is too small the lists are truncated, never overrun."""
-    sc = make_scene("cfg3", seed=13, N=80000, W=330, H=250, D=8)
+    sc = make_scene("cfg3", seed=13, N=80000, W=330, H=250, D=6)      # D = 6: a deterministic blend (the tcgen05 path's summation order follows a race)
     proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
     g = P.upload(sc)
     M = len(isect)
@@ -153,6 +153,9 @@ FWD_CASES = [
     ("cfg3", dict(N=40000, W=96, H=64, D=64), 200),             # K large
     ("cfg1", dict(W=70, H=50, D=256), 40),                      # tcgen05 blend on a ragged image (store guard, skipped half tiles)
     ("cfg3", dict(N=60000, W=100, H=72, D=512), 5),
+    ("cfg3", dict(N=40000, W=100, H=72, D=160), 40),            # tcgen05 path on padded tiles: 128 + 32 channels
+    ("cfg2", dict(N=20000, W=70, H=50, D=96), 12),              # ... one partial tile, ragged image
+    ("cfg1", dict(W=70, H=50, D=4), 40),                        # ... the smallest: 4 of 128 channels
     ("cfg3", dict(N=40000, W=100, H=72, D=3), 40),              # thread = pixel blend (D <= 8, D % 4 != 0)
     ("cfg2", dict(N=20000, W=64, H=48, D=7), 12),
     ("cfg1", dict(W=33, H=17, D=1), 3),
@@ -262,6 +265,11 @@ def test_dense_forward(qr, orc, name, kw, t_min):
                                        ("cfg2", dict(N=30000, W=64, H=40, D=128), 256),
                                        # thread = pixel backward (D <= 8, D % 4 != 0); K = 200 on the blob scene overflows
                                        # the tile's shared-memory hash table (direct global atomics for the rest)
+                                       # tcgen05 path on padded 128-channel tiles (TMA zero fill, epilogue guard)
+                                       ("cfg3", dict(N=40000, W=100, H=72, D=160), 10),
+                                       ("cfg2", dict(N=20000, W=70, H=50, D=96), 12),
+                                       ("cfg1", dict(W=70, H=50, D=16, backward=True), 40),
+                                       ("cfg1", dict(W=70, H=50, D=4, backward=True), 40),
                                        ("cfg3", dict(N=40000, W=100, H=72, D=3), 40),
                                        ("cfg3", dict(N=40000, W=64, H=48, D=3), 200),
                                        ("cfg2", dict(N=20000, W=64, H=48, D=7), 12),
@@ -610,11 +618,11 @@ def test_stratified_forward_and_backward(qr, orc, name, kw, K, t_min):
 
 
 def test_stratified_unsupported_shapes_are_status_codes(qr):
-    sc = make_scene("cfg1", seed=1)
+    sc = make_scene("cfg1", seed=1, D=36)
     g = P.upload(sc)
     fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
     with pytest.raises(qr.QRError) as e:
-        qr.pipeline.stratified_forward(sc.cam, fe, g.features, 8)          # D = 16: not on the tcgen05 path
+        qr.pipeline.stratified_forward(sc.cam, fe, g.features, 8)          # D = 36: not on the tcgen05 path (D % 32 != 0)
     assert e.value.code == -3
 
 
