@@ -591,7 +591,9 @@ def test_batch_of_views_equals_the_oracle_per_view(qr, orc, D, K, n_views):
 @pytest.mark.parametrize("name,kw,K,t_min", [("cfg3", dict(N=60000, W=160, H=112, D=512), 40, 1e-4),
                                              ("cfg2", dict(N=20000, W=96, H=64, D=256), 8, 1e-4),
                                              ("cfg1", dict(W=70, H=50, D=128), 16, 0.0),          # ragged image, whole-list statistics
-                                             ("cfg3", dict(N=60000, W=100, H=72, D=128), 1, 1e-4)])
+                                             ("cfg3", dict(N=60000, W=100, H=72, D=128), 1, 1e-4),
+                                             ("cfg2", dict(N=20000, W=96, H=64, D=64), 8, 1e-4),            # padded 128-channel tile
+                                             ("cfg1", dict(W=70, H=50), 16, 1e-4)])                         # D = 16
 def test_stratified_forward_and_backward(qr, orc, name, kw, K, t_min):
     sc = make_scene(name, seed=25, backward=True, **kw)
     proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
