@@ -210,6 +210,19 @@ int qr_dense_forward(const qr_camera* cam, int32_t D, qr_dtype feat_dtype, float
                      float* out_map, float* final_T, void* stream);
 
 /*
+ * qr_dense_forward_tc -- qr_dense_forward (same definition, same outputs) with the blend on the tensor cores: the walk emits every
+ * blended (Gaussian, pixel) pair with its weight T alpha' as selection lists and the tcgen05 contraction of qr_forward renders
+ * them, so that Q-Render is compared with a dense renderer built from the same parts.  `cap` = entries per pixel the lists hold
+ * (average over each 32-pixel list; 1..QR_MAX_K); half tiles that need more are rendered by qr_dense_forward's FFMA kernel
+ * inside the same call.  Shapes of the tcgen05 path only (see qr_forward; QR_ERR_UNSUPPORTED otherwise).  ws must hold
+ * qr_dense_workspace_bytes(cam, cap) bytes (scratch).  Results equal qr_dense_forward's to fp32 rounding (summation order).
+ */
+size_t qr_dense_workspace_bytes(const qr_camera* cam, int32_t cap);
+int qr_dense_forward_tc(const qr_camera* cam, int32_t D, qr_dtype feat_dtype, float t_min, int32_t cap,
+                        const float* mean2d, const float* conic_opac, const uint32_t* isect_gauss, const int32_t* tile_range,
+                        const void* features, float* out_map, float* final_T, void* ws, size_t ws_bytes, void* stream);
+
+/*
  * qr_topk_forward -- the paper's second comparator, top-K render ("top-K sampling ... requires additional
  * complexity to sort values, O(N log K + KC)"; complexity table; "top-K sorts and selects K
  * Gaussians").  The paper gives no procedure; this is the reconstruction of SPEC.md:221-229 (reading R17):

@@ -27,7 +27,7 @@ STATUS = {0: "QR_OK", -1: "QR_ERR_INVALID_ARG", -2: "QR_ERR_NULL_POINTER", -3: "
 # every symbol include/qr.h declares (tests check that the library exports exactly these)
 SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_bin_workspace_bytes", "qr_bin_count",
            "qr_bin_sort", "qr_forward_workspace_bytes", "qr_forward", "qr_backward_workspace_bytes", "qr_backward",
-           "qr_backward_lists", "qr_backward_clear", "qr_dense_forward", "qr_topk_workspace_bytes", "qr_topk_forward",
+           "qr_backward_lists", "qr_backward_clear", "qr_dense_forward", "qr_dense_workspace_bytes", "qr_dense_forward_tc", "qr_topk_workspace_bytes", "qr_topk_forward",
            "qr_launch_count", "qr_forward_stats", "qr_batch_camera", "qr_preprocess_batch", "qr_forward_batch",
            "qr_stratified_workspace_bytes", "qr_forward_stratified", "qr_devoxelize_workspace_bytes", "qr_devoxelize",
            "qr_devoxelize_backward", "qr_mask_loss_workspace_bytes", "qr_mask_loss", "qr_pooled_loss", "qr_sh_colors", "qr_mask_loss_static"]
@@ -90,6 +90,9 @@ def load() -> C.CDLL:
     lib.qr_backward_clear.argtypes = [cam, i32, i32, i64, vp, vp, vp, vp, sz, vp]
     lib.qr_dense_forward.restype = C.c_int
     lib.qr_dense_forward.argtypes = [cam, i32, C.c_int, f32, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.qr_dense_workspace_bytes.restype = sz; lib.qr_dense_workspace_bytes.argtypes = [cam, i32]
+    lib.qr_dense_forward_tc.restype = C.c_int
+    lib.qr_dense_forward_tc.argtypes = [cam, i32, C.c_int, f32, i32, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.qr_launch_count.restype = C.c_longlong; lib.qr_launch_count.argtypes = []
     lib.qr_forward_stats.restype = C.c_int; lib.qr_forward_stats.argtypes = [cam, i32, vp, sz, vp, vp]
     lib.qr_batch_camera.restype = C.c_int; lib.qr_batch_camera.argtypes = [cam, i32, cam]
@@ -372,6 +375,31 @@ def qr_dense_forward(cam, mean2d, conic_opac, isect_gauss, tile_range, features,
                                    _dev(features, features.dtype, "features"), out_map.data_ptr(), final_T.data_ptr(),
                                    _stream()))
     return out_map, final_T
+
+
+def qr_dense_forward_tc(cam, mean2d, conic_opac, isect_gauss, tile_range, features, t_min: float = 1e-4, cap: int = 128,
+                        out_map: Optional[torch.Tensor] = None, final_T: Optional[torch.Tensor] = None,
+                        ws: Optional[torch.Tensor] = None):
+    """qr_dense_forward with the blend on the tensor cores (include/qr.h qr_dense_forward_tc); cap = list capacity in
+    entries per pixel.  Returns (out_map, final_T, ws)."""
+    c = make_camera(cam)
+    H, W = c.height, c.width
+    D = int(features.shape[1])
+    dev = features.device
+    if out_map is None:
+        out_map = torch.empty((H, W, D), dtype=torch.float32, device=dev)
+    if final_T is None:
+        final_T = torch.empty((H, W), dtype=torch.float32, device=dev)
+    need = int(load().qr_dense_workspace_bytes(C.byref(c), int(cap)))
+    if ws is None or ws.numel() < need:
+        ws = torch.empty((max(need, 256),), dtype=torch.uint8, device=dev)
+    _check(load().qr_dense_forward_tc(C.byref(c), D, _feat_dtype(features), float(t_min), int(cap),
+                                      _dev(mean2d, torch.float32, "mean2d"), _dev(conic_opac, torch.float32, "conic_opac"),
+                                      isect_gauss.data_ptr() if isect_gauss.numel() else None,
+                                      _dev(tile_range, torch.int32, "tile_range"),
+                                      _dev(features, features.dtype, "features"), out_map.data_ptr(), final_T.data_ptr(),
+                                      ws.data_ptr(), ws.numel(), _stream()))
+    return out_map, final_T, ws
 
 
 def qr_topk_forward(cam, K: int, mean2d, conic_opac, isect_gauss, tile_range, features, t_min: float = 1e-4,

@@ -20,7 +20,9 @@
 //
 // fp32 decision arithmetic (power, alpha', T) uses explicit rounding intrinsics in the order fixed in DESIGN.md; the
 // library is also compiled with -fmad=false.
+#include "qr_blend.cuh"
 #include "qr_common.cuh"
+#include "qr_sel.cuh"
 
 namespace qr {
 
@@ -41,6 +43,7 @@ struct RenderParams {
     const void* features;
     float* out_map;
     float* final_T;
+    const int32_t* only_hdr = nullptr;   // qr_dense_forward_tc: headers of the selection lists; a band runs only if its half tile is flagged
 };
 
 template <typename FeatT, int VW> struct RowLoad;
@@ -100,6 +103,7 @@ __global__ void __launch_bounds__(kRenderThreads, 1) render_kernel(const RenderP
     const int tile_x = tile % p.cam.tiles_x, tile_y = tile / p.cam.tiles_x;
     const int x0 = tile_x * kTile, y0 = tile_y * kTile + band * kBandH;
     if (y0 >= p.cam.height) return;   // band entirely below the image
+    if (p.only_hdr && p.only_hdr[(size_t)(tile * 2 + (band >> 1)) * kHdrWords + 5] != 1) return;    // not left to this kernel
 
     // ---- init ----
     for (int i = tid; i < kBatch * kBandPx; i += kRenderThreads) Wb[i] = 0.0f;
@@ -352,4 +356,65 @@ extern "C" int qr_dense_forward(const qr_camera* cam, int32_t D, qr_dtype feat_d
     p.isect = isect_gauss; p.tile_range = reinterpret_cast<const int2*>(tile_range); p.features = features;
     p.out_map = out_map; p.final_T = final_T;
     return launch_render(p, feat_dtype, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// qr_dense_forward_tc: the same Eq. 1 on the tensor cores, so that the comparator is not an FFMA kernel measured against a
+// tcgen05 one.  walk2_kernel in dense mode emits every blended (Gaussian, pixel) pair with its weight T alpha' into the
+// selection-list format of qr_sel.cuh (columns = the Gaussians of the half tile's list prefix that some pixel blends), and
+// blend_mma_kernel -- unchanged -- contracts W[128 px, U] with F[U, D] in rounds of 64 columns.  The lists hold `cap`
+// entries per pixel on average over each 32-pixel list; a half tile that needs more is flagged by the walk and rendered
+// by render_kernel afterwards (it returns at once for every other band).
+// ------------------------------------------------------------------------------------------------------------------
+extern "C" size_t qr_dense_workspace_bytes(const qr_camera* cam, int32_t cap)
+{
+    if (!cam || cam->width < 1 || cam->height < 1 || cap < 1 || cap > QR_MAX_K) return 0;
+    return qr::ws_layout(qr::make_cam(cam), cap).total;
+}
+
+extern "C" int qr_dense_forward_tc(const qr_camera* cam, int32_t D, qr_dtype feat_dtype, float t_min, int32_t cap,
+                                   const float* mean2d, const float* conic_opac, const uint32_t* isect_gauss,
+                                   const int32_t* tile_range, const void* features, float* out_map, float* final_T,
+                                   void* ws, size_t ws_bytes, void* stream)
+{
+    using namespace qr;
+    if (int rc = check_cam(cam)) return rc;
+    if (int rc = check_feat(D, feat_dtype, "qr_dense_forward_tc")) return rc;
+    if (!(t_min >= 0.0f)) return fail(QR_ERR_INVALID_ARG, "qr_dense_forward_tc: t_min must be >= 0");
+    if (cap < 1 || cap > QR_MAX_K) return fail(QR_ERR_INVALID_ARG, "qr_dense_forward_tc: cap = %d outside [1, QR_MAX_K]", cap);
+    if (!blend_mma_supported(D, feat_dtype))
+        return fail(QR_ERR_UNSUPPORTED, "qr_dense_forward_tc: shapes of the tcgen05 path only (D %% 32 == 0, or D < 32 with D %% 4 == 0; D = %d): "
+                                        "use qr_dense_forward", D);
+    if (!tile_range || !out_map || !final_T || !mean2d || !conic_opac || !features || !ws)
+        return fail(QR_ERR_NULL_POINTER, "qr_dense_forward_tc: NULL argument");
+    if (!aligned16(out_map) || !aligned16(features) || !aligned16(conic_opac) || !aligned16(mean2d) || !aligned16(ws))
+        return fail(QR_ERR_MISALIGNED, "qr_dense_forward_tc: 16-byte alignment");
+    const Cam c = make_cam(cam);
+    const WsLayout L = ws_layout(c, cap);
+    if (ws_bytes < L.total) return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_dense_forward_tc: workspace %zu < %zu bytes", ws_bytes, L.total);
+    cudaStream_t st = (cudaStream_t)stream;
+    WalkParams2 w2;
+    w2.cam = c; w2.K = cap;
+    w2.mean2d = reinterpret_cast<const float2*>(mean2d);
+    w2.conic_opac = reinterpret_cast<const float4*>(conic_opac);
+    w2.isect = isect_gauss; w2.tile_range = reinterpret_cast<const int2*>(tile_range);
+    w2.n_sel = nullptr; w2.resid = final_T; w2.sel_idx = nullptr; w2.sel_w = nullptr;
+    w2.sl = sel_view(L.sel, ws);
+    w2.t_min = t_min;
+    if (int rc = launch_walk2_dense(w2, st)) return rc;
+    BlendParams bp;
+    bp.cam = c; bp.K = cap; bp.D = D; bp.cap = 0; bp.num_tiles = c.tiles_x * c.tiles_y; bp.tile_ticket = nullptr;
+    bp.features = features; bp.gcount = nullptr; bp.ucount = nullptr; bp.rec = nullptr;
+    bp.n_sel = nullptr; bp.resid = nullptr; bp.out_map = out_map; bp.sel_idx = nullptr; bp.sel_w = nullptr;
+    bp.sl = w2.sl;
+    bp.feat_f16 = feat_dtype == QR_F16 ? 1 : 0;
+    if (int rc = launch_blend_mma(bp, st)) return rc;
+    // half tiles whose lists were too small (flag in their header): the FFMA kernel, after the blend has written zeros there
+    RenderParams p;
+    p.cam = c; p.D = D; p.t_min = t_min;
+    p.mean2d = w2.mean2d; p.conic_opac = w2.conic_opac;
+    p.isect = isect_gauss; p.tile_range = w2.tile_range; p.features = features;
+    p.out_map = out_map; p.final_T = final_T;
+    p.only_hdr = w2.sl.hdr;
+    return launch_render(p, feat_dtype, st);
 }

@@ -128,5 +128,8 @@ struct WalkParams2 {
 };
 int launch_walk2(const WalkParams2& p, cudaStream_t st);
 int launch_walk2_stratified(const WalkParams2& p, cudaStream_t st);
+// dense comparator: entries = every blended (Gaussian, pixel) pair with its weight T alpha' (p.t_min: stop rule R7; p.resid receives
+// the final transmittance; p.K = list capacity in entries per pixel; no records: p.sel_idx / p.sel_w / p.n_sel unused)
+int launch_walk2_dense(const WalkParams2& p, cudaStream_t st);
 
 }  // namespace qr

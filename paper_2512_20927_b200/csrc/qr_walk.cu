@@ -53,7 +53,10 @@ __device__ __forceinline__ bool rect_hit(float mx, float my, float a, float b, f
 // MODE 0: Q-Render (Algorithm 1).  MODE 1: stratified-K pass 2 (reading R18): the same walk with
 // the per-pixel boundaries b_k = clamp(mu + sigma z_k, 0, 1) in place of 1 - (k+1)/(K+1).  MODE 2: stratified-K pass 1: the
 // dense transmittance statistics (mu, sigma) of every pixel, nothing else.
-enum { kWalkQ = 0, kWalkStrat = 1, kWalkStats = 2 };
+// MODE 3: DENSE (the comparator, Eq. 1 / qr_dense_forward on the tensor cores): every blended entry is emitted with its dense weight
+// T alpha' (stop rule R7 at t_min, no normalisation, no records); the lists have the capacity of K = p.K entries per pixel on
+// average, a half tile that needs more is flagged (hdr[5] = 1, empty lists) and left to the FFMA kernel.
+enum { kWalkQ = 0, kWalkStrat = 1, kWalkStats = 2, kWalkDense = 3 };
 
 template <int WX, int MODE>
 __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2 p)
@@ -66,7 +69,7 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
     __shared__ int32_t s_col[kW2Batch];    // column of a staged entry in the union, -1 = not selected yet, -2 = being numbered
     __shared__ float thr[QR_MAX_K + 1];
     __shared__ float zs[MODE == kWalkStrat ? QR_MAX_K + 1 : 1];     // z_k of the stratified boundaries
-    __shared__ int32_t s_ucount, s_evals, s_consumed;
+    __shared__ int32_t s_ucount, s_evals, s_consumed, s_ovf;
 
     __shared__ int32_t s_ht;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -108,9 +111,10 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
         if (MODE != kWalkStats && prev_ht >= 0) {
             int32_t* h = p.sl.hdr + (size_t)prev_ht * kHdrWords;
             h[4] = s_ucount; h[5] = 0; h[6] = s_consumed; h[7] = s_evals; h[8] = (int32_t)(clock64() - prev_start);
+            if (MODE == kWalkDense && s_ovf) { h[0] = h[1] = h[2] = h[3] = 0; h[4] = 0; h[5] = 1; }      // lists too small: FFMA kernel
             st_release(p.sl.flags + prev_ht, 1);
         }
-        s_ht = atomicAdd(p.sl.ctrl, 1); s_ucount = 0; s_evals = 0; s_consumed = 0;
+        s_ht = atomicAdd(p.sl.ctrl, 1); s_ucount = 0; s_evals = 0; s_consumed = 0; s_ovf = 0;
     }
     __syncthreads();
     const int ht = s_ht;
@@ -197,7 +201,12 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
             }
             return;
         }
-        const bool sel = T_test < thr_k;                                         // line 6
+        bool sel;
+        if (MODE == kWalkDense) {                                                // R7: stop before blending the entry that takes T below t_min
+            const bool stop = a > 0.0f && T_test < t_break;
+            sel = a > 0.0f && !stop;
+            if (stop) done = true;
+        } else sel = T_test < thr_k;                                             // line 6
         const uint32_t sm = __ballot_sync(0xffffffffu, sel);
         if (sm) {
             // column of this Gaussian in the half tile's union: the first warp to select it numbers it
@@ -210,7 +219,7 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
                 asm volatile("atom.shared.cas.b32 %0, [%1], -1, -2;" : "=r"(old) : "r"(slot) : "memory");
                 if (old == -1) {
                     asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(col) : "r"(s_ucount_addr) : "memory");
-                    uid_g[col] = id;
+                    if (MODE != kWalkDense || col < p.sl.ucap) uid_g[col] = id;
                     asm volatile("st.volatile.shared.b32 [%0], %1;" ::"r"(slot), "r"(col) : "memory");
                 } else {
                     col = old;
@@ -218,6 +227,16 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
                 }
             }
             col = __shfl_sync(0xffffffffu, col, 0);
+            if (MODE == kWalkDense) {
+                const int ne = __popc(sm);
+                if (n_ent + ne <= p.sl.qcap && col < p.sl.ucap) {                // warp-uniform
+                    if (sel) ent_ptr[__popc(sm & lt_mask)] = make_uint2(__float_as_uint(__fmul_rn(T, a)), ((uint32_t)col << 15) | (uint32_t)mpix);
+                    ent_ptr += ne;
+                    n_ent += ne;
+                } else if (lane == 0) s_ovf = 1;
+                if (sel) T = T_test;
+                return;
+            }
             if (sel) {
                 const float wQ = __fmul_rn(TQ, a);                               // line 8
                 *idx_ptr++ = id;
@@ -238,6 +257,7 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
             ent_ptr += ne;
             n_ent += ne;
         }
+        if (MODE == kWalkDense) return;                                          // (nothing selected in the warp: sel is false here)
         if (T_test < t_break) done = true;                                       // lines 15-17
         else T = T_test;                                                         // line 18
     };
@@ -309,6 +329,16 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
         }
         continue;
     }
+    if (MODE == kWalkDense) {                  // weights are final (Eq. 1 is not normalised); final_T = T
+        if (inside) p.resid[pix] = T;
+        if (lane == 0) {
+            hdr[warp] = n_ent;
+            atomicAdd(&s_evals, n_eval);
+            atomicMax(&s_consumed, consumed);
+        }
+        prev_ht = ht; prev_start = t_start;
+        continue;
+    }
     const float inv = ns > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, TQ)) : 0.0f;
     if (inside) {
         p.n_sel[pix] = ns;
@@ -366,6 +396,7 @@ static int launch_walk2_mode(const WalkParams2& p, cudaStream_t st)
 }
 
 int launch_walk2(const WalkParams2& p, cudaStream_t st) { return launch_walk2_mode<kWalkQ>(p, st); }
+int launch_walk2_dense(const WalkParams2& p, cudaStream_t st) { return launch_walk2_mode<kWalkDense>(p, st); }
 
 // stratified-K: pass 1 (statistics into p.stats), then pass 2 (the walk with the stratified boundaries)
 int launch_walk2_stratified(const WalkParams2& p, cudaStream_t st)

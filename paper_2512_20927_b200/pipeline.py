@@ -64,6 +64,12 @@ def dense_forward(cam, fe: Frontend, features: torch.Tensor, t_min: float = 1e-4
                               out_map, final_T)
 
 
+def dense_forward_tc(cam, fe: Frontend, features: torch.Tensor, t_min: float = 1e-4, cap: int = 128, out_map=None, final_T=None, ws=None):
+    """The dense comparator with the blend on the tensor cores (binding.qr_dense_forward_tc).  Returns (out_map, final_T, ws)."""
+    return B.qr_dense_forward_tc(cam, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, t_min, cap,
+                                 out_map, final_T, ws)
+
+
 def topk_forward(cam, fe: Frontend, features: torch.Tensor, K: int, t_min: float = 1e-4, out: Optional[B.ForwardOut] = None):
     """The top-K comparator on the same front end."""
     return B.qr_topk_forward(cam, K, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, t_min, out)

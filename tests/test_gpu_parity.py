@@ -248,6 +248,38 @@ def test_dense_forward(qr, orc, name, kw, t_min):
     np.testing.assert_allclose(fT[ok], v.final_T[ok], rtol=1e-4, atol=1e-7)
 
 
+@pytest.mark.parametrize("name,kw,t_min,cap", [("cfg3", dict(N=60000, W=128, H=80, D=512), 1e-4, 128),
+                                               ("cfg3", dict(N=60000, W=100, H=72, D=256), 0.0, 256),      # ragged, exact Eq. 1
+                                               ("cfg2", dict(N=20000, W=96, H=96), 1e-4, 64),              # D = 16: padded tile
+                                               ("cfg1", dict(W=70, H=50, D=128), 1e-4, 128),
+                                               # lists far too small: most half tiles are flagged and go to the FFMA kernel
+                                               ("cfg3", dict(N=60000, W=128, H=80, D=128), 1e-4, 4),
+                                               ("cfg3", dict(N=60000, W=128, H=80, D=128), 1e-4, 24)])
+def test_dense_forward_on_tensor_cores(qr, orc, name, kw, t_min, cap):
+    """qr_dense_forward_tc against the oracle's V-Render (the same bar as qr_dense_forward) and against qr_dense_forward."""
+    sc = make_scene(name, seed=8, **kw)
+    proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
+    lists = orc.pixel_lists(sc.cam, proj)
+    v = orc.vrender(lists, sc.features, t_min=t_min)
+    args = (sc.cam, P.to_dev(proj.mean2d), P.to_dev(proj.conic_opac), P.to_dev(isect.view(np.int32)), P.to_dev(rng), P.to_dev(sc.features), t_min)
+    om_t, fT_t, ws = qr.binding.qr_dense_forward_tc(*args, cap)
+    om_f, fT_f = qr.qr_dense_forward(*args)
+    H, W = sc.cam.height, sc.cam.width
+    om = om_t.cpu().numpy().reshape(H * W, -1).astype(np.float64); fT = fT_t.cpu().numpy().reshape(-1)
+    ok = ~((v.stop_margin <= 1e-5) | lists.borderline.astype(bool))       # early-stop decision within rounding
+    assert ok.mean() > 0.99
+    ref = v.out_map.astype(np.float64)
+    tol = P.ATOL + P.RTOL * np.abs(ref)
+    assert (np.abs(om - ref)[ok] <= tol[ok]).all(), float((np.abs(om - ref)[ok] / tol[ok]).max())
+    np.testing.assert_allclose(fT[ok], v.final_T[ok], rtol=1e-4, atol=1e-7)
+    assert torch.equal(fT_t, fT_f)                                        # the same fp32 decision arithmetic: identical T
+    torch.testing.assert_close(om_t, om_f, rtol=2e-4, atol=2e-5)
+    # second call into the same workspace (flags, tickets and lists of the first call are stale)
+    om2, fT2, _ = qr.binding.qr_dense_forward_tc(*args, cap, ws=ws)
+    assert torch.equal(fT2, fT_t)
+    torch.testing.assert_close(om2, om_t, rtol=2e-4, atol=2e-5)
+
+
 # ------------------------------------------------------------------------------------------------
 # qr_backward
 # ------------------------------------------------------------------------------------------------
