@@ -171,6 +171,29 @@ def workload_config(sc, name):
 # ----------------------------------------------------------------------------------------------------------------
 # CUDA arm
 # ----------------------------------------------------------------------------------------------------------------
+def _time_dense_tc(qr, pl, fr, cam, fe, out_map, out_T, cap=128, n=10, warm=3):
+    """qr_dense_forward_tc on the frame of `fr` (None where the shape is not one of the tcgen05 path): ms per call, list capacity,
+    half tiles the walk flagged (lists too small: rendered by the FFMA kernel inside the call)."""
+    import torch
+    feats = fr.d["features"]
+    if not qr.binding.lists_supported(feats.dtype, int(feats.shape[1])):
+        return None
+    st = {"ws": None}
+
+    def call():
+        _, _, st["ws"] = pl.dense_forward_tc(cam, fe, feats, 1e-4, cap, out_map, out_T, st["ws"])
+    ms = fr.time_call(call, n=n, warm=warm)
+    al = lambda v: (v + 255) // 256 * 256
+    nh = 2 * ((cam.width + 15) // 16) * ((cam.height + 15) // 16)
+    o = al(256 + 64)
+    hdr = al(o + (64 + nh) * 4)
+    h = st["ws"][hdr:hdr + nh * 64].view(torch.int32).view(nh, 16)
+    rec = {"ms": ms, "cap": cap, "flagged_half_tiles": int((h[:, 5] == 1).sum().item()), "half_tiles": nh,
+           "entries": int(h[:, :4].sum().item()), "union_mean": float(h[:, 4].float().mean().item())}
+    st["ws"] = None
+    return rec
+
+
 def _traffic(workload, D, K):
     """dram__bytes_read.sum + dram__bytes_write.sum per call from the committed ncu --set full capture of exactly this
     (workload, D, K) -- profiles/traffic.json names the capture -- else None."""
@@ -442,6 +465,7 @@ def run_cuda(args):
     dense_map = torch.empty((H, W, D), dtype=torch.float32, device=dev)
     dense_T = torch.empty((H, W), dtype=torch.float32, device=dev)
     dense_ms = fr.time_call(lambda: pl.dense_forward(cam, fe, fr.d["features"], 1e-4, dense_map, dense_T))
+    dense_tc = _time_dense_tc(qr, pl, fr, cam, fe, dense_map, dense_T)
     del dense_map
     topk_ms = None
     if K <= 64:
@@ -700,7 +724,10 @@ def run_cuda(args):
                            "topk_fwd_kernel": (npix / topk_ms / 1e3) if topk_ms else None},
                 "dense": {"ms": dense_ms, "speedup_qr_forward_over_dense": dense_ms / fwd_ms, "t_min": 1e-4,
                           "note": "render_kernel<1>: FFMA formulation without the tensor-core blend (DESIGN.md 5.5); the ratio "
-                                  "compares a tuned kernel with an untuned one"},
+                                  "compares a tuned kernel with an untuned one: see dense_tc for the like-for-like figure"},
+                "dense_tc": (dict(dense_tc, speedup_qr_forward_over_dense_tc=dense_tc["ms"] / fwd_ms,
+                                  note="qr_dense_forward_tc: walk2_kernel in dense mode + the same tcgen05 blend as Q-Render "
+                                       "(PAPER.md:353 reports 1.5x for Q-Render over V-Render at 512-D)") if dense_tc else None),
                 "topk": ({"ms": topk_ms, "K": K, "n_sel_mean": topk_nsel, "qr_forward_over_topk": topk_ms / fwd_ms,
                           "note": "same tcgen05 blend as Q-Render; selection by a per-pixel heap (O(N log K), PAPER.md:187)"}
                          if topk_ms else None),
@@ -761,6 +788,11 @@ def run_sweep(args, qr, dev, barrier):
             dT = torch.empty((cam.height, cam.width), dtype=torch.float32, device=dev)
             rec["dense_ms"] = fr.time_call(lambda: pl.dense_forward(cam, fe, fr.d["features"], 1e-4, dm, dT), n=3, warm=1)
             rec["dense_over_qr_forward"] = rec["dense_ms"] / r["fwd_ms"]
+            dtc = _time_dense_tc(qr, pl, fr, cam, fe, dm, dT, n=3, warm=1)
+            if dtc:
+                rec["dense_tc_ms"] = dtc["ms"]
+                rec["dense_tc_over_qr_forward"] = dtc["ms"] / r["fwd_ms"]
+                rec["dense_tc_flagged_half_tiles"] = dtc["flagged_half_tiles"]
             del dm
         if K <= 64:
             tk = {"out": None}

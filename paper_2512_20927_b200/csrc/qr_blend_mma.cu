@@ -536,10 +536,22 @@ blend_mma_kernel(const BlendParams p, const __grid_constant__ CUtensorMap out_tm
                 asm volatile("cp.async.wait_all;" ::: "memory");     // this warp's staged entries have landed
                 prod_sync();
                 const int c_lo = r * kWCols;
-                for (int i = lane; i < cur.n; i += 32) {
-                    const uint2 e = i < kEbuf ? ebuf[i] : __ldcg(tail + i);
+                for (int i = lane; i < min(cur.n, kEbuf); i += 32) {
+                    const uint2 e = ebuf[i];
                     const int cl = sel_col(e.y) - c_lo;
                     if (cl >= 0 && cl < kWCols) ws[sel_pixel(e.y) * kWsRow + cl] = __uint_as_float(e.x);
+                }
+                // the tail of a long list (rare for Q-Render; the rule for the dense comparator's lists, ~60 entries per pixel)
+                // comes straight from global memory, eight loads per lane in flight
+                for (int i0 = kEbuf + lane; i0 < cur.n; i0 += 32 * 8) {
+                    uint2 e[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) e[u] = i0 + 32 * u < cur.n ? __ldcg(tail + i0 + 32 * u) : make_uint2(0u, 0xFFFFFFFFu);
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const int cl = sel_col(e[u].y) - c_lo;            // padding: column 2^17 - 1, never in range
+                        if (cl >= 0 && cl < kWCols) ws[sel_pixel(e[u].y) * kWsRow + cl] = __uint_as_float(e[u].x);
+                    }
                 }
                 prod_sync();
 #ifdef QR_PROF

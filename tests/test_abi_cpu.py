@@ -65,6 +65,11 @@ def test_bad_arguments_are_status_codes(lib):
     assert lib.qr_preprocess(C.byref(cam), -1, p, p, p, p, p, p, p, p, p, None) == -1
     assert lib.qr_preprocess(C.byref(cam), 0, z, z, z, z, z, z, z, z, z, None) == 0      # N = 0 is legal
     assert lib.qr_dense_forward(C.byref(cam), 16, 0, C.c_float(-1.0), p, p, p, p, p, p, p, None) == -1
+    dtc = lambda D, t, cap, wsb: lib.qr_dense_forward_tc(C.byref(cam), D, 0, C.c_float(t), cap, p, p, p, p, p, p, p, p, wsb, None)
+    assert dtc(128, -1.0, 64, 1 << 30) == -1 and dtc(128, 1e-4, 0, 1 << 30) == -1 and dtc(128, 1e-4, 257, 1 << 30) == -1
+    assert dtc(36, 1e-4, 64, 1 << 30) == -3                    # not a shape of the tcgen05 path
+    assert dtc(128, 1e-4, 64, 1024) == -4 and lib.qr_dense_workspace_bytes(C.byref(cam), 64) > 1024
+    assert lib.qr_dense_workspace_bytes(C.byref(cam), 0) == 0
     assert lib.qr_backward(C.byref(cam), 0, 16, 10, p, p, p, p, p, None, 0, None) == -1
     # top-K comparator: K = 0 domain error, K > QR_TOPK_MAX_K unsupported, t_min < 0, NULL, small workspace
     tk = lambda K, D, t, out, wsb: lib.qr_topk_forward(C.byref(cam), K, D, 0, C.c_float(t), p, p, p, p, p, out, p, p, p, p, p, wsb, None)

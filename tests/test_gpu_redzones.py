@@ -119,6 +119,12 @@ def test_no_call_writes_outside_its_arrays(qr, name, kw, K):
     B._check(lib.qr_dense_forward(C.byref(c), D, 0, C.c_float(1e-4), ptr(mean2d), ptr(conic), ptr(isect), ptr(rng),
                                   ptr(inputs["features"]), ptr(dmap), ptr(dT), st))
     z.check("qr_dense_forward")
+    if B.lists_supported(torch.float32, D):
+        for cap in (64, 2):              # roomy lists; lists so small that the walk must stop emitting (flagged half tiles)
+            dws = z.alloc((int(lib.qr_dense_workspace_bytes(C.byref(c), cap)),), torch.uint8)
+            B._check(lib.qr_dense_forward_tc(C.byref(c), D, 0, C.c_float(1e-4), cap, ptr(mean2d), ptr(conic), ptr(isect), ptr(rng),
+                                             ptr(inputs["features"]), ptr(dmap), ptr(dT), ptr(dws), dws.numel(), st))
+            z.check(f"qr_dense_forward_tc(cap {cap})")
     kt = min(K, 64)
     t_map, t_idx, t_w, t_n, t_r = records(kt)
     tws = z.alloc((max(int(lib.qr_topk_workspace_bytes(C.byref(c), kt, D)), 256),), torch.uint8)
