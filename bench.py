@@ -810,6 +810,13 @@ def run_sweep(args, qr, dev, barrier):
         c = fr.counts()
         c.pop("n_sel_histogram", None)
         rec["counts"] = c
+        # the headline line's byte model at this point: fraction of the measured HBM peak each call reaches
+        esz = 2 if fr.d["features"].dtype == torch.float16 else 4
+        fb = r["M_found"] * 4 + c["N_visible"] * 32 + c["S_distinct_selected"] * D * esz + npix * D * 4 + npix * 4
+        bb = npix * D * 4 + c["S_distinct_selected"] * D * 4 + npix * (8 * K + 4)
+        peak, _src = _peaks()
+        rec["roofline"] = {"peak_gb_s": peak, "fwd_bytes": fb, "fwd_frac": fb / (r["fwd_ms"] * 1e-3) / 1e9 / peak,
+                           "bwd_bytes": bb, "bwd_frac": bb / (r["bwd_ms"] * 1e-3) / 1e9 / peak}
         if lists is not None:
             rec["parity"] = _parity_counts(orc, lists, K, fr.fwd_out)
         print(json.dumps(rec), file=sys.stderr, flush=True)
