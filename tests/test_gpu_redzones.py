@@ -142,3 +142,61 @@ def test_no_call_writes_outside_its_arrays(qr, name, kw, K):
         assert torch.equal(shc, keep), "sh was modified"
     for k, v in inputs.items():
         assert torch.equal(v, before[k]), f"input {k} was modified"
+
+
+@pytest.mark.parametrize("W,H,D,S,K", [(96, 64, 128, 12, 16), (70, 50, 512, 5, 40)])
+def test_neighbour_calls_write_inside_their_arrays(qr, W, H, D, S, K):
+    """The same canaries around the outputs and workspaces of the path's neighbours and variants: qr_forward_stratified,
+    qr_pooled_loss, qr_mask_loss, qr_mask_loss_static, qr_devoxelize / qr_devoxelize_backward, qr_sh_colors is covered above."""
+    import ctypes as C
+    B = qr.binding
+    lib = B.load()
+    sc = make_scene("cfg2", seed=33, N=20000, W=W, H=H, D=D)
+    cam, N = sc.cam, sc.N
+    c = B.make_camera(cam)
+    st = B._stream()
+    ptr = lambda t: t.data_ptr()
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    g = {k: dev(getattr(sc, k)) for k in ("means", "scales", "quats", "opac", "features")}
+    fe = qr.pipeline.frontend(cam, g["means"], g["scales"], g["quats"], g["opac"])
+    rng = np.random.default_rng(5)
+    z = Zones()
+    # qr_forward_stratified
+    out_map, sel_idx, sel_w = z.alloc((H, W, D), torch.float32), z.alloc((H, W, K), torch.int32), z.alloc((H, W, K), torch.float32)
+    n_sel, resid = z.alloc((H, W), torch.int32), z.alloc((H, W), torch.float32)
+    sws = z.alloc((int(lib.qr_stratified_workspace_bytes(C.byref(c), K, D)),), torch.uint8)
+    B._check(lib.qr_forward_stratified(C.byref(c), K, D, 0, C.c_float(1e-4), C.c_float(2.0), ptr(fe.proj.mean2d), ptr(fe.proj.conic_opac),
+                                       ptr(fe.isect_gauss), ptr(fe.tile_range), ptr(g["features"]), ptr(out_map), ptr(sel_idx), ptr(sel_w),
+                                       ptr(n_sel), ptr(resid), ptr(sws), sws.numel(), st))
+    z.check("qr_forward_stratified")
+    # qr_forward (lists in its workspace) -> qr_pooled_loss
+    fws = z.alloc((int(B.qr_forward_workspace_bytes(cam, K, D)),), torch.uint8)
+    B._check(lib.qr_forward(C.byref(c), K, D, 0, ptr(fe.proj.mean2d), ptr(fe.proj.conic_opac), ptr(fe.isect_gauss), ptr(fe.tile_range),
+                            ptr(g["features"]), ptr(out_map), ptr(sel_idx), ptr(sel_w), ptr(n_sel), ptr(resid), ptr(fws), fws.numel(), st))
+    mid = dev(((np.arange(H)[:, None] // 16) * 3 + np.arange(W)[None, :] // 32).astype(np.int32) % S)
+    tg = dev(rng.standard_normal((S, D)).astype(np.float32))
+    loss, per = z.alloc((1,), torch.float32), z.alloc((S,), torch.float32)
+    dF = z.alloc((N, D), torch.float32); dF.zero_()
+    mws = z.alloc((int(lib.qr_mask_loss_workspace_bytes(S, D)),), torch.uint8)
+    B._check(lib.qr_pooled_loss(C.byref(c), K, D, N, ptr(fws), fws.numel(), ptr(g["features"]), ptr(mid), S, ptr(tg), ptr(loss), ptr(per),
+                                ptr(dF), ptr(mws), mws.numel(), st))
+    z.check("qr_pooled_loss")
+    # qr_mask_loss with a workspace, and with the library's static scratch
+    d_map = z.alloc((H, W, D), torch.float32)
+    B._check(lib.qr_mask_loss(C.byref(c), D, S, ptr(out_map), ptr(mid), ptr(tg), ptr(loss), ptr(per), ptr(d_map), ptr(mws), mws.numel(), st))
+    z.check("qr_mask_loss")
+    B._check(lib.qr_mask_loss_static(C.byref(c), D, S, ptr(out_map), ptr(mid), ptr(tg), ptr(loss), ptr(per), ptr(d_map), st))
+    z.check("qr_mask_loss_static")
+    # qr_devoxelize / qr_devoxelize_backward, both reductions
+    U, G = 3000, 2000
+    uni = dev(rng.standard_normal((U, D)).astype(np.float32))
+    counts = dev(rng.integers(0, 6, G).astype(np.int32))
+    inv = dev(rng.integers(0, U, int(counts.sum().item())).astype(np.int64))
+    for reduce in (0, 1):
+        gs, am = z.alloc((G, D), torch.float32), z.alloc((G, D), torch.int32)
+        dws = z.alloc((int(lib.qr_devoxelize_workspace_bytes(G)),), torch.uint8)
+        B._check(lib.qr_devoxelize(U, D, G, ptr(uni), ptr(inv), ptr(counts), reduce, ptr(gs), ptr(am), ptr(dws), dws.numel(), st))
+        z.check(f"qr_devoxelize(reduce {reduce})")
+        d_uni = z.alloc((U, D), torch.float32); d_uni.zero_()
+        B._check(lib.qr_devoxelize_backward(U, D, G, ptr(inv), reduce, ptr(am), ptr(gs), ptr(d_uni), ptr(dws), dws.numel(), st))
+        z.check(f"qr_devoxelize_backward(reduce {reduce})")
