@@ -188,8 +188,9 @@ def test_forward_end_to_end(qr, orc, name, kw, K):
     print(stats)
 
 
-def test_forward_fp16_features(qr, orc):
-    sc = make_scene("cfg4", seed=6, N=60000, W=128, H=96, D=512, pose=2)      # fp16 storage, fp32 accumulation (R14)
+@pytest.mark.parametrize("D", [512, 64, 24, 40])      # 64, 24: padded 128-channel tile; 40: D % 32 != 0 -> blend_tu_kernel
+def test_forward_fp16_features(qr, orc, D):
+    sc = make_scene("cfg4", seed=6, N=60000, W=128, H=96, D=D, pose=2)        # fp16 storage, fp32 accumulation (R14)
     assert sc.features.dtype == np.float16
     proj, rect, touched, isect, rng = P.oracle_frontend(orc, sc)
     lists = orc.pixel_lists(sc.cam, proj)
