@@ -210,6 +210,23 @@ int qr_dense_forward(const qr_camera* cam, int32_t D, qr_dtype feat_dtype, float
                      float* out_map, float* final_T, void* stream);
 
 /*
+ * qr_forward_multik -- qr_forward for nK values of K in ONE walk ("multi-K in one walk"; the K sweep of
+ * BASELINE.json configs[3]).  Staging, culling, alpha' and the dense transmittance are computed once; every K
+ * has its own boundaries, records and selection lists, and its own blend.  For each K the outputs are those of
+ * qr_forward(cam, K, ...): identical n_sel, sel_idx, sel_w and resid_TQ; the same map to fp32 summation order; the same
+ * selection lists in ws[j] (qr_backward_lists / qr_backward_clear / qr_pooled_loss take ws[j] with K[j]).
+ *   Ks: HOST array of nK values in [1, QR_MAX_K], nK in [1, QR_MAX_MULTI_K].
+ *   out_map, sel_idx, sel_w, n_sel, resid_TQ, ws: HOST arrays of nK DEVICE pointers (out_map[j] may be NULL: selection only);
+ *   ws_bytes[j] >= qr_forward_workspace_bytes(cam, K[j], D); the workspaces must be distinct.
+ * Shapes of the tcgen05 path only (QR_ERR_UNSUPPORTED otherwise).
+ */
+#define QR_MAX_MULTI_K 4
+int qr_forward_multik(const qr_camera* cam, int32_t nK, const int32_t* Ks, int32_t D, qr_dtype feat_dtype,
+                      const float* mean2d, const float* conic_opac, const uint32_t* isect_gauss, const int32_t* tile_range,
+                      const void* features, float* const* out_map, int32_t* const* sel_idx, float* const* sel_w,
+                      int32_t* const* n_sel, float* const* resid_TQ, void* const* ws, const size_t* ws_bytes, void* stream);
+
+/*
  * qr_dense_forward_tc -- qr_dense_forward (same definition, same outputs) with the blend on the tensor cores: the walk emits every
  * blended (Gaussian, pixel) pair with its weight T alpha' as selection lists and the tcgen05 contraction of qr_forward renders
  * them, so that Q-Render is compared with a dense renderer built from the same parts.  `cap` = entries per pixel the lists hold

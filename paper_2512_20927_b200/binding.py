@@ -30,7 +30,7 @@ SYMBOLS = ["qr_version", "qr_last_error", "qr_num_tiles", "qr_preprocess", "qr_b
            "qr_backward_lists", "qr_backward_clear", "qr_dense_forward", "qr_dense_workspace_bytes", "qr_dense_forward_tc", "qr_topk_workspace_bytes", "qr_topk_forward",
            "qr_launch_count", "qr_forward_stats", "qr_batch_camera", "qr_preprocess_batch", "qr_forward_batch",
            "qr_stratified_workspace_bytes", "qr_forward_stratified", "qr_devoxelize_workspace_bytes", "qr_devoxelize",
-           "qr_devoxelize_backward", "qr_mask_loss_workspace_bytes", "qr_mask_loss", "qr_pooled_loss", "qr_sh_colors", "qr_mask_loss_static"]
+           "qr_devoxelize_backward", "qr_mask_loss_workspace_bytes", "qr_mask_loss", "qr_pooled_loss", "qr_sh_colors", "qr_mask_loss_static", "qr_forward_multik"]
 
 
 class QRError(RuntimeError):
@@ -109,6 +109,8 @@ def load() -> C.CDLL:
     lib.qr_devoxelize_backward.argtypes = [i64, i32, i64, vp, i32, vp, vp, vp, vp, sz, vp]
     lib.qr_mask_loss_workspace_bytes.restype = sz; lib.qr_mask_loss_workspace_bytes.argtypes = [i32, i32]
     lib.qr_mask_loss.restype = C.c_int; lib.qr_mask_loss.argtypes = [cam, i32, i32, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.qr_forward_multik.restype = C.c_int
+    lib.qr_forward_multik.argtypes = [cam, i32, vp, i32, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.qr_mask_loss_static.restype = C.c_int; lib.qr_mask_loss_static.argtypes = [cam, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.qr_pooled_loss.restype = C.c_int
     lib.qr_pooled_loss.argtypes = [cam, i32, i32, i64, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, sz, vp]
@@ -650,3 +652,37 @@ def qr_mask_loss_static(cam, feature_map, mask_id, targets, loss: Optional[torch
                                       _dev(targets, torch.float32, "targets"), _dev(loss, torch.float32, "loss"),
                                       _dev(loss_per_mask, torch.float32, "loss_per_mask"), _dev(d_map, torch.float32, "d_map"), _stream()))
     return loss, loss_per_mask, d_map
+
+
+def qr_forward_multik(cam, Ks, mean2d, conic_opac, isect_gauss, tile_range, features, outs=None):
+    """qr_forward for up to four K in one walk (include/qr.h qr_forward_multik).  Returns a list of ForwardOut, one per K, each
+    with a workspace of its own that holds that K's selection lists (pass `outs` to reuse the outputs of an earlier call)."""
+    c = make_camera(cam)
+    H, W = c.height, c.width
+    D = int(features.shape[1])
+    dev = features.device
+    Ks = [int(k) for k in Ks]
+    n = len(Ks)
+    if outs is None:
+        outs = []
+        for K in Ks:
+            kk = max(K, 1)
+            o = ForwardOut(torch.empty((H, W, D), dtype=torch.float32, device=dev),
+                           torch.empty((H, W, kk), dtype=torch.int32, device=dev),
+                           torch.empty((H, W, kk), dtype=torch.float32, device=dev),
+                           torch.empty((H, W), dtype=torch.int32, device=dev),
+                           torch.empty((H, W), dtype=torch.float32, device=dev))
+            o.ws = torch.empty((max(qr_forward_workspace_bytes(c, K, D), 256),), dtype=torch.uint8, device=dev)
+            outs.append(o)
+    arr_i = (C.c_int32 * max(n, 1))(*Ks)
+    parr = lambda ts: (C.c_void_p * max(n, 1))(*[t.data_ptr() for t in ts])
+    sizes = (C.c_size_t * max(n, 1))(*[o.ws.numel() for o in outs])
+    _check(load().qr_forward_multik(C.byref(c), n, arr_i, D, _feat_dtype(features), _dev(mean2d, torch.float32, "mean2d"),
+                                    _dev(conic_opac, torch.float32, "conic_opac"), _dev(isect_gauss, torch.int32, "isect_gauss"),
+                                    _dev(tile_range, torch.int32, "tile_range"), _dev(features, features.dtype, "features"),
+                                    parr([o.out_map for o in outs]), parr([o.sel_idx for o in outs]), parr([o.sel_w for o in outs]),
+                                    parr([o.n_sel for o in outs]), parr([o.resid_TQ for o in outs]), parr([o.ws for o in outs]),
+                                    sizes, _stream()))
+    for o in outs:
+        o.has_lists = True
+    return outs

@@ -1070,6 +1070,63 @@ extern "C" int qr_forward_batch(const qr_camera* tall, int32_t B, int64_t N, int
                         n_sel, resid_TQ, ws, ws_bytes, stream, (int32_t)N, tall->height / B);
 }
 
+// Several K in one walk: walk2_multi_kernel fills the selection lists of every K, then one tcgen05
+// blend per K renders its map.  Pointer arrays are HOST arrays of nK device pointers.
+extern "C" int qr_forward_multik(const qr_camera* cam, int32_t nK, const int32_t* Ks, int32_t D, qr_dtype feat_dtype,
+                                 const float* mean2d, const float* conic_opac, const uint32_t* isect_gauss,
+                                 const int32_t* tile_range, const void* features, float* const* out_map,
+                                 int32_t* const* sel_idx, float* const* sel_w, int32_t* const* n_sel, float* const* resid_TQ,
+                                 void* const* ws, const size_t* ws_bytes, void* stream)
+{
+    using namespace qr;
+    if (int rc = check_cam(cam)) return rc;
+    if (nK < 1 || nK > QR_MAX_MULTI_K) return fail(QR_ERR_INVALID_ARG, "qr_forward_multik: nK = %d outside [1, QR_MAX_MULTI_K]", nK);
+    if (!Ks || !out_map || !sel_idx || !sel_w || !n_sel || !resid_TQ || !ws || !ws_bytes)
+        return fail(QR_ERR_NULL_POINTER, "qr_forward_multik: NULL pointer array");
+    if (int rc = check_feat(D, feat_dtype, "qr_forward_multik")) return rc;
+    if (!blend_mma_supported(D, feat_dtype))
+        return fail(QR_ERR_UNSUPPORTED, "qr_forward_multik: shapes of the tcgen05 path only (D %% 32 == 0, or D < 32 with D %% 4 == 0; D = %d)", D);
+    if (!tile_range || !mean2d || !conic_opac || !features) return fail(QR_ERR_NULL_POINTER, "qr_forward_multik: NULL input");
+    if (!aligned16(features) || !aligned16(conic_opac) || !aligned16(mean2d))
+        return fail(QR_ERR_MISALIGNED, "qr_forward_multik: features / conic_opac / mean2d must be 16-byte aligned");
+    const Cam c = make_cam(cam);
+    WalkParamsMulti wp;
+    wp.cam = c; wp.nK = nK;
+    wp.mean2d = reinterpret_cast<const float2*>(mean2d);
+    wp.conic_opac = reinterpret_cast<const float4*>(conic_opac);
+    wp.isect = isect_gauss; wp.tile_range = reinterpret_cast<const int2*>(tile_range);
+    for (int j = 0; j < kMaxMultiK; ++j) {
+        const int jj = j < nK ? j : 0;                      // unused slots repeat slot 0 (never touched by the kernel)
+        const int K = Ks[jj];
+        if (K < 1) return fail(QR_ERR_INVALID_ARG, "qr_forward_multik: K[%d] = %d < 1", jj, K);
+        if (K > QR_MAX_K) return fail(QR_ERR_UNSUPPORTED, "qr_forward_multik: K[%d] = %d > QR_MAX_K", jj, K);
+        if (!sel_idx[jj] || !sel_w[jj] || !n_sel[jj] || !resid_TQ[jj] || !ws[jj])
+            return fail(QR_ERR_NULL_POINTER, "qr_forward_multik: NULL output or workspace for K[%d]", jj);
+        if (!aligned16(out_map[jj]) || !aligned16(ws[jj])) return fail(QR_ERR_MISALIGNED, "qr_forward_multik: out_map / ws of K[%d]", jj);
+        const FwdLayout L = fwd_layout(c, K);
+        if (ws_bytes[jj] < L.total)
+            return fail(QR_ERR_WORKSPACE_TOO_SMALL, "qr_forward_multik: workspace of K[%d]: %zu < %zu bytes", jj, ws_bytes[jj], L.total);
+        for (int i = 0; i < jj; ++i)
+            if (j < nK && ws[i] == ws[jj]) return fail(QR_ERR_INVALID_ARG, "qr_forward_multik: K[%d] and K[%d] share a workspace", i, jj);
+        wp.K[j] = K;
+        wp.n_sel[j] = n_sel[jj]; wp.resid[j] = resid_TQ[jj]; wp.sel_idx[j] = sel_idx[jj]; wp.sel_w[j] = sel_w[jj];
+        wp.sl[j] = sel_view(L.sel, ws[jj]);
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    if (int rc = launch_walk2_multi(wp, st)) return rc;
+    for (int j = 0; j < nK; ++j) {
+        if (!out_map[j]) continue;                          // selection only for this K
+        BlendParams bp;
+        bp.cam = c; bp.K = wp.K[j]; bp.D = D; bp.cap = 0; bp.num_tiles = c.tiles_x * c.tiles_y; bp.tile_ticket = nullptr;
+        bp.features = features; bp.gcount = nullptr; bp.ucount = nullptr; bp.rec = nullptr;
+        bp.n_sel = wp.n_sel[j]; bp.resid = wp.resid[j]; bp.out_map = out_map[j]; bp.sel_idx = wp.sel_idx[j]; bp.sel_w = wp.sel_w[j];
+        bp.sl = wp.sl[j];
+        bp.feat_f16 = feat_dtype == QR_F16 ? 1 : 0;
+        if (int rc = launch_blend_mma(bp, st, j == 0)) return rc;      // the first blend overlaps the walk's tail (PDL), the others follow
+    }
+    return QR_OK;
+}
+
 extern "C" size_t qr_stratified_workspace_bytes(const qr_camera* cam, int32_t K, int32_t D)
 {
     const size_t base = qr_forward_workspace_bytes(cam, K, D);

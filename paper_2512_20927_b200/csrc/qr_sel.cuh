@@ -126,6 +126,25 @@ struct WalkParams2 {
     float2* stats = nullptr;   // stratified-K: per pixel (mu, sigma) of the dense transmittance values (pass 1 writes, pass 2 reads)
     float t_min = 0.0f, z_max = 2.0f;
 };
+// Several K in ONE walk (second half): staging, culling, alpha' and the dense transmittance T are shared,
+// every K has its own boundaries, T^Q, records and selection lists.
+constexpr int kMaxMultiK = 4;
+struct WalkParamsMulti {
+    Cam cam;
+    int32_t nK;
+    int32_t K[kMaxMultiK];
+    const float2* mean2d;
+    const float4* conic_opac;
+    const uint32_t* isect;
+    const int2* tile_range;
+    int32_t* n_sel[kMaxMultiK];
+    float* resid[kMaxMultiK];
+    int32_t* sel_idx[kMaxMultiK];
+    float* sel_w[kMaxMultiK];
+    SelLists sl[kMaxMultiK];
+};
+int launch_walk2_multi(const WalkParamsMulti& p, cudaStream_t st);
+
 int launch_walk2(const WalkParams2& p, cudaStream_t st);
 int launch_walk2_stratified(const WalkParams2& p, cudaStream_t st);
 // dense comparator: entries = every blended (Gaussian, pixel) pair with its weight T alpha' (p.t_min: stop rule R7; p.resid receives

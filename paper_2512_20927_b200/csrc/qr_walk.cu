@@ -376,6 +376,303 @@ __global__ void __launch_bounds__(kW2Threads, 10) walk2_kernel(const WalkParams2
   }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// walk2_multi_kernel: Algorithm 1 for NK values of K in ONE pass over the lists ("multi-K in one walk").
+// What the K share: the staged batch, the culling test, alpha' and the dense transmittance T (line 5 / line 18 do not depend
+// on K).  What each K keeps: its boundaries 1 - (k+1)/(K+1), its index k, T^Q, its stop test T_test < 1/(K+1), its records and
+// its selection lists with their own union numbering (the workspaces are qr_forward's, one per K, so qr_backward_lists and
+// the blend take them as they are).  For every K the decisions and the fp32 values are those of walk2_kernel run with that K:
+// T evolves identically while the K is active, and a K that has stopped for a pixel selects nothing more there.
+// ------------------------------------------------------------------------------------------------------------------
+template <int NK>
+__global__ void __launch_bounds__(kW2Threads, 4) walk2_multi_kernel(const WalkParamsMulti p)
+{
+    constexpr int WX = 16, WY = 2;
+    __shared__ float4 s_co[kW2Batch];
+    __shared__ float4 s_cull[kW2Batch];
+    __shared__ float2 s_xy[kW2Batch];
+    __shared__ int32_t s_id[kW2Batch];
+    __shared__ int32_t s_col[NK][kW2Batch];
+    __shared__ float thr[NK][QR_MAX_K + 1];
+    __shared__ int32_t s_ucount[NK], s_evals, s_consumed, s_ht;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    int Kj[NK];
+    float t_break[NK];
+#pragma unroll
+    for (int j = 0; j < NK; ++j) {
+        Kj[j] = p.K[j];
+        for (int k = tid; k <= Kj[j]; k += kW2Threads)                    // thresholds as printed (R3)
+            thr[j][k] = __fsub_rn(1.0f, __fdiv_rn((float)(k + 1), (float)(Kj[j] + 1)));
+        t_break[j] = __fdiv_rn(1.0f, (float)(Kj[j] + 1));
+    }
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (blockIdx.x == 0 && tid == 0) {
+#pragma unroll
+        for (int j = 0; j < NK; ++j) {
+            int32_t* sp = p.sl[j].stamp;
+            sp[0] = kSelMagic; sp[1] = p.cam.width; sp[2] = p.cam.height; sp[3] = Kj[j];
+            const unsigned long long a = (unsigned long long)p.sel_idx[j];
+            sp[4] = (int32_t)(a & 0xffffffffull); sp[5] = (int32_t)(a >> 32);
+            stamp_time(p.sl[j].ctrl, 0, true);
+        }
+    }
+
+  int prev_ht = -1;
+  long long prev_start = 0;
+  while (true) {
+    __syncthreads();
+    if (tid == 0) {
+        if (prev_ht >= 0) {
+#pragma unroll
+            for (int j = 0; j < NK; ++j) {
+                int32_t* h = p.sl[j].hdr + (size_t)prev_ht * kHdrWords;
+                h[4] = s_ucount[j]; h[5] = 0; h[6] = s_consumed; h[7] = s_evals; h[8] = (int32_t)(clock64() - prev_start);
+                st_release(p.sl[j].flags + prev_ht, 1);
+            }
+        }
+        s_ht = atomicAdd(p.sl[0].ctrl, 1); s_evals = 0; s_consumed = 0;
+#pragma unroll
+        for (int j = 0; j < NK; ++j) s_ucount[j] = 0;
+    }
+    __syncthreads();
+    const int ht = s_ht;
+    if (ht >= num_half) {
+        if (tid == 0)
+            for (int j = 0; j < NK; ++j) stamp_time(p.sl[j].ctrl, 1, false);
+        break;
+    }
+    prev_ht = -1;
+    const int tile = ht >> 1;
+    const int x0 = (tile % p.cam.tiles_x) * kTile, y0 = (tile / p.cam.tiles_x) * kTile + (ht & 1) * 8;
+    if (y0 >= p.cam.height) {                         // half tile below the image: empty lists
+#pragma unroll
+        for (int j = 0; j < NK; ++j)
+            if (tid < kHdrWords) p.sl[j].hdr[(size_t)ht * kHdrWords + tid] = 0;
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence();
+            for (int j = 0; j < NK; ++j) st_release(p.sl[j].flags + ht, 1);
+        }
+        continue;
+    }
+    const int by0 = 2 * warp;
+    const int lx = lane & (WX - 1), ly = lane / WX;
+    const int mpix = (by0 + ly) * kTile + lx;
+    const int px = x0 + lx, py = y0 + by0 + ly;
+    const bool inside = px < p.cam.width && py < p.cam.height;
+    const float fpx = (float)px + 0.5f, fpy = (float)py + 0.5f;          // R5
+    const float X0 = (float)x0 + 0.5f, X1 = X0 + (float)(WX - 1);
+    const float Y0 = (float)(y0 + by0) + 0.5f, Y1 = Y0 + (float)(WY - 1);
+    const int64_t pix = (int64_t)py * p.cam.width + px;
+    const long long t_start = clock64();
+    const int2 range = p.tile_range[tile];
+
+    // per-K state of this pixel / this warp
+    int32_t* idx_ptr[NK]; uint2* my_ent[NK]; uint2* ent_ptr[NK]; int32_t* uid_g[NK];
+    float thr_k[NK], TQ[NK];
+    int k[NK], ns[NK], n_ent[NK];
+    uint32_t slotpix[NK];
+    bool dn[NK];
+#pragma unroll
+    for (int j = 0; j < NK; ++j) {
+        idx_ptr[j] = p.sel_idx[j] + pix * Kj[j];
+        my_ent[j] = p.sl[j].ent + ((size_t)ht * kSelLists + warp) * p.sl[j].qcap;
+        ent_ptr[j] = my_ent[j];
+        uid_g[j] = p.sl[j].uid + (size_t)ht * p.sl[j].ucap;
+        thr_k[j] = thr[j][0]; TQ[j] = 1.0f; k[j] = 0; ns[j] = 0; n_ent[j] = 0; slotpix[j] = (uint32_t)mpix; dn[j] = !inside;
+    }
+    bool done = !inside;                        // every K has stopped for this pixel
+    float T = 1.0f;
+    int n_eval = 0, consumed = 0;
+    bool warp_done = __all_sync(0xffffffffu, done);
+
+    // alpha' of staged entry e at this pixel (Eq. 1) with inclusion rule R4, fp32 decision arithmetic
+    auto alpha_of = [&](int e) -> float {
+        const float4 co = s_co[e];
+        const float2 xy = s_xy[e];
+        const float dx = __fsub_rn(fpx, xy.x), dy = __fsub_rn(fpy, xy.y);
+        const float q1 = __fmul_rn(__fmul_rn(co.x, dx), dx);
+        const float q2 = __fmaf_rn(__fmul_rn(co.z, dy), dy, q1);
+        const float q3 = __fmul_rn(__fmul_rn(co.y, dx), dy);
+        const float power = __fmaf_rn(-0.5f, q2, -q3);
+        float a = fminf(kAlphaMax, __fmul_rn(co.w, expf(power)));
+        if (power > 0.0f || power < kPowerMin || a < kAlphaMin) a = 0.0f;
+        return a;
+    };
+    // Algorithm 1 lines 5-18 for staged entry e, once for the shared T and once per K for the selection
+    auto step = [&](int e, float a) {
+        if (done) a = 0.0f;
+        const float oma = __fsub_rn(1.0f, a);
+        const float T_test = __fmul_rn(T, oma);                                  // line 5
+        const int32_t id = s_id[e];
+        bool all = true;
+#pragma unroll
+        for (int j = 0; j < NK; ++j) {
+            const bool sel = !dn[j] && T_test < thr_k[j];                        // line 6
+            const uint32_t sm = __ballot_sync(0xffffffffu, sel);
+            if (sm) {
+                int col = 0;
+                if (lane == 0) {
+                    const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&s_col[j][e]);
+                    int old;
+                    asm volatile("atom.shared.cas.b32 %0, [%1], -1, -2;" : "=r"(old) : "r"(slot) : "memory");
+                    if (old == -1) {
+                        col = atomicAdd(&s_ucount[j], 1);
+                        uid_g[j][col] = id;
+                        asm volatile("st.volatile.shared.b32 [%0], %1;" ::"r"(slot), "r"(col) : "memory");
+                    } else {
+                        col = old;
+                        while (col == -2) asm volatile("ld.volatile.shared.b32 %0, [%1];" : "=r"(col) : "r"(slot) : "memory");
+                    }
+                }
+                col = __shfl_sync(0xffffffffu, col, 0);
+                if (sel) {
+                    const float wQ = __fmul_rn(TQ[j], a);                        // line 8
+                    *idx_ptr[j]++ = id;
+                    ent_ptr[j][__popc(sm & lt_mask)] = make_uint2(__float_as_uint(wQ), ((uint32_t)col << 15) | slotpix[j]);
+                    slotpix[j] += 128u;
+                    ++ns[j];
+                    k[j] = k[j] + 1;                                             // line 7
+                    TQ[j] = __fmul_rn(TQ[j], oma);                               // line 10
+                    float tk;
+                    while (true) {                                               // lines 11-13
+                        tk = thr[j][k[j]];
+                        if (!(T_test < tk)) break;
+                        k[j] = k[j] + 1;
+                    }
+                    thr_k[j] = tk;
+                }
+                const int ne = __popc(sm);
+                ent_ptr[j] += ne;
+                n_ent[j] += ne;
+            }
+            if (!dn[j] && T_test < t_break[j]) dn[j] = true;                     // lines 15-17 for this K
+            all = all && dn[j];
+        }
+        if (all) done = true;
+        else T = T_test;                                                         // line 18
+    };
+
+    for (int b0 = range.x; b0 < range.y; b0 += kW2Batch) {
+        if (__syncthreads_and(warp_done)) break;                          // every pixel of the half tile has stopped for every K
+        {   // ---- stage the batch (as walk2_kernel) ----
+            const int idx = b0 + tid;
+            int32_t id = -1;
+            float4 co = make_float4(1.f, 0.f, 1.f, 0.f), cull = make_float4(1.f, 1.f, -1.f, 0.f);   // never hit
+            float2 xy = make_float2(0.f, 0.f);
+            if (idx < range.y) {
+                id = (int32_t)p.isect[idx];
+                xy = __ldg(p.mean2d + id);
+                co = __ldg(p.conic_opac + id);
+                float qmax = fminf(9.0f, 2.0f * __logf(255.0f * co.w)) * 1.0001f + 1e-3f;
+                const bool valid = co.x > 0.0f && co.z > 0.0f && co.x * co.z - co.y * co.y > 0.0f;
+                float ia = 0.0f, ic = 0.0f;
+                if (valid) { ia = 1.0f / co.x; ic = 1.0f / co.z; }
+                else qmax = 3.0e38f;
+                if (!(co.w > 0.0f)) qmax = -1.0f;
+                cull = make_float4(ia, ic, qmax, 0.f);
+            }
+            s_id[tid] = id; s_co[tid] = co; s_xy[tid] = xy; s_cull[tid] = cull;
+#pragma unroll
+            for (int j = 0; j < NK; ++j) s_col[j][tid] = -1;
+        }
+        __syncthreads();
+        if (warp_done) continue;
+        const int nb = min(kW2Batch, range.y - b0);
+        consumed = b0 + nb - range.x;
+        for (int c = 0; c < nb; c += 32) {
+            uint32_t m;
+            {
+                const float4 co = s_co[c + lane], cu = s_cull[c + lane];
+                const float2 xy = s_xy[c + lane];
+                m = __ballot_sync(0xffffffffu, rect_hit(xy.x, xy.y, co.x, co.y, co.z, cu.x, cu.y, cu.z, X0, X1, Y0, Y1));
+            }
+            n_eval += __popc(m);
+            while (m) {
+                const int e0 = c + __ffs(m) - 1;
+                m &= m - 1;
+                const bool two = m != 0;
+                const int e1 = two ? c + __ffs(m) - 1 : e0;
+                m &= m - 1;
+                float a0 = alpha_of(e0), a1 = alpha_of(e1);
+                if (!two) a1 = 0.0f;
+                step(e0, a0);
+                step(e1, a1);
+            }
+            if (__all_sync(0xffffffffu, done)) { warp_done = true; break; }
+        }
+    }
+
+    // ---- per K: n_sel, T^Q; the warp's entries x 1/(1 - T^Q) (line 20), scattered to sel_w ----
+    int32_t* hdr0 = nullptr;
+#pragma unroll
+    for (int j = 0; j < NK; ++j) {
+        const int K = Kj[j];
+        const float inv = ns[j] > 0 ? __fdiv_rn(1.0f, __fsub_rn(1.0f, TQ[j])) : 0.0f;
+        if (inside) {
+            p.n_sel[j][pix] = ns[j];
+            p.resid[j][pix] = ns[j] > 0 ? TQ[j] : 1.0f;                                  // R8
+        }
+        __syncwarp();
+        constexpr int kPre = 8;
+        for (int i0 = 0; i0 < n_ent[j]; i0 += 32 * kPre) {
+            uint2 en[kPre];
+#pragma unroll
+            for (int u = 0; u < kPre; ++u) {
+                const int i = i0 + u * 32 + lane;
+                en[u] = i < n_ent[j] ? __ldcg(my_ent[j] + i) : make_uint2(0u, 0u);
+            }
+#pragma unroll
+            for (int u = 0; u < kPre; ++u) {
+                const int i = i0 + u * 32 + lane;
+                const int pm = sel_pixel(en[u].y);
+                const float inv_p = __shfl_sync(0xffffffffu, inv, pm & 31);              // lane that owns pixel pm (WX = 16)
+                if (i < n_ent[j]) {
+                    const float w = __fmul_rn(__uint_as_float(en[u].x), inv_p);
+                    my_ent[j][i].x = __float_as_uint(w);
+                    const int64_t q = (int64_t)(y0 + (pm >> 4)) * p.cam.width + x0 + (pm & 15);
+                    p.sel_w[j][q * K + sel_slot(en[u].y)] = w;
+                }
+            }
+        }
+        if (lane == 0) p.sl[j].hdr[(size_t)ht * kHdrWords + warp] = n_ent[j];
+    }
+    (void)hdr0;
+    if (lane == 0) {
+        atomicAdd(&s_evals, n_eval);
+        atomicMax(&s_consumed, consumed);
+    }
+    prev_ht = ht; prev_start = t_start;
+  }
+}
+
+int launch_walk2_multi(const WalkParamsMulti& p, cudaStream_t st)
+{
+    const int num_half = p.cam.tiles_x * p.cam.tiles_y * 2;
+    for (int j = 0; j < p.nK; ++j)
+        QR_CUDA_OK(cudaMemsetAsync(p.sl[j].ctrl, 0, (size_t)(kCtrlWords + num_half) * 4, st));
+    const unsigned grid = (unsigned)min(num_half, sm_count() * 4);
+    switch (p.nK) {
+    case 1:
+        QR_CUDA_OK(cudaFuncSetAttribute(walk2_multi_kernel<1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        walk2_multi_kernel<1><<<grid, kW2Threads, 0, st>>>(p); break;
+    case 2:
+        QR_CUDA_OK(cudaFuncSetAttribute(walk2_multi_kernel<2>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        walk2_multi_kernel<2><<<grid, kW2Threads, 0, st>>>(p); break;
+    case 3:
+        QR_CUDA_OK(cudaFuncSetAttribute(walk2_multi_kernel<3>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        walk2_multi_kernel<3><<<grid, kW2Threads, 0, st>>>(p); break;
+    default:
+        QR_CUDA_OK(cudaFuncSetAttribute(walk2_multi_kernel<4>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        walk2_multi_kernel<4><<<grid, kW2Threads, 0, st>>>(p); break;
+    }
+    QR_LAUNCH_OK("walk2_multi_kernel");
+    return QR_OK;
+}
+
 template <int MODE>
 static int launch_walk2_mode(const WalkParams2& p, cudaStream_t st)
 {

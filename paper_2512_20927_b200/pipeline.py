@@ -119,3 +119,9 @@ def sh_colors(cam, means, sh, degree: int, colors=None):
     """RGB payload: per-view colours from spherical harmonics; feed the result to forward() as the
     D = 3 feature table.  See binding.qr_sh_colors."""
     return B.qr_sh_colors(cam, means, sh, degree, colors)
+
+
+def forward_multik(cam, fe: Frontend, features: torch.Tensor, Ks, outs=None):
+    """Q-Render for several K in one walk (binding.qr_forward_multik): a list of ForwardOut, one per K; backward() and
+    backward_clear() take each of them as they take forward()'s."""
+    return B.qr_forward_multik(cam, Ks, fe.proj.mean2d, fe.proj.conic_opac, fe.isect_gauss, fe.tile_range, features, outs)

@@ -821,3 +821,38 @@ def test_rgb_render_from_sh_colors(qr, orc):
     q = orc.qrender(lists, sc.K, cref)
     stats = P.compare_forward(out, q, lists, sc.K, 3)
     assert stats["mismatch_nonexempt"] == 0
+
+
+# ------------------------------------------------------------------------------------------------
+# several K in one walk (NEXT-3, second half): every K's outputs are those of qr_forward with that K
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,kw,Ks", [("cfg4", dict(N=60000, W=128, H=96, D=512, pose=1), (4, 8, 16, 32)),    # BASELINE config 4's sweep
+                                        ("cfg3", dict(N=60000, W=100, H=72, D=128), (40, 7)),                  # ragged image, descending K
+                                        ("cfg2", dict(N=20000, W=96, H=64, D=64), (1, 200, 12)),               # K = 1, K large, padded tile
+                                        ("cfg1", dict(W=70, H=50), (40,))])
+def test_forward_multik_equals_single_k_forwards(qr, orc, name, kw, Ks):
+    sc = make_scene(name, seed=21, **kw)
+    g = P.upload(sc)
+    fe = qr.pipeline.frontend(sc.cam, g.means, g.scales, g.quats, g.opac)
+    outs = qr.pipeline.forward_multik(sc.cam, fe, g.features, Ks)
+    torch.cuda.synchronize()
+    proj = orc.project(sc.cam, sc.means, sc.scales, sc.quats, sc.opac)
+    lists = orc.pixel_lists(sc.cam, proj)
+    G = P.to_dev(sc.dL_dmap) if sc.dL_dmap is not None else None
+    for K, o in zip(Ks, outs):
+        ref = qr.pipeline.forward(sc.cam, fe, g.features, K)
+        # the decision arithmetic is the same instruction sequence: records identical, bit for bit
+        assert torch.equal(o.n_sel, ref.n_sel) and torch.equal(o.resid_TQ, ref.resid_TQ)
+        ia, wa, na = P.masked_records(o)
+        ib, wb, nb = P.masked_records(ref)
+        assert (ia == ib).all() and (wa == wb).all()
+        torch.testing.assert_close(o.out_map, ref.out_map, rtol=2e-4, atol=2e-5)      # union numbering is a race: summation order
+        # and against the oracle, as qr_forward is
+        q = orc.qrender(lists, K, sc.features)
+        stats = P.compare_forward(o, q, lists, K, sc.D, f16=sc.features.dtype == np.float16)
+        assert stats["mismatch_nonexempt"] == 0
+        # the lists each K leaves behind feed the backward as qr_forward's do
+        if G is not None:
+            dF = qr.pipeline.backward(sc.cam, sc.N, o, G)
+            dF_ref = qr.pipeline.backward(sc.cam, sc.N, ref, G)
+            torch.testing.assert_close(dF, dF_ref, rtol=1e-3, atol=1e-4 * float(dF_ref.abs().max()) + 1e-6)
