@@ -846,6 +846,22 @@ def run_sweep(args, qr, dev, barrier):
             for K in (4, 8, 16, 32):
                 fr.reset(cam=cam, K=K)
                 measure(fr, {"workload": "cfg4", "pose": pose, "K": K, "D": sc.D, "dtype": sc.feat_dtype}, lists)
+            # the four K of this pose in ONE walk (qr_forward_multik) against the four qr_forward calls measured above
+            if qr.binding.lists_supported(fr.d["features"].dtype, sc.D):
+                Ks = (4, 8, 16, 32)
+                fe_p = fr.fe
+                mk = {"outs": None}
+
+                def multik_call():
+                    mk["outs"] = pl.forward_multik(cam, fe_p, fr.d["features"], Ks, mk["outs"])
+                mk_ms = fr.time_call(multik_call, n=5, warm=2)
+                sel_ms = None
+                singles = [p for p in points if p.get("pose") == pose and "views" not in p and p.get("workload") == "cfg4" and "K" in p]
+                rec = {"workload": "cfg4", "pose": pose, "multik": list(Ks), "qr_forward_multik_ms": mk_ms,
+                       "sum_of_single_k_forwards_ms": sum(p["qr_forward_ms"] for p in singles if p["K"] in Ks)}
+                print(json.dumps(rec), file=sys.stderr, flush=True)
+                points.append(rec)
+                del mk
         # the same poses as ONE batch (include/qr.h "Multi-camera batching": B views stacked as one tall tile grid, one set of
         # launches, one backward into one dL_dfeat), against the sum of the single-view steps above
         ev = lambda: torch.cuda.Event(enable_timing=True)
