@@ -98,6 +98,20 @@ def test_bad_arguments_are_status_codes(lib):
     assert lib.qr_mask_loss_static(C.byref(cam), 512, 0, p, p, p, p, p, p, None) == -1
     assert lib.qr_mask_loss_static(C.byref(cam), 512, 256, p, z, p, p, p, p, None) == -2
     assert lib.qr_mask_loss_workspace_bytes(256, 512) == 256 * 512 * 4 + 3 * 1024
+    # several K in one walk: nK out of range, NULL arrays, a shape outside the tcgen05 path, a bad K, a workspace that is too small
+    ks = (C.c_int32 * 2)(8, 0)
+    arr = (C.c_void_p * 2)(16, 16)
+    szs = (C.c_size_t * 2)(1 << 30, 1 << 30)
+    mk = lambda n, D, K_, a_, s_: lib.qr_forward_multik(C.byref(cam), n, K_, D, 0, p, p, p, p, p, a_, a_, a_, a_, a_, a_, s_, None)
+    assert mk(0, 128, ks, arr, szs) == -1 and mk(5, 128, ks, arr, szs) == -1
+    assert mk(2, 128, None, arr, szs) == -2 and mk(2, 128, ks, None, szs) == -2
+    assert mk(1, 36, ks, arr, szs) == -3
+    assert mk(2, 128, ks, arr, szs) == -1 and b"K[1] = 0" in lib.qr_last_error()
+    ks[1] = 16
+    assert mk(2, 128, ks, arr, szs) == -1 and b"share a workspace" in lib.qr_last_error()
+    arr2 = (C.c_void_p * 2)(16, 32)
+    small = (C.c_size_t * 2)(1 << 30, 64)
+    assert lib.qr_forward_multik(C.byref(cam), 2, ks, 128, 0, p, p, p, p, p, arr, arr, arr, arr, arr, arr2, small, None) == -4
     m = C.c_int64(-1)
     assert lib.qr_bin_count(0, z, z, C.byref(m), z, 0, None) == 0 and m.value == 0
     assert lib.qr_bin_workspace_bytes(1000, 5000, 16) >= 5000 * 16 + 16 * 16 * 4      # keys + scratch + bucket cursors

@@ -169,6 +169,16 @@ def test_neighbour_calls_write_inside_their_arrays(qr, W, H, D, S, K):
                                        ptr(fe.isect_gauss), ptr(fe.tile_range), ptr(g["features"]), ptr(out_map), ptr(sel_idx), ptr(sel_w),
                                        ptr(n_sel), ptr(resid), ptr(sws), sws.numel(), st))
     z.check("qr_forward_stratified")
+    # qr_forward_multik: three K, guarded outputs and workspaces each
+    Ks = (K, 3, 2 * K)
+    mo = [(z.alloc((H, W, D), torch.float32), z.alloc((H, W, k_), torch.int32), z.alloc((H, W, k_), torch.float32),
+           z.alloc((H, W), torch.int32), z.alloc((H, W), torch.float32), z.alloc((int(B.qr_forward_workspace_bytes(cam, k_, D)),), torch.uint8))
+          for k_ in Ks]
+    pa = lambda i: (C.c_void_p * 3)(*[ptr(t[i]) for t in mo])
+    B._check(lib.qr_forward_multik(C.byref(c), 3, (C.c_int32 * 3)(*Ks), D, 0, ptr(fe.proj.mean2d), ptr(fe.proj.conic_opac), ptr(fe.isect_gauss),
+                                   ptr(fe.tile_range), ptr(g["features"]), pa(0), pa(1), pa(2), pa(3), pa(4), pa(5),
+                                   (C.c_size_t * 3)(*[t[5].numel() for t in mo]), st))
+    z.check("qr_forward_multik")
     # qr_forward (lists in its workspace) -> qr_pooled_loss
     fws = z.alloc((int(B.qr_forward_workspace_bytes(cam, K, D)),), torch.uint8)
     B._check(lib.qr_forward(C.byref(c), K, D, 0, ptr(fe.proj.mean2d), ptr(fe.proj.conic_opac), ptr(fe.isect_gauss), ptr(fe.tile_range),
