@@ -366,7 +366,7 @@ int qr_mask_loss_static(const qr_camera* cam, int32_t D, int32_t S, const float*
  * out_map = NULL for a training step).
  *   in : fwd_ws (only read; stamp checked on the device as in qr_backward_lists), features[N,D] fp32, mask_id[H,W], targets[S,D]
  *   out: loss[1], loss_per_mask[S]; dL_dfeat[N,D] ACCUMULATED INTO (may be NULL: loss only)
- * fp32, D % 128 == 0, D <= 512.  ws must hold qr_mask_loss_workspace_bytes(S, D) bytes.
+ * fp32, shapes of the tcgen05 path (see qr_forward), D <= 512.  ws must hold qr_mask_loss_workspace_bytes(S, D) bytes.
  */
 int qr_pooled_loss(const qr_camera* cam, int32_t K, int32_t D, int64_t N, void* fwd_ws, size_t fwd_ws_bytes,
                    const float* features, const int32_t* mask_id, int32_t S, const float* targets,

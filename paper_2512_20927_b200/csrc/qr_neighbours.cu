@@ -676,7 +676,8 @@ extern "C" int qr_pooled_loss(const qr_camera* cam, int32_t K, int32_t D, int64_
     using namespace qr;
     if (int rc = check_cam(cam)) return rc;
     if (K < 1 || K > QR_MAX_K) return fail(QR_ERR_INVALID_ARG, "qr_pooled_loss: K out of range");
-    if (D < 128 || D % 128 != 0 || D > kNbMaxC) return fail(QR_ERR_UNSUPPORTED, "qr_pooled_loss: needs fp32 features with D %% 128 == 0 (D = %d)", D);
+    if (!tc_channels_supported(D) || D > kNbMaxC)
+        return fail(QR_ERR_UNSUPPORTED, "qr_pooled_loss: needs fp32 features on a shape of the tcgen05 path (D %% 32 == 0, or D < 32 with D %% 4 == 0; D = %d)", D);
     if (S < 1 || S > QR_MAX_MASKS) return fail(QR_ERR_INVALID_ARG, "qr_pooled_loss: S = %d outside [1, QR_MAX_MASKS]", S);
     if (N < 1) return fail(QR_ERR_INVALID_ARG, "qr_pooled_loss: N < 1");
     if (!fwd_ws || !features || !mask_id || !targets || !loss || !loss_per_mask || !ws) return fail(QR_ERR_NULL_POINTER, "qr_pooled_loss: NULL argument");

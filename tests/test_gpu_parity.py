@@ -707,7 +707,9 @@ def test_mask_loss_and_gradient(qr, orc, W, H, D, S):
     assert (got[mid.reshape(-1) < 0] == 0).all()
 
 
-@pytest.mark.parametrize("name,kw,K,S", [("cfg3", dict(N=60000, W=160, H=112, D=512), 40, 9), ("cfg2", dict(N=20000, W=100, H=72, D=128), 16, 30)])
+@pytest.mark.parametrize("name,kw,K,S", [("cfg3", dict(N=60000, W=160, H=112, D=512), 40, 9), ("cfg2", dict(N=20000, W=100, H=72, D=128), 16, 30),
+                                         ("cfg2", dict(N=20000, W=100, H=72, D=64), 16, 30),        # padded 128-channel tile
+                                         ("cfg1", dict(W=70, H=50), 40, 6)])                        # D = 16
 def test_pooled_loss_equals_loss_on_the_map_then_backward(qr, orc, name, kw, K, S):
     """qr_pooled_loss (no map, no dL/dmap) against the oracle's unfused chain: Algorithm 1 map -> mask loss -> d_map -> backward;
     and selection-only forward leaves the same lists as the full forward."""
