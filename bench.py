@@ -172,6 +172,7 @@ def workload_config(sc, name):
 # CUDA arm
 # ----------------------------------------------------------------------------------------------------------------
 def _time_dense_tc(qr, pl, fr, cam, fe, out_map, out_T, cap=128, n=10, warm=3):
+    # out_map / out_T hold the FFMA kernel's result on entry: keep every 37th row of it to check the tensor-core path against
     """qr_dense_forward_tc on the frame of `fr` (None where the shape is not one of the tcgen05 path): ms per call, list capacity,
     half tiles the walk flagged (lists too small: rendered by the FFMA kernel inside the call)."""
     import torch
@@ -179,16 +180,18 @@ def _time_dense_tc(qr, pl, fr, cam, fe, out_map, out_T, cap=128, n=10, warm=3):
     if not qr.binding.lists_supported(feats.dtype, int(feats.shape[1])):
         return None
     st = {"ws": None}
+    ref_rows, ref_T = out_map[::37].clone(), out_T.clone()
 
     def call():
         _, _, st["ws"] = pl.dense_forward_tc(cam, fe, feats, 1e-4, cap, out_map, out_T, st["ws"])
     ms = fr.time_call(call, n=n, warm=warm)
+    same = bool(torch.equal(out_T, ref_T)) and bool(torch.allclose(out_map[::37], ref_rows, rtol=2e-4, atol=2e-5))
     al = lambda v: (v + 255) // 256 * 256
     nh = 2 * ((cam.width + 15) // 16) * ((cam.height + 15) // 16)
     o = al(256 + 64)
     hdr = al(o + (64 + nh) * 4)
     h = st["ws"][hdr:hdr + nh * 64].view(torch.int32).view(nh, 16)
-    rec = {"ms": ms, "cap": cap, "flagged_half_tiles": int((h[:, 5] == 1).sum().item()), "half_tiles": nh,
+    rec = {"ms": ms, "cap": cap, "matches_ffma_dense": same, "flagged_half_tiles": int((h[:, 5] == 1).sum().item()), "half_tiles": nh,
            "entries": int(h[:, :4].sum().item()), "union_mean": float(h[:, 4].float().mean().item())}
     st["ws"] = None
     return rec
